@@ -1,0 +1,164 @@
+"""Pins for the oracle's hand-derived reverse-mode gradient (O9): central finite differences with one
+Richardson step, in fp64, for every partial of every component and end to end on tiny grids.  CPU only.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+
+
+def fd(f, x, h):
+    """Richardson-extrapolated central difference, O(h^4)."""
+    d1 = (f(x + h) - f(x - h)) / (2 * h)
+    d2 = (f(x + h / 2) - f(x - h / 2)) / h
+    return (4 * d2 - d1) / 3
+
+
+def close(a, b, rtol=2e-7, atol=1e-9):
+    return abs(a - b) <= atol + rtol * max(abs(a), abs(b))
+
+
+# --------------------------------------------------------------------------- point-wise partials
+@pytest.mark.parametrize("t", [0.6, 1.0, 1.4])
+def test_epl_frame_partials(t):
+    b, q, x, y = 1.1, 0.62, 0.8, -0.55
+    r = oracle.epl_frame(b, t, q, x, y)
+    A = lambda **k: oracle.epl_frame(**{**dict(b=b, t=t, q=q, x=x, y=y), **k})["alpha"]
+    h = 1e-3
+    for name, key in (("d_b", "b"), ("d_t", "t"), ("d_q", "q")):
+        ref = fd(lambda v: A(**{key: v}), dict(b=b, t=t, q=q)[key], h)
+        assert abs(r[name] - ref) < 3e-9 * max(1, abs(ref)), (name, r[name], ref)
+    jx = fd(lambda v: A(x=v), x, h); jy = fd(lambda v: A(y=v), y, h)
+    Jxx, Jyy, Jxy = r["J"]
+    assert close(Jxx, jx.real, 1e-8) and close(Jxy, jx.imag, 1e-8) and close(Jxy, jy.real, 1e-8) and close(Jyy, jy.imag, 1e-8)
+
+
+def test_epl_frame_q_derivative_near_circular():
+    # f -> 0: the S1/f series must stay finite and correct
+    b, t, x, y = 1.0, 1.3, 0.7, 0.4
+    for q in (0.999999, 0.9999):
+        r = oracle.epl_frame(b, t, q, x, y)
+        ref = fd(lambda v: oracle.epl_frame(b, t, v, x, y)["alpha"], q, 5e-5 if q < 0.99999 else 5e-7)
+        assert abs(r["d_q"] - ref) < 1e-6
+
+
+def test_sie_frame_partials_and_agreement_with_epl():
+    b, q, x, y = 0.9, 0.55, -0.7, 0.45
+    r = oracle.sie_frame(b, q, x, y)
+    A = lambda **k: oracle.sie_frame(**{**dict(b=b, q=q, x=x, y=y), **k})["alpha"]
+    assert abs(r["d_b"] - fd(lambda v: A(b=v), b, 1e-3)) < 1e-9
+    assert abs(r["d_q"] - fd(lambda v: A(q=v), q, 1e-3)) < 1e-9
+    jx = fd(lambda v: A(x=v), x, 1e-3); jy = fd(lambda v: A(y=v), y, 1e-3)
+    Jxx, Jyy, Jxy = r["J"]
+    assert close(Jxx, jx.real, 1e-8) and close(Jxy, jx.imag, 1e-8) and close(Jyy, jy.imag, 1e-8)
+    e = oracle.epl_frame(b, 1.0, q, x, y)                 # same function, two derivations
+    for k in ("alpha", "d_b", "d_q"):
+        assert abs(e[k] - r[k]) < 1e-13
+    assert np.allclose(e["J"], r["J"], atol=1e-13)
+
+
+@pytest.mark.parametrize("p", [[0.3, 1.7, 0.12, -0.2, 0.05, -0.04, 7.0], [0.9, 4.2, -0.05, 0.08, 0.01, 0.02, 3.0],
+                               [0.25, 0.8, 0.3, 0.1, -0.1, 0.1, 1.0]])
+def test_sersic_partials(p):
+    x, y = 0.31, -0.22
+    v, dp, dxy = oracle.sersic(p, x, y, want_grad=True)
+    for k in range(7):
+        def f(val, k=k):
+            pp = list(p); pp[k] = val; return oracle.sersic(pp, x, y)
+        assert close(dp[k], fd(f, p[k], 1e-3 * max(1, abs(p[k]))), 1e-8), k
+    assert close(dxy[0], fd(lambda xx: oracle.sersic(p, xx, y), x, 1e-3), 1e-8)
+    assert close(dxy[1], fd(lambda yy: oracle.sersic(p, x, yy), y, 1e-3), 1e-8)
+
+
+def test_shapelet_partials():
+    rng = np.random.default_rng(0)
+    nmax = 4; nc = W.n_shapelet_coef(nmax)
+    p = np.concatenate([[0.17], rng.normal(size=nc)])
+    x0, y0, x, y = 0.03, -0.02, 0.21, 0.09
+    v, da, dxy = oracle.shapelets(nmax, p, x0, y0, x, y, want_grad=True)
+    for k in range(nc + 1):
+        def f(val, k=k):
+            pp = p.copy(); pp[k] = val; return oracle.shapelets(nmax, pp, x0, y0, x, y)
+        assert close(da[k], fd(f, p[k], 1e-3), 1e-8), k
+    assert close(dxy[0], fd(lambda xx: oracle.shapelets(nmax, p, x0, y0, xx, y), x, 1e-3), 1e-8)
+    assert close(dxy[1], fd(lambda yy: oracle.shapelets(nmax, p, x0, y0, x, yy), y, 1e-3), 1e-8)
+    assert close(-dxy[0], fd(lambda xx: oracle.shapelets(nmax, p, xx, y0, x, y), x0, 1e-3), 1e-8)
+
+
+# --------------------------------------------------------------------------- end to end
+def _tiny(kind, param_space):
+    rng = np.random.default_rng(11)
+    if kind == "sie":
+        sp = W.LensSpec(6, 2, 3, 0.30, mass_model=0, param_space=param_space)
+        pri = W._default_priors(0)
+        th = [0.55, 0.10, -0.05, 0.02, -0.03, 0.03, -0.02, 0.20, 1.5, 0.10, 0.05, 0.05, -0.04, 8.0,
+              0.60, 3.0, -0.05, 0.08, 0.01, 0.02, 4.0]
+        # widen supports so the fixed theta above is inside them
+        pri[0] = W.Uniform(0.3, 1.5)
+    else:
+        sp = W.LensSpec(8, 2, 5, 0.25, mass_model=1, multipole_mask=3, shapelet_nmax=3, n_lens_sersic=2,
+                        param_space=param_space)
+        pri = W._default_priors(1, multipoles=True, shapelet_nmax=3, n_lens=2)
+        pri[0] = W.LogNormal(math.log(0.6), 0.4)            # exercise every prior family
+        th = ([0.62, 2.2, 0.12, -0.07, 0.03, -0.02, 0.04, -0.03, 0.012, -0.006, 0.004, 0.009,
+               0.22, 1.6, 0.1, 0.06, 0.06, -0.05, 9.0, 0.15] + list(rng.normal(0, 1, 10)) +
+              [0.7, 3.1, -0.05, 0.08, 0.01, 0.02, 4.0, 1.2, 2.4, 0.04, -0.03, -0.01, 0.015, 1.5])
+    sp.priors = pri
+    K = sp.psf_size
+    psf = rng.uniform(0.2, 1.0, (1, K, K)); psf /= psf.sum()
+    obs = rng.normal(0.5, 0.3, (1, sp.n_pix, sp.n_pix))
+    sig = rng.uniform(0.05, 0.2, (1, sp.n_pix, sp.n_pix))
+    th = np.array(th)
+    assert len(th) == sp.n_params
+    x = th if param_space == 1 else W.z_of(pri, th)[0]
+    return sp, psf, obs, sig, x
+
+
+@pytest.mark.parametrize("kind", ["sie", "epl_full"])
+@pytest.mark.parametrize("param_space", [1, 0])
+def test_gradient_vs_finite_differences(kind, param_space):
+    sp, psf, obs, sig, x0 = _tiny(kind, param_space)
+    o = oracle.logpost_grad(sp, obs, sig, psf, [x0], want_gabs=True)
+    assert np.isfinite(o["logp"][0])
+    g = o["grad"][0]
+
+    def lp(x):
+        return oracle.logpost_grad(sp, obs, sig, psf, [x], want_grad=False)["logp"][0]
+    for k in range(sp.n_params):
+        def f(v, k=k):
+            x = x0.copy(); x[k] = v; return lp(x)
+        h = 2e-4 * max(1.0, abs(x0[k]))
+        ref = fd(f, x0[k], h)
+        assert abs(g[k] - ref) < 2e-6 * abs(ref) + 1e-5, (k, g[k], ref)
+
+
+def test_gradient_truncated_series_matches_its_own_finite_difference():
+    """The epl_terms>0 (debug) mode differentiates the truncated sum term by term."""
+    sp, psf, obs, sig, x0 = _tiny("epl_full", 1)
+    o = oracle.logpost_grad(sp, obs, sig, psf, [x0], epl_terms=12)
+    for k in (0, 1, 2, 3, 4, 5):
+        def f(v, k=k):
+            x = x0.copy(); x[k] = v
+            return oracle.logpost_grad(sp, obs, sig, psf, [x], want_grad=False, epl_terms=12)["logp"][0]
+        ref = fd(f, x0[k], 2e-4)
+        assert abs(o["grad"][0][k] - ref) < 2e-6 * abs(ref) + 1e-5
+
+
+def test_gradient_config1_prior_particles_fd_spotcheck():
+    """Realistic scale (config 1, 40x40, s=2): a few parameters of a few prior-drawn particles."""
+    wl = W.make_workload(1, n_particles=3)
+    sp = wl.spec
+    truth = oracle.model_image(sp, wl.psf.astype(np.float64), wl.truth_theta)
+    obs, sig = W.finish_observation(wl, truth)
+    z = wl.params.astype(np.float64)
+    o = oracle.logpost_grad(sp, obs, sig, wl.psf, z, want_gabs=True)
+    for p in range(3):
+        for k in (0, 2, 4, 6, 7, 8, 11, 13, 15, 20):
+            def f(v):
+                x = z[p].copy(); x[k] = v
+                return oracle.logpost_grad(sp, obs, sig, wl.psf, [x], want_grad=False)["logp"][0]
+            ref = fd(f, z[p, k], 1e-4 * max(1, abs(z[p, k])))
+            assert abs(o["grad"][p, k] - ref) < 1e-6 * abs(ref) + 1e-9 * o["gabs"][p, k] + 1e-4, (p, k, o["grad"][p, k], ref)
