@@ -1,0 +1,158 @@
+/*
+ * gigalens.h -- C ABI of the B200-native batched lens-model log-posterior and gradient.
+ *
+ * What the library computes (citations: P:Lnn = /root/reference/PAPER.md line nn; S# / O# = the readings
+ * and the operation list of SURVEY.md section 8(c), restated in DESIGN.md section 3):
+ *
+ *   For each of n_particles independent parameter vectors ("particles": multi-start MAP starts, SVI
+ *   draws, HMC chain positions -- P:L72) the log joint  log p~(I_obs, Theta~)  of P:L89 (Eq. 2) in
+ *   the unconstrained space of P:L76, and its gradient with respect to Theta~.
+ *   The forward model is the one the paper names at P:L64: elliptical power-law (or SIE) mass +
+ *   external shear (+ m=3,4 multipoles, BASELINE.json configs[4]); elliptical Sersic and Cartesian
+ *   shapelet source light; Sersic lens light; "forward" amplitudes; on a pixel grid supersampled by an
+ *   integer factor (P:L189 fn 6); PSF convolution at ray resolution, binning to detector pixels and a
+ *   Gaussian chi-square against the observed image (BASELINE.json north_star; readings S10-S12).
+ *
+ * Conventions common to every call
+ *   - Every array argument is a DEVICE pointer owned by the caller unless it says HOST.  The library never
+ *     allocates or frees device memory inside a call and keeps no reference to caller memory after return.
+ *   - All arrays are fp32 (system_id: int32), C-contiguous, row index = y, column index = x (reading S1).
+ *   - Calls are asynchronous on `stream`: no host synchronisation, no device-to-host copy.  Re-entrant on
+ *     different streams with different workspaces.  The caller must not touch outputs or workspace until the
+ *     stream has reached the end of the call.
+ *   - Errors are returned as gl_status; nothing is thrown or aborted across the ABI.  All argument checks run
+ *     on the host before the first launch; on any error no kernel has been launched.
+ *   - Results are bit-identical for the same particle irrespective of batch composition, order or size
+ *     (fixed reduction orders, no atomics): the analogue of P:L83 fn 2.
+ *   - There is no CPU fallback.
+ */
+#ifndef GIGALENS_H
+#define GIGALENS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    GL_OK = 0,
+    GL_ERR_NULL = -1,         /* a required pointer is NULL */
+    GL_ERR_BAD_CONFIG = -2,   /* inconsistent gl_config_desc (even psf_size, supersample < 1, n_params mismatch, ...) */
+    GL_ERR_BAD_SHAPE = -3,    /* n_particles < 0 */
+    GL_ERR_UNSUPPORTED = -4,  /* a valid configuration this build has no kernel for */
+    GL_ERR_WORKSPACE = -5,    /* workspace_bytes < gl_workspace_bytes(cfg, n_particles) or misaligned */
+    GL_ERR_CUDA = -6          /* a CUDA runtime call or launch failed (sticky error left to the caller) */
+} gl_status;
+
+/* Prior / bijector family of one parameter (O1, reading S13).
+ *   NONE        theta = z,                       log prior 0
+ *   NORMAL      theta = z,                       N(a, b)
+ *   LOGNORMAL   theta = exp z,                   ln theta ~ N(a, b)
+ *   UNIFORM     theta = lo + (hi-lo) sigmoid z,  U(lo, hi)
+ *   TRUNCNORMAL theta = lo + (hi-lo) sigmoid z,  N(a, b) truncated to [lo, hi]
+ *   LOGUNIFORM  ln theta = ln lo + (ln hi - ln lo) sigmoid z,  density 1/(theta ln(hi/lo)) */
+typedef enum {
+    GL_PRIOR_NONE = 0, GL_PRIOR_NORMAL = 1, GL_PRIOR_LOGNORMAL = 2, GL_PRIOR_UNIFORM = 3,
+    GL_PRIOR_TRUNCNORMAL = 4, GL_PRIOR_LOGUNIFORM = 5
+} gl_prior_kind;
+
+typedef struct { int32_t kind; float a, b, lo, hi; } gl_prior;
+
+/* Model configuration.  The flat parameter vector has the block order of reading S18:
+ *   main mass [theta_E, (gamma if EPL), e1, e2, x, y] . shear [g1, g2] . multipoles [c3, s3][c4, s4] .
+ *   source Sersic [R, n, e1, e2, x, y, I] . shapelets [beta_s, a_0 .. a_{Nc-1}] . lens Sersic 1 . lens Sersic 2
+ * with Nc = (nmax+1)(nmax+2)/2 coefficients ordered by n1+n2 then n2 (O5, S9); the shapelet centre is the
+ * source Sersic centre, so shapelets require n_source_sersic = 1. */
+typedef struct {
+    int32_t n_pix;            /* N: detector pixels per side, >= 1 */
+    int32_t supersample;      /* s: rays per pixel per side, >= 1 */
+    int32_t psf_size;         /* K: PSF taps per side on the RAY grid, odd (S10) */
+    float   pix_scale;        /* Delta: arcsec per detector pixel, > 0 */
+    int32_t psf_grid;         /* 0: taps on the ray grid, convolve then bin (S10). Other values: GL_ERR_UNSUPPORTED */
+    int32_t mass_model;       /* 0 SIE closed form, 1 EPL series */
+    int32_t epl_terms;        /* number of series terms kept for EPL, 2..30 (S5; BASELINE.json: 30) */
+    int32_t has_shear;        /* 0/1 */
+    int32_t multipole_mask;   /* bit0: m=3, bit1: m=4 (S7) */
+    int32_t n_source_sersic;  /* 0 or 1 */
+    int32_t shapelet_nmax;    /* -1 none, else 0..10 */
+    int32_t n_lens_sersic;    /* 0, 1 or 2 */
+    int32_t param_space;      /* 0: params are unconstrained z (bijector + log-det); 1: physical theta */
+    int32_t n_systems;        /* number of (obs, noise_sigma, psf) triples, >= 1 (S19) */
+    int32_t n_params;         /* must equal the count implied by the fields above (<= 128) */
+    const gl_prior* priors;   /* HOST pointer, n_params entries, copied by gl_config_create */
+} gl_config_desc;
+
+typedef struct gl_config gl_config;   /* opaque, immutable, host-side, library-owned */
+
+/* Validate `desc`, copy it (priors included) and return a handle in *out.  HOST pointers.
+ * Errors: GL_ERR_NULL, GL_ERR_BAD_CONFIG, GL_ERR_UNSUPPORTED.  No CUDA call is made. */
+gl_status gl_config_create(const gl_config_desc* desc, gl_config** out);
+
+/* Free a handle from gl_config_create (NULL is a no-op).  Must not race with a host call using it;
+ * work already enqueued on a stream does not reference the handle. */
+void gl_config_destroy(gl_config* cfg);
+
+/* Parameter count implied by a configuration (S18); 0 if cfg is NULL. */
+int32_t gl_config_n_params(const gl_config* cfg);
+
+/* Bytes of device workspace gl_logpost / gl_logpost_grad / gl_model_image need for n_particles
+ * (0 if cfg is NULL or n_particles <= 0).  Grows with n_particles up to an internal chunk size, then stays
+ * flat: larger batches are processed in chunks on the same stream.  The workspace must be 256-byte aligned. */
+size_t gl_workspace_bytes(const gl_config* cfg, int64_t n_particles);
+
+/* log p~ for each particle (O1-O8):
+ *   out_logp[p] = logL + sum_i log prior_i(theta_i) + sum_i log|dtheta_i/dz_i|,
+ *   logL = -1/2 sum_pix ((model - obs)/sigma)^2 - sum_pix ln sigma - (N^2/2) ln 2 pi      (S12)
+ *   obs, noise_sigma : [n_systems][N][N]   observed image and FIXED per-pixel noise sigma (> 0)
+ *   psf              : [n_systems][K][K]   used as given (no renormalisation), true convolution, zero padding
+ *   params           : [n_particles][n_params]
+ *   system_id        : [n_particles] in [0, n_systems), or NULL (all 0)                    (S19)
+ *   out_logp         : [n_particles]
+ * A particle whose parameters are non-finite or outside the model's domain (theta_E <= 0, gamma outside
+ * (1,3), |eps| >= 1, R <= 0, n <= 0, beta_s <= 0, or outside a bounded prior support when param_space = 1),
+ * or whose result is non-finite, gets out_logp = -INF; NaN is never written.
+ * n_particles = 0 returns GL_OK without a launch. */
+gl_status gl_logpost(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
+                     const float* params, const int32_t* system_id, int64_t n_particles,
+                     float* out_logp, void* workspace, size_t workspace_bytes, void* stream /* cudaStream_t */);
+
+/* As gl_logpost, plus out_grad[p][i] = d out_logp[p] / d params[p][i] (O9: hand-written reverse mode of
+ * the whole path, priors and bijector log-determinants included).  Invalid particles get a zero row. */
+gl_status gl_logpost_grad(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
+                          const float* params, const int32_t* system_id, int64_t n_particles,
+                          float* out_logp, float* out_grad, void* workspace, size_t workspace_bytes,
+                          void* stream /* cudaStream_t */);
+
+/* Diagnostic: the noise-free model image (O3-O6) of each particle, out_image [n_particles][N][N].
+ * Invalid particles get an all-zero image. */
+gl_status gl_model_image(const gl_config* cfg, const float* psf, const float* params, const int32_t* system_id,
+                         int64_t n_particles, float* out_image, void* workspace, size_t workspace_bytes,
+                         void* stream /* cudaStream_t */);
+
+/* Host-buffer convenience forms (what bench.py's `e2e` times).  params_host, out_logp_host and out_grad_host
+ * are HOST pointers (pinned memory for true asynchrony; pageable memory works but serialises); everything else
+ * is as above (obs / noise_sigma / psf / system_id stay DEVICE pointers: the observation is resident across the
+ * steps of an optimiser or sampler, only the particles move).  The call enqueues, on `stream`, the host-to-device
+ * copy of params, the kernels, and the device-to-host copies of the results; it does not synchronise.  The
+ * workspace must hold gl_workspace_bytes_host(cfg, n) bytes.  out_grad_host == NULL selects gl_logpost. */
+size_t gl_workspace_bytes_host(const gl_config* cfg, int64_t n_particles);
+gl_status gl_logpost_grad_host(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
+                               const float* params_host, const int32_t* system_id, int64_t n_particles,
+                               float* out_logp_host, float* out_grad_host, void* workspace, size_t workspace_bytes,
+                               void* stream /* cudaStream_t */);
+
+/* Number of kernel launches the last call on this thread enqueued (bench.py's gpu_launches claim). */
+int64_t gl_last_launch_count(void);
+
+/* Static string for a status code. */
+const char* gl_status_string(gl_status s);
+
+/* Library version, "major.minor". */
+const char* gl_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GIGALENS_H */

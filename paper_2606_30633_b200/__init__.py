@@ -1,0 +1,250 @@
+"""paper_2606_30633_b200 -- thin Python binding of libgigalens (include/gigalens.h).
+
+Argument marshalling only: every step of the path runs in the hand-written sm_100a kernels of
+csrc/.  PyTorch is used for device memory and streams.  There is NO CPU fallback: importing works without
+a GPU (so the symbol-export test can run), but every compute call raises if the shared library is missing or
+CUDA is unavailable.  This package never imports oracle/.
+
+Function names follow the C ABI: gl_config_create, gl_workspace_bytes, gl_logpost, gl_logpost_grad,
+gl_model_image, gl_logpost_grad_host.  `LensModel` bundles a config handle with a cached workspace.
+"""
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libgigalens.so")
+
+GL_OK = 0
+STATUS = {0: "GL_OK", -1: "GL_ERR_NULL", -2: "GL_ERR_BAD_CONFIG", -3: "GL_ERR_BAD_SHAPE", -4: "GL_ERR_UNSUPPORTED",
+          -5: "GL_ERR_WORKSPACE", -6: "GL_ERR_CUDA"}
+EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_workspace_bytes", "gl_logpost",
+           "gl_logpost_grad", "gl_model_image", "gl_workspace_bytes_host", "gl_logpost_grad_host",
+           "gl_last_launch_count", "gl_status_string", "gl_version"]
+
+
+class GLError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        super().__init__("%s failed: %s (%d)" % (where, STATUS.get(status, "?"), status))
+
+
+class gl_prior(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("a", C.c_float), ("b", C.c_float), ("lo", C.c_float), ("hi", C.c_float)]
+
+
+class gl_config_desc(C.Structure):
+    _fields_ = [("n_pix", C.c_int32), ("supersample", C.c_int32), ("psf_size", C.c_int32), ("pix_scale", C.c_float),
+                ("psf_grid", C.c_int32), ("mass_model", C.c_int32), ("epl_terms", C.c_int32), ("has_shear", C.c_int32),
+                ("multipole_mask", C.c_int32), ("n_source_sersic", C.c_int32), ("shapelet_nmax", C.c_int32),
+                ("n_lens_sersic", C.c_int32), ("param_space", C.c_int32), ("n_systems", C.c_int32),
+                ("n_params", C.c_int32), ("priors", C.POINTER(gl_prior))]
+
+
+_lib = None
+
+
+def lib():
+    """Load libgigalens.so (built in-tree by paper_2606_30633_b200.build); fail loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("libgigalens.so not built: run `python -m paper_2606_30633_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i64, sz = C.c_void_p, C.c_int64, C.c_size_t
+        L.gl_config_create.restype = C.c_int
+        L.gl_config_create.argtypes = [C.POINTER(gl_config_desc), C.POINTER(vp)]
+        L.gl_config_destroy.restype = None
+        L.gl_config_destroy.argtypes = [vp]
+        L.gl_config_n_params.restype = C.c_int32
+        L.gl_config_n_params.argtypes = [vp]
+        L.gl_workspace_bytes.restype = sz
+        L.gl_workspace_bytes.argtypes = [vp, i64]
+        L.gl_workspace_bytes_host.restype = sz
+        L.gl_workspace_bytes_host.argtypes = [vp, i64]
+        L.gl_logpost.restype = C.c_int
+        L.gl_logpost.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, sz, vp]
+        L.gl_logpost_grad.restype = C.c_int
+        L.gl_logpost_grad.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, sz, vp]
+        L.gl_logpost_grad_host.restype = C.c_int
+        L.gl_logpost_grad_host.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, sz, vp]
+        L.gl_model_image.restype = C.c_int
+        L.gl_model_image.argtypes = [vp, vp, vp, vp, i64, vp, vp, sz, vp]
+        L.gl_last_launch_count.restype = i64
+        L.gl_status_string.restype = C.c_char_p
+        L.gl_status_string.argtypes = [C.c_int]
+        L.gl_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(status, where):
+    if status != GL_OK:
+        raise GLError(status, where)
+
+
+def gl_config_create(spec):
+    """spec: any object with the gl_config_desc field names (e.g. workloads.LensSpec) and
+    priors = [(kind, a, b, lo, hi), ...].  Returns an opaque handle (c_void_p)."""
+    n = len(spec.priors)
+    pri = (gl_prior * max(n, 1))()
+    for i, (k, a, b, lo, hi) in enumerate(spec.priors):
+        pri[i] = gl_prior(int(k), float(a), float(b), float(lo), float(hi))
+    d = gl_config_desc(spec.n_pix, spec.supersample, spec.psf_size, float(spec.pix_scale),
+                       int(getattr(spec, "psf_grid", 0)), spec.mass_model, spec.epl_terms, spec.has_shear,
+                       spec.multipole_mask, spec.n_source_sersic, spec.shapelet_nmax, spec.n_lens_sersic,
+                       spec.param_space, spec.n_systems, int(getattr(spec, "n_params", n)), pri)
+    h = C.c_void_p()
+    _check(lib().gl_config_create(C.byref(d), C.byref(h)), "gl_config_create")
+    return h
+
+
+def gl_config_destroy(h):
+    lib().gl_config_destroy(h)
+
+
+def gl_workspace_bytes(h, n):
+    return lib().gl_workspace_bytes(h, int(n))
+
+
+def gl_workspace_bytes_host(h, n):
+    return lib().gl_workspace_bytes_host(h, int(n))
+
+
+def gl_last_launch_count():
+    return lib().gl_last_launch_count()
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("CUDA device required: libgigalens has no CPU fallback")
+    return torch
+
+
+def _dev(t, dtype, name):
+    torch = _torch()
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError("%s must be a contiguous CUDA tensor of dtype %s" % (name, dtype))
+    return t
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+def _stream(stream):
+    torch = _torch()
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def gl_logpost(h, obs, noise_sigma, psf, params, system_id, out_logp, workspace, stream=None):
+    torch = _torch()
+    f32 = torch.float32
+    n = params.shape[0]
+    _check(lib().gl_logpost(h, _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
+                            _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
+                            _ptr(_dev(system_id, torch.int32, "system_id")), n, _ptr(_dev(out_logp, f32, "out_logp")),
+                            _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)), "gl_logpost")
+
+
+def gl_logpost_grad(h, obs, noise_sigma, psf, params, system_id, out_logp, out_grad, workspace, stream=None):
+    torch = _torch()
+    f32 = torch.float32
+    n = params.shape[0]
+    _check(lib().gl_logpost_grad(h, _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
+                                 _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
+                                 _ptr(_dev(system_id, torch.int32, "system_id")), n,
+                                 _ptr(_dev(out_logp, f32, "out_logp")), _ptr(_dev(out_grad, f32, "out_grad")),
+                                 _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)),
+           "gl_logpost_grad")
+
+
+def gl_model_image(h, psf, params, system_id, out_image, workspace, stream=None):
+    torch = _torch()
+    f32 = torch.float32
+    n = params.shape[0]
+    _check(lib().gl_model_image(h, _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
+                                _ptr(_dev(system_id, torch.int32, "system_id")), n,
+                                _ptr(_dev(out_image, f32, "out_image")), _ptr(workspace),
+                                workspace.numel() * workspace.element_size(), _stream(stream)), "gl_model_image")
+
+
+def gl_logpost_grad_host(h, obs, noise_sigma, psf, params_host, system_id, out_logp_host, out_grad_host, workspace,
+                         stream=None):
+    """params_host / out_*_host: CPU tensors (pinned for asynchrony); the rest on the device."""
+    torch = _torch()
+    f32 = torch.float32
+    for t, nm in ((params_host, "params_host"), (out_logp_host, "out_logp_host"), (out_grad_host, "out_grad_host")):
+        if t is not None and not (isinstance(t, torch.Tensor) and (not t.is_cuda) and t.dtype == f32 and t.is_contiguous()):
+            raise TypeError("%s must be a contiguous CPU float32 tensor" % nm)
+    n = params_host.shape[0]
+    _check(lib().gl_logpost_grad_host(h, _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
+                                      _ptr(_dev(psf, f32, "psf")), _ptr(params_host),
+                                      _ptr(_dev(system_id, torch.int32, "system_id")), n, _ptr(out_logp_host),
+                                      _ptr(out_grad_host), _ptr(workspace),
+                                      workspace.numel() * workspace.element_size(), _stream(stream)),
+           "gl_logpost_grad_host")
+
+
+class LensModel:
+    """A config handle plus device-resident observation and a cached workspace (the call a user makes)."""
+
+    def __init__(self, spec, obs, noise_sigma, psf, device="cuda:0"):
+        torch = _torch()
+        self.spec = spec
+        self.h = gl_config_create(spec)
+        self.device = torch.device(device)
+        as_dev = lambda a: torch.as_tensor(a, dtype=torch.float32).contiguous().to(self.device) if a is not None else None
+        self.obs, self.noise_sigma, self.psf = as_dev(obs), as_dev(noise_sigma), as_dev(psf)
+        self.n_params = lib().gl_config_n_params(self.h)
+        self._ws = None
+
+    def close(self):
+        if self.h is not None:
+            gl_config_destroy(self.h); self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def workspace(self, n, host=False):
+        torch = _torch()
+        need = gl_workspace_bytes_host(self.h, n) if host else gl_workspace_bytes(self.h, n)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = torch.empty(max(need, 256), dtype=torch.uint8, device=self.device)
+        return self._ws
+
+    def _sid(self, system_id):
+        torch = _torch()
+        if system_id is None:
+            return None
+        return torch.as_tensor(system_id, dtype=torch.int32).contiguous().to(self.device)
+
+    def logpost(self, params, system_id=None, stream=None):
+        torch = _torch()
+        out = torch.empty(params.shape[0], dtype=torch.float32, device=self.device)
+        gl_logpost(self.h, self.obs, self.noise_sigma, self.psf, params, self._sid(system_id), out,
+                   self.workspace(params.shape[0]), stream)
+        return out
+
+    def logpost_grad(self, params, system_id=None, stream=None, out_logp=None, out_grad=None):
+        torch = _torch()
+        n = params.shape[0]
+        lp = out_logp if out_logp is not None else torch.empty(n, dtype=torch.float32, device=self.device)
+        g = out_grad if out_grad is not None else torch.empty((n, self.n_params), dtype=torch.float32, device=self.device)
+        gl_logpost_grad(self.h, self.obs, self.noise_sigma, self.psf, params, self._sid(system_id), lp, g,
+                        self.workspace(n), stream)
+        return lp, g
+
+    def model_image(self, params, system_id=None, stream=None):
+        torch = _torch()
+        n = params.shape[0]
+        out = torch.empty((n, self.spec.n_pix, self.spec.n_pix), dtype=torch.float32, device=self.device)
+        gl_model_image(self.h, self.psf, params, self._sid(system_id), out, self.workspace(n), stream)
+        return out

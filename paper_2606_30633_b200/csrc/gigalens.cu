@@ -1,0 +1,310 @@
+// gigalens.cu -- C-ABI entry points (include/gigalens.h) and launch logic of libgigalens.
+// Product path: hand-written CUDA for sm_100a only; no CPU fallback; nothing here touches oracle/.
+#include "../../include/gigalens.h"
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "gl_common.cuh"
+#include "gl_conv.cuh"
+#include "gl_conv_tiled.cuh"
+#include "gl_particle.cuh"
+#include "gl_ray.cuh"
+
+using namespace gl;
+
+struct gl_config {
+    gl_config_desc desc;
+    std::vector<gl_prior> priors;
+    Layout L;
+    Geom G;
+    PriorTable pt;
+    int variant;        // 0: <.,0,1,-1,1>  1: <.,0,1,6,2>  2: <.,3,1,10,2>
+    int na;             // natural accumulators per chunk for the variant
+    int rpt_fwd, rpt_adj, n_chunk_fwd, n_chunk_adj, n_ctile;
+    int conv_kind;      // 0 generic, >0 tiled specialisation id
+    size_t per_particle_bytes;
+};
+
+static thread_local int64_t t_launches = 0;
+
+static constexpr int NT_FWD = 256;
+static constexpr int NT_ADJ = 128;
+static constexpr size_t WS_BUDGET = (size_t)1536 << 20;   // chunk so that per-chunk buffers stay below ~1.5 GiB
+
+static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+extern "C" const char* gl_status_string(gl_status s) {
+    switch (s) {
+        case GL_OK: return "GL_OK";
+        case GL_ERR_NULL: return "GL_ERR_NULL: a required pointer is NULL";
+        case GL_ERR_BAD_CONFIG: return "GL_ERR_BAD_CONFIG: inconsistent configuration";
+        case GL_ERR_BAD_SHAPE: return "GL_ERR_BAD_SHAPE: negative particle count";
+        case GL_ERR_UNSUPPORTED: return "GL_ERR_UNSUPPORTED: no kernel for this configuration";
+        case GL_ERR_WORKSPACE: return "GL_ERR_WORKSPACE: workspace too small or misaligned";
+        case GL_ERR_CUDA: return "GL_ERR_CUDA: CUDA runtime error";
+    }
+    return "unknown gl_status";
+}
+
+extern "C" const char* gl_version(void) { return "0.1"; }
+extern "C" int64_t gl_last_launch_count(void) { return t_launches; }
+
+static int layout_from_desc(const gl_config_desc& d, Layout& L) {
+    int k = 0;
+    L.mass = k; k += 1;
+    if (d.mass_model == 1) { L.gamma = k; k += 1; } else L.gamma = -1;
+    L.ell = k; k += 4;
+    if (d.has_shear) { L.shear = k; k += 2; } else L.shear = -1;
+    if (d.multipole_mask & 1) { L.mp3 = k; k += 2; } else L.mp3 = -1;
+    if (d.multipole_mask & 2) { L.mp4 = k; k += 2; } else L.mp4 = -1;
+    if (d.n_source_sersic > 0) { L.src = k; k += 7; } else L.src = -1;
+    L.nmax = d.shapelet_nmax; L.n_coef = 0;
+    if (d.shapelet_nmax >= 0) { L.n_coef = (d.shapelet_nmax + 1) * (d.shapelet_nmax + 2) / 2; L.shp = k; k += 1 + L.n_coef; } else L.shp = -1;
+    if (d.n_lens_sersic >= 1) { L.ll0 = k; k += 7; } else L.ll0 = -1;
+    if (d.n_lens_sersic >= 2) { L.ll1 = k; k += 7; } else L.ll1 = -1;
+    L.n_params = k; L.param_space = d.param_space; L.mass_model = d.mass_model;
+    return k;
+}
+
+extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) {
+    if (!d || !out) return GL_ERR_NULL;
+    *out = nullptr;
+    if (!d->priors) return GL_ERR_NULL;
+    if (d->n_pix < 1 || d->supersample < 1 || d->psf_size < 1 || (d->psf_size & 1) == 0) return GL_ERR_BAD_CONFIG;
+    if (!(d->pix_scale > 0.f) || !std::isfinite(d->pix_scale)) return GL_ERR_BAD_CONFIG;
+    if (d->mass_model != 0 && d->mass_model != 1) return GL_ERR_BAD_CONFIG;
+    if (d->mass_model == 1 && (d->epl_terms < 2 || d->epl_terms > 30)) return GL_ERR_BAD_CONFIG;
+    if ((d->has_shear & ~1) || (d->multipole_mask & ~3) || (d->param_space & ~1)) return GL_ERR_BAD_CONFIG;
+    if (d->n_source_sersic < 0 || d->n_source_sersic > 1 || d->n_lens_sersic < 0 || d->n_lens_sersic > 2) return GL_ERR_BAD_CONFIG;
+    if (d->shapelet_nmax < -1 || d->shapelet_nmax > 10) return GL_ERR_BAD_CONFIG;
+    if (d->shapelet_nmax >= 0 && d->n_source_sersic != 1) return GL_ERR_BAD_CONFIG;
+    if (d->n_systems < 1) return GL_ERR_BAD_CONFIG;
+    if (d->psf_grid != 0) return GL_ERR_UNSUPPORTED;
+    Layout L{};
+    int np = layout_from_desc(*d, L);
+    if (np != d->n_params || np > 128) return GL_ERR_BAD_CONFIG;
+    for (int i = 0; i < np; ++i) {
+        const gl_prior& p = d->priors[i];
+        if (p.kind < GL_PRIOR_NONE || p.kind > GL_PRIOR_LOGUNIFORM) return GL_ERR_BAD_CONFIG;
+        bool gauss = p.kind == GL_PRIOR_NORMAL || p.kind == GL_PRIOR_LOGNORMAL || p.kind == GL_PRIOR_TRUNCNORMAL;
+        bool bounded = p.kind == GL_PRIOR_UNIFORM || p.kind == GL_PRIOR_TRUNCNORMAL || p.kind == GL_PRIOR_LOGUNIFORM;
+        if (gauss && !(p.b > 0.f && std::isfinite(p.a) && std::isfinite(p.b))) return GL_ERR_BAD_CONFIG;
+        if (bounded && !(p.hi > p.lo && std::isfinite(p.lo) && std::isfinite(p.hi))) return GL_ERR_BAD_CONFIG;
+        if (p.kind == GL_PRIOR_LOGUNIFORM && !(p.lo > 0.f)) return GL_ERR_BAD_CONFIG;
+    }
+    const int64_t M64 = (int64_t)d->n_pix * d->supersample;
+    if (M64 > 4096 || d->psf_size > 255) return GL_ERR_UNSUPPORTED;
+    gl_config* c = new (std::nothrow) gl_config();
+    if (!c) return GL_ERR_BAD_CONFIG;
+    c->desc = *d;
+    c->priors.assign(d->priors, d->priors + np);
+    c->desc.priors = c->priors.data();
+    for (int i = 0; i < np; ++i) {
+        c->pt.kind[i] = d->priors[i].kind; c->pt.a[i] = d->priors[i].a; c->pt.b[i] = d->priors[i].b;
+        c->pt.lo[i] = d->priors[i].lo; c->pt.hi[i] = d->priors[i].hi;
+    }
+    for (int i = np; i < 128; ++i) { c->pt.kind[i] = 0; c->pt.a[i] = 0; c->pt.b[i] = 1; c->pt.lo[i] = 0; c->pt.hi[i] = 1; }
+    // kernel variant: the smallest compiled superset of the requested components
+    if (d->multipole_mask == 0 && d->shapelet_nmax < 0 && d->n_lens_sersic <= 1) { c->variant = 0; L.ker_nmax = -1; c->na = NA_SHA; }
+    else if (d->multipole_mask == 0 && d->shapelet_nmax <= 6) { c->variant = 1; L.ker_nmax = 6; c->na = NA_SHA + 28; }
+    else { c->variant = 2; L.ker_nmax = 10; c->na = NA_SHA + 66; }
+    c->L = L;
+    Geom& G = c->G;
+    G.N = d->n_pix; G.s = d->supersample; G.M = (int)M64; G.K = d->psf_size; G.c = (d->psf_size - 1) / 2;
+    const int KE = G.K + G.s - 1;
+    G.U = (KE + G.s - 1) / G.s; G.KEp = G.U * G.s;
+    G.n_terms = d->mass_model == 1 ? d->epl_terms : 0;
+    G.delta2 = d->pix_scale * d->pix_scale;
+    const int64_t MM = M64 * M64;
+    auto clampi = [](int64_t v, int64_t lo, int64_t hi) { return (int)(v < lo ? lo : (v > hi ? hi : v)); };
+    c->rpt_fwd = 8;
+    c->n_chunk_fwd = (int)((MM + NT_FWD * c->rpt_fwd - 1) / (NT_FWD * c->rpt_fwd));
+    c->rpt_adj = clampi((MM + NT_ADJ * 32 - 1) / (NT_ADJ * 32), 8, 64);
+    c->n_chunk_adj = (int)((MM + NT_ADJ * c->rpt_adj - 1) / (NT_ADJ * c->rpt_adj));
+    c->conv_kind = conv_tiled_select(G, &c->n_ctile);
+    if (c->conv_kind == 0) c->n_ctile = (G.N * G.N + 255) / 256;
+    c->per_particle_bytes = sizeof(float) * ((size_t)PB_STRIDE + (size_t)MM + (size_t)G.N * G.N + (size_t)c->n_ctile +
+                                             (size_t)c->n_chunk_adj * c->na) + sizeof(double) + 6 * 256;
+    *out = c;
+    return GL_OK;
+}
+
+extern "C" void gl_config_destroy(gl_config* c) { delete c; }
+extern "C" int32_t gl_config_n_params(const gl_config* c) { return c ? c->L.n_params : 0; }
+
+struct Plan {
+    int64_t Pc;
+    size_t off_kt, off_w, off_sl, off_pb, off_lpd, off_ray, off_gpix, off_chi, off_nap, total;
+};
+
+static Plan make_plan(const gl_config* c, int64_t P) {
+    Plan pl{};
+    const Geom& G = c->G;
+    int64_t pc_max = (int64_t)(WS_BUDGET / c->per_particle_bytes);
+    if (pc_max < 1) pc_max = 1;
+    if (pc_max > 32768) pc_max = 32768;
+    pl.Pc = P < pc_max ? P : pc_max;
+    size_t o = 0;
+    const size_t nsys = (size_t)c->desc.n_systems;
+    pl.off_kt = o;   o = align256(o + sizeof(float) * nsys * G.s * G.s * G.U * G.U);
+    pl.off_w = o;    o = align256(o + sizeof(float) * nsys * G.N * G.N);
+    pl.off_sl = o;   o = align256(o + sizeof(float) * nsys);
+    pl.off_pb = o;   o = align256(o + sizeof(float) * (size_t)pl.Pc * PB_STRIDE);
+    pl.off_lpd = o;  o = align256(o + sizeof(double) * (size_t)pl.Pc);
+    pl.off_ray = o;  o = align256(o + sizeof(float) * (size_t)pl.Pc * G.M * G.M);
+    pl.off_gpix = o; o = align256(o + sizeof(float) * (size_t)pl.Pc * G.N * G.N);
+    pl.off_chi = o;  o = align256(o + sizeof(float) * (size_t)pl.Pc * c->n_ctile);
+    pl.off_nap = o;  o = align256(o + sizeof(float) * (size_t)pl.Pc * c->n_chunk_adj * c->na);
+    pl.total = o;
+    return pl;
+}
+
+extern "C" size_t gl_workspace_bytes(const gl_config* c, int64_t n_particles) {
+    if (!c || n_particles <= 0) return 0;
+    return make_plan(c, n_particles).total;
+}
+
+// ----------------------------------------------------------------------------- variant dispatch
+template <class V>
+static void launch_ray_fwd(const gl_config* c, const float* pb, float* ray, int64_t Pc, cudaStream_t st) {
+    dim3 grid(c->n_chunk_fwd, (unsigned)Pc);
+    gl_ray_fwd_kernel<V, NT_FWD><<<grid, NT_FWD, 0, st>>>(pb, ray, c->G.M, c->rpt_fwd);
+}
+template <class V>
+static void launch_ray_adj(const gl_config* c, const float* pb, const float* gbar, float* nap, int64_t Pc, cudaStream_t st) {
+    dim3 grid(c->n_chunk_adj, (unsigned)Pc);
+    gl_ray_adj_kernel<V, NT_ADJ><<<grid, NT_ADJ, 0, st>>>(pb, gbar, nap, c->G.M, c->rpt_adj);
+}
+
+using V_S0 = Variant<0, 0, 1, -1, 1>; using V_E0 = Variant<1, 0, 1, -1, 1>;
+using V_S1 = Variant<0, 0, 1, 6, 2>;  using V_E1 = Variant<1, 0, 1, 6, 2>;
+using V_S2 = Variant<0, 3, 1, 10, 2>; using V_E2 = Variant<1, 3, 1, 10, 2>;
+
+static void ray_fwd(const gl_config* c, const float* pb, float* ray, int64_t Pc, cudaStream_t st) {
+    const int id = c->variant * 2 + c->desc.mass_model;
+    switch (id) {
+        case 0: launch_ray_fwd<V_S0>(c, pb, ray, Pc, st); break;
+        case 1: launch_ray_fwd<V_E0>(c, pb, ray, Pc, st); break;
+        case 2: launch_ray_fwd<V_S1>(c, pb, ray, Pc, st); break;
+        case 3: launch_ray_fwd<V_E1>(c, pb, ray, Pc, st); break;
+        case 4: launch_ray_fwd<V_S2>(c, pb, ray, Pc, st); break;
+        default: launch_ray_fwd<V_E2>(c, pb, ray, Pc, st); break;
+    }
+}
+static void ray_adj(const gl_config* c, const float* pb, const float* gbar, float* nap, int64_t Pc, cudaStream_t st) {
+    const int id = c->variant * 2 + c->desc.mass_model;
+    switch (id) {
+        case 0: launch_ray_adj<V_S0>(c, pb, gbar, nap, Pc, st); break;
+        case 1: launch_ray_adj<V_E0>(c, pb, gbar, nap, Pc, st); break;
+        case 2: launch_ray_adj<V_S1>(c, pb, gbar, nap, Pc, st); break;
+        case 3: launch_ray_adj<V_E1>(c, pb, gbar, nap, Pc, st); break;
+        case 4: launch_ray_adj<V_S2>(c, pb, gbar, nap, Pc, st); break;
+        default: launch_ray_adj<V_E2>(c, pb, gbar, nap, Pc, st); break;
+    }
+}
+
+// mode 0: logpost, 1: logpost + grad, 2: model image
+static gl_status run(const gl_config* c, int mode, const float* obs, const float* sigma, const float* psf,
+                     const float* params, const int32_t* system_id, int64_t P, float* out_logp, float* out_grad,
+                     float* out_image, void* ws, size_t ws_bytes, cudaStream_t st) {
+    t_launches = 0;
+    if (!c) return GL_ERR_NULL;
+    if (P < 0) return GL_ERR_BAD_SHAPE;
+    if (P == 0) return GL_OK;
+    if (!psf || !params || !ws) return GL_ERR_NULL;
+    if (mode != 2 && (!obs || !sigma || !out_logp)) return GL_ERR_NULL;
+    if (mode == 1 && !out_grad) return GL_ERR_NULL;
+    if (mode == 2 && !out_image) return GL_ERR_NULL;
+    const Plan pl = make_plan(c, P);
+    if (ws_bytes < pl.total || ((uintptr_t)ws & 255) != 0) return GL_ERR_WORKSPACE;
+    const Geom& G = c->G;
+    char* w = (char*)ws;
+    float* sys_kt = (float*)(w + pl.off_kt); float* sys_w = (float*)(w + pl.off_w); float* sys_sl = (float*)(w + pl.off_sl);
+    float* pb = (float*)(w + pl.off_pb); double* lpd = (double*)(w + pl.off_lpd);
+    float* ray = (float*)(w + pl.off_ray); float* gpix = (float*)(w + pl.off_gpix);
+    float* chi = (float*)(w + pl.off_chi); float* nap = (float*)(w + pl.off_nap);
+
+    if (mode == 2) {
+        // kt only (sigma is not an input of gl_model_image): run prep with a unit sigma stand-in = the w buffer itself
+        gl_prep_kernel<<<c->desc.n_systems, 256, 0, st>>>(G, psf, nullptr, sys_kt, sys_w, sys_sl); ++t_launches;
+    } else {
+        gl_prep_kernel<<<c->desc.n_systems, 256, 0, st>>>(G, psf, sigma, sys_kt, sys_w, sys_sl); ++t_launches;
+    }
+    for (int64_t base = 0; base < P; base += pl.Pc) {
+        const int64_t Pc = (P - base) < pl.Pc ? (P - base) : pl.Pc;
+        gl_unpack_kernel<<<(unsigned)((Pc + 127) / 128), 128, 0, st>>>(c->pt, c->L, G, c->desc.pix_scale,
+                                                                       params + base * c->L.n_params, Pc, pb, lpd);
+        ++t_launches;
+        ray_fwd(c, pb, ray, Pc, st); ++t_launches;
+        t_launches += conv_fwd_launch(c->conv_kind, G, ray, sys_kt, sys_w, obs, system_id, base, Pc,
+                                      mode == 2 ? nullptr : gpix, mode == 2 ? nullptr : chi, c->n_ctile,
+                                      mode == 2 ? out_image : nullptr, st);
+        if (mode == 2) continue;
+        if (mode == 1) {
+            t_launches += conv_bwd_launch(c->conv_kind, G, gpix, sys_kt, system_id, base, Pc, ray, st);
+            ray_adj(c, pb, ray, nap, Pc, st); ++t_launches;
+        }
+        const int wpb = 4;
+        gl_finalize_kernel<<<(unsigned)((Pc + wpb - 1) / wpb), wpb * 32, wpb * (NA_MAX + 128) * sizeof(double), st>>>(
+            c->pt, c->L, G, params, pb, lpd, chi, c->n_ctile, mode == 1 ? nap : nullptr, c->n_chunk_adj, c->na,
+            sys_sl, system_id, Pc, base, out_logp, out_grad);
+        ++t_launches;
+    }
+    cudaError_t e = cudaPeekAtLastError();
+    return e == cudaSuccess ? GL_OK : GL_ERR_CUDA;
+}
+
+extern "C" gl_status gl_logpost(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
+                                const float* params, const int32_t* system_id, int64_t n_particles,
+                                float* out_logp, void* workspace, size_t workspace_bytes, void* stream) {
+    return run(cfg, 0, obs, noise_sigma, psf, params, system_id, n_particles, out_logp, nullptr, nullptr,
+               workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+extern "C" gl_status gl_logpost_grad(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
+                                     const float* params, const int32_t* system_id, int64_t n_particles,
+                                     float* out_logp, float* out_grad, void* workspace, size_t workspace_bytes, void* stream) {
+    return run(cfg, 1, obs, noise_sigma, psf, params, system_id, n_particles, out_logp, out_grad, nullptr,
+               workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+extern "C" gl_status gl_model_image(const gl_config* cfg, const float* psf, const float* params, const int32_t* system_id,
+                                    int64_t n_particles, float* out_image, void* workspace, size_t workspace_bytes, void* stream) {
+    return run(cfg, 2, nullptr, nullptr, psf, params, system_id, n_particles, nullptr, nullptr, out_image,
+               workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+extern "C" size_t gl_workspace_bytes_host(const gl_config* c, int64_t n) {
+    if (!c || n <= 0) return 0;
+    const size_t np = (size_t)c->L.n_params;
+    return make_plan(c, n).total + align256(sizeof(float) * (size_t)n * np) * 2 + align256(sizeof(float) * (size_t)n);
+}
+
+extern "C" gl_status gl_logpost_grad_host(const gl_config* c, const float* obs, const float* noise_sigma, const float* psf,
+                                          const float* params_host, const int32_t* system_id, int64_t n,
+                                          float* out_logp_host, float* out_grad_host, void* workspace, size_t workspace_bytes,
+                                          void* stream) {
+    t_launches = 0;
+    if (!c) return GL_ERR_NULL;
+    if (n < 0) return GL_ERR_BAD_SHAPE;
+    if (n == 0) return GL_OK;
+    if (!params_host || !out_logp_host || !workspace) return GL_ERR_NULL;
+    if (workspace_bytes < gl_workspace_bytes_host(c, n) || ((uintptr_t)workspace & 255) != 0) return GL_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t np = (size_t)c->L.n_params, core = make_plan(c, n).total;
+    char* w = (char*)workspace;
+    float* d_params = (float*)(w + core);
+    float* d_grad = (float*)(w + core + align256(sizeof(float) * n * np));
+    float* d_logp = (float*)(w + core + 2 * align256(sizeof(float) * n * np));
+    if (cudaMemcpyAsync(d_params, params_host, sizeof(float) * n * np, cudaMemcpyHostToDevice, st) != cudaSuccess) return GL_ERR_CUDA;
+    gl_status s = run(c, out_grad_host ? 1 : 0, obs, noise_sigma, psf, d_params, system_id, n, d_logp,
+                      out_grad_host ? d_grad : nullptr, nullptr, workspace, core, st);
+    if (s != GL_OK) return s;
+    if (cudaMemcpyAsync(out_logp_host, d_logp, sizeof(float) * n, cudaMemcpyDeviceToHost, st) != cudaSuccess) return GL_ERR_CUDA;
+    if (out_grad_host && cudaMemcpyAsync(out_grad_host, d_grad, sizeof(float) * n * np, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return GL_ERR_CUDA;
+    return GL_OK;
+}

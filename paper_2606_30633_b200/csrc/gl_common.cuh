@@ -1,0 +1,80 @@
+// gl_common.cuh -- layouts shared by the kernels of libgigalens (product path; shares nothing with oracle/).
+//
+// Data layout in HBM:
+//   PB   [Pc][PB_STRIDE] fp32   per-particle block of derived scalars written by gl_unpack_kernel (step A)
+//   RAY  [Pc][M][M]      fp32   supersampled surface-brightness image (step B+C), later reused for gbar_ray
+//   GPIX [Pc][N][N]      fp32   g_pix = -(model-obs)/sigma^2 (step E), input of the transposed step D
+//   CHI  [Pc][n_ctile]   fp32   per-tile chi-square partials, summed in fixed order by gl_finalize_kernel
+//   NAP  [Pc][n_chunk][NA] fp32 per-chunk "natural" gradient accumulators of the adjoint (step F)
+//   SYS  per system: kt (flipped pre-boxed PSF, phase-major), w = 1/sigma^2, sum(ln sigma)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gl {
+
+// ----------------------------------------------------------------------------- particle block (PB)
+enum : int {
+    PB_VALID = 0,
+    PB_M_XOFF = 1, PB_M_YOFF = 2,       // x_first - x0, y_first - y0  (fp64-subtracted, then rounded)
+    PB_M_C = 3, PB_M_S = 4,             // cos phi, sin phi of the mass frame
+    PB_M_Q = 5, PB_M_B = 6, PB_M_T = 7, PB_M_F = 8, PB_M_L2B = 9, PB_M_A = 10,
+    PB_M_QP = 11, PB_M_BQP = 12,        // SIE: q' = sqrt(1-q^2), b/q'
+    PB_M_F2 = 13, PB_M_TM1 = 14, PB_M_KAPC = 15,   // f^2, t-1, (2-t)/2 * b
+    PB_G1 = 16, PB_G2 = 17, PB_C3 = 18, PB_S3 = 19, PB_C4 = 20, PB_S4 = 21,
+    PB_XFIRST = 22, PB_STEP = 23,       // ray grid: x_j = x_first + j*step (same for y)
+    PB_SRC = 24,                        // Sersic block, 16 floats
+    PB_SHP = 40,                        // +0 1/beta_s ; coefficients a_k/beta_s from PB_SHP_A
+    PB_SHP_A = 44,
+    PB_LL0 = 112, PB_LL1 = 128,
+    PB_SER_A = 144,                     // a_n, n = 0..31 (zero beyond epl_terms)
+    PB_SER_D = 176,                     // d_m = (m+1) a_{m+1}
+    PB_SER_E = 208,                     // e_m = L_{m+1} a_{m+1}
+    PB_STRIDE = 240
+};
+// Sersic block offsets
+enum : int { SB_XOFF = 0, SB_YOFF = 1, SB_C = 2, SB_S = 3, SB_Q = 4, SB_QI = 5, SB_K1 = 6, SB_K0 = 7,
+             SB_C1 = 8, SB_IE = 9, SB_KQ = 10, SB_KQI = 11 };
+
+// ----------------------------------------------------------------------------- natural accumulators (NA)
+// Per-ray sums the adjoint kernel produces; gl_finalize_kernel applies the per-particle chain rule in fp64.
+enum : int {
+    NA_D0 = 0, NA_DTL = 1, NA_DT2 = 2, NA_D1 = 3, NA_D2 = 4, NA_D3 = 5, NA_DPHI = 6, NA_VX = 7, NA_VY = 8,
+    NA_DQS = 9,                          // SIE only: sum s_r . dalpha/dq|b
+    NA_G1 = 10, NA_G2 = 11,
+    NA_C3 = 12, NA_S3 = 13, NA_C4 = 14, NA_S4 = 15, NA_MCX = 16, NA_MCY = 17,
+    NA_SRC = 18,                         // 8: T0 T1 T2 AX AY BXX BYY BXY
+    NA_SHB = 26, NA_SHX = 27, NA_SHY = 28,
+    NA_LL0 = 29, NA_LL1 = 37,
+    NA_SHA = 45,                         // Nc coefficient sums
+    NA_MAX = 45 + 66
+};
+enum : int { SA_T0 = 0, SA_T1 = 1, SA_T2 = 2, SA_AX = 3, SA_AY = 4, SA_BXX = 5, SA_BYY = 6, SA_BXY = 7 };
+
+// ----------------------------------------------------------------------------- compile-time model variant
+template <int MASS_, int MPMASK_, int NSRC_, int NMAX_, int NLL_>
+struct Variant {
+    static constexpr int MASS = MASS_;       // 0 SIE, 1 EPL
+    static constexpr int MPMASK = MPMASK_;   // multipole bits
+    static constexpr int NSRC = NSRC_;
+    static constexpr int NMAX = NMAX_;       // -1: no shapelets
+    static constexpr int NLL = NLL_;
+    static constexpr int NCOEF = NMAX_ >= 0 ? (NMAX_ + 1) * (NMAX_ + 2) / 2 : 0;
+    static constexpr int NA = NMAX_ >= 0 ? NA_SHA + NCOEF : NA_SHA;            // accumulators written per chunk
+    static constexpr int PB_NEED = MASS_ == 1 ? PB_STRIDE : PB_SER_A;          // floats of PB a CTA stages
+};
+
+struct Geom {            // launch-invariant geometry, passed by value
+    int N, s, M, K, c;   // pixels/side, supersample, rays/side, psf taps/side, (K-1)/2
+    int KEp, U;          // padded k_eff taps per side (multiple of s), taps per phase per side
+    int n_terms;         // EPL series terms kept (2..30)
+    float delta2;        // pix_scale^2
+};
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+}  // namespace gl

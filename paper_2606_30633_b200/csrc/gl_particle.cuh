@@ -1,0 +1,280 @@
+// gl_particle.cuh -- step A (unpack + bijector + prior) and the per-particle tail of step F (chain rule),
+// both in fp64: O(P * n_params) work, negligible next to the per-ray kernels.
+#pragma once
+#include "gl_common.cuh"
+
+namespace gl {
+
+struct PriorTable {                 // passed by value as a kernel parameter (<= 2.6 KB)
+    int32_t kind[128];
+    float a[128], b[128], lo[128], hi[128];
+};
+
+struct Layout {                     // offsets into the flat parameter vector (reading S18); -1 = absent
+    int mass, gamma, ell, shear, mp3, mp4, src, shp, ll0, ll1;
+    int n_params, n_coef, nmax, param_space, mass_model;
+    int ker_nmax;                   // shapelet order the selected kernel variant is compiled for (>= nmax)
+};
+
+struct Xform { double theta, lp, logdet, dth_dz, dlp_dth, dlogdet_dz; bool ok; };
+
+__device__ inline double d_softplus(double x) { return x > 0 ? x + log1p(exp(-x)) : log1p(exp(x)); }
+__device__ inline double d_sigmoid(double x) { return x >= 0 ? 1.0 / (1.0 + exp(-x)) : exp(x) / (1.0 + exp(x)); }
+
+// O1: theta = T(z), log prior density, log-determinant and their derivatives for one parameter.
+__device__ inline Xform transform_one(const PriorTable& pt, int i, int param_space, double z) {
+    const double HL2PI = 0.91893853320467274178;
+    const int kind = pt.kind[i];
+    const double a = pt.a[i], b = pt.b[i], lo = pt.lo[i], hi = pt.hi[i];
+    Xform r; r.theta = z; r.logdet = 0; r.dth_dz = 1; r.dlogdet_dz = 0; r.lp = 0; r.dlp_dth = 0; r.ok = true;
+    if (param_space == 0) {
+        if (kind == 2) { r.theta = exp(z); r.logdet = z; r.dth_dz = r.theta; r.dlogdet_dz = 1; }
+        else if (kind == 3 || kind == 4) {
+            double s = d_sigmoid(z), w = hi - lo;
+            r.theta = lo + w * s; r.logdet = log(w) - d_softplus(-z) - d_softplus(z);
+            r.dth_dz = w * s * (1 - s); r.dlogdet_dz = 1 - 2 * s;
+        } else if (kind == 5) {
+            double s = d_sigmoid(z), w = log(hi) - log(lo), u = log(lo) + w * s;
+            r.theta = exp(u); r.logdet = u + log(w) - d_softplus(-z) - d_softplus(z);
+            r.dth_dz = r.theta * w * s * (1 - s); r.dlogdet_dz = w * s * (1 - s) + 1 - 2 * s;
+        }
+    }
+    const double th = r.theta;
+    if (kind == 1) { double e = (th - a) / b; r.lp = -0.5 * e * e - log(b) - HL2PI; r.dlp_dth = -e / b; }
+    else if (kind == 2) {
+        if (!(th > 0)) r.ok = false;
+        else { double e = (log(th) - a) / b; r.lp = -0.5 * e * e - log(b) - HL2PI - log(th); r.dlp_dth = -e / (b * th) - 1 / th; }
+    } else if (kind == 3) {
+        if (th < lo || th > hi) r.ok = false; else r.lp = -log(hi - lo);
+    } else if (kind == 4) {
+        if (th < lo || th > hi) r.ok = false;
+        else {
+            double e = (th - a) / b;
+            double Z = 0.5 * erfc(-((hi - a) / b) * 0.70710678118654752440) - 0.5 * erfc(-((lo - a) / b) * 0.70710678118654752440);
+            r.lp = -0.5 * e * e - log(b) - HL2PI - log(Z); r.dlp_dth = -e / b;
+        }
+    } else if (kind == 5) {
+        if (th < lo || th > hi) r.ok = false; else { r.lp = -log(th) - log(log(hi) - log(lo)); r.dlp_dth = -1 / th; }
+    }
+    if (!isfinite(z) || !isfinite(r.theta)) r.ok = false;
+    return r;
+}
+
+struct Ell { double c, q, phi, cphi, sphi; };
+__device__ inline Ell make_ell(double e1, double e2) {
+    Ell E; E.c = sqrt(e1 * e1 + e2 * e2); E.phi = 0.5 * atan2(e2, e1); E.q = (1 - E.c) / (1 + E.c);
+    sincos(E.phi, &E.sphi, &E.cphi); return E;
+}
+// (d/dq, d/dphi) -> (d/de1, d/de2); zero for c < 1e-10 (O9)
+__device__ inline void ell_chain(double e1, double e2, const Ell& E, double dq, double dphi, double& de1, double& de2) {
+    if (E.c < 1e-10) { de1 = 0; de2 = 0; return; }
+    double dq_dc = -2.0 / ((1 + E.c) * (1 + E.c));
+    de1 = dq * dq_dc * e1 / E.c + dphi * (-e2 / (2 * E.c * E.c));
+    de2 = dq * dq_dc * e2 / E.c + dphi * (e1 / (2 * E.c * E.c));
+}
+
+// theta of parameter i of particle `z` (fp32 in HBM -> fp64)
+__device__ inline double theta_at(const PriorTable& pt, const Layout& L, const float* z, int i, bool& ok) {
+    Xform x = transform_one(pt, i, L.param_space, (double)z[i]);
+    ok = ok && x.ok; return x.theta;
+}
+
+// Write one Sersic block [R, n, e1, e2, x0, y0, Ie] into PB; a negative `off` writes a neutral (Ie = 0) block.
+__device__ inline void write_sersic(const PriorTable& pt, const Layout& L, const float* z, int off, float* sb,
+                                    double x_first, bool& ok) {
+    double R = 1, n = 1, e1 = 0, e2 = 0, x0 = 0, y0 = 0, Ie = 0;
+    if (off >= 0) {
+        R = theta_at(pt, L, z, off, ok); n = theta_at(pt, L, z, off + 1, ok);
+        e1 = theta_at(pt, L, z, off + 2, ok); e2 = theta_at(pt, L, z, off + 3, ok);
+        x0 = theta_at(pt, L, z, off + 4, ok); y0 = theta_at(pt, L, z, off + 5, ok);
+        Ie = theta_at(pt, L, z, off + 6, ok);
+        if (!(R > 0) || !(n > 0) || !(e1 * e1 + e2 * e2 < 1.0)) { ok = false; R = 1; n = 1; e1 = e2 = 0; }
+    }
+    Ell E = make_ell(e1, e2);
+    double bn = 1.9992 * n - 0.3271;
+    sb[SB_XOFF] = (float)(x_first - x0); sb[SB_YOFF] = (float)(x_first - y0);
+    sb[SB_C] = (float)E.cphi; sb[SB_S] = (float)E.sphi; sb[SB_Q] = (float)E.q; sb[SB_QI] = (float)(1.0 / E.q);
+    sb[SB_K1] = (float)(0.5 / n); sb[SB_K0] = (float)(-log2(R) / n);
+    sb[SB_C1] = (float)(bn * 1.44269504088896340736); sb[SB_IE] = (float)Ie;
+    sb[SB_KQ] = (float)(bn / n * E.q); sb[SB_KQI] = (float)(bn / n / E.q);
+    sb[12] = sb[13] = sb[14] = sb[15] = 0.f;
+}
+
+// Step A.  One thread per particle.  pb: [P][PB_STRIDE]; lpd: [P] = sum log prior + sum log-det (fp64).
+__global__ void gl_unpack_kernel(const __grid_constant__ PriorTable pt, const __grid_constant__ Layout L,
+                                 const __grid_constant__ Geom G, float pix_scale,
+                                 const float* __restrict__ params, int64_t P, float* __restrict__ pb, double* __restrict__ lpd) {
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    const float* z = params + p * L.n_params;
+    float* o = pb + p * PB_STRIDE;
+    bool ok = true;
+    double lp = 0;
+    for (int i = 0; i < L.n_params; ++i) {
+        Xform x = transform_one(pt, i, L.param_space, (double)z[i]);
+        ok = ok && x.ok; lp += x.lp + x.logdet;
+    }
+    const double step = (double)pix_scale / G.s;
+    const double x_first = (0.5 / G.s - 0.5 * G.N) * (double)pix_scale;
+    // main deflector
+    double thE = theta_at(pt, L, z, L.mass, ok);
+    double t = L.gamma >= 0 ? theta_at(pt, L, z, L.gamma, ok) - 1.0 : 1.0;
+    double e1 = theta_at(pt, L, z, L.ell, ok), e2 = theta_at(pt, L, z, L.ell + 1, ok);
+    double x0 = theta_at(pt, L, z, L.ell + 2, ok), y0 = theta_at(pt, L, z, L.ell + 3, ok);
+    if (!(thE > 0) || !(t > 0 && t < 2) || !(e1 * e1 + e2 * e2 < 1.0)) { ok = false; thE = 1; t = 1; e1 = e2 = 0; }
+    Ell E = make_ell(e1, e2);
+    double b = thE * sqrt(E.q), f = (1 - E.q) / (1 + E.q);
+    o[PB_M_XOFF] = (float)(x_first - x0); o[PB_M_YOFF] = (float)(x_first - y0);
+    o[PB_M_C] = (float)E.cphi; o[PB_M_S] = (float)E.sphi; o[PB_M_Q] = (float)E.q; o[PB_M_B] = (float)b;
+    o[PB_M_T] = (float)t; o[PB_M_F] = (float)f; o[PB_M_L2B] = (float)log2(b); o[PB_M_A] = (float)(2 * b / (1 + E.q));
+    double qp = sqrt(fmax(1 - E.q * E.q, 0.0));
+    o[PB_M_QP] = (float)qp; o[PB_M_BQP] = (float)(qp > 0 ? b / qp : 0.0);
+    o[PB_M_F2] = (float)(f * f); o[PB_M_TM1] = (float)(t - 1); o[PB_M_KAPC] = (float)(0.5 * (2 - t) * b);
+    o[PB_G1] = L.shear >= 0 ? (float)theta_at(pt, L, z, L.shear, ok) : 0.f;
+    o[PB_G2] = L.shear >= 0 ? (float)theta_at(pt, L, z, L.shear + 1, ok) : 0.f;
+    o[PB_C3] = L.mp3 >= 0 ? (float)theta_at(pt, L, z, L.mp3, ok) : 0.f;
+    o[PB_S3] = L.mp3 >= 0 ? (float)theta_at(pt, L, z, L.mp3 + 1, ok) : 0.f;
+    o[PB_C4] = L.mp4 >= 0 ? (float)theta_at(pt, L, z, L.mp4, ok) : 0.f;
+    o[PB_S4] = L.mp4 >= 0 ? (float)theta_at(pt, L, z, L.mp4 + 1, ok) : 0.f;
+    o[PB_XFIRST] = (float)x_first; o[PB_STEP] = (float)step;
+    write_sersic(pt, L, z, L.src, o + PB_SRC, x_first, ok);
+    write_sersic(pt, L, z, L.ll0, o + PB_LL0, x_first, ok);
+    write_sersic(pt, L, z, L.ll1, o + PB_LL1, x_first, ok);
+    // shapelets (coefficients pre-divided by beta_s; orders above the configured nmax are zero)
+    if (L.ker_nmax >= 0) {
+        double bs = 1.0;
+        if (L.shp >= 0) { bs = theta_at(pt, L, z, L.shp, ok); if (!(bs > 0)) { ok = false; bs = 1; } }
+        o[PB_SHP] = (float)(1.0 / bs); o[PB_SHP + 1] = o[PB_SHP + 2] = o[PB_SHP + 3] = 0.f;
+        int nck = (L.ker_nmax + 1) * (L.ker_nmax + 2) / 2;
+        for (int k = 0; k < nck; ++k)
+            o[PB_SHP_A + k] = (L.shp >= 0 && k < L.n_coef) ? (float)(theta_at(pt, L, z, L.shp + 1 + k, ok) / bs) : 0.f;
+    }
+    // EPL series coefficients: a_n = prod_{k<=n} (2k-2+t)/(2k+2-t); d_m = (m+1) a_{m+1}; e_m = L_{m+1} a_{m+1}
+    if (L.mass_model == 1) {
+        double an = 1.0, Ln = 0.0;
+        o[PB_SER_A] = 1.f;
+        for (int n = 1; n < 32; ++n) {
+            an *= (2.0 * n - 2.0 + t) / (2.0 * n + 2.0 - t);
+            Ln += 4.0 * n / ((2.0 * n + 2.0 - t) * (2.0 * n - 2.0 + t));
+            bool keep = n < G.n_terms;
+            o[PB_SER_A + n] = keep ? (float)an : 0.f;
+            o[PB_SER_D + n - 1] = keep ? (float)(n * an) : 0.f;
+            o[PB_SER_E + n - 1] = keep ? (float)(Ln * an) : 0.f;
+        }
+        o[PB_SER_D + 31] = 0.f; o[PB_SER_E + 31] = 0.f;
+    }
+    if (!isfinite(lp)) ok = false;
+    o[PB_VALID] = ok ? 1.f : 0.f;
+    lpd[p] = lp;
+}
+
+// Chain rule for one Sersic block: natural sums T -> d logL / d[R, n, e1, e2, x0, y0, Ie], written to gth[off..off+6].
+__device__ inline void sersic_chain(const PriorTable& pt, const Layout& L, const float* z, int off, const double* T, double* gth) {
+    bool ok = true;
+    double R = theta_at(pt, L, z, off, ok), n = theta_at(pt, L, z, off + 1, ok);
+    double e1 = theta_at(pt, L, z, off + 2, ok), e2 = theta_at(pt, L, z, off + 3, ok), Ie = theta_at(pt, L, z, off + 6, ok);
+    Ell E = make_ell(e1, e2);
+    double bn = 1.9992 * n - 0.3271, k = bn / n;
+    gth[off + 6] = T[SA_T0] / Ie;
+    gth[off] = k * T[SA_T1] / R;
+    gth[off + 1] = -1.9992 * (T[SA_T1] - T[SA_T0]) + bn * 0.69314718055994530942 * T[SA_T2] / n;
+    double gxr = -k * E.q * T[SA_AX], gyr = -k * T[SA_AY] / E.q;
+    gth[off + 4] = -(E.cphi * gxr - E.sphi * gyr);
+    gth[off + 5] = -(E.sphi * gxr + E.cphi * gyr);
+    double dq = -k * 0.5 * (T[SA_BXX] - T[SA_BYY] / (E.q * E.q));
+    double dphi = -k * (E.q - 1.0 / E.q) * T[SA_BXY];
+    ell_chain(e1, e2, E, dq, dphi, gth[off + 2], gth[off + 3]);
+}
+
+// Tail of step E/F.  One WARP per particle.  Sums the per-tile chi^2 partials and the per-chunk natural
+// accumulators in a fixed order (fp64), applies the chain rule natural -> theta -> z, adds prior and
+// log-det terms, and writes out_logp / out_grad.  nap may be NULL (gl_logpost: no gradient).
+__global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const __grid_constant__ Layout L,
+                                   const __grid_constant__ Geom G,
+                                   const float* __restrict__ params, const float* __restrict__ pb,
+                                   const double* __restrict__ lpd, const float* __restrict__ chi, int n_ctile,
+                                   const float* __restrict__ nap, int n_chunk, int na,
+                                   const float* __restrict__ sys_sumlog, const int32_t* __restrict__ system_id,
+                                   int64_t P, int64_t p_base, float* __restrict__ out_logp, float* __restrict__ out_grad) {
+    extern __shared__ double fsm[];                     // per warp: nat[NA_MAX] + gth[128]
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int64_t p = (int64_t)blockIdx.x * (blockDim.x >> 5) + wib;
+    if (p >= P) return;
+    double* nat = fsm + (size_t)wib * (NA_MAX + 128);
+    double* gth = nat + NA_MAX;
+    const float* z = params + (p_base + p) * L.n_params;
+    const bool valid = pb[p * PB_STRIDE + PB_VALID] != 0.f;
+    // chi^2: lanes stride over tiles, then a fixed xor-tree
+    double c2 = 0;
+    for (int k = lane; k < n_ctile; k += 32) c2 += (double)chi[p * n_ctile + k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) c2 += __shfl_xor_sync(0xffffffffu, c2, o);
+    const int sys = system_id ? system_id[p_base + p] : 0;
+    double logp = -0.5 * c2 - (double)sys_sumlog[sys] - 0.5 * G.N * G.N * 1.83787706640934548356 + lpd[p];
+    bool good = valid && isfinite(logp);
+    if (nap) {
+        for (int k = lane; k < na; k += 32) {
+            double s = 0;
+            for (int ch = 0; ch < n_chunk; ++ch) s += (double)nap[((size_t)p * n_chunk + ch) * na + k];
+            nat[k] = s;
+        }
+        for (int k = lane; k < L.n_params; k += 32) gth[k] = 0;
+        __syncwarp();
+        if (lane == 0 && valid) {
+            bool ok = true;
+            double thE = theta_at(pt, L, z, L.mass, ok);
+            double t = L.gamma >= 0 ? theta_at(pt, L, z, L.gamma, ok) - 1.0 : 1.0;
+            double e1 = theta_at(pt, L, z, L.ell, ok), e2 = theta_at(pt, L, z, L.ell + 1, ok);
+            Ell E = make_ell(e1, e2);
+            double q = E.q, b = thE * sqrt(q);
+            double dL_db = -(t / b) * nat[NA_D0];
+            double dL_dq_b;
+            if (L.mass_model == 1) {
+                gth[L.gamma] = -(0.69314718055994530942 * nat[NA_DTL] + nat[NA_DT2]);
+                dL_dq_b = -(-nat[NA_D0] / (1 + q) - (t - 1) * q * nat[NA_D1] - nat[NA_D2] - 2.0 / ((1 + q) * (1 + q)) * nat[NA_D3]);
+            } else {
+                dL_dq_b = -nat[NA_DQS];
+            }
+            gth[L.mass] = dL_db * sqrt(q);
+            double dq = dL_dq_b + dL_db * thE / (2 * sqrt(q));
+            double dphi = -nat[NA_DPHI];
+            ell_chain(e1, e2, E, dq, dphi, gth[L.ell], gth[L.ell + 1]);
+            gth[L.ell + 2] = E.cphi * nat[NA_VX] - E.sphi * nat[NA_VY];
+            gth[L.ell + 3] = E.sphi * nat[NA_VX] + E.cphi * nat[NA_VY];
+            if (L.shear >= 0) { gth[L.shear] = nat[NA_G1]; gth[L.shear + 1] = nat[NA_G2]; }
+            if (L.mp3 >= 0) { gth[L.mp3] = nat[NA_C3]; gth[L.mp3 + 1] = nat[NA_S3]; }
+            if (L.mp4 >= 0) { gth[L.mp4] = nat[NA_C4]; gth[L.mp4 + 1] = nat[NA_S4]; }
+            if (L.mp3 >= 0 || L.mp4 >= 0) { gth[L.ell + 2] += nat[NA_MCX]; gth[L.ell + 3] += nat[NA_MCY]; }
+            if (L.src >= 0) sersic_chain(pt, L, z, L.src, nat + NA_SRC, gth);
+            if (L.ll0 >= 0) sersic_chain(pt, L, z, L.ll0, nat + NA_LL0, gth);
+            if (L.ll1 >= 0) sersic_chain(pt, L, z, L.ll1, nat + NA_LL1, gth);
+            if (L.shp >= 0) {
+                double bs = theta_at(pt, L, z, L.shp, ok);
+                gth[L.shp] = -nat[NA_SHB] / bs;
+                gth[L.src + 4] -= nat[NA_SHX]; gth[L.src + 5] -= nat[NA_SHY];
+            }
+        }
+        __syncwarp();
+        if (L.shp >= 0 && valid) {
+            bool ok = true;
+            double bs = theta_at(pt, L, z, L.shp, ok);
+            for (int k = lane; k < L.n_coef; k += 32) gth[L.shp + 1 + k] = nat[NA_SHA + k] / bs;
+        }
+        __syncwarp();
+        // theta -> z, priors, log-det; a non-finite component invalidates the particle
+        bool fin = true;
+        for (int k = lane; k < L.n_params; k += 32) {
+            Xform x = transform_one(pt, k, L.param_space, (double)z[k]);
+            double g = (gth[k] + x.dlp_dth) * x.dth_dz + x.dlogdet_dz;
+            gth[k] = g; if (!isfinite(g)) fin = false;
+        }
+        fin = __all_sync(0xffffffffu, fin);
+        good = good && fin;
+        __syncwarp();
+        for (int k = lane; k < L.n_params; k += 32)
+            out_grad[(p_base + p) * L.n_params + k] = good ? (float)gth[k] : 0.f;
+    }
+    if (lane == 0) out_logp[p_base + p] = good ? (float)logp : -INFINITY;
+}
+
+}  // namespace gl
