@@ -121,9 +121,9 @@ def logpost_grad(spec, obs, sigma, psf, params, system_id=None, want_grad=True, 
     return dict(logp=logp, grad=grad, gabs=gabs, model=model)
 
 
-def model_image(spec, psf, theta, epl_terms=None):
-    """Noise-free model image(s) for PHYSICAL parameter rows theta (O3-O6), system 0's PSF unless the
-    spec has one system per row."""
+def model_image(spec, psf, theta, epl_terms=None, system_id=None):
+    """Noise-free model image(s) for PHYSICAL parameter rows theta (O3-O6); row i uses the PSF of system
+    system_id[i] (default: system 0)."""
     N = spec.n_pix
     theta = _f64(theta).reshape(-1, spec.n_params)
     obs = np.zeros((spec.n_systems, N, N)); sig = np.ones((spec.n_systems, N, N))
@@ -134,7 +134,7 @@ def model_image(spec, psf, theta, epl_terms=None):
         "shapelet_nmax n_lens_sersic n_systems n_params").split()})
     s.param_space = 1
     s.priors = [(PRIOR_NONE, 0, 1, 0, 1)] * spec.n_params
-    out = logpost_grad(s, obs, sig, psf, theta, None, want_grad=False, want_model=True, epl_terms=epl_terms)
+    out = logpost_grad(s, obs, sig, psf, theta, system_id, want_grad=False, want_model=True, epl_terms=epl_terms)
     return out["model"]
 
 

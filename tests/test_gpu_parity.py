@@ -1,0 +1,191 @@
+"""Parity of the CUDA path (through the C ABI, via the thin binding) against the fp64 oracle, element by element,
+on the same seeded fp32-rounded inputs.  Bars (BASELINE.json north_star): |dlogp| <= 1e-4 |logp|; per gradient
+component |dg| <= max(1e-3 |g|, 1e-5).  Run on the B200 box: python -m pytest tests -m gpu.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import workloads as W
+from _cases import ATOL_GRAD, RTOL_GRAD, RTOL_LOGP, grad_report, observation, oracle_subset
+
+pytestmark = pytest.mark.gpu
+
+OUT = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+
+
+def _gl():
+    import paper_2606_30633_b200 as gl
+    gl.lib()                                   # fail loudly if the extension is missing
+    return gl
+
+
+def _model(k):
+    import torch
+    gl = _gl()
+    wl, obs, sig = observation(k)
+    m = gl.LensModel(wl.spec, obs, sig, wl.psf)
+    return gl, torch, wl, m
+
+
+def _dump(name, rep):
+    try:
+        os.makedirs(OUT, exist_ok=True)
+        with open(os.path.join(OUT, "parity_%s.json" % name), "w") as f:
+            json.dump(rep, f, indent=1)
+    except OSError:
+        pass
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_parity_subset(k):
+    """All parity-subset particles of config k: logp and every gradient component against the oracle."""
+    gl, torch, wl, m = _model(k)
+    idx, ref = oracle_subset(k)
+    z = torch.from_numpy(wl.params[idx]).cuda()
+    sid = wl.system_id[idx] if wl.system_id is not None else None
+    lp, g = m.logpost_grad(z, sid)
+    lp0 = m.logpost(z, sid)
+    torch.cuda.synchronize()
+    lp, g, lp0 = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64), lp0.cpu().numpy()
+    assert np.array_equal(lp0.astype(np.float64), lp), "gl_logpost and gl_logpost_grad disagree on logp"
+    assert np.all(np.isfinite(ref["logp"])) and np.all(np.isfinite(lp))
+    rel_lp = np.abs(lp - ref["logp"]) / np.abs(ref["logp"])
+    ok, rep = grad_report(g, ref["grad"], ref["gabs"])
+    rep.update(k=k, n_particles=int(len(idx)), max_rel_logp=float(rel_lp.max()))
+    bad = np.argwhere(~ok)
+    rep["failing"] = [dict(particle=int(idx[i]), param=wl.spec.names[j], gpu=float(g[i, j]), oracle=float(ref["grad"][i, j]),
+                           gabs=float(ref["gabs"][i, j])) for i, j in bad[:40]]
+    _dump("cfg%d" % k, rep)
+    assert rel_lp.max() <= RTOL_LOGP, rep
+    assert rep["n_fail"] == 0, rep
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 5])
+def test_model_image_matches_oracle(k):
+    """gl_model_image (steps A-D) against the oracle's model image, pixel by pixel, on a few particles."""
+    import oracle
+    gl, torch, wl, m = _model(k)
+    n = 4 if k != 5 else 2
+    z = wl.params[:n]
+    ref = oracle.logpost_grad(wl.spec, *observation(k)[1:], wl.psf, z.astype(np.float64), None, want_grad=False,
+                              want_model=True)["model"]
+    img = m.model_image(torch.from_numpy(z).cuda()).cpu().numpy().astype(np.float64)
+    scale = np.abs(ref).max(axis=(1, 2), keepdims=True)
+    assert np.max(np.abs(img - ref) / scale) < 2e-5
+
+
+def test_full_batch_rows_are_bit_identical_to_subset_rows():
+    """BASELINE-size launch (config 2, 4096 particles, the configuration bench.py times): rows of the full batch
+    equal the same particles evaluated alone (PAPER.md L83 fn 2: no cross-particle dependence), hence the oracle."""
+    gl, torch, wl, m = _model(2)
+    idx, ref = oracle_subset(2)
+    zf = torch.from_numpy(wl.params).cuda()
+    lpf, gf = m.logpost_grad(zf)
+    lps, gs = m.logpost_grad(zf[torch.from_numpy(idx).cuda()].contiguous())
+    torch.cuda.synchronize()
+    ii = torch.from_numpy(idx).cuda()
+    assert torch.equal(lpf[ii], lps) and torch.equal(gf[ii], gs)
+    # properties that hold at any size: finite or -inf, never NaN; zero gradient rows where -inf
+    assert not torch.isnan(lpf).any() and not torch.isnan(gf).any()
+    dead = torch.isinf(lpf)
+    assert torch.all(gf[dead] == 0)
+
+
+def test_config4_gather_full_size_sampled():
+    """Config 4 at full size (102,400 particles, 100 systems): sampled rows equal the subset run (and the oracle
+    through test_parity_subset[4]); permuting particles permutes results (gather by system_id)."""
+    gl, torch, wl, m = _model(4)
+    idx, ref = oracle_subset(4)
+    zf = torch.from_numpy(wl.params).cuda()
+    sidf = torch.from_numpy(wl.system_id).cuda()
+    lp = torch.empty(zf.shape[0], device="cuda"); g = torch.empty_like(zf)
+    ws = m.workspace(zf.shape[0])
+    gl.gl_logpost_grad(m.h, m.obs, m.noise_sigma, m.psf, zf, sidf, lp, g, ws)
+    ii = torch.from_numpy(idx).cuda()
+    lps = torch.empty(len(idx), device="cuda"); gs = torch.empty((len(idx), zf.shape[1]), device="cuda")
+    gl.gl_logpost_grad(m.h, m.obs, m.noise_sigma, m.psf, zf[ii].contiguous(), sidf[ii].contiguous(), lps, gs, ws)
+    torch.cuda.synchronize()
+    assert torch.equal(lp[ii], lps) and torch.equal(g[ii], gs)
+    rel = np.abs(lps.cpu().numpy().astype(np.float64) - ref["logp"]) / np.abs(ref["logp"])
+    assert rel.max() <= RTOL_LOGP
+
+
+def test_golden_b4_on_gpu():
+    """SURVEY Appendix B4 explicit case (param_space = 1, no priors) through the CUDA path."""
+    import torch
+    gl = _gl()
+    G = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "survey_appendix_b.json")))["B4"]
+    sp = W.LensSpec(6, 2, 3, 0.30, mass_model=0, param_space=1)
+    sp.priors = [W.NoPrior()] * 21
+    k1 = np.array([0.25, 0.5, 0.25]); psf = np.outer(k1, k1)[None]
+    m = gl.LensModel(sp, np.zeros((1, 6, 6)), np.full((1, 6, 6), 0.1), psf)
+    th = torch.tensor([G["theta"]], dtype=torch.float32, device="cuda")
+    lp, g = m.logpost_grad(th)
+    img = m.model_image(th)[0].cpu().numpy()
+    assert abs(float(lp[0]) - G["logL"]) <= 2e-5 * abs(G["logL"])
+    assert abs(img.sum() - G["sum_model"]) <= 1e-5 * G["sum_model"]
+    for key, (i, j) in {"model_0_0": (0, 0), "model_2_3": (2, 3), "model_3_4": (3, 4), "model_5_5": (5, 5)}.items():
+        assert abs(img[i, j] - G[key]) <= 1e-5 * abs(G[key])
+    gg = g[0].cpu().numpy().astype(np.float64); gr = np.array(G["grad"])
+    assert np.all(np.abs(gg - gr) <= np.maximum(RTOL_GRAD * np.abs(gr), ATOL_GRAD))
+
+
+def test_edge_cases_invalid_empty_ragged():
+    import torch
+    gl, torch, wl, m = _model(1)
+    z = torch.from_numpy(wl.params[:7].copy()).cuda()          # ragged: 7 particles
+    lp_ok, g_ok = m.logpost_grad(z)
+    zb = z.clone()
+    zb[1, 0] = float("nan"); zb[3, 1] = 40.0                    # NaN; e1 = 40 -> |eps| >= 1
+    zb[5, 2] = float("inf")
+    lp, g = m.logpost_grad(zb)
+    torch.cuda.synchronize()
+    for i in (1, 3, 5):
+        assert lp[i] == -float("inf") and torch.all(g[i] == 0)
+    for i in (0, 2, 4, 6):                                      # neighbours unaffected, bit for bit
+        assert lp[i] == lp_ok[i] and torch.equal(g[i], g_ok[i])
+    assert not torch.isnan(lp).any() and not torch.isnan(g).any()
+    # empty batch: GL_OK, no launch
+    e = torch.empty((0, wl.spec.n_params), device="cuda")
+    out = torch.empty(0, device="cuda")
+    gl.gl_logpost(m.h, m.obs, m.noise_sigma, m.psf, e, None, out, m.workspace(1))
+    assert gl.gl_last_launch_count() == 0
+    # single particle
+    lp1, g1 = m.logpost_grad(z[:1].contiguous())
+    assert lp1[0] == lp_ok[0] and torch.equal(g1[0], g_ok[0])
+
+
+def test_error_codes_on_device_calls():
+    import torch
+    gl, torch, wl, m = _model(1)
+    z = torch.from_numpy(wl.params[:4]).cuda()
+    out = torch.empty(4, device="cuda")
+    small = torch.empty(256, dtype=torch.uint8, device="cuda")
+    with pytest.raises(gl.GLError) as e:
+        gl.gl_logpost(m.h, m.obs, m.noise_sigma, m.psf, z, None, out, small)
+    assert e.value.status == -5
+    with pytest.raises(gl.GLError) as e:
+        gl.gl_logpost(m.h, None, m.noise_sigma, m.psf, z, None, out, m.workspace(4))
+    assert e.value.status == -1
+
+
+def test_host_buffer_entry_matches_device_entry():
+    import torch
+    gl, torch, wl, m = _model(1)
+    zh = torch.from_numpy(wl.params[:16].copy()).pin_memory()
+    lph = torch.empty(16).pin_memory(); gh = torch.empty((16, wl.spec.n_params)).pin_memory()
+    gl.gl_logpost_grad_host(m.h, m.obs, m.noise_sigma, m.psf, zh, None, lph, gh, m.workspace(16, host=True))
+    torch.cuda.synchronize()
+    lp, g = m.logpost_grad(zh.cuda())
+    assert torch.equal(lp.cpu(), lph) and torch.equal(g.cpu(), gh)
+
+
+def test_determinism_repeat_calls():
+    gl, torch, wl, m = _model(3)
+    z = torch.from_numpy(wl.params[:64]).cuda()
+    a = m.logpost_grad(z); a = (a[0].clone(), a[1].clone())
+    b = m.logpost_grad(z)
+    assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
