@@ -146,6 +146,18 @@ gl_status gl_logpost_grad_host(const gl_config* cfg, const float* obs, const flo
 /* Number of kernel launches the last call on this thread enqueued (bench.py's gpu_launches claim). */
 int64_t gl_last_launch_count(void);
 
+/* Diagnostic per-stage device timing (what bench.py's `roofline` uses).  After gl_stage_timing_enable(1) every
+ * compute call made by THIS host thread records a CUDA event pair around each kernel stage on the caller's stream
+ * (event records only: still no host synchronisation inside the compute call).  gl_stage_times then waits for
+ * the events of the most recent call and writes, per stage, the summed device time in milliseconds to
+ * ms_host[0..n) and the number of launches to launches_host[0..n) (HOST pointers; launches_host may be NULL);
+ * n must be >= gl_stage_count().  Returns gl_stage_count(), or -1 on error.  Stage i is named gl_stage_name(i):
+ * prep, unpack_prior (A), ray_fwd (B+C), conv_chi2 (D+E), conv_transpose (F: D^T), ray_adjoint (F), finalize. */
+void        gl_stage_timing_enable(int32_t on);
+int32_t     gl_stage_count(void);
+const char* gl_stage_name(int32_t i);
+int32_t     gl_stage_times(float* ms_host, int32_t* launches_host, int32_t n);
+
 /* Static string for a status code. */
 const char* gl_status_string(gl_status s);
 

@@ -19,7 +19,8 @@ STATUS = {0: "GL_OK", -1: "GL_ERR_NULL", -2: "GL_ERR_BAD_CONFIG", -3: "GL_ERR_BA
           -5: "GL_ERR_WORKSPACE", -6: "GL_ERR_CUDA"}
 EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_workspace_bytes", "gl_logpost",
            "gl_logpost_grad", "gl_model_image", "gl_workspace_bytes_host", "gl_logpost_grad_host",
-           "gl_last_launch_count", "gl_status_string", "gl_version"]
+           "gl_last_launch_count", "gl_status_string", "gl_version", "gl_stage_timing_enable", "gl_stage_count",
+           "gl_stage_name", "gl_stage_times"]
 
 
 class GLError(RuntimeError):
@@ -74,6 +75,13 @@ def lib():
         L.gl_status_string.restype = C.c_char_p
         L.gl_status_string.argtypes = [C.c_int]
         L.gl_version.restype = C.c_char_p
+        L.gl_stage_timing_enable.restype = None
+        L.gl_stage_timing_enable.argtypes = [C.c_int32]
+        L.gl_stage_count.restype = C.c_int32
+        L.gl_stage_name.restype = C.c_char_p
+        L.gl_stage_name.argtypes = [C.c_int32]
+        L.gl_stage_times.restype = C.c_int32
+        L.gl_stage_times.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_int32), C.c_int32]
         _lib = L
     return _lib
 
@@ -113,6 +121,20 @@ def gl_workspace_bytes_host(h, n):
 
 def gl_last_launch_count():
     return lib().gl_last_launch_count()
+
+
+def gl_stage_timing_enable(on):
+    lib().gl_stage_timing_enable(1 if on else 0)
+
+
+def gl_stage_times():
+    """{stage name: (milliseconds, launches)} of the most recent compute call of this thread (waits for it)."""
+    L = lib()
+    n = L.gl_stage_count()
+    ms = (C.c_float * n)(); cnt = (C.c_int32 * n)()
+    if L.gl_stage_times(ms, cnt, n) != n:
+        raise RuntimeError("gl_stage_times failed")
+    return {L.gl_stage_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(n)}
 
 
 def _torch():

@@ -30,6 +30,46 @@ struct gl_config {
 
 static thread_local int64_t t_launches = 0;
 
+// ----------------------------------------------------------------------------- optional per-stage timing (diagnostic)
+enum { ST_PREP = 0, ST_UNPACK, ST_RAY_FWD, ST_CONV_FWD, ST_CONV_BWD, ST_RAY_ADJ, ST_FINALIZE, ST_COUNT };
+static const char* const k_stage_names[ST_COUNT] = {"prep", "unpack_prior", "ray_fwd", "conv_chi2", "conv_transpose",
+                                                    "ray_adjoint", "finalize"};
+struct StageTimer {
+    bool on = false;
+    std::vector<cudaEvent_t> ev;      // pairs (begin, end)
+    std::vector<int> stage;           // stage id of pair i
+    size_t used = 0;
+    void reset() { used = 0; stage.clear(); }
+    void begin(int id, cudaStream_t st) {
+        if (!on) return;
+        while (ev.size() < 2 * (used + 1)) { cudaEvent_t e; if (cudaEventCreate(&e) != cudaSuccess) { on = false; return; } ev.push_back(e); }
+        stage.push_back(id);
+        cudaEventRecord(ev[2 * used], st);
+    }
+    void end(cudaStream_t st) {
+        if (!on) return;
+        cudaEventRecord(ev[2 * used + 1], st); ++used;
+    }
+};
+static thread_local StageTimer t_timer;
+
+extern "C" void gl_stage_timing_enable(int32_t on) { t_timer.on = on != 0; t_timer.reset(); }
+extern "C" int32_t gl_stage_count(void) { return ST_COUNT; }
+extern "C" const char* gl_stage_name(int32_t i) { return (i >= 0 && i < ST_COUNT) ? k_stage_names[i] : ""; }
+extern "C" int32_t gl_stage_times(float* ms_host, int32_t* launches_host, int32_t n) {
+    if (!ms_host || n < ST_COUNT) return -1;
+    for (int i = 0; i < n; ++i) { ms_host[i] = 0.f; if (launches_host) launches_host[i] = 0; }
+    for (size_t i = 0; i < t_timer.used; ++i) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(t_timer.ev[2 * i + 1]) != cudaSuccess) return -1;
+        if (cudaEventElapsedTime(&ms, t_timer.ev[2 * i], t_timer.ev[2 * i + 1]) != cudaSuccess) return -1;
+        ms_host[t_timer.stage[i]] += ms;
+        if (launches_host) launches_host[t_timer.stage[i]] += 1;
+    }
+    return ST_COUNT;
+}
+#define GL_STAGE(id, st, ...) do { t_timer.begin(id, st); __VA_ARGS__; t_timer.end(st); } while (0)
+
 static constexpr int NT_FWD = 256;
 static constexpr int NT_ADJ = 128;
 static constexpr size_t WS_BUDGET = (size_t)1536 << 20;   // chunk so that per-chunk buffers stay below ~1.5 GiB
@@ -211,6 +251,7 @@ static gl_status run(const gl_config* c, int mode, const float* obs, const float
                      const float* params, const int32_t* system_id, int64_t P, float* out_logp, float* out_grad,
                      float* out_image, void* ws, size_t ws_bytes, cudaStream_t st) {
     t_launches = 0;
+    t_timer.reset();
     if (!c) return GL_ERR_NULL;
     if (P < 0) return GL_ERR_BAD_SHAPE;
     if (P == 0) return GL_OK;
@@ -229,28 +270,28 @@ static gl_status run(const gl_config* c, int mode, const float* obs, const float
 
     if (mode == 2) {
         // kt only (sigma is not an input of gl_model_image): run prep with a unit sigma stand-in = the w buffer itself
-        gl_prep_kernel<<<c->desc.n_systems, 256, 0, st>>>(G, psf, nullptr, sys_kt, sys_w, sys_sl); ++t_launches;
+        GL_STAGE(ST_PREP, st, (gl_prep_kernel<<<c->desc.n_systems, 256, 0, st>>>(G, psf, nullptr, sys_kt, sys_w, sys_sl))); ++t_launches;
     } else {
-        gl_prep_kernel<<<c->desc.n_systems, 256, 0, st>>>(G, psf, sigma, sys_kt, sys_w, sys_sl); ++t_launches;
+        GL_STAGE(ST_PREP, st, (gl_prep_kernel<<<c->desc.n_systems, 256, 0, st>>>(G, psf, sigma, sys_kt, sys_w, sys_sl))); ++t_launches;
     }
     for (int64_t base = 0; base < P; base += pl.Pc) {
         const int64_t Pc = (P - base) < pl.Pc ? (P - base) : pl.Pc;
-        gl_unpack_kernel<<<(unsigned)((Pc + 127) / 128), 128, 0, st>>>(c->pt, c->L, G, c->desc.pix_scale,
-                                                                       params + base * c->L.n_params, Pc, pb, lpd);
+        GL_STAGE(ST_UNPACK, st, (gl_unpack_kernel<<<(unsigned)((Pc + 127) / 128), 128, 0, st>>>(
+            c->pt, c->L, G, c->desc.pix_scale, params + base * c->L.n_params, Pc, pb, lpd)));
         ++t_launches;
-        ray_fwd(c, pb, ray, Pc, st); ++t_launches;
-        t_launches += conv_fwd_launch(c->conv_kind, G, ray, sys_kt, sys_w, obs, system_id, base, Pc,
+        GL_STAGE(ST_RAY_FWD, st, ray_fwd(c, pb, ray, Pc, st)); ++t_launches;
+        GL_STAGE(ST_CONV_FWD, st, t_launches += conv_fwd_launch(c->conv_kind, G, ray, sys_kt, sys_w, obs, system_id, base, Pc,
                                       mode == 2 ? nullptr : gpix, mode == 2 ? nullptr : chi, c->n_ctile,
-                                      mode == 2 ? out_image : nullptr, st);
+                                      mode == 2 ? out_image : nullptr, st));
         if (mode == 2) continue;
         if (mode == 1) {
-            t_launches += conv_bwd_launch(c->conv_kind, G, gpix, sys_kt, system_id, base, Pc, ray, st);
-            ray_adj(c, pb, ray, nap, Pc, st); ++t_launches;
+            GL_STAGE(ST_CONV_BWD, st, t_launches += conv_bwd_launch(c->conv_kind, G, gpix, sys_kt, system_id, base, Pc, ray, st));
+            GL_STAGE(ST_RAY_ADJ, st, ray_adj(c, pb, ray, nap, Pc, st)); ++t_launches;
         }
         const int wpb = 4;
-        gl_finalize_kernel<<<(unsigned)((Pc + wpb - 1) / wpb), wpb * 32, wpb * (NA_MAX + 128) * sizeof(double), st>>>(
+        GL_STAGE(ST_FINALIZE, st, (gl_finalize_kernel<<<(unsigned)((Pc + wpb - 1) / wpb), wpb * 32, wpb * (NA_MAX + 128) * sizeof(double), st>>>(
             c->pt, c->L, G, params, pb, lpd, chi, c->n_ctile, mode == 1 ? nap : nullptr, c->n_chunk_adj, c->na,
-            sys_sl, system_id, Pc, base, out_logp, out_grad);
+            sys_sl, system_id, Pc, base, out_logp, out_grad)));
         ++t_launches;
     }
     cudaError_t e = cudaPeekAtLastError();
