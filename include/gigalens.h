@@ -158,6 +158,18 @@ int32_t     gl_stage_count(void);
 const char* gl_stage_name(int32_t i);
 int32_t     gl_stage_times(float* ms_host, int32_t* launches_host, int32_t n);
 
+/* Measurement utility (NOT part of the hot path; the only call that synchronises): issue-rate probe of one SM
+ * pipe, so that bench.py can state a MEASURED ALU peak beside the one derived from unit counts and clocks
+ * (BASELINE.json north_star: "achieved fraction of the binding roofline"; MEASURED_PEAKS.json has no FP32, FP64
+ * or MUFU figure).  kind 0: FP32 FMA, 1: FP64 FMA, 2: MUFU ex2, 3: FP32 and FP64 FMA interleaved 1:1 (both
+ * counted).  Launches 8 CTAs of 256 threads per SM, each thread running 8 independent chains of
+ * n_outer * 64 operations, once untimed and once between two CUDA events on `stream`, waits for it, and writes
+ * 1e-12 * lane-operations per second (an FMA counts once) to *tera_lane_ops_per_s_host and the kernel time to
+ * *ms_host (HOST pointers; ms_host may be NULL).  workspace: DEVICE pointer, >= 256 bytes (never written in
+ * practice).  Errors: GL_ERR_NULL, GL_ERR_BAD_SHAPE (kind or n_outer out of range), GL_ERR_WORKSPACE, GL_ERR_CUDA. */
+gl_status gl_probe_pipe(int32_t kind, int32_t n_outer, void* workspace, size_t workspace_bytes, void* stream,
+                        double* tera_lane_ops_per_s_host, float* ms_host);
+
 /* Static string for a status code. */
 const char* gl_status_string(gl_status s);
 

@@ -20,7 +20,7 @@ STATUS = {0: "GL_OK", -1: "GL_ERR_NULL", -2: "GL_ERR_BAD_CONFIG", -3: "GL_ERR_BA
 EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_workspace_bytes", "gl_logpost",
            "gl_logpost_grad", "gl_model_image", "gl_workspace_bytes_host", "gl_logpost_grad_host",
            "gl_last_launch_count", "gl_status_string", "gl_version", "gl_stage_timing_enable", "gl_stage_count",
-           "gl_stage_name", "gl_stage_times"]
+           "gl_stage_name", "gl_stage_times", "gl_probe_pipe"]
 
 
 class GLError(RuntimeError):
@@ -82,6 +82,8 @@ def lib():
         L.gl_stage_name.argtypes = [C.c_int32]
         L.gl_stage_times.restype = C.c_int32
         L.gl_stage_times.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_int32), C.c_int32]
+        L.gl_probe_pipe.restype = C.c_int
+        L.gl_probe_pipe.argtypes = [C.c_int32, C.c_int32, vp, sz, vp, C.POINTER(C.c_double), C.POINTER(C.c_float)]
         _lib = L
     return _lib
 
@@ -135,6 +137,16 @@ def gl_stage_times():
     if L.gl_stage_times(ms, cnt, n) != n:
         raise RuntimeError("gl_stage_times failed")
     return {L.gl_stage_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(n)}
+
+
+def gl_probe_pipe(kind, n_outer=2048, stream=None):
+    """(tera lane-ops/s, kernel ms) of one SM pipe: kind 0 FP32 FMA, 1 FP64 FMA, 2 MUFU ex2, 3 FP32+FP64 interleaved."""
+    torch = _torch()
+    ws = torch.zeros(256, dtype=torch.uint8, device="cuda")
+    rate = C.c_double(); ms = C.c_float()
+    _check(lib().gl_probe_pipe(int(kind), int(n_outer), _ptr(ws), 256, _stream(stream), C.byref(rate), C.byref(ms)),
+           "gl_probe_pipe")
+    return rate.value, ms.value
 
 
 def _torch():

@@ -11,6 +11,7 @@
 #include "gl_conv.cuh"
 #include "gl_conv_tiled.cuh"
 #include "gl_particle.cuh"
+#include "gl_probe.cuh"
 #include "gl_ray.cuh"
 
 using namespace gl;
@@ -347,5 +348,42 @@ extern "C" gl_status gl_logpost_grad_host(const gl_config* c, const float* obs, 
     if (cudaMemcpyAsync(out_logp_host, d_logp, sizeof(float) * n, cudaMemcpyDeviceToHost, st) != cudaSuccess) return GL_ERR_CUDA;
     if (out_grad_host && cudaMemcpyAsync(out_grad_host, d_grad, sizeof(float) * n * np, cudaMemcpyDeviceToHost, st) != cudaSuccess)
         return GL_ERR_CUDA;
+    return GL_OK;
+}
+
+// ----------------------------------------------------------------------------- pipe probe (measurement utility)
+extern "C" gl_status gl_probe_pipe(int32_t kind, int32_t n_outer, void* workspace, size_t workspace_bytes, void* stream,
+                                   double* tera_lane_ops_per_s_host, float* ms_host) {
+    if (!workspace || !tera_lane_ops_per_s_host) return GL_ERR_NULL;
+    if (kind < 0 || kind > 3 || n_outer < 1) return GL_ERR_BAD_SHAPE;
+    if (workspace_bytes < 256) return GL_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, n_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return GL_ERR_CUDA;
+    const int ctas = n_sm * 8, nt = 256;
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return GL_ERR_CUDA;
+    float* sink = (float*)workspace;
+    auto launch = [&](int n) {
+        switch (kind) {
+            case 0: gl_probe_kernel<0><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+            case 1: gl_probe_kernel<1><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+            case 2: gl_probe_kernel<2><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+            default: gl_probe_kernel<3><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+        }
+    };
+    launch(n_outer);                                   // warm-up
+    cudaEventRecord(e0, st);
+    launch(n_outer);
+    cudaEventRecord(e1, st);
+    float ms = 0.f;
+    cudaError_t e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (e != cudaSuccess || !(ms > 0.f)) return GL_ERR_CUDA;
+    const double ops = (double)ctas * nt * (double)n_outer * PROBE_INNER * PROBE_CHAINS * (kind == 3 ? 2.0 : 1.0);
+    *tera_lane_ops_per_s_host = ops / (ms * 1e-3) * 1e-12;
+    if (ms_host) *ms_host = ms;
     return GL_OK;
 }
