@@ -9,7 +9,7 @@
 
 #include "gl_common.cuh"
 #include "gl_conv.cuh"
-#include "gl_conv_tiled.cuh"
+#include "gl_conv_launch.cuh"
 #include "gl_particle.cuh"
 #include "gl_probe.cuh"
 #include "gl_ray.cuh"
@@ -24,8 +24,10 @@ struct gl_config {
     PriorTable pt;
     int variant;        // 0: <.,0,1,-1,1>  1: <.,0,1,6,2>  2: <.,3,1,10,2>
     int na;             // natural accumulators per chunk for the variant
-    int rpt_fwd, rpt_adj, n_chunk_fwd, n_chunk_adj, n_ctile;
-    int conv_kind;      // 0 generic, >0 tiled specialisation id
+    int nt_fwd, nt_adj, rpt_fwd, rpt_adj, n_chunk_fwd, n_chunk_adj;   // per phase plane
+    int n_nap;          // adjoint partials per particle = s*s*n_chunk_adj
+    int n_ctile;        // chi^2 partials per particle
+    ConvPlan conv;
     size_t per_particle_bytes;
 };
 
@@ -71,7 +73,7 @@ extern "C" int32_t gl_stage_times(float* ms_host, int32_t* launches_host, int32_
 }
 #define GL_STAGE(id, st, ...) do { t_timer.begin(id, st); __VA_ARGS__; t_timer.end(st); } while (0)
 
-static constexpr int NT_FWD = 256;
+static constexpr int NT_FWD = 256;     // compiled launch bounds; the block size actually used is chosen per config
 static constexpr int NT_ADJ = 128;
 static constexpr size_t WS_BUDGET = (size_t)1536 << 20;   // chunk so that per-chunk buffers stay below ~1.5 GiB
 
@@ -159,16 +161,28 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     G.U = (KE + G.s - 1) / G.s; G.KEp = G.U * G.s;
     G.n_terms = d->mass_model == 1 ? d->epl_terms : 0;
     G.delta2 = d->pix_scale * d->pix_scale;
-    const int64_t MM = M64 * M64;
-    auto clampi = [](int64_t v, int64_t lo, int64_t hi) { return (int)(v < lo ? lo : (v > hi ? hi : v)); };
-    c->rpt_fwd = 8;
-    c->n_chunk_fwd = (int)((MM + NT_FWD * c->rpt_fwd - 1) / (NT_FWD * c->rpt_fwd));
-    c->rpt_adj = clampi((MM + NT_ADJ * 32 - 1) / (NT_ADJ * 32), 8, 64);
-    c->n_chunk_adj = (int)((MM + NT_ADJ * c->rpt_adj - 1) / (NT_ADJ * c->rpt_adj));
-    c->conv_kind = conv_tiled_select(G, &c->n_ctile);
-    if (c->conv_kind == 0) c->n_ctile = (G.N * G.N + 255) / 256;
-    c->per_particle_bytes = sizeof(float) * ((size_t)PB_STRIDE + (size_t)MM + (size_t)G.N * G.N + (size_t)c->n_ctile +
-                                             (size_t)c->n_chunk_adj * c->na) + sizeof(double) + 6 * 256;
+    (void)M64;
+    c->conv = conv_plan(G);                 // also fills the padded-layout fields of G
+    c->n_ctile = c->conv.n_ctile;
+    // ray kernels: one CTA per (particle, phase plane, chunk); pick the block size that wastes the fewest lanes
+    const int NN = G.N * G.N;
+    auto pick = [&](int nt_max, int rpt_target, int& nt, int& rpt, int& n_chunk) {
+        int best = nt_max; double best_w = 1e30;
+        for (int t = nt_max; t >= nt_max / 2 && t >= 32; t -= 32) {
+            const int it = (NN + t - 1) / t;
+            const double w = (double)it * t / NN;
+            if (w < best_w - 1e-9) { best_w = w; best = t; }
+        }
+        nt = best;
+        const int iters = (NN + nt - 1) / nt;
+        n_chunk = (iters + rpt_target - 1) / rpt_target;
+        rpt = (iters + n_chunk - 1) / n_chunk;
+    };
+    pick(NT_FWD, 10, c->nt_fwd, c->rpt_fwd, c->n_chunk_fwd);
+    pick(NT_ADJ, 32, c->nt_adj, c->rpt_adj, c->n_chunk_adj);
+    c->n_nap = G.s * G.s * c->n_chunk_adj;
+    c->per_particle_bytes = sizeof(float) * ((size_t)PB_STRIDE + ray_stride(G) + gpix_stride(G) + (size_t)c->n_ctile +
+                                             (size_t)c->n_nap * c->na) + sizeof(double) + 6 * 256;
     *out = c;
     return GL_OK;
 }
@@ -195,10 +209,10 @@ static Plan make_plan(const gl_config* c, int64_t P) {
     pl.off_sl = o;   o = align256(o + sizeof(float) * nsys);
     pl.off_pb = o;   o = align256(o + sizeof(float) * (size_t)pl.Pc * PB_STRIDE);
     pl.off_lpd = o;  o = align256(o + sizeof(double) * (size_t)pl.Pc);
-    pl.off_ray = o;  o = align256(o + sizeof(float) * (size_t)pl.Pc * G.M * G.M);
-    pl.off_gpix = o; o = align256(o + sizeof(float) * (size_t)pl.Pc * G.N * G.N);
+    pl.off_ray = o;  o = align256(o + sizeof(float) * (size_t)pl.Pc * ray_stride(G));
+    pl.off_gpix = o; o = align256(o + sizeof(float) * (size_t)pl.Pc * gpix_stride(G));
     pl.off_chi = o;  o = align256(o + sizeof(float) * (size_t)pl.Pc * c->n_ctile);
-    pl.off_nap = o;  o = align256(o + sizeof(float) * (size_t)pl.Pc * c->n_chunk_adj * c->na);
+    pl.off_nap = o;  o = align256(o + sizeof(float) * (size_t)pl.Pc * c->n_nap * c->na);
     pl.total = o;
     return pl;
 }
@@ -211,13 +225,13 @@ extern "C" size_t gl_workspace_bytes(const gl_config* c, int64_t n_particles) {
 // ----------------------------------------------------------------------------- variant dispatch
 template <class V>
 static void launch_ray_fwd(const gl_config* c, const float* pb, float* ray, int64_t Pc, cudaStream_t st) {
-    dim3 grid(c->n_chunk_fwd, (unsigned)Pc);
-    gl_ray_fwd_kernel<V, NT_FWD><<<grid, NT_FWD, 0, st>>>(pb, ray, c->G.M, c->rpt_fwd);
+    dim3 grid(c->G.s * c->G.s * c->n_chunk_fwd, (unsigned)Pc);
+    gl_ray_fwd_kernel<V, NT_FWD><<<grid, c->nt_fwd, 0, st>>>(c->G, pb, ray, c->rpt_fwd, c->n_chunk_fwd);
 }
 template <class V>
 static void launch_ray_adj(const gl_config* c, const float* pb, const float* gbar, float* nap, int64_t Pc, cudaStream_t st) {
-    dim3 grid(c->n_chunk_adj, (unsigned)Pc);
-    gl_ray_adj_kernel<V, NT_ADJ><<<grid, NT_ADJ, 0, st>>>(pb, gbar, nap, c->G.M, c->rpt_adj);
+    dim3 grid(c->n_nap, (unsigned)Pc);
+    gl_ray_adj_kernel<V, NT_ADJ><<<grid, c->nt_adj, 0, st>>>(c->G, pb, gbar, nap, c->rpt_adj, c->n_chunk_adj);
 }
 
 using V_S0 = Variant<0, 0, 1, -1, 1>; using V_E0 = Variant<1, 0, 1, -1, 1>;
@@ -281,17 +295,22 @@ static gl_status run(const gl_config* c, int mode, const float* obs, const float
             c->pt, c->L, G, c->desc.pix_scale, params + base * c->L.n_params, Pc, pb, lpd)));
         ++t_launches;
         GL_STAGE(ST_RAY_FWD, st, ray_fwd(c, pb, ray, Pc, st)); ++t_launches;
-        GL_STAGE(ST_CONV_FWD, st, t_launches += conv_fwd_launch(c->conv_kind, G, ray, sys_kt, sys_w, obs, system_id, base, Pc,
-                                      mode == 2 ? nullptr : gpix, mode == 2 ? nullptr : chi, c->n_ctile,
+        int nl = 0;
+        GL_STAGE(ST_CONV_FWD, st, nl = conv_fwd_launch(c->conv, G, ray, sys_kt, sys_w, obs, system_id, base, Pc,
+                                      mode == 2 ? nullptr : gpix, mode == 2 ? nullptr : chi,
                                       mode == 2 ? out_image : nullptr, st));
+        if (nl < 0) return GL_ERR_CUDA;
+        t_launches += nl;
         if (mode == 2) continue;
         if (mode == 1) {
-            GL_STAGE(ST_CONV_BWD, st, t_launches += conv_bwd_launch(c->conv_kind, G, gpix, sys_kt, system_id, base, Pc, ray, st));
+            GL_STAGE(ST_CONV_BWD, st, nl = conv_bwd_launch(c->conv, G, gpix, sys_kt, system_id, base, Pc, ray, st));
+            if (nl < 0) return GL_ERR_CUDA;
+            t_launches += nl;
             GL_STAGE(ST_RAY_ADJ, st, ray_adj(c, pb, ray, nap, Pc, st)); ++t_launches;
         }
         const int wpb = 4;
         GL_STAGE(ST_FINALIZE, st, (gl_finalize_kernel<<<(unsigned)((Pc + wpb - 1) / wpb), wpb * 32, wpb * (NA_MAX + 128) * sizeof(double), st>>>(
-            c->pt, c->L, G, params, pb, lpd, chi, c->n_ctile, mode == 1 ? nap : nullptr, c->n_chunk_adj, c->na,
+            c->pt, c->L, G, params, pb, lpd, chi, c->n_ctile, mode == 1 ? nap : nullptr, c->n_nap, c->na,
             sys_sl, system_id, Pc, base, out_logp, out_grad)));
         ++t_launches;
     }

@@ -2,9 +2,14 @@
 //
 // Data layout in HBM:
 //   PB   [Pc][PB_STRIDE] fp32   per-particle block of derived scalars written by gl_unpack_kernel (step A)
-//   RAY  [Pc][M][M]      fp32   supersampled surface-brightness image (step B+C), later reused for gbar_ray
-//   GPIX [Pc][N][N]      fp32   g_pix = -(model-obs)/sigma^2 (step E), input of the transposed step D
-//   CHI  [Pc][n_ctile]   fp32   per-tile chi-square partials, summed in fixed order by gl_finalize_kernel
+//   RAY  [Pc][s*s][Hp][Wp] fp32 supersampled surface-brightness image (step B+C) as s*s PHASE PLANES: ray (i, j) =
+//                               (s*i1 + a, s*j1 + b) lives in plane (a, b) at row i1 + o_a, column j1 + o_b with
+//                               o_a = (a + c) div s; everything outside that N x N interior is ZERO.  The shift and
+//                               the zero border turn step D into s*s plain "valid" stride-1 correlations that need no
+//                               bounds checks and read 16-byte-aligned row segments.  Reused for gbar_ray (step F).
+//   GPIX [Pc][Hg][Wg]    fp32   g_pix = -(model-obs)/sigma^2 (step E), zero-padded by U-1 on every side: input of the
+//                               transposed step D
+//   CHI  [Pc][n_ctile]   fp32   per-band chi-square partials, summed in fixed order by gl_finalize_kernel
 //   NAP  [Pc][n_chunk][NA] fp32 per-chunk "natural" gradient accumulators of the adjoint (step F)
 //   SYS  per system: kt (flipped pre-boxed PSF, phase-major), w = 1/sigma^2, sum(ln sigma)
 #pragma once
@@ -16,13 +21,13 @@ namespace gl {
 // ----------------------------------------------------------------------------- particle block (PB)
 enum : int {
     PB_VALID = 0,
-    PB_M_XOFF = 1, PB_M_YOFF = 2,       // x_first - x0, y_first - y0  (fp64-subtracted, then rounded)
+    PB_M_XOFF = 1, PB_M_YOFF = 2,       // -x0, -y0 of the mass centre (ray coordinates are relative to the grid centre)
     PB_M_C = 3, PB_M_S = 4,             // cos phi, sin phi of the mass frame
     PB_M_Q = 5, PB_M_B = 6, PB_M_T = 7, PB_M_F = 8, PB_M_L2B = 9, PB_M_A = 10,
     PB_M_QP = 11, PB_M_BQP = 12,        // SIE: q' = sqrt(1-q^2), b/q'
     PB_M_F2 = 13, PB_M_TM1 = 14, PB_M_KAPC = 15,   // f^2, t-1, (2-t)/2 * b
     PB_G1 = 16, PB_G2 = 17, PB_C3 = 18, PB_S3 = 19, PB_C4 = 20, PB_S4 = 21,
-    PB_XFIRST = 22, PB_STEP = 23,       // ray grid: x_j = x_first + j*step (same for y)
+    PB_XFIRST = 22, PB_STEP = 23,       // ray grid: x_j = x_first + fj*step with fj = j - (M-1)/2, x_first = 0
     PB_SRC = 24,                        // Sersic block, 16 floats
     PB_SHP = 40,                        // +0 1/beta_s ; coefficients a_k/beta_s from PB_SHP_A
     PB_SHP_A = 44,
@@ -69,7 +74,13 @@ struct Geom {            // launch-invariant geometry, passed by value
     int KEp, U;          // padded k_eff taps per side (multiple of s), taps per phase per side
     int n_terms;         // EPL series terms kept (2..30)
     float delta2;        // pix_scale^2
+    int UP;              // U rounded up to a multiple of the tap rows one conv thread handles
+    int Hp, Wp;          // rows / row pitch of one padded phase plane of RAY
+    int Hg, Wg, PADg;    // rows / row pitch / border of the padded GPIX image
 };
+__host__ __device__ inline int phase_shift(const Geom& G, int a) { return (a + G.c) / G.s; }      // o_a
+__host__ __device__ inline size_t ray_stride(const Geom& G) { return (size_t)G.s * G.s * G.Hp * G.Wp; }
+__host__ __device__ inline size_t gpix_stride(const Geom& G) { return (size_t)G.Hg * G.Wg; }
 
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll

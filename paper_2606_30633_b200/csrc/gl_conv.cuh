@@ -3,9 +3,20 @@
 // Fused form (checked in tests/test_oracle_pins.py::test_conv_bin_vs_scipy_and_fused_keff_form):
 //   model[p][q] = sum_{u,v < KE} kt[u][v] * I_ray[s p - c + u][s q - c + v],   KE = K + s - 1,
 //   kt[u][v] = Delta^2/s^2 * k_eff[KE-1-u][KE-1-v],  k_eff = psf (*) ones(s,s)   (rays outside the cutout are 0)
-// kt is stored PHASE-MAJOR: kt[a][b][u1][v1] with u = s*u1 + a, v = s*v1 + b, u1,v1 < U = ceil(KE/s) (zero padded),
-// which turns the stride-s correlation into s^2 stride-1 correlations of the ray image's phase planes.
-// The transpose is  gbar[i][j] = sum_{u1,v1} kt[a][b][u1][v1] * g[pp - u1][qq - v1],  pp = (i+c) div s, a = (i+c) mod s.
+// kt is stored PHASE-MAJOR: kt[a'][b'][u1][v1] with u = s*u1 + a', v = s*v1 + b', u1,v1 < U = ceil(KE/s) (zero padded).
+//
+// The ray image lives in HBM as s*s zero-bordered, shifted PHASE PLANES (gl_common.cuh): ray (s i1 + a, s j1 + b) is
+// element [i1 + o_a][j1 + o_b] of plane (a, b), o_a = (a + c) div s.  With a' = (a + c) mod s the stride-s correlation
+// becomes, per plane, a plain stride-1 "valid" correlation with U x U taps and no bounds checks:
+//   model[p][q] = sum_{a,b} sum_{u1,v1 < U} kt[a'][b'][u1][v1] * plane_ab[p + u1][q + v1]                (step D)
+//   gbar_ab[n + o_a][j'] = sum_{k,l < U} kt[a'][b'][U-1-k][U-1-l] * gp[n + o_a + k][j' + l]           (transpose)
+// where gp is g_pix zero-padded by U-1 on every side and gbar is produced directly in the plane layout.
+//
+// Both directions run the same inner loop (gl_conv_*_sw): one thread owns 4 adjacent output columns of ONE plane and
+// UR consecutive tap rows, keeps its UR x U taps and a UR-row sliding window of the input in registers, and sweeps
+// down the image: per output row it loads one new input row segment (U+3 floats, 16-byte aligned) and issues
+// 4*UR*U FMAs.  Step D then sums the s*s*ceil(U/UR) partial results per pixel through shared memory in a fixed
+// order (deterministic), and applies step E in the same pass.
 #pragma once
 #include "gl_common.cuh"
 
@@ -46,84 +57,261 @@ __global__ void gl_prep_kernel(const __grid_constant__ Geom G, const float* __re
     if (threadIdx.x == 0) sys_sumlog[sys] = (float)red[0];
 }
 
-// fixed-order block sum of one float per thread (NT threads), result valid in thread 0
-template <int NT>
-__device__ __forceinline__ float block_sum(float v, float* red /* NT/32 */) {
+// fixed-order block sum of one float per thread (blockDim.x a multiple of 32, <= 1024), result valid in thread 0
+__device__ __forceinline__ float block_sum(float v, float* red /* 32 */) {
     v = warp_sum(v);
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
     __syncthreads();
     float s = 0.f;
     if (threadIdx.x == 0) {
-#pragma unroll
-        for (int w = 0; w < NT / 32; ++w) s += red[w];
+        const int nw = blockDim.x >> 5;
+        for (int w = 0; w < nw; ++w) s += red[w];
     }
     return s;
 }
 
-// Generic (any s, K) step D + E: one thread per detector pixel, taps and rays through L1/L2.  Used for shapes
-// without a tiled specialisation.  grid = (ceil(N*N/256), Pc).  chi: [Pc][gridDim.x].
-// out_model may be NULL; gpix may be NULL (gl_model_image).
+// Zero the border of this particle's padded g_pix image (the interior is written by the step-E epilogue).
+__device__ __forceinline__ void zero_gpix_border(const Geom& G, float* __restrict__ gp, int first, int stride) {
+    const int tot = G.Hg * G.Wg;
+    for (int e = first; e < tot; e += stride) {
+        const int r = e / G.Wg, cc = e - r * G.Wg;
+        if (r < G.PADg || r >= G.PADg + G.N || cc < G.PADg || cc >= G.PADg + G.N) gp[e] = 0.f;
+    }
+}
+
+// Step E for one pixel: writes the model / g_pix and returns the chi^2 term.
+__device__ __forceinline__ float pixel_epilogue(const Geom& G, float m, int pr, int pq, int sys, size_t p_out, int p,
+                                                const float* __restrict__ obs, const float* __restrict__ sys_w,
+                                                float* __restrict__ gpix, float* __restrict__ out_model) {
+    const size_t NN = (size_t)G.N * G.N, pix = (size_t)pr * G.N + pq;
+    if (out_model) out_model[p_out * NN + pix] = m;
+    if (!gpix) return 0.f;
+    const float r = m - obs[(size_t)sys * NN + pix], w = sys_w[(size_t)sys * NN + pix];
+    gpix[(size_t)p * gpix_stride(G) + (size_t)(pr + G.PADg) * G.Wg + pq + G.PADg] = -r * w;
+    return r * r * w;
+}
+
+// ----------------------------------------------------------------------------- generic kernels (any s, K)
+// One thread per detector pixel, taps and rays through L1/L2.  grid = (ceil(N*N/256), Pc).  chi: [Pc][gridDim.x].
 __global__ void __launch_bounds__(256) gl_conv_fwd_generic(const __grid_constant__ Geom G, const float* __restrict__ ray,
                                                            const float* __restrict__ sys_kt, const float* __restrict__ sys_w,
                                                            const float* __restrict__ obs, const int32_t* __restrict__ system_id,
                                                            int64_t p_base, float* __restrict__ gpix, float* __restrict__ chi,
                                                            float* __restrict__ out_model) {
-    __shared__ float red[8];
-    const int p = blockIdx.y, NN = G.N * G.N, M = G.M, s = G.s, U = G.U;
+    __shared__ float red[32];
+    const int p = blockIdx.y, NN = G.N * G.N, s = G.s, U = G.U;
     const int sys = system_id ? system_id[p_base + p] : 0;
     const float* kt = sys_kt + (size_t)sys * s * s * U * U;
-    const float* I = ray + (size_t)p * M * M;
+    const float* I = ray + (size_t)p * ray_stride(G);
+    if (gpix) zero_gpix_border(G, gpix + (size_t)p * gpix_stride(G), blockIdx.x * 256 + threadIdx.x, gridDim.x * 256);
     const int pix = blockIdx.x * 256 + threadIdx.x;
     float c2 = 0.f;
     if (pix < NN) {
         const int pr = pix / G.N, pq = pix - pr * G.N;
         float acc = 0.f;
-        for (int a = 0; a < s; ++a) for (int u1 = 0; u1 < U; ++u1) {
-            const int i = s * pr - G.c + s * u1 + a;
-            if (i < 0 || i >= M) continue;
-            for (int b = 0; b < s; ++b) {
-                const float* kr = kt + ((a * s + b) * U + u1) * U;
-                for (int v1 = 0; v1 < U; ++v1) {
-                    const int j = s * pq - G.c + s * v1 + b;
-                    if (j >= 0 && j < M) acc = fmaf(kr[v1], I[i * M + j], acc);
-                }
-            }
+        for (int a = 0; a < s; ++a) for (int b = 0; b < s; ++b) {
+            const float* kr = kt + (size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U;
+            const float* pl = I + ((size_t)(a * s + b) * G.Hp + pr) * G.Wp + pq;
+            for (int u1 = 0; u1 < U; ++u1)
+                for (int v1 = 0; v1 < U; ++v1) acc = fmaf(kr[u1 * U + v1], pl[(size_t)u1 * G.Wp + v1], acc);
         }
-        if (out_model) out_model[(size_t)(p_base + p) * NN + pix] = acc;
-        if (gpix) {
-            const float r = acc - obs[(size_t)sys * NN + pix], w = sys_w[(size_t)sys * NN + pix];
-            gpix[(size_t)p * NN + pix] = -r * w;
-            c2 = r * r * w;
-        }
+        c2 = pixel_epilogue(G, acc, pr, pq, sys, (size_t)(p_base + p), p, obs, sys_w, gpix, out_model);
     }
     if (chi) {
-        float tot = block_sum<256>(c2, red);
+        float tot = block_sum(c2, red);
         if (threadIdx.x == 0) chi[(size_t)p * gridDim.x + blockIdx.x] = tot;
     }
 }
 
-// Generic transpose of step D: one thread per ray.  grid = (ceil(M*M/256), Pc).  gbar overwrites the ray buffer.
+// Generic transpose of step D: one thread per ray.  grid = (ceil(s*s*N*N/256), Pc).  gbar is written in plane layout.
 __global__ void __launch_bounds__(256) gl_conv_bwd_generic(const __grid_constant__ Geom G, const float* __restrict__ gpix,
                                                            const float* __restrict__ sys_kt, const int32_t* __restrict__ system_id,
                                                            int64_t p_base, float* __restrict__ gbar) {
-    const int p = blockIdx.y, M = G.M, s = G.s, U = G.U, N = G.N;
+    const int p = blockIdx.y, s = G.s, U = G.U, N = G.N;
     const int idx = blockIdx.x * 256 + threadIdx.x;
-    if (idx >= M * M) return;
+    if (idx >= s * s * N * N) return;
     const int sys = system_id ? system_id[p_base + p] : 0;
-    const float* kt = sys_kt + (size_t)sys * s * s * U * U;
-    const float* g = gpix + (size_t)p * N * N;
-    const int i = idx / M, j = idx - i * M;
-    const int pp = (i + G.c) / s, a = (i + G.c) - pp * s, qq = (j + G.c) / s, b = (j + G.c) - qq * s;
-    const float* kr = kt + (a * s + b) * U * U;
+    const int ph = idx / (N * N), rem = idx - ph * N * N, n = rem / N, j1 = rem - n * N;
+    const int a = ph / s, b = ph - a * s, oa = phase_shift(G, a), ob = phase_shift(G, b);
+    const float* kr = sys_kt + (size_t)sys * s * s * U * U + (size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U;
+    const float* g = gpix + (size_t)p * gpix_stride(G) + (size_t)(n + oa) * G.Wg + j1 + ob;
     float acc = 0.f;
-    for (int u1 = 0; u1 < U; ++u1) {
-        const int pr = pp - u1; if (pr < 0 || pr >= N) continue;
-        for (int v1 = 0; v1 < U; ++v1) {
-            const int pq = qq - v1;
-            if (pq >= 0 && pq < N) acc = fmaf(kr[u1 * U + v1], g[pr * N + pq], acc);
+    for (int k = 0; k < U; ++k)
+        for (int l = 0; l < U; ++l) acc = fmaf(kr[(U - 1 - k) * U + (U - 1 - l)], g[(size_t)k * G.Wg + l], acc);
+    gbar[(size_t)p * ray_stride(G) + ((size_t)ph * G.Hp + n + oa) * G.Wp + j1 + ob] = acc;
+}
+
+// ----------------------------------------------------------------------------- sliding-window kernels
+template <int U>
+struct RowSeg {                                  // the U+3 input floats that 4 adjacent outputs need from one row
+    static constexpr int NEED = U + 3;
+    static constexpr int NV4 = (NEED % 4 <= 1) ? NEED / 4 : (NEED + 3) / 4;
+    static constexpr int NSC = (NEED % 4 <= 1) ? NEED % 4 : 0;
+    static constexpr int NVAL = NV4 * 4 + NSC;
+    static constexpr int WL = 4 * ((NEED + 3) / 4);                 // floats a row segment may touch
+    static __device__ __forceinline__ void load(float (&w)[NVAL], const float* __restrict__ p) {
+#pragma unroll
+        for (int v = 0; v < NV4; ++v) {
+            const float4 x = __ldg(reinterpret_cast<const float4*>(p) + v);
+            w[4 * v] = x.x; w[4 * v + 1] = x.y; w[4 * v + 2] = x.z; w[4 * v + 3] = x.w;
+        }
+#pragma unroll
+        for (int i = 0; i < NSC; ++i) w[4 * NV4 + i] = __ldg(p + 4 * NV4 + i);
+    }
+};
+
+template <int U, int NVAL>
+__device__ __forceinline__ void fma_row(float (&acc)[4], const float (&T)[U], const float (&w)[NVAL]) {
+#pragma unroll
+    for (int l = 0; l < U; ++l) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) acc[q] = fmaf(T[l], w[q + l], acc[q]);
+    }
+}
+
+constexpr int CONV_R = 4;                        // output rows between two reductions
+
+// Step D + E.  grid = (n_band, Pc); block = roundup32(ncgb * s*s * ceil(U/UR)); dynamic smem = conv_sw_smem(...).
+// Thread t: column group g = t % ncgb (4 pixels), virtual phase vp = t / ncgb = (plane, tap-row group).
+template <int UR, int U, int NT_MAX>
+__global__ void __launch_bounds__(NT_MAX) gl_conv_fwd_sw(const __grid_constant__ Geom G, int ncgb,
+                                                         const float* __restrict__ ray, const float* __restrict__ sys_kt,
+                                                         const float* __restrict__ sys_w, const float* __restrict__ obs,
+                                                         const int32_t* __restrict__ system_id, int64_t p_base,
+                                                         float* __restrict__ gpix, float* __restrict__ chi,
+                                                         float* __restrict__ out_model) {
+    constexpr int NRG = (U + UR - 1) / UR;
+    constexpr int NVAL = RowSeg<U>::NVAL;
+    extern __shared__ __align__(16) float part[];                  // [2][NVP][CONV_R][NQ]
+    __shared__ float red[32];
+    const int s = G.s, N = G.N, NVP = s * s * NRG, NQ = 4 * ncgb;
+    const int p = blockIdx.y, band = blockIdx.x, t = threadIdx.x;
+    const bool active = t < ncgb * NVP;
+    const int g = active ? t % ncgb : 0, vp = active ? t / ncgb : 0;
+    const int rho = vp % NRG, ph = vp / NRG, a = ph / s, b = ph - a * s;
+    const int sys = system_id ? system_id[p_base + p] : 0;
+    if (gpix) zero_gpix_border(G, gpix + (size_t)p * gpix_stride(G), band * blockDim.x + t, gridDim.x * blockDim.x);
+    float T[UR][U];
+    {
+        const float* kph = sys_kt + (size_t)sys * s * s * U * U + (size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U;
+#pragma unroll
+        for (int k = 0; k < UR; ++k) {
+            const int u1 = rho * UR + k;
+#pragma unroll
+            for (int l = 0; l < U; ++l) T[k][l] = (u1 < U) ? __ldg(kph + u1 * U + l) : 0.f;
         }
     }
-    gbar[(size_t)p * M * M + idx] = acc;
+    const int gg = min(band * ncgb + g, (G.Wp - RowSeg<U>::WL) / 4);      // clamp keeps idle lanes in bounds
+    const float* in = ray + (size_t)p * ray_stride(G) + ((size_t)ph * G.Hp + rho * UR) * G.Wp + 4 * gg;
+    const size_t Wp = (size_t)G.Wp;
+    float w[UR][NVAL];
+#pragma unroll
+    for (int k = 0; k < UR; ++k) RowSeg<U>::load(w[k], in + k * Wp);
+    float c2 = 0.f;
+    int buf = 0;
+    for (int pr0 = 0; pr0 < N; pr0 += UR) {
+#pragma unroll
+        for (int j = 0; j < UR; ++j) {
+            const int pr = pr0 + j;
+            if (pr < N) {
+                float acc[4] = {0.f, 0.f, 0.f, 0.f};
+                fma_row<U, NVAL>(acc, T[0], w[j % UR]);
+                if (pr + 1 < N) RowSeg<U>::load(w[j % UR], in + (size_t)(pr + UR) * Wp);   // row for the next step
+#pragma unroll
+                for (int k = 1; k < UR; ++k) fma_row<U, NVAL>(acc, T[k], w[(j + k) % UR]);
+                if (active)
+                    *reinterpret_cast<float4*>(&part[((size_t)(buf * NVP + vp) * CONV_R + (pr & (CONV_R - 1))) * NQ + 4 * g]) =
+                        make_float4(acc[0], acc[1], acc[2], acc[3]);
+                if ((pr & (CONV_R - 1)) == CONV_R - 1 || pr == N - 1) {
+                    __syncthreads();
+                    const int rows = (pr & (CONV_R - 1)) + 1, r0 = pr - rows + 1;
+                    for (int o = t; o < rows * NQ; o += blockDim.x) {
+                        const int r = o / NQ, q = o - r * NQ, pq = band * NQ + q;
+                        float m = 0.f;
+                        for (int v = 0; v < NVP; ++v) m += part[((size_t)(buf * NVP + v) * CONV_R + r) * NQ + q];
+                        if (pq < N) c2 += pixel_epilogue(G, m, r0 + r, pq, sys, (size_t)(p_base + p), p, obs, sys_w, gpix, out_model);
+                    }
+                    buf ^= 1;
+                }
+            }
+        }
+    }
+    if (chi) {
+        const float tot = block_sum(c2, red);
+        if (t == 0) chi[(size_t)p * gridDim.x + band] = tot;
+    }
+}
+
+// Transpose of step D.  grid = (n_band, Pc); block = roundup32(ncgb * s*s * ceil(U/UR)).  gbar (plane layout)
+// overwrites the ray buffer; only the N x N interior of each plane is meaningful afterwards.
+template <int UR, int U, int NT_MAX>
+__global__ void __launch_bounds__(NT_MAX) gl_conv_bwd_sw(const __grid_constant__ Geom G, int ncgb,
+                                                         const float* __restrict__ gpix, const float* __restrict__ sys_kt,
+                                                         const int32_t* __restrict__ system_id, int64_t p_base,
+                                                         float* __restrict__ gbar) {
+    constexpr int NRG = (U + UR - 1) / UR;
+    constexpr int NVAL = RowSeg<U>::NVAL;
+    extern __shared__ __align__(16) float part[];                  // [2][NVP][CONV_R][NQ] (only if NRG > 1)
+    const int s = G.s, N = G.N, NPH = s * s, NVP = NPH * NRG, NQ = 4 * ncgb;
+    const int p = blockIdx.y, band = blockIdx.x, t = threadIdx.x;
+    const bool active = t < ncgb * NVP;
+    const int g = active ? t % ncgb : 0, vp = active ? t / ncgb : 0;
+    const int rho = vp % NRG, ph = vp / NRG, a = ph / s, b = ph - a * s, oa = phase_shift(G, a);
+    const int sys = system_id ? system_id[p_base + p] : 0;
+    float T[UR][U];
+    {
+        const float* kph = sys_kt + (size_t)sys * s * s * U * U + (size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U;
+#pragma unroll
+        for (int k = 0; k < UR; ++k) {
+            const int u1 = rho * UR + k;
+#pragma unroll
+            for (int l = 0; l < U; ++l) T[k][l] = (u1 < U) ? __ldg(kph + (U - 1 - u1) * U + (U - 1 - l)) : 0.f;
+        }
+    }
+    const int gcol = band * ncgb + g;
+    const bool in_range = active && 4 * gcol + 3 < G.Wp && 4 * gcol + RowSeg<U>::WL <= G.Wg;
+    const int gg = min(gcol, (G.Wg - RowSeg<U>::WL) / 4);
+    const size_t Wg = (size_t)G.Wg, Wp = (size_t)G.Wp;
+    const float* in = gpix + (size_t)p * gpix_stride(G) + (size_t)(oa + rho * UR) * Wg + 4 * gg;
+    float* out = gbar + (size_t)p * ray_stride(G) + ((size_t)ph * G.Hp + oa) * Wp + 4 * gcol;
+    float w[UR][NVAL];
+#pragma unroll
+    for (int k = 0; k < UR; ++k) RowSeg<U>::load(w[k], in + k * Wg);
+    int buf = 0;
+    for (int n0 = 0; n0 < N; n0 += UR) {
+#pragma unroll
+        for (int j = 0; j < UR; ++j) {
+            const int n = n0 + j;
+            if (n < N) {
+                float acc[4] = {0.f, 0.f, 0.f, 0.f};
+                fma_row<U, NVAL>(acc, T[0], w[j % UR]);
+                if (n + 1 < N) RowSeg<U>::load(w[j % UR], in + (size_t)(n + UR) * Wg);
+#pragma unroll
+                for (int k = 1; k < UR; ++k) fma_row<U, NVAL>(acc, T[k], w[(j + k) % UR]);
+                if constexpr (NRG == 1) {
+                    if (in_range) *reinterpret_cast<float4*>(out + (size_t)n * Wp) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+                } else {
+                    if (active)
+                        *reinterpret_cast<float4*>(&part[((size_t)(buf * NVP + vp) * CONV_R + (n & (CONV_R - 1))) * NQ + 4 * g]) =
+                            make_float4(acc[0], acc[1], acc[2], acc[3]);
+                    if ((n & (CONV_R - 1)) == CONV_R - 1 || n == N - 1) {
+                        __syncthreads();
+                        const int rows = (n & (CONV_R - 1)) + 1, r0 = n - rows + 1;
+                        for (int o = t; o < rows * NPH * NQ; o += blockDim.x) {
+                            const int q = o % NQ, r = (o / NQ) % rows, ph2 = o / (NQ * rows);
+                            float m = 0.f;
+#pragma unroll
+                            for (int v = 0; v < NRG; ++v) m += part[((size_t)(buf * NVP + ph2 * NRG + v) * CONV_R + r) * NQ + q];
+                            const int col = band * NQ + q;
+                            if (col < G.Wp)
+                                gbar[(size_t)p * ray_stride(G) + ((size_t)ph2 * G.Hp + phase_shift(G, ph2 / s) + r0 + r) * Wp + col] = m;
+                        }
+                        buf ^= 1;
+                    }
+                }
+            }
+        }
+    }
 }
 
 }  // namespace gl

@@ -115,7 +115,9 @@ __global__ void gl_unpack_kernel(const __grid_constant__ PriorTable pt, const __
         ok = ok && x.ok; lp += x.lp + x.logdet;
     }
     const double step = (double)pix_scale / G.s;
-    const double x_first = (0.5 / G.s - 0.5 * G.N) * (double)pix_scale;
+    // Ray coordinates are x_j = (j - (M-1)/2) * step (O3 rewritten about the grid centre, which the ray kernels use so
+    // that position - centre keeps its RELATIVE accuracy near a component centre): the per-component offsets are -x0.
+    const double x_first = 0.0;
     // main deflector
     double thE = theta_at(pt, L, z, L.mass, ok);
     double t = L.gamma >= 0 ? theta_at(pt, L, z, L.gamma, ok) - 1.0 : 1.0;

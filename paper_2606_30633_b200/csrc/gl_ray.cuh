@@ -1,6 +1,6 @@
 // gl_ray.cuh -- steps B + C (ray-trace + paint light) and the per-ray part of step F (adjoint).
 //
-// One CTA = one chunk of consecutive rays of ONE particle; the particle's derived scalars (PB) are staged in
+// One CTA = one chunk of rays of one phase plane of ONE particle; the particle's derived scalars (PB) are staged in
 // shared memory once per CTA and every per-ray quantity lives in registers.  FP32 FMA pipe + MUFU
 // (rsqrt / lg2 / ex2 / rcp).  The 30-term EPL series (BASELINE.json configs[1]; reading S5) is a real-
 // coefficient polynomial in w = -f e^{2 i phi}; because |w|^2 = f^2 is a per-particle constant it is
@@ -264,55 +264,86 @@ __device__ __forceinline__ float ray_eval(const float* __restrict__ pb, float fj
 }
 
 // ----------------------------------------------------------------------------- kernels
-// Steps B + C.  grid = (n_chunk, Pc).  Each CTA renders NT * RPT consecutive rays of one particle.
+// Ray <-> thread mapping shared by both kernels: one CTA works on ONE phase plane (a, b) of one particle, so the
+// plane shift (o_a, o_b) is CTA-uniform and consecutive threads touch consecutive addresses of a plane row.
+// grid = (s*s*n_chunk, Pc); CTA (ph, ck) handles plane rays [ck*nt*RPT, (ck+1)*nt*RPT) of the N*N in plane ph.
+// Ray coordinates are taken relative to the grid CENTRE (fj = j - (M-1)/2, exact in fp32), so that a position minus a
+// component centre keeps its relative accuracy near that centre, where the light profiles are steepest.
+struct PlaneIter {
+    int ph, a, b, oa, ob, idx, i1, j1, di, dj;
+    float half;
+    __device__ __forceinline__ PlaneIter(const Geom& G, int n_chunk, int RPT) {
+        ph = blockIdx.x / n_chunk;
+        const int ck = blockIdx.x - ph * n_chunk;
+        a = ph / G.s; b = ph - a * G.s; oa = phase_shift(G, a); ob = phase_shift(G, b);
+        idx = ck * (blockDim.x * RPT) + threadIdx.x;
+        i1 = idx / G.N; j1 = idx - i1 * G.N;
+        di = blockDim.x / G.N; dj = blockDim.x - di * G.N;
+        half = 0.5f * (float)(G.M - 1);
+    }
+    __device__ __forceinline__ void next(const Geom& G) {
+        idx += blockDim.x; i1 += di; j1 += dj;
+        if (j1 >= G.N) { j1 -= G.N; ++i1; }
+    }
+    __device__ __forceinline__ float fj(const Geom& G) const { return (float)(G.s * j1 + b) - half; }
+    __device__ __forceinline__ float fi(const Geom& G) const { return (float)(G.s * i1 + a) - half; }
+    __device__ __forceinline__ size_t offset(const Geom& G) const { return (size_t)(i1 + oa) * G.Wp + (j1 + ob); }
+};
+
+// Steps B + C.  Writes the plane interior and zeroes this CTA's share of the plane border.
 template <class V, int NT>
-__global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const float* __restrict__ pbg, float* __restrict__ ray, int M, int RPT) {
+__global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ Geom G, const float* __restrict__ pbg,
+                                                        float* __restrict__ ray, int RPT, int n_chunk) {
     __shared__ __align__(16) float pb[PB_STRIDE];
     const int p = blockIdx.y;
     const float* src = pbg + (size_t)p * PB_STRIDE;
-    for (int k = threadIdx.x; k < V::PB_NEED; k += NT) pb[k] = src[k];
+    for (int k = threadIdx.x; k < V::PB_NEED; k += blockDim.x) pb[k] = src[k];
     __syncthreads();
-    const int MM = M * M;
-    float* out = ray + (size_t)p * MM;
+    PlaneIter it(G, n_chunk, RPT);
+    float* out = ray + (size_t)p * ray_stride(G) + (size_t)it.ph * G.Hp * G.Wp;
+    {
+        const int ck = blockIdx.x - it.ph * n_chunk, tot = G.Hp * G.Wp;
+        for (int e = ck * blockDim.x + threadIdx.x; e < tot; e += n_chunk * blockDim.x) {
+            const int r = e / G.Wp, cc = e - r * G.Wp;
+            if (r < it.oa || r >= it.oa + G.N || cc < it.ob || cc >= it.ob + G.N) out[e] = 0.f;
+        }
+    }
+    const int NN = G.N * G.N;
     const bool valid = pb[PB_VALID] != 0.f;
-    int idx = blockIdx.x * (NT * RPT) + threadIdx.x;
-    int i = idx / M, j = idx - i * M;
-    const int di = NT / M, dj = NT - di * M;
 #pragma unroll 2
     for (int r = 0; r < RPT; ++r) {
-        if (idx < MM) {
-            float v = ray_eval<V, false>(pb, (float)j, (float)i, 0.f, nullptr);
-            out[idx] = valid ? v : 0.f;
+        if (it.idx < NN) {
+            float v = ray_eval<V, false>(pb, it.fj(G), it.fi(G), 0.f, nullptr);
+            out[it.offset(G)] = valid ? v : 0.f;
         }
-        idx += NT; i += di; j += dj; if (j >= M) { j -= M; ++i; }
+        it.next(G);
     }
 }
 
-// Per-ray part of step F.  grid = (n_chunk, Pc).  gbar: [Pc][M][M]; nap: [Pc][n_chunk][V::NA].
+// Per-ray part of step F.  gbar: plane layout; nap: [Pc][gridDim.x][V::NA].
 template <class V, int NT>
-__global__ void __launch_bounds__(NT) gl_ray_adj_kernel(const float* __restrict__ pbg, const float* __restrict__ gbar,
-                                                        float* __restrict__ nap, int M, int RPT) {
+__global__ void __launch_bounds__(NT) gl_ray_adj_kernel(const __grid_constant__ Geom G, const float* __restrict__ pbg,
+                                                        const float* __restrict__ gbar, float* __restrict__ nap, int RPT,
+                                                        int n_chunk) {
     __shared__ __align__(16) float pb[PB_STRIDE];
     __shared__ float red[NT / 32][V::NA];
     const int p = blockIdx.y;
     const float* src = pbg + (size_t)p * PB_STRIDE;
-    for (int k = threadIdx.x; k < V::PB_NEED; k += NT) pb[k] = src[k];
+    for (int k = threadIdx.x; k < V::PB_NEED; k += blockDim.x) pb[k] = src[k];
     __syncthreads();
-    const int MM = M * M;
-    const float* gb = gbar + (size_t)p * MM;
+    PlaneIter it(G, n_chunk, RPT);
+    const float* gb = gbar + (size_t)p * ray_stride(G) + (size_t)it.ph * G.Hp * G.Wp;
+    const int NN = G.N * G.N;
     float acc[V::NA];
 #pragma unroll
     for (int k = 0; k < V::NA; ++k) acc[k] = 0.f;
-    int idx = blockIdx.x * (NT * RPT) + threadIdx.x;
-    int i = idx / M, j = idx - i * M;
-    const int di = NT / M, dj = NT - di * M;
     if (pb[PB_VALID] != 0.f) {
         for (int r = 0; r < RPT; ++r) {
-            if (idx < MM) ray_eval<V, true>(pb, (float)j, (float)i, gb[idx], acc);
-            idx += NT; i += di; j += dj; if (j >= M) { j -= M; ++i; }
+            if (it.idx < NN) ray_eval<V, true>(pb, it.fj(G), it.fi(G), gb[it.offset(G)], acc);
+            it.next(G);
         }
     }
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
 #pragma unroll
     for (int k = 0; k < V::NA; ++k) {
         float v = warp_sum(acc[k]);
@@ -320,10 +351,9 @@ __global__ void __launch_bounds__(NT) gl_ray_adj_kernel(const float* __restrict_
     }
     __syncthreads();
     float* o = nap + ((size_t)p * gridDim.x + blockIdx.x) * V::NA;
-    for (int k = threadIdx.x; k < V::NA; k += NT) {
+    for (int k = threadIdx.x; k < V::NA; k += blockDim.x) {
         float s = 0.f;
-#pragma unroll
-        for (int ww = 0; ww < NT / 32; ++ww) s += red[ww][k];
+        for (int ww = 0; ww < nw; ++ww) s += red[ww][k];
         o[k] = s;
     }
 }
