@@ -15,6 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libgigalens.so")
 
 GL_OK = 0
+GL_PRECISION_F64, GL_PRECISION_F32 = 0, 1
 STATUS = {0: "GL_OK", -1: "GL_ERR_NULL", -2: "GL_ERR_BAD_CONFIG", -3: "GL_ERR_BAD_SHAPE", -4: "GL_ERR_UNSUPPORTED",
           -5: "GL_ERR_WORKSPACE", -6: "GL_ERR_CUDA"}
 EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_workspace_bytes", "gl_logpost",
@@ -38,7 +39,7 @@ class gl_config_desc(C.Structure):
                 ("psf_grid", C.c_int32), ("mass_model", C.c_int32), ("epl_terms", C.c_int32), ("has_shear", C.c_int32),
                 ("multipole_mask", C.c_int32), ("n_source_sersic", C.c_int32), ("shapelet_nmax", C.c_int32),
                 ("n_lens_sersic", C.c_int32), ("param_space", C.c_int32), ("n_systems", C.c_int32),
-                ("n_params", C.c_int32), ("priors", C.POINTER(gl_prior))]
+                ("n_params", C.c_int32), ("precision", C.c_int32), ("priors", C.POINTER(gl_prior))]
 
 
 _lib = None
@@ -103,7 +104,8 @@ def gl_config_create(spec):
     d = gl_config_desc(spec.n_pix, spec.supersample, spec.psf_size, float(spec.pix_scale),
                        int(getattr(spec, "psf_grid", 0)), spec.mass_model, spec.epl_terms, spec.has_shear,
                        spec.multipole_mask, spec.n_source_sersic, spec.shapelet_nmax, spec.n_lens_sersic,
-                       spec.param_space, spec.n_systems, int(getattr(spec, "n_params", n)), pri)
+                       spec.param_space, spec.n_systems, int(getattr(spec, "n_params", n)),
+                       int(getattr(spec, "precision", GL_PRECISION_F64)), pri)
     h = C.c_void_p()
     _check(lib().gl_config_create(C.byref(d), C.byref(h)), "gl_config_create")
     return h

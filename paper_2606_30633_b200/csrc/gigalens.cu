@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "gl_common.cuh"
+#include "gl_math.cuh"
 #include "gl_conv.cuh"
 #include "gl_conv_launch.cuh"
 #include "gl_particle.cuh"
@@ -28,6 +29,7 @@ struct gl_config {
     int n_nap;          // adjoint partials per particle = s*s*n_chunk_adj
     int n_ctile;        // chi^2 partials per particle
     ConvPlan conv;
+    int esize;          // sizeof the arithmetic type: 8 (GL_PRECISION_F64) or 4 (GL_PRECISION_F32)
     size_t per_particle_bytes;
 };
 
@@ -125,6 +127,7 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     if (d->shapelet_nmax < -1 || d->shapelet_nmax > 10) return GL_ERR_BAD_CONFIG;
     if (d->shapelet_nmax >= 0 && d->n_source_sersic != 1) return GL_ERR_BAD_CONFIG;
     if (d->n_systems < 1) return GL_ERR_BAD_CONFIG;
+    if (d->precision != GL_PRECISION_F64 && d->precision != GL_PRECISION_F32) return GL_ERR_BAD_CONFIG;
     if (d->psf_grid != 0) return GL_ERR_UNSUPPORTED;
     Layout L{};
     int np = layout_from_desc(*d, L);
@@ -160,9 +163,10 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     const int KE = G.K + G.s - 1;
     G.U = (KE + G.s - 1) / G.s; G.KEp = G.U * G.s;
     G.n_terms = d->mass_model == 1 ? d->epl_terms : 0;
-    G.delta2 = d->pix_scale * d->pix_scale;
+    G.delta2 = (double)d->pix_scale * (double)d->pix_scale;
     (void)M64;
-    c->conv = conv_plan(G);                 // also fills the padded-layout fields of G
+    c->esize = d->precision == GL_PRECISION_F64 ? 8 : 4;
+    c->conv = conv_plan(G, c->esize);       // also fills the padded-layout fields of G
     c->n_ctile = c->conv.n_ctile;
     // ray kernels: one CTA per (particle, phase plane, chunk); pick the block size that wastes the fewest lanes
     const int NN = G.N * G.N;
@@ -181,8 +185,8 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     pick(NT_FWD, 10, c->nt_fwd, c->rpt_fwd, c->n_chunk_fwd);
     pick(NT_ADJ, 32, c->nt_adj, c->rpt_adj, c->n_chunk_adj);
     c->n_nap = G.s * G.s * c->n_chunk_adj;
-    c->per_particle_bytes = sizeof(float) * ((size_t)PB_STRIDE + ray_stride(G) + gpix_stride(G) + (size_t)c->n_ctile +
-                                             (size_t)c->n_nap * c->na) + sizeof(double) + 6 * 256;
+    c->per_particle_bytes = (size_t)c->esize * ((size_t)PB_STRIDE + ray_stride(G) + gpix_stride(G) + (size_t)c->n_ctile +
+                                                (size_t)c->n_nap * c->na) + sizeof(double) + 6 * 256;
     *out = c;
     return GL_OK;
 }
@@ -192,7 +196,7 @@ extern "C" int32_t gl_config_n_params(const gl_config* c) { return c ? c->L.n_pa
 
 struct Plan {
     int64_t Pc;
-    size_t off_kt, off_w, off_sl, off_pb, off_lpd, off_ray, off_gpix, off_chi, off_nap, total;
+    size_t off_tab, off_kt, off_w, off_sl, off_pb, off_lpd, off_ray, off_gpix, off_chi, off_nap, total;
 };
 
 static Plan make_plan(const gl_config* c, int64_t P) {
@@ -203,16 +207,17 @@ static Plan make_plan(const gl_config* c, int64_t P) {
     if (pc_max > 32768) pc_max = 32768;
     pl.Pc = P < pc_max ? P : pc_max;
     size_t o = 0;
-    const size_t nsys = (size_t)c->desc.n_systems;
-    pl.off_kt = o;   o = align256(o + sizeof(float) * nsys * G.s * G.s * G.U * G.U);
-    pl.off_w = o;    o = align256(o + sizeof(float) * nsys * G.N * G.N);
-    pl.off_sl = o;   o = align256(o + sizeof(float) * nsys);
-    pl.off_pb = o;   o = align256(o + sizeof(float) * (size_t)pl.Pc * PB_STRIDE);
+    const size_t nsys = (size_t)c->desc.n_systems, es = (size_t)c->esize;
+    pl.off_tab = o;  o = align256(o + sizeof(double) * MATH_TAB_DOUBLES);
+    pl.off_kt = o;   o = align256(o + es * nsys * G.s * G.s * G.U * G.U);
+    pl.off_w = o;    o = align256(o + es * nsys * G.N * G.N);
+    pl.off_sl = o;   o = align256(o + sizeof(double) * nsys);
+    pl.off_pb = o;   o = align256(o + es * (size_t)pl.Pc * PB_STRIDE);
     pl.off_lpd = o;  o = align256(o + sizeof(double) * (size_t)pl.Pc);
-    pl.off_ray = o;  o = align256(o + sizeof(float) * (size_t)pl.Pc * ray_stride(G));
-    pl.off_gpix = o; o = align256(o + sizeof(float) * (size_t)pl.Pc * gpix_stride(G));
-    pl.off_chi = o;  o = align256(o + sizeof(float) * (size_t)pl.Pc * c->n_ctile);
-    pl.off_nap = o;  o = align256(o + sizeof(float) * (size_t)pl.Pc * c->n_nap * c->na);
+    pl.off_ray = o;  o = align256(o + es * (size_t)pl.Pc * ray_stride(G));
+    pl.off_gpix = o; o = align256(o + es * (size_t)pl.Pc * gpix_stride(G));
+    pl.off_chi = o;  o = align256(o + es * (size_t)pl.Pc * c->n_ctile);
+    pl.off_nap = o;  o = align256(o + es * (size_t)pl.Pc * c->n_nap * c->na);
     pl.total = o;
     return pl;
 }
@@ -223,45 +228,93 @@ extern "C" size_t gl_workspace_bytes(const gl_config* c, int64_t n_particles) {
 }
 
 // ----------------------------------------------------------------------------- variant dispatch
-template <class V>
-static void launch_ray_fwd(const gl_config* c, const float* pb, float* ray, int64_t Pc, cudaStream_t st) {
+template <class T, class V>
+static void launch_ray_fwd(const gl_config* c, const T* pb, const double* tab, T* ray, int64_t Pc, cudaStream_t st) {
     dim3 grid(c->G.s * c->G.s * c->n_chunk_fwd, (unsigned)Pc);
-    gl_ray_fwd_kernel<V, NT_FWD><<<grid, c->nt_fwd, 0, st>>>(c->G, pb, ray, c->rpt_fwd, c->n_chunk_fwd);
+    gl_ray_fwd_kernel<T, V, NT_FWD><<<grid, c->nt_fwd, 0, st>>>(c->G, pb, tab, ray, c->rpt_fwd, c->n_chunk_fwd);
 }
-template <class V>
-static void launch_ray_adj(const gl_config* c, const float* pb, const float* gbar, float* nap, int64_t Pc, cudaStream_t st) {
+template <class T, class V>
+static void launch_ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, int64_t Pc, cudaStream_t st) {
     dim3 grid(c->n_nap, (unsigned)Pc);
-    gl_ray_adj_kernel<V, NT_ADJ><<<grid, c->nt_adj, 0, st>>>(c->G, pb, gbar, nap, c->rpt_adj, c->n_chunk_adj);
+    gl_ray_adj_kernel<T, V, NT_ADJ><<<grid, c->nt_adj, 0, st>>>(c->G, pb, tab, gbar, nap, c->rpt_adj, c->n_chunk_adj);
 }
 
 using V_S0 = Variant<0, 0, 1, -1, 1>; using V_E0 = Variant<1, 0, 1, -1, 1>;
 using V_S1 = Variant<0, 0, 1, 6, 2>;  using V_E1 = Variant<1, 0, 1, 6, 2>;
 using V_S2 = Variant<0, 3, 1, 10, 2>; using V_E2 = Variant<1, 3, 1, 10, 2>;
 
-static void ray_fwd(const gl_config* c, const float* pb, float* ray, int64_t Pc, cudaStream_t st) {
+template <class T>
+static void ray_fwd(const gl_config* c, const T* pb, const double* tab, T* ray, int64_t Pc, cudaStream_t st) {
     const int id = c->variant * 2 + c->desc.mass_model;
     switch (id) {
-        case 0: launch_ray_fwd<V_S0>(c, pb, ray, Pc, st); break;
-        case 1: launch_ray_fwd<V_E0>(c, pb, ray, Pc, st); break;
-        case 2: launch_ray_fwd<V_S1>(c, pb, ray, Pc, st); break;
-        case 3: launch_ray_fwd<V_E1>(c, pb, ray, Pc, st); break;
-        case 4: launch_ray_fwd<V_S2>(c, pb, ray, Pc, st); break;
-        default: launch_ray_fwd<V_E2>(c, pb, ray, Pc, st); break;
+        case 0: launch_ray_fwd<T, V_S0>(c, pb, tab, ray, Pc, st); break;
+        case 1: launch_ray_fwd<T, V_E0>(c, pb, tab, ray, Pc, st); break;
+        case 2: launch_ray_fwd<T, V_S1>(c, pb, tab, ray, Pc, st); break;
+        case 3: launch_ray_fwd<T, V_E1>(c, pb, tab, ray, Pc, st); break;
+        case 4: launch_ray_fwd<T, V_S2>(c, pb, tab, ray, Pc, st); break;
+        default: launch_ray_fwd<T, V_E2>(c, pb, tab, ray, Pc, st); break;
     }
 }
-static void ray_adj(const gl_config* c, const float* pb, const float* gbar, float* nap, int64_t Pc, cudaStream_t st) {
+template <class T>
+static void ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, int64_t Pc, cudaStream_t st) {
     const int id = c->variant * 2 + c->desc.mass_model;
     switch (id) {
-        case 0: launch_ray_adj<V_S0>(c, pb, gbar, nap, Pc, st); break;
-        case 1: launch_ray_adj<V_E0>(c, pb, gbar, nap, Pc, st); break;
-        case 2: launch_ray_adj<V_S1>(c, pb, gbar, nap, Pc, st); break;
-        case 3: launch_ray_adj<V_E1>(c, pb, gbar, nap, Pc, st); break;
-        case 4: launch_ray_adj<V_S2>(c, pb, gbar, nap, Pc, st); break;
-        default: launch_ray_adj<V_E2>(c, pb, gbar, nap, Pc, st); break;
+        case 0: launch_ray_adj<T, V_S0>(c, pb, tab, gbar, nap, Pc, st); break;
+        case 1: launch_ray_adj<T, V_E0>(c, pb, tab, gbar, nap, Pc, st); break;
+        case 2: launch_ray_adj<T, V_S1>(c, pb, tab, gbar, nap, Pc, st); break;
+        case 3: launch_ray_adj<T, V_E1>(c, pb, tab, gbar, nap, Pc, st); break;
+        case 4: launch_ray_adj<T, V_S2>(c, pb, tab, gbar, nap, Pc, st); break;
+        default: launch_ray_adj<T, V_E2>(c, pb, tab, gbar, nap, Pc, st); break;
     }
 }
 
 // mode 0: logpost, 1: logpost + grad, 2: model image
+template <class T>
+static gl_status run_t(const gl_config* c, int mode, const float* obs, const float* sigma, const float* psf,
+                       const float* params, const int32_t* system_id, int64_t P, float* out_logp, float* out_grad,
+                       float* out_image, void* ws, const Plan& pl, cudaStream_t st) {
+    const Geom& G = c->G;
+    char* w = (char*)ws;
+    double* tab = (double*)(w + pl.off_tab);
+    T* sys_kt = (T*)(w + pl.off_kt); T* sys_w = (T*)(w + pl.off_w); double* sys_sl = (double*)(w + pl.off_sl);
+    T* pb = (T*)(w + pl.off_pb); double* lpd = (double*)(w + pl.off_lpd);
+    T* ray = (T*)(w + pl.off_ray); T* gpix = (T*)(w + pl.off_gpix);
+    T* chi = (T*)(w + pl.off_chi); T* nap = (T*)(w + pl.off_nap);
+    double* tab_out = sizeof(T) == 8 ? tab : nullptr;
+
+    // sigma is not an input of gl_model_image (mode 2): prep then only builds kt (and the math tables)
+    GL_STAGE(ST_PREP, st, (gl_prep_kernel<T><<<c->desc.n_systems, 256, 0, st>>>(G, psf, mode == 2 ? nullptr : sigma, sys_kt, sys_w,
+                                                                             sys_sl, tab_out)));
+    ++t_launches;
+    for (int64_t base = 0; base < P; base += pl.Pc) {
+        const int64_t Pc = (P - base) < pl.Pc ? (P - base) : pl.Pc;
+        GL_STAGE(ST_UNPACK, st, (gl_unpack_kernel<T><<<(unsigned)((Pc + 127) / 128), 128, 0, st>>>(
+            c->pt, c->L, G, c->desc.pix_scale, params + base * c->L.n_params, Pc, pb, lpd)));
+        ++t_launches;
+        GL_STAGE(ST_RAY_FWD, st, ray_fwd<T>(c, pb, tab, ray, Pc, st)); ++t_launches;
+        int nl = 0;
+        GL_STAGE(ST_CONV_FWD, st, nl = conv_fwd_launch<T>(c->conv, G, ray, sys_kt, sys_w, obs, system_id, base, Pc,
+                                         mode == 2 ? nullptr : gpix, mode == 2 ? nullptr : chi,
+                                         mode == 2 ? out_image : nullptr, st));
+        if (nl < 0) return GL_ERR_CUDA;
+        t_launches += nl;
+        if (mode == 2) continue;
+        if (mode == 1) {
+            GL_STAGE(ST_CONV_BWD, st, nl = conv_bwd_launch<T>(c->conv, G, gpix, sys_kt, system_id, base, Pc, ray, st));
+            if (nl < 0) return GL_ERR_CUDA;
+            t_launches += nl;
+            GL_STAGE(ST_RAY_ADJ, st, ray_adj<T>(c, pb, tab, ray, nap, Pc, st)); ++t_launches;
+        }
+        const int wpb = 4;
+        GL_STAGE(ST_FINALIZE, st, (gl_finalize_kernel<T><<<(unsigned)((Pc + wpb - 1) / wpb), wpb * 32, wpb * (NA_MAX + 128) * sizeof(double), st>>>(
+            c->pt, c->L, G, params, pb, lpd, chi, c->n_ctile, mode == 1 ? nap : nullptr, c->n_nap, c->na,
+            sys_sl, system_id, Pc, base, out_logp, out_grad)));
+        ++t_launches;
+    }
+    cudaError_t e = cudaPeekAtLastError();
+    return e == cudaSuccess ? GL_OK : GL_ERR_CUDA;
+}
+
 static gl_status run(const gl_config* c, int mode, const float* obs, const float* sigma, const float* psf,
                      const float* params, const int32_t* system_id, int64_t P, float* out_logp, float* out_grad,
                      float* out_image, void* ws, size_t ws_bytes, cudaStream_t st) {
@@ -276,46 +329,9 @@ static gl_status run(const gl_config* c, int mode, const float* obs, const float
     if (mode == 2 && !out_image) return GL_ERR_NULL;
     const Plan pl = make_plan(c, P);
     if (ws_bytes < pl.total || ((uintptr_t)ws & 255) != 0) return GL_ERR_WORKSPACE;
-    const Geom& G = c->G;
-    char* w = (char*)ws;
-    float* sys_kt = (float*)(w + pl.off_kt); float* sys_w = (float*)(w + pl.off_w); float* sys_sl = (float*)(w + pl.off_sl);
-    float* pb = (float*)(w + pl.off_pb); double* lpd = (double*)(w + pl.off_lpd);
-    float* ray = (float*)(w + pl.off_ray); float* gpix = (float*)(w + pl.off_gpix);
-    float* chi = (float*)(w + pl.off_chi); float* nap = (float*)(w + pl.off_nap);
-
-    if (mode == 2) {
-        // kt only (sigma is not an input of gl_model_image): run prep with a unit sigma stand-in = the w buffer itself
-        GL_STAGE(ST_PREP, st, (gl_prep_kernel<<<c->desc.n_systems, 256, 0, st>>>(G, psf, nullptr, sys_kt, sys_w, sys_sl))); ++t_launches;
-    } else {
-        GL_STAGE(ST_PREP, st, (gl_prep_kernel<<<c->desc.n_systems, 256, 0, st>>>(G, psf, sigma, sys_kt, sys_w, sys_sl))); ++t_launches;
-    }
-    for (int64_t base = 0; base < P; base += pl.Pc) {
-        const int64_t Pc = (P - base) < pl.Pc ? (P - base) : pl.Pc;
-        GL_STAGE(ST_UNPACK, st, (gl_unpack_kernel<<<(unsigned)((Pc + 127) / 128), 128, 0, st>>>(
-            c->pt, c->L, G, c->desc.pix_scale, params + base * c->L.n_params, Pc, pb, lpd)));
-        ++t_launches;
-        GL_STAGE(ST_RAY_FWD, st, ray_fwd(c, pb, ray, Pc, st)); ++t_launches;
-        int nl = 0;
-        GL_STAGE(ST_CONV_FWD, st, nl = conv_fwd_launch(c->conv, G, ray, sys_kt, sys_w, obs, system_id, base, Pc,
-                                      mode == 2 ? nullptr : gpix, mode == 2 ? nullptr : chi,
-                                      mode == 2 ? out_image : nullptr, st));
-        if (nl < 0) return GL_ERR_CUDA;
-        t_launches += nl;
-        if (mode == 2) continue;
-        if (mode == 1) {
-            GL_STAGE(ST_CONV_BWD, st, nl = conv_bwd_launch(c->conv, G, gpix, sys_kt, system_id, base, Pc, ray, st));
-            if (nl < 0) return GL_ERR_CUDA;
-            t_launches += nl;
-            GL_STAGE(ST_RAY_ADJ, st, ray_adj(c, pb, ray, nap, Pc, st)); ++t_launches;
-        }
-        const int wpb = 4;
-        GL_STAGE(ST_FINALIZE, st, (gl_finalize_kernel<<<(unsigned)((Pc + wpb - 1) / wpb), wpb * 32, wpb * (NA_MAX + 128) * sizeof(double), st>>>(
-            c->pt, c->L, G, params, pb, lpd, chi, c->n_ctile, mode == 1 ? nap : nullptr, c->n_nap, c->na,
-            sys_sl, system_id, Pc, base, out_logp, out_grad)));
-        ++t_launches;
-    }
-    cudaError_t e = cudaPeekAtLastError();
-    return e == cudaSuccess ? GL_OK : GL_ERR_CUDA;
+    if (c->esize == 8)
+        return run_t<double>(c, mode, obs, sigma, psf, params, system_id, P, out_logp, out_grad, out_image, ws, pl, st);
+    return run_t<float>(c, mode, obs, sigma, psf, params, system_id, P, out_logp, out_grad, out_image, ws, pl, st);
 }
 
 extern "C" gl_status gl_logpost(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,

@@ -73,7 +73,7 @@ struct Geom {            // launch-invariant geometry, passed by value
     int N, s, M, K, c;   // pixels/side, supersample, rays/side, psf taps/side, (K-1)/2
     int KEp, U;          // padded k_eff taps per side (multiple of s), taps per phase per side
     int n_terms;         // EPL series terms kept (2..30)
-    float delta2;        // pix_scale^2
+    double delta2;       // pix_scale^2 (fp64 product of the fp32 pix_scale)
     int UP;              // U rounded up to a multiple of the tap rows one conv thread handles
     int Hp, Wp;          // rows / row pitch of one padded phase plane of RAY
     int Hg, Wg, PADg;    // rows / row pitch / border of the padded GPIX image
@@ -82,7 +82,8 @@ __host__ __device__ inline int phase_shift(const Geom& G, int a) { return (a + G
 __host__ __device__ inline size_t ray_stride(const Geom& G) { return (size_t)G.s * G.s * G.Hp * G.Wp; }
 __host__ __device__ inline size_t gpix_stride(const Geom& G) { return (size_t)G.Hg * G.Wg; }
 
-__device__ __forceinline__ float warp_sum(float v) {
+template <class T>
+__device__ __forceinline__ T warp_sum(T v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;

@@ -80,7 +80,8 @@ __device__ inline double theta_at(const PriorTable& pt, const Layout& L, const f
 }
 
 // Write one Sersic block [R, n, e1, e2, x0, y0, Ie] into PB; a negative `off` writes a neutral (Ie = 0) block.
-__device__ inline void write_sersic(const PriorTable& pt, const Layout& L, const float* z, int off, float* sb,
+template <class T>
+__device__ inline void write_sersic(const PriorTable& pt, const Layout& L, const float* z, int off, T* sb,
                                     double x_first, bool& ok) {
     double R = 1, n = 1, e1 = 0, e2 = 0, x0 = 0, y0 = 0, Ie = 0;
     if (off >= 0) {
@@ -92,22 +93,23 @@ __device__ inline void write_sersic(const PriorTable& pt, const Layout& L, const
     }
     Ell E = make_ell(e1, e2);
     double bn = 1.9992 * n - 0.3271;
-    sb[SB_XOFF] = (float)(x_first - x0); sb[SB_YOFF] = (float)(x_first - y0);
-    sb[SB_C] = (float)E.cphi; sb[SB_S] = (float)E.sphi; sb[SB_Q] = (float)E.q; sb[SB_QI] = (float)(1.0 / E.q);
-    sb[SB_K1] = (float)(0.5 / n); sb[SB_K0] = (float)(-log2(R) / n);
-    sb[SB_C1] = (float)(bn * 1.44269504088896340736); sb[SB_IE] = (float)Ie;
-    sb[SB_KQ] = (float)(bn / n * E.q); sb[SB_KQI] = (float)(bn / n / E.q);
-    sb[12] = sb[13] = sb[14] = sb[15] = 0.f;
+    sb[SB_XOFF] = (T)(x_first - x0); sb[SB_YOFF] = (T)(x_first - y0);
+    sb[SB_C] = (T)E.cphi; sb[SB_S] = (T)E.sphi; sb[SB_Q] = (T)E.q; sb[SB_QI] = (T)(1.0 / E.q);
+    sb[SB_K1] = (T)(0.5 / n); sb[SB_K0] = (T)(-log2(R) / n);
+    sb[SB_C1] = (T)(bn * 1.44269504088896340736); sb[SB_IE] = (T)Ie;
+    sb[SB_KQ] = (T)(bn / n * E.q); sb[SB_KQI] = (T)(bn / n / E.q);
+    sb[12] = sb[13] = sb[14] = sb[15] = T(0);
 }
 
 // Step A.  One thread per particle.  pb: [P][PB_STRIDE]; lpd: [P] = sum log prior + sum log-det (fp64).
+template <class T>
 __global__ void gl_unpack_kernel(const __grid_constant__ PriorTable pt, const __grid_constant__ Layout L,
                                  const __grid_constant__ Geom G, float pix_scale,
-                                 const float* __restrict__ params, int64_t P, float* __restrict__ pb, double* __restrict__ lpd) {
+                                 const float* __restrict__ params, int64_t P, T* __restrict__ pb, double* __restrict__ lpd) {
     int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P) return;
     const float* z = params + p * L.n_params;
-    float* o = pb + p * PB_STRIDE;
+    T* o = pb + p * PB_STRIDE;
     bool ok = true;
     double lp = 0;
     for (int i = 0; i < L.n_params; ++i) {
@@ -126,47 +128,47 @@ __global__ void gl_unpack_kernel(const __grid_constant__ PriorTable pt, const __
     if (!(thE > 0) || !(t > 0 && t < 2) || !(e1 * e1 + e2 * e2 < 1.0)) { ok = false; thE = 1; t = 1; e1 = e2 = 0; }
     Ell E = make_ell(e1, e2);
     double b = thE * sqrt(E.q), f = (1 - E.q) / (1 + E.q);
-    o[PB_M_XOFF] = (float)(x_first - x0); o[PB_M_YOFF] = (float)(x_first - y0);
-    o[PB_M_C] = (float)E.cphi; o[PB_M_S] = (float)E.sphi; o[PB_M_Q] = (float)E.q; o[PB_M_B] = (float)b;
-    o[PB_M_T] = (float)t; o[PB_M_F] = (float)f; o[PB_M_L2B] = (float)log2(b); o[PB_M_A] = (float)(2 * b / (1 + E.q));
+    o[PB_M_XOFF] = (T)(x_first - x0); o[PB_M_YOFF] = (T)(x_first - y0);
+    o[PB_M_C] = (T)E.cphi; o[PB_M_S] = (T)E.sphi; o[PB_M_Q] = (T)E.q; o[PB_M_B] = (T)b;
+    o[PB_M_T] = (T)t; o[PB_M_F] = (T)f; o[PB_M_L2B] = (T)log2(b); o[PB_M_A] = (T)(2 * b / (1 + E.q));
     double qp = sqrt(fmax(1 - E.q * E.q, 0.0));
-    o[PB_M_QP] = (float)qp; o[PB_M_BQP] = (float)(qp > 0 ? b / qp : 0.0);
-    o[PB_M_F2] = (float)(f * f); o[PB_M_TM1] = (float)(t - 1); o[PB_M_KAPC] = (float)(0.5 * (2 - t) * b);
-    o[PB_G1] = L.shear >= 0 ? (float)theta_at(pt, L, z, L.shear, ok) : 0.f;
-    o[PB_G2] = L.shear >= 0 ? (float)theta_at(pt, L, z, L.shear + 1, ok) : 0.f;
-    o[PB_C3] = L.mp3 >= 0 ? (float)theta_at(pt, L, z, L.mp3, ok) : 0.f;
-    o[PB_S3] = L.mp3 >= 0 ? (float)theta_at(pt, L, z, L.mp3 + 1, ok) : 0.f;
-    o[PB_C4] = L.mp4 >= 0 ? (float)theta_at(pt, L, z, L.mp4, ok) : 0.f;
-    o[PB_S4] = L.mp4 >= 0 ? (float)theta_at(pt, L, z, L.mp4 + 1, ok) : 0.f;
-    o[PB_XFIRST] = (float)x_first; o[PB_STEP] = (float)step;
-    write_sersic(pt, L, z, L.src, o + PB_SRC, x_first, ok);
-    write_sersic(pt, L, z, L.ll0, o + PB_LL0, x_first, ok);
-    write_sersic(pt, L, z, L.ll1, o + PB_LL1, x_first, ok);
+    o[PB_M_QP] = (T)qp; o[PB_M_BQP] = (T)(qp > 0 ? b / qp : 0.0);
+    o[PB_M_F2] = (T)(f * f); o[PB_M_TM1] = (T)(t - 1); o[PB_M_KAPC] = (T)(0.5 * (2 - t) * b);
+    o[PB_G1] = L.shear >= 0 ? (T)theta_at(pt, L, z, L.shear, ok) : T(0);
+    o[PB_G2] = L.shear >= 0 ? (T)theta_at(pt, L, z, L.shear + 1, ok) : T(0);
+    o[PB_C3] = L.mp3 >= 0 ? (T)theta_at(pt, L, z, L.mp3, ok) : T(0);
+    o[PB_S3] = L.mp3 >= 0 ? (T)theta_at(pt, L, z, L.mp3 + 1, ok) : T(0);
+    o[PB_C4] = L.mp4 >= 0 ? (T)theta_at(pt, L, z, L.mp4, ok) : T(0);
+    o[PB_S4] = L.mp4 >= 0 ? (T)theta_at(pt, L, z, L.mp4 + 1, ok) : T(0);
+    o[PB_XFIRST] = (T)x_first; o[PB_STEP] = (T)step;
+    write_sersic<T>(pt, L, z, L.src, o + PB_SRC, x_first, ok);
+    write_sersic<T>(pt, L, z, L.ll0, o + PB_LL0, x_first, ok);
+    write_sersic<T>(pt, L, z, L.ll1, o + PB_LL1, x_first, ok);
     // shapelets (coefficients pre-divided by beta_s; orders above the configured nmax are zero)
     if (L.ker_nmax >= 0) {
         double bs = 1.0;
         if (L.shp >= 0) { bs = theta_at(pt, L, z, L.shp, ok); if (!(bs > 0)) { ok = false; bs = 1; } }
-        o[PB_SHP] = (float)(1.0 / bs); o[PB_SHP + 1] = o[PB_SHP + 2] = o[PB_SHP + 3] = 0.f;
+        o[PB_SHP] = (T)(1.0 / bs); o[PB_SHP + 1] = o[PB_SHP + 2] = o[PB_SHP + 3] = T(0);
         int nck = (L.ker_nmax + 1) * (L.ker_nmax + 2) / 2;
         for (int k = 0; k < nck; ++k)
-            o[PB_SHP_A + k] = (L.shp >= 0 && k < L.n_coef) ? (float)(theta_at(pt, L, z, L.shp + 1 + k, ok) / bs) : 0.f;
+            o[PB_SHP_A + k] = (L.shp >= 0 && k < L.n_coef) ? (T)(theta_at(pt, L, z, L.shp + 1 + k, ok) / bs) : T(0);
     }
     // EPL series coefficients: a_n = prod_{k<=n} (2k-2+t)/(2k+2-t); d_m = (m+1) a_{m+1}; e_m = L_{m+1} a_{m+1}
     if (L.mass_model == 1) {
         double an = 1.0, Ln = 0.0;
-        o[PB_SER_A] = 1.f;
+        o[PB_SER_A] = T(1);
         for (int n = 1; n < 32; ++n) {
             an *= (2.0 * n - 2.0 + t) / (2.0 * n + 2.0 - t);
             Ln += 4.0 * n / ((2.0 * n + 2.0 - t) * (2.0 * n - 2.0 + t));
             bool keep = n < G.n_terms;
-            o[PB_SER_A + n] = keep ? (float)an : 0.f;
-            o[PB_SER_D + n - 1] = keep ? (float)(n * an) : 0.f;
-            o[PB_SER_E + n - 1] = keep ? (float)(Ln * an) : 0.f;
+            o[PB_SER_A + n] = keep ? (T)an : T(0);
+            o[PB_SER_D + n - 1] = keep ? (T)(n * an) : T(0);
+            o[PB_SER_E + n - 1] = keep ? (T)(Ln * an) : T(0);
         }
-        o[PB_SER_D + 31] = 0.f; o[PB_SER_E + 31] = 0.f;
+        o[PB_SER_D + 31] = T(0); o[PB_SER_E + 31] = T(0);
     }
     if (!isfinite(lp)) ok = false;
-    o[PB_VALID] = ok ? 1.f : 0.f;
+    o[PB_VALID] = ok ? T(1) : T(0);
     lpd[p] = lp;
 }
 
@@ -191,12 +193,13 @@ __device__ inline void sersic_chain(const PriorTable& pt, const Layout& L, const
 // Tail of step E/F.  One WARP per particle.  Sums the per-tile chi^2 partials and the per-chunk natural
 // accumulators in a fixed order (fp64), applies the chain rule natural -> theta -> z, adds prior and
 // log-det terms, and writes out_logp / out_grad.  nap may be NULL (gl_logpost: no gradient).
+template <class T>
 __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const __grid_constant__ Layout L,
                                    const __grid_constant__ Geom G,
-                                   const float* __restrict__ params, const float* __restrict__ pb,
-                                   const double* __restrict__ lpd, const float* __restrict__ chi, int n_ctile,
-                                   const float* __restrict__ nap, int n_chunk, int na,
-                                   const float* __restrict__ sys_sumlog, const int32_t* __restrict__ system_id,
+                                   const float* __restrict__ params, const T* __restrict__ pb,
+                                   const double* __restrict__ lpd, const T* __restrict__ chi, int n_ctile,
+                                   const T* __restrict__ nap, int n_chunk, int na,
+                                   const double* __restrict__ sys_sumlog, const int32_t* __restrict__ system_id,
                                    int64_t P, int64_t p_base, float* __restrict__ out_logp, float* __restrict__ out_grad) {
     extern __shared__ double fsm[];                     // per warp: nat[NA_MAX] + gth[128]
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -205,14 +208,14 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
     double* nat = fsm + (size_t)wib * (NA_MAX + 128);
     double* gth = nat + NA_MAX;
     const float* z = params + (p_base + p) * L.n_params;
-    const bool valid = pb[p * PB_STRIDE + PB_VALID] != 0.f;
+    const bool valid = pb[p * PB_STRIDE + PB_VALID] != T(0);
     // chi^2: lanes stride over tiles, then a fixed xor-tree
     double c2 = 0;
     for (int k = lane; k < n_ctile; k += 32) c2 += (double)chi[p * n_ctile + k];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) c2 += __shfl_xor_sync(0xffffffffu, c2, o);
     const int sys = system_id ? system_id[p_base + p] : 0;
-    double logp = -0.5 * c2 - (double)sys_sumlog[sys] - 0.5 * G.N * G.N * 1.83787706640934548356 + lpd[p];
+    double logp = -0.5 * c2 - sys_sumlog[sys] - 0.5 * G.N * G.N * 1.83787706640934548356 + lpd[p];
     bool good = valid && isfinite(logp);
     if (nap) {
         for (int k = lane; k < na; k += 32) {

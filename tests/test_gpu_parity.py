@@ -22,11 +22,13 @@ def _gl():
     return gl
 
 
-def _model(k):
+def _model(k, precision=0):
+    """precision 0 = GL_PRECISION_F64 (the default mode, the one bench.py times), 1 = GL_PRECISION_F32."""
+    import dataclasses
     import torch
     gl = _gl()
     wl, obs, sig = observation(k)
-    m = gl.LensModel(wl.spec, obs, sig, wl.psf)
+    m = gl.LensModel(dataclasses.replace(wl.spec, precision=precision), obs, sig, wl.psf)
     return gl, torch, wl, m
 
 
@@ -61,6 +63,29 @@ def test_parity_subset(k):
     _dump("cfg%d" % k, rep)
     assert rel_lp.max() <= RTOL_LOGP, rep
     assert rep["n_fail"] == 0, rep
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_f32_mode_statistical_parity(k):
+    """GL_PRECISION_F32 (FP32 FMA + MUFU, the fast mode): fp32 arithmetic cannot meet the per-component bar on
+    ill-conditioned components, so this mode is held to the documented statistical bar:
+    >= 99 % of the gradient components inside max(1e-3 |g|, 1e-5), norm-wise gradient error <= 2e-2 per particle,
+    >= 97 % of the particles inside the 1e-4 log-posterior bar and no log-posterior off by more than 1e-3 relative
+    or 10 absolute."""
+    gl, torch, wl, m = _model(k, precision=1)
+    idx, ref = oracle_subset(k)
+    z = torch.from_numpy(wl.params[idx]).cuda()
+    sid = wl.system_id[idx] if wl.system_id is not None else None
+    lp, g = m.logpost_grad(z, sid)
+    torch.cuda.synchronize()
+    lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+    dlp = np.abs(lp - ref["logp"])
+    rel_lp = dlp / np.abs(ref["logp"])
+    ok, rep = grad_report(g, ref["grad"], ref["gabs"])
+    rep.update(k=k, n_particles=int(len(idx)), max_rel_logp=float(rel_lp.max()), frac_logp_in_bar=float(np.mean(rel_lp <= RTOL_LOGP)))
+    _dump("f32_cfg%d" % k, rep)
+    assert rep["pass_frac"] >= 0.99 and rep["normwise"] <= 2e-2, rep
+    assert np.mean(rel_lp <= RTOL_LOGP) >= 0.97 and np.all((rel_lp <= 1e-3) | (dlp <= 10.0)), rep
 
 
 @pytest.mark.parametrize("k", [1, 2, 3, 5])
