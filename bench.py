@@ -51,6 +51,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
+                    help="arithmetic of the CUDA path: f64 = GL_PRECISION_F64 (default; strict parity), f32 = GL_PRECISION_F32")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -194,6 +196,7 @@ def run_ours(a):
     k = a.config
     wl = W.make_workload(k)
     sp = wl.spec
+    sp.precision = 0 if a.precision == "f64" else 1
     P, n_p, N = wl.params.shape[0], sp.n_params, sp.n_pix
     # observation: truth rendered by THIS side (gl_model_image), noise from the seeded stream (workloads docstring)
     zeros = np.zeros((sp.n_systems, N, N), np.float32)
@@ -289,7 +292,7 @@ def run_ours(a):
         roof["frac_at_measured_clock"] = achieved / (N_SM * FP32_LANES * clocks["sm_mhz"] * 1e6 / 1e12)
     out = {"metric": METRIC, "value": world * P * a.steps / t_dev, "unit": UNIT, "n_gpus": world, "steps": a.steps,
            "warmup": max(a.warmup, 3), "ms_per_step": t_dev / a.steps * 1e3, "higher_is_better": True,
-           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "scaling": "weak", "vs_baseline": None, "dtype": a.precision, "data": "synthetic",
            "config": {"workload": WORKLOAD_NAMES[k], "n_particles_per_gpu": P, "n_params": n_p,
                       "rays_per_particle": wm["rays"], "parallelism": "replicas x%d" % world,
                       "l2": "256 MiB flush write between timed iterations; workspace %.0f MB" % (ws_bytes / 1e6),

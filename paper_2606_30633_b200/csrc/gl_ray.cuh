@@ -348,7 +348,8 @@ __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ 
 #pragma unroll 2
     for (int r = 0; r < RPT; ++r) {
         if (it.idx < NN) {
-            T v = ray_eval<T, V, false>(tb, pb, it.fj<T>(G), it.fi<T>(G), T(0.), nullptr);
+            int off = 0; asm volatile("" : "+r"(off));      // opaque: keeps the PB scalars in shared memory, not in registers
+            T v = ray_eval<T, V, false>(tb, pb + off, it.fj<T>(G), it.fi<T>(G), T(0.), nullptr);
             out[it.offset(G)] = valid ? v : T(0.);
         }
         it.next(G);
@@ -376,7 +377,8 @@ __global__ void __launch_bounds__(NT) gl_ray_adj_kernel(const __grid_constant__ 
     for (int k = 0; k < V::NA; ++k) acc[k] = T(0.);
     if (pb[PB_VALID] != T(0.)) {
         for (int r = 0; r < RPT; ++r) {
-            if (it.idx < NN) ray_eval<T, V, true>(tb, pb, it.fj<T>(G), it.fi<T>(G), gb[it.offset(G)], acc);
+            int off = 0; asm volatile("" : "+r"(off));      // opaque: keeps the PB scalars in shared memory, not in registers
+            if (it.idx < NN) ray_eval<T, V, true>(tb, pb + off, it.fj<T>(G), it.fi<T>(G), gb[it.offset(G)], acc);
             it.next(G);
         }
     }
