@@ -77,7 +77,7 @@ extern "C" int32_t gl_stage_times(float* ms_host, int32_t* launches_host, int32_
 
 static constexpr int NT_FWD = 256;     // compiled launch bounds; the block size actually used is chosen per config
 static constexpr int NT_ADJ = 128;
-static constexpr size_t WS_BUDGET = (size_t)1536 << 20;   // chunk so that per-chunk buffers stay below ~1.5 GiB
+static constexpr size_t WS_BUDGET = (size_t)4096 << 20;   // chunk so that per-chunk buffers stay below ~4 GiB
 
 static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 

@@ -12,11 +12,13 @@
 //   gbar_ab[n + o_a][j'] = sum_{k,l < U} kt[a'][b'][U-1-k][U-1-l] * gp[n + o_a + k][j' + l]           (transpose)
 // where gp is g_pix zero-padded by U-1 on every side and gbar is produced directly in the plane layout.
 //
-// Both directions run the same inner loop (gl_conv_*_sw): one thread owns 4 adjacent output columns of ONE plane and
-// UR consecutive tap rows, keeps its UR x U taps and a UR-row sliding window of the input in registers, and sweeps
-// down the image: per output row it loads one new input row segment (U+3 floats, 16-byte aligned) and issues
-// 4*UR*U FMAs.  Step D then sums the s*s*ceil(U/UR) partial results per pixel through shared memory in a fixed
-// order (deterministic), and applies step E in the same pass.
+// Both directions run the same inner loop (conv_slide): "input-stationary" sliding accumulators.  One thread owns CW
+// adjacent output columns and a few phase planes; it walks down the input rows ONCE, and every input row segment
+// (CW+U-1 values, loaded one step ahead) is scattered into the U output rows it contributes to, held as acc[U][CW]
+// registers; the finished row leaves at the bottom and the accumulators shift by one.  Per step: U*U*CW FMAs on
+// CW+U-1 loaded values, taps read from shared memory as 16-byte broadcasts.  Four adjacent lanes share a column
+// group and split the s*s planes between them; step D sums their partial rows with two shuffles (fixed order) and
+// applies step E in the same pass.  No tap or window registers -> ~100 registers in fp64, many resident warps.
 #pragma once
 #include "gl_common.cuh"
 #include "gl_math.cuh"
@@ -150,184 +152,207 @@ __global__ void __launch_bounds__(256) gl_conv_bwd_generic(const __grid_constant
     gbar[(size_t)p * ray_stride(G) + ((size_t)ph * G.Hp + n + oa) * G.Wp + j1 + ob] = acc;
 }
 
-// ----------------------------------------------------------------------------- sliding-window kernels
-// 4 consecutive T, 4-element aligned: one 16-byte load for float, two for double.
-__device__ __forceinline__ void load4(const float* __restrict__ p, float* w) {
-    const float4 x = __ldg(reinterpret_cast<const float4*>(p));
-    w[0] = x.x; w[1] = x.y; w[2] = x.z; w[3] = x.w;
-}
-__device__ __forceinline__ void load4(const double* __restrict__ p, double* w) {
-    const double2 x = __ldg(reinterpret_cast<const double2*>(p)), y = __ldg(reinterpret_cast<const double2*>(p) + 1);
-    w[0] = x.x; w[1] = x.y; w[2] = y.x; w[3] = y.y;
-}
-__device__ __forceinline__ void store4(float* p, const float* a) { *reinterpret_cast<float4*>(p) = make_float4(a[0], a[1], a[2], a[3]); }
-__device__ __forceinline__ void store4(double* p, const double* a) {
-    reinterpret_cast<double2*>(p)[0] = make_double2(a[0], a[1]); reinterpret_cast<double2*>(p)[1] = make_double2(a[2], a[3]);
-}
+// ----------------------------------------------------------------------------- input-stationary sliding kernels
+template <class T> struct Vec2;
+template <> struct Vec2<float>  { using type = float2; };
+template <> struct Vec2<double> { using type = double2; };
 
-template <class T, int U>
-struct RowSeg {                                  // the U+3 input values that 4 adjacent outputs need from one row
-    static constexpr int NEED = U + 3;
-    static constexpr int NV4 = (NEED % 4 <= 1) ? NEED / 4 : (NEED + 3) / 4;
-    static constexpr int NSC = (NEED % 4 <= 1) ? NEED % 4 : 0;
-    static constexpr int NVAL = NV4 * 4 + NSC;
-    static constexpr int WL = 4 * ((NEED + 3) / 4);                 // values a row segment may touch
-    static __device__ __forceinline__ void load(T (&w)[NVAL], const T* __restrict__ p) {
-#pragma unroll
-        for (int v = 0; v < NV4; ++v) load4(p + 4 * v, &w[4 * v]);
-#pragma unroll
-        for (int i = 0; i < NSC; ++i) w[4 * NV4 + i] = __ldg(p + 4 * NV4 + i);
-    }
+// Launch-invariant description of the sliding kernels (filled by conv_plan).
+struct SlidePlan {
+    int ncg;      // column groups per particle
+    int tpp;      // threads per particle slot (multiple of 32) = roundup32(4 * ncg)
+    int ppc;      // particle slots per CTA
+    int ps;       // tap stride between phases in shared memory (elements)
 };
 
-template <class T, int U, int NVAL>
-__device__ __forceinline__ void fma_row(T (&acc)[4], const T (&Tp)[U], const T (&w)[NVAL]) {
+// acc[u][q] += sum_v tap[u][v] * seg[q + v] for one input row segment.  tap: shared memory, row pitch UP2 (even).
+template <class T, int U, int CW, int SEG>
+__device__ __forceinline__ void conv_slide(T (&acc)[U][CW], const T* __restrict__ tap, const T (&seg)[SEG]) {
+    using V2 = typename Vec2<T>::type;
+    constexpr int UP2 = (U + 1) & ~1;
 #pragma unroll
-    for (int l = 0; l < U; ++l) {
+    for (int u = 0; u < U; ++u) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) acc[q] = Real<T>::fma(Tp[l], w[q + l], acc[q]);
+        for (int v = 0; v < UP2; v += 2) {
+            const V2 k = *reinterpret_cast<const V2*>(tap + u * UP2 + v);
+#pragma unroll
+            for (int q = 0; q < CW; ++q) {
+                acc[u][q] = Real<T>::fma(k.x, seg[q + v], acc[u][q]);
+                if (v + 1 < U) acc[u][q] = Real<T>::fma(k.y, seg[q + v + 1], acc[u][q]);
+            }
+        }
     }
 }
 
-constexpr int CONV_R = 4;                        // output rows between two reductions
+template <class T, int SEG>
+__device__ __forceinline__ void load_seg(T (&seg)[SEG], const T* __restrict__ p) {
+    using V2 = typename Vec2<T>::type;
+#pragma unroll
+    for (int v = 0; v < SEG; v += 2) {
+        const V2 x = __ldg(reinterpret_cast<const V2*>(p + v));
+        seg[v] = x.x; seg[v + 1] = x.y;
+    }
+}
 
-// Step D + E.  grid = (n_band, Pc); block = roundup32(ncgb * s*s * ceil(U/UR)); dynamic smem = conv_sw_smem(...).
-// Thread t: column group g = t % ncgb (4 pixels), virtual phase vp = t / ncgb = (plane, tap-row group).
-template <class T, int UR, int U, int NT_MAX>
-__global__ void __launch_bounds__(NT_MAX) gl_conv_fwd_sw(const __grid_constant__ Geom G, int ncgb,
-                                                         const T* __restrict__ ray, const T* __restrict__ sys_kt,
-                                                         const T* __restrict__ sys_w, const float* __restrict__ obs,
-                                                         const int32_t* __restrict__ system_id, int64_t p_base,
-                                                         T* __restrict__ gpix, T* __restrict__ chi,
-                                                         float* __restrict__ out_model) {
-    constexpr int NRG = (U + UR - 1) / UR;
-    constexpr int NVAL = RowSeg<T, U>::NVAL;
-    extern __shared__ __align__(16) unsigned char conv_smem[];     // part [2][NVP][CONV_R][NQ]
-    T* part = reinterpret_cast<T*>(conv_smem);
-    __shared__ T red[32];
-    const int s = G.s, N = G.N, NVP = s * s * NRG, NQ = 4 * ncgb;
-    const int p = blockIdx.y, band = blockIdx.x, t = threadIdx.x;
-    const bool active = t < ncgb * NVP;
-    const int g = active ? t % ncgb : 0, vp = active ? t / ncgb : 0;
-    const int rho = vp % NRG, ph = vp / NRG, a = ph / s, b = ph - a * s;
-    const int sys = system_id ? system_id[p_base + p] : 0;
-    if (gpix) zero_gpix_border(G, gpix + (size_t)p * gpix_stride(G), band * blockDim.x + t, gridDim.x * blockDim.x);
-    T Tp[UR][U];
+// Step D + E.  grid = (ceil(Pc / ppc)); block = ppc * tpp.  Dynamic smem: ppc * s*s * ps taps.
+// Lane lt of a particle slot: column group g = lt / 4, plane subset pq = lt % 4 (planes pq, pq + 4, ...).
+template <class T, int U, int CW, int NT_MAX>
+__global__ void __launch_bounds__(NT_MAX) gl_conv_fwd_is(const __grid_constant__ Geom G, const SlidePlan sp, int64_t Pc,
+                                                      const T* __restrict__ ray, const T* __restrict__ sys_kt,
+                                                      const T* __restrict__ sys_w, const float* __restrict__ obs,
+                                                      const int32_t* __restrict__ system_id, int64_t p_base,
+                                                      T* __restrict__ gpix, T* __restrict__ chi, float* __restrict__ out_model) {
+    constexpr int SEG = (CW + U - 1 + 1) & ~1, UP2 = (U + 1) & ~1;
+    extern __shared__ __align__(16) unsigned char conv_smem[];
+    T* taps = reinterpret_cast<T*>(conv_smem);                   // [ppc][s*s][ps]
+    __shared__ T red[16];
+    const int s = G.s, N = G.N, NPH = s * s;
+    const int slot = threadIdx.x / sp.tpp, lt = threadIdx.x - slot * sp.tpp;
+    const int64_t p = (int64_t)blockIdx.x * sp.ppc + slot;
+    const bool live = p < Pc;
+    const int sys = (live && system_id) ? system_id[p_base + p] : 0;
+    // stage this slot's taps in PLANE order: plane (a,b) uses kt[(a+c)%s][(b+c)%s]
     {
-        const T* kph = sys_kt + (size_t)sys * s * s * U * U + (size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U;
-#pragma unroll
-        for (int k = 0; k < UR; ++k) {
-            const int u1 = rho * UR + k;
-#pragma unroll
-            for (int l = 0; l < U; ++l) Tp[k][l] = (u1 < U) ? __ldg(kph + u1 * U + l) : T(0);
+        T* tp = taps + (size_t)slot * NPH * sp.ps;
+        const T* kt = sys_kt + (size_t)sys * NPH * U * U;
+        for (int e = lt; e < NPH * U * UP2; e += sp.tpp) {
+            const int v = e % UP2, u = (e / UP2) % U, ph = e / (UP2 * U);
+            const int a = ph / s, b = ph - a * s;
+            tp[(size_t)ph * sp.ps + u * UP2 + v] = (v < U) ? kt[(size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U + u * U + v] : T(0);
         }
     }
-    const int gg = min(band * ncgb + g, (G.Wp - RowSeg<T, U>::WL) / 4);      // clamp keeps idle lanes in bounds
-    const T* in = ray + (size_t)p * ray_stride(G) + ((size_t)ph * G.Hp + rho * UR) * G.Wp + 4 * gg;
-    const size_t Wp = (size_t)G.Wp;
-    T w[UR][NVAL];
-#pragma unroll
-    for (int k = 0; k < UR; ++k) RowSeg<T, U>::load(w[k], in + k * Wp);
+    if (live && gpix) zero_gpix_border(G, gpix + (size_t)p * gpix_stride(G), lt, sp.tpp);
+    __syncthreads();
+    const int g = lt >> 2, pq = lt & 3;
+    const bool active = live && g < sp.ncg;
+    const unsigned amask = __ballot_sync(0xffffffffu, active);   // the 4 lanes of a column group are active together
     T c2 = T(0);
-    int buf = 0;
-    for (int pr0 = 0; pr0 < N; pr0 += UR) {
+    if (active) {
+        const int nj = NPH >> 2;                                 // planes per lane
+        const size_t plane = (size_t)G.Hp * G.Wp;
+        const T* in = ray + (size_t)p * ray_stride(G) + (size_t)CW * g;
+        const T* tp = taps + (size_t)slot * NPH * sp.ps;
+        T acc[U][CW];
 #pragma unroll
-        for (int j = 0; j < UR; ++j) {
-            const int pr = pr0 + j;
-            if (pr < N) {
-                T acc[4] = {T(0), T(0), T(0), T(0)};
-                fma_row<T, U, NVAL>(acc, Tp[0], w[j % UR]);
-                if (pr + 1 < N) RowSeg<T, U>::load(w[j % UR], in + (size_t)(pr + UR) * Wp);   // row for the next step
+        for (int u = 0; u < U; ++u)
 #pragma unroll
-                for (int k = 1; k < UR; ++k) fma_row<T, U, NVAL>(acc, Tp[k], w[(j + k) % UR]);
-                if (active) store4(&part[((size_t)(buf * NVP + vp) * CONV_R + (pr & (CONV_R - 1))) * NQ + 4 * g], acc);
-                if ((pr & (CONV_R - 1)) == CONV_R - 1 || pr == N - 1) {
-                    __syncthreads();
-                    const int rows = (pr & (CONV_R - 1)) + 1, r0 = pr - rows + 1;
-                    for (int o = t; o < rows * NQ; o += blockDim.x) {
-                        const int r = o / NQ, q = o - r * NQ, pq = band * NQ + q;
-                        T m = T(0);
-                        for (int v = 0; v < NVP; ++v) m += part[((size_t)(buf * NVP + v) * CONV_R + r) * NQ + q];
-                        if (pq < N) c2 += pixel_epilogue<T>(G, m, r0 + r, pq, sys, (size_t)(p_base + p), p, obs, sys_w, gpix, out_model);
-                    }
-                    buf ^= 1;
+            for (int q = 0; q < CW; ++q) acc[u][q] = T(0);
+        T cur[SEG], nxt[SEG];
+        load_seg<T, SEG>(nxt, in + (size_t)pq * plane);
+        const int steps = G.Hp * nj;
+        int i = 0, j = 0;
+        for (int t = 0; t < steps; ++t) {
+#pragma unroll
+            for (int v = 0; v < SEG; ++v) cur[v] = nxt[v];
+            const int ph = pq + 4 * j;
+            int jn = j + 1, in_ = i;
+            if (jn == nj) { jn = 0; in_ = i + 1; }
+            if (t + 1 < steps) load_seg<T, SEG>(nxt, in + (size_t)(pq + 4 * jn) * plane + (size_t)in_ * G.Wp);
+            conv_slide<T, U, CW, SEG>(acc, tp + (size_t)ph * sp.ps, cur);
+            if (jn == 0) {                                       // input row i done: output row i - U + 1 is complete
+                const int pr = i - (U - 1);
+                T m[CW];
+#pragma unroll
+                for (int q = 0; q < CW; ++q) {
+                    T v = acc[U - 1][q];
+                    v += __shfl_xor_sync(amask, v, 1);
+                    v += __shfl_xor_sync(amask, v, 2);
+                    m[q] = v;
                 }
+                if (pr >= 0) {
+                    T mine = m[0];
+#pragma unroll
+                    for (int q = 1; q < CW; ++q) mine = (pq == q) ? m[q] : mine;
+                    const int pc = CW * g + pq;
+                    if (pq < CW && pc < N)
+                        c2 += pixel_epilogue<T>(G, mine, pr, pc, sys, (size_t)(p_base + p), (int)p, obs, sys_w, gpix, out_model);
+                }
+#pragma unroll
+                for (int u = U - 1; u > 0; --u)
+#pragma unroll
+                    for (int q = 0; q < CW; ++q) acc[u][q] = acc[u - 1][q];
+#pragma unroll
+                for (int q = 0; q < CW; ++q) acc[0][q] = T(0);
             }
+            i = in_; j = jn;
         }
     }
-    if (chi) {
-        const T tot = block_sum(c2, red);
-        if (t == 0) chi[(size_t)p * gridDim.x + band] = tot;
+    if (chi) {                                                   // fixed-order sum over the slot's warps
+        const T ws = warp_sum(c2);
+        const int wps = sp.tpp >> 5, wi = lt >> 5;
+        if ((lt & 31) == 0) red[slot * wps + wi] = ws;
+        __syncthreads();
+        if (lt == 0 && live) {
+            T tot = T(0);
+            for (int w = 0; w < wps; ++w) tot += red[slot * wps + w];
+            chi[p] = tot;
+        }
     }
 }
 
-// Transpose of step D.  grid = (n_band, Pc); block = roundup32(ncgb * s*s * ceil(U/UR)).  gbar (plane layout)
-// overwrites the ray buffer; only the N x N interior of each plane is meaningful afterwards.
-template <class T, int UR, int U, int NT_MAX>
-__global__ void __launch_bounds__(NT_MAX) gl_conv_bwd_sw(const __grid_constant__ Geom G, int ncgb,
-                                                         const T* __restrict__ gpix, const T* __restrict__ sys_kt,
-                                                         const int32_t* __restrict__ system_id, int64_t p_base,
-                                                         T* __restrict__ gbar) {
-    constexpr int NRG = (U + UR - 1) / UR;
-    constexpr int NVAL = RowSeg<T, U>::NVAL;
-    extern __shared__ __align__(16) unsigned char conv_smem[];     // part [2][NVP][CONV_R][NQ] (only if NRG > 1)
-    T* part = reinterpret_cast<T*>(conv_smem);
-    const int s = G.s, N = G.N, NPH = s * s, NVP = NPH * NRG, NQ = 4 * ncgb;
-    const int p = blockIdx.y, band = blockIdx.x, t = threadIdx.x;
-    const bool active = t < ncgb * NVP;
-    const int g = active ? t % ncgb : 0, vp = active ? t / ncgb : 0;
-    const int rho = vp % NRG, ph = vp / NRG, a = ph / s, b = ph - a * s, oa = phase_shift(G, a);
-    const int sys = system_id ? system_id[p_base + p] : 0;
-    T Tp[UR][U];
+// Transpose of step D.  grid = (ceil(Pc / ppc)); block = ppc * tpp (sp is the BACKWARD SlidePlan: ncg covers the
+// N + max plane shift output columns).  For plane (a,b), rows R in [oa, oa + N):
+//   gbar_ab[R][j'] = sum_{k,l<U} F[k][l] gp[R + k][j' + l],  F[k][l] = kt[(a+c)%s][(b+c)%s][U-1-k][U-1-l]
+// gbar (plane layout) overwrites the ray buffer; only the N x N interior of each plane is meaningful afterwards.
+template <class T, int U, int CW, int NT_MAX>
+__global__ void __launch_bounds__(NT_MAX) gl_conv_bwd_is(const __grid_constant__ Geom G, const SlidePlan sp, int64_t Pc,
+                                                      const T* __restrict__ gpix, const T* __restrict__ sys_kt,
+                                                      const int32_t* __restrict__ system_id, int64_t p_base,
+                                                      T* __restrict__ gbar) {
+    using V2 = typename Vec2<T>::type;
+    constexpr int SEG = (CW + U - 1 + 1) & ~1, UP2 = (U + 1) & ~1;
+    extern __shared__ __align__(16) unsigned char conv_smem[];
+    T* taps = reinterpret_cast<T*>(conv_smem);                   // [ppc][s*s][ps], flipped
+    const int s = G.s, N = G.N, NPH = s * s;
+    const int slot = threadIdx.x / sp.tpp, lt = threadIdx.x - slot * sp.tpp;
+    const int64_t p = (int64_t)blockIdx.x * sp.ppc + slot;
+    const bool live = p < Pc;
+    const int sys = (live && system_id) ? system_id[p_base + p] : 0;
     {
-        const T* kph = sys_kt + (size_t)sys * s * s * U * U + (size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U;
-#pragma unroll
-        for (int k = 0; k < UR; ++k) {
-            const int u1 = rho * UR + k;
-#pragma unroll
-            for (int l = 0; l < U; ++l) Tp[k][l] = (u1 < U) ? __ldg(kph + (U - 1 - u1) * U + (U - 1 - l)) : T(0);
+        T* tp = taps + (size_t)slot * NPH * sp.ps;
+        const T* kt = sys_kt + (size_t)sys * NPH * U * U;
+        for (int e = lt; e < NPH * U * UP2; e += sp.tpp) {
+            const int v = e % UP2, u = (e / UP2) % U, ph = e / (UP2 * U);
+            const int a = ph / s, b = ph - a * s;
+            tp[(size_t)ph * sp.ps + u * UP2 + v] =
+                (v < U) ? kt[(size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U + (U - 1 - u) * U + (U - 1 - v)] : T(0);
         }
     }
-    const int gcol = band * ncgb + g;
-    const bool in_range = active && 4 * gcol + 3 < G.Wp && 4 * gcol + RowSeg<T, U>::WL <= G.Wg;
-    const int gg = min(gcol, (G.Wg - RowSeg<T, U>::WL) / 4);
-    const size_t Wg = (size_t)G.Wg, Wp = (size_t)G.Wp;
-    const T* in = gpix + (size_t)p * gpix_stride(G) + (size_t)(oa + rho * UR) * Wg + 4 * gg;
-    T* out = gbar + (size_t)p * ray_stride(G) + ((size_t)ph * G.Hp + oa) * Wp + 4 * gcol;
-    T w[UR][NVAL];
+    __syncthreads();
+    const int g = lt >> 2, pq = lt & 3;
+    if (!(live && g < sp.ncg)) return;
+    const int nj = NPH >> 2;
+    const T* tp = taps + (size_t)slot * NPH * sp.ps;
+    const T* gp = gpix + (size_t)p * gpix_stride(G) + (size_t)CW * g;
+    const int rows = N + U - 1;
+    for (int j = 0; j < nj; ++j) {
+        const int ph = pq + 4 * j, a = ph / s, oa = phase_shift(G, a);
+        T* out = gbar + (size_t)p * ray_stride(G) + ((size_t)ph * G.Hp) * G.Wp + (size_t)CW * g;
+        const T* in = gp + (size_t)oa * G.Wg;
+        T acc[U][CW];
 #pragma unroll
-    for (int k = 0; k < UR; ++k) RowSeg<T, U>::load(w[k], in + k * Wg);
-    int buf = 0;
-    for (int n0 = 0; n0 < N; n0 += UR) {
+        for (int u = 0; u < U; ++u)
 #pragma unroll
-        for (int j = 0; j < UR; ++j) {
-            const int n = n0 + j;
-            if (n < N) {
-                T acc[4] = {T(0), T(0), T(0), T(0)};
-                fma_row<T, U, NVAL>(acc, Tp[0], w[j % UR]);
-                if (n + 1 < N) RowSeg<T, U>::load(w[j % UR], in + (size_t)(n + UR) * Wg);
+            for (int q = 0; q < CW; ++q) acc[u][q] = T(0);
+        T cur[SEG], nxt[SEG];
+        load_seg<T, SEG>(nxt, in);
+        for (int r = 0; r < rows; ++r) {
 #pragma unroll
-                for (int k = 1; k < UR; ++k) fma_row<T, U, NVAL>(acc, Tp[k], w[(j + k) % UR]);
-                if constexpr (NRG == 1) {
-                    if (in_range) store4(out + (size_t)n * Wp, acc);
-                } else {
-                    if (active) store4(&part[((size_t)(buf * NVP + vp) * CONV_R + (n & (CONV_R - 1))) * NQ + 4 * g], acc);
-                    if ((n & (CONV_R - 1)) == CONV_R - 1 || n == N - 1) {
-                        __syncthreads();
-                        const int rows = (n & (CONV_R - 1)) + 1, r0 = n - rows + 1;
-                        for (int o = t; o < rows * NPH * NQ; o += blockDim.x) {
-                            const int q = o % NQ, r = (o / NQ) % rows, ph2 = o / (NQ * rows);
-                            T m = T(0);
+            for (int v = 0; v < SEG; ++v) cur[v] = nxt[v];
+            if (r + 1 < rows) load_seg<T, SEG>(nxt, in + (size_t)(r + 1) * G.Wg);
+            conv_slide<T, U, CW, SEG>(acc, tp + (size_t)ph * sp.ps, cur);
+            const int n = r - (U - 1);                           // finished output row (relative to oa)
+            if (n >= 0) {
+                T* o = out + (size_t)(oa + n) * G.Wp;
 #pragma unroll
-                            for (int v = 0; v < NRG; ++v) m += part[((size_t)(buf * NVP + ph2 * NRG + v) * CONV_R + r) * NQ + q];
-                            const int col = band * NQ + q;
-                            if (col < G.Wp)
-                                gbar[(size_t)p * ray_stride(G) + ((size_t)ph2 * G.Hp + phase_shift(G, ph2 / s) + r0 + r) * Wp + col] = m;
-                        }
-                        buf ^= 1;
-                    }
-                }
+                for (int q = 0; q < CW; q += 2) { V2 v; v.x = acc[U - 1][q]; v.y = acc[U - 1][q + 1]; *reinterpret_cast<V2*>(o + q) = v; }
             }
+#pragma unroll
+            for (int u = U - 1; u > 0; --u)
+#pragma unroll
+                for (int q = 0; q < CW; ++q) acc[u][q] = acc[u - 1][q];
+#pragma unroll
+            for (int q = 0; q < CW; ++q) acc[0][q] = T(0);
         }
     }
 }
