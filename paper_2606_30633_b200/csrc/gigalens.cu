@@ -77,6 +77,10 @@ extern "C" int32_t gl_stage_times(float* ms_host, int32_t* launches_host, int32_
 
 static constexpr int NT_FWD = 256;     // compiled launch bounds; the block size actually used is chosen per config
 static constexpr int NT_ADJ = 128;
+#ifndef GL_RB_FWD
+#define GL_RB_FWD 1
+#endif
+static constexpr int RB_FWD = GL_RB_FWD;  // rays a forward thread evaluates concurrently
 static constexpr size_t WS_BUDGET = (size_t)4096 << 20;   // chunk so that per-chunk buffers stay below ~4 GiB
 
 static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -231,7 +235,7 @@ extern "C" size_t gl_workspace_bytes(const gl_config* c, int64_t n_particles) {
 template <class T, class V>
 static void launch_ray_fwd(const gl_config* c, const T* pb, const double* tab, T* ray, int64_t Pc, cudaStream_t st) {
     dim3 grid(c->G.s * c->G.s * c->n_chunk_fwd, (unsigned)Pc);
-    gl_ray_fwd_kernel<T, V, NT_FWD><<<grid, c->nt_fwd, 0, st>>>(c->G, pb, tab, ray, c->rpt_fwd, c->n_chunk_fwd);
+    gl_ray_fwd_kernel<T, V, NT_FWD, RB_FWD><<<grid, c->nt_fwd, 0, st>>>(c->G, pb, tab, ray, c->rpt_fwd, c->n_chunk_fwd);
 }
 template <class T, class V>
 static void launch_ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, int64_t Pc, cudaStream_t st) {

@@ -323,7 +323,7 @@ template <> struct TabStage<double> {
 };
 
 // Steps B + C.  Writes the plane interior and zeroes this CTA's share of the plane border.
-template <class T, class V, int NT>
+template <class T, class V, int NT, int RB>
 __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
                                                         const double* __restrict__ tabg, T* __restrict__ ray, int RPT,
                                                         int n_chunk) {
@@ -345,14 +345,21 @@ __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ 
     }
     const int NN = G.N * G.N;
     const bool valid = pb[PB_VALID] != T(0.);
-#pragma unroll 2
-    for (int r = 0; r < RPT; ++r) {
-        if (it.idx < NN) {
-            int off = 0; asm volatile("" : "+r"(off));      // opaque: keeps the PB scalars in shared memory, not in registers
-            T v = ray_eval<T, V, false>(tb, pb + off, it.fj<T>(G), it.fi<T>(G), T(0.), nullptr);
-            out[it.offset(G)] = valid ? v : T(0.);
+    // RB rays per step, evaluated unconditionally in one basic block so that the scheduler interleaves their
+    // dependency chains (the FP64 pipe needs ~4 independent DFMAs in flight per warp); only the store is predicated.
+    for (int r = 0; r < RPT; r += RB) {
+        int off = 0; asm volatile("" : "+r"(off));      // opaque: keeps the PB scalars in shared memory, not in registers
+        T v[RB]; size_t o[RB]; bool ok[RB];
+#pragma unroll
+        for (int b = 0; b < RB; ++b) {
+            ok[b] = it.idx < NN && r + b < RPT;
+            o[b] = it.offset(G);
+            v[b] = ray_eval<T, V, false>(tb, pb + off, it.fj<T>(G), it.fi<T>(G), T(0.), nullptr);
+            it.next(G);
         }
-        it.next(G);
+#pragma unroll
+        for (int b = 0; b < RB; ++b)
+            if (ok[b]) out[o[b]] = valid ? v[b] : T(0.);
     }
 }
 
