@@ -31,8 +31,9 @@ WORKLOAD_NAMES = {1: "cfg1 tiny SIE 40x40 s2 K11 P64", 2: "cfg2 DESI-Legacy-like
                   3: "cfg3 HST-like EPL+shear+shapelets(6) 100x100 s2 K31 P8192",
                   4: "cfg4 100-system ensemble 60x60 s4 K21 P102400", 5: "cfg5 EPL+multipoles+shapelets(10) 200x200 s4 K41 P2048"}
 
-# FP32 peak of one B200 from unit counts and clocks: 148 SMs x 128 FP32 lanes x sm_max_mhz.
-N_SM, FP32_LANES = 148, 128
+# ALU peaks of one B200 from unit counts and clocks: 148 SMs x 128 FP32 lanes (64 FP64 lanes)
+# x sm_max_mhz; an FMA counts as ONE lane-operation.
+N_SM, FP32_LANES, FP64_LANES = 148, 128, 64
 
 
 def _peaks():
@@ -273,15 +274,25 @@ def run_ours(a):
         return
 
     mhz_max, peak_src = _peaks()
-    peak = N_SM * FP32_LANES * mhz_max * 1e6 / 1e12                   # T lane-op/s
-    wm = workmodel.per_eval(sp)
+    lanes = FP64_LANES if a.precision == "f64" else FP32_LANES
+    pipe = "FP64" if a.precision == "f64" else "FP32"
+    peak = N_SM * lanes * mhz_max * 1e6 / 1e12                        # T lane-op/s
+    wm = workmodel.per_eval(sp, a.precision)
+    probe = {}
+    for kind, name in ((0, "fp32_fma"), (1, "fp64_fma"), (2, "mufu_ex2")):
+        try:
+            probe[name] = round(gl.gl_probe_pipe(kind, 1024)[0], 3)
+        except Exception as e:                                        # measurement utility only
+            probe[name] = None
     dom = max(stage_ms, key=stage_ms.get)
     dom_ops = wm.get(dom, 0) * P
     dom_t = stage_ms[dom] * 1e-3
     achieved = dom_ops / dom_t / 1e12 if dom_t > 0 else 0.0
     clocks = sampler.summary()
-    roof = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "T FP32 lane-op/s (FMA=1)",
-            "frac": achieved / peak, "traffic": None, "peak_source": "148 SM x 128 lanes x %g MHz (%s)" % (mhz_max, peak_src),
+    roof = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "T %s lane-op/s (FMA=1)" % pipe,
+            "frac": achieved / peak, "traffic": None,
+            "peak_source": "148 SM x %d %s lanes x %g MHz (%s)" % (lanes, pipe, mhz_max, peak_src),
+            "probe_T_laneops_per_s": probe,
             "kernel_ms_per_launch": stage_ms[dom] / max(stage_n[dom], 1), "kernel_launches_per_step": stage_n[dom],
             "algorithmic_laneops_per_eval": wm.get(dom, 0),
             "stage_ms": {s: round(v, 4) for s, v in stage_ms.items()},
@@ -289,7 +300,7 @@ def run_ours(a):
             "step_frac": wm["total_fwd_grad"] * P * a.steps / t_dev / 1e12 / peak,
             "step_algorithmic_laneops_per_eval": wm["total_fwd_grad"]}
     if clocks.get("sm_mhz"):
-        roof["frac_at_measured_clock"] = achieved / (N_SM * FP32_LANES * clocks["sm_mhz"] * 1e6 / 1e12)
+        roof["frac_at_measured_clock"] = achieved / (N_SM * lanes * clocks["sm_mhz"] * 1e6 / 1e12)
     out = {"metric": METRIC, "value": world * P * a.steps / t_dev, "unit": UNIT, "n_gpus": world, "steps": a.steps,
            "warmup": max(a.warmup, 3), "ms_per_step": t_dev / a.steps * 1e3, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": a.precision, "data": "synthetic",

@@ -33,6 +33,32 @@ ADJ = {
 }
 
 
+# GL_PRECISION_F64: the same formulation on the FP64 pipe.  Counts are FP64 lane-operations (DFMA, DMUL and DADD
+# count 1 each; compares, selects, integer and FP32/MUFU seed instructions count 0).  exp2 = 8 (split 3, degree-4
+# polynomial 3, table product 2), log2 = 7, rsqrt = 4, rcp = 2 (csrc/gl_math.cuh).  Hand counts of csrc/gl_ray.cuh,
+# cross-checked against the SASS loop bodies of the config-2 kernels (195 forward, 438 adjoint FP64 instructions).
+FWD64 = {
+    "frame":          (22, 0),    # 18 arithmetic + rsqrt 4
+    "epl_series":     (63, 0),
+    "epl_amp":        (22, 0),    # log2 7 + exp2 8 + 7
+    "sie_closed":     (120, 0),   # libdevice atan + atanh (config 1 only; latency-bound, not rooflined)
+    "rotate_shear":   (12, 0),
+    "multipoles":     (34, 0),
+    "sersic":         (38, 0),    # 15 arithmetic + log2 7 + 2 exp2 16
+    "shapelet_fixed": (22, 0),    # u, v, two Gaussians through exp2
+    "sum":            (0, 0),     # folded into the component counts
+}
+ADJ64 = {
+    "epl_series":     (130, 0),
+    "mass_chain":     (75, 0),    # includes rcp 2
+    "sie_chain":      (45, 0),
+    "multipoles":     (40, 0),
+    "sersic":         (17, 0),    # 8 natural sums + radial factor + rcp
+    "sersic_src_grad": (8, 0),
+    "shapelet_fixed": (20, 0),
+}
+
+
 def shapelet_fwd(nmax):
     ncoef = (nmax + 1) * (nmax + 2) // 2
     return 4 * nmax + ncoef + (nmax + 1)          # two recurrences (2 ops/step each) + triangular contraction
@@ -43,16 +69,18 @@ def shapelet_adj(nmax):
     return 4 * (nmax + 1) + 2 * ncoef + 2 * (nmax + 1) + ncoef     # derivatives, d/du d/dv contractions, coefficient sums
 
 
-def per_ray(spec):
-    """(fwd lane-ops, fwd mufu, adjoint-sweep lane-ops, adjoint-sweep mufu) per ray for a LensSpec-like object."""
+def per_ray(spec, precision="f32"):
+    """(fwd lane-ops, fwd mufu, adjoint-sweep lane-ops, adjoint-sweep mufu) per ray for a LensSpec-like object;
+    precision "f32": FP32 lane-ops + MUFU, "f64": FP64 lane-ops (mufu = 0)."""
     f = m = a = am = 0
+    F_, A_ = (FWD64, ADJ64) if precision == "f64" else (FWD, ADJ)
 
     def add(tab, key, times=1):
         nonlocal f, m, a, am
         if tab is FWD:
-            f += tab[key][0] * times; m += tab[key][1] * times
+            f += F_[key][0] * times; m += F_[key][1] * times
         else:
-            a += tab[key][0] * times; am += tab[key][1] * times
+            a += A_[key][0] * times; am += A_[key][1] * times
 
     add(FWD, "frame"); add(FWD, "rotate_shear"); add(FWD, "sum")
     if spec.mass_model == 1:
@@ -71,11 +99,11 @@ def per_ray(spec):
     return f, m, a, am
 
 
-def per_eval(spec):
-    """Algorithmic FP32 lane-ops of one particle evaluation, by stage, for gl_logpost_grad."""
+def per_eval(spec, precision="f32"):
+    """Algorithmic lane-ops (FP32 or FP64, by `precision`) of one particle evaluation, by stage, for gl_logpost_grad."""
     M = spec.n_pix * spec.supersample
     rays = M * M
-    f, m, a, am = per_ray(spec)
+    f, m, a, am = per_ray(spec, precision)
     ke = spec.psf_size + spec.supersample - 1
     conv = spec.n_pix * spec.n_pix * ke * ke              # stride-s correlation with the pre-boxed kernel (step D)
     return {
