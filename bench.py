@@ -170,6 +170,23 @@ def run_reference(a):
         "gpu_launches": 0}))
 
 
+# ----------------------------------------------------------------------------------------------- multi-rank host logic
+def max_over_ranks(values, device="cpu"):
+    """Max over ranks of each entry of `values` (device seconds).  Replicas exchange nothing else (DESIGN.md section 9);
+    works on any initialised backend (nccl on the box, gloo in tests/test_bench_host.py)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.cpu()]
+
+
+def whole_job_rate(world, particles_per_rank, steps, seconds):
+    """Replicas: every rank evaluates its own full batch, so the job processed world * P * steps evaluations."""
+    return world * particles_per_rank * steps / seconds
+
+
 # ----------------------------------------------------------------------------------------------- GPU arm
 def run_ours(a):
     import torch
@@ -264,10 +281,7 @@ def run_ours(a):
             stage_n[name] = cnt
     gl.gl_stage_timing_enable(False)
 
-    if world > 1:
-        t = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_dev, t_e2e = float(t[0]), float(t[1])
+    t_dev, t_e2e = max_over_ranks([t_dev, t_e2e], dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -301,14 +315,14 @@ def run_ours(a):
             "step_algorithmic_laneops_per_eval": wm["total_fwd_grad"]}
     if clocks.get("sm_mhz"):
         roof["frac_at_measured_clock"] = achieved / (N_SM * lanes * clocks["sm_mhz"] * 1e6 / 1e12)
-    out = {"metric": METRIC, "value": world * P * a.steps / t_dev, "unit": UNIT, "n_gpus": world, "steps": a.steps,
+    out = {"metric": METRIC, "value": whole_job_rate(world, P, a.steps, t_dev), "unit": UNIT, "n_gpus": world, "steps": a.steps,
            "warmup": max(a.warmup, 3), "ms_per_step": t_dev / a.steps * 1e3, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": a.precision, "data": "synthetic",
            "config": {"workload": WORKLOAD_NAMES[k], "n_particles_per_gpu": P, "n_params": n_p,
                       "rays_per_particle": wm["rays"], "parallelism": "replicas x%d" % world,
                       "l2": "256 MiB flush write between timed iterations; workspace %.0f MB" % (ws_bytes / 1e6),
                       "finite_fraction": finite},
-           "e2e": {"value": world * P * a.steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(zh.numel() * 4),
+           "e2e": {"value": whole_job_rate(world, P, a.steps, t_e2e), "unit": UNIT, "h2d_bytes_per_step": int(zh.numel() * 4),
                    "d2h_bytes_per_step": int((lph.numel() + gh.numel()) * 4), "ms_per_step": t_e2e / a.steps * 1e3},
            "gpu_launches": launches_per_step * a.steps, "clocks": clocks, "roofline": roof}
     if not a.no_cpu_baseline:

@@ -1,0 +1,111 @@
+"""Host side of the C ABI without a GPU: libgigalens.so loads, exports every symbol include/gigalens.h declares,
+and validates its arguments before any CUDA call (include/gigalens.h "Errors").  No compute call is made here."""
+import ctypes as C
+import dataclasses
+import os
+import re
+
+import pytest
+
+import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def gl():
+    import __graft_entry__ as ge
+    from paper_2606_30633_b200 import build as gl_build
+    gl_build.build()
+    import paper_2606_30633_b200 as gl
+    gl.lib()
+    return gl
+
+
+def test_every_declared_symbol_is_exported(gl):
+    hdr = open(os.path.join(ROOT, "include", "gigalens.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(gl_[a-z0-9_]+)\s*\(", hdr))
+    assert len(declared) >= 17
+    L = gl.lib()
+    for name in sorted(declared):
+        assert getattr(L, name) is not None, name
+    assert declared == set(gl.EXPORTS), declared ^ set(gl.EXPORTS)
+    assert L.gl_version().decode().count(".") == 1
+
+
+@pytest.mark.parametrize("k, n_params", [(1, 21), (2, 22), (3, 58), (4, 22), (5, 100)])
+def test_config_create_and_param_count(gl, k, n_params):
+    sp = W.make_spec(k)
+    for prec in (0, 1):
+        h = gl.gl_config_create(dataclasses.replace(sp, precision=prec))
+        assert gl.lib().gl_config_n_params(h) == n_params == sp.n_params
+        w1, w2 = gl.gl_workspace_bytes(h, 1), gl.gl_workspace_bytes(h, 64)
+        assert 0 < w1 < w2 and gl.gl_workspace_bytes(h, 0) == 0
+        assert gl.gl_workspace_bytes(h, 10 ** 7) == gl.gl_workspace_bytes(h, 10 ** 8)     # flat beyond the chunk size
+        assert gl.gl_workspace_bytes_host(h, 64) > w2
+        gl.gl_config_destroy(h)
+    h64 = gl.gl_config_create(dataclasses.replace(sp, precision=0))
+    h32 = gl.gl_config_create(dataclasses.replace(sp, precision=1))
+    assert gl.gl_workspace_bytes(h64, 16) > gl.gl_workspace_bytes(h32, 16)
+    gl.gl_config_destroy(h64); gl.gl_config_destroy(h32)
+
+
+@pytest.mark.parametrize("field, value, status", [
+    ("psf_size", 10, -2), ("supersample", 0, -2), ("n_pix", 0, -2), ("pix_scale", 0.0, -2), ("mass_model", 2, -2),
+    ("epl_terms", 31, -2), ("epl_terms", 1, -2), ("n_lens_sersic", 3, -2), ("shapelet_nmax", 11, -2),
+    ("n_systems", 0, -2), ("precision", 2, -2), ("param_space", 2, -2), ("multipole_mask", 4, -2),
+    ("psf_grid", 1, -4), ("n_pix", 5000, -4)])
+def test_config_validation(gl, field, value, status):
+    sp = W.make_spec(2)
+    if field == "psf_grid":
+        sp = dataclasses.replace(sp); sp.psf_grid = value
+    else:
+        sp = dataclasses.replace(sp, **{field: value})
+    with pytest.raises(gl.GLError) as e:
+        gl.gl_config_create(sp)
+    assert e.value.status == status
+
+
+def test_param_count_mismatch_and_bad_priors(gl):
+    sp = W.make_spec(2)
+    bad = dataclasses.replace(sp, priors=sp.priors[:-1])
+    with pytest.raises(gl.GLError) as e:
+        gl.gl_config_create(bad)
+    assert e.value.status == -2
+    pri = list(sp.priors); pri[0] = (W.PRIOR_UNIFORM, 0.0, 1.0, 2.0, 1.0)            # hi < lo
+    with pytest.raises(gl.GLError):
+        gl.gl_config_create(dataclasses.replace(sp, priors=pri))
+    pri[0] = (W.PRIOR_NORMAL, 0.0, 0.0, 0.0, 0.0)                                     # sigma = 0
+    with pytest.raises(gl.GLError):
+        gl.gl_config_create(dataclasses.replace(sp, priors=pri))
+    pri[0] = (W.PRIOR_LOGUNIFORM, 0.0, 1.0, 0.0, 1.0)                                 # lo = 0
+    with pytest.raises(gl.GLError):
+        gl.gl_config_create(dataclasses.replace(sp, priors=pri))
+
+
+def test_argument_checks_precede_any_cuda_call(gl):
+    """NULL handle, negative and zero particle counts are answered on the host (this box has no GPU)."""
+    L = gl.lib()
+    h = gl.gl_config_create(W.make_spec(1))
+    null = C.c_void_p(0)
+    assert L.gl_logpost(null, null, null, null, null, null, 4, null, null, 0, null) == -1
+    assert L.gl_logpost(h, null, null, null, null, null, -1, null, null, 0, null) == -3
+    assert L.gl_logpost(h, null, null, null, null, null, 0, null, null, 0, null) == 0
+    assert L.gl_last_launch_count() == 0
+    assert L.gl_logpost_grad(h, null, null, null, null, null, 4, null, null, null, 0, null) == -1     # NULL arrays
+    assert L.gl_model_image(h, null, null, null, 0, null, null, 0, null) == 0
+    assert L.gl_logpost_grad_host(h, null, null, null, null, null, 0, null, null, null, 0, null) == 0
+    assert L.gl_workspace_bytes(null, 8) == 0 and L.gl_config_n_params(null) == 0
+    for s in range(0, -7, -1):
+        assert L.gl_status_string(s).decode().startswith("GL_")
+    assert L.gl_stage_count() == 7 and L.gl_stage_name(2).decode() == "ray_fwd"
+    gl.gl_config_destroy(h)
+
+
+def test_binding_refuses_to_compute_without_cuda(gl):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA present")
+    with pytest.raises(RuntimeError):
+        gl.LensModel(W.make_spec(1), None, None, None)
