@@ -295,7 +295,7 @@ def run_ours(a):
     probe = {}
     for kind, name in ((0, "fp32_fma"), (1, "fp64_fma"), (2, "mufu_ex2")):
         try:
-            probe[name] = round(gl.gl_probe_pipe(kind, 1024)[0], 3)
+            probe[name] = round(gl.gl_probe_pipe(kind, 256)[0], 3)
         except Exception as e:                                        # measurement utility only
             probe[name] = None
     dom = max(stage_ms, key=stage_ms.get)
