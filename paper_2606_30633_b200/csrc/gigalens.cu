@@ -80,6 +80,12 @@ static constexpr int NT_ADJ = 128;
 #ifndef GL_RB_FWD
 #define GL_RB_FWD 1
 #endif
+#ifndef GL_RPT_FWD
+#define GL_RPT_FWD 40
+#endif
+#ifndef GL_RPT_ADJ
+#define GL_RPT_ADJ 64
+#endif
 static constexpr int RB_FWD = GL_RB_FWD;  // rays a forward thread evaluates concurrently
 static constexpr size_t WS_BUDGET = (size_t)4096 << 20;   // chunk so that per-chunk buffers stay below ~4 GiB
 
@@ -170,7 +176,7 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     G.delta2 = (double)d->pix_scale * (double)d->pix_scale;
     (void)M64;
     c->esize = d->precision == GL_PRECISION_F64 ? 8 : 4;
-    c->conv = conv_plan(G, c->esize);       // also fills the padded-layout fields of G
+    c->conv = conv_plan(G, c->esize, d->n_systems);       // also fills the padded-layout fields of G
     c->n_ctile = c->conv.n_ctile;
     // ray kernels: one CTA per (particle, phase plane, chunk); pick the block size that wastes the fewest lanes
     const int NN = G.N * G.N;
@@ -186,8 +192,8 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
         n_chunk = (iters + rpt_target - 1) / rpt_target;
         rpt = (iters + n_chunk - 1) / n_chunk;
     };
-    pick(NT_FWD, 10, c->nt_fwd, c->rpt_fwd, c->n_chunk_fwd);
-    pick(NT_ADJ, 32, c->nt_adj, c->rpt_adj, c->n_chunk_adj);
+    pick(NT_FWD, GL_RPT_FWD, c->nt_fwd, c->rpt_fwd, c->n_chunk_fwd);
+    pick(NT_ADJ, GL_RPT_ADJ, c->nt_adj, c->rpt_adj, c->n_chunk_adj);
     c->n_nap = G.s * G.s * c->n_chunk_adj;
     c->per_particle_bytes = (size_t)c->esize * ((size_t)PB_STRIDE + ray_stride(G) + gpix_stride(G) + (size_t)c->n_ctile +
                                                 (size_t)c->n_nap * c->na) + sizeof(double) + 6 * 256;
@@ -240,7 +246,9 @@ static void launch_ray_fwd(const gl_config* c, const T* pb, const double* tab, T
 template <class T, class V>
 static void launch_ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, int64_t Pc, cudaStream_t st) {
     dim3 grid(c->n_nap, (unsigned)Pc);
-    gl_ray_adj_kernel<T, V, NT_ADJ><<<grid, c->nt_adj, 0, st>>>(c->G, pb, tab, gbar, nap, c->rpt_adj, c->n_chunk_adj);
+    const size_t smem = coef_in_smem<T, V>() ? sizeof(T) * (size_t)V::NCOEF * c->nt_adj : 0;   // coefficient sums, one column per thread
+    if (smem > 40 * 1024) cudaFuncSetAttribute(gl_ray_adj_kernel<T, V, NT_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    gl_ray_adj_kernel<T, V, NT_ADJ><<<grid, c->nt_adj, smem, st>>>(c->G, pb, tab, gbar, nap, c->rpt_adj, c->n_chunk_adj);
 }
 
 using V_S0 = Variant<0, 0, 1, -1, 1>; using V_E0 = Variant<1, 0, 1, -1, 1>;

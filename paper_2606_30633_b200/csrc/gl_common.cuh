@@ -35,7 +35,8 @@ enum : int {
     PB_SER_A = 144,                     // a_n, n = 0..31 (zero beyond epl_terms)
     PB_SER_D = 176,                     // d_m = (m+1) a_{m+1}
     PB_SER_E = 208,                     // e_m = L_{m+1} a_{m+1}
-    PB_STRIDE = 240
+    PB_SER_M1 = 240, PB_SER_M2 = 241,   // series bands: 4*M1 steps in T, 4*M2 steps in fp32 above them, the rest skipped
+    PB_STRIDE = 244
 };
 // Sersic block offsets
 enum : int { SB_XOFF = 0, SB_YOFF = 1, SB_C = 2, SB_S = 3, SB_Q = 4, SB_QI = 5, SB_K1 = 6, SB_K0 = 7,

@@ -160,9 +160,10 @@ template <> struct Vec2<double> { using type = double2; };
 // Launch-invariant description of the sliding kernels (filled by conv_plan).
 struct SlidePlan {
     int ncg;      // column groups per particle
-    int tpp;      // threads per particle slot (multiple of 32) = roundup32(4 * ncg)
+    int tpp;      // threads per particle slot = ncg (one thread per column group, all phase planes)
     int ppc;      // particle slots per CTA
     int ps;       // tap stride between phases in shared memory (elements)
+    int shared_taps;  // 1: one system -> one tap copy per CTA (uniform addresses); 0: one copy per slot
 };
 
 // acc[u][q] += sum_v tap[u][v] * seg[q + v] for one input row segment.  tap: shared memory, row pitch UP2 (even).
@@ -194,44 +195,51 @@ __device__ __forceinline__ void load_seg(T (&seg)[SEG], const T* __restrict__ p)
     }
 }
 
-// Step D + E.  grid = (ceil(Pc / ppc)); block = ppc * tpp.  Dynamic smem: ppc * s*s * ps taps.
-// Lane lt of a particle slot: column group g = lt / 4, plane subset pq = lt % 4 (planes pq, pq + 4, ...).
-template <class T, int U, int CW, int NT_MAX>
+// Step D + E.  grid = (ceil(Pc / ppc)); block = roundup32(ppc * tpp).  Dynamic smem: tap copies [n_copy][s*s][ps].
+// Thread lt of a particle slot owns column group g = lt and walks through ALL s*s planes of every input row, so the
+// tap address is uniform across a slot (a pure shared-memory broadcast: splitting the planes between lanes made the
+// U = 16 kernels shared-memory bound) and an output row is complete inside one thread (no cross-lane reduction).
+template <class T, int U, int CW, int LS, int NT_MAX>
 __global__ void __launch_bounds__(NT_MAX) gl_conv_fwd_is(const __grid_constant__ Geom G, const SlidePlan sp, int64_t Pc,
-                                                      const T* __restrict__ ray, const T* __restrict__ sys_kt,
-                                                      const T* __restrict__ sys_w, const float* __restrict__ obs,
-                                                      const int32_t* __restrict__ system_id, int64_t p_base,
-                                                      T* __restrict__ gpix, T* __restrict__ chi, float* __restrict__ out_model) {
+                                                         const T* __restrict__ ray, const T* __restrict__ sys_kt,
+                                                         const T* __restrict__ sys_w, const float* __restrict__ obs,
+                                                         const int32_t* __restrict__ system_id, int64_t p_base,
+                                                         T* __restrict__ gpix, T* __restrict__ chi, float* __restrict__ out_model) {
     constexpr int SEG = (CW + U - 1 + 1) & ~1, UP2 = (U + 1) & ~1;
     extern __shared__ __align__(16) unsigned char conv_smem[];
-    T* taps = reinterpret_cast<T*>(conv_smem);                   // [ppc][s*s][ps]
-    __shared__ T red[16];
+    T* taps = reinterpret_cast<T*>(conv_smem);                   // [n_copy][s*s][ps]
+    __shared__ T red[NT_MAX];
     const int s = G.s, N = G.N, NPH = s * s;
     const int slot = threadIdx.x / sp.tpp, lt = threadIdx.x - slot * sp.tpp;
     const int64_t p = (int64_t)blockIdx.x * sp.ppc + slot;
-    const bool live = p < Pc;
+    const bool live = slot < sp.ppc && p < Pc;
     const int sys = (live && system_id) ? system_id[p_base + p] : 0;
-    // stage this slot's taps in PLANE order: plane (a,b) uses kt[(a+c)%s][(b+c)%s]
+    // stage the taps in PLANE order: plane (a,b) uses kt[(a+c)%s][(b+c)%s]
+    const int copy = sp.shared_taps ? 0 : slot;
     {
-        T* tp = taps + (size_t)slot * NPH * sp.ps;
+        const int first = sp.shared_taps ? threadIdx.x : lt, stride = sp.shared_taps ? blockDim.x : sp.tpp;
+        T* tp = taps + (size_t)copy * NPH * sp.ps;
         const T* kt = sys_kt + (size_t)sys * NPH * U * U;
-        for (int e = lt; e < NPH * U * UP2; e += sp.tpp) {
-            const int v = e % UP2, u = (e / UP2) % U, ph = e / (UP2 * U);
-            const int a = ph / s, b = ph - a * s;
-            tp[(size_t)ph * sp.ps + u * UP2 + v] = (v < U) ? kt[(size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U + u * U + v] : T(0);
-        }
+        if (sp.shared_taps || slot < sp.ppc)
+            for (int e = first; e < NPH * U * UP2; e += stride) {
+                const int v = e % UP2, u = (e / UP2) % U, ph = e / (UP2 * U);
+                const int a = ph / s, b = ph - a * s;
+                tp[(size_t)ph * sp.ps + u * UP2 + v] = (v < U) ? kt[(size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U + u * U + v] : T(0);
+            }
     }
     if (live && gpix) zero_gpix_border(G, gpix + (size_t)p * gpix_stride(G), lt, sp.tpp);
     __syncthreads();
-    const int g = lt >> 2, pq = lt & 3;
+    // LS lanes share a column group and split the planes (LS = 4 where a particle has too few column groups to fill
+    // the machine, with a shuffle reduction per output row; LS = 1: one thread walks all planes).
+    const int g = lt / LS, pq = lt - g * LS;
     const bool active = live && g < sp.ncg;
-    const unsigned amask = __ballot_sync(0xffffffffu, active);   // the 4 lanes of a column group are active together
+    const unsigned amask = __ballot_sync(0xffffffffu, active);   // the LS lanes of a column group are active together
     T c2 = T(0);
     if (active) {
-        const int nj = NPH >> 2;                                 // planes per lane
+        const int nj = NPH / LS;                                 // planes per lane
         const size_t plane = (size_t)G.Hp * G.Wp;
         const T* in = ray + (size_t)p * ray_stride(G) + (size_t)CW * g;
-        const T* tp = taps + (size_t)slot * NPH * sp.ps;
+        const T* tp = taps + (size_t)copy * NPH * sp.ps;
         T acc[U][CW];
 #pragma unroll
         for (int u = 0; u < U; ++u)
@@ -244,28 +252,39 @@ __global__ void __launch_bounds__(NT_MAX) gl_conv_fwd_is(const __grid_constant__
         for (int t = 0; t < steps; ++t) {
 #pragma unroll
             for (int v = 0; v < SEG; ++v) cur[v] = nxt[v];
-            const int ph = pq + 4 * j;
             int jn = j + 1, in_ = i;
             if (jn == nj) { jn = 0; in_ = i + 1; }
-            if (t + 1 < steps) load_seg<T, SEG>(nxt, in + (size_t)(pq + 4 * jn) * plane + (size_t)in_ * G.Wp);
-            conv_slide<T, U, CW, SEG>(acc, tp + (size_t)ph * sp.ps, cur);
+            if (t + 1 < steps) load_seg<T, SEG>(nxt, in + (size_t)(pq + LS * jn) * plane + (size_t)in_ * G.Wp);
+            conv_slide<T, U, CW, SEG>(acc, tp + (size_t)(pq + LS * j) * sp.ps, cur);
             if (jn == 0) {                                       // input row i done: output row i - U + 1 is complete
                 const int pr = i - (U - 1);
-                T m[CW];
+                if constexpr (LS == 1) {
+                    if (pr >= 0) {
 #pragma unroll
-                for (int q = 0; q < CW; ++q) {
-                    T v = acc[U - 1][q];
-                    v += __shfl_xor_sync(amask, v, 1);
-                    v += __shfl_xor_sync(amask, v, 2);
-                    m[q] = v;
-                }
-                if (pr >= 0) {
-                    T mine = m[0];
+                        for (int q = 0; q < CW; ++q) {
+                            const int pc = CW * g + q;
+                            if (pc < N)
+                                c2 += pixel_epilogue<T>(G, acc[U - 1][q], pr, pc, sys, (size_t)(p_base + p), (int)p, obs, sys_w, gpix, out_model);
+                        }
+                    }
+                } else {
+                    static_assert(LS == 1 || (LS == 4 && CW <= 4), "lane split: 4 lanes, at most 4 columns");
+                    T m[CW];
 #pragma unroll
-                    for (int q = 1; q < CW; ++q) mine = (pq == q) ? m[q] : mine;
-                    const int pc = CW * g + pq;
-                    if (pq < CW && pc < N)
-                        c2 += pixel_epilogue<T>(G, mine, pr, pc, sys, (size_t)(p_base + p), (int)p, obs, sys_w, gpix, out_model);
+                    for (int q = 0; q < CW; ++q) {
+                        T v = acc[U - 1][q];
+                        v += __shfl_xor_sync(amask, v, 1);
+                        v += __shfl_xor_sync(amask, v, 2);
+                        m[q] = v;
+                    }
+                    if (pr >= 0) {
+                        T mine = m[0];
+#pragma unroll
+                        for (int q = 1; q < CW; ++q) mine = (pq == q) ? m[q] : mine;
+                        const int pc = CW * g + pq;
+                        if (pq < CW && pc < N)
+                            c2 += pixel_epilogue<T>(G, mine, pr, pc, sys, (size_t)(p_base + p), (int)p, obs, sys_w, gpix, out_model);
+                    }
                 }
 #pragma unroll
                 for (int u = U - 1; u > 0; --u)
@@ -277,56 +296,56 @@ __global__ void __launch_bounds__(NT_MAX) gl_conv_fwd_is(const __grid_constant__
             i = in_; j = jn;
         }
     }
-    if (chi) {                                                   // fixed-order sum over the slot's warps
-        const T ws = warp_sum(c2);
-        const int wps = sp.tpp >> 5, wi = lt >> 5;
-        if ((lt & 31) == 0) red[slot * wps + wi] = ws;
+    if (chi) {                                                   // fixed-order sum over the slot's threads
+        red[threadIdx.x] = c2;
         __syncthreads();
         if (lt == 0 && live) {
             T tot = T(0);
-            for (int w = 0; w < wps; ++w) tot += red[slot * wps + w];
+            for (int k = 0; k < sp.tpp; ++k) tot += red[slot * sp.tpp + k];
             chi[p] = tot;
         }
     }
 }
 
-// Transpose of step D.  grid = (ceil(Pc / ppc)); block = ppc * tpp (sp is the BACKWARD SlidePlan: ncg covers the
-// N + max plane shift output columns).  For plane (a,b), rows R in [oa, oa + N):
+// Transpose of step D.  Same mapping (sp is the BACKWARD SlidePlan: ncg covers the N + max plane shift output
+// columns).  For plane (a,b), rows R in [oa, oa + N):
 //   gbar_ab[R][j'] = sum_{k,l<U} F[k][l] gp[R + k][j' + l],  F[k][l] = kt[(a+c)%s][(b+c)%s][U-1-k][U-1-l]
 // gbar (plane layout) overwrites the ray buffer; only the N x N interior of each plane is meaningful afterwards.
-template <class T, int U, int CW, int NT_MAX>
+template <class T, int U, int CW, int LS, int NT_MAX>
 __global__ void __launch_bounds__(NT_MAX) gl_conv_bwd_is(const __grid_constant__ Geom G, const SlidePlan sp, int64_t Pc,
-                                                      const T* __restrict__ gpix, const T* __restrict__ sys_kt,
-                                                      const int32_t* __restrict__ system_id, int64_t p_base,
-                                                      T* __restrict__ gbar) {
+                                                         const T* __restrict__ gpix, const T* __restrict__ sys_kt,
+                                                         const int32_t* __restrict__ system_id, int64_t p_base,
+                                                         T* __restrict__ gbar) {
     using V2 = typename Vec2<T>::type;
     constexpr int SEG = (CW + U - 1 + 1) & ~1, UP2 = (U + 1) & ~1;
     extern __shared__ __align__(16) unsigned char conv_smem[];
-    T* taps = reinterpret_cast<T*>(conv_smem);                   // [ppc][s*s][ps], flipped
+    T* taps = reinterpret_cast<T*>(conv_smem);                   // [n_copy][s*s][ps], flipped
     const int s = G.s, N = G.N, NPH = s * s;
     const int slot = threadIdx.x / sp.tpp, lt = threadIdx.x - slot * sp.tpp;
     const int64_t p = (int64_t)blockIdx.x * sp.ppc + slot;
-    const bool live = p < Pc;
+    const bool live = slot < sp.ppc && p < Pc;
     const int sys = (live && system_id) ? system_id[p_base + p] : 0;
+    const int copy = sp.shared_taps ? 0 : slot;
     {
-        T* tp = taps + (size_t)slot * NPH * sp.ps;
+        const int first = sp.shared_taps ? threadIdx.x : lt, stride = sp.shared_taps ? blockDim.x : sp.tpp;
+        T* tp = taps + (size_t)copy * NPH * sp.ps;
         const T* kt = sys_kt + (size_t)sys * NPH * U * U;
-        for (int e = lt; e < NPH * U * UP2; e += sp.tpp) {
-            const int v = e % UP2, u = (e / UP2) % U, ph = e / (UP2 * U);
-            const int a = ph / s, b = ph - a * s;
-            tp[(size_t)ph * sp.ps + u * UP2 + v] =
-                (v < U) ? kt[(size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U + (U - 1 - u) * U + (U - 1 - v)] : T(0);
-        }
+        if (sp.shared_taps || slot < sp.ppc)
+            for (int e = first; e < NPH * U * UP2; e += stride) {
+                const int v = e % UP2, u = (e / UP2) % U, ph = e / (UP2 * U);
+                const int a = ph / s, b = ph - a * s;
+                tp[(size_t)ph * sp.ps + u * UP2 + v] =
+                    (v < U) ? kt[(size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U + (U - 1 - u) * U + (U - 1 - v)] : T(0);
+            }
     }
     __syncthreads();
-    const int g = lt >> 2, pq = lt & 3;
+    const int g = lt / LS, pq = lt - g * LS;
     if (!(live && g < sp.ncg)) return;
-    const int nj = NPH >> 2;
-    const T* tp = taps + (size_t)slot * NPH * sp.ps;
+    const T* tp = taps + (size_t)copy * NPH * sp.ps;
     const T* gp = gpix + (size_t)p * gpix_stride(G) + (size_t)CW * g;
     const int rows = N + U - 1;
-    for (int j = 0; j < nj; ++j) {
-        const int ph = pq + 4 * j, a = ph / s, oa = phase_shift(G, a);
+    for (int ph = pq; ph < NPH; ph += LS) {
+        const int a = ph / s, oa = phase_shift(G, a);
         T* out = gbar + (size_t)p * ray_stride(G) + ((size_t)ph * G.Hp) * G.Wp + (size_t)CW * g;
         const T* in = gp + (size_t)oa * G.Wg;
         T acc[U][CW];

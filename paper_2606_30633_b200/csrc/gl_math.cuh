@@ -16,13 +16,15 @@ __device__ __forceinline__ float f_rsqrt(float x) { float y; asm("rsqrt.approx.f
 __device__ __forceinline__ float f_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
 // ----------------------------------------------------------------------------- fp64 exp2 / log2
-// exp2(x) = 2^n * 2^(j/64) * P(r),  x = n + j/64 + r, |r| <= 1/128;  P = degree-4 Taylor of 2^r (error < 4e-14).
-// log2(x) = e + log2(c_j) + log1p(r)/ln2,  x = 2^e m, m in [1,2), c_j = 1 + (j+0.5)/128, r = m/c_j - 1,
-//           |r| <= 1/256 (+ rounding of the tabulated 1/c_j); log1p by a degree-5 alternating series (error < 1e-15).
-// Tables are generated on the device in fp64 once per call by gl_prep_kernel (block 0) into the workspace and
-// staged into shared memory by the kernels that use them (they are indexed per LANE): 64 + 2*128 doubles = 2.5 KB.
-constexpr int EXP2_TAB = 64, LOG2_TAB = 128;
-constexpr int MATH_TAB_DOUBLES = EXP2_TAB + 2 * LOG2_TAB;      // [2^(j/64)] [rc_j = fl(1/c_j)] [-log2 rc_j]
+// exp2(x) = 2^n * 2^(j/16) * (1 + r P(r)),  x = n + j/16 + r, |r| <= 1/32;  P = degree-4 (2^r to r^5: error < 1.5e-13).
+// log2(x) = e + log2(c_j) + log1p(r)/ln2,  x = 2^e m, m in [1,2), c_j = 1 + (j+0.5)/16, r = m rc_j - 1, |r| <= 1/32;
+//           log1p through r^7 (absolute error < 1.7e-13).
+// The tables have 16 doubles = 128 bytes = ONE shared-memory bank row each, so a lookup with 32 arbitrary per-lane
+// indices is always a single conflict-free wavefront (larger tables made the ray kernels shared-memory bound:
+// profiles/r1b_cfg2_f64.md).  They are generated on the device in fp64 once per call by gl_prep_kernel (block 0) into
+// the workspace and staged into 128-byte aligned shared memory by the kernels that use them.
+constexpr int EXP2_TAB = 16, LOG2_TAB = 16;
+constexpr int MATH_TAB_DOUBLES = EXP2_TAB + 2 * LOG2_TAB;      // [2^(j/16)] [rc_j = fl(1/c_j)] [-log2 rc_j]
 
 __device__ inline void fill_math_tab(double* g) {               // any block shape
     for (int k = threadIdx.x; k < EXP2_TAB; k += blockDim.x) g[k] = exp2((double)k / EXP2_TAB);
@@ -42,50 +44,57 @@ __device__ __forceinline__ MathTab math_tab(const double* sm) { return MathTab{s
 
 // Polynomial and splitting constants live in __constant__ memory so that DFMA takes them as constant-bank operands
 // (a 64-bit literal costs two extra move instructions per use, and the ray kernels are co-limited by issue slots).
-__constant__ double c_dm[16] = {
+__constant__ double c_dm[20] = {
     6755399441055744.0,        // 0: 1.5 * 2^52: adding it rounds to an integer in the low word
-    64.0,                      // 1
-    -0.015625,                 // 2: -1/64
-    6.9314718055994531e-1,     // 3: ln2
-    2.4022650695910071e-1,     // 4: ln2^2/2
-    5.5504108664821580e-2,     // 5: ln2^3/6
-    9.6181291076284772e-3,     // 6: ln2^4/24
-    1.4426950408889634e+0,     // 7:  1/ln2
-    -7.2134752044448170e-1,    // 8: -1/(2 ln2)
-    4.8089834696298783e-1,     // 9:  1/(3 ln2)
-    -3.6067376022224085e-1,    // 10: -1/(4 ln2)
-    2.8853900817779268e-1,     // 11:  1/(5 ln2)
-    0.5, 1.0, -1.0, 0.0};
+    16.0,                      // 1
+    -0.0625,                   // 2: -1/16
+    6.93147180559945286e-01,   // 3: ln2^1/1!
+    2.40226506959100694e-01,   // 4: ln2^2/2!
+    5.55041086648215762e-02,   // 5: ln2^3/3!
+    9.61812910762847688e-03,   // 6: ln2^4/4!
+    1.33335581464284411e-03,   // 7: ln2^5/5!
+    1.44269504088896339e+00,   // 8:  1/(1 ln2)
+    -7.21347520444481694e-01,   // 9: -1/(2 ln2)
+    4.80898346962987833e-01,   // 10:  1/(3 ln2)
+    -3.60673760222240847e-01,   // 11: -1/(4 ln2)
+    2.88539008177792655e-01,   // 12:  1/(5 ln2)
+    -2.40449173481493916e-01,   // 13: -1/(6 ln2)
+    2.06099291555566222e-01,   // 14:  1/(7 ln2)
+    0.5, 1.0, -1.0, 0.0,       // 15..18
+    0.0};
 
-// 2^x, relative error < 5e-14 (degree-4 Taylor of 2^r on |r| <= 1/128).  x < -1000 returns 0; x must stay below 1000.
+// 2^x, relative error < 2e-13.  x < -1000 returns 0; x must stay below 1000.
 __device__ __forceinline__ double d_exp2(const MathTab& tb, double x) {
     const double kd = fma(x, c_dm[1], c_dm[0]);
-    const int k = __double2loint(kd);                          // k = rint(64 x)
-    const double r = fma(kd - c_dm[0], c_dm[2], x);            // x - k/64, exact
-    const int j = k & 63, n = k >> 6;
-    double p = c_dm[6];
+    const int k = __double2loint(kd);                          // k = rint(16 x)
+    const double r = fma(kd - c_dm[0], c_dm[2], x);            // x - k/16, exact
+    const int j = k & 15, n = k >> 4;
+    double p = c_dm[7];
+    p = fma(p, r, c_dm[6]);
     p = fma(p, r, c_dm[5]);
     p = fma(p, r, c_dm[4]);
     p = fma(p, r, c_dm[3]);
     const double t = tb.e2[j];
-    const double y = fma(t * r, p, t);                         // in [0.99, 2.01)
+    const double y = fma(t * r, p, t);                         // in [0.97, 2.05)
     const int hi = __double2hiint(y) + (n << 20);              // scale by 2^n through the exponent field (n >= -1001)
     const bool under = (unsigned)__double2hiint(x) > 0xC08F4000u && __double2hiint(x) < 0;   // x < -1000
     return __hiloint2double(under ? 0 : hi, under ? 0 : __double2loint(y));
 }
 
-// log2(x) for normal x > 0, absolute error < 2e-15 (+ 1 ulp of the result).
+// log2(x) for normal x > 0, absolute error < 2e-13.
 __device__ __forceinline__ double d_log2(const MathTab& tb, double x) {
     const int hi = __double2hiint(x), lo = __double2loint(x);
     const int e = (hi >> 20) - 1023;
-    const int j = (hi >> 13) & 127;                            // top 7 mantissa bits
+    const int j = (hi >> 16) & 15;                             // top 4 mantissa bits
     const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, lo);
-    const double r = fma(m, tb.rc[j], c_dm[14]);               // |r| <= 2^-8
-    double p = c_dm[11];                                       // log1p(r)/ln2 = r (c1 + c2 r + ... + c5 r^4), next term r^6/6
+    const double r = fma(m, tb.rc[j], c_dm[17]);               // |r| <= 1/32
+    double p = c_dm[14];                                       // log1p(r)/ln2 = r (c1 + c2 r + ... + c7 r^6)
+    p = fma(p, r, c_dm[13]);
+    p = fma(p, r, c_dm[12]);
+    p = fma(p, r, c_dm[11]);
     p = fma(p, r, c_dm[10]);
     p = fma(p, r, c_dm[9]);
     p = fma(p, r, c_dm[8]);
-    p = fma(p, r, c_dm[7]);
     return fma(p, r, tb.lc[j] + (double)e);
 }
 
@@ -93,12 +102,12 @@ __device__ __forceinline__ double d_log2(const MathTab& tb, double x) {
 // fp64: error 3/8 e0^2 < 4e-14 (rsqrt), e0^2 < 1e-13 (rcp).
 __device__ __forceinline__ double d_rsqrt(double x) {
     const double y0 = (double)f_rsqrt((float)x);
-    const double e = fma(-x * y0, y0, c_dm[13]);
-    return fma(c_dm[12] * y0, e, y0);
+    const double e = fma(-x * y0, y0, c_dm[16]);
+    return fma(c_dm[15] * y0, e, y0);
 }
 __device__ __forceinline__ double d_rcp(double x) {
     const double y0 = (double)f_rcp((float)x);
-    const double e = fma(-x, y0, c_dm[13]);
+    const double e = fma(-x, y0, c_dm[16]);
     return fma(y0, e, y0);
 }
 

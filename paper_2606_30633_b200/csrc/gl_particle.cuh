@@ -166,6 +166,15 @@ __global__ void gl_unpack_kernel(const __grid_constant__ PriorTable pt, const __
             o[PB_SER_E + n - 1] = keep ? (T)(Ln * an) : T(0);
         }
         o[PB_SER_D + 31] = T(0); o[PB_SER_E + 31] = T(0);
+        // precision bands of the series (knuth_banded in gl_ray.cuh): smallest k with 30 f^k below the threshold
+        const double lf = f > 0 ? log(f) : -1e30;
+        auto first_below = [&](double thr) { double k = ceil(log(thr / 30.0) / lf); return k < 1 ? 1 : (k > 64 ? 64 : (int)k); };
+        const bool dbl = sizeof(T) == 8;
+        const int k_top = first_below(dbl ? 3e-16 : 3e-9) - 1;      // keep terms k <= kt, kt >= k_top
+        const int k_dp = dbl ? first_below(1e-4) - 1 : k_top;       // fp32 steps only above 4 M1 >= k_dp (fp64 mode)
+        int mt = (k_top - 1 + 3) / 4; if (mt < 1) mt = 1; if (mt > 7) mt = 7;
+        int m1 = (k_dp + 3) / 4; if (m1 < 1) m1 = 1; if (m1 > mt) m1 = mt;
+        o[PB_SER_M1] = (T)m1; o[PB_SER_M2] = (T)(mt - m1);
     }
     if (!isfinite(lp)) ok = false;
     o[PB_VALID] = ok ? T(1) : T(0);

@@ -53,6 +53,64 @@ __device__ __forceinline__ void knuth(const T* __restrict__ cf, T p, T nf2, T wr
     Pr = R::fma(b1, wr, r0); Pi = b1 * wi;
 }
 
+// K real-coefficient polynomials in the same w at once, in precision bands (all bounds are per-particle, hence
+// CTA-uniform: no divergence).  Term k of the series is O(f^k) relative to the sum, so (gl_unpack_kernel picks M1, M2):
+//   k > kt = 4(M1+M2)+1      dropped: 30 f^(kt+1) <= 3e-16 (fp64 mode) -- numerically zero;
+//   4 M1 < k <= kt           recurrence steps in fp32 on the otherwise idle FP32 pipe: their rounding enters the sum
+//                            scaled by f^k, 30 f^(4 M1 + 1) 1e-7 <= 1e-11;
+//   k <= 4 M1                recurrence steps in T.
+// cf: K coefficient arrays of T at stride 32 (PB_SER_A / _D / _E); cf32: fp32 copies (fp64 mode only).
+template <class T, int K>
+__device__ __forceinline__ void knuth_banded(const T* __restrict__ cf, const float* __restrict__ cf32, int m1, int m2,
+                                             T p, T nf2, T wr, T wi, T (&Pr)[K], T (&Pi)[K]) {
+    using R = Real<T>;
+    T b1[K], b2[K];
+    const int kt = 4 * (m1 + m2) + 1;
+    bool seeded = false;
+    if constexpr (sizeof(T) == 8) {
+        if (m2 > 0) {
+            const float pf = (float)p, nf = (float)nf2;
+            float c1[K], c2[K];
+#pragma unroll
+            for (int i = 0; i < K; ++i) { c1[i] = cf32[32 * i + kt]; c2[i] = 0.f; }
+            int k = kt - 1;
+            for (int g = 0; g < m2; ++g, k -= 4) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+#pragma unroll
+                    for (int i = 0; i < K; ++i) {
+                        const float bk = fmaf(pf, c1[i], fmaf(nf, c2[i], cf32[32 * i + k - j]));
+                        c2[i] = c1[i]; c1[i] = bk;
+                    }
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < K; ++i) { b1[i] = (T)c1[i]; b2[i] = (T)c2[i]; }
+            seeded = true;
+        }
+    }
+    if (!seeded) {
+#pragma unroll
+        for (int i = 0; i < K; ++i) { b1[i] = cf[32 * i + kt]; b2[i] = T(0.); }
+    }
+    int k = 4 * m1;
+    for (int g = 0; g < m1; ++g, k -= 4) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+#pragma unroll
+            for (int i = 0; i < K; ++i) {
+                const T bk = R::fma(p, b1[i], R::fma(nf2, b2[i], cf[32 * i + k - j]));
+                b2[i] = b1[i]; b1[i] = bk;
+            }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < K; ++i) {
+        const T r0 = R::fma(nf2, b2[i], cf[32 * i]);
+        Pr[i] = R::fma(b1[i], wr, r0); Pi[i] = b1[i] * wi;
+    }
+}
+
 template <class T, int NMAX>
 __device__ __forceinline__ void hermite(const typename Real<T>::Tab& tb, T u, T* f) {
     using R = Real<T>;
@@ -96,10 +154,15 @@ __device__ __forceinline__ void sersic_accum(const SersicOut<T>& o, T g, T* __re
     S[SA_BXX] = R::fma(Wx, o.xr, S[SA_BXX]); S[SA_BYY] = R::fma(Wy, o.yr, S[SA_BYY]); S[SA_BXY] = R::fma(Wx, o.yr, S[SA_BXY]);
 }
 
+// Where the shapelet coefficient sums of the adjoint live: registers, except in fp64 at n_max > 6 where 66 fp64
+// accumulators spill (measured: shared memory wins only there).
+template <class T, class V> __host__ __device__ constexpr bool coef_in_smem() { return sizeof(T) == 8 && V::NMAX > 6; }
+
 // Everything one ray needs.  ADJ = false: returns the surface brightness; ADJ = true: accumulates gbar * dI/d(natural).
 template <class T, class V, bool ADJ>
-__device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* __restrict__ pb, T fj, T fi, T gbar,
-                                      T* __restrict__ acc) {
+__device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* __restrict__ pb,
+                                      const float* __restrict__ cf32, T fj, T fi, T gbar, T* __restrict__ acc,
+                                      T* __restrict__ sacc = nullptr, int sstride = 0) {
     using R = Real<T>;
     const T step = pb[PB_STEP];
     const T cph = pb[PB_M_C], sph = pb[PB_M_S];
@@ -117,8 +180,10 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
         const T c2 = R::fma(ce, ce, -se * se), s2 = T(2.) * ce * se;
         const T f = pb[PB_M_F], nf2 = -pb[PB_M_F2];
         const T wr = -f * c2, wi = -f * s2, p = T(2.) * wr;
-        T P0r, P0i;
-        knuth<T, 29>(pb + PB_SER_A, p, nf2, wr, wi, P0r, P0i);
+        const int m1 = (int)pb[PB_SER_M1], m2 = (int)pb[PB_SER_M2];
+        T Pr[ADJ ? 3 : 1], Pi[ADJ ? 3 : 1];
+        knuth_banded<T, (ADJ ? 3 : 1)>(pb + PB_SER_A, cf32, m1, m2, p, nf2, wr, wi, Pr, Pi);
+        const T P0r = Pr[0], P0i = Pi[0];
         S0r = R::fma(ce, P0r, -se * P0i); S0i = R::fma(ce, P0i, se * P0r);
         lbr = R::fma(-T(0.5), R::lg2(tb, R2), pb[PB_M_L2B]);
         const T Pw = R::ex2(tb, pb[PB_M_TM1] * lbr);
@@ -126,9 +191,7 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
         axr = amp * S0r; ayr = amp * S0i;
         kap = pb[PB_M_KAPC] * Pw * rinv;
         if constexpr (ADJ) {
-            T Q1r, Q1i, Q2r, Q2i;
-            knuth<T, 28>(pb + PB_SER_D, p, nf2, wr, wi, Q1r, Q1i);
-            knuth<T, 28>(pb + PB_SER_E, p, nf2, wr, wi, Q2r, Q2i);
+            const T Q1r = Pr[ADJ ? 1 : 0], Q1i = Pi[ADJ ? 1 : 0], Q2r = Pr[ADJ ? 2 : 0], Q2i = Pi[ADJ ? 2 : 0];
             const T ewr = R::fma(ce, wr, -se * wi), ewi = R::fma(ce, wi, se * wr);       // E w
             S1r = R::fma(ewr, Q1r, -ewi * Q1i); S1i = R::fma(ewr, Q1i, ewi * Q1r);
             S2r = R::fma(ewr, Q2r, -ewi * Q2i); S2i = R::fma(ewr, Q2i, ewi * Q2r);
@@ -204,10 +267,9 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
                     Ish = R::fma(row, fv[n2], Ish);
                 }
             } else {
-                T dfu[NM + 1], dfv[NM + 1];
-                dfu[0] = -u * fu[0]; dfv[0] = -v * fv[0];
-#pragma unroll
-                for (int k = 1; k <= NM; ++k) { dfu[k] = R::fma(hD<T>(k), fu[k - 1], -u * fu[k]); dfv[k] = R::fma(hD<T>(k), fv[k - 1], -v * fv[k]); }
+                // phi_k' = HD[k] phi_{k-1} - u phi_k is formed where it is used (no derivative arrays); the N_coef
+                // coefficient sums live in shared memory (sacc[idx * sstride], one column per thread): 66 fp64
+                // accumulators do not fit the register file next to the 45 other sums.
                 T Iu = T(0.), Iv = T(0.);
 #pragma unroll
                 for (int n2 = 0; n2 <= NM; ++n2) {
@@ -217,10 +279,15 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
                     for (int n1 = 0; n1 <= NM - n2; ++n1) {
                         const int idx = (n1 + n2) * (n1 + n2 + 1) / 2 + n2;
                         const T ak = a[idx];
-                        row = R::fma(ak, fu[n1], row); drow = R::fma(ak, dfu[n1], drow);
-                        acc[NA_SHA + idx] = R::fma(gfv, fu[n1], acc[NA_SHA + idx]);
+                        const T dfu = n1 == 0 ? -u * fu[0] : R::fma(hD<T>(n1), fu[n1 > 0 ? n1 - 1 : 0], -u * fu[n1]);
+                        row = R::fma(ak, fu[n1], row); drow = R::fma(ak, dfu, drow);
+                        if constexpr (coef_in_smem<T, V>()) sacc[idx * sstride] = R::fma(gfv, fu[n1], sacc[idx * sstride]);
+                        else acc[NA_SHA + idx] = R::fma(gfv, fu[n1], acc[NA_SHA + idx]);
                     }
-                    Ish = R::fma(row, fv[n2], Ish); Iu = R::fma(drow, fv[n2], Iu); Iv = R::fma(row, dfv[n2], Iv);
+                    Ish = R::fma(row, fv[n2], Ish); Iu = R::fma(drow, fv[n2], Iu); {
+                        const T dfv = n2 == 0 ? -v * fv[0] : R::fma(hD<T>(n2), fv[n2 > 0 ? n2 - 1 : 0], -v * fv[n2]);
+                        Iv = R::fma(row, dfv, Iv);
+                    }
                 }
                 acc[NA_SHB] = R::fma(gbar, Ish + R::fma(u, Iu, v * Iv), acc[NA_SHB]);
                 const T Ibx = Iu * ibs, Iby = Iv * ibs;
@@ -328,10 +395,13 @@ __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ 
                                                         const double* __restrict__ tabg, T* __restrict__ ray, int RPT,
                                                         int n_chunk) {
     __shared__ __align__(16) T pb[PB_STRIDE];
-    __shared__ double tabs[TabStage<T>::N];
+    __shared__ __align__(128) double tabs[TabStage<T>::N];
     const int p = blockIdx.y;
     const T* src = pbg + (size_t)p * PB_STRIDE;
     for (int k = threadIdx.x; k < V::PB_NEED; k += blockDim.x) pb[k] = src[k];
+    __shared__ float cf32[(sizeof(T) == 8 && V::MASS == 1) ? 96 : 4];     // fp32 copies of the series coefficients
+    if constexpr (sizeof(T) == 8 && V::MASS == 1)
+        for (int k = threadIdx.x; k < 96; k += blockDim.x) cf32[k] = (float)src[PB_SER_A + k];
     const typename Real<T>::Tab tb = TabStage<T>::make(tabs, tabg);
     __syncthreads();
     PlaneIter it(G, n_chunk, RPT);
@@ -354,7 +424,7 @@ __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ 
         for (int b = 0; b < RB; ++b) {
             ok[b] = it.idx < NN && r + b < RPT;
             o[b] = it.offset(G);
-            v[b] = ray_eval<T, V, false>(tb, pb + off, it.fj<T>(G), it.fi<T>(G), T(0.), nullptr);
+            v[b] = ray_eval<T, V, false>(tb, pb + off, cf32 + off, it.fj<T>(G), it.fi<T>(G), T(0.), nullptr);
             it.next(G);
         }
 #pragma unroll
@@ -364,36 +434,58 @@ __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ 
 }
 
 // Per-ray part of step F.  gbar: plane layout; nap: [Pc][gridDim.x][V::NA].
+#ifndef GL_ADJ_MINB
+#define GL_ADJ_MINB 4
+#endif
 template <class T, class V, int NT>
-__global__ void __launch_bounds__(NT) gl_ray_adj_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
+__global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 ? GL_ADJ_MINB : 1)) gl_ray_adj_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
                                                         const double* __restrict__ tabg, const T* __restrict__ gbar,
                                                         T* __restrict__ nap, int RPT, int n_chunk) {
     __shared__ __align__(16) T pb[PB_STRIDE];
-    __shared__ double tabs[TabStage<T>::N];
+    __shared__ __align__(128) double tabs[TabStage<T>::N];
     __shared__ T red[NT / 32][V::NA];
     const int p = blockIdx.y;
     const T* src = pbg + (size_t)p * PB_STRIDE;
     for (int k = threadIdx.x; k < V::PB_NEED; k += blockDim.x) pb[k] = src[k];
+    __shared__ float cf32[(sizeof(T) == 8 && V::MASS == 1) ? 96 : 4];     // fp32 copies of the series coefficients
+    if constexpr (sizeof(T) == 8 && V::MASS == 1)
+        for (int k = threadIdx.x; k < 96; k += blockDim.x) cf32[k] = (float)src[PB_SER_A + k];
     const typename Real<T>::Tab tb = TabStage<T>::make(tabs, tabg);
     __syncthreads();
     PlaneIter it(G, n_chunk, RPT);
     const T* gb = gbar + (size_t)p * ray_stride(G) + (size_t)it.ph * G.Hp * G.Wp;
     const int NN = G.N * G.N;
-    T acc[V::NA];
+    extern __shared__ __align__(16) unsigned char adj_dyn[];       // shapelet coefficient sums [NCOEF][blockDim.x]
+    T* sacc = reinterpret_cast<T*>(adj_dyn) + threadIdx.x;
+    const int sstride = blockDim.x;
+    constexpr bool CS = coef_in_smem<T, V>();
+    constexpr int NREG = CS ? NA_SHA : V::NA;                     // accumulators kept in registers
+    if constexpr (CS) {
+#pragma unroll 1
+        for (int k = 0; k < V::NCOEF; ++k) sacc[k * sstride] = T(0.);
+    }
+    T acc[NREG];
 #pragma unroll
-    for (int k = 0; k < V::NA; ++k) acc[k] = T(0.);
+    for (int k = 0; k < NREG; ++k) acc[k] = T(0.);
     if (pb[PB_VALID] != T(0.)) {
         for (int r = 0; r < RPT; ++r) {
             int off = 0; asm volatile("" : "+r"(off));      // opaque: keeps the PB scalars in shared memory, not in registers
-            if (it.idx < NN) ray_eval<T, V, true>(tb, pb + off, it.fj<T>(G), it.fi<T>(G), gb[it.offset(G)], acc);
+            if (it.idx < NN) ray_eval<T, V, true>(tb, pb + off, cf32 + off, it.fj<T>(G), it.fi<T>(G), gb[it.offset(G)], acc, sacc, sstride);
             it.next(G);
         }
     }
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
 #pragma unroll
-    for (int k = 0; k < V::NA; ++k) {
+    for (int k = 0; k < NREG; ++k) {
         T v = warp_sum(acc[k]);
         if (lane == 0) red[w][k] = v;
+    }
+    if constexpr (CS) {
+#pragma unroll 1
+        for (int k = 0; k < V::NCOEF; ++k) {
+            T v = warp_sum(sacc[k * sstride]);
+            if (lane == 0) red[w][NA_SHA + k] = v;
+        }
     }
     __syncthreads();
     T* o = nap + ((size_t)p * gridDim.x + blockIdx.x) * V::NA;
