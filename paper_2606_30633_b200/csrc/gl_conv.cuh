@@ -199,8 +199,19 @@ __device__ __forceinline__ void load_seg(T (&seg)[SEG], const T* __restrict__ p)
 // Thread lt of a particle slot owns column group g = lt and walks through ALL s*s planes of every input row, so the
 // tap address is uniform across a slot (a pure shared-memory broadcast: splitting the planes between lanes made the
 // U = 16 kernels shared-memory bound) and an output row is complete inside one thread (no cross-lane reduction).
+// PF: prefetch the next row segment into a second register buffer (off for U = 16 in fp64, where the registers buy more
+// as a second resident CTA); MINB: minimum CTAs per SM handed to the register allocator.
+#ifndef GL_CONV16_PF
+#define GL_CONV16_PF 1
+#endif
+#ifndef GL_CONV16_MINB
+#define GL_CONV16_MINB 1
+#endif
+template <class T, int U> __host__ __device__ constexpr bool conv_pf() { return !(U == 16 && sizeof(T) == 8) || GL_CONV16_PF; }
+template <class T, int U> __host__ __device__ constexpr int conv_minb() { return (U == 16 && sizeof(T) == 8) ? GL_CONV16_MINB : 1; }
+
 template <class T, int U, int CW, int LS, int NT_MAX>
-__global__ void __launch_bounds__(NT_MAX) gl_conv_fwd_is(const __grid_constant__ Geom G, const SlidePlan sp, int64_t Pc,
+__global__ void __launch_bounds__(NT_MAX, (conv_minb<T, U>())) gl_conv_fwd_is(const __grid_constant__ Geom G, const SlidePlan sp, int64_t Pc,
                                                          const T* __restrict__ ray, const T* __restrict__ sys_kt,
                                                          const T* __restrict__ sys_w, const float* __restrict__ obs,
                                                          const int32_t* __restrict__ system_id, int64_t p_base,
@@ -245,16 +256,21 @@ __global__ void __launch_bounds__(NT_MAX) gl_conv_fwd_is(const __grid_constant__
         for (int u = 0; u < U; ++u)
 #pragma unroll
             for (int q = 0; q < CW; ++q) acc[u][q] = T(0);
-        T cur[SEG], nxt[SEG];
-        load_seg<T, SEG>(nxt, in + (size_t)pq * plane);
+        constexpr bool PF = conv_pf<T, U>();
+        T cur[SEG], nxt[PF ? SEG : 2];
+        if constexpr (PF) load_seg<T, SEG>(nxt, in + (size_t)pq * plane);
         const int steps = G.Hp * nj;
         int i = 0, j = 0;
         for (int t = 0; t < steps; ++t) {
-#pragma unroll
-            for (int v = 0; v < SEG; ++v) cur[v] = nxt[v];
             int jn = j + 1, in_ = i;
             if (jn == nj) { jn = 0; in_ = i + 1; }
-            if (t + 1 < steps) load_seg<T, SEG>(nxt, in + (size_t)(pq + LS * jn) * plane + (size_t)in_ * G.Wp);
+            if constexpr (PF) {
+#pragma unroll
+                for (int v = 0; v < SEG; ++v) cur[v] = nxt[v];
+                if (t + 1 < steps) load_seg<T, SEG>(nxt, in + (size_t)(pq + LS * jn) * plane + (size_t)in_ * G.Wp);
+            } else {
+                load_seg<T, SEG>(cur, in + (size_t)(pq + LS * j) * plane + (size_t)i * G.Wp);
+            }
             conv_slide<T, U, CW, SEG>(acc, tp + (size_t)(pq + LS * j) * sp.ps, cur);
             if (jn == 0) {                                       // input row i done: output row i - U + 1 is complete
                 const int pr = i - (U - 1);
@@ -312,7 +328,7 @@ __global__ void __launch_bounds__(NT_MAX) gl_conv_fwd_is(const __grid_constant__
 //   gbar_ab[R][j'] = sum_{k,l<U} F[k][l] gp[R + k][j' + l],  F[k][l] = kt[(a+c)%s][(b+c)%s][U-1-k][U-1-l]
 // gbar (plane layout) overwrites the ray buffer; only the N x N interior of each plane is meaningful afterwards.
 template <class T, int U, int CW, int LS, int NT_MAX>
-__global__ void __launch_bounds__(NT_MAX) gl_conv_bwd_is(const __grid_constant__ Geom G, const SlidePlan sp, int64_t Pc,
+__global__ void __launch_bounds__(NT_MAX, (conv_minb<T, U>())) gl_conv_bwd_is(const __grid_constant__ Geom G, const SlidePlan sp, int64_t Pc,
                                                          const T* __restrict__ gpix, const T* __restrict__ sys_kt,
                                                          const int32_t* __restrict__ system_id, int64_t p_base,
                                                          T* __restrict__ gbar) {
@@ -353,12 +369,17 @@ __global__ void __launch_bounds__(NT_MAX) gl_conv_bwd_is(const __grid_constant__
         for (int u = 0; u < U; ++u)
 #pragma unroll
             for (int q = 0; q < CW; ++q) acc[u][q] = T(0);
-        T cur[SEG], nxt[SEG];
-        load_seg<T, SEG>(nxt, in);
+        constexpr bool PF = conv_pf<T, U>();
+        T cur[SEG], nxt[PF ? SEG : 2];
+        if constexpr (PF) load_seg<T, SEG>(nxt, in);
         for (int r = 0; r < rows; ++r) {
+            if constexpr (PF) {
 #pragma unroll
-            for (int v = 0; v < SEG; ++v) cur[v] = nxt[v];
-            if (r + 1 < rows) load_seg<T, SEG>(nxt, in + (size_t)(r + 1) * G.Wg);
+                for (int v = 0; v < SEG; ++v) cur[v] = nxt[v];
+                if (r + 1 < rows) load_seg<T, SEG>(nxt, in + (size_t)(r + 1) * G.Wg);
+            } else {
+                load_seg<T, SEG>(cur, in + (size_t)r * G.Wg);
+            }
             conv_slide<T, U, CW, SEG>(acc, tp + (size_t)ph * sp.ps, cur);
             const int n = r - (U - 1);                           // finished output row (relative to oa)
             if (n >= 0) {
@@ -372,6 +393,191 @@ __global__ void __launch_bounds__(NT_MAX) gl_conv_bwd_is(const __grid_constant__
                 for (int q = 0; q < CW; ++q) acc[u][q] = acc[u - 1][q];
 #pragma unroll
             for (int q = 0; q < CW; ++q) acc[0][q] = T(0);
+        }
+    }
+}
+
+// ----------------------------------------------------------------------------- two input rows per step (U = 11, 16)
+// With many taps the 16-byte tap broadcasts saturate the shared-memory return path (512 B per warp per load, 128 B per
+// clock per SM) before the FP64 pipe fills: measured 0.36-0.41 of the FP64 peak with one row per step.  Here every tap
+// pair loaded feeds TWO input rows (rows i and i+1 of the same plane), i.e. 4*CW FMAs per load: A[s] is the accumulator
+// of output row i + 1 - s, row i adds tap row u into A[u + 1], row i + 1 adds it into A[u]; after the pair, A[U] and
+// A[U - 1] are complete and the accumulators shift by two.
+template <class T, int U, int CW, int SEG>
+__device__ __forceinline__ void conv_slide2(T (&A)[U + 1][CW], const T* __restrict__ tap, const T (&s0)[SEG], const T (&s1)[SEG]) {
+    using V2 = typename Vec2<T>::type;
+    constexpr int UP2 = (U + 1) & ~1;
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+#pragma unroll
+        for (int v = 0; v < UP2; v += 2) {
+            const V2 k = *reinterpret_cast<const V2*>(tap + u * UP2 + v);
+#pragma unroll
+            for (int q = 0; q < CW; ++q) {
+                A[u + 1][q] = Real<T>::fma(k.x, s0[q + v], A[u + 1][q]);
+                A[u][q] = Real<T>::fma(k.x, s1[q + v], A[u][q]);
+                if (v + 1 < U) {
+                    A[u + 1][q] = Real<T>::fma(k.y, s0[q + v + 1], A[u + 1][q]);
+                    A[u][q] = Real<T>::fma(k.y, s1[q + v + 1], A[u][q]);
+                }
+            }
+        }
+    }
+}
+
+template <class T, int U, int CW>
+__device__ __forceinline__ void shift2(T (&A)[U + 1][CW]) {
+#pragma unroll
+    for (int u = U; u > 1; --u)
+#pragma unroll
+        for (int q = 0; q < CW; ++q) A[u][q] = A[u - 2][q];
+#pragma unroll
+    for (int q = 0; q < CW; ++q) { A[0][q] = T(0); A[1][q] = T(0); }
+}
+
+template <class T, int SEG>
+__device__ __forceinline__ void load_seg_or_zero(T (&seg)[SEG], const T* __restrict__ p, bool ok) {
+    if (ok) load_seg<T, SEG>(seg, p);
+    else {
+#pragma unroll
+        for (int v = 0; v < SEG; ++v) seg[v] = T(0);
+    }
+}
+
+// Step D + E, one thread per column group, all planes, two rows per step.  Launch geometry as gl_conv_fwd_is (LS = 1).
+template <class T, int U, int CW, int NT_MAX>
+__global__ void __launch_bounds__(NT_MAX) gl_conv_fwd_is2(const __grid_constant__ Geom G, const SlidePlan sp, int64_t Pc,
+                                                          const T* __restrict__ ray, const T* __restrict__ sys_kt,
+                                                          const T* __restrict__ sys_w, const float* __restrict__ obs,
+                                                          const int32_t* __restrict__ system_id, int64_t p_base,
+                                                          T* __restrict__ gpix, T* __restrict__ chi, float* __restrict__ out_model) {
+    constexpr int SEG = (CW + U - 1 + 1) & ~1, UP2 = (U + 1) & ~1;
+    extern __shared__ __align__(16) unsigned char conv_smem[];
+    T* taps = reinterpret_cast<T*>(conv_smem);
+    __shared__ T red[NT_MAX];
+    const int s = G.s, N = G.N, NPH = s * s;
+    const int slot = threadIdx.x / sp.tpp, lt = threadIdx.x - slot * sp.tpp;
+    const int64_t p = (int64_t)blockIdx.x * sp.ppc + slot;
+    const bool live = slot < sp.ppc && p < Pc;
+    const int sys = (live && system_id) ? system_id[p_base + p] : 0;
+    const int copy = sp.shared_taps ? 0 : slot;
+    {
+        const int first = sp.shared_taps ? threadIdx.x : lt, stride = sp.shared_taps ? blockDim.x : sp.tpp;
+        T* tp = taps + (size_t)copy * NPH * sp.ps;
+        const T* kt = sys_kt + (size_t)sys * NPH * U * U;
+        if (sp.shared_taps || slot < sp.ppc)
+            for (int e = first; e < NPH * U * UP2; e += stride) {
+                const int v = e % UP2, u = (e / UP2) % U, ph = e / (UP2 * U);
+                const int a = ph / s, b = ph - a * s;
+                tp[(size_t)ph * sp.ps + u * UP2 + v] = (v < U) ? kt[(size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U + u * U + v] : T(0);
+            }
+    }
+    if (live && gpix) zero_gpix_border(G, gpix + (size_t)p * gpix_stride(G), lt, sp.tpp);
+    __syncthreads();
+    const int g = lt;
+    T c2 = T(0);
+    if (live && g < sp.ncg) {
+        const size_t plane = (size_t)G.Hp * G.Wp;
+        const T* in = ray + (size_t)p * ray_stride(G) + (size_t)CW * g;
+        const T* tp = taps + (size_t)copy * NPH * sp.ps;
+        T A[U + 1][CW];
+#pragma unroll
+        for (int u = 0; u <= U; ++u)
+#pragma unroll
+            for (int q = 0; q < CW; ++q) A[u][q] = T(0);
+        for (int i = 0; i < G.Hp; i += 2) {
+            const bool two = i + 1 < G.Hp;
+            for (int j = 0; j < NPH; ++j) {
+                T s0[SEG], s1[SEG];
+                const T* row = in + (size_t)j * plane + (size_t)i * G.Wp;
+                load_seg<T, SEG>(s0, row);
+                load_seg_or_zero<T, SEG>(s1, row + G.Wp, two);
+                conv_slide2<T, U, CW, SEG>(A, tp + (size_t)j * sp.ps, s0, s1);
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {                        // A[U] is output row i - U + 1, A[U - 1] is row i - U + 2
+                const int pr = i - (U - 1) + h;
+                if (pr >= 0 && pr < N) {
+#pragma unroll
+                    for (int q = 0; q < CW; ++q) {
+                        const int pc = CW * g + q;
+                        if (pc < N)
+                            c2 += pixel_epilogue<T>(G, A[U - h][q], pr, pc, sys, (size_t)(p_base + p), (int)p, obs, sys_w, gpix, out_model);
+                    }
+                }
+            }
+            shift2<T, U, CW>(A);
+        }
+    }
+    if (chi) {
+        red[threadIdx.x] = c2;
+        __syncthreads();
+        if (lt == 0 && live) {
+            T tot = T(0);
+            for (int k = 0; k < sp.tpp; ++k) tot += red[slot * sp.tpp + k];
+            chi[p] = tot;
+        }
+    }
+}
+
+// Transpose of step D, two rows per step.  Launch geometry as gl_conv_bwd_is (LS = 1).
+template <class T, int U, int CW, int NT_MAX>
+__global__ void __launch_bounds__(NT_MAX) gl_conv_bwd_is2(const __grid_constant__ Geom G, const SlidePlan sp, int64_t Pc,
+                                                          const T* __restrict__ gpix, const T* __restrict__ sys_kt,
+                                                          const int32_t* __restrict__ system_id, int64_t p_base,
+                                                          T* __restrict__ gbar) {
+    using V2 = typename Vec2<T>::type;
+    constexpr int SEG = (CW + U - 1 + 1) & ~1, UP2 = (U + 1) & ~1;
+    extern __shared__ __align__(16) unsigned char conv_smem[];
+    T* taps = reinterpret_cast<T*>(conv_smem);
+    const int s = G.s, N = G.N, NPH = s * s;
+    const int slot = threadIdx.x / sp.tpp, lt = threadIdx.x - slot * sp.tpp;
+    const int64_t p = (int64_t)blockIdx.x * sp.ppc + slot;
+    const bool live = slot < sp.ppc && p < Pc;
+    const int sys = (live && system_id) ? system_id[p_base + p] : 0;
+    const int copy = sp.shared_taps ? 0 : slot;
+    {
+        const int first = sp.shared_taps ? threadIdx.x : lt, stride = sp.shared_taps ? blockDim.x : sp.tpp;
+        T* tp = taps + (size_t)copy * NPH * sp.ps;
+        const T* kt = sys_kt + (size_t)sys * NPH * U * U;
+        if (sp.shared_taps || slot < sp.ppc)
+            for (int e = first; e < NPH * U * UP2; e += stride) {
+                const int v = e % UP2, u = (e / UP2) % U, ph = e / (UP2 * U);
+                const int a = ph / s, b = ph - a * s;
+                tp[(size_t)ph * sp.ps + u * UP2 + v] =
+                    (v < U) ? kt[(size_t)(((a + G.c) % s) * s + (b + G.c) % s) * U * U + (U - 1 - u) * U + (U - 1 - v)] : T(0);
+            }
+    }
+    __syncthreads();
+    const int g = lt;
+    if (!(live && g < sp.ncg)) return;
+    const T* tp = taps + (size_t)copy * NPH * sp.ps;
+    const T* gp = gpix + (size_t)p * gpix_stride(G) + (size_t)CW * g;
+    const int rows = N + U - 1;
+    for (int ph = 0; ph < NPH; ++ph) {
+        const int a = ph / s, oa = phase_shift(G, a);
+        T* out = gbar + (size_t)p * ray_stride(G) + ((size_t)ph * G.Hp) * G.Wp + (size_t)CW * g;
+        const T* in = gp + (size_t)oa * G.Wg;
+        T A[U + 1][CW];
+#pragma unroll
+        for (int u = 0; u <= U; ++u)
+#pragma unroll
+            for (int q = 0; q < CW; ++q) A[u][q] = T(0);
+        for (int r = 0; r < rows; r += 2) {
+            T s0[SEG], s1[SEG];
+            load_seg<T, SEG>(s0, in + (size_t)r * G.Wg);
+            load_seg_or_zero<T, SEG>(s1, in + (size_t)(r + 1) * G.Wg, r + 1 < rows);
+            conv_slide2<T, U, CW, SEG>(A, tp + (size_t)ph * sp.ps, s0, s1);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int n = r - (U - 1) + h;                   // finished output row (relative to oa)
+                if (n >= 0 && n < N) {
+                    T* o = out + (size_t)(oa + n) * G.Wp;
+#pragma unroll
+                    for (int q = 0; q < CW; q += 2) { V2 v; v.x = A[U - h][q]; v.y = A[U - h][q + 1]; *reinterpret_cast<V2*>(o + q) = v; }
+                }
+            }
+            shift2<T, U, CW>(A);
         }
     }
 }

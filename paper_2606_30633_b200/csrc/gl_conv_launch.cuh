@@ -57,7 +57,7 @@ static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems) {
         sp.ppc = 1; double best = 0;
         for (int k = 1; k <= 8; ++k) {
             const int nt = round_up(k * sp.tpp, 32);
-            if (nt > GL_CONV_CTA && k > 1) break;
+            if (nt > ((LS > 1 || esize == 8) ? GL_CONV_CTA : 256) && k > 1) break;   // fp32, LS = 1: registers allow the fullest CTA up to 256
             const double eff = (double)(k * LS * ncg) / nt;
             if (eff > best + 1e-9) { best = eff; sp.ppc = k; }
         }
@@ -101,6 +101,34 @@ static inline cudaError_t conv_bwd_is_launch(const ConvPlan& pl, const Geom& G, 
     return cudaSuccess;
 }
 
+template <class T, int U, int CW, int NT_MAX>
+static inline cudaError_t conv_fwd_is2_launch(const ConvPlan& pl, const Geom& G, const T* ray, const T* sys_kt,
+                                              const T* sys_w, const float* obs, const int32_t* system_id, int64_t p_base,
+                                              int64_t Pc, T* gpix, T* chi, float* out_model, cudaStream_t st) {
+    auto kern = gl_conv_fwd_is2<T, U, CW, NT_MAX>;
+    if (pl.fwd_smem > 40 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.fwd_smem);
+        if (e != cudaSuccess) return e;
+    }
+    const unsigned grid = (unsigned)((Pc + pl.fwd.ppc - 1) / pl.fwd.ppc);
+    kern<<<grid, round_up(pl.fwd.ppc * pl.fwd.tpp, 32), pl.fwd_smem, st>>>(G, pl.fwd, Pc, ray, sys_kt, sys_w, obs, system_id, p_base,
+                                                                          gpix, chi, out_model);
+    return cudaSuccess;
+}
+
+template <class T, int U, int CW, int NT_MAX>
+static inline cudaError_t conv_bwd_is2_launch(const ConvPlan& pl, const Geom& G, const T* gpix, const T* sys_kt,
+                                              const int32_t* system_id, int64_t p_base, int64_t Pc, T* gbar, cudaStream_t st) {
+    auto kern = gl_conv_bwd_is2<T, U, CW, NT_MAX>;
+    if (pl.bwd_smem > 40 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.bwd_smem);
+        if (e != cudaSuccess) return e;
+    }
+    const unsigned grid = (unsigned)((Pc + pl.bwd.ppc - 1) / pl.bwd.ppc);
+    kern<<<grid, round_up(pl.bwd.ppc * pl.bwd.tpp, 32), pl.bwd_smem, st>>>(G, pl.bwd, Pc, gpix, sys_kt, system_id, p_base, gbar);
+    return cudaSuccess;
+}
+
 // Step D + E.  Returns the number of kernels launched (negative on a CUDA error).
 template <class T>
 static inline int conv_fwd_launch(const ConvPlan& pl, const Geom& G, const T* ray, const T* sys_kt, const T* sys_w,
@@ -109,8 +137,8 @@ static inline int conv_fwd_launch(const ConvPlan& pl, const Geom& G, const T* ra
     cudaError_t e = cudaSuccess;
     switch (pl.kind) {
         case 1: e = conv_fwd_is_launch<T, 6, 4, 4, 256>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st); break;
-        case 2: e = conv_fwd_is_launch<T, 11, 2, 1, 256>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st); break;
-        case 3: e = conv_fwd_is_launch<T, 16, 2, 1, 256>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st); break;
+        case 2: e = conv_fwd_is2_launch<T, 11, 2, 256>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st); break;
+        case 3: e = conv_fwd_is2_launch<T, 16, 2, 256>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st); break;
         default: {
             dim3 grid((G.N * G.N + 255) / 256, (unsigned)Pc);
             gl_conv_fwd_generic<T><<<grid, 256, 0, st>>>(G, ray, sys_kt, sys_w, obs, system_id, p_base, gpix, chi, out_model);
@@ -126,8 +154,8 @@ static inline int conv_bwd_launch(const ConvPlan& pl, const Geom& G, const T* gp
     cudaError_t e = cudaSuccess;
     switch (pl.kind) {
         case 1: e = conv_bwd_is_launch<T, 6, 4, 4, 256>(pl, G, gpix, sys_kt, system_id, p_base, Pc, gbar, st); break;
-        case 2: e = conv_bwd_is_launch<T, 11, 2, 1, 256>(pl, G, gpix, sys_kt, system_id, p_base, Pc, gbar, st); break;
-        case 3: e = conv_bwd_is_launch<T, 16, 2, 1, 256>(pl, G, gpix, sys_kt, system_id, p_base, Pc, gbar, st); break;
+        case 2: e = conv_bwd_is2_launch<T, 11, 2, 256>(pl, G, gpix, sys_kt, system_id, p_base, Pc, gbar, st); break;
+        case 3: e = conv_bwd_is2_launch<T, 16, 2, 256>(pl, G, gpix, sys_kt, system_id, p_base, Pc, gbar, st); break;
         default: {
             dim3 grid((G.s * G.s * G.N * G.N + 255) / 256, (unsigned)Pc);
             gl_conv_bwd_generic<T><<<grid, 256, 0, st>>>(G, gpix, sys_kt, system_id, p_base, gbar);
