@@ -214,3 +214,74 @@ def test_determinism_repeat_calls():
     a = m.logpost_grad(z); a = (a[0].clone(), a[1].clone())
     b = m.logpost_grad(z)
     assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
+
+
+def _small_case(n_pix, s, K, mass_model, multipole_mask, shapelet_nmax, n_lens, seed, n_particles=6, epl_terms=30):
+    """A seeded small problem of arbitrary shape: spec with config-style priors, Gaussian PSF, oracle-rendered truth."""
+    import oracle
+    pri = W._default_priors(mass_model, multipoles=bool(multipole_mask), shapelet_nmax=shapelet_nmax, n_lens=n_lens)
+    if multipole_mask and multipole_mask != 3:
+        # _default_priors adds 4 multipole entries; keep 2 for a single order
+        k0 = 1 + (1 if mass_model == 1 else 0) + 4 + 2
+        pri = pri[:k0] + pri[k0 + 2:]
+    sp = W.LensSpec(n_pix, s, K, W._r32(0.11 * 40 / n_pix * 2.4), mass_model=mass_model, epl_terms=epl_terms,
+                    multipole_mask=multipole_mask, shapelet_nmax=shapelet_nmax, n_lens_sersic=n_lens, priors=pri)
+    sp.names = W.param_names(mass_model, 1, multipole_mask, 1, shapelet_nmax, n_lens)
+    assert len(sp.names) == sp.n_params
+    rng = np.random.default_rng(seed)
+    step = sp.pix_scale / s
+    psf = W.gaussian_psf(K, 2.5 * step, step)[None].astype(np.float32)
+    truth_z = W.z_of(pri, W.draw(rng, pri, 1)).astype(np.float32)
+    truth = oracle.model_image(sp, psf.astype(np.float64), W.theta_of(pri, truth_z.astype(np.float64)))
+    sigma = np.full((1, n_pix, n_pix), 0.05, np.float32)
+    obs = (truth + 0.05 * rng.standard_normal(truth.shape)).astype(np.float32)
+    z = W.z_of(pri, W.draw(rng, pri, n_particles)).astype(np.float32)
+    return sp, obs, sigma, psf, z
+
+
+@pytest.mark.parametrize("shape", [(12, 3, 5), (9, 1, 3), (16, 2, 7), (10, 4, 9), (7, 5, 1)])
+@pytest.mark.parametrize("model", [(0, 0, -1, 1), (1, 3, 4, 2), (1, 2, -1, 0)])
+def test_generic_shapes_strict_parity(shape, model):
+    """Shapes outside the tuned specialisations (odd supersampling, other tap counts, no lens light, one multipole
+    order, n_max = 4): the generic step-D kernels and every model variant against the oracle, strict bar, fp64 mode;
+    fp32 mode must agree with fp64 mode to 1e-3 norm-wise."""
+    import dataclasses
+    import oracle
+    import torch
+    gl = _gl()
+    n_pix, s, K = shape
+    mass_model, mp, nmax, n_lens = model
+    sp, obs, sigma, psf, z = _small_case(n_pix, s, K, mass_model, mp, nmax, n_lens, seed=1000 * n_pix + 10 * K + mass_model)
+    ref = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), None)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    lp, g = m.logpost_grad(torch.from_numpy(z).cuda())
+    lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+    fin = np.isfinite(ref["logp"])
+    assert np.array_equal(fin, np.isfinite(lp))
+    assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+    ok, rep = grad_report(g[fin], ref["grad"][fin])
+    assert rep["n_fail"] == 0, rep
+    m32 = gl.LensModel(dataclasses.replace(sp, precision=1), obs, sigma, psf)
+    lp32, g32 = m32.logpost_grad(torch.from_numpy(z).cuda())
+    g32 = g32.cpu().numpy().astype(np.float64)
+    nrm = np.linalg.norm(g32[fin] - g[fin], axis=1) / np.linalg.norm(g[fin], axis=1)
+    assert nrm.max() <= 1e-3, nrm
+
+
+def test_truncated_series_matches_truncated_oracle():
+    """epl_terms = 8 on a strongly elliptical lens: the CUDA path must reproduce the oracle's 8-term sum (reading S5),
+    which differs visibly from the converged series."""
+    import oracle
+    import torch
+    gl = _gl()
+    sp, obs, sigma, psf, z = _small_case(14, 2, 5, 1, 0, -1, 1, seed=77, n_particles=8, epl_terms=8)
+    z[:, 2] = 0.45; z[:, 3] = -0.2                                  # |eps| ~ 0.49
+    ref8 = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), None, epl_terms=8)
+    refc = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), None)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    lp, g = m.logpost_grad(torch.from_numpy(z).cuda())
+    lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(lp - ref8["logp"]) <= RTOL_LOGP * np.abs(ref8["logp"]))
+    ok, rep = grad_report(g, ref8["grad"])
+    assert rep["n_fail"] == 0, rep
+    assert np.max(np.abs(refc["logp"] - ref8["logp"]) / np.abs(refc["logp"])) > 1e-6      # the truncation is visible
