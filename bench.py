@@ -54,6 +54,8 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
                     help="arithmetic of the CUDA path: f64 = GL_PRECISION_F64 (default; strict parity), f32 = GL_PRECISION_F32")
+    ap.add_argument("--stage", default="grad", choices=["grad", "map"],
+                    help="grad: one gl_logpost_grad call per step (the headline); map: one fused gl_map_step (Adam) per step")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -232,8 +234,17 @@ def run_ours(a):
     ws_bytes = gl.gl_workspace_bytes(m.h, P)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # 256 MiB > 126 MB L2
 
+    if a.stage == "map":
+        zm, om, ov = z.clone(), torch.zeros_like(z), torch.zeros_like(z)
+        adam = dict(kind=gl.GL_OPT_ADAM, lr=1e-3, b1=0.9, b2=0.999, eps=1e-8, eps_root=0.0)
+        tstep = [0]
+
     def step():
-        gl.gl_logpost_grad(m.h, m.obs, m.noise_sigma, m.psf, z, sid, lp, g, ws)
+        if a.stage == "map":
+            tstep[0] += 1
+            gl.gl_map_step(m.h, adam, m.obs, m.noise_sigma, m.psf, zm, sid, om, ov, tstep[0], lp, g, ws)
+        else:
+            gl.gl_logpost_grad(m.h, m.obs, m.noise_sigma, m.psf, z, sid, lp, g, ws)
 
     for _ in range(max(a.warmup, 3)):
         step()
@@ -266,7 +277,8 @@ def run_ours(a):
     sampler.stop_flag = True
     sampler.join(timeout=2)
     t_e2e = sum(e0.elapsed_time(e1) for e0, e1 in ev2) * 1e-3
-    assert torch.equal(lph, lp.cpu()) and torch.equal(gh, g.cpu()), "host-buffer path disagrees with the device path"
+    if a.stage == "grad":
+        assert torch.equal(lph, lp.cpu()) and torch.equal(gh, g.cpu()), "host-buffer path disagrees with the device path"
     finite = float(torch.isfinite(lp).float().mean())
 
     # dominant-kernel roofline: per-stage device time from the library's own CUDA events on the launching stream
@@ -319,7 +331,7 @@ def run_ours(a):
            "warmup": max(a.warmup, 3), "ms_per_step": t_dev / a.steps * 1e3, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": a.precision, "data": "synthetic",
            "config": {"workload": WORKLOAD_NAMES[k], "n_particles_per_gpu": P, "n_params": n_p,
-                      "rays_per_particle": wm["rays"], "parallelism": "replicas x%d" % world,
+                      "rays_per_particle": wm["rays"], "parallelism": "replicas x%d" % world, "stage": a.stage,
                       "l2": "256 MiB flush write between timed iterations; workspace %.0f MB" % (ws_bytes / 1e6),
                       "finite_fraction": finite},
            "e2e": {"value": whole_job_rate(world, P, a.steps, t_e2e), "unit": UNIT, "h2d_bytes_per_step": int(zh.numel() * 4),

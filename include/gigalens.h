@@ -153,6 +153,29 @@ gl_status gl_logpost_grad_host(const gl_config* cfg, const float* obs, const flo
                                float* out_logp_host, float* out_grad_host, void* workspace, size_t workspace_bytes,
                                void* stream /* cudaStream_t */);
 
+/* ---- one multi-start MAP optimiser step on the device -------------------------------------
+ * Every particle descends  -log p~  independently (P:L83 fn 2) with Adam (the paper's default for MAP) or
+ * AdaBelief (lr 1e-4, b1 0.95, b2 0.99 at P:L112).  Update rules as published:
+ *   g = -d log p~/dz;  m <- b1 m + (1-b1) g
+ *   ADAM       v <- b2 v + (1-b2) g^2
+ *   ADABELIEF  v <- b2 v + (1-b2) (g - m)^2 + eps_root          (m already updated)
+ *   z <- z - lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps)
+ * gl_map_step = gl_logpost_grad at the current params, then the update, fused on `stream` (no host round trip):
+ *   opt        HOST pointer, copied
+ *   params     [n][n_params] DEVICE, in/out: z before -> z after
+ *   opt_m/opt_v [n][n_params] DEVICE, in/out: optimiser state (zero before step 1)
+ *   step       t = 1, 2, ... (bias correction)
+ *   out_logp   [n] log p~ at the params BEFORE the update;  out_grad [n][n_params] its gradient (also scratch)
+ * A particle whose log-posterior or gradient is not finite keeps its params and state.  Update arithmetic in fp64,
+ * storage fp32.  Errors as gl_logpost_grad, plus GL_ERR_BAD_CONFIG for an invalid `opt` (lr <= 0, b outside [0,1),
+ * eps < 0, step < 1). */
+typedef enum { GL_OPT_ADAM = 0, GL_OPT_ADABELIEF = 1 } gl_opt_kind;
+typedef struct { int32_t kind; float lr, b1, b2, eps, eps_root; } gl_opt_desc;
+gl_status gl_map_step(const gl_config* cfg, const gl_opt_desc* opt, const float* obs, const float* noise_sigma,
+                      const float* psf, float* params, const int32_t* system_id, int64_t n_particles,
+                      float* opt_m, float* opt_v, int64_t step, float* out_logp, float* out_grad,
+                      void* workspace, size_t workspace_bytes, void* stream /* cudaStream_t */);
+
 /* Number of kernel launches the last call on this thread enqueued (bench.py's gpu_launches claim). */
 int64_t gl_last_launch_count(void);
 

@@ -21,7 +21,7 @@ STATUS = {0: "GL_OK", -1: "GL_ERR_NULL", -2: "GL_ERR_BAD_CONFIG", -3: "GL_ERR_BA
 EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_workspace_bytes", "gl_logpost",
            "gl_logpost_grad", "gl_model_image", "gl_workspace_bytes_host", "gl_logpost_grad_host",
            "gl_last_launch_count", "gl_status_string", "gl_version", "gl_stage_timing_enable", "gl_stage_count",
-           "gl_stage_name", "gl_stage_times", "gl_probe_pipe"]
+           "gl_stage_name", "gl_stage_times", "gl_probe_pipe", "gl_map_step"]
 
 
 class GLError(RuntimeError):
@@ -32,6 +32,14 @@ class GLError(RuntimeError):
 
 class gl_prior(C.Structure):
     _fields_ = [("kind", C.c_int32), ("a", C.c_float), ("b", C.c_float), ("lo", C.c_float), ("hi", C.c_float)]
+
+
+class gl_opt_desc(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("lr", C.c_float), ("b1", C.c_float), ("b2", C.c_float), ("eps", C.c_float),
+                ("eps_root", C.c_float)]
+
+
+GL_OPT_ADAM, GL_OPT_ADABELIEF = 0, 1
 
 
 class gl_config_desc(C.Structure):
@@ -70,6 +78,8 @@ def lib():
         L.gl_logpost_grad.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, sz, vp]
         L.gl_logpost_grad_host.restype = C.c_int
         L.gl_logpost_grad_host.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, sz, vp]
+        L.gl_map_step.restype = C.c_int
+        L.gl_map_step.argtypes = [vp, C.POINTER(gl_opt_desc), vp, vp, vp, vp, vp, i64, vp, vp, i64, vp, vp, vp, sz, vp]
         L.gl_model_image.restype = C.c_int
         L.gl_model_image.argtypes = [vp, vp, vp, vp, i64, vp, vp, sz, vp]
         L.gl_last_launch_count.restype = i64
@@ -199,6 +209,23 @@ def gl_logpost_grad(h, obs, noise_sigma, psf, params, system_id, out_logp, out_g
            "gl_logpost_grad")
 
 
+def gl_map_step(h, opt, obs, noise_sigma, psf, params, system_id, opt_m, opt_v, step, out_logp, out_grad, workspace,
+                stream=None):
+    """opt: dict(kind, lr, b1, b2, eps, eps_root) or a gl_opt_desc.  params / opt_m / opt_v are updated in place."""
+    torch = _torch()
+    f32 = torch.float32
+    if not isinstance(opt, gl_opt_desc):
+        opt = gl_opt_desc(int(opt["kind"]), float(opt["lr"]), float(opt["b1"]), float(opt["b2"]), float(opt["eps"]),
+                          float(opt.get("eps_root", 0.0)))
+    n = params.shape[0]
+    _check(lib().gl_map_step(h, C.byref(opt), _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
+                             _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
+                             _ptr(_dev(system_id, torch.int32, "system_id")), n, _ptr(_dev(opt_m, f32, "opt_m")),
+                             _ptr(_dev(opt_v, f32, "opt_v")), int(step), _ptr(_dev(out_logp, f32, "out_logp")),
+                             _ptr(_dev(out_grad, f32, "out_grad")), _ptr(workspace),
+                             workspace.numel() * workspace.element_size(), _stream(stream)), "gl_map_step")
+
+
 def gl_model_image(h, psf, params, system_id, out_image, workspace, stream=None):
     torch = _torch()
     f32 = torch.float32
@@ -277,6 +304,19 @@ class LensModel:
         gl_logpost_grad(self.h, self.obs, self.noise_sigma, self.psf, params, self._sid(system_id), lp, g,
                         self.workspace(n), stream)
         return lp, g
+
+    def map_run(self, params, opt, n_steps, system_id=None, first_step=1, state=None, stream=None):
+        """n_steps fused MAP steps (gl_map_step) on `params` IN PLACE; no host synchronisation between steps.
+        Returns (logp at the last evaluated params, (m, v) optimiser state)."""
+        torch = _torch()
+        n = params.shape[0]
+        m, v = state if state is not None else (torch.zeros_like(params), torch.zeros_like(params))
+        lp = torch.empty(n, dtype=torch.float32, device=self.device)
+        g = torch.empty((n, self.n_params), dtype=torch.float32, device=self.device)
+        sid, ws = self._sid(system_id), self.workspace(n)
+        for t in range(first_step, first_step + n_steps):
+            gl_map_step(self.h, opt, self.obs, self.noise_sigma, self.psf, params, sid, m, v, t, lp, g, ws, stream)
+        return lp, (m, v)
 
     def model_image(self, params, system_id=None, stream=None):
         torch = _torch()

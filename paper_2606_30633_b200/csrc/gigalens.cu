@@ -366,6 +366,33 @@ extern "C" gl_status gl_model_image(const gl_config* cfg, const float* psf, cons
                workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
+extern "C" gl_status gl_map_step(const gl_config* cfg, const gl_opt_desc* opt, const float* obs, const float* noise_sigma,
+                                 const float* psf, float* params, const int32_t* system_id, int64_t n_particles,
+                                 float* opt_m, float* opt_v, int64_t step, float* out_logp, float* out_grad,
+                                 void* workspace, size_t workspace_bytes, void* stream) {
+    t_launches = 0;
+    if (!cfg || !opt) return GL_ERR_NULL;
+    if (opt->kind != GL_OPT_ADAM && opt->kind != GL_OPT_ADABELIEF) return GL_ERR_BAD_CONFIG;
+    if (!(opt->lr > 0.f) || !(opt->b1 >= 0.f && opt->b1 < 1.f) || !(opt->b2 >= 0.f && opt->b2 < 1.f) || !(opt->eps >= 0.f) ||
+        !(opt->eps_root >= 0.f) || step < 1)
+        return GL_ERR_BAD_CONFIG;
+    if (n_particles < 0) return GL_ERR_BAD_SHAPE;
+    if (n_particles == 0) return GL_OK;
+    if (!opt_m || !opt_v) return GL_ERR_NULL;
+    cudaStream_t st = (cudaStream_t)stream;
+    gl_status s = run(cfg, 1, obs, noise_sigma, psf, params, system_id, n_particles, out_logp, out_grad, nullptr,
+                      workspace, workspace_bytes, st);
+    if (s != GL_OK) return s;
+    OptParams o{};
+    o.kind = opt->kind; o.lr = opt->lr; o.b1 = opt->b1; o.b2 = opt->b2; o.eps = opt->eps; o.eps_root = opt->eps_root;
+    o.c1 = 1.0 / (1.0 - std::pow(o.b1, (double)step)); o.c2 = 1.0 / (1.0 - std::pow(o.b2, (double)step));
+    const int64_t n_elem = n_particles * cfg->L.n_params;
+    gl_opt_update_kernel<<<(unsigned)((n_elem + 255) / 256), 256, 0, st>>>(o, n_elem, cfg->L.n_params, out_logp, out_grad,
+                                                                          params, opt_m, opt_v);
+    ++t_launches;
+    return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
+}
+
 extern "C" size_t gl_workspace_bytes_host(const gl_config* c, int64_t n) {
     if (!c || n <= 0) return 0;
     const size_t np = (size_t)c->L.n_params;

@@ -291,4 +291,25 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
     if (lane == 0) out_logp[p_base + p] = good ? (float)logp : -INFINITY;
 }
 
+// Adam / AdaBelief update of every (particle, parameter), fp64 arithmetic on fp32 storage.
+// One thread per element; a particle with a non-finite log-posterior or gradient row is left untouched (the
+// gradient row of such a particle is all zero by construction of gl_finalize_kernel, its logp is -INF).
+struct OptParams { int kind; double lr, b1, b2, eps, eps_root, c1, c2; };   // c1 = 1/(1-b1^t), c2 = 1/(1-b2^t)
+
+__global__ void gl_opt_update_kernel(const __grid_constant__ OptParams o, int64_t n_elem, int n_params,
+                                     const float* __restrict__ logp, const float* __restrict__ grad,
+                                     float* __restrict__ z, float* __restrict__ m, float* __restrict__ v) {
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_elem) return;
+    const int64_t p = e / n_params;
+    const float lp = logp[p];
+    const double g = -(double)grad[e];
+    if (!isfinite(lp) || !isfinite(g)) return;
+    const double m1 = o.b1 * (double)m[e] + (1.0 - o.b1) * g;
+    const double d = o.kind == 1 ? g - m1 : g;
+    const double v1 = o.b2 * (double)v[e] + (1.0 - o.b2) * d * d + (o.kind == 1 ? o.eps_root : 0.0);
+    const double z1 = (double)z[e] - o.lr * (m1 * o.c1) / (sqrt(v1 * o.c2) + o.eps);
+    m[e] = (float)m1; v[e] = (float)v1; z[e] = (float)z1;
+}
+
 }  // namespace gl

@@ -42,7 +42,7 @@ def test_adabelief_belief_term_vanishes_for_constant_gradient():
     for t in range(1, 200):
         z0 = z.copy()
         z, m, s = optim.update(optim.ADABELIEF, z, -g, np.zeros(1), m, s, t, 1e-4, 0.95, 0.99, 1e-16, 1e-16)
-        steps.append(float(z0 - z))
+        steps.append(float((z0 - z)[0, 0]))
     assert abs(g - m).max() < 2.0 * 0.95 ** 199 * 1.0001
     assert steps[-1] > steps[0] > 0
 
