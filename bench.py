@@ -61,6 +61,12 @@ def parse():
     return ap.parse_args()
 
 
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel at the default
+# workload, from the committed `ncu --set full` capture profiles/r1c_cfg2_f64.md (bench.py cannot run a profiler):
+# keyed by (config, precision, stage).  None elsewhere.
+NCU_TRAFFIC_BYTES = {(2, "f64", "ray_adjoint"): 2.152173e9 + 0.028176e9}
+
+
 # ----------------------------------------------------------------------------------------------- clocks
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
@@ -316,7 +322,7 @@ def run_ours(a):
     achieved = dom_ops / dom_t / 1e12 if dom_t > 0 else 0.0
     clocks = sampler.summary()
     roof = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "T %s lane-op/s (FMA=1)" % pipe,
-            "frac": achieved / peak, "traffic": None,
+            "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((k, a.precision, dom)),
             "peak_source": "148 SM x %d %s lanes x %g MHz (%s)" % (lanes, pipe, mhz_max, peak_src),
             "probe_T_laneops_per_s": probe,
             "kernel_ms_per_launch": stage_ms[dom] / max(stage_n[dom], 1), "kernel_launches_per_step": stage_n[dom],
