@@ -48,3 +48,64 @@ def map_step(oracle_mod, spec, obs, sigma, psf, z, m, v, t, opt, system_id=None)
     z1, m1, v1 = update(opt["kind"], z, r["grad"], r["logp"], m, v, t, opt["lr"], opt["b1"], opt["b2"], opt["eps"],
                         opt.get("eps_root", 0.0))
     return r["logp"], z1, m1, v1
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-2: SVI step
+# a multivariate-normal surrogate q~(Theta~; mu~, Sigma~) is fitted by minimising the loss
+#   ELBO = E_q[ log q~(Theta~) - log p~(I_obs, Theta~) ]                                   (Eq. 2; a LOSS, as printed)
+# estimated at each iteration from n_VI draws (L91); the gradient with respect to (mu~, Sigma~) is obtained "with JAX's
+# automatic differentiation" from the draws (L98) and an optimiser step is applied to (mu~, Sigma~) (L100); AdaBelief
+# with lr 1e-4, b1 0.95, b2 0.99 is the default (L112).
+# Readings: Sigma~ = L L^T with L lower triangular, positive diagonal, optimised entry by entry
+# (packed row-major: L00, L10, L11, L20, ...); draws are reparameterised, z_i = mu + L xi_i with xi_i ~ N(0, I) supplied
+# by the caller; differentiating the sampled loss through the draws gives the pathwise estimator
+#   loss^   = -sum_j log L_jj - (n/2) log(2 pi e) + (1/N) sum_i [ -log p~(z_i) ]
+#             (E_q[log q] = -entropy is taken in closed form; with xi fixed the sampled -1/2 |xi|^2 term has no gradient)
+#   d/dmu_j   = -(1/N) sum_i g_ij                      g_i = grad log p~(z_i)
+#   d/dL_jk   = -(1/N) sum_i g_ij xi_ik - delta_jk / L_jj          (k <= j)
+# Eq. 3 as printed (L95) is the score-function form of the same gradient; both are unbiased, the text's autodiff of
+# reparameterised draws yields the pathwise one, which is also the one that uses the hot path's gradient.
+# Draws whose log p~ is not finite are left out of the averages (N = number of finite draws).
+
+def tril_unpack(n, packed):
+    L = np.zeros((n, n))
+    L[np.tril_indices(n)] = np.asarray(packed, np.float64)
+    return L
+
+
+def tril_pack(L):
+    return np.asarray(L, np.float64)[np.tril_indices(L.shape[0])]
+
+
+def svi_draw(mu, L_packed, xi):
+    mu = np.asarray(mu, np.float64); xi = np.asarray(xi, np.float64)
+    return mu[None, :] + xi @ tril_unpack(mu.size, L_packed).T
+
+
+def svi_loss_and_grad(mu, L_packed, xi, logp, grad_logp):
+    """Sampled ELBO loss and its gradient w.r.t. (mu, packed L) from per-draw logp [N] and grad log p [N][n]."""
+    n = np.asarray(mu).size
+    L = tril_unpack(n, L_packed)
+    xi = np.asarray(xi, np.float64); g = np.asarray(grad_logp, np.float64); lp = np.asarray(logp, np.float64)
+    ok = np.isfinite(lp) & np.all(np.isfinite(g), axis=1)
+    N = int(ok.sum())
+    d = np.diag(L)
+    loss = -np.sum(np.log(np.abs(d))) - 0.5 * n * np.log(2.0 * np.pi * np.e) - lp[ok].sum() / N
+    g_mu = -g[ok].sum(axis=0) / N
+    g_L = -(g[ok].T @ xi[ok]) / N - np.diag(1.0 / d)
+    return loss, g_mu, tril_pack(g_L), N
+
+
+def svi_step(logp_grad_fn, mu, L_packed, xi, m, v, t, opt):
+    """One SVI iteration.  logp_grad_fn(z [N][n]) -> (logp [N], grad [N][n]).  State m, v over the concatenated
+    parameter vector [mu; packed L].  Returns (loss, mu_new, L_new, m_new, v_new, logp)."""
+    n = np.asarray(mu).size
+    z = svi_draw(mu, L_packed, xi)
+    lp, g = logp_grad_fn(z)
+    loss, g_mu, g_L, N = svi_loss_and_grad(mu, L_packed, xi, lp, g)
+    theta = np.concatenate([np.asarray(mu, np.float64), np.asarray(L_packed, np.float64)])[None, :]
+    grad_loss = np.concatenate([g_mu, g_L])[None, :]
+    th1, m1, v1 = update(opt["kind"], theta, -grad_loss, np.zeros(1), np.asarray(m, np.float64)[None, :],
+                         np.asarray(v, np.float64)[None, :], t, opt["lr"], opt["b1"], opt["b2"], opt["eps"],
+                         opt.get("eps_root", 0.0))
+    return loss, th1[0, :n], th1[0, n:], m1[0], v1[0], lp

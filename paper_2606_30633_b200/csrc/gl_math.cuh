@@ -88,7 +88,8 @@ __device__ __forceinline__ double d_log2(const MathTab& tb, double x) {
     const int j = (hi >> 16) & 15;                             // top 4 mantissa bits
     const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, lo);
     const double r = fma(m, tb.rc[j], c_dm[17]);               // |r| <= 1/32
-    double p = c_dm[14];                                       // log1p(r)/ln2 = r (c1 + c2 r + ... + c7 r^6)
+    // log1p(r)/ln2 = r (c1 + c2 r + ... + c7 r^6)
+    double p = c_dm[14];
     p = fma(p, r, c_dm[13]);
     p = fma(p, r, c_dm[12]);
     p = fma(p, r, c_dm[11]);

@@ -67,3 +67,87 @@ def test_non_finite_rows_are_left_unchanged():
     for r in (0, 4):
         assert not np.array_equal(z1[r], z[r])
     assert np.all(np.isfinite(z1))
+
+
+# ------------------------------------------------------------------------------------------------ SVI (NEXT-2)
+def _toy_target(a, A):
+    """A smooth non-Gaussian log density with closed-form gradient: -1/2 (z-a)^T A (z-a) - sum log cosh z."""
+    def f(z):
+        d = z - a
+        return -0.5 * np.einsum("ij,jk,ik->i", d, A, d) - np.log(np.cosh(z)).sum(axis=1), -(d @ A.T) - np.tanh(z)
+    return f
+
+
+def _svi_setup(n=4, N=64, seed=3):
+    rng = np.random.default_rng(seed)
+    B = rng.standard_normal((n, n)); A = B @ B.T + n * np.eye(n)
+    a = rng.standard_normal(n)
+    L = np.tril(rng.standard_normal((n, n)) * 0.2) + np.diag(0.5 + rng.random(n))
+    return rng.standard_normal(n), optim.tril_pack(L), rng.standard_normal((N, n)), _toy_target(a, A), a, A
+
+
+def test_svi_gradient_is_the_derivative_of_the_sampled_loss():
+    """With the draws xi held fixed, the assembled gradient must equal central finite differences of the sampled loss
+    in every entry of mu and of the packed L (the pathwise estimator IS the derivative of the sampled objective)."""
+    mu, Lp, xi, f, a, A = _svi_setup()
+
+    def loss(mu_, Lp_):
+        lp, g = f(optim.svi_draw(mu_, Lp_, xi))
+        return optim.svi_loss_and_grad(mu_, Lp_, xi, lp, g)[0]
+
+    lp, g = f(optim.svi_draw(mu, Lp, xi))
+    _, g_mu, g_L, N = optim.svi_loss_and_grad(mu, Lp, xi, lp, g)
+    assert N == 64
+    h = 1e-6
+    for j in range(mu.size):
+        e = np.zeros_like(mu); e[j] = h
+        assert abs((loss(mu + e, Lp) - loss(mu - e, Lp)) / (2 * h) - g_mu[j]) < 1e-6 * max(1, abs(g_mu[j]))
+    for j in range(Lp.size):
+        e = np.zeros_like(Lp); e[j] = h
+        assert abs((loss(mu, Lp + e) - loss(mu, Lp - e)) / (2 * h) - g_L[j]) < 1e-6 * max(1, abs(g_L[j]))
+
+
+def test_svi_gaussian_target_closed_form():
+    """Quadratic log p: grad_mu = A (mu + L xbar - a), grad_L = tril(A (mu - a) xbar^T + A L S) - diag(1/L_jj) with the
+    SAMPLE moments xbar, S of the draws; and the entropy term is the closed form of a Gaussian's."""
+    mu, Lp, xi, _, a, A = _svi_setup(seed=8)
+    L = optim.tril_unpack(mu.size, Lp)
+    z = optim.svi_draw(mu, Lp, xi)
+    assert np.allclose(z, mu + xi @ L.T)
+    d = z - a
+    lp = -0.5 * np.einsum("ij,jk,ik->i", d, A, d); g = -(d @ A.T)
+    loss, g_mu, g_L, _ = optim.svi_loss_and_grad(mu, Lp, xi, lp, g)
+    xbar = xi.mean(axis=0); S = xi.T @ xi / xi.shape[0]
+    assert np.allclose(g_mu, A @ (mu + L @ xbar - a), rtol=1e-12)
+    full = np.outer(A @ (mu - a), xbar) + A @ L @ S - np.diag(1 / np.diag(L))
+    assert np.allclose(g_L, optim.tril_pack(full), rtol=1e-12, atol=1e-12)
+    ent = 0.5 * np.linalg.slogdet(2 * np.pi * np.e * (L @ L.T))[1]
+    assert np.isclose(loss, -ent - lp.mean(), rtol=1e-13)
+
+
+def test_svi_fits_a_gaussian_target():
+    """Minimising the loss on a Gaussian target recovers its mean and covariance (KL = 0 at the optimum, Eq. 1)."""
+    rng = np.random.default_rng(0)
+    n = 3
+    A = np.array([[2.0, 0.3, 0.0], [0.3, 1.0, -0.2], [0.0, -0.2, 0.5]]); a = np.array([0.5, -1.0, 0.25])
+
+    def f(z):
+        d = z - a
+        return -0.5 * np.einsum("ij,jk,ik->i", d, A, d), -(d @ A.T)
+
+    mu = np.zeros(n); Lp = optim.tril_pack(np.eye(n)); m = np.zeros(n + 6); v = np.zeros(n + 6)
+    opt = dict(kind=optim.ADAM, lr=2e-2, b1=0.9, b2=0.999, eps=1e-8)
+    for t in range(1, 1501):
+        _, mu, Lp, m, v, _ = optim.svi_step(f, mu, Lp, rng.standard_normal((256, n)), m, v, t, opt)
+    L = optim.tril_unpack(n, Lp)
+    assert np.allclose(mu, a, atol=0.05)
+    assert np.allclose(L @ L.T, np.linalg.inv(A), atol=0.08)
+
+
+def test_svi_non_finite_draws_are_left_out():
+    mu, Lp, xi, f, a, A = _svi_setup(N=16)
+    lp, g = f(optim.svi_draw(mu, Lp, xi))
+    lp2 = lp.copy(); lp2[3] = -np.inf
+    l1, gm1, gl1, N1 = optim.svi_loss_and_grad(mu, Lp, np.delete(xi, 3, 0), np.delete(lp, 3), np.delete(g, 3, 0))
+    l2, gm2, gl2, N2 = optim.svi_loss_and_grad(mu, Lp, xi, lp2, g)
+    assert N2 == 15 == N1 and np.isclose(l1, l2) and np.allclose(gm1, gm2) and np.allclose(gl1, gl2)
