@@ -176,6 +176,25 @@ gl_status gl_map_step(const gl_config* cfg, const gl_opt_desc* opt, const float*
                       float* opt_m, float* opt_v, int64_t step, float* out_logp, float* out_grad,
                       void* workspace, size_t workspace_bytes, void* stream /* cudaStream_t */);
 
+/* ---- one SVI iteration on the device ---------------------------------------------------------
+ * Fits the multivariate-normal surrogate q~(Theta~; mu~, Sigma~ = L L^T) of P:L78-100 by one optimiser step on the
+ * sampled loss  ELBO^ = -sum_j log L_jj - (n/2) log(2 pi e) - (1/N) sum_i log p~(z_i)  (Eq. 2 with E_q[log q] in closed
+ * form), z_i = mu + L xi_i, through its pathwise gradient:
+ *   d/dmu_j = -(1/N) sum_i g_ij,   d/dL_jk = -(1/N) sum_i g_ij xi_ik - delta_jk / L_jj  (k <= j),  g_i = grad log p~(z_i).
+ * The reduction over the draws runs on the device in a fixed order (it replaces the cross-device pmean of Fig. 1 box 5).
+ *   opt      HOST pointer (Adam or AdaBelief; P:L112 gives AdaBelief lr 1e-4, b1 0.95, b2 0.99)
+ *   mu       [n_params]                DEVICE in/out
+ *   l_tril   [n_params (n_params+1)/2] DEVICE in/out, lower triangle packed row-major (L00, L10, L11, L20, ...)
+ *   xi       [n_draws][n_params]       DEVICE, standard-normal draws supplied by the caller (counter-based or any RNG)
+ *   opt_m/opt_v [n_params + n_tril]    DEVICE in/out optimiser state over [mu; l_tril]
+ *   out_stats [2] DEVICE: loss estimate, number of draws with a finite log p~ (the others are left out of the means)
+ * workspace >= gl_svi_workspace_bytes(cfg, n_draws).  Errors as gl_map_step. */
+size_t gl_svi_workspace_bytes(const gl_config* cfg, int64_t n_draws);
+gl_status gl_svi_step(const gl_config* cfg, const gl_opt_desc* opt, const float* obs, const float* noise_sigma,
+                      const float* psf, float* mu, float* l_tril, const float* xi, const int32_t* system_id,
+                      int64_t n_draws, float* opt_m, float* opt_v, int64_t step, float* out_stats,
+                      void* workspace, size_t workspace_bytes, void* stream /* cudaStream_t */);
+
 /* Number of kernel launches the last call on this thread enqueued (bench.py's gpu_launches claim). */
 int64_t gl_last_launch_count(void);
 

@@ -21,7 +21,8 @@ STATUS = {0: "GL_OK", -1: "GL_ERR_NULL", -2: "GL_ERR_BAD_CONFIG", -3: "GL_ERR_BA
 EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_workspace_bytes", "gl_logpost",
            "gl_logpost_grad", "gl_model_image", "gl_workspace_bytes_host", "gl_logpost_grad_host",
            "gl_last_launch_count", "gl_status_string", "gl_version", "gl_stage_timing_enable", "gl_stage_count",
-           "gl_stage_name", "gl_stage_times", "gl_probe_pipe", "gl_map_step"]
+           "gl_stage_name", "gl_stage_times", "gl_probe_pipe", "gl_map_step",
+           "gl_svi_workspace_bytes", "gl_svi_step"]
 
 
 class GLError(RuntimeError):
@@ -80,6 +81,10 @@ def lib():
         L.gl_logpost_grad_host.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, sz, vp]
         L.gl_map_step.restype = C.c_int
         L.gl_map_step.argtypes = [vp, C.POINTER(gl_opt_desc), vp, vp, vp, vp, vp, i64, vp, vp, i64, vp, vp, vp, sz, vp]
+        L.gl_svi_workspace_bytes.restype = sz
+        L.gl_svi_workspace_bytes.argtypes = [vp, i64]
+        L.gl_svi_step.restype = C.c_int
+        L.gl_svi_step.argtypes = [vp, C.POINTER(gl_opt_desc), vp, vp, vp, vp, vp, vp, vp, i64, vp, vp, i64, vp, vp, sz, vp]
         L.gl_model_image.restype = C.c_int
         L.gl_model_image.argtypes = [vp, vp, vp, vp, i64, vp, vp, sz, vp]
         L.gl_last_launch_count.restype = i64
@@ -224,6 +229,31 @@ def gl_map_step(h, opt, obs, noise_sigma, psf, params, system_id, opt_m, opt_v, 
                              _ptr(_dev(opt_v, f32, "opt_v")), int(step), _ptr(_dev(out_logp, f32, "out_logp")),
                              _ptr(_dev(out_grad, f32, "out_grad")), _ptr(workspace),
                              workspace.numel() * workspace.element_size(), _stream(stream)), "gl_map_step")
+
+
+def _opt_desc(opt):
+    if isinstance(opt, gl_opt_desc):
+        return opt
+    return gl_opt_desc(int(opt["kind"]), float(opt["lr"]), float(opt["b1"]), float(opt["b2"]), float(opt["eps"]),
+                       float(opt.get("eps_root", 0.0)))
+
+
+def gl_svi_workspace_bytes(h, n):
+    return lib().gl_svi_workspace_bytes(h, int(n))
+
+
+def gl_svi_step(h, opt, obs, noise_sigma, psf, mu, l_tril, xi, system_id, opt_m, opt_v, step, out_stats, workspace,
+                stream=None):
+    """One SVI iteration; mu, l_tril (packed lower triangle), opt_m, opt_v are updated in place; xi: [n_draws][n_params]."""
+    torch = _torch()
+    f32 = torch.float32
+    opt = _opt_desc(opt)
+    _check(lib().gl_svi_step(h, C.byref(opt), _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
+                             _ptr(_dev(psf, f32, "psf")), _ptr(_dev(mu, f32, "mu")), _ptr(_dev(l_tril, f32, "l_tril")),
+                             _ptr(_dev(xi, f32, "xi")), _ptr(_dev(system_id, torch.int32, "system_id")), xi.shape[0],
+                             _ptr(_dev(opt_m, f32, "opt_m")), _ptr(_dev(opt_v, f32, "opt_v")), int(step),
+                             _ptr(_dev(out_stats, f32, "out_stats")), _ptr(workspace),
+                             workspace.numel() * workspace.element_size(), _stream(stream)), "gl_svi_step")
 
 
 def gl_model_image(h, psf, params, system_id, out_image, workspace, stream=None):

@@ -14,6 +14,7 @@
 #include "gl_particle.cuh"
 #include "gl_probe.cuh"
 #include "gl_ray.cuh"
+#include "gl_svi.cuh"
 
 using namespace gl;
 
@@ -366,16 +367,16 @@ extern "C" gl_status gl_model_image(const gl_config* cfg, const float* psf, cons
                workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
+static gl_status check_opt(const gl_opt_desc* opt, int64_t step);
+static OptParams opt_params(const gl_opt_desc* opt, int64_t step);
+
 extern "C" gl_status gl_map_step(const gl_config* cfg, const gl_opt_desc* opt, const float* obs, const float* noise_sigma,
                                  const float* psf, float* params, const int32_t* system_id, int64_t n_particles,
                                  float* opt_m, float* opt_v, int64_t step, float* out_logp, float* out_grad,
                                  void* workspace, size_t workspace_bytes, void* stream) {
     t_launches = 0;
-    if (!cfg || !opt) return GL_ERR_NULL;
-    if (opt->kind != GL_OPT_ADAM && opt->kind != GL_OPT_ADABELIEF) return GL_ERR_BAD_CONFIG;
-    if (!(opt->lr > 0.f) || !(opt->b1 >= 0.f && opt->b1 < 1.f) || !(opt->b2 >= 0.f && opt->b2 < 1.f) || !(opt->eps >= 0.f) ||
-        !(opt->eps_root >= 0.f) || step < 1)
-        return GL_ERR_BAD_CONFIG;
+    if (!cfg) return GL_ERR_NULL;
+    { gl_status so = check_opt(opt, step); if (so != GL_OK) return so; }
     if (n_particles < 0) return GL_ERR_BAD_SHAPE;
     if (n_particles == 0) return GL_OK;
     if (!opt_m || !opt_v) return GL_ERR_NULL;
@@ -383,13 +384,73 @@ extern "C" gl_status gl_map_step(const gl_config* cfg, const gl_opt_desc* opt, c
     gl_status s = run(cfg, 1, obs, noise_sigma, psf, params, system_id, n_particles, out_logp, out_grad, nullptr,
                       workspace, workspace_bytes, st);
     if (s != GL_OK) return s;
-    OptParams o{};
-    o.kind = opt->kind; o.lr = opt->lr; o.b1 = opt->b1; o.b2 = opt->b2; o.eps = opt->eps; o.eps_root = opt->eps_root;
-    o.c1 = 1.0 / (1.0 - std::pow(o.b1, (double)step)); o.c2 = 1.0 / (1.0 - std::pow(o.b2, (double)step));
+    const OptParams o = opt_params(opt, step);
     const int64_t n_elem = n_particles * cfg->L.n_params;
     gl_opt_update_kernel<<<(unsigned)((n_elem + 255) / 256), 256, 0, st>>>(o, n_elem, cfg->L.n_params, out_logp, out_grad,
                                                                           params, opt_m, opt_v);
     ++t_launches;
+    return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
+}
+
+struct SviPlan { size_t core, off_z, off_lp, off_g, off_part, total; };
+static SviPlan svi_plan(const gl_config* c, int64_t n) {
+    SviPlan p{};
+    const size_t np = (size_t)c->L.n_params, nslot = 2 + np + np * (np + 1) / 2;
+    p.core = make_plan(c, n).total;
+    size_t o = p.core;
+    p.off_z = o;    o = align256(o + sizeof(float) * (size_t)n * np);
+    p.off_lp = o;   o = align256(o + sizeof(float) * (size_t)n);
+    p.off_g = o;    o = align256(o + sizeof(float) * (size_t)n * np);
+    p.off_part = o; o = align256(o + sizeof(double) * SVI_NCHUNK * nslot);
+    p.total = o;
+    return p;
+}
+
+extern "C" size_t gl_svi_workspace_bytes(const gl_config* c, int64_t n) {
+    if (!c || n <= 0) return 0;
+    return svi_plan(c, n).total;
+}
+
+static gl_status check_opt(const gl_opt_desc* opt, int64_t step) {
+    if (!opt) return GL_ERR_NULL;
+    if (opt->kind != GL_OPT_ADAM && opt->kind != GL_OPT_ADABELIEF) return GL_ERR_BAD_CONFIG;
+    if (!(opt->lr > 0.f) || !(opt->b1 >= 0.f && opt->b1 < 1.f) || !(opt->b2 >= 0.f && opt->b2 < 1.f) || !(opt->eps >= 0.f) ||
+        !(opt->eps_root >= 0.f) || step < 1)
+        return GL_ERR_BAD_CONFIG;
+    return GL_OK;
+}
+static OptParams opt_params(const gl_opt_desc* opt, int64_t step) {
+    OptParams o{};
+    o.kind = opt->kind; o.lr = opt->lr; o.b1 = opt->b1; o.b2 = opt->b2; o.eps = opt->eps; o.eps_root = opt->eps_root;
+    o.c1 = 1.0 / (1.0 - std::pow(o.b1, (double)step)); o.c2 = 1.0 / (1.0 - std::pow(o.b2, (double)step));
+    return o;
+}
+
+extern "C" gl_status gl_svi_step(const gl_config* cfg, const gl_opt_desc* opt, const float* obs, const float* noise_sigma,
+                                 const float* psf, float* mu, float* l_tril, const float* xi, const int32_t* system_id,
+                                 int64_t n, float* opt_m, float* opt_v, int64_t step, float* out_stats,
+                                 void* workspace, size_t workspace_bytes, void* stream) {
+    t_launches = 0;
+    if (!cfg) return GL_ERR_NULL;
+    gl_status s = check_opt(opt, step);
+    if (s != GL_OK) return s;
+    if (n < 0) return GL_ERR_BAD_SHAPE;
+    if (n == 0) return GL_OK;
+    if (!mu || !l_tril || !xi || !opt_m || !opt_v || !out_stats || !workspace) return GL_ERR_NULL;
+    const SviPlan pl = svi_plan(cfg, n);
+    if (workspace_bytes < pl.total || ((uintptr_t)workspace & 255) != 0) return GL_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    char* w = (char*)workspace;
+    float* z = (float*)(w + pl.off_z); float* lp = (float*)(w + pl.off_lp); float* g = (float*)(w + pl.off_g);
+    double* part = (double*)(w + pl.off_part);
+    const int np = cfg->L.n_params, nslot = 2 + np + np * (np + 1) / 2;
+    gl_svi_draw_kernel<<<(unsigned)((n * np + 255) / 256), 256, 0, st>>>(n, np, mu, l_tril, xi, z);
+    s = run(cfg, 1, obs, noise_sigma, psf, z, system_id, n, lp, g, nullptr, workspace, pl.core, st);
+    if (s != GL_OK) return s;
+    const int64_t launches = t_launches + 1;
+    gl_svi_reduce_kernel<<<dim3((nslot + 127) / 128, SVI_NCHUNK), 128, 0, st>>>(n, np, lp, g, xi, part);
+    gl_svi_update_kernel<<<1, 256, 0, st>>>(opt_params(opt, step), np, part, mu, l_tril, opt_m, opt_v, out_stats);
+    t_launches = launches + 2;
     return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
 }
 
