@@ -109,3 +109,47 @@ def svi_step(logp_grad_fn, mu, L_packed, xi, m, v, t, opt):
                          np.asarray(v, np.float64)[None, :], t, opt["lr"], opt["b1"], opt["b2"], opt["eps"],
                          opt.get("eps_root", 0.0))
     return loss, th1[0, :n], th1[0, n:], m1[0], v1[0], lp
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-3: HMC transition
+# every chain runs Hamiltonian Monte Carlo independently on log p~ in the unconstrained
+# space; the surrogate covariance from SVI (or from the mass-matrix adaptation, L128) sets the scale of each dimension.
+# The paper uses TFP's HMC and prints neither the integrator nor the step size or trajectory length.
+# Readings: the standard leapfrog HMC transition (Neal 2011) with mass matrix M = Sigma^-1,
+# Sigma = L L^T (L lower triangular, packed as for SVI), written in the whitened momentum xi = L^T p ~ N(0, I):
+#   H(z, xi) = -log p~(z) + 1/2 |xi|^2
+#   one leapfrog step:  xi <- xi + (eps/2) L^T g(z);  z <- z + eps L xi;  xi <- xi + (eps/2) L^T g(z)       g = grad log p~
+#   accept the end point of n_leapfrog steps iff  log u < H(z0, xi0) - H(z1, xi1),  u ~ U(0, 1)
+# xi0 and log u are INPUTS (both sides must see the same random numbers).  A proposal whose log p~ is not finite is
+# rejected; the cached log p~ and gradient of the current state travel with it.
+
+def _tril_matvecs(n, L_packed):
+    L = tril_unpack(n, L_packed)
+    return L, (lambda x: x @ L.T), (lambda g: g @ L)            # rows: L xi  and  L^T g
+
+
+def hmc_leapfrog(logp_grad_fn, z, grad, L_packed, xi, eps, n_leapfrog):
+    """n_leapfrog leapfrog steps from (z, xi) with grad = g(z).  Returns (z1, xi1, logp1, grad1)."""
+    z = np.array(z, np.float64); xi = np.array(xi, np.float64); g = np.array(grad, np.float64)
+    _, Lx, LTg = _tril_matvecs(z.shape[1], L_packed)
+    lp = None
+    for _ in range(n_leapfrog):
+        xi = xi + 0.5 * eps * LTg(g)
+        z = z + eps * Lx(xi)
+        lp, g = logp_grad_fn(z)
+        g = np.where(np.isfinite(lp)[:, None], g, 0.0)
+        xi = xi + 0.5 * eps * LTg(g)
+    return z, xi, lp, g
+
+
+def hmc_transition(logp_grad_fn, z, logp, grad, L_packed, xi, log_u, eps, n_leapfrog):
+    """One HMC transition for every chain (row).  Returns (z_new, logp_new, grad_new, accepted [bool], dH)."""
+    z0 = np.asarray(z, np.float64); lp0 = np.asarray(logp, np.float64); g0 = np.asarray(grad, np.float64)
+    xi0 = np.asarray(xi, np.float64)
+    z1, xi1, lp1, g1 = hmc_leapfrog(logp_grad_fn, z0, g0, L_packed, xi0, eps, n_leapfrog)
+    h0 = -lp0 + 0.5 * np.sum(xi0 * xi0, axis=1)
+    h1 = np.where(np.isfinite(lp1), -lp1 + 0.5 * np.sum(xi1 * xi1, axis=1), np.inf)
+    dH = h0 - h1
+    acc = np.isfinite(lp1) & (np.asarray(log_u, np.float64) < dH)
+    a = acc[:, None]
+    return np.where(a, z1, z0), np.where(acc, lp1, lp0), np.where(a, g1, g0), acc, dH

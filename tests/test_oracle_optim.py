@@ -151,3 +151,81 @@ def test_svi_non_finite_draws_are_left_out():
     l1, gm1, gl1, N1 = optim.svi_loss_and_grad(mu, Lp, np.delete(xi, 3, 0), np.delete(lp, 3), np.delete(g, 3, 0))
     l2, gm2, gl2, N2 = optim.svi_loss_and_grad(mu, Lp, xi, lp2, g)
     assert N2 == 15 == N1 and np.isclose(l1, l2) and np.allclose(gm1, gm2) and np.allclose(gl1, gl2)
+
+
+# ------------------------------------------------------------------------------------------------ HMC (NEXT-3)
+def _gauss(a, A):
+    def f(z):
+        d = z - a
+        return -0.5 * np.einsum("ij,jk,ik->i", d, A, d), -(d @ A.T)
+    return f
+
+
+def test_leapfrog_is_time_reversible():
+    """Integrate, flip the momentum, integrate again: back at the start (the property that makes HMC valid)."""
+    mu, Lp, xi, f, a, A = _svi_setup(n=5, N=7, seed=12)
+    z0 = np.random.default_rng(1).standard_normal((7, 5))
+    lp0, g0 = f(z0)
+    z1, x1, lp1, g1 = optim.hmc_leapfrog(f, z0, g0, Lp, xi, 0.03, 25)
+    z2, x2, _, _ = optim.hmc_leapfrog(f, z1, g1, Lp, -x1, 0.03, 25)
+    assert np.allclose(z2, z0, atol=1e-11) and np.allclose(-x2, xi, atol=1e-11)
+
+
+def test_leapfrog_energy_error_is_second_order():
+    """Fixed trajectory length: halving the step size divides the energy error by ~4."""
+    mu, Lp, xi, f, a, A = _svi_setup(n=4, N=32, seed=5)
+    z0 = a + 0.3 * np.random.default_rng(2).standard_normal((32, 4))
+    lp0, g0 = f(z0)
+    errs = []
+    for eps, n in ((0.04, 10), (0.02, 20), (0.01, 40)):
+        z1, x1, lp1, _ = optim.hmc_leapfrog(f, z0, g0, Lp, xi, eps, n)
+        errs.append(np.abs((-lp1 + 0.5 * (x1 ** 2).sum(1)) - (-lp0 + 0.5 * (xi ** 2).sum(1))).mean())
+    assert 3.0 < errs[0] / errs[1] < 5.0 and 3.0 < errs[1] / errs[2] < 5.0
+
+
+def test_whitened_dynamics_half_period_maps_to_mirror_point():
+    """Gaussian target N(a, Sigma) with L = chol(Sigma): in whitened coordinates the flow is a rotation, so after time pi
+    every chain sits at 2a - z0 whatever its momentum: pins the roles of L (position) and L^T (force)."""
+    rng = np.random.default_rng(9)
+    n = 4
+    B = rng.standard_normal((n, n)); Sigma = B @ B.T + np.eye(n); a = rng.standard_normal(n)
+    L = np.linalg.cholesky(Sigma)
+    f = _gauss(a, np.linalg.inv(Sigma))
+    z0 = a + rng.standard_normal((6, n)); xi = rng.standard_normal((6, n))
+    lp0, g0 = f(z0)
+    nstep = 2000
+    z1, x1, _, _ = optim.hmc_leapfrog(f, z0, g0, optim.tril_pack(L), xi, np.pi / nstep, nstep)
+    assert np.allclose(z1, 2 * a - z0, atol=1e-5) and np.allclose(x1, -xi, atol=1e-5)
+
+
+def test_hmc_samples_a_gaussian_target():
+    """2000 transitions of 64 chains reproduce mean and covariance of a correlated Gaussian within Monte-Carlo error;
+    acceptance is high at this step size and rejected chains keep their state and cache."""
+    rng = np.random.default_rng(3)
+    a = np.array([1.0, -2.0, 0.5]); A = np.array([[2.0, 0.6, 0.0], [0.6, 1.0, -0.3], [0.0, -0.3, 0.8]])
+    f = _gauss(a, A)
+    Lp = optim.tril_pack(np.eye(3))
+    z = rng.standard_normal((64, 3)); lp, g = f(z)
+    acc_n = 0; samples = []
+    for t in range(2000):
+        z_old, lp_old = z.copy(), lp.copy()
+        z, lp, g, acc, dH = optim.hmc_transition(f, z, lp, g, Lp, rng.standard_normal((64, 3)), np.log(rng.random(64)), 0.35, 5)
+        assert np.array_equal(z[~acc], z_old[~acc]) and np.array_equal(lp[~acc], lp_old[~acc])
+        lp_chk, g_chk = f(z)
+        assert np.allclose(lp_chk, lp) and np.allclose(g_chk, g)
+        acc_n += acc.sum()
+        if t >= 200: samples.append(z.copy())
+    s = np.concatenate(samples)
+    assert acc_n / (2000 * 64) > 0.8
+    assert np.allclose(s.mean(0), a, atol=0.03)
+    assert np.allclose(np.cov(s.T), np.linalg.inv(A), atol=0.06)
+
+
+def test_hmc_rejects_non_finite_proposals():
+    def f(z):                                             # support z_0 < 1
+        lp = np.where(z[:, 0] < 1.0, -0.5 * (z ** 2).sum(1), -np.inf)
+        return lp, np.where(np.isfinite(lp)[:, None], -z, 0.0)
+    z = np.array([[0.9, 0.0], [-0.5, 0.2]]); lp, g = f(z)
+    xi = np.array([[3.0, 0.0], [0.1, 0.1]])
+    z1, lp1, g1, acc, dH = optim.hmc_transition(f, z, lp, g, optim.tril_pack(np.eye(2)), xi, np.log([0.999, 1e-9]), 0.2, 3)
+    assert not acc[0] and np.array_equal(z1[0], z[0]) and acc[1]
