@@ -195,6 +195,28 @@ gl_status gl_svi_step(const gl_config* cfg, const gl_opt_desc* opt, const float*
                       int64_t n_draws, float* opt_m, float* opt_v, int64_t step, float* out_stats,
                       void* workspace, size_t workspace_bytes, void* stream /* cudaStream_t */);
 
+/* ---- one HMC transition of n independent chains on the device -------------------------------
+ * Standard leapfrog HMC (mass matrix from the surrogate covariance) in the whitened momentum
+ * xi = L^T p, Sigma = L L^T = M^-1:  H = -log p~(z) + |xi|^2/2;  per leapfrog step
+ * xi += (eps/2) L^T g(z); z += eps L xi; xi += (eps/2) L^T g(z);  the end point of n_leapfrog steps is accepted iff
+ * log_u < H(start) - H(end) and its log p~ is finite.
+ *   z        [n][n_params] DEVICE in/out: chain positions
+ *   logp     [n]           DEVICE in/out: log p~ at z   (cached; fill with gl_logpost_grad before the first transition)
+ *   grad     [n][n_params] DEVICE in/out: its gradient  (cached likewise)
+ *   l_tril   packed lower triangle of L shared by all chains, or NULL for the identity
+ *   xi       [n][n_params] DEVICE: initial whitened momenta ~ N(0, I), supplied by the caller
+ *   log_u    [n]           DEVICE: log of uniform(0,1) draws, supplied by the caller
+ *   out_accept [n] int32 (1 accepted), out_dh [n] = H(start) - H(end) (-INF for a non-finite proposal)
+ * n_params <= 128.  workspace >= gl_hmc_workspace_bytes(cfg, n).  The trajectory is carried in fp64; the hot path is
+ * evaluated at the fp32-rounded positions.  Errors as gl_logpost_grad, plus GL_ERR_BAD_CONFIG for step_size <= 0 or
+ * n_leapfrog < 1. */
+size_t gl_hmc_workspace_bytes(const gl_config* cfg, int64_t n_chains);
+gl_status gl_hmc_step(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
+                      float* z, float* logp, float* grad, const float* l_tril, const float* xi, const float* log_u,
+                      const int32_t* system_id, int64_t n_chains, float step_size, int32_t n_leapfrog,
+                      int32_t* out_accept, float* out_dh, void* workspace, size_t workspace_bytes,
+                      void* stream /* cudaStream_t */);
+
 /* Number of kernel launches the last call on this thread enqueued (bench.py's gpu_launches claim). */
 int64_t gl_last_launch_count(void);
 

@@ -22,7 +22,7 @@ EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_wo
            "gl_logpost_grad", "gl_model_image", "gl_workspace_bytes_host", "gl_logpost_grad_host",
            "gl_last_launch_count", "gl_status_string", "gl_version", "gl_stage_timing_enable", "gl_stage_count",
            "gl_stage_name", "gl_stage_times", "gl_probe_pipe", "gl_map_step",
-           "gl_svi_workspace_bytes", "gl_svi_step"]
+           "gl_svi_workspace_bytes", "gl_svi_step", "gl_hmc_workspace_bytes", "gl_hmc_step"]
 
 
 class GLError(RuntimeError):
@@ -81,6 +81,10 @@ def lib():
         L.gl_logpost_grad_host.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, sz, vp]
         L.gl_map_step.restype = C.c_int
         L.gl_map_step.argtypes = [vp, C.POINTER(gl_opt_desc), vp, vp, vp, vp, vp, i64, vp, vp, i64, vp, vp, vp, sz, vp]
+        L.gl_hmc_workspace_bytes.restype = sz
+        L.gl_hmc_workspace_bytes.argtypes = [vp, i64]
+        L.gl_hmc_step.restype = C.c_int
+        L.gl_hmc_step.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, C.c_float, C.c_int32, vp, vp, vp, sz, vp]
         L.gl_svi_workspace_bytes.restype = sz
         L.gl_svi_workspace_bytes.argtypes = [vp, i64]
         L.gl_svi_step.restype = C.c_int
@@ -236,6 +240,24 @@ def _opt_desc(opt):
         return opt
     return gl_opt_desc(int(opt["kind"]), float(opt["lr"]), float(opt["b1"]), float(opt["b2"]), float(opt["eps"]),
                        float(opt.get("eps_root", 0.0)))
+
+
+def gl_hmc_workspace_bytes(h, n):
+    return lib().gl_hmc_workspace_bytes(h, int(n))
+
+
+def gl_hmc_step(h, obs, noise_sigma, psf, z, logp, grad, l_tril, xi, log_u, system_id, step_size, n_leapfrog,
+                out_accept, out_dh, workspace, stream=None):
+    """One HMC transition of every chain (row of z); z, logp, grad are updated in place where the proposal is accepted."""
+    torch = _torch()
+    f32 = torch.float32
+    _check(lib().gl_hmc_step(h, _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
+                             _ptr(_dev(psf, f32, "psf")), _ptr(_dev(z, f32, "z")), _ptr(_dev(logp, f32, "logp")),
+                             _ptr(_dev(grad, f32, "grad")), _ptr(_dev(l_tril, f32, "l_tril")), _ptr(_dev(xi, f32, "xi")),
+                             _ptr(_dev(log_u, f32, "log_u")), _ptr(_dev(system_id, torch.int32, "system_id")), z.shape[0],
+                             float(step_size), int(n_leapfrog), _ptr(_dev(out_accept, torch.int32, "out_accept")),
+                             _ptr(_dev(out_dh, f32, "out_dh")), _ptr(workspace),
+                             workspace.numel() * workspace.element_size(), _stream(stream)), "gl_hmc_step")
 
 
 def gl_svi_workspace_bytes(h, n):

@@ -15,6 +15,7 @@
 #include "gl_probe.cuh"
 #include "gl_ray.cuh"
 #include "gl_svi.cuh"
+#include "gl_hmc.cuh"
 
 using namespace gl;
 
@@ -450,6 +451,59 @@ extern "C" gl_status gl_svi_step(const gl_config* cfg, const gl_opt_desc* opt, c
     const int64_t launches = t_launches + 1;
     gl_svi_reduce_kernel<<<dim3((nslot + 127) / 128, SVI_NCHUNK), 128, 0, st>>>(n, np, lp, g, xi, part);
     gl_svi_update_kernel<<<1, 256, 0, st>>>(opt_params(opt, step), np, part, mu, l_tril, opt_m, opt_v, out_stats);
+    t_launches = launches + 2;
+    return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
+}
+
+struct HmcPlan { size_t core, off_zd, off_xd, off_zf, off_g, off_lp, total; };
+static HmcPlan hmc_plan(const gl_config* c, int64_t n) {
+    HmcPlan p{};
+    const size_t np = (size_t)c->L.n_params;
+    p.core = make_plan(c, n).total;
+    size_t o = p.core;
+    p.off_zd = o; o = align256(o + sizeof(double) * (size_t)n * np);
+    p.off_xd = o; o = align256(o + sizeof(double) * (size_t)n * np);
+    p.off_zf = o; o = align256(o + sizeof(float) * (size_t)n * np);
+    p.off_g = o;  o = align256(o + sizeof(float) * (size_t)n * np);
+    p.off_lp = o; o = align256(o + sizeof(float) * (size_t)n);
+    p.total = o;
+    return p;
+}
+
+extern "C" size_t gl_hmc_workspace_bytes(const gl_config* c, int64_t n) {
+    if (!c || n <= 0) return 0;
+    return hmc_plan(c, n).total;
+}
+
+extern "C" gl_status gl_hmc_step(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
+                                 float* z, float* logp, float* grad, const float* l_tril, const float* xi, const float* log_u,
+                                 const int32_t* system_id, int64_t n, float step_size, int32_t n_leapfrog,
+                                 int32_t* out_accept, float* out_dh, void* workspace, size_t workspace_bytes, void* stream) {
+    t_launches = 0;
+    if (!cfg) return GL_ERR_NULL;
+    if (!(step_size > 0.f) || !std::isfinite(step_size) || n_leapfrog < 1 || cfg->L.n_params > 128) return GL_ERR_BAD_CONFIG;
+    if (n < 0) return GL_ERR_BAD_SHAPE;
+    if (n == 0) return GL_OK;
+    if (!z || !logp || !grad || !xi || !log_u || !out_accept || !out_dh || !workspace) return GL_ERR_NULL;
+    const HmcPlan pl = hmc_plan(cfg, n);
+    if (workspace_bytes < pl.total || ((uintptr_t)workspace & 255) != 0) return GL_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    char* w = (char*)workspace;
+    double* zd = (double*)(w + pl.off_zd); double* xd = (double*)(w + pl.off_xd);
+    float* zf = (float*)(w + pl.off_zf); float* g1 = (float*)(w + pl.off_g); float* lp1 = (float*)(w + pl.off_lp);
+    const int np = cfg->L.n_params;
+    const double eps = (double)step_size;
+    int64_t launches = 0;
+    for (int s = 0; s < n_leapfrog; ++s) {
+        // half kick at the first step, the two half kicks of consecutive steps merged into one full kick afterwards
+        gl_hmc_kick_drift_kernel<<<(unsigned)n, 128, 0, st>>>(np, l_tril, s == 0 ? grad : g1, s == 0 ? 0.5 * eps : eps, eps, 1,
+                                                             s == 0, z, xi, zd, xd, zf);
+        gl_status r = run(cfg, 1, obs, noise_sigma, psf, zf, system_id, n, lp1, g1, nullptr, workspace, pl.core, st);
+        if (r != GL_OK) return r;
+        launches += 1 + t_launches;
+    }
+    gl_hmc_kick_drift_kernel<<<(unsigned)n, 128, 0, st>>>(np, l_tril, g1, 0.5 * eps, eps, 0, 0, z, xi, zd, xd, zf);
+    gl_hmc_accept_kernel<<<(unsigned)n, 128, 0, st>>>(np, xi, xd, zd, lp1, g1, log_u, z, logp, grad, out_accept, out_dh);
     t_launches = launches + 2;
     return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
 }
