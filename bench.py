@@ -54,8 +54,9 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
                     help="arithmetic of the CUDA path: f64 = GL_PRECISION_F64 (default; strict parity), f32 = GL_PRECISION_F32")
-    ap.add_argument("--stage", default="grad", choices=["grad", "map"],
-                    help="grad: one gl_logpost_grad call per step (the headline); map: one fused gl_map_step (Adam) per step")
+    ap.add_argument("--stage", default="grad", choices=["grad", "map", "svi", "hmc"],
+                    help="grad: one gl_logpost_grad call per step (the headline); map / svi / hmc: one fused gl_map_step (Adam), "
+                         "gl_svi_step (AdaBelief) or gl_hmc_step (4 leapfrog steps) per step")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -240,17 +241,72 @@ def run_ours(a):
     ws_bytes = gl.gl_workspace_bytes(m.h, P)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # 256 MiB > 126 MB L2
 
-    if a.stage == "map":
+    # ---- the timed call of each stage (device-resident inputs) and its host-buffer form (pinned copies inside)
+    evals_per_particle = 1
+    pin = lambda t: t.cpu().pin_memory()
+    if a.stage == "grad":
+        zh = torch.from_numpy(wl.params).pin_memory()
+        lph = torch.empty(P, dtype=torch.float32).pin_memory()
+        gh = torch.empty((P, n_p), dtype=torch.float32).pin_memory()
+        h2d_bytes, d2h_bytes = zh.numel() * 4, (lph.numel() + gh.numel()) * 4
+
+        def step():
+            gl.gl_logpost_grad(m.h, m.obs, m.noise_sigma, m.psf, z, sid, lp, g, ws)
+
+        def step_host():
+            gl.gl_logpost_grad_host(m.h, m.obs, m.noise_sigma, m.psf, zh, sid, lph, gh, ws)
+    elif a.stage == "map":                                   # NEXT-1: fused gradient + Adam update; logp read back
         zm, om, ov = z.clone(), torch.zeros_like(z), torch.zeros_like(z)
         adam = dict(kind=gl.GL_OPT_ADAM, lr=1e-3, b1=0.9, b2=0.999, eps=1e-8, eps_root=0.0)
         tstep = [0]
+        lph = torch.empty(P, dtype=torch.float32).pin_memory()
+        h2d_bytes, d2h_bytes = 0, lph.numel() * 4
 
-    def step():
-        if a.stage == "map":
+        def step():
             tstep[0] += 1
             gl.gl_map_step(m.h, adam, m.obs, m.noise_sigma, m.psf, zm, sid, om, ov, tstep[0], lp, g, ws)
-        else:
-            gl.gl_logpost_grad(m.h, m.obs, m.noise_sigma, m.psf, z, sid, lp, g, ws)
+
+        def step_host():
+            step(); lph.copy_(lp, non_blocking=True)
+    elif a.stage == "svi":                                   # NEXT-2: P draws of one surrogate; xi in, loss out
+        if sp.n_systems != 1:
+            raise SystemExit("--stage svi needs a single-system config")
+        nt = n_p * (n_p + 1) // 2
+        mu = torch.from_numpy(wl.truth_z[0].copy()).to(dev)
+        lt = torch.zeros(nt, device=dev); lt[torch.arange(n_p, device=dev) * (torch.arange(n_p, device=dev) + 3) // 2] = 0.01
+        sm, sv, stats = torch.zeros(n_p + nt, device=dev), torch.zeros(n_p + nt, device=dev), torch.zeros(2, device=dev)
+        xi = torch.randn((P, n_p), device=dev, generator=torch.Generator(device=dev).manual_seed(1))
+        xih, statsh = pin(xi), torch.empty(2).pin_memory()
+        belief = dict(kind=gl.GL_OPT_ADABELIEF, lr=1e-4, b1=0.95, b2=0.99, eps=1e-16, eps_root=1e-16)
+        ws = torch.empty(gl.gl_svi_workspace_bytes(m.h, P), dtype=torch.uint8, device=dev)
+        tstep = [0]
+        h2d_bytes, d2h_bytes = xih.numel() * 4, 8
+
+        def step():
+            tstep[0] += 1
+            gl.gl_svi_step(m.h, belief, m.obs, m.noise_sigma, m.psf, mu, lt, xi, sid, sm, sv, tstep[0], stats, ws)
+
+        def step_host():
+            xi.copy_(xih, non_blocking=True); step(); statsh.copy_(stats, non_blocking=True)
+    else:                                                    # NEXT-3: P chains, one transition of 4 leapfrog steps
+        n_leap = 4
+        evals_per_particle = n_leap
+        zc = z.clone()
+        gl.gl_logpost_grad(m.h, m.obs, m.noise_sigma, m.psf, zc, sid, lp, g, ws)
+        lpc, gc = lp.clone(), g.clone()
+        gen = torch.Generator(device=dev).manual_seed(2)
+        xi = torch.randn((P, n_p), device=dev, generator=gen)
+        lu = torch.log(torch.rand(P, device=dev, generator=gen))
+        acc, dh = torch.zeros(P, dtype=torch.int32, device=dev), torch.zeros(P, device=dev)
+        xih, luh, acch = pin(xi), pin(lu), torch.empty(P, dtype=torch.int32).pin_memory()
+        ws = torch.empty(gl.gl_hmc_workspace_bytes(m.h, P), dtype=torch.uint8, device=dev)
+        h2d_bytes, d2h_bytes = (xih.numel() + luh.numel()) * 4, acch.numel() * 4
+
+        def step():
+            gl.gl_hmc_step(m.h, m.obs, m.noise_sigma, m.psf, zc, lpc, gc, None, xi, lu, sid, 2e-5, n_leap, acc, dh, ws)
+
+        def step_host():
+            xi.copy_(xih, non_blocking=True); lu.copy_(luh, non_blocking=True); step(); acch.copy_(acc, non_blocking=True)
 
     for _ in range(max(a.warmup, 3)):
         step()
@@ -264,14 +320,7 @@ def run_ours(a):
         e0.record(); step(); e1.record()
     barrier()
     t_dev = sum(e0.elapsed_time(e1) for e0, e1 in ev) * 1e-3
-    # e2e: host buffers through the C ABI, copies inside the timed region
-    zh = torch.from_numpy(wl.params).pin_memory()
-    lph = torch.empty(P, dtype=torch.float32).pin_memory()
-    gh = torch.empty((P, n_p), dtype=torch.float32).pin_memory()
-
-    def step_host():
-        gl.gl_logpost_grad_host(m.h, m.obs, m.noise_sigma, m.psf, zh, sid, lph, gh, ws)
-
+    # e2e: host buffers (pinned), copies inside the timed region
     for _ in range(3):
         step_host()
     barrier()
@@ -285,6 +334,8 @@ def run_ours(a):
     t_e2e = sum(e0.elapsed_time(e1) for e0, e1 in ev2) * 1e-3
     if a.stage == "grad":
         assert torch.equal(lph, lp.cpu()) and torch.equal(gh, g.cpu()), "host-buffer path disagrees with the device path"
+    if a.stage == "hmc":
+        lp = lpc
     finite = float(torch.isfinite(lp).float().mean())
 
     # dominant-kernel roofline: per-stage device time from the library's own CUDA events on the launching stream
@@ -329,19 +380,19 @@ def run_ours(a):
             "algorithmic_laneops_per_eval": wm.get(dom, 0),
             "stage_ms": {s: round(v, 4) for s, v in stage_ms.items()},
             "stage_share": {s: round(v / max(sum(stage_ms.values()), 1e-12), 4) for s, v in stage_ms.items()},
-            "step_frac": wm["total_fwd_grad"] * P * a.steps / t_dev / 1e12 / peak,
+            "step_frac": wm["total_fwd_grad"] * P * evals_per_particle * a.steps / t_dev / 1e12 / peak,
             "step_algorithmic_laneops_per_eval": wm["total_fwd_grad"]}
     if clocks.get("sm_mhz"):
         roof["frac_at_measured_clock"] = achieved / (N_SM * lanes * clocks["sm_mhz"] * 1e6 / 1e12)
-    out = {"metric": METRIC, "value": whole_job_rate(world, P, a.steps, t_dev), "unit": UNIT, "n_gpus": world, "steps": a.steps,
+    out = {"metric": METRIC, "value": whole_job_rate(world, P * evals_per_particle, a.steps, t_dev), "unit": UNIT, "n_gpus": world, "steps": a.steps,
            "warmup": max(a.warmup, 3), "ms_per_step": t_dev / a.steps * 1e3, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": a.precision, "data": "synthetic",
            "config": {"workload": WORKLOAD_NAMES[k], "n_particles_per_gpu": P, "n_params": n_p,
                       "rays_per_particle": wm["rays"], "parallelism": "replicas x%d" % world, "stage": a.stage,
                       "l2": "256 MiB flush write between timed iterations; workspace %.0f MB" % (ws_bytes / 1e6),
                       "finite_fraction": finite},
-           "e2e": {"value": whole_job_rate(world, P, a.steps, t_e2e), "unit": UNIT, "h2d_bytes_per_step": int(zh.numel() * 4),
-                   "d2h_bytes_per_step": int((lph.numel() + gh.numel()) * 4), "ms_per_step": t_e2e / a.steps * 1e3},
+           "e2e": {"value": whole_job_rate(world, P * evals_per_particle, a.steps, t_e2e), "unit": UNIT, "h2d_bytes_per_step": int(h2d_bytes),
+                   "d2h_bytes_per_step": int(d2h_bytes), "ms_per_step": t_e2e / a.steps * 1e3},
            "gpu_launches": launches_per_step * a.steps, "clocks": clocks, "roofline": roof}
     if not a.no_cpu_baseline:
         rate, cores, sample, _ = oracle_rate(k, a.cpu_seconds)
