@@ -26,7 +26,7 @@ class _Config(C.Structure):
                 ("mass_model", C.c_int32), ("epl_terms", C.c_int32), ("has_shear", C.c_int32),
                 ("multipole_mask", C.c_int32), ("n_source_sersic", C.c_int32), ("shapelet_nmax", C.c_int32),
                 ("n_lens_sersic", C.c_int32), ("param_space", C.c_int32), ("n_systems", C.c_int32),
-                ("n_params", C.c_int32), ("priors", C.POINTER(_Prior))]
+                ("n_params", C.c_int32), ("psf_grid", C.c_int32), ("priors", C.POINTER(_Prior))]
 
 
 _lib = None
@@ -56,6 +56,8 @@ def lib():
         L.glo_ray_coord.argtypes = [C.POINTER(_Config), C.c_int]
         L.glo_conv_bin.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, dp, dp, dp]
         L.glo_conv_bin_transpose.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, dp, dp, dp]
+        L.glo_bin_conv.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, dp, dp, dp]
+        L.glo_bin_conv_transpose.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, dp, dp, dp]
         L.glo_num_threads.restype = C.c_int
         L.glo_set_num_threads.argtypes = [C.c_int]
         _lib = L
@@ -78,7 +80,7 @@ def _make_config(spec, epl_terms=None, param_space=None):
                   0 if epl_terms is None else int(epl_terms), spec.has_shear, spec.multipole_mask,
                   spec.n_source_sersic, spec.shapelet_nmax, spec.n_lens_sersic,
                   spec.param_space if param_space is None else int(param_space),
-                  spec.n_systems, spec.n_params, pri)
+                  spec.n_systems, spec.n_params, int(getattr(spec, "psf_grid", 0)), pri)
     cfg._keep = pri
     return cfg
 
@@ -132,6 +134,7 @@ def model_image(spec, psf, theta, epl_terms=None, system_id=None):
     s = _S(); s.__dict__.update({k: getattr(spec, k) for k in (
         "n_pix supersample psf_size pix_scale mass_model epl_terms has_shear multipole_mask n_source_sersic "
         "shapelet_nmax n_lens_sersic n_systems n_params").split()})
+    s.psf_grid = int(getattr(spec, "psf_grid", 0))
     s.param_space = 1
     s.priors = [(PRIOR_NONE, 0, 1, 0, 1)] * spec.n_params
     out = logpost_grad(s, obs, sig, psf, theta, system_id, want_grad=False, want_model=True, epl_terms=epl_terms)
@@ -211,6 +214,19 @@ def ray_coord(spec, idx):
 def conv_bin(n_pix, s, K, pix_scale, psf, ray):
     psf = _f64(psf); ray = _f64(ray); out = np.empty((n_pix, n_pix))
     lib().glo_conv_bin(n_pix, s, K, float(pix_scale), _dp(psf), _dp(ray), _dp(out))
+    return out
+
+
+def bin_conv(n_pix, s, K, pix_scale, psf, ray):
+    """psf_grid = 1: bin to detector pixels, then convolve with the PSF sampled at the pixel scale."""
+    psf = _f64(psf); ray = _f64(ray); out = np.empty((n_pix, n_pix))
+    lib().glo_bin_conv(n_pix, s, K, float(pix_scale), _dp(psf), _dp(ray), _dp(out))
+    return out
+
+
+def bin_conv_transpose(n_pix, s, K, pix_scale, psf, g):
+    psf = _f64(psf); g = _f64(g); M = n_pix * s; out = np.empty((M, M))
+    lib().glo_bin_conv_transpose(n_pix, s, K, float(pix_scale), _dp(psf), _dp(g), _dp(out))
     return out
 
 

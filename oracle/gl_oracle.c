@@ -53,6 +53,8 @@ typedef struct {
     int32_t param_space;     /* 0: z (bijector + log-det); 1: physical theta */
     int32_t n_systems;
     int32_t n_params;
+    int32_t psf_grid;        /* 0: PSF taps on the RAY grid, convolve then bin (S10); 1: taps on the DETECTOR grid,
+                                bin then convolve (reading S10b) */
     const glo_prior* priors;
 } glo_config;
 
@@ -456,6 +458,42 @@ static void conv_bin_transpose(int n_pix, int s, int K, double pix_scale, const 
     free(gC);
 }
 
+/* psf_grid = 1 (reading S10b): bin first, B = Delta^2 * (s x s mean of I_ray), then a true convolution of the N x N
+ * image B with the K x K PSF sampled at the DETECTOR pixel scale, zero padding. */
+void glo_bin_conv(int n_pix, int s, int K, double pix_scale, const double* psf, const double* ray, double* model) {
+    int M = n_pix * s, c = (K - 1) / 2;
+    double* B = (double*)malloc(sizeof(double) * (size_t)n_pix * n_pix);
+    for (int p = 0; p < n_pix; ++p) for (int q = 0; q < n_pix; ++q) {
+        double acc = 0.0;
+        for (int di = 0; di < s; ++di) for (int dj = 0; dj < s; ++dj) acc += ray[(s * p + di) * M + s * q + dj];
+        B[p * n_pix + q] = pix_scale * pix_scale * acc / (s * s);
+    }
+    for (int p = 0; p < n_pix; ++p) for (int q = 0; q < n_pix; ++q) {
+        double acc = 0.0;
+        for (int a = 0; a < K; ++a) { int pp = p - (a - c); if (pp < 0 || pp >= n_pix) continue;
+            for (int bb = 0; bb < K; ++bb) { int qq = q - (bb - c); if (qq < 0 || qq >= n_pix) continue;
+                acc += psf[a * K + bb] * B[pp * n_pix + qq]; } }
+        model[p * n_pix + q] = acc;
+    }
+    free(B);
+}
+
+/* Transpose of glo_bin_conv, as the literal scatter. */
+void glo_bin_conv_transpose(int n_pix, int s, int K, double pix_scale, const double* psf, const double* g, double* gbar) {
+    int M = n_pix * s, c = (K - 1) / 2;
+    double* gB = (double*)calloc((size_t)n_pix * n_pix, sizeof(double));
+    for (int p = 0; p < n_pix; ++p) for (int q = 0; q < n_pix; ++q) {
+        double gv = g[p * n_pix + q];
+        for (int a = 0; a < K; ++a) { int pp = p - (a - c); if (pp < 0 || pp >= n_pix) continue;
+            for (int bb = 0; bb < K; ++bb) { int qq = q - (bb - c); if (qq < 0 || qq >= n_pix) continue;
+                gB[pp * n_pix + qq] += psf[a * K + bb] * gv; } }
+    }
+    for (int p = 0; p < n_pix; ++p) for (int q = 0; q < n_pix; ++q)
+        for (int di = 0; di < s; ++di) for (int dj = 0; dj < s; ++dj)
+            gbar[(s * p + di) * M + s * q + dj] = pix_scale * pix_scale * gB[p * n_pix + q] / (s * s);
+    free(gB);
+}
+
 /* ---------------------------------------------------------------- per-particle evaluation ------- */
 static int theta_valid(const glo_config* c, const layout_t* L, const double* th) {
     for (int i = 0; i < L->n; ++i) if (!isfinite(th[i])) return 0;
@@ -500,7 +538,8 @@ static void eval_particle(const glo_config* c, const layout_t* L, const double* 
     double* ray = (double*)malloc(sizeof(double) * (size_t)M * M);
     double* model = (double*)malloc(sizeof(double) * (size_t)N * N);
     render_rays(c, L, th, ray);
-    glo_conv_bin(N, s, c->psf_size, c->pix_scale, psf, ray, model);
+    if (c->psf_grid == 1) glo_bin_conv(N, s, c->psf_size, c->pix_scale, psf, ray, model);
+    else glo_conv_bin(N, s, c->psf_size, c->pix_scale, psf, ray, model);
     if (model_out) memcpy(model_out, model, sizeof(double) * (size_t)N * N);
     double chi2 = 0.0, slog = 0.0;
     for (int p = 0; p < N * N; ++p) { double r = (model[p] - obs[p]) / sig[p]; chi2 += r * r; slog += log(sig[p]); }
@@ -513,7 +552,8 @@ static void eval_particle(const glo_config* c, const layout_t* L, const double* 
         double* g = (double*)malloc(sizeof(double) * (size_t)N * N);
         double* gbar = (double*)malloc(sizeof(double) * (size_t)M * M);
         for (int p = 0; p < N * N; ++p) g[p] = -(model[p] - obs[p]) / (sig[p] * sig[p]);
-        conv_bin_transpose(N, s, c->psf_size, c->pix_scale, psf, g, gbar);
+        if (c->psf_grid == 1) glo_bin_conv_transpose(N, s, c->psf_size, c->pix_scale, psf, g, gbar);
+        else conv_bin_transpose(N, s, c->psf_size, c->pix_scale, psf, g, gbar);
         double dL[128], dA[128], contrib[128];
         memset(dL, 0, sizeof dL); memset(dA, 0, sizeof dA);
         for (int i = 0; i < M; ++i) { double y = ray_coord(c, i);

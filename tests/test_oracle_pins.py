@@ -414,3 +414,46 @@ def test_batch_composition_invariance():
     t = oracle.logpost_grad(sp, obs, sig, wl.psf, wl.truth_z.astype(np.float64), want_model=True)
     chi2 = (((t["model"][0] - obs[0]) / sig[0]) ** 2).sum()
     assert abs(chi2 / sp.n_pix ** 2 - 1) < 0.15
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-4: detector-grid PSF
+def test_bin_conv_detector_grid_pins():
+    """psf_grid = 1 (bin, then convolve at the pixel scale): equals scipy's zero-padded convolution of the binned image;
+    coincides with the ray-grid operator at s = 1; a delta PSF gives the plain binned image; a shifted delta moves the
+    image by one DETECTOR pixel; flux of an interior source is conserved; the transpose is the adjoint."""
+    from scipy.signal import convolve2d
+    rng = np.random.default_rng(42)
+    N, s, K, D = 9, 3, 5, 0.2
+    ray = rng.random((N * s, N * s)); psf = rng.random((K, K)); psf /= psf.sum()
+    binned = D * D * ray.reshape(N, s, N, s).mean(axis=(1, 3))
+    got = oracle.bin_conv(N, s, K, D, psf, ray)
+    assert np.allclose(got, convolve2d(binned, psf, mode="same"), rtol=1e-13, atol=1e-15)
+    ray1 = rng.random((N, N))
+    assert np.allclose(oracle.bin_conv(N, 1, K, D, psf, ray1), oracle.conv_bin(N, 1, K, D, psf, ray1), rtol=1e-13)
+    delta = np.zeros((K, K)); delta[2, 2] = 1.0
+    assert np.allclose(oracle.bin_conv(N, s, K, D, delta, ray), binned, rtol=1e-14)
+    sh = np.zeros((K, K)); sh[3, 2] = 1.0                                  # tap (c+1, c): +1 row
+    moved = oracle.bin_conv(N, s, K, D, sh, ray)
+    assert np.allclose(moved[1:], binned[:-1], rtol=1e-14) and np.allclose(moved[0], 0.0)
+    src = np.zeros_like(ray); src[12:15, 12:15] = rng.random((3, 3))       # interior: nothing leaves the cutout
+    assert np.isclose(oracle.bin_conv(N, s, K, D, psf, src).sum(), D * D * src.sum() / (s * s), rtol=1e-13)
+    g = rng.standard_normal((N, N))
+    assert np.isclose((oracle.bin_conv(N, s, K, D, psf, ray) * g).sum(),
+                      (oracle.bin_conv_transpose(N, s, K, D, psf, g) * ray).sum(), rtol=1e-12)
+
+
+def test_detector_grid_gradient_vs_finite_differences():
+    """Full log-posterior gradient with psf_grid = 1 against central differences (every parameter, tiny grid)."""
+    import dataclasses
+    sp = dataclasses.replace(W.make_spec(2), n_pix=8, supersample=2, psf_size=3, psf_grid=1)
+    rng = np.random.default_rng(6)
+    psf = W.gaussian_psf(3, 0.4, sp.pix_scale)[None]
+    z = W.z_of(sp.priors, W.draw(rng, sp.priors, 2))
+    obs = rng.random((1, 8, 8)); sig = np.full((1, 8, 8), 0.3)
+    r = oracle.logpost_grad(sp, obs, sig, psf, z)
+    for j in range(sp.n_params):
+        h = 1e-6 * max(1.0, abs(z[0, j]))
+        zp, zm = z.copy(), z.copy(); zp[:, j] += h; zm[:, j] -= h
+        fd = (oracle.logpost_grad(sp, obs, sig, psf, zp, want_grad=False)["logp"] -
+              oracle.logpost_grad(sp, obs, sig, psf, zm, want_grad=False)["logp"]) / (2 * h)
+        assert np.allclose(fd, r["grad"][:, j], rtol=2e-5, atol=1e-6 * np.abs(r["grad"]).max()), j

@@ -48,6 +48,7 @@ class LensSpec:
     n_lens_sersic: int = 1
     param_space: int = 0         # 0 unconstrained z, 1 physical theta
     n_systems: int = 1
+    psf_grid: int = 0            # 0: PSF taps on the ray grid (S10); 1: on the detector grid (NEXT-4, S10b)
     precision: int = 0           # 0 GL_PRECISION_F64, 1 GL_PRECISION_F32 (CUDA path only; the oracle is always fp64)
     priors: list = field(default_factory=list)
     names: list = field(default_factory=list)
