@@ -77,9 +77,10 @@ typedef enum { GL_PRECISION_F64 = 0, GL_PRECISION_F32 = 1 } gl_precision;
 typedef struct {
     int32_t n_pix;            /* N: detector pixels per side, >= 1 */
     int32_t supersample;      /* s: rays per pixel per side, >= 1 */
-    int32_t psf_size;         /* K: PSF taps per side on the RAY grid, odd (S10) */
+    int32_t psf_size;         /* K: PSF taps per side, odd: on the RAY grid (psf_grid 0) or the DETECTOR grid (psf_grid 1) */
     float   pix_scale;        /* Delta: arcsec per detector pixel, > 0 */
-    int32_t psf_grid;         /* 0: taps on the ray grid, convolve then bin (S10). Other values: GL_ERR_UNSUPPORTED */
+    int32_t psf_grid;         /* 0: taps on the ray grid, convolve then bin (S10); 1: taps on the detector grid, bin then
+                                 convolve (NEXT-4, S10b).  Other values: GL_ERR_UNSUPPORTED */
     int32_t mass_model;       /* 0 SIE closed form, 1 EPL series */
     int32_t epl_terms;        /* number of series terms kept for EPL, 2..30 (S5; BASELINE.json: 30) */
     int32_t has_shear;        /* 0/1 */

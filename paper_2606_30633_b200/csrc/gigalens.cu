@@ -140,7 +140,7 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     if (d->shapelet_nmax >= 0 && d->n_source_sersic != 1) return GL_ERR_BAD_CONFIG;
     if (d->n_systems < 1) return GL_ERR_BAD_CONFIG;
     if (d->precision != GL_PRECISION_F64 && d->precision != GL_PRECISION_F32) return GL_ERR_BAD_CONFIG;
-    if (d->psf_grid != 0) return GL_ERR_UNSUPPORTED;
+    if (d->psf_grid != 0 && d->psf_grid != 1) return GL_ERR_UNSUPPORTED;
     Layout L{};
     int np = layout_from_desc(*d, L);
     if (np != d->n_params || np > 128) return GL_ERR_BAD_CONFIG;
@@ -171,8 +171,12 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     else { c->variant = 2; L.ker_nmax = 10; c->na = NA_SHA + 66; }
     c->L = L;
     Geom& G = c->G;
-    G.N = d->n_pix; G.s = d->supersample; G.M = (int)M64; G.K = d->psf_size; G.c = (d->psf_size - 1) / 2;
-    const int KE = G.K + G.s - 1;
+    G.N = d->n_pix; G.s = d->supersample; G.M = (int)M64; G.K = d->psf_size; G.pgrid = d->psf_grid;
+    // psf_grid 1 (bin, then convolve at the pixel scale) is the same stride-s correlation with
+    // the box-expanded kernel k_eff[m][n] = psf[m / s][n / s]: s*K taps per side, half-width s*(K-1)/2
+    G.c = d->psf_grid == 1 ? G.s * ((d->psf_size - 1) / 2) : (d->psf_size - 1) / 2;
+    G.KE = d->psf_grid == 1 ? G.s * G.K : G.K + G.s - 1;
+    const int KE = G.KE;
     G.U = (KE + G.s - 1) / G.s; G.KEp = G.U * G.s;
     G.n_terms = d->mass_model == 1 ? d->epl_terms : 0;
     G.delta2 = (double)d->pix_scale * (double)d->pix_scale;

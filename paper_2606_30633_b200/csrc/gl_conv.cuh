@@ -33,7 +33,7 @@ __global__ void gl_prep_kernel(const __grid_constant__ Geom G, const float* __re
                                double* __restrict__ math_tab_out) {
     const int sys = blockIdx.x;
     if (sys == 0 && math_tab_out != nullptr) fill_math_tab(math_tab_out);
-    const int KE = G.K + G.s - 1, U = G.U, s = G.s;
+    const int KE = G.KE, U = G.U, s = G.s;
     const float* ps = psf + (size_t)sys * G.K * G.K;
     T* kt = sys_kt + (size_t)sys * s * s * U * U;
     for (int t = threadIdx.x; t < s * s * U * U; t += blockDim.x) {
@@ -41,8 +41,9 @@ __global__ void gl_prep_kernel(const __grid_constant__ Geom G, const float* __re
         int u = s * u1 + a, v = s * v1 + b;
         double acc = 0.0;
         if (u < KE && v < KE) {
-            int m = KE - 1 - u, n = KE - 1 - v;           // k_eff[m][n] = sum_{di,dj<s} psf[m-di][n-dj]
-            for (int di = 0; di < s; ++di) for (int dj = 0; dj < s; ++dj) {
+            int m = KE - 1 - u, n = KE - 1 - v;           // psf_grid 0: k_eff[m][n] = sum_{di,dj<s} psf[m-di][n-dj]
+            if (G.pgrid == 1) acc = (double)ps[(m / s) * G.K + n / s];     // psf_grid 1: box-expanded detector-grid taps
+            else for (int di = 0; di < s; ++di) for (int dj = 0; dj < s; ++dj) {
                 int r = m - di, cc = n - dj;
                 if (r >= 0 && r < G.K && cc >= 0 && cc < G.K) acc += (double)ps[r * G.K + cc];
             }

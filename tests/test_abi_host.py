@@ -55,7 +55,7 @@ def test_config_create_and_param_count(gl, k, n_params):
     ("psf_size", 10, -2), ("supersample", 0, -2), ("n_pix", 0, -2), ("pix_scale", 0.0, -2), ("mass_model", 2, -2),
     ("epl_terms", 31, -2), ("epl_terms", 1, -2), ("n_lens_sersic", 3, -2), ("shapelet_nmax", 11, -2),
     ("n_systems", 0, -2), ("precision", 2, -2), ("param_space", 2, -2), ("multipole_mask", 4, -2),
-    ("psf_grid", 1, -4), ("n_pix", 5000, -4)])
+    ("psf_grid", 2, -4), ("n_pix", 5000, -4)])
 def test_config_validation(gl, field, value, status):
     sp = W.make_spec(2)
     if field == "psf_grid":

@@ -216,7 +216,8 @@ def test_determinism_repeat_calls():
     assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
 
 
-def _small_case(n_pix, s, K, mass_model, multipole_mask, shapelet_nmax, n_lens, seed, n_particles=6, epl_terms=30):
+def _small_case(n_pix, s, K, mass_model, multipole_mask, shapelet_nmax, n_lens, seed, n_particles=6, epl_terms=30,
+                psf_grid=0):
     """A seeded small problem of arbitrary shape: spec with config-style priors, Gaussian PSF, oracle-rendered truth."""
     import oracle
     pri = W._default_priors(mass_model, multipoles=bool(multipole_mask), shapelet_nmax=shapelet_nmax, n_lens=n_lens)
@@ -225,11 +226,12 @@ def _small_case(n_pix, s, K, mass_model, multipole_mask, shapelet_nmax, n_lens, 
         k0 = 1 + (1 if mass_model == 1 else 0) + 4 + 2
         pri = pri[:k0] + pri[k0 + 2:]
     sp = W.LensSpec(n_pix, s, K, W._r32(0.11 * 40 / n_pix * 2.4), mass_model=mass_model, epl_terms=epl_terms,
-                    multipole_mask=multipole_mask, shapelet_nmax=shapelet_nmax, n_lens_sersic=n_lens, priors=pri)
+                    multipole_mask=multipole_mask, shapelet_nmax=shapelet_nmax, n_lens_sersic=n_lens, psf_grid=psf_grid,
+                    priors=pri)
     sp.names = W.param_names(mass_model, 1, multipole_mask, 1, shapelet_nmax, n_lens)
     assert len(sp.names) == sp.n_params
     rng = np.random.default_rng(seed)
-    step = sp.pix_scale / s
+    step = sp.pix_scale / s if psf_grid == 0 else sp.pix_scale      # taps at ray spacing (S10) or pixel spacing (S10b)
     psf = W.gaussian_psf(K, 2.5 * step, step)[None].astype(np.float32)
     truth_z = W.z_of(pri, W.draw(rng, pri, 1)).astype(np.float32)
     truth = oracle.model_image(sp, psf.astype(np.float64), W.theta_of(pri, truth_z.astype(np.float64)))
@@ -285,3 +287,27 @@ def test_truncated_series_matches_truncated_oracle():
     ok, rep = grad_report(g, ref8["grad"])
     assert rep["n_fail"] == 0, rep
     assert np.max(np.abs(refc["logp"] - ref8["logp"]) / np.abs(refc["logp"])) > 1e-6      # the truncation is visible
+
+
+@pytest.mark.parametrize("shape", [(12, 2, 5), (14, 4, 11), (16, 2, 11), (9, 3, 3), (10, 1, 7)])
+def test_detector_grid_psf_strict_parity(shape):
+    """SURVEY 8(f) NEXT-4, psf_grid = 1 (bin, then convolve with a PSF sampled at the pixel scale): the CUDA path runs it
+    as the same stride-s correlation with the box-expanded kernel; strict bar against the oracle's literal
+    bin-then-convolve, model image included.  (14,4,11) and (16,2,11) take the tuned U = 11 kernels, the rest the generic."""
+    import oracle
+    import torch
+    gl = _gl()
+    n_pix, s, K = shape
+    sp, obs, sigma, psf, z = _small_case(n_pix, s, K, 1, 0, -1, 1, seed=500 + n_pix, psf_grid=1)
+    ref = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), None, want_model=True)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    zt = torch.from_numpy(z).cuda()
+    lp, g = m.logpost_grad(zt)
+    img = m.model_image(zt).cpu().numpy().astype(np.float64)
+    lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+    fin = np.isfinite(ref["logp"])
+    assert fin.sum() >= 4 and np.array_equal(fin, np.isfinite(lp))
+    assert np.max(np.abs(img[fin] - ref["model"][fin]) / np.abs(ref["model"][fin]).max(axis=(1, 2), keepdims=True)) < 2e-7
+    assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+    ok, rep = grad_report(g[fin], ref["grad"][fin])
+    assert rep["n_fail"] == 0, rep
