@@ -26,7 +26,8 @@ class _Config(C.Structure):
                 ("mass_model", C.c_int32), ("epl_terms", C.c_int32), ("has_shear", C.c_int32),
                 ("multipole_mask", C.c_int32), ("n_source_sersic", C.c_int32), ("shapelet_nmax", C.c_int32),
                 ("n_lens_sersic", C.c_int32), ("param_space", C.c_int32), ("n_systems", C.c_int32),
-                ("n_params", C.c_int32), ("psf_grid", C.c_int32), ("priors", C.POINTER(_Prior))]
+                ("n_params", C.c_int32), ("psf_grid", C.c_int32), ("noise_model", C.c_int32), ("t_exp", C.c_double),
+                ("priors", C.POINTER(_Prior))]
 
 
 _lib = None
@@ -80,7 +81,8 @@ def _make_config(spec, epl_terms=None, param_space=None):
                   0 if epl_terms is None else int(epl_terms), spec.has_shear, spec.multipole_mask,
                   spec.n_source_sersic, spec.shapelet_nmax, spec.n_lens_sersic,
                   spec.param_space if param_space is None else int(param_space),
-                  spec.n_systems, spec.n_params, int(getattr(spec, "psf_grid", 0)), pri)
+                  spec.n_systems, spec.n_params, int(getattr(spec, "psf_grid", 0)),
+                  int(getattr(spec, "noise_model", 0)), float(getattr(spec, "t_exp", 1.0)), pri)
     cfg._keep = pri
     return cfg
 

@@ -55,6 +55,9 @@ typedef struct {
     int32_t n_params;
     int32_t psf_grid;        /* 0: PSF taps on the RAY grid, convolve then bin (S10); 1: taps on the DETECTOR grid,
                                 bin then convolve (reading S10b) */
+    int32_t noise_model;     /* 0: fixed sigma map (S12); 1: model-dependent variance
+                                v_p = sigma_p^2 + max(model_p, 0) / t_exp (NEXT-4, reading S12b) */
+    double  t_exp;           /* exposure time of noise_model 1 (> 0) */
     const glo_prior* priors;
 } glo_config;
 
@@ -542,7 +545,15 @@ static void eval_particle(const glo_config* c, const layout_t* L, const double* 
     else glo_conv_bin(N, s, c->psf_size, c->pix_scale, psf, ray, model);
     if (model_out) memcpy(model_out, model, sizeof(double) * (size_t)N * N);
     double chi2 = 0.0, slog = 0.0;
-    for (int p = 0; p < N * N; ++p) { double r = (model[p] - obs[p]) / sig[p]; chi2 += r * r; slog += log(sig[p]); }
+    if (c->noise_model == 1) {
+        /* S12b: Gaussian likelihood whose variance follows the MODEL: v = sigma_bkg^2 + max(model, 0) / t_exp;
+         * log L = -1/2 sum [ (model - obs)^2 / v + ln v ] - (N^2/2) ln 2 pi */
+        for (int p = 0; p < N * N; ++p) {
+            double v = sig[p] * sig[p] + (model[p] > 0 ? model[p] : 0.0) / c->t_exp, r = model[p] - obs[p];
+            chi2 += r * r / v; slog += 0.5 * log(v);
+        }
+    } else
+        for (int p = 0; p < N * N; ++p) { double r = (model[p] - obs[p]) / sig[p]; chi2 += r * r; slog += log(sig[p]); }
     double logL = -0.5 * chi2 - slog - 0.5 * N * N * log(2.0 * GLO_PI);
     double lpv = logL + lp_sum + ld_sum;
     if (!isfinite(lpv)) { *logp = -INFINITY; if (grad) memset(grad, 0, sizeof(double) * (size_t)n);
@@ -551,7 +562,14 @@ static void eval_particle(const glo_config* c, const layout_t* L, const double* 
     if (grad) {
         double* g = (double*)malloc(sizeof(double) * (size_t)N * N);
         double* gbar = (double*)malloc(sizeof(double) * (size_t)M * M);
-        for (int p = 0; p < N * N; ++p) g[p] = -(model[p] - obs[p]) / (sig[p] * sig[p]);
+        if (c->noise_model == 1)
+            for (int p = 0; p < N * N; ++p) {   /* d logL / d model with v' = [model > 0] / t_exp */
+                double vp = model[p] > 0 ? 1.0 / c->t_exp : 0.0;
+                double v = sig[p] * sig[p] + (model[p] > 0 ? model[p] : 0.0) / c->t_exp, r = model[p] - obs[p];
+                g[p] = -r / v + 0.5 * r * r / (v * v) * vp - 0.5 * vp / v;
+            }
+        else
+            for (int p = 0; p < N * N; ++p) g[p] = -(model[p] - obs[p]) / (sig[p] * sig[p]);
         if (c->psf_grid == 1) glo_bin_conv_transpose(N, s, c->psf_size, c->pix_scale, psf, g, gbar);
         else conv_bin_transpose(N, s, c->psf_size, c->pix_scale, psf, g, gbar);
         double dL[128], dA[128], contrib[128];

@@ -50,20 +50,23 @@ static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems) {
     int ps = U * ((U + 1) & ~1);
     if (LS > 1) while ((2 * ps) % 32 != 8 && (2 * ps) % 32 != 24) ps += 2;   // 4 consecutive planes -> disjoint bank groups
     const int nt_max = 256;                 // launch bounds of the compiled specialisations
-    auto mk = [&](int ncg) {
+    auto mk = [&](int ncg, int cta_f64) {
         SlidePlan sp{};
         sp.ncg = ncg; sp.tpp = LS > 1 ? round_up(LS * ncg, 32) : ncg; sp.ps = ps; sp.shared_taps = n_systems == 1 ? 1 : 0;
         // particles per CTA: the count (<= 8) that wastes the fewest lanes of a CTA of at most GL_CONV_CTA threads
         sp.ppc = 1; double best = 0;
         for (int k = 1; k <= 8; ++k) {
             const int nt = round_up(k * sp.tpp, 32);
-            if (nt > ((LS > 1 || esize == 8) ? GL_CONV_CTA : 256) && k > 1) break;   // fp32, LS = 1: registers allow the fullest CTA up to 256
+            if (nt > (LS > 1 ? GL_CONV_CTA : (esize == 8 ? cta_f64 : 256)) && k > 1) break;   // LS = 1: the fullest CTA the registers allow
             const double eff = (double)(k * LS * ncg) / nt;
             if (eff > best + 1e-9) { best = eff; sp.ppc = k; }
         }
         return sp;
     };
-    pl.fwd = mk(ncg_f); pl.bwd = mk(ncg_b);
+#ifndef GL_CONV_CTA_BWD64
+#define GL_CONV_CTA_BWD64 160
+#endif
+    pl.fwd = mk(ncg_f, GL_CONV_CTA); pl.bwd = mk(ncg_b, GL_CONV_CTA_BWD64);   // fp64: 220 / 168 registers per thread at U = 16
     pl.fwd_smem = (size_t)esize * (pl.fwd.shared_taps ? 1 : pl.fwd.ppc) * NPH * ps;
     pl.bwd_smem = (size_t)esize * (pl.bwd.shared_taps ? 1 : pl.bwd.ppc) * NPH * ps;
     pl.n_ctile = 1;

@@ -457,3 +457,42 @@ def test_detector_grid_gradient_vs_finite_differences():
         fd = (oracle.logpost_grad(sp, obs, sig, psf, zp, want_grad=False)["logp"] -
               oracle.logpost_grad(sp, obs, sig, psf, zm, want_grad=False)["logp"]) / (2 * h)
         assert np.allclose(fd, r["grad"][:, j], rtol=2e-5, atol=1e-6 * np.abs(r["grad"]).max()), j
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-4: model-dependent variance
+def _noise_case(noise_model, t_exp):
+    import dataclasses
+    sp = dataclasses.replace(W.make_spec(2), n_pix=8, supersample=2, psf_size=3, noise_model=noise_model, t_exp=t_exp)
+    rng = np.random.default_rng(16)
+    psf = W.gaussian_psf(3, 0.4, sp.pix_scale / 2)[None]
+    z = W.z_of(sp.priors, W.draw(rng, sp.priors, 3))
+    obs = 0.5 * rng.random((1, 8, 8)); sig = np.full((1, 8, 8), 0.2) + 0.1 * rng.random((1, 8, 8))
+    return sp, psf, z, obs, sig
+
+
+def test_model_variance_likelihood_definition_and_limits():
+    """noise_model = 1: logL equals the written-out definition on the oracle's own model image; t_exp -> infinity gives
+    the fixed-sigma likelihood; and it differs visibly at a finite exposure."""
+    sp, psf, z, obs, sig = _noise_case(1, 50.0)
+    r = oracle.logpost_grad(sp, obs, sig, psf, z, want_grad=False, want_model=True)
+    sp0 = __import__("dataclasses").replace(sp, noise_model=0)
+    r0 = oracle.logpost_grad(sp0, obs, sig, psf, z, want_grad=False, want_model=True)
+    assert np.allclose(r["model"], r0["model"], rtol=1e-14)
+    m = r["model"]; v = sig ** 2 + np.maximum(m, 0) / 50.0
+    logL = -0.5 * (((m - obs) ** 2 / v) + np.log(v)).sum(axis=(1, 2)) - 32 * np.log(2 * np.pi)
+    logL0 = -0.5 * (((m - obs) / sig) ** 2).sum(axis=(1, 2)) - np.log(sig).sum() - 32 * np.log(2 * np.pi)
+    assert np.allclose(r["logp"] - r0["logp"], logL - logL0, rtol=1e-10)
+    assert np.all(np.abs(logL - logL0) > 1e-3 * np.abs(logL0))
+    rinf = oracle.logpost_grad(__import__("dataclasses").replace(sp, t_exp=1e30), obs, sig, psf, z, want_grad=False)
+    assert np.allclose(rinf["logp"], r0["logp"], rtol=1e-13)
+
+
+def test_model_variance_gradient_vs_finite_differences():
+    sp, psf, z, obs, sig = _noise_case(1, 50.0)
+    r = oracle.logpost_grad(sp, obs, sig, psf, z)
+    for j in range(sp.n_params):
+        h = 1e-6 * max(1.0, abs(z[0, j]))
+        zp, zm = z.copy(), z.copy(); zp[:, j] += h; zm[:, j] -= h
+        fd = (oracle.logpost_grad(sp, obs, sig, psf, zp, want_grad=False)["logp"] -
+              oracle.logpost_grad(sp, obs, sig, psf, zm, want_grad=False)["logp"]) / (2 * h)
+        assert np.allclose(fd, r["grad"][:, j], rtol=2e-5, atol=1e-6 * np.abs(r["grad"]).max()), j
