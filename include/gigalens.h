@@ -92,6 +92,10 @@ typedef struct {
     int32_t n_systems;        /* number of (obs, noise_sigma, psf) triples, >= 1 (S19) */
     int32_t n_params;         /* must equal the count implied by the fields above (<= 128) */
     int32_t precision;        /* gl_precision: 0 = GL_PRECISION_F64 (default), 1 = GL_PRECISION_F32 */
+    int32_t noise_model;      /* 0: fixed per-pixel sigma map (S12); 1: model-dependent variance (NEXT-4, S12b):
+                                 v = noise_sigma^2 + max(model, 0) / exposure_time,
+                                 logL = -1/2 sum [ (model - obs)^2 / v + ln v ] - (N^2/2) ln 2 pi */
+    float   exposure_time;    /* t_exp of noise_model 1 (> 0; ignored otherwise) */
     const gl_prior* priors;   /* HOST pointer, n_params entries, copied by gl_config_create */
 } gl_config_desc;
 

@@ -141,6 +141,8 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     if (d->n_systems < 1) return GL_ERR_BAD_CONFIG;
     if (d->precision != GL_PRECISION_F64 && d->precision != GL_PRECISION_F32) return GL_ERR_BAD_CONFIG;
     if (d->psf_grid != 0 && d->psf_grid != 1) return GL_ERR_UNSUPPORTED;
+    if (d->noise_model != 0 && d->noise_model != 1) return GL_ERR_BAD_CONFIG;
+    if (d->noise_model == 1 && !(d->exposure_time > 0.f && std::isfinite(d->exposure_time))) return GL_ERR_BAD_CONFIG;
     Layout L{};
     int np = layout_from_desc(*d, L);
     if (np != d->n_params || np > 128) return GL_ERR_BAD_CONFIG;
@@ -172,6 +174,7 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     c->L = L;
     Geom& G = c->G;
     G.N = d->n_pix; G.s = d->supersample; G.M = (int)M64; G.K = d->psf_size; G.pgrid = d->psf_grid;
+    G.noise_model = d->noise_model; G.inv_texp = d->noise_model == 1 ? 1.0 / (double)d->exposure_time : 0.0;
     // psf_grid 1 (bin, then convolve at the pixel scale) is the same stride-s correlation with
     // the box-expanded kernel k_eff[m][n] = psf[m / s][n / s]: s*K taps per side, half-width s*(K-1)/2
     G.c = d->psf_grid == 1 ? G.s * ((d->psf_size - 1) / 2) : (d->psf_size - 1) / 2;

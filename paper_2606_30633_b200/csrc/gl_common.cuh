@@ -74,6 +74,8 @@ struct Geom {            // launch-invariant geometry, passed by value
     int N, s, M, K, c;   // pixels/side, supersample, rays/side, psf taps/side, half-width of the ray-level kernel
                          // ((K-1)/2 for psf_grid 0, s*(K-1)/2 for psf_grid 1)
     int KE, pgrid;       // ray-level taps per side of the effective kernel (K+s-1 or s*K); psf_grid
+    int noise_model;     // 0 fixed sigma map, 1 variance sigma^2 + max(model,0) * inv_texp (SYS w then holds sigma^2)
+    double inv_texp;
     int KEp, U;          // padded k_eff taps per side (multiple of s), taps per phase per side
     int n_terms;         // EPL series terms kept (2..30)
     double delta2;       // pix_scale^2 (fp64 product of the fp32 pix_scale)

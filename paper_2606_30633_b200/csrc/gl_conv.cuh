@@ -56,8 +56,8 @@ __global__ void gl_prep_kernel(const __grid_constant__ Geom G, const float* __re
     T* w = sys_w + (size_t)sys * G.N * G.N;
     for (int t = threadIdx.x; sigma != nullptr && t < G.N * G.N; t += blockDim.x) {
         double sv = (double)sg[t];
-        w[t] = (T)(1.0 / (sv * sv));
-        sl += log(sv);
+        w[t] = G.noise_model == 1 ? (T)(sv * sv) : (T)(1.0 / (sv * sv));   // noise model 1: the background VARIANCE
+        sl += G.noise_model == 1 ? 0.0 : log(sv);                        // (ln v is then part of the per-pixel term)
     }
     red[threadIdx.x] = sl; __syncthreads();
     for (int o = 128; o > 0; o >>= 1) { if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o]; __syncthreads(); }
@@ -97,7 +97,15 @@ __device__ __forceinline__ T pixel_epilogue(const Geom& G, T m, int pr, int pq, 
     if (out_model) out_model[p_out * NN + pix] = (float)m;
     if (!gpix) return T(0);
     const T r = m - (T)obs[(size_t)sys * NN + pix], w = sys_w[(size_t)sys * NN + pix];
-    gpix[(size_t)p * gpix_stride(G) + (size_t)(pr + G.PADg) * G.Wg + pq + G.PADg] = -r * w;
+    T* gp = gpix + (size_t)p * gpix_stride(G) + (size_t)(pr + G.PADg) * G.Wg + pq + G.PADg;
+    if (G.noise_model == 1) {                   // S12b: v = sigma^2 + max(m, 0) / t_exp; term = r^2 / v + ln v
+        const bool pos = m > T(0);
+        const double v = (double)w + (pos ? (double)m * G.inv_texp : 0.0), iv = 1.0 / v, vp = pos ? G.inv_texp : 0.0;
+        const double rd = (double)r;
+        *gp = (T)(-rd * iv + 0.5 * rd * rd * iv * iv * vp - 0.5 * vp * iv);
+        return (T)(rd * rd * iv + log(v));
+    }
+    *gp = -r * w;
     return r * r * w;
 }
 

@@ -311,3 +311,49 @@ def test_detector_grid_psf_strict_parity(shape):
     assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
     ok, rep = grad_report(g[fin], ref["grad"][fin])
     assert rep["n_fail"] == 0, rep
+
+
+@pytest.mark.parametrize("shape", [(12, 2, 5), (9, 3, 3)])
+@pytest.mark.parametrize("precision", [0, 1])
+def test_model_variance_small_shapes(shape, precision):
+    """SURVEY 8(f) NEXT-4, noise_model = 1 (variance sigma^2 + max(model, 0)/t_exp follows the model): strict bar in
+    fp64 mode, norm-wise 1e-3 in fp32 mode."""
+    import dataclasses
+    import oracle
+    import torch
+    gl = _gl()
+    n_pix, s, K = shape
+    sp, obs, sigma, psf, z = _small_case(n_pix, s, K, 1, 0, -1, 1, seed=900 + n_pix)
+    sp = dataclasses.replace(sp, noise_model=1, t_exp=W._r32(20.0), precision=precision)
+    ref = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), None)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    lp, g = m.logpost_grad(torch.from_numpy(z).cuda())
+    lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+    fin = np.isfinite(ref["logp"])
+    assert fin.sum() >= 4 and np.array_equal(fin, np.isfinite(lp))
+    assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+    ok, rep = grad_report(g[fin], ref["grad"][fin])
+    if precision == 0:
+        assert rep["n_fail"] == 0, rep
+    else:
+        assert rep["normwise"] <= 1e-3, rep
+
+
+def test_model_variance_config2_subset():
+    """Config 2 with its 'Poisson-like variance term' taken literally as model-dependent (sigma_bkg = 0.02, t_exp = 1000)
+    instead of baked into a fixed map: 32 particles of the full batch, strict bar."""
+    import dataclasses
+    import oracle
+    gl, torch, wl, m0 = _model(2)
+    _, obs, _ = observation(2)
+    sp = dataclasses.replace(wl.spec, noise_model=1, t_exp=1000.0)
+    sig = np.full_like(obs, 0.02)
+    idx = np.arange(0, 4096, 128)
+    z = wl.params[idx]
+    ref = oracle.logpost_grad(sp, obs, sig, wl.psf, z.astype(np.float64), None)
+    m = gl.LensModel(sp, obs, sig, wl.psf)
+    lp, g = m.logpost_grad(torch.from_numpy(z).cuda())
+    lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+    assert np.all(np.isfinite(lp)) and np.all(np.abs(lp - ref["logp"]) <= RTOL_LOGP * np.abs(ref["logp"]))
+    ok, rep = grad_report(g, ref["grad"])
+    assert rep["n_fail"] == 0, rep
