@@ -77,8 +77,14 @@ extern "C" int32_t gl_stage_times(float* ms_host, int32_t* launches_host, int32_
 }
 #define GL_STAGE(id, st, ...) do { t_timer.begin(id, st); __VA_ARGS__; t_timer.end(st); } while (0)
 
-static constexpr int NT_FWD = 256;     // compiled launch bounds; the block size actually used is chosen per config
-static constexpr int NT_ADJ = 128;
+#ifndef GL_NT_FWD
+#define GL_NT_FWD 256
+#endif
+#ifndef GL_NT_ADJ
+#define GL_NT_ADJ 128
+#endif
+static constexpr int NT_FWD = GL_NT_FWD;     // compiled launch bounds; the block size actually used is chosen per config
+static constexpr int NT_ADJ = GL_NT_ADJ;
 #ifndef GL_RB_FWD
 #define GL_RB_FWD 1
 #endif

@@ -63,12 +63,12 @@ __constant__ double c_dm[20] = {
     0.5, 1.0, -1.0, 0.0,       // 15..18
     0.0};
 
-// 2^x, relative error < 2e-13.  x < -1000 returns 0; x must stay below 1000.
+// 2^x, relative error < 2e-13, for -1e8 < x < 1000; below -1021 the result saturates at ~1e-308.
 __device__ __forceinline__ double d_exp2(const MathTab& tb, double x) {
     const double kd = fma(x, c_dm[1], c_dm[0]);
     const int k = __double2loint(kd);                          // k = rint(16 x)
     const double r = fma(kd - c_dm[0], c_dm[2], x);            // x - k/16, exact
-    const int j = k & 15, n = k >> 4;
+    const int j = k & 15, n = max(k >> 4, -1021);              // x < -1021: result 2^-1021 y ~ 1e-308 (stands for 0)
     double p = c_dm[7];
     p = fma(p, r, c_dm[6]);
     p = fma(p, r, c_dm[5]);
@@ -76,9 +76,7 @@ __device__ __forceinline__ double d_exp2(const MathTab& tb, double x) {
     p = fma(p, r, c_dm[3]);
     const double t = tb.e2[j];
     const double y = fma(t * r, p, t);                         // in [0.97, 2.05)
-    const int hi = __double2hiint(y) + (n << 20);              // scale by 2^n through the exponent field (n >= -1001)
-    const bool under = (unsigned)__double2hiint(x) > 0xC08F4000u && __double2hiint(x) < 0;   // x < -1000
-    return __hiloint2double(under ? 0 : hi, under ? 0 : __double2loint(y));
+    return __hiloint2double(__double2hiint(y) + (n << 20), __double2loint(y));   // scale by 2^n through the exponent field
 }
 
 // log2(x) for normal x > 0, absolute error < 2e-13.

@@ -59,7 +59,31 @@ __device__ __forceinline__ void knuth(const T* __restrict__ cf, T p, T nf2, T wr
 //   4 M1 < k <= kt           recurrence steps in fp32 on the otherwise idle FP32 pipe: their rounding enters the sum
 //                            scaled by f^k, 30 f^(4 M1 + 1) 1e-7 <= 1e-11;
 //   k <= 4 M1                recurrence steps in T.
-// cf: K coefficient arrays of T at stride 32 (PB_SER_A / _D / _E); cf32: fp32 copies (fp64 mode only).
+// cf: K coefficient arrays of T, cf32: fp32 copies (fp64 mode only); both in the SHIFTED shared-memory layout written by
+// stage_series: coefficient idx of polynomial i sits at [SER_PITCH * i + idx + 3], so that the four coefficients
+// k-3 .. k of one 4-step group (k a multiple of 4) are one aligned 16-byte (fp32) or two aligned 16-byte (fp64) loads.
+constexpr int SER_PITCH = 36;
+
+__device__ __forceinline__ void load_coef4(const float* __restrict__ c, int k, float (&v)[4]) {   // v[j] = coef[k - j]
+    const float4 x = *reinterpret_cast<const float4*>(c + k);
+    v[0] = x.w; v[1] = x.z; v[2] = x.y; v[3] = x.x;
+}
+__device__ __forceinline__ void load_coef4(const double* __restrict__ c, int k, double (&v)[4]) {
+    const double2 lo = *reinterpret_cast<const double2*>(c + k), hi = *reinterpret_cast<const double2*>(c + k + 2);
+    v[0] = hi.y; v[1] = hi.x; v[2] = lo.y; v[3] = lo.x;
+}
+
+// Stage the K_ALL = 3 coefficient arrays of a particle (PB_SER_A / _D / _E, stride 32 in PB) into the shifted layout.
+template <class T>
+__device__ __forceinline__ void stage_series(const T* __restrict__ src, T* __restrict__ cfs, float* __restrict__ cf32) {
+    for (int e = threadIdx.x; e < 3 * SER_PITCH; e += blockDim.x) {
+        const int i = e / SER_PITCH, pos = e - i * SER_PITCH, idx = pos - 3;
+        const T v = (idx >= 0 && idx < 32) ? src[PB_SER_A + 32 * i + idx] : T(0.);
+        cfs[e] = v;
+        if constexpr (sizeof(T) == 8) cf32[e] = (float)v;
+    }
+}
+
 template <class T, int K>
 __device__ __forceinline__ void knuth_banded(const T* __restrict__ cf, const float* __restrict__ cf32, int m1, int m2,
                                              T p, T nf2, T wr, T wi, T (&Pr)[K], T (&Pi)[K]) {
@@ -72,14 +96,17 @@ __device__ __forceinline__ void knuth_banded(const T* __restrict__ cf, const flo
             const float pf = (float)p, nf = (float)nf2;
             float c1[K], c2[K];
 #pragma unroll
-            for (int i = 0; i < K; ++i) { c1[i] = cf32[32 * i + kt]; c2[i] = 0.f; }
+            for (int i = 0; i < K; ++i) { c1[i] = cf32[SER_PITCH * i + kt + 3]; c2[i] = 0.f; }
             int k = kt - 1;
             for (int g = 0; g < m2; ++g, k -= 4) {
+                float v[K][4];
+#pragma unroll
+                for (int i = 0; i < K; ++i) load_coef4(cf32 + SER_PITCH * i, k, v[i]);
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
 #pragma unroll
                     for (int i = 0; i < K; ++i) {
-                        const float bk = fmaf(pf, c1[i], fmaf(nf, c2[i], cf32[32 * i + k - j]));
+                        const float bk = fmaf(pf, c1[i], fmaf(nf, c2[i], v[i][j]));
                         c2[i] = c1[i]; c1[i] = bk;
                     }
                 }
@@ -91,22 +118,25 @@ __device__ __forceinline__ void knuth_banded(const T* __restrict__ cf, const flo
     }
     if (!seeded) {
 #pragma unroll
-        for (int i = 0; i < K; ++i) { b1[i] = cf[32 * i + kt]; b2[i] = T(0.); }
+        for (int i = 0; i < K; ++i) { b1[i] = cf[SER_PITCH * i + kt + 3]; b2[i] = T(0.); }
     }
     int k = 4 * m1;
     for (int g = 0; g < m1; ++g, k -= 4) {
+        T v[K][4];
+#pragma unroll
+        for (int i = 0; i < K; ++i) load_coef4(cf + SER_PITCH * i, k, v[i]);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
 #pragma unroll
             for (int i = 0; i < K; ++i) {
-                const T bk = R::fma(p, b1[i], R::fma(nf2, b2[i], cf[32 * i + k - j]));
+                const T bk = R::fma(p, b1[i], R::fma(nf2, b2[i], v[i][j]));
                 b2[i] = b1[i]; b1[i] = bk;
             }
         }
     }
 #pragma unroll
     for (int i = 0; i < K; ++i) {
-        const T r0 = R::fma(nf2, b2[i], cf[32 * i]);
+        const T r0 = R::fma(nf2, b2[i], cf[SER_PITCH * i + 3]);
         Pr[i] = R::fma(b1[i], wr, r0); Pi[i] = b1[i] * wi;
     }
 }
@@ -161,7 +191,8 @@ template <class T, class V> __host__ __device__ constexpr bool coef_in_smem() { 
 // Everything one ray needs.  ADJ = false: returns the surface brightness; ADJ = true: accumulates gbar * dI/d(natural).
 template <class T, class V, bool ADJ>
 __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* __restrict__ pb,
-                                      const float* __restrict__ cf32, T fj, T fi, T gbar, T* __restrict__ acc,
+                                      const T* __restrict__ cfs, const float* __restrict__ cf32, T fj, T fi, T gbar,
+                                      T* __restrict__ acc,
                                       T* __restrict__ sacc = nullptr, int sstride = 0) {
     using R = Real<T>;
     const T step = pb[PB_STEP];
@@ -182,7 +213,7 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
         const T wr = -f * c2, wi = -f * s2, p = T(2.) * wr;
         const int m1 = (int)pb[PB_SER_M1], m2 = (int)pb[PB_SER_M2];
         T Pr[ADJ ? 3 : 1], Pi[ADJ ? 3 : 1];
-        knuth_banded<T, (ADJ ? 3 : 1)>(pb + PB_SER_A, cf32, m1, m2, p, nf2, wr, wi, Pr, Pi);
+        knuth_banded<T, (ADJ ? 3 : 1)>(cfs, cf32, m1, m2, p, nf2, wr, wi, Pr, Pi);
         const T P0r = Pr[0], P0i = Pi[0];
         S0r = R::fma(ce, P0r, -se * P0i); S0i = R::fma(ce, P0i, se * P0r);
         lbr = R::fma(-T(0.5), R::lg2(tb, R2), pb[PB_M_L2B]);
@@ -399,9 +430,9 @@ __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ 
     const int p = blockIdx.y;
     const T* src = pbg + (size_t)p * PB_STRIDE;
     for (int k = threadIdx.x; k < V::PB_NEED; k += blockDim.x) pb[k] = src[k];
-    __shared__ float cf32[(sizeof(T) == 8 && V::MASS == 1) ? 96 : 4];     // fp32 copies of the series coefficients
-    if constexpr (sizeof(T) == 8 && V::MASS == 1)
-        for (int k = threadIdx.x; k < 96; k += blockDim.x) cf32[k] = (float)src[PB_SER_A + k];
+    __shared__ __align__(16) T cfs[V::MASS == 1 ? 3 * SER_PITCH : 4];                          // series coefficients, shifted layout
+    __shared__ __align__(16) float cf32[(sizeof(T) == 8 && V::MASS == 1) ? 3 * SER_PITCH : 4];  // their fp32 copies
+    if constexpr (V::MASS == 1) stage_series<T>(src, cfs, cf32);
     const typename Real<T>::Tab tb = TabStage<T>::make(tabs, tabg);
     __syncthreads();
     PlaneIter it(G, n_chunk, RPT);
@@ -424,7 +455,7 @@ __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ 
         for (int b = 0; b < RB; ++b) {
             ok[b] = it.idx < NN && r + b < RPT;
             o[b] = it.offset(G);
-            v[b] = ray_eval<T, V, false>(tb, pb + off, cf32 + off, it.fj<T>(G), it.fi<T>(G), T(0.), nullptr);
+            v[b] = ray_eval<T, V, false>(tb, pb + off, cfs + off, cf32 + off, it.fj<T>(G), it.fi<T>(G), T(0.), nullptr);
             it.next(G);
         }
 #pragma unroll
@@ -447,9 +478,9 @@ __global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 ? GL_ADJ_MI
     const int p = blockIdx.y;
     const T* src = pbg + (size_t)p * PB_STRIDE;
     for (int k = threadIdx.x; k < V::PB_NEED; k += blockDim.x) pb[k] = src[k];
-    __shared__ float cf32[(sizeof(T) == 8 && V::MASS == 1) ? 96 : 4];     // fp32 copies of the series coefficients
-    if constexpr (sizeof(T) == 8 && V::MASS == 1)
-        for (int k = threadIdx.x; k < 96; k += blockDim.x) cf32[k] = (float)src[PB_SER_A + k];
+    __shared__ __align__(16) T cfs[V::MASS == 1 ? 3 * SER_PITCH : 4];                          // series coefficients, shifted layout
+    __shared__ __align__(16) float cf32[(sizeof(T) == 8 && V::MASS == 1) ? 3 * SER_PITCH : 4];  // their fp32 copies
+    if constexpr (V::MASS == 1) stage_series<T>(src, cfs, cf32);
     const typename Real<T>::Tab tb = TabStage<T>::make(tabs, tabg);
     __syncthreads();
     PlaneIter it(G, n_chunk, RPT);
@@ -470,7 +501,7 @@ __global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 ? GL_ADJ_MI
     if (pb[PB_VALID] != T(0.)) {
         for (int r = 0; r < RPT; ++r) {
             int off = 0; asm volatile("" : "+r"(off));      // opaque: keeps the PB scalars in shared memory, not in registers
-            if (it.idx < NN) ray_eval<T, V, true>(tb, pb + off, cf32 + off, it.fj<T>(G), it.fi<T>(G), gb[it.offset(G)], acc, sacc, sstride);
+            if (it.idx < NN) ray_eval<T, V, true>(tb, pb + off, cfs + off, cf32 + off, it.fj<T>(G), it.fi<T>(G), gb[it.offset(G)], acc, sacc, sstride);
             it.next(G);
         }
     }
