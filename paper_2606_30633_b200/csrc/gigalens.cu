@@ -315,7 +315,7 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
     ++t_launches;
     for (int64_t base = 0; base < P; base += pl.Pc) {
         const int64_t Pc = (P - base) < pl.Pc ? (P - base) : pl.Pc;
-        GL_STAGE(ST_UNPACK, st, (gl_unpack_kernel<T><<<(unsigned)((Pc + 127) / 128), 128, 0, st>>>(
+        GL_STAGE(ST_UNPACK, st, (gl_unpack_kernel<T><<<(unsigned)((Pc + UNPACK_WPB - 1) / UNPACK_WPB), UNPACK_WPB * 32, 0, st>>>(
             c->pt, c->L, G, c->desc.pix_scale, params + base * c->L.n_params, Pc, pb, lpd)));
         ++t_launches;
         GL_STAGE(ST_RAY_FWD, st, ray_fwd<T>(c, pb, tab, ray, Pc, st)); ++t_launches;
@@ -333,7 +333,7 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
             GL_STAGE(ST_RAY_ADJ, st, ray_adj<T>(c, pb, tab, ray, nap, Pc, st)); ++t_launches;
         }
         const int wpb = 4;
-        GL_STAGE(ST_FINALIZE, st, (gl_finalize_kernel<T><<<(unsigned)((Pc + wpb - 1) / wpb), wpb * 32, wpb * (NA_MAX + 128) * sizeof(double), st>>>(
+        GL_STAGE(ST_FINALIZE, st, (gl_finalize_kernel<T><<<(unsigned)((Pc + wpb - 1) / wpb), wpb * 32, wpb * (NA_MAX + 256) * sizeof(double), st>>>(
             c->pt, c->L, G, params, pb, lpd, chi, c->n_ctile, mode == 1 ? nap : nullptr, c->n_nap, c->na,
             sys_sl, system_id, Pc, base, out_logp, out_grad)));
         ++t_launches;

@@ -73,22 +73,19 @@ __device__ inline void ell_chain(double e1, double e2, const Ell& E, double dq, 
     de2 = dq * dq_dc * e2 / E.c + dphi * (e1 / (2 * E.c * E.c));
 }
 
-// theta of parameter i of particle `z` (fp32 in HBM -> fp64)
-__device__ inline double theta_at(const PriorTable& pt, const Layout& L, const float* z, int i, bool& ok) {
-    Xform x = transform_one(pt, i, L.param_space, (double)z[i]);
-    ok = ok && x.ok; return x.theta;
-}
+// theta of parameter i from the warp's cache th[] (filled once per particle by the lanes in parallel: transform_one is
+// a few hundred fp64 instructions, and the serial per-particle code below used to call it 2-3 times per parameter)
+__device__ __forceinline__ double theta_at(const double* __restrict__ th, int i) { return th[i]; }
 
 // Write one Sersic block [R, n, e1, e2, x0, y0, Ie] into PB; a negative `off` writes a neutral (Ie = 0) block.
 template <class T>
-__device__ inline void write_sersic(const PriorTable& pt, const Layout& L, const float* z, int off, T* sb,
-                                    double x_first, bool& ok) {
+__device__ inline void write_sersic(const double* __restrict__ th, int off, T* sb, double x_first, bool& ok) {
     double R = 1, n = 1, e1 = 0, e2 = 0, x0 = 0, y0 = 0, Ie = 0;
     if (off >= 0) {
-        R = theta_at(pt, L, z, off, ok); n = theta_at(pt, L, z, off + 1, ok);
-        e1 = theta_at(pt, L, z, off + 2, ok); e2 = theta_at(pt, L, z, off + 3, ok);
-        x0 = theta_at(pt, L, z, off + 4, ok); y0 = theta_at(pt, L, z, off + 5, ok);
-        Ie = theta_at(pt, L, z, off + 6, ok);
+        R = theta_at(th, off); n = theta_at(th, off + 1);
+        e1 = theta_at(th, off + 2); e2 = theta_at(th, off + 3);
+        x0 = theta_at(th, off + 4); y0 = theta_at(th, off + 5);
+        Ie = theta_at(th, off + 6);
         if (!(R > 0) || !(n > 0) || !(e1 * e1 + e2 * e2 < 1.0)) { ok = false; R = 1; n = 1; e1 = e2 = 0; }
     }
     Ell E = make_ell(e1, e2);
@@ -101,30 +98,43 @@ __device__ inline void write_sersic(const PriorTable& pt, const Layout& L, const
     sb[12] = sb[13] = sb[14] = sb[15] = T(0);
 }
 
-// Step A.  One thread per particle.  pb: [P][PB_STRIDE]; lpd: [P] = sum log prior + sum log-det (fp64).
+// Step A.  One WARP per particle (4 per CTA): the lanes transform the parameters in parallel into a shared-memory cache,
+// lane 0 derives the per-particle scalars into a shared-memory PB row, all lanes copy the row out (coalesced).
+// pb: [P][PB_STRIDE]; lpd: [P] = sum log prior + sum log-det (fp64, fixed-order lane tree).
+constexpr int UNPACK_WPB = 4;
 template <class T>
-__global__ void gl_unpack_kernel(const __grid_constant__ PriorTable pt, const __grid_constant__ Layout L,
+__global__ void __launch_bounds__(UNPACK_WPB * 32) gl_unpack_kernel(const __grid_constant__ PriorTable pt, const __grid_constant__ Layout L,
                                  const __grid_constant__ Geom G, float pix_scale,
                                  const float* __restrict__ params, int64_t P, T* __restrict__ pb, double* __restrict__ lpd) {
-    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= P) return;
+    __shared__ double s_th[UNPACK_WPB][128];
+    __shared__ __align__(16) T s_pb[UNPACK_WPB][PB_STRIDE];
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t p = (int64_t)blockIdx.x * UNPACK_WPB + wib;
+    if (p >= P) return;                                           // warp-uniform
     const float* z = params + p * L.n_params;
-    T* o = pb + p * PB_STRIDE;
+    double* th = s_th[wib];
+    T* o = s_pb[wib];
     bool ok = true;
     double lp = 0;
-    for (int i = 0; i < L.n_params; ++i) {
+    for (int i = lane; i < L.n_params; i += 32) {
         Xform x = transform_one(pt, i, L.param_space, (double)z[i]);
-        ok = ok && x.ok; lp += x.lp + x.logdet;
+        ok = ok && x.ok; lp += x.lp + x.logdet; th[i] = x.theta;
     }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) lp += __shfl_xor_sync(0xffffffffu, lp, d);
+    ok = __all_sync(0xffffffffu, ok);
+    for (int k = lane; k < PB_STRIDE; k += 32) o[k] = T(0);
+    __syncwarp();
+    if (lane == 0) {
     const double step = (double)pix_scale / G.s;
     // Ray coordinates are x_j = (j - (M-1)/2) * step (O3 rewritten about the grid centre, which the ray kernels use so
     // that position - centre keeps its RELATIVE accuracy near a component centre): the per-component offsets are -x0.
     const double x_first = 0.0;
     // main deflector
-    double thE = theta_at(pt, L, z, L.mass, ok);
-    double t = L.gamma >= 0 ? theta_at(pt, L, z, L.gamma, ok) - 1.0 : 1.0;
-    double e1 = theta_at(pt, L, z, L.ell, ok), e2 = theta_at(pt, L, z, L.ell + 1, ok);
-    double x0 = theta_at(pt, L, z, L.ell + 2, ok), y0 = theta_at(pt, L, z, L.ell + 3, ok);
+    double thE = theta_at(th, L.mass);
+    double t = L.gamma >= 0 ? theta_at(th, L.gamma) - 1.0 : 1.0;
+    double e1 = theta_at(th, L.ell), e2 = theta_at(th, L.ell + 1);
+    double x0 = theta_at(th, L.ell + 2), y0 = theta_at(th, L.ell + 3);
     if (!(thE > 0) || !(t > 0 && t < 2) || !(e1 * e1 + e2 * e2 < 1.0)) { ok = false; thE = 1; t = 1; e1 = e2 = 0; }
     Ell E = make_ell(e1, e2);
     double b = thE * sqrt(E.q), f = (1 - E.q) / (1 + E.q);
@@ -134,24 +144,24 @@ __global__ void gl_unpack_kernel(const __grid_constant__ PriorTable pt, const __
     double qp = sqrt(fmax(1 - E.q * E.q, 0.0));
     o[PB_M_QP] = (T)qp; o[PB_M_BQP] = (T)(qp > 0 ? b / qp : 0.0);
     o[PB_M_F2] = (T)(f * f); o[PB_M_TM1] = (T)(t - 1); o[PB_M_KAPC] = (T)(0.5 * (2 - t) * b);
-    o[PB_G1] = L.shear >= 0 ? (T)theta_at(pt, L, z, L.shear, ok) : T(0);
-    o[PB_G2] = L.shear >= 0 ? (T)theta_at(pt, L, z, L.shear + 1, ok) : T(0);
-    o[PB_C3] = L.mp3 >= 0 ? (T)theta_at(pt, L, z, L.mp3, ok) : T(0);
-    o[PB_S3] = L.mp3 >= 0 ? (T)theta_at(pt, L, z, L.mp3 + 1, ok) : T(0);
-    o[PB_C4] = L.mp4 >= 0 ? (T)theta_at(pt, L, z, L.mp4, ok) : T(0);
-    o[PB_S4] = L.mp4 >= 0 ? (T)theta_at(pt, L, z, L.mp4 + 1, ok) : T(0);
+    o[PB_G1] = L.shear >= 0 ? (T)theta_at(th, L.shear) : T(0);
+    o[PB_G2] = L.shear >= 0 ? (T)theta_at(th, L.shear + 1) : T(0);
+    o[PB_C3] = L.mp3 >= 0 ? (T)theta_at(th, L.mp3) : T(0);
+    o[PB_S3] = L.mp3 >= 0 ? (T)theta_at(th, L.mp3 + 1) : T(0);
+    o[PB_C4] = L.mp4 >= 0 ? (T)theta_at(th, L.mp4) : T(0);
+    o[PB_S4] = L.mp4 >= 0 ? (T)theta_at(th, L.mp4 + 1) : T(0);
     o[PB_XFIRST] = (T)x_first; o[PB_STEP] = (T)step;
-    write_sersic<T>(pt, L, z, L.src, o + PB_SRC, x_first, ok);
-    write_sersic<T>(pt, L, z, L.ll0, o + PB_LL0, x_first, ok);
-    write_sersic<T>(pt, L, z, L.ll1, o + PB_LL1, x_first, ok);
+    write_sersic<T>(th, L.src, o + PB_SRC, x_first, ok);
+    write_sersic<T>(th, L.ll0, o + PB_LL0, x_first, ok);
+    write_sersic<T>(th, L.ll1, o + PB_LL1, x_first, ok);
     // shapelets (coefficients pre-divided by beta_s; orders above the configured nmax are zero)
     if (L.ker_nmax >= 0) {
         double bs = 1.0;
-        if (L.shp >= 0) { bs = theta_at(pt, L, z, L.shp, ok); if (!(bs > 0)) { ok = false; bs = 1; } }
+        if (L.shp >= 0) { bs = theta_at(th, L.shp); if (!(bs > 0)) { ok = false; bs = 1; } }
         o[PB_SHP] = (T)(1.0 / bs); o[PB_SHP + 1] = o[PB_SHP + 2] = o[PB_SHP + 3] = T(0);
         int nck = (L.ker_nmax + 1) * (L.ker_nmax + 2) / 2;
         for (int k = 0; k < nck; ++k)
-            o[PB_SHP_A + k] = (L.shp >= 0 && k < L.n_coef) ? (T)(theta_at(pt, L, z, L.shp + 1 + k, ok) / bs) : T(0);
+            o[PB_SHP_A + k] = (L.shp >= 0 && k < L.n_coef) ? (T)(theta_at(th, L.shp + 1 + k) / bs) : T(0);
     }
     // EPL series coefficients: a_n = prod_{k<=n} (2k-2+t)/(2k+2-t); d_m = (m+1) a_{m+1}; e_m = L_{m+1} a_{m+1}
     if (L.mass_model == 1) {
@@ -179,13 +189,16 @@ __global__ void gl_unpack_kernel(const __grid_constant__ PriorTable pt, const __
     if (!isfinite(lp)) ok = false;
     o[PB_VALID] = ok ? T(1) : T(0);
     lpd[p] = lp;
+    }   // lane 0
+    __syncwarp();
+    T* dst = pb + p * PB_STRIDE;
+    for (int k = lane; k < PB_STRIDE; k += 32) dst[k] = o[k];
 }
 
 // Chain rule for one Sersic block: natural sums T -> d logL / d[R, n, e1, e2, x0, y0, Ie], written to gth[off..off+6].
-__device__ inline void sersic_chain(const PriorTable& pt, const Layout& L, const float* z, int off, const double* T, double* gth) {
-    bool ok = true;
-    double R = theta_at(pt, L, z, off, ok), n = theta_at(pt, L, z, off + 1, ok);
-    double e1 = theta_at(pt, L, z, off + 2, ok), e2 = theta_at(pt, L, z, off + 3, ok), Ie = theta_at(pt, L, z, off + 6, ok);
+__device__ inline void sersic_chain(const double* __restrict__ th, int off, const double* T, double* gth) {
+    double R = theta_at(th, off), n = theta_at(th, off + 1);
+    double e1 = theta_at(th, off + 2), e2 = theta_at(th, off + 3), Ie = theta_at(th, off + 6);
     Ell E = make_ell(e1, e2);
     double bn = 1.9992 * n - 0.3271, k = bn / n;
     gth[off + 6] = T[SA_T0] / Ie;
@@ -210,12 +223,13 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
                                    const T* __restrict__ nap, int n_chunk, int na,
                                    const double* __restrict__ sys_sumlog, const int32_t* __restrict__ system_id,
                                    int64_t P, int64_t p_base, float* __restrict__ out_logp, float* __restrict__ out_grad) {
-    extern __shared__ double fsm[];                     // per warp: nat[NA_MAX] + gth[128]
+    extern __shared__ double fsm[];                     // per warp: nat[NA_MAX] + gth[128] + th[128]
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int64_t p = (int64_t)blockIdx.x * (blockDim.x >> 5) + wib;
     if (p >= P) return;
-    double* nat = fsm + (size_t)wib * (NA_MAX + 128);
+    double* nat = fsm + (size_t)wib * (NA_MAX + 256);
     double* gth = nat + NA_MAX;
+    double* th = gth + 128;                             // theta cache (see theta_at)
     const float* z = params + (p_base + p) * L.n_params;
     const bool valid = pb[p * PB_STRIDE + PB_VALID] != T(0);
     // chi^2: lanes stride over tiles, then a fixed xor-tree
@@ -232,13 +246,12 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
             for (int ch = 0; ch < n_chunk; ++ch) s += (double)nap[((size_t)p * n_chunk + ch) * na + k];
             nat[k] = s;
         }
-        for (int k = lane; k < L.n_params; k += 32) gth[k] = 0;
+        for (int k = lane; k < L.n_params; k += 32) { gth[k] = 0; th[k] = transform_one(pt, k, L.param_space, (double)z[k]).theta; }
         __syncwarp();
         if (lane == 0 && valid) {
-            bool ok = true;
-            double thE = theta_at(pt, L, z, L.mass, ok);
-            double t = L.gamma >= 0 ? theta_at(pt, L, z, L.gamma, ok) - 1.0 : 1.0;
-            double e1 = theta_at(pt, L, z, L.ell, ok), e2 = theta_at(pt, L, z, L.ell + 1, ok);
+            double thE = theta_at(th, L.mass);
+            double t = L.gamma >= 0 ? theta_at(th, L.gamma) - 1.0 : 1.0;
+            double e1 = theta_at(th, L.ell), e2 = theta_at(th, L.ell + 1);
             Ell E = make_ell(e1, e2);
             double q = E.q, b = thE * sqrt(q);
             double dL_db = -(t / b) * nat[NA_D0];
@@ -259,19 +272,18 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
             if (L.mp3 >= 0) { gth[L.mp3] = nat[NA_C3]; gth[L.mp3 + 1] = nat[NA_S3]; }
             if (L.mp4 >= 0) { gth[L.mp4] = nat[NA_C4]; gth[L.mp4 + 1] = nat[NA_S4]; }
             if (L.mp3 >= 0 || L.mp4 >= 0) { gth[L.ell + 2] += nat[NA_MCX]; gth[L.ell + 3] += nat[NA_MCY]; }
-            if (L.src >= 0) sersic_chain(pt, L, z, L.src, nat + NA_SRC, gth);
-            if (L.ll0 >= 0) sersic_chain(pt, L, z, L.ll0, nat + NA_LL0, gth);
-            if (L.ll1 >= 0) sersic_chain(pt, L, z, L.ll1, nat + NA_LL1, gth);
+            if (L.src >= 0) sersic_chain(th, L.src, nat + NA_SRC, gth);
+            if (L.ll0 >= 0) sersic_chain(th, L.ll0, nat + NA_LL0, gth);
+            if (L.ll1 >= 0) sersic_chain(th, L.ll1, nat + NA_LL1, gth);
             if (L.shp >= 0) {
-                double bs = theta_at(pt, L, z, L.shp, ok);
+                double bs = theta_at(th, L.shp);
                 gth[L.shp] = -nat[NA_SHB] / bs;
                 gth[L.src + 4] -= nat[NA_SHX]; gth[L.src + 5] -= nat[NA_SHY];
             }
         }
         __syncwarp();
         if (L.shp >= 0 && valid) {
-            bool ok = true;
-            double bs = theta_at(pt, L, z, L.shp, ok);
+            double bs = theta_at(th, L.shp);
             for (int k = lane; k < L.n_coef; k += 32) gth[L.shp + 1 + k] = nat[NA_SHA + k] / bs;
         }
         __syncwarp();
