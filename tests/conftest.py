@@ -10,6 +10,15 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+    # Build the two native libraries in-tree if they are missing or stale (nvcc cross-compiles without a GPU).  This is
+    # a build step, not a fallback: without libgigalens.so every product call still fails loudly.
+    try:
+        from paper_2606_30633_b200 import build as gl_build
+        from oracle import build as oracle_build
+        gl_build.build()
+        oracle_build.build()
+    except Exception as e:                                   # reported by the tests that need the libraries
+        print("native build failed: %s" % e, file=sys.stderr)
 
 
 def pytest_collection_modifyitems(config, items):
