@@ -362,7 +362,7 @@ def run_ours(a):
     peak = N_SM * lanes * mhz_max * 1e6 / 1e12                        # T lane-op/s
     wm = workmodel.per_eval(sp, a.precision)
     probe = {}
-    for kind, name in ((0, "fp32_fma"), (1, "fp64_fma"), (2, "mufu_ex2")):
+    for kind, name in ((0, "fp32_fma"), (1, "fp64_fma"), (2, "mufu_ex2"), (4, "fp64_fma_distinct_operands")):
         try:
             probe[name] = round(gl.gl_probe_pipe(kind, 256)[0], 3)
         except Exception as e:                                        # measurement utility only

@@ -241,7 +241,7 @@ int32_t     gl_stage_times(float* ms_host, int32_t* launches_host, int32_t n);
  * pipe, so that bench.py can state a MEASURED ALU peak beside the one derived from unit counts and clocks
  * (BASELINE.json north_star: "achieved fraction of the binding roofline"; MEASURED_PEAKS.json has no FP32, FP64
  * or MUFU figure).  kind 0: FP32 FMA, 1: FP64 FMA, 2: MUFU ex2, 3: FP32 and FP64 FMA interleaved 1:1 (both
- * counted).  Launches 8 CTAs of 256 threads per SM, each thread running 8 independent chains of
+ * counted), 4: FP64 FMA with three distinct register operands per chain (kinds 0-3 share multiplier and addend).  Launches 8 CTAs of 256 threads per SM, each thread running 8 independent chains of
  * n_outer * 64 operations, once untimed and once between two CUDA events on `stream`, waits for it, and writes
  * 1e-12 * lane-operations per second (an FMA counts once) to *tera_lane_ops_per_s_host and the kernel time to
  * *ms_host (HOST pointers; ms_host may be NULL).  workspace: DEVICE pointer, >= 256 bytes (never written in

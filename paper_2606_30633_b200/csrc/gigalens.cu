@@ -557,7 +557,7 @@ extern "C" gl_status gl_logpost_grad_host(const gl_config* c, const float* obs, 
 extern "C" gl_status gl_probe_pipe(int32_t kind, int32_t n_outer, void* workspace, size_t workspace_bytes, void* stream,
                                    double* tera_lane_ops_per_s_host, float* ms_host) {
     if (!workspace || !tera_lane_ops_per_s_host) return GL_ERR_NULL;
-    if (kind < 0 || kind > 3 || n_outer < 1) return GL_ERR_BAD_SHAPE;
+    if (kind < 0 || kind > 4 || n_outer < 1) return GL_ERR_BAD_SHAPE;
     if (workspace_bytes < 256) return GL_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, n_sm = 0;
@@ -572,7 +572,8 @@ extern "C" gl_status gl_probe_pipe(int32_t kind, int32_t n_outer, void* workspac
             case 0: gl_probe_kernel<0><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
             case 1: gl_probe_kernel<1><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
             case 2: gl_probe_kernel<2><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
-            default: gl_probe_kernel<3><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+            case 3: gl_probe_kernel<3><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+            default: gl_probe_kernel<4><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
         }
     };
     launch(n_outer);                                   // warm-up

@@ -10,12 +10,18 @@ namespace gl {
 constexpr int PROBE_CHAINS = 8;     // independent dependency chains per thread
 constexpr int PROBE_INNER = 64;     // FMAs per chain per outer iteration
 
-// kind 0: FP32 FMA;  1: FP64 FMA;  2: MUFU ex2;  3: FP32 and FP64 FMA interleaved 1:1 (counts both)
+// kind 0: FP32 FMA;  1: FP64 FMA;  2: MUFU ex2;  3: FP32 and FP64 FMA interleaved 1:1 (counts both);
+// 4: FP64 FMA whose three operands are distinct registers in every chain (kinds 0-3 share multiplier and addend across
+//    the chains, which lets the operand-reuse cache feed the pipe: kind 4 is what ordinary fp64 code can sustain)
 template <int KIND>
 __global__ void __launch_bounds__(256) gl_probe_kernel(int n_outer, float seed, float* __restrict__ sink) {
-    float a[PROBE_CHAINS]; double d[PROBE_CHAINS];
+    float a[PROBE_CHAINS]; double d[PROBE_CHAINS], e[PROBE_CHAINS], f[PROBE_CHAINS];
 #pragma unroll
-    for (int k = 0; k < PROBE_CHAINS; ++k) { a[k] = seed + k + threadIdx.x * 1e-3f; d[k] = (double)a[k]; }
+    for (int k = 0; k < PROBE_CHAINS; ++k) {
+        a[k] = seed + k + threadIdx.x * 1e-3f; d[k] = (double)a[k];
+        e[k] = 0.999 + 1e-12 * (double)(threadIdx.x + k) * (double)seed;          // per-thread values: not uniform registers
+        f[k] = 1e-3 * (1.0 + 1e-6 * (double)threadIdx.x) * (double)seed * (k + 1);
+    }
     const float m = 0.999f + seed * 1e-6f, c = 1e-3f;
     const double md = (double)m, cd = (double)c;
     for (int o = 0; o < n_outer; ++o) {
@@ -26,6 +32,7 @@ __global__ void __launch_bounds__(256) gl_probe_kernel(int n_outer, float seed, 
                 if constexpr (KIND == 0 || KIND == 3) a[k] = fmaf(a[k], m, c);
                 if constexpr (KIND == 1 || KIND == 3) d[k] = fma(d[k], md, cd);
                 if constexpr (KIND == 2) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(a[k]));
+                if constexpr (KIND == 4) d[k] = fma(d[k], e[k], f[k]);
             }
         }
     }
