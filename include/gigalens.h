@@ -181,6 +181,12 @@ gl_status gl_map_step(const gl_config* cfg, const gl_opt_desc* opt, const float*
                       float* opt_m, float* opt_v, int64_t step, float* out_logp, float* out_grad,
                       void* workspace, size_t workspace_bytes, void* stream /* cudaStream_t */);
 
+/* Best particle of a MAP run ("multi-start"): index and value of the largest FINITE entry of
+ * logp[0..n) (DEVICE), ties resolved to the lowest index; out_index[0] = -1 and out_logp[0] = -INF if none is finite.
+ * out_index (int64) and out_logp (float) are DEVICE pointers; one single-CTA launch on `stream`. */
+gl_status gl_best_particle(const float* logp, int64_t n_particles, int64_t* out_index, float* out_logp,
+                           void* stream /* cudaStream_t */);
+
 /* ---- one SVI iteration on the device ---------------------------------------------------------
  * Fits the multivariate-normal surrogate q~(Theta~; mu~, Sigma~ = L L^T) of P:L78-100 by one optimiser step on the
  * sampled loss  ELBO^ = -sum_j log L_jj - (n/2) log(2 pi e) - (1/N) sum_i log p~(z_i)  (Eq. 2 with E_q[log q] in closed

@@ -22,7 +22,8 @@ EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_wo
            "gl_logpost_grad", "gl_model_image", "gl_workspace_bytes_host", "gl_logpost_grad_host",
            "gl_last_launch_count", "gl_status_string", "gl_version", "gl_stage_timing_enable", "gl_stage_count",
            "gl_stage_name", "gl_stage_times", "gl_probe_pipe", "gl_map_step",
-           "gl_svi_workspace_bytes", "gl_svi_step", "gl_hmc_workspace_bytes", "gl_hmc_step"]
+           "gl_svi_workspace_bytes", "gl_svi_step", "gl_hmc_workspace_bytes", "gl_hmc_step",
+           "gl_best_particle"]
 
 
 class GLError(RuntimeError):
@@ -82,6 +83,8 @@ def lib():
         L.gl_logpost_grad_host.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, sz, vp]
         L.gl_map_step.restype = C.c_int
         L.gl_map_step.argtypes = [vp, C.POINTER(gl_opt_desc), vp, vp, vp, vp, vp, i64, vp, vp, i64, vp, vp, vp, sz, vp]
+        L.gl_best_particle.restype = C.c_int
+        L.gl_best_particle.argtypes = [vp, i64, vp, vp, vp]
         L.gl_hmc_workspace_bytes.restype = sz
         L.gl_hmc_workspace_bytes.argtypes = [vp, i64]
         L.gl_hmc_step.restype = C.c_int
@@ -242,6 +245,16 @@ def _opt_desc(opt):
         return opt
     return gl_opt_desc(int(opt["kind"]), float(opt["lr"]), float(opt["b1"]), float(opt["b2"]), float(opt["eps"]),
                        float(opt.get("eps_root", 0.0)))
+
+
+def gl_best_particle(logp, stream=None):
+    """(index tensor [1] int64, value tensor [1] float32) of the largest finite log-posterior, on the device."""
+    torch = _torch()
+    idx = torch.empty(1, dtype=torch.int64, device=logp.device)
+    val = torch.empty(1, dtype=torch.float32, device=logp.device)
+    _check(lib().gl_best_particle(_ptr(_dev(logp, torch.float32, "logp")), logp.shape[0], _ptr(idx), _ptr(val),
+                                  _stream(stream)), "gl_best_particle")
+    return idx, val
 
 
 def gl_hmc_workspace_bytes(h, n):

@@ -406,6 +406,15 @@ extern "C" gl_status gl_map_step(const gl_config* cfg, const gl_opt_desc* opt, c
     return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
 }
 
+extern "C" gl_status gl_best_particle(const float* logp, int64_t n, int64_t* out_index, float* out_logp, void* stream) {
+    t_launches = 0;
+    if (n < 0) return GL_ERR_BAD_SHAPE;
+    if (!out_index || !out_logp || (n > 0 && !logp)) return GL_ERR_NULL;
+    gl_best_particle_kernel<<<1, 1024, 0, (cudaStream_t)stream>>>(logp, n, out_index, out_logp);
+    t_launches = 1;
+    return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
+}
+
 struct SviPlan { size_t core, off_z, off_lp, off_g, off_part, total; };
 static SviPlan svi_plan(const gl_config* c, int64_t n) {
     SviPlan p{};

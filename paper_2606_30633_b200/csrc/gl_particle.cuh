@@ -303,6 +303,31 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
     if (lane == 0) out_logp[p_base + p] = good ? (float)logp : -INFINITY;
 }
 
+// arg max over the particles (largest finite logp, lowest index on ties).  ONE block of 1024 threads:
+// each thread scans a strided subset keeping (value, index), then a fixed tree in shared memory.
+__global__ void __launch_bounds__(1024) gl_best_particle_kernel(const float* __restrict__ logp, int64_t n,
+                                                                int64_t* __restrict__ out_index, float* __restrict__ out_logp) {
+    __shared__ float sv[1024];
+    __shared__ int64_t si[1024];
+    float bv = -INFINITY; int64_t bi = -1;
+    for (int64_t i = threadIdx.x; i < n; i += 1024) {
+        const float v = logp[i];
+        if (isfinite(v) && (bi < 0 || v > bv)) { bv = v; bi = i; }        // strided scan: indices increase, '>' keeps the first
+    }
+    sv[threadIdx.x] = bv; si[threadIdx.x] = bi;
+    __syncthreads();
+    for (int o = 512; o > 0; o >>= 1) {
+        if (threadIdx.x < o) {
+            const float v2 = sv[threadIdx.x + o]; const int64_t i2 = si[threadIdx.x + o];
+            const float v1 = sv[threadIdx.x]; const int64_t i1 = si[threadIdx.x];
+            const bool take = i2 >= 0 && (i1 < 0 || v2 > v1 || (v2 == v1 && i2 < i1));
+            if (take) { sv[threadIdx.x] = v2; si[threadIdx.x] = i2; }
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { out_index[0] = si[0]; out_logp[0] = si[0] >= 0 ? sv[0] : -INFINITY; }
+}
+
 // Adam / AdaBelief update of every (particle, parameter), fp64 arithmetic on fp32 storage.
 // One thread per element; a particle with a non-finite log-posterior or gradient row is left untouched (the
 // gradient row of such a particle is all zero by construction of gl_finalize_kernel, its logp is -INF).

@@ -84,3 +84,24 @@ def test_map_step_argument_checks():
     with pytest.raises(gl.GLError) as e:
         gl.gl_map_step(m.h, ADAM, m.obs, m.noise_sigma, m.psf, z, None, mm, vv, 0, lp, g, m.workspace(4))
     assert e.value.status == -2
+
+
+def test_best_particle_matches_numpy_argmax():
+    """gl_best_particle against the plain definition (largest finite entry, lowest index on ties), including ties,
+    non-finite entries, sizes around the block size and the all-invalid case.  Integer result: exact."""
+    import torch
+    import paper_2606_30633_b200 as gl
+    rng = np.random.default_rng(4)
+    for n in (1, 7, 1023, 1024, 1025, 4096, 100003):
+        v = rng.standard_normal(n).astype(np.float32)
+        v[rng.random(n) < 0.1] = -np.inf
+        if n > 3:
+            v[rng.integers(0, n, 3)] = np.nan
+            j = rng.integers(0, n, 4); v[j] = np.float32(7.5)             # a four-way tie for the maximum
+        w = np.where(np.isfinite(v), v, -np.inf)
+        want = int(np.argmax(w)) if np.isfinite(w).any() else -1
+        idx, val = gl.gl_best_particle(torch.from_numpy(v).cuda())
+        assert int(idx[0]) == want, (n, int(idx[0]), want)
+        assert float(val[0]) == (float(v[want]) if want >= 0 else -np.inf)
+    idx, val = gl.gl_best_particle(torch.full((50,), -np.inf).cuda())
+    assert int(idx[0]) == -1 and float(val[0]) == -np.inf
