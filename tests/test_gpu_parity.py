@@ -102,11 +102,13 @@ def test_model_image_matches_oracle(k):
     assert np.max(np.abs(img - ref) / scale) < 2e-5
 
 
-def test_full_batch_rows_are_bit_identical_to_subset_rows():
-    """BASELINE-size launch (config 2, 4096 particles, the configuration bench.py times): rows of the full batch
-    equal the same particles evaluated alone (PAPER.md L83 fn 2: no cross-particle dependence), hence the oracle."""
-    gl, torch, wl, m = _model(2)
-    idx, ref = oracle_subset(2)
+@pytest.mark.parametrize("k", [2, 3, 5])
+def test_full_batch_rows_are_bit_identical_to_subset_rows(k):
+    """BASELINE-size launches (config 2 = 4096 particles, the configuration bench.py times; config 3 = 8192; config 5 =
+    2048): rows of the full batch equal the same particles evaluated alone (PAPER.md L83 fn 2: no cross-particle
+    dependence), hence the oracle through test_parity_subset."""
+    gl, torch, wl, m = _model(k)
+    idx, ref = oracle_subset(k)
     zf = torch.from_numpy(wl.params).cuda()
     lpf, gf = m.logpost_grad(zf)
     lps, gs = m.logpost_grad(zf[torch.from_numpy(idx).cuda()].contiguous())
