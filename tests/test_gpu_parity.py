@@ -359,3 +359,34 @@ def test_model_variance_config2_subset():
     assert np.all(np.isfinite(lp)) and np.all(np.abs(lp - ref["logp"]) <= RTOL_LOGP * np.abs(ref["logp"]))
     ok, rep = grad_report(g, ref["grad"])
     assert rep["n_fail"] == 0, rep
+
+
+@pytest.mark.parametrize("shape", [(37, 2, 11), (13, 4, 21), (23, 2, 21), (9, 4, 41), (21, 2, 31), (5, 2, 31), (1, 2, 11),
+                                   (3, 4, 21)])
+@pytest.mark.parametrize("precision", [0, 1])
+def test_tuned_conv_kernels_at_awkward_sizes(shape, precision):
+    """The step-D specialisations (U = 6, 11, 16) at sizes that are not multiples of their column blocking, smaller than
+    the tap count, and down to a single pixel: model image, log-posterior and gradient against the oracle."""
+    import dataclasses
+    import oracle
+    import torch
+    gl = _gl()
+    n_pix, s, K = shape
+    sp, obs, sigma, psf, z = _small_case(n_pix, s, K, 1, 0, -1, 1, seed=40 * n_pix + K, n_particles=5)
+    sp = dataclasses.replace(sp, precision=precision)
+    ref = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), None, want_model=True)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    zt = torch.from_numpy(z).cuda()
+    lp, g = m.logpost_grad(zt)
+    img = m.model_image(zt).cpu().numpy().astype(np.float64)
+    lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+    fin = np.isfinite(ref["logp"])
+    assert fin.sum() >= 3 and np.array_equal(fin, np.isfinite(lp))
+    scale = np.abs(ref["model"][fin]).max(axis=(1, 2), keepdims=True)
+    assert np.max(np.abs(img[fin] - ref["model"][fin]) / scale) < (2e-7 if precision == 0 else 2e-5)
+    assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+    ok, rep = grad_report(g[fin], ref["grad"][fin])
+    if precision == 0:
+        assert rep["n_fail"] == 0, rep
+    else:
+        assert rep["normwise"] <= 2e-3, rep
