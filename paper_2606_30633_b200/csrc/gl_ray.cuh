@@ -84,7 +84,50 @@ __device__ __forceinline__ void stage_series(const T* __restrict__ src, T* __res
     }
 }
 
-template <class T, int K>
+// G groups of 4 recurrence steps, fully unrolled (G is a compile-time count: no loop control, immediate load offsets).
+// c points at the shifted coefficient array position of index k_hi - 3 ... i.e. coefficient idx sits at c[idx + 3];
+// the groups use indices k_hi, k_hi - 1, ..., k_hi - 4 G + 1 with k_hi a multiple of 4 (passed through the pointer).
+template <class S, int K, int G>
+__device__ __forceinline__ void knuth_groups(const S* __restrict__ c_at_khi, S p, S nf2, S (&b1)[K], S (&b2)[K]) {
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        S v[K][4];
+#pragma unroll
+        for (int i = 0; i < K; ++i) load_coef4(c_at_khi + SER_PITCH * i, -4 * g, v[i]);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+#pragma unroll
+            for (int i = 0; i < K; ++i) {
+                S bk;
+                if constexpr (sizeof(S) == 8) bk = fma(p, b1[i], fma(nf2, b2[i], v[i][j]));
+                else bk = fmaf(p, b1[i], fmaf(nf2, b2[i], v[i][j]));
+                b2[i] = b1[i]; b1[i] = bk;
+            }
+        }
+    }
+}
+// run-time group count 0..7 -> the unrolled instance (one CTA-uniform switch per polynomial set instead of a loop)
+// UNR = false: a plain loop over the groups instead (smaller code: measured better for the shapelet variants and for
+// the fp32 adjoint, whose register budgets are tight).
+template <class S, int K, bool UNR>
+__device__ __forceinline__ void knuth_groups_n(int n, const S* __restrict__ c_at_khi, S p, S nf2, S (&b1)[K], S (&b2)[K]) {
+    if constexpr (!UNR) {
+        for (int g = 0; g < n; ++g) knuth_groups<S, K, 1>(c_at_khi - 4 * g, p, nf2, b1, b2);
+        return;
+    }
+    switch (n) {
+        case 1: knuth_groups<S, K, 1>(c_at_khi, p, nf2, b1, b2); break;
+        case 2: knuth_groups<S, K, 2>(c_at_khi, p, nf2, b1, b2); break;
+        case 3: knuth_groups<S, K, 3>(c_at_khi, p, nf2, b1, b2); break;
+        case 4: knuth_groups<S, K, 4>(c_at_khi, p, nf2, b1, b2); break;
+        case 5: knuth_groups<S, K, 5>(c_at_khi, p, nf2, b1, b2); break;
+        case 6: knuth_groups<S, K, 6>(c_at_khi, p, nf2, b1, b2); break;
+        case 7: knuth_groups<S, K, 7>(c_at_khi, p, nf2, b1, b2); break;
+        default: break;
+    }
+}
+
+template <class T, int K, bool UNR>
 __device__ __forceinline__ void knuth_banded(const T* __restrict__ cf, const float* __restrict__ cf32, int m1, int m2,
                                              T p, T nf2, T wr, T wi, T (&Pr)[K], T (&Pi)[K]) {
     using R = Real<T>;
@@ -97,20 +140,7 @@ __device__ __forceinline__ void knuth_banded(const T* __restrict__ cf, const flo
             float c1[K], c2[K];
 #pragma unroll
             for (int i = 0; i < K; ++i) { c1[i] = cf32[SER_PITCH * i + kt + 3]; c2[i] = 0.f; }
-            int k = kt - 1;
-            for (int g = 0; g < m2; ++g, k -= 4) {
-                float v[K][4];
-#pragma unroll
-                for (int i = 0; i < K; ++i) load_coef4(cf32 + SER_PITCH * i, k, v[i]);
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-#pragma unroll
-                    for (int i = 0; i < K; ++i) {
-                        const float bk = fmaf(pf, c1[i], fmaf(nf, c2[i], v[i][j]));
-                        c2[i] = c1[i]; c1[i] = bk;
-                    }
-                }
-            }
+            knuth_groups_n<float, K, UNR>(m2, cf32 + (kt - 1), pf, nf, c1, c2);
 #pragma unroll
             for (int i = 0; i < K; ++i) { b1[i] = (T)c1[i]; b2[i] = (T)c2[i]; }
             seeded = true;
@@ -120,20 +150,7 @@ __device__ __forceinline__ void knuth_banded(const T* __restrict__ cf, const flo
 #pragma unroll
         for (int i = 0; i < K; ++i) { b1[i] = cf[SER_PITCH * i + kt + 3]; b2[i] = T(0.); }
     }
-    int k = 4 * m1;
-    for (int g = 0; g < m1; ++g, k -= 4) {
-        T v[K][4];
-#pragma unroll
-        for (int i = 0; i < K; ++i) load_coef4(cf + SER_PITCH * i, k, v[i]);
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-#pragma unroll
-            for (int i = 0; i < K; ++i) {
-                const T bk = R::fma(p, b1[i], R::fma(nf2, b2[i], v[i][j]));
-                b2[i] = b1[i]; b1[i] = bk;
-            }
-        }
-    }
+    knuth_groups_n<T, K, UNR>(m1, cf + 4 * m1, p, nf2, b1, b2);
 #pragma unroll
     for (int i = 0; i < K; ++i) {
         const T r0 = R::fma(nf2, b2[i], cf[SER_PITCH * i + 3]);
@@ -213,7 +230,8 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
         const T wr = -f * c2, wi = -f * s2, p = T(2.) * wr;
         const int m1 = (int)pb[PB_SER_M1], m2 = (int)pb[PB_SER_M2];
         T Pr[ADJ ? 3 : 1], Pi[ADJ ? 3 : 1];
-        knuth_banded<T, (ADJ ? 3 : 1)>(cfs, cf32, m1, m2, p, nf2, wr, wi, Pr, Pi);
+        constexpr bool UNR = V::NMAX < 0 && (!ADJ || sizeof(T) == 8);      // where the unrolled band switch pays (measured)
+        knuth_banded<T, (ADJ ? 3 : 1), UNR>(cfs, cf32, m1, m2, p, nf2, wr, wi, Pr, Pi);
         const T P0r = Pr[0], P0i = Pi[0];
         S0r = R::fma(ce, P0r, -se * P0i); S0i = R::fma(ce, P0i, se * P0r);
         lbr = R::fma(-T(0.5), R::lg2(tb, R2), pb[PB_M_L2B]);
