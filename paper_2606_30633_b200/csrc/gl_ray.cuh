@@ -110,9 +110,25 @@ __device__ __forceinline__ void knuth_groups(const S* __restrict__ c_at_khi, S p
 // UNR = false: a plain loop over the groups instead (smaller code: measured better for the shapelet variants and for
 // the fp32 adjoint, whose register budgets are tight).
 template <class S, int K, bool UNR>
-__device__ __forceinline__ void knuth_groups_n(int n, const S* __restrict__ c_at_khi, S p, S nf2, S (&b1)[K], S (&b2)[K]) {
+__device__ __forceinline__ void knuth_groups_n(int n, const S* __restrict__ c_base, int k_hi, S p, S nf2, S (&b1)[K], S (&b2)[K]) {
+    const S* c_at_khi = c_base + k_hi;
     if constexpr (!UNR) {
-        for (int g = 0; g < n; ++g) knuth_groups<S, K, 1>(c_at_khi - 4 * g, p, nf2, b1, b2);
+        int k = k_hi;                                              // index form of the plain loop (measured faster than pointer steps)
+        for (int g = 0; g < n; ++g, k -= 4) {
+            S v[K][4];
+#pragma unroll
+            for (int i = 0; i < K; ++i) load_coef4(c_base + SER_PITCH * i, k, v[i]);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+#pragma unroll
+                for (int i = 0; i < K; ++i) {
+                    S bk;
+                    if constexpr (sizeof(S) == 8) bk = fma(p, b1[i], fma(nf2, b2[i], v[i][j]));
+                    else bk = fmaf(p, b1[i], fmaf(nf2, b2[i], v[i][j]));
+                    b2[i] = b1[i]; b1[i] = bk;
+                }
+            }
+        }
         return;
     }
     switch (n) {
@@ -140,7 +156,7 @@ __device__ __forceinline__ void knuth_banded(const T* __restrict__ cf, const flo
             float c1[K], c2[K];
 #pragma unroll
             for (int i = 0; i < K; ++i) { c1[i] = cf32[SER_PITCH * i + kt + 3]; c2[i] = 0.f; }
-            knuth_groups_n<float, K, UNR>(m2, cf32 + (kt - 1), pf, nf, c1, c2);
+            knuth_groups_n<float, K, UNR>(m2, cf32, kt - 1, pf, nf, c1, c2);
 #pragma unroll
             for (int i = 0; i < K; ++i) { b1[i] = (T)c1[i]; b2[i] = (T)c2[i]; }
             seeded = true;
@@ -150,7 +166,7 @@ __device__ __forceinline__ void knuth_banded(const T* __restrict__ cf, const flo
 #pragma unroll
         for (int i = 0; i < K; ++i) { b1[i] = cf[SER_PITCH * i + kt + 3]; b2[i] = T(0.); }
     }
-    knuth_groups_n<T, K, UNR>(m1, cf + 4 * m1, p, nf2, b1, b2);
+    knuth_groups_n<T, K, UNR>(m1, cf, 4 * m1, p, nf2, b1, b2);
 #pragma unroll
     for (int i = 0; i < K; ++i) {
         const T r0 = R::fma(nf2, b2[i], cf[SER_PITCH * i + 3]);
