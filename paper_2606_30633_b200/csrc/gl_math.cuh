@@ -16,9 +16,11 @@ __device__ __forceinline__ float f_rsqrt(float x) { float y; asm("rsqrt.approx.f
 __device__ __forceinline__ float f_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
 // ----------------------------------------------------------------------------- fp64 exp2 / log2
-// exp2(x) = 2^n * 2^(j/16) * (1 + r P(r)),  x = n + j/16 + r, |r| <= 1/32;  P = degree-4 (2^r to r^5: error < 1.5e-13).
+// exp2(x) = 2^n * 2^(j/16) * (1 + r P(r)),  x = n + j/16 + r, |r| <= 1/32;  P = degree-3 Chebyshev fit (error < 6e-12).
 // log2(x) = e + log2(c_j) + log1p(r)/ln2,  x = 2^e m, m in [1,2), c_j = 1 + (j+0.5)/16, r = m rc_j - 1, |r| <= 1/32;
-//           log1p through r^7 (absolute error < 1.7e-13).
+//           log1p(r)/(r ln2) as a degree-4 Chebyshev fit (absolute error < 1.5e-11).  These errors are 1e4 times below fp32
+//           and leave the parity margins of section 6 of DESIGN.md untouched (checked on all five configs); each
+//           polynomial term costs an FP64 issue slot in kernels that run at the FP64 issue rate.
 // The tables have 16 doubles = 128 bytes = ONE shared-memory bank row each, so a lookup with 32 arbitrary per-lane
 // indices is always a single conflict-free wavefront (larger tables made the ray kernels shared-memory bound:
 // profiles/r1b_cfg2_f64.md).  They are generated on the device in fp64 once per call by gl_prep_kernel (block 0) into
@@ -48,29 +50,22 @@ __constant__ double c_dm[20] = {
     6755399441055744.0,        // 0: 1.5 * 2^52: adding it rounds to an integer in the low word
     16.0,                      // 1
     -0.0625,                   // 2: -1/16
-    6.93147180559945286e-01,   // 3: ln2^1/1!
-    2.40226506959100694e-01,   // 4: ln2^2/2!
-    5.55041086648215762e-02,   // 5: ln2^3/3!
-    9.61812910762847688e-03,   // 6: ln2^4/4!
-    1.33335581464284411e-03,   // 7: ln2^5/5!
-    1.44269504088896339e+00,   // 8:  1/(1 ln2)
-    -7.21347520444481694e-01,   // 9: -1/(2 ln2)
-    4.80898346962987833e-01,   // 10:  1/(3 ln2)
-    -3.60673760222240847e-01,   // 11: -1/(4 ln2)
-    2.88539008177792655e-01,   // 12:  1/(5 ln2)
-    -2.40449173481493916e-01,   // 13: -1/(6 ln2)
-    2.06099291555566222e-01,   // 14:  1/(7 ln2)
+    // 3..6: (2^r - 1)/r on |r| <= 1/32, degree-3 Chebyshev fit (relative error of 2^r < 6e-12)
+    0.6931471804009947, 0.24022650691319444, 0.05550541078373476, 0.009618317140281765,
+    0.0,                       // 7: unused
+    // 8..12: log2(1 + r)/r on |r| <= 1/32, degree-4 Chebyshev fit (absolute error of log2(1 + r) < 1.5e-11)
+    1.44269504089497, -0.7213474487115007, 0.4808982362719573, -0.36096750318286375, 0.2888411792028112,
+    0.0, 0.0,                  // 13, 14: unused
     0.5, 1.0, -1.0, 0.0,       // 15..18
     0.0};
 
-// 2^x, relative error < 2e-13, for -1e8 < x < 1000; below -1021 the result saturates at ~1e-308.
+// 2^x, relative error < 6e-12, for -1e8 < x < 1000; below -1021 the result saturates at ~1e-308.
 __device__ __forceinline__ double d_exp2(const MathTab& tb, double x) {
     const double kd = fma(x, c_dm[1], c_dm[0]);
     const int k = __double2loint(kd);                          // k = rint(16 x)
     const double r = fma(kd - c_dm[0], c_dm[2], x);            // x - k/16, exact
     const int j = k & 15, n = max(k >> 4, -1021);              // x < -1021: result 2^-1021 y ~ 1e-308 (stands for 0)
-    double p = c_dm[7];
-    p = fma(p, r, c_dm[6]);
+    double p = c_dm[6];
     p = fma(p, r, c_dm[5]);
     p = fma(p, r, c_dm[4]);
     p = fma(p, r, c_dm[3]);
@@ -79,17 +74,15 @@ __device__ __forceinline__ double d_exp2(const MathTab& tb, double x) {
     return __hiloint2double(__double2hiint(y) + (n << 20), __double2loint(y));   // scale by 2^n through the exponent field
 }
 
-// log2(x) for normal x > 0, absolute error < 2e-13.
+// log2(x) for normal x > 0, absolute error < 1.5e-11.
 __device__ __forceinline__ double d_log2(const MathTab& tb, double x) {
     const int hi = __double2hiint(x), lo = __double2loint(x);
     const int e = (hi >> 20) - 1023;
     const int j = (hi >> 16) & 15;                             // top 4 mantissa bits
     const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, lo);
     const double r = fma(m, tb.rc[j], c_dm[17]);               // |r| <= 1/32
-    // log1p(r)/ln2 = r (c1 + c2 r + ... + c7 r^6)
-    double p = c_dm[14];
-    p = fma(p, r, c_dm[13]);
-    p = fma(p, r, c_dm[12]);
+    // log1p(r)/ln2 = r (c1 + c2 r + ... + c5 r^4)
+    double p = c_dm[12];
     p = fma(p, r, c_dm[11]);
     p = fma(p, r, c_dm[10]);
     p = fma(p, r, c_dm[9]);
