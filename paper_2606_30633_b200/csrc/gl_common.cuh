@@ -39,8 +39,12 @@ enum : int {
     PB_STRIDE = 244
 };
 // Sersic block offsets
-enum : int { SB_XOFF = 0, SB_YOFF = 1, SB_C = 2, SB_S = 3, SB_Q = 4, SB_QI = 5, SB_K1 = 6, SB_K0 = 7,
-             SB_C1 = 8, SB_IE = 9, SB_KQ = 10, SB_KQI = 11 };
+// The component frame is stored PRE-SCALED: x' = sqrt(q) x_r = A11 px + A12 py, y' = y_r / sqrt(q) = A21 px + A22 py, so that
+// r^2 = q x_r^2 + y_r^2 / q = x'^2 + y'^2 costs two FP64 operations instead of four.  KQ = (b_n/n) sqrt(q), KQI = (b_n/n)/sqrt(q);
+// C, S (unscaled cos/sin phi) rotate source-plane gradients back.  The adjoint's moment sums are taken in (x', y') and
+// unscaled per particle in gl_finalize_kernel (sersic_chain).
+enum : int { SB_XOFF = 0, SB_YOFF = 1, SB_C = 2, SB_S = 3, SB_A11 = 4, SB_A12 = 5, SB_K1 = 6, SB_K0 = 7,
+             SB_C1 = 8, SB_IE = 9, SB_KQ = 10, SB_KQI = 11, SB_A21 = 12, SB_A22 = 13 };
 
 // ----------------------------------------------------------------------------- natural accumulators (NA)
 // Per-ray sums the adjoint kernel produces; gl_finalize_kernel applies the per-particle chain rule in fp64.

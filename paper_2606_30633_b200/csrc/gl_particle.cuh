@@ -91,11 +91,13 @@ __device__ inline void write_sersic(const double* __restrict__ th, int off, T* s
     Ell E = make_ell(e1, e2);
     double bn = 1.9992 * n - 0.3271;
     sb[SB_XOFF] = (T)(x_first - x0); sb[SB_YOFF] = (T)(x_first - y0);
-    sb[SB_C] = (T)E.cphi; sb[SB_S] = (T)E.sphi; sb[SB_Q] = (T)E.q; sb[SB_QI] = (T)(1.0 / E.q);
+    const double sq = sqrt(E.q);
+    sb[SB_C] = (T)E.cphi; sb[SB_S] = (T)E.sphi;
+    sb[SB_A11] = (T)(sq * E.cphi); sb[SB_A12] = (T)(sq * E.sphi); sb[SB_A21] = (T)(-E.sphi / sq); sb[SB_A22] = (T)(E.cphi / sq);
     sb[SB_K1] = (T)(0.5 / n); sb[SB_K0] = (T)(-log2(R) / n);
     sb[SB_C1] = (T)(bn * 1.44269504088896340736); sb[SB_IE] = (T)Ie;
-    sb[SB_KQ] = (T)(bn / n * E.q); sb[SB_KQI] = (T)(bn / n / E.q);
-    sb[12] = sb[13] = sb[14] = sb[15] = T(0);
+    sb[SB_KQ] = (T)(bn / n * sq); sb[SB_KQI] = (T)(bn / n / sq);
+    sb[14] = sb[15] = T(0);
 }
 
 // Step A.  One WARP per particle (4 per CTA): the lanes transform the parameters in parallel into a shared-memory cache,
@@ -204,10 +206,12 @@ __device__ inline void sersic_chain(const double* __restrict__ th, int off, cons
     gth[off + 6] = T[SA_T0] / Ie;
     gth[off] = k * T[SA_T1] / R;
     gth[off + 1] = -1.9992 * (T[SA_T1] - T[SA_T0]) + bn * 0.69314718055994530942 * T[SA_T2] / n;
-    double gxr = -k * E.q * T[SA_AX], gyr = -k * T[SA_AY] / E.q;
+    // the sums were taken in the pre-scaled frame x' = sqrt(q) x_r, y' = y_r / sqrt(q) (gl_common.cuh): unscale here
+    const double sq = sqrt(E.q);
+    double gxr = -k * sq * T[SA_AX], gyr = -k * T[SA_AY] / sq;
     gth[off + 4] = -(E.cphi * gxr - E.sphi * gyr);
     gth[off + 5] = -(E.sphi * gxr + E.cphi * gyr);
-    double dq = -k * 0.5 * (T[SA_BXX] - T[SA_BYY] / (E.q * E.q));
+    double dq = -k * 0.5 * (T[SA_BXX] - T[SA_BYY]) / E.q;
     double dphi = -k * (E.q - 1.0 / E.q) * T[SA_BXY];
     ell_chain(e1, e2, E, dq, dphi, gth[off + 2], gth[off + 3]);
 }

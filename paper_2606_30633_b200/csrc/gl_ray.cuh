@@ -191,9 +191,8 @@ template <class T, bool ADJ>
 __device__ __forceinline__ SersicOut<T> sersic_eval(const typename Real<T>::Tab& tb, const T* __restrict__ sb, T px, T py) {
     using R = Real<T>;
     SersicOut<T> o;
-    const T c = sb[SB_C], s = sb[SB_S];
-    o.xr = R::fma(c, px, s * py); o.yr = R::fma(c, py, -s * px);
-    T r2 = R::fma(sb[SB_Q] * o.xr, o.xr, sb[SB_QI] * o.yr * o.yr);
+    o.xr = R::fma(sb[SB_A11], px, sb[SB_A12] * py); o.yr = R::fma(sb[SB_A21], px, sb[SB_A22] * py);   // pre-scaled frame (x', y')
+    T r2 = R::fma(o.xr, o.xr, o.yr * o.yr);
     r2 = R::max(r2, T(1e-16));
     T lr = R::lg2(tb, r2);
     o.lu = R::fma(sb[SB_K1], lr, sb[SB_K0]);
