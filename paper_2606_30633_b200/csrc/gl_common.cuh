@@ -36,6 +36,7 @@ enum : int {
     PB_SER_D = 176,                     // d_m = (m+1) a_{m+1}
     PB_SER_E = 208,                     // e_m = L_{m+1} a_{m+1}
     PB_SER_M1 = 240, PB_SER_M2 = 241,   // series bands: 4*M1 steps in T, 4*M2 steps in fp32 above them, the rest skipped
+    PB_M_H1 = 242, PB_M_H0 = 243,       // amplitude A (b/R)^(t-1) = 2^(H1 log2 R^2 + H0): H1 = -(t-1)/2, H0 = (t-1) log2 b + log2 A
     PB_STRIDE = 244
 };
 // Sersic block offsets

@@ -145,7 +145,12 @@ __global__ void __launch_bounds__(UNPACK_WPB * 32) gl_unpack_kernel(const __grid
     o[PB_M_T] = (T)t; o[PB_M_F] = (T)f; o[PB_M_L2B] = (T)log2(b); o[PB_M_A] = (T)(2 * b / (1 + E.q));
     double qp = sqrt(fmax(1 - E.q * E.q, 0.0));
     o[PB_M_QP] = (T)qp; o[PB_M_BQP] = (T)(qp > 0 ? b / qp : 0.0);
-    o[PB_M_F2] = (T)(f * f); o[PB_M_TM1] = (T)(t - 1); o[PB_M_KAPC] = (T)(0.5 * (2 - t) * b);
+    o[PB_M_F2] = (T)(f * f); o[PB_M_TM1] = (T)(t - 1);
+    {   // kappa = KAPC * amp / R with amp = A (b/R)^(t-1) (the amplitude the ray kernels form in one exp2, PB_M_H1 / _H0)
+        const double A = 2 * b / (1 + E.q);
+        o[PB_M_KAPC] = (T)(0.5 * (2 - t) * b / A);
+        o[PB_M_H1] = (T)(-0.5 * (t - 1)); o[PB_M_H0] = (T)((t - 1) * log2(b) + log2(A));
+    }
     o[PB_G1] = L.shear >= 0 ? (T)theta_at(th, L.shear) : T(0);
     o[PB_G2] = L.shear >= 0 ? (T)theta_at(th, L.shear + 1) : T(0);
     o[PB_C3] = L.mp3 >= 0 ? (T)theta_at(th, L.mp3) : T(0);

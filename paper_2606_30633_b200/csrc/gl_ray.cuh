@@ -249,11 +249,11 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
         knuth_banded<T, (ADJ ? 3 : 1), UNR>(cfs, cf32, m1, m2, p, nf2, wr, wi, Pr, Pi);
         const T P0r = Pr[0], P0i = Pi[0];
         S0r = R::fma(ce, P0r, -se * P0i); S0i = R::fma(ce, P0i, se * P0r);
-        lbr = R::fma(-T(0.5), R::lg2(tb, R2), pb[PB_M_L2B]);
-        const T Pw = R::ex2(tb, pb[PB_M_TM1] * lbr);
-        amp = pb[PB_M_A] * Pw;
+        const T lgR2 = R::lg2(tb, R2);
+        amp = R::ex2(tb, R::fma(pb[PB_M_H1], lgR2, pb[PB_M_H0]));        // A (b/R)^(t-1) in one exp2
+        if constexpr (ADJ) lbr = R::fma(-T(0.5), lgR2, pb[PB_M_L2B]);    // log2(b/R), needed by the slope derivative only
         axr = amp * S0r; ayr = amp * S0i;
-        kap = pb[PB_M_KAPC] * Pw * rinv;
+        kap = pb[PB_M_KAPC] * amp * rinv;
         if constexpr (ADJ) {
             const T Q1r = Pr[ADJ ? 1 : 0], Q1i = Pi[ADJ ? 1 : 0], Q2r = Pr[ADJ ? 2 : 0], Q2i = Pi[ADJ ? 2 : 0];
             const T ewr = R::fma(ce, wr, -se * wi), ewi = R::fma(ce, wi, se * wr);       // E w
@@ -284,8 +284,8 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
     }
     const T x = R::fma(fj, step, pb[PB_XFIRST]), y = R::fma(fi, step, pb[PB_XFIRST]);
     const T g1 = pb[PB_G1], g2 = pb[PB_G2];
-    T ax = R::fma(cph, axr, -sph * ayr) + R::fma(g1, x, g2 * y);
-    T ay = R::fma(sph, axr, cph * ayr) + R::fma(g2, x, -g1 * y);
+    T ax = R::fma(cph, axr, R::fma(-sph, ayr, R::fma(g1, x, g2 * y)));      // rotate back + shear as one FMA chain
+    T ay = R::fma(sph, axr, R::fma(cph, ayr, R::fma(g2, x, -g1 * y)));
     // multipoles about the mass centre, lab frame (S7)
     T ct = 0, st = 0, c3 = 0, s3 = 0, c4 = 0, s4 = 0, rinv_m = 0;
     if constexpr (V::MPMASK != 0) {
