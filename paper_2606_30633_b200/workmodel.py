@@ -36,15 +36,16 @@ ADJ = {
 # GL_PRECISION_F64: the same formulation on the FP64 pipe.  Counts are FP64 lane-operations (DFMA, DMUL and DADD
 # count 1 each; compares, selects, integer and FP32/MUFU seed instructions count 0).  exp2 = 8 (split 3, degree-4
 # polynomial 3, table product 2), log2 = 7, rsqrt = 4, rcp = 2 (csrc/gl_math.cuh).  Hand counts of csrc/gl_ray.cuh,
-# cross-checked against the SASS loop bodies of the config-2 kernels (195 forward, 438 adjoint FP64 instructions).
+# cross-checked against the SASS loop bodies of the config-2 kernels; revised downward whenever the formulation got
+# cheaper (round 1: 195 -> 187 forward operations per config-2 ray), never for work moved to the FP32 pipe.
 FWD64 = {
     "frame":          (22, 0),    # 18 arithmetic + rsqrt 4
     "epl_series":     (63, 0),
-    "epl_amp":        (22, 0),    # log2 7 + exp2 8 + 7
+    "epl_amp":        (20, 0),    # log2 7 + exp2 8 (A and b folded into the exponent) + 5
     "sie_closed":     (120, 0),   # libdevice atan + atanh (config 1 only; latency-bound, not rooflined)
-    "rotate_shear":   (12, 0),
+    "rotate_shear":   (10, 0),    # two 4-FMA chains + the two lab coordinates
     "multipoles":     (34, 0),
-    "sersic":         (38, 0),    # 15 arithmetic + log2 7 + 2 exp2 16
+    "sersic":         (36, 0),    # 13 arithmetic (pre-scaled frame) + log2 7 + 2 exp2 16
     "shapelet_fixed": (22, 0),    # u, v, two Gaussians through exp2
     "sum":            (0, 0),     # folded into the component counts
 }
