@@ -390,3 +390,25 @@ def test_tuned_conv_kernels_at_awkward_sizes(shape, precision):
         assert rep["n_fail"] == 0, rep
     else:
         assert rep["normwise"] <= 2e-3, rep
+
+
+@pytest.mark.parametrize("ell", [0.0, 1e-12, 1e-6, 1e-3, 0.03, 0.12, 0.3, 0.45, 0.62, 0.8, 0.95])
+def test_series_bands_across_ellipticity(ell):
+    """Every precision-band configuration of the 30-term series (gl_unpack_kernel picks the bands from f = |eps|): mass
+    ellipticity from exactly circular (the c = 0 guard of O9) to extreme, against the oracle's 30-term sum, strict bar.
+    At |eps| >= 0.62 all 30 terms run in fp64; near 0 one group of four does."""
+    import oracle
+    import torch
+    gl = _gl()
+    sp, obs, sigma, psf, z = _small_case(18, 2, 5, 1, 0, -1, 1, seed=321, n_particles=8)
+    ang = np.linspace(0.1, 2.9, 8)
+    z[:, 2] = (ell * np.cos(ang)).astype(np.float32); z[:, 3] = (ell * np.sin(ang)).astype(np.float32)
+    ref = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), None, epl_terms=30)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    lp, g = m.logpost_grad(torch.from_numpy(z).cuda())
+    lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+    fin = np.isfinite(ref["logp"])
+    assert fin.all() and np.isfinite(lp).all()
+    assert np.all(np.abs(lp - ref["logp"]) <= RTOL_LOGP * np.abs(ref["logp"]))
+    ok, rep = grad_report(g, ref["grad"])
+    assert rep["n_fail"] == 0, rep
