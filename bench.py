@@ -57,6 +57,8 @@ def parse():
     ap.add_argument("--stage", default="grad", choices=["grad", "map", "svi", "hmc"],
                     help="grad: one gl_logpost_grad call per step (the headline); map / svi / hmc: one fused gl_map_step (Adam), "
                          "gl_svi_step (AdaBelief) or gl_hmc_step (4 leapfrog steps) per step")
+    ap.add_argument("--amplitudes", default="sampled", choices=["sampled", "solved"],
+                    help="solved: backward modelling (amplitude_mode 1, DESIGN.md section 15); a diagnostic line, no cpu_baseline")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -232,6 +234,9 @@ def run_ours(a):
     truth = m0.model_image(torch.from_numpy(wl.truth_z).to(dev), sid_sys).cpu().numpy()
     m0.close()
     obs, sig = W.finish_observation(wl, truth)
+    if a.amplitudes == "solved":
+        sp.amplitude_mode = 1
+        a.no_cpu_baseline = True
     m = gl.LensModel(sp, obs, sig, wl.psf, device=dev)
     z = torch.from_numpy(wl.params).to(dev)
     sid = torch.from_numpy(wl.system_id).to(dev) if wl.system_id is not None else None
@@ -390,7 +395,7 @@ def run_ours(a):
            "config": {"workload": WORKLOAD_NAMES[k], "n_particles_per_gpu": P, "n_params": n_p,
                       "rays_per_particle": wm["rays"], "parallelism": "replicas x%d" % world, "stage": a.stage,
                       "l2": "256 MiB flush write between timed iterations; workspace %.0f MB" % (ws_bytes / 1e6),
-                      "finite_fraction": finite},
+                      "finite_fraction": finite, "amplitudes": a.amplitudes},
            "e2e": {"value": whole_job_rate(world, P * evals_per_particle, a.steps, t_e2e), "unit": UNIT, "h2d_bytes_per_step": int(h2d_bytes),
                    "d2h_bytes_per_step": int(d2h_bytes), "ms_per_step": t_e2e / a.steps * 1e3},
            "gpu_launches": launches_per_step * a.steps, "clocks": clocks, "roofline": roof}

@@ -96,6 +96,15 @@ typedef struct {
                                  v = noise_sigma^2 + max(model, 0) / exposure_time,
                                  logL = -1/2 sum [ (model - obs)^2 / v + ln v ] - (N^2/2) ln 2 pi */
     float   exposure_time;    /* t_exp of noise_model 1 (> 0; ignored otherwise) */
+    int32_t amplitude_mode;   /* 0: light amplitudes are sampled parameters ("forward" modelling);
+                                 1: "backward" modelling (NEXT-4, reading S21): every call first solves the
+                                    amplitudes (I of each Sersic block, the shapelet coefficients) by weighted least
+                                    squares against obs, a* = argmin chi^2, and evaluates logp and its gradient at a*.
+                                    The amplitude entries of params are IGNORED on input (any value, NaN included),
+                                    carry no prior and no bijector, and their gradient entries are 0; a particle whose
+                                    normal matrix is not positive definite gets logp = -INF.  Needs noise_model 0
+                                    (else GL_ERR_UNSUPPORTED).  In gl_model_image, which has no obs to invert, the
+                                    amplitude entries ARE the amplitudes, untransformed. */
     const gl_prior* priors;   /* HOST pointer, n_params entries, copied by gl_config_create */
 } gl_config_desc;
 
@@ -227,6 +236,18 @@ gl_status gl_hmc_step(const gl_config* cfg, const float* obs, const float* noise
                       const int32_t* system_id, int64_t n_chains, float step_size, int32_t n_leapfrog,
                       int32_t* out_accept, float* out_dh, void* workspace, size_t workspace_bytes,
                       void* stream /* cudaStream_t */);
+
+/* Number of light amplitudes of a configuration (S18 order: source Sersic I, shapelet coefficients, lens Sersic I's);
+ * 0 if cfg is NULL.  Defined for every amplitude_mode. */
+int32_t gl_config_n_amplitudes(const gl_config* cfg);
+
+/* Backward modelling (reading S21): solved amplitudes a* and log p~_B at a* for each particle.
+ * cfg must have amplitude_mode 1 (else GL_ERR_BAD_CONFIG).  DEVICE pointers; arguments as gl_logpost, plus
+ *   out_amp  [n_particles][gl_config_n_amplitudes] fp32, physical amplitudes (0 where logp = -INF).
+ * Workspace: gl_workspace_bytes(cfg, n_particles).  Errors as gl_logpost. */
+gl_status gl_linear_amplitudes(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
+                               const float* params, const int32_t* system_id, int64_t n_particles,
+                               float* out_amp, float* out_logp, void* workspace, size_t workspace_bytes, void* stream);
 
 /* Number of kernel launches the last call on this thread enqueued (bench.py's gpu_launches claim). */
 int64_t gl_last_launch_count(void);

@@ -50,7 +50,7 @@ class gl_config_desc(C.Structure):
                 ("multipole_mask", C.c_int32), ("n_source_sersic", C.c_int32), ("shapelet_nmax", C.c_int32),
                 ("n_lens_sersic", C.c_int32), ("param_space", C.c_int32), ("n_systems", C.c_int32),
                 ("n_params", C.c_int32), ("precision", C.c_int32), ("noise_model", C.c_int32),
-                ("exposure_time", C.c_float), ("priors", C.POINTER(gl_prior))]
+                ("exposure_time", C.c_float), ("amplitude_mode", C.c_int32), ("priors", C.POINTER(gl_prior))]
 
 
 _lib = None
@@ -93,6 +93,10 @@ def lib():
         L.gl_svi_workspace_bytes.argtypes = [vp, i64]
         L.gl_svi_step.restype = C.c_int
         L.gl_svi_step.argtypes = [vp, C.POINTER(gl_opt_desc), vp, vp, vp, vp, vp, vp, vp, i64, vp, vp, i64, vp, vp, sz, vp]
+        L.gl_config_n_amplitudes.restype = C.c_int32
+        L.gl_config_n_amplitudes.argtypes = [vp]
+        L.gl_linear_amplitudes.restype = C.c_int
+        L.gl_linear_amplitudes.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, sz, vp]
         L.gl_model_image.restype = C.c_int
         L.gl_model_image.argtypes = [vp, vp, vp, vp, i64, vp, vp, sz, vp]
         L.gl_last_launch_count.restype = i64
@@ -129,7 +133,7 @@ def gl_config_create(spec):
                        spec.multipole_mask, spec.n_source_sersic, spec.shapelet_nmax, spec.n_lens_sersic,
                        spec.param_space, spec.n_systems, int(getattr(spec, "n_params", n)),
                        int(getattr(spec, "precision", GL_PRECISION_F64)), int(getattr(spec, "noise_model", 0)),
-                       float(getattr(spec, "t_exp", 1.0)), pri)
+                       float(getattr(spec, "t_exp", 1.0)), int(getattr(spec, "amplitude_mode", 0)), pri)
     h = C.c_void_p()
     _check(lib().gl_config_create(C.byref(d), C.byref(h)), "gl_config_create")
     return h
@@ -209,6 +213,22 @@ def gl_logpost(h, obs, noise_sigma, psf, params, system_id, out_logp, workspace,
                             _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
                             _ptr(_dev(system_id, torch.int32, "system_id")), n, _ptr(_dev(out_logp, f32, "out_logp")),
                             _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)), "gl_logpost")
+
+
+def gl_config_n_amplitudes(h):
+    return int(lib().gl_config_n_amplitudes(h))
+
+
+def gl_linear_amplitudes(h, obs, noise_sigma, psf, params, system_id, out_amp, out_logp, workspace, stream=None):
+    torch = _torch()
+    f32 = torch.float32
+    n = params.shape[0]
+    _check(lib().gl_linear_amplitudes(h, _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
+                                      _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
+                                      _ptr(_dev(system_id, torch.int32, "system_id")), n,
+                                      _ptr(_dev(out_amp, f32, "out_amp")), _ptr(_dev(out_logp, f32, "out_logp")),
+                                      _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)),
+           "gl_linear_amplitudes")
 
 
 def gl_logpost_grad(h, obs, noise_sigma, psf, params, system_id, out_logp, out_grad, workspace, stream=None):
@@ -362,6 +382,16 @@ class LensModel:
         gl_logpost(self.h, self.obs, self.noise_sigma, self.psf, params, self._sid(system_id), out,
                    self.workspace(params.shape[0]), stream)
         return out
+
+    def linear_amplitudes(self, params, system_id=None, stream=None):
+        """Backward modelling (amplitude_mode 1): (solved amplitudes [n][n_amp], logp [n])."""
+        torch = _torch()
+        n = params.shape[0]
+        amp = torch.empty((n, gl_config_n_amplitudes(self.h)), dtype=torch.float32, device=self.device)
+        lp = torch.empty(n, dtype=torch.float32, device=self.device)
+        gl_linear_amplitudes(self.h, self.obs, self.noise_sigma, self.psf, params, self._sid(system_id), amp, lp,
+                             self.workspace(n), stream)
+        return amp, lp
 
     def logpost_grad(self, params, system_id=None, stream=None, out_logp=None, out_grad=None):
         torch = _torch()

@@ -16,6 +16,7 @@
 #include "gl_ray.cuh"
 #include "gl_svi.cuh"
 #include "gl_hmc.cuh"
+#include "gl_linear.cuh"
 
 using namespace gl;
 
@@ -31,6 +32,8 @@ struct gl_config {
     int n_nap;          // adjoint partials per particle = s*s*n_chunk_adj
     int n_ctile;        // chi^2 partials per particle
     ConvPlan conv;
+    AmpMap amp;         // light amplitudes (n = 0 unless amplitude_mode 1 ... see n_amp)
+    int n_amp;          // amplitude count of the model, whatever the mode
     int esize;          // sizeof the arithmetic type: 8 (GL_PRECISION_F64) or 4 (GL_PRECISION_F32)
     size_t per_particle_bytes;
 };
@@ -38,9 +41,9 @@ struct gl_config {
 static thread_local int64_t t_launches = 0;
 
 // ----------------------------------------------------------------------------- optional per-stage timing (diagnostic)
-enum { ST_PREP = 0, ST_UNPACK, ST_RAY_FWD, ST_CONV_FWD, ST_CONV_BWD, ST_RAY_ADJ, ST_FINALIZE, ST_COUNT };
+enum { ST_PREP = 0, ST_UNPACK, ST_RAY_FWD, ST_CONV_FWD, ST_CONV_BWD, ST_RAY_ADJ, ST_FINALIZE, ST_AMP, ST_COUNT };
 static const char* const k_stage_names[ST_COUNT] = {"prep", "unpack_prior", "ray_fwd", "conv_chi2", "conv_transpose",
-                                                    "ray_adjoint", "finalize"};
+                                                    "ray_adjoint", "finalize", "amplitude_solve"};
 struct StageTimer {
     bool on = false;
     std::vector<cudaEvent_t> ev;      // pairs (begin, end)
@@ -149,6 +152,8 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     if (d->psf_grid != 0 && d->psf_grid != 1) return GL_ERR_UNSUPPORTED;
     if (d->noise_model != 0 && d->noise_model != 1) return GL_ERR_BAD_CONFIG;
     if (d->noise_model == 1 && !(d->exposure_time > 0.f && std::isfinite(d->exposure_time))) return GL_ERR_BAD_CONFIG;
+    if (d->amplitude_mode != 0 && d->amplitude_mode != 1) return GL_ERR_BAD_CONFIG;
+    if (d->amplitude_mode == 1 && d->noise_model != 0) return GL_ERR_UNSUPPORTED;     // chi^2 must be quadratic in the amplitudes
     Layout L{};
     int np = layout_from_desc(*d, L);
     if (np != d->n_params || np > 128) return GL_ERR_BAD_CONFIG;
@@ -171,6 +176,20 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     for (int i = 0; i < np; ++i) {
         c->pt.kind[i] = d->priors[i].kind; c->pt.a[i] = d->priors[i].a; c->pt.b[i] = d->priors[i].b;
         c->pt.lo[i] = d->priors[i].lo; c->pt.hi[i] = d->priors[i].hi;
+    }
+    {   // light amplitudes in the flat order S18 and their PB slots
+        AmpMap& A = c->amp; A.n = 0;
+        auto add = [&](int pb_off, int shp) { A.off[A.n] = (short)pb_off; A.shp[A.n] = (unsigned char)shp; ++A.n; };
+        if (L.src >= 0) add(PB_SRC + SB_IE, 0);
+        for (int k = 0; k < L.n_coef; ++k) add(PB_SHP_A + k, 1);
+        if (L.ll0 >= 0) add(PB_LL0 + SB_IE, 0);
+        if (L.ll1 >= 0) add(PB_LL1 + SB_IE, 0);
+        c->n_amp = A.n;
+        L.amp_mode = d->amplitude_mode;
+        if (d->amplitude_mode == 1) {
+            if (A.n == 0) { delete c; return GL_ERR_BAD_CONFIG; }
+            for (int i = 0; i < np; ++i) if (is_amp(L, i)) c->pt.kind[i] = GL_PRIOR_NONE;   // no prior, no bijector (S21)
+        }
     }
     for (int i = np; i < 128; ++i) { c->pt.kind[i] = 0; c->pt.a[i] = 0; c->pt.b[i] = 1; c->pt.lo[i] = 0; c->pt.hi[i] = 1; }
     // kernel variant: the smallest compiled superset of the requested components
@@ -212,16 +231,18 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     c->n_nap = G.s * G.s * c->n_chunk_adj;
     c->per_particle_bytes = (size_t)c->esize * ((size_t)PB_STRIDE + ray_stride(G) + gpix_stride(G) + (size_t)c->n_ctile +
                                                 (size_t)c->n_nap * c->na) + sizeof(double) + 6 * 256;
+    if (d->amplitude_mode == 1) c->per_particle_bytes += (size_t)c->esize * c->n_amp * gpix_stride(G);
     *out = c;
     return GL_OK;
 }
 
 extern "C" void gl_config_destroy(gl_config* c) { delete c; }
 extern "C" int32_t gl_config_n_params(const gl_config* c) { return c ? c->L.n_params : 0; }
+extern "C" int32_t gl_config_n_amplitudes(const gl_config* c) { return c ? c->n_amp : 0; }
 
 struct Plan {
     int64_t Pc;
-    size_t off_tab, off_kt, off_w, off_sl, off_pb, off_lpd, off_ray, off_gpix, off_chi, off_nap, total;
+    size_t off_tab, off_kt, off_w, off_sl, off_pb, off_lpd, off_ray, off_gpix, off_chi, off_nap, off_comp, off_zobs, off_uw, total;
 };
 
 static Plan make_plan(const gl_config* c, int64_t P) {
@@ -243,6 +264,12 @@ static Plan make_plan(const gl_config* c, int64_t P) {
     pl.off_gpix = o; o = align256(o + es * (size_t)pl.Pc * gpix_stride(G));
     pl.off_chi = o;  o = align256(o + es * (size_t)pl.Pc * c->n_ctile);
     pl.off_nap = o;  o = align256(o + es * (size_t)pl.Pc * c->n_nap * c->na);
+    pl.off_comp = pl.off_zobs = pl.off_uw = o;
+    if (c->desc.amplitude_mode == 1) {
+        pl.off_comp = o; o = align256(o + es * (size_t)c->n_amp * pl.Pc * gpix_stride(G));
+        pl.off_zobs = o; o = align256(o + sizeof(float) * nsys * G.N * G.N);
+        pl.off_uw = o;   o = align256(o + es * nsys * G.N * G.N);
+    }
     pl.total = o;
     return pl;
 }
@@ -299,7 +326,7 @@ static void ray_adj(const gl_config* c, const T* pb, const double* tab, const T*
 template <class T>
 static gl_status run_t(const gl_config* c, int mode, const float* obs, const float* sigma, const float* psf,
                        const float* params, const int32_t* system_id, int64_t P, float* out_logp, float* out_grad,
-                       float* out_image, void* ws, const Plan& pl, cudaStream_t st) {
+                       float* out_image, float* out_amp, void* ws, const Plan& pl, cudaStream_t st) {
     const Geom& G = c->G;
     char* w = (char*)ws;
     double* tab = (double*)(w + pl.off_tab);
@@ -308,16 +335,44 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
     T* ray = (T*)(w + pl.off_ray); T* gpix = (T*)(w + pl.off_gpix);
     T* chi = (T*)(w + pl.off_chi); T* nap = (T*)(w + pl.off_nap);
     double* tab_out = sizeof(T) == 8 ? tab : nullptr;
+    const bool solve = c->desc.amplitude_mode == 1 && mode != 2;
+    T* comp = (T*)(w + pl.off_comp); float* zobs = (float*)(w + pl.off_zobs); T* unit_w = (T*)(w + pl.off_uw);
+    Layout L = c->L;
+    if (mode == 2) L.amp_mode = 0;          // gl_model_image: the amplitude entries of params are the amplitudes
 
     // sigma is not an input of gl_model_image (mode 2): prep then only builds kt (and the math tables)
     GL_STAGE(ST_PREP, st, (gl_prep_kernel<T><<<c->desc.n_systems, 256, 0, st>>>(G, psf, mode == 2 ? nullptr : sigma, sys_kt, sys_w,
                                                                              sys_sl, tab_out)));
     ++t_launches;
+    if (solve) {
+        const size_t n = (size_t)c->desc.n_systems * G.N * G.N;
+        gl_amp_fill_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, zobs, unit_w);
+        ++t_launches;
+    }
     for (int64_t base = 0; base < P; base += pl.Pc) {
         const int64_t Pc = (P - base) < pl.Pc ? (P - base) : pl.Pc;
         GL_STAGE(ST_UNPACK, st, (gl_unpack_kernel<T><<<(unsigned)((Pc + UNPACK_WPB - 1) / UNPACK_WPB), UNPACK_WPB * 32, 0, st>>>(
-            c->pt, c->L, G, c->desc.pix_scale, params + base * c->L.n_params, Pc, pb, lpd)));
+            c->pt, L, G, c->desc.pix_scale, params + base * c->L.n_params, Pc, pb, lpd)));
         ++t_launches;
+        if (solve) {     // unit-amplitude component images through steps B-D, then the normal equations (gl_linear.cuh)
+            const int na = c->amp.n;
+            for (int k = 0; k < na; ++k) {
+                gl_amp_select_kernel<T><<<(unsigned)((Pc * na + 255) / 256), 256, 0, st>>>(c->amp, k, Pc, pb);
+                ++t_launches;
+                GL_STAGE(ST_RAY_FWD, st, ray_fwd<T>(c, pb, tab, ray, Pc, st)); ++t_launches;
+                int nk = 0;
+                GL_STAGE(ST_CONV_FWD, st, nk = conv_fwd_launch<T>(c->conv, G, ray, sys_kt, unit_w, zobs, system_id, base, Pc,
+                                                 comp + (size_t)k * Pc * gpix_stride(G), chi, nullptr, st));
+                if (nk < 0) return GL_ERR_CUDA;
+                t_launches += nk;
+            }
+            const size_t sm = amp_solve_smem(na);
+            if (sm > 40 * 1024 && cudaFuncSetAttribute(gl_amp_solve_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess)
+                return GL_ERR_CUDA;
+            GL_STAGE(ST_AMP, st, (gl_amp_solve_kernel<T><<<(unsigned)Pc, 256, sm, st>>>(G, c->amp, comp, Pc, obs, sys_w, system_id, base,
+                                                                                 pb, out_amp)));
+            ++t_launches;
+        }
         GL_STAGE(ST_RAY_FWD, st, ray_fwd<T>(c, pb, tab, ray, Pc, st)); ++t_launches;
         int nl = 0;
         GL_STAGE(ST_CONV_FWD, st, nl = conv_fwd_launch<T>(c->conv, G, ray, sys_kt, sys_w, obs, system_id, base, Pc,
@@ -334,7 +389,7 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
         }
         const int wpb = 4;
         GL_STAGE(ST_FINALIZE, st, (gl_finalize_kernel<T><<<(unsigned)((Pc + wpb - 1) / wpb), wpb * 32, wpb * (NA_MAX + 256) * sizeof(double), st>>>(
-            c->pt, c->L, G, params, pb, lpd, chi, c->n_ctile, mode == 1 ? nap : nullptr, c->n_nap, c->na,
+            c->pt, L, G, params, pb, lpd, chi, c->n_ctile, mode == 1 ? nap : nullptr, c->n_nap, c->na,
             sys_sl, system_id, Pc, base, out_logp, out_grad)));
         ++t_launches;
     }
@@ -344,7 +399,7 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
 
 static gl_status run(const gl_config* c, int mode, const float* obs, const float* sigma, const float* psf,
                      const float* params, const int32_t* system_id, int64_t P, float* out_logp, float* out_grad,
-                     float* out_image, void* ws, size_t ws_bytes, cudaStream_t st) {
+                     float* out_image, void* ws, size_t ws_bytes, cudaStream_t st, float* out_amp = nullptr) {
     t_launches = 0;
     t_timer.reset();
     if (!c) return GL_ERR_NULL;
@@ -357,8 +412,8 @@ static gl_status run(const gl_config* c, int mode, const float* obs, const float
     const Plan pl = make_plan(c, P);
     if (ws_bytes < pl.total || ((uintptr_t)ws & 255) != 0) return GL_ERR_WORKSPACE;
     if (c->esize == 8)
-        return run_t<double>(c, mode, obs, sigma, psf, params, system_id, P, out_logp, out_grad, out_image, ws, pl, st);
-    return run_t<float>(c, mode, obs, sigma, psf, params, system_id, P, out_logp, out_grad, out_image, ws, pl, st);
+        return run_t<double>(c, mode, obs, sigma, psf, params, system_id, P, out_logp, out_grad, out_image, out_amp, ws, pl, st);
+    return run_t<float>(c, mode, obs, sigma, psf, params, system_id, P, out_logp, out_grad, out_image, out_amp, ws, pl, st);
 }
 
 extern "C" gl_status gl_logpost(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
@@ -373,6 +428,16 @@ extern "C" gl_status gl_logpost_grad(const gl_config* cfg, const float* obs, con
                                      float* out_logp, float* out_grad, void* workspace, size_t workspace_bytes, void* stream) {
     return run(cfg, 1, obs, noise_sigma, psf, params, system_id, n_particles, out_logp, out_grad, nullptr,
                workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+extern "C" gl_status gl_linear_amplitudes(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
+                                          const float* params, const int32_t* system_id, int64_t n_particles,
+                                          float* out_amp, float* out_logp, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!cfg) return GL_ERR_NULL;
+    if (cfg->desc.amplitude_mode != 1) return GL_ERR_BAD_CONFIG;
+    if (n_particles > 0 && !out_amp) return GL_ERR_NULL;
+    return run(cfg, 0, obs, noise_sigma, psf, params, system_id, n_particles, out_logp, nullptr, nullptr,
+               workspace, workspace_bytes, (cudaStream_t)stream, out_amp);
 }
 
 extern "C" gl_status gl_model_image(const gl_config* cfg, const float* psf, const float* params, const int32_t* system_id,

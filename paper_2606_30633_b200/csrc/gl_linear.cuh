@@ -1,0 +1,152 @@
+// gl_linear.cuh -- "backward" amplitude modelling (light intensities solved "by linear inversion";
+// SURVEY 8(f) NEXT-4; reading S21 in DESIGN.md section 15).
+//
+// The model image is linear in the light amplitudes a_k (I of each Sersic block, the shapelet coefficients).  With
+// amplitude_mode = 1 a call first renders the n_amp unit-amplitude component images A_k through the SAME step B-D
+// kernels (one pass per component with the amplitudes of PB set to the unit vector e_k), then one CTA per particle
+// forms the normal equations  M_kl = sum A_k A_l / sigma^2,  b_k = sum A_k obs / sigma^2  in fp64, factors M = L L^T,
+// writes a* = M^-1 b into PB, and the ordinary forward + adjoint path runs at a*.  Since dL/da = 0 there, the gradient
+// with respect to the other parameters is the ordinary adjoint's (envelope theorem); gl_finalize_kernel zeroes the
+// amplitude entries.  Product path only; shares nothing with oracle/.
+#pragma once
+#include "gl_common.cuh"
+
+namespace gl {
+
+constexpr int AMP_MAX = 72;          // 1 + 66 + 2 amplitudes at most (n_max = 10, two lens Sersic blocks)
+
+struct AmpMap {                      // component k -> its slot in PB
+    int n;
+    short off[AMP_MAX];              // PB offset of the amplitude
+    unsigned char shp[AMP_MAX];      // 1: shapelet coefficient (PB holds a_k / beta_s: scale by PB[PB_SHP] = 1/beta_s)
+};
+
+// PB amplitudes := unit vector e_k.  One thread per (particle, component).
+template <class T>
+__global__ void gl_amp_select_kernel(const __grid_constant__ AmpMap am, int k, int64_t Pc, T* __restrict__ pb) {
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= Pc * am.n) return;
+    const int64_t p = e / am.n; const int j = (int)(e - p * am.n);
+    T* o = pb + p * PB_STRIDE;
+    o[am.off[j]] = j == k ? (am.shp[j] ? o[PB_SHP] : T(1)) : T(0);
+}
+
+// obs = 0 and w = 1 for the component passes: step E then leaves -A_k in its g_pix output.
+template <class T>
+__global__ void gl_amp_fill_kernel(size_t n, float* __restrict__ zero_obs, T* __restrict__ unit_w) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) { zero_obs[i] = 0.f; unit_w[i] = T(1); }
+}
+
+// Normal equations + Cholesky solve.  grid = Pc, 256 threads.
+// comp: [n_amp][Pc][gpix_stride] = -A_k in the padded g_pix layout.  sys_w: 1/sigma^2.  out_amp may be NULL.
+// A particle whose normal matrix is not positive definite (a component that leaves no light on the cutout) is
+// marked invalid (PB_VALID = 0: logp = -INF, zero gradient).
+constexpr int AMP_TP = 64;           // pixels per tile
+constexpr int AMP_PPT = 10;          // pairs per thread: (AMP_MAX + 1)(AMP_MAX + 2) / 2 <= 256 * 11
+template <class T>
+__global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant__ Geom G, const __grid_constant__ AmpMap am,
+                                                           const T* __restrict__ comp, int64_t Pc,
+                                                           const float* __restrict__ obs, const T* __restrict__ sys_w,
+                                                           const int32_t* __restrict__ system_id, int64_t p_base,
+                                                           T* __restrict__ pb, float* __restrict__ out_amp) {
+    extern __shared__ double asm_[];
+    const int n = am.n, np = n + 1, NN = G.N * G.N, tid = threadIdx.x;
+    const int64_t p = blockIdx.x;
+    const int sys = system_id ? system_id[p_base + p] : 0;
+    const int npair = np * (np + 1) / 2;
+    double* ct = asm_;                                   // [np][AMP_TP + 1] tile of A_k / sigma (row n: obs / sigma); later M [n][n]
+    const int ct_sz = np * (AMP_TP + 1) > n * n ? np * (AMP_TP + 1) : n * n;
+    double* pr = asm_ + ct_sz;                           // [npair] sums, pair (k, l), l <= k, at k(k+1)/2 + l
+    double* rhs = pr + npair;                            // [n]
+    __shared__ int s_fail;
+    if (tid == 0) s_fail = 0;
+    double acc[AMP_PPT + 1]; int pk[AMP_PPT + 1], pl[AMP_PPT + 1];
+#pragma unroll
+    for (int j = 0; j <= AMP_PPT; ++j) {
+        acc[j] = 0; pk[j] = 0; pl[j] = 0;
+        const int i = tid + j * 256;
+        if (i < npair) {
+            int k = (int)((sqrt(8.0 * i + 1.0) - 1.0) * 0.5);
+            while (k * (k + 1) / 2 > i) --k;
+            while ((k + 1) * (k + 2) / 2 <= i) ++k;
+            pk[j] = k; pl[j] = i - k * (k + 1) / 2;
+        }
+    }
+    const size_t gs = gpix_stride(G);
+    for (int t0 = 0; t0 < NN; t0 += AMP_TP) {
+        __syncthreads();
+        for (int idx = tid; idx < np * AMP_TP; idx += 256) {
+            const int k = idx / AMP_TP, x = idx - k * AMP_TP, pix = t0 + x;
+            double v = 0;
+            if (pix < NN) {
+                const int r = pix / G.N, q = pix - r * G.N;
+                const double isg = sqrt((double)sys_w[(size_t)sys * NN + pix]);
+                v = k < n ? -(double)comp[((size_t)k * Pc + p) * gs + (size_t)(r + G.PADg) * G.Wg + q + G.PADg]
+                          : (double)obs[(size_t)sys * NN + pix];
+                v *= isg;
+            }
+            ct[k * (AMP_TP + 1) + x] = v;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j <= AMP_PPT; ++j) {
+            if (tid + j * 256 < npair) {
+                const double* a = ct + pk[j] * (AMP_TP + 1); const double* b = ct + pl[j] * (AMP_TP + 1);
+                double s = acc[j];
+                for (int x = 0; x < AMP_TP; ++x) s = fma(a[x], b[x], s);
+                acc[j] = s;
+            }
+        }
+    }
+#pragma unroll
+    for (int j = 0; j <= AMP_PPT; ++j) if (tid + j * 256 < npair) pr[tid + j * 256] = acc[j];
+    __syncthreads();
+    // full symmetric M and rhs
+    double* M = ct;
+    for (int idx = tid; idx < n * n; idx += 256) {
+        const int k = idx / n, l = idx - k * n; const int a = k > l ? k : l, b = k > l ? l : k;
+        M[idx] = pr[a * (a + 1) / 2 + b];
+    }
+    for (int k = tid; k < n; k += 256) rhs[k] = pr[n * (n + 1) / 2 + k];
+    __syncthreads();
+    // Cholesky, column by column (lower triangle in place)
+    for (int j = 0; j < n; ++j) {
+        if (tid == 0) {
+            const double d = M[j * n + j], d0 = pr[j * (j + 1) / 2 + j];
+            if (!(d > 1e-13 * d0) || !isfinite(d)) { s_fail = 1; M[j * n + j] = 1.0; } else M[j * n + j] = sqrt(d);
+        }
+        __syncthreads();
+        const double dj = M[j * n + j];
+        for (int i = j + 1 + tid; i < n; i += 256) M[i * n + j] /= dj;
+        __syncthreads();
+        const int m = n - j - 1;                          // trailing update of the lower triangle
+        for (int idx = tid; idx < m * m; idx += 256) {
+            const int i = j + 1 + idx / m, k = j + 1 + idx % m;
+            if (k <= i) M[i * n + k] -= M[i * n + j] * M[k * n + j];
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        for (int i = 0; i < n; ++i) { double s = rhs[i]; for (int k = 0; k < i; ++k) s -= M[i * n + k] * rhs[k]; rhs[i] = s / M[i * n + i]; }
+        for (int i = n - 1; i >= 0; --i) { double s = rhs[i]; for (int k = i + 1; k < n; ++k) s -= M[k * n + i] * rhs[k]; rhs[i] = s / M[i * n + i]; }
+        for (int i = 0; i < n; ++i) if (!isfinite(rhs[i])) s_fail = 1;
+    }
+    __syncthreads();
+    T* o = pb + p * PB_STRIDE;
+    const bool fail = s_fail != 0;
+    for (int k = tid; k < n; k += 256) {
+        const double a = fail ? 0.0 : rhs[k];
+        o[am.off[k]] = am.shp[k] ? (T)(a * (double)o[PB_SHP]) : (T)a;
+        if (out_amp) out_amp[(p_base + p) * n + k] = (float)a;
+    }
+    if (tid == 0 && fail) o[PB_VALID] = T(0);
+}
+
+static inline size_t amp_solve_smem(int n) {
+    const int np = n + 1;
+    const int ct_sz = np * (AMP_TP + 1) > n * n ? np * (AMP_TP + 1) : n * n;
+    return sizeof(double) * ((size_t)ct_sz + (size_t)np * (np + 1) / 2 + n);
+}
+
+}  // namespace gl

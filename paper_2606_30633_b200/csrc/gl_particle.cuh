@@ -14,7 +14,17 @@ struct Layout {                     // offsets into the flat parameter vector (r
     int mass, gamma, ell, shear, mp3, mp4, src, shp, ll0, ll1;
     int n_params, n_coef, nmax, param_space, mass_model;
     int ker_nmax;                   // shapelet order the selected kernel variant is compiled for (>= nmax)
+    int amp_mode;                   // 1: light amplitudes solved by linear inversion (gl_linear.cuh); their z entries are ignored
 };
+// Amplitude parameters in the flat order S18: I of each Sersic block, the shapelet coefficients.
+__host__ __device__ inline bool is_amp(const Layout& L, int i) {
+    return (L.src >= 0 && i == L.src + 6) || (L.ll0 >= 0 && i == L.ll0 + 6) || (L.ll1 >= 0 && i == L.ll1 + 6) ||
+           (L.shp >= 0 && i > L.shp && i <= L.shp + L.n_coef);
+}
+// z of parameter i as the kernels see it: a solved amplitude (amp_mode 1) reads as 1 whatever the caller stored
+__device__ __forceinline__ double z_in(const Layout& L, const float* __restrict__ z, int i) {
+    return (L.amp_mode == 1 && is_amp(L, i)) ? 1.0 : (double)z[i];
+}
 
 struct Xform { double theta, lp, logdet, dth_dz, dlp_dth, dlogdet_dz; bool ok; };
 
@@ -119,7 +129,7 @@ __global__ void __launch_bounds__(UNPACK_WPB * 32) gl_unpack_kernel(const __grid
     bool ok = true;
     double lp = 0;
     for (int i = lane; i < L.n_params; i += 32) {
-        Xform x = transform_one(pt, i, L.param_space, (double)z[i]);
+        Xform x = transform_one(pt, i, L.param_space, z_in(L, z, i));
         ok = ok && x.ok; lp += x.lp + x.logdet; th[i] = x.theta;
     }
 #pragma unroll
@@ -255,7 +265,7 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
             for (int ch = 0; ch < n_chunk; ++ch) s += (double)nap[((size_t)p * n_chunk + ch) * na + k];
             nat[k] = s;
         }
-        for (int k = lane; k < L.n_params; k += 32) { gth[k] = 0; th[k] = transform_one(pt, k, L.param_space, (double)z[k]).theta; }
+        for (int k = lane; k < L.n_params; k += 32) { gth[k] = 0; th[k] = transform_one(pt, k, L.param_space, z_in(L, z, k)).theta; }
         __syncwarp();
         if (lane == 0 && valid) {
             double thE = theta_at(th, L.mass);
@@ -299,8 +309,9 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
         // theta -> z, priors, log-det; a non-finite component invalidates the particle
         bool fin = true;
         for (int k = lane; k < L.n_params; k += 32) {
-            Xform x = transform_one(pt, k, L.param_space, (double)z[k]);
+            Xform x = transform_one(pt, k, L.param_space, z_in(L, z, k));
             double g = (gth[k] + x.dlp_dth) * x.dth_dz + x.dlogdet_dz;
+            if (L.amp_mode == 1 && is_amp(L, k)) g = 0;           // dL/da = 0 at the solved amplitudes (envelope theorem, S21)
             gth[k] = g; if (!isfinite(g)) fin = false;
         }
         fin = __all_sync(0xffffffffu, fin);

@@ -1,0 +1,123 @@
+"""GPU parity of backward amplitude modelling (amplitude_mode 1, reading S21) against
+oracle/linear.py: solved amplitudes, log-posterior at them and the envelope gradient, strict north_star bar in fp64
+mode; the amplitude entries of params are ignored (NaN included) and their gradient entries are exactly zero."""
+import copy
+
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+RTOL_LOGP = 1e-4
+
+
+def _gl():
+    import paper_2606_30633_b200 as gl
+    return gl
+
+
+def _case(n_pix, s, K, shapelet_nmax, n_lens, seed, n_particles, mass_model=1, multipoles=False):
+    import oracle
+    pri = W._default_priors(mass_model, multipoles=multipoles, shapelet_nmax=shapelet_nmax, n_lens=n_lens)
+    sp = W.LensSpec(n_pix, s, K, W._r32(0.11 * 40 / n_pix * 2.4), mass_model=mass_model, epl_terms=30,
+                    multipole_mask=3 if multipoles else 0, shapelet_nmax=shapelet_nmax, n_lens_sersic=n_lens, priors=pri,
+                    amplitude_mode=1)
+    rng = np.random.default_rng(seed)
+    step = sp.pix_scale / s
+    psf = W.gaussian_psf(K, 2.5 * step, step)[None].astype(np.float32)
+    th_true = W.draw(rng, pri, 1)
+    truth = oracle.model_image(sp, psf.astype(np.float64), th_true)
+    sigma = np.full((1, n_pix, n_pix), 0.05, np.float32)
+    obs = (truth + 0.05 * rng.standard_normal(truth.shape)).astype(np.float32)
+    z = W.z_of(pri, W.draw(rng, pri, n_particles)).astype(np.float32)
+    return sp, obs, sigma, psf, z
+
+
+def _grad_ok(g, ref):
+    tol = np.maximum(1e-3 * np.abs(ref), 1e-5)
+    return np.abs(g - ref) <= tol
+
+
+@pytest.mark.parametrize("shape", [(40, 2, 11, -1, 1), (24, 2, 5, 3, 1), (20, 3, 7, 2, 2), (16, 1, 5, -1, 0), (22, 2, 5, 7, 1)])
+def test_backward_mode_matches_oracle(shape):
+    import oracle.linear as OL
+    import torch
+    gl = _gl()
+    n_pix, s, K, nmax, nl = shape
+    sp, obs, sigma, psf, z = _case(n_pix, s, K, nmax, nl, seed=11 + n_pix, n_particles=6, multipoles=(nmax == 7))
+    amp_idx = OL.amplitude_indices(sp)
+    z[:, amp_idx] = np.float32(np.nan)                                   # ignored by contract
+    z[1, amp_idx] = 3.0
+    ref = OL.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64))
+    m = gl.LensModel(sp, obs, sigma, psf)
+    assert gl.gl_config_n_amplitudes(m.h) == len(amp_idx)
+    zt = torch.from_numpy(z).cuda()
+    lp, g = m.logpost_grad(zt)
+    amp, lp2 = m.linear_amplitudes(zt)
+    lp0 = m.logpost(zt)
+    lp, g, amp = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64), amp.cpu().numpy().astype(np.float64)
+    assert np.array_equal(lp2.cpu().numpy(), lp0.cpu().numpy())
+    fin = np.isfinite(ref["logp"])
+    assert fin.sum() >= 4 and np.array_equal(np.isfinite(lp), fin)
+    assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+    assert np.all(np.abs(lp0.cpu().numpy()[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+    assert np.all(g[:, amp_idx] == 0)
+    ok = _grad_ok(g[fin], ref["grad"][fin])
+    assert ok.all(), (np.argwhere(~ok)[:5], g[fin][~ok][:5], ref["grad"][fin][~ok][:5])
+    scale = np.abs(ref["amp"][fin]).max(axis=1, keepdims=True)
+    assert np.all(np.abs(amp[fin] - ref["amp"][fin]) <= 1e-4 * scale + 1e-6)
+
+
+def test_backward_mode_fp32_and_multi_system():
+    """fp32 arithmetic mode: norm-wise agreement; two systems with a gather map: each particle is inverted against
+    its own obs / sigma / PSF."""
+    import oracle.linear as OL
+    import torch
+    gl = _gl()
+    sp, obs, sigma, psf, z = _case(24, 2, 5, -1, 1, seed=3, n_particles=8)
+    sp2 = copy.copy(sp); sp2.n_systems = 2
+    rng = np.random.default_rng(0)
+    obs2 = np.concatenate([obs, obs[:, ::-1].copy() * 0.7]); sig2 = np.concatenate([sigma, sigma * 1.5])
+    psf2 = np.concatenate([psf, W.gaussian_psf(5, 3.5 * sp.pix_scale / 2, sp.pix_scale / 2)[None].astype(np.float32)])
+    sid = np.array([0, 1, 1, 0, 1, 0, 0, 1], dtype=np.int32)
+    ref = OL.logpost_grad(sp2, obs2, sig2, psf2, z.astype(np.float64), system_id=sid)
+    for prec, tol in [(0, 1e-5), (1, 2e-2)]:
+        spp = copy.copy(sp2); spp.precision = prec
+        m = gl.LensModel(spp, obs2, sig2, psf2)
+        lp, g = m.logpost_grad(torch.from_numpy(z).cuda(), system_id=sid)
+        lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+        fin = np.isfinite(ref["logp"])
+        assert np.array_equal(np.isfinite(lp), fin)
+        assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= (1e-4 if prec == 0 else 1e-3) * np.abs(ref["logp"][fin]))
+        num = np.linalg.norm(g[fin] - ref["grad"][fin], axis=1); den = np.linalg.norm(ref["grad"][fin], axis=1)
+        assert np.all(num <= tol * den), (prec, num / den)
+
+
+def test_backward_mode_config_errors_and_model_image():
+    import torch
+    gl = _gl()
+    sp, obs, sigma, psf, z = _case(16, 2, 5, -1, 1, seed=2, n_particles=3)
+    bad = copy.copy(sp); bad.noise_model = 1; bad.t_exp = 100.0
+    with pytest.raises(gl.GLError):
+        gl.gl_config_create(bad)
+    fwd = copy.copy(sp); fwd.amplitude_mode = 0
+    m0 = gl.LensModel(fwd, obs, sigma, psf)
+    with pytest.raises(gl.GLError):
+        m0.linear_amplitudes(torch.from_numpy(z).cuda())
+    # gl_model_image in backward mode: the amplitude entries are the amplitudes -> image at a* has the solved chi^2
+    m = gl.LensModel(sp, obs, sigma, psf)
+    zt = torch.from_numpy(z).cuda()
+    amp, lp = m.linear_amplitudes(zt)
+    import oracle.linear as OL
+    idx = OL.amplitude_indices(sp)
+    z2 = zt.clone(); z2[:, torch.as_tensor(idx).cuda()] = amp
+    img = m.model_image(z2).cpu().numpy().astype(np.float64)
+    ref = OL.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), want_grad=False)
+    import oracle
+    sb = OL.backward_spec(sp)
+    rows = z.astype(np.float64).copy(); rows[:, idx] = ref["amp"]
+    theta = np.array([[oracle.transform_one(sb.priors[i], 0, v)["theta"] for i, v in enumerate(r)] for r in rows])
+    ref_img = oracle.model_image(sb, psf.astype(np.float64), theta)
+    assert np.allclose(img, ref_img, rtol=2e-4, atol=2e-4 * np.abs(ref_img).max())

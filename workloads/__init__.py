@@ -51,6 +51,7 @@ class LensSpec:
     psf_grid: int = 0            # 0: PSF taps on the ray grid (S10); 1: on the detector grid (NEXT-4, S10b)
     noise_model: int = 0         # 0: fixed sigma map (S12); 1: variance sigma^2 + max(model,0)/t_exp (NEXT-4, S12b)
     t_exp: float = 1.0           # exposure time of noise_model 1
+    amplitude_mode: int = 0      # 0: amplitudes sampled ("forward"); 1: solved by linear inversion ("backward", NEXT-4, S21)
     precision: int = 0           # 0 GL_PRECISION_F64, 1 GL_PRECISION_F32 (CUDA path only; the oracle is always fp64)
     priors: list = field(default_factory=list)
     names: list = field(default_factory=list)
