@@ -58,7 +58,7 @@ def parse():
                     help="grad: one gl_logpost_grad call per step (the headline); map / svi / hmc: one fused gl_map_step (Adam), "
                          "gl_svi_step (AdaBelief) or gl_hmc_step (4 leapfrog steps) per step")
     ap.add_argument("--amplitudes", default="sampled", choices=["sampled", "solved"],
-                    help="solved: backward modelling (amplitude_mode 1, DESIGN.md section 15); a diagnostic line, no cpu_baseline")
+                    help="solved: backward modelling (amplitude_mode 1, DESIGN.md section 16); a diagnostic line, no cpu_baseline")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()

@@ -3,7 +3,7 @@
 
 TEST INFRASTRUCTURE ONLY (see oracle/__init__.py).  Plain numpy on top of the C oracle's model images.
 
-Reading S21 (DESIGN.md section 15; the paper gives no formula).  The model image is linear in the light
+Reading S21 (DESIGN.md section 16; the paper gives no formula).  The model image is linear in the light
 amplitudes a = (I of the source Sersic, the shapelet coefficients, I of each lens Sersic), in the flat order S18:
     model = sum_k a_k A_k,     A_k = image of component k with unit amplitude, PSF-convolved and binned (O3-O6).
 With the fixed noise map sigma (S12) the Gaussian likelihood is quadratic in a, and linear inversion is the weighted

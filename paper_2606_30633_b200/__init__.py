@@ -23,7 +23,7 @@ EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_wo
            "gl_last_launch_count", "gl_status_string", "gl_version", "gl_stage_timing_enable", "gl_stage_count",
            "gl_stage_name", "gl_stage_times", "gl_probe_pipe", "gl_map_step",
            "gl_svi_workspace_bytes", "gl_svi_step", "gl_hmc_workspace_bytes", "gl_hmc_step",
-           "gl_best_particle"]
+           "gl_best_particle", "gl_config_n_amplitudes", "gl_linear_amplitudes"]
 
 
 class GLError(RuntimeError):

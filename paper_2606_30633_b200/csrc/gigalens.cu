@@ -3,6 +3,7 @@
 #include "../../include/gigalens.h"
 
 #include <cmath>
+#include <algorithm>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -32,6 +33,7 @@ struct gl_config {
     int n_nap;          // adjoint partials per particle = s*s*n_chunk_adj
     int n_ctile;        // chi^2 partials per particle
     ConvPlan conv;
+    CompIdx cidx;       // component index of each light block (gl_ray_comp_kernel)
     AmpMap amp;         // light amplitudes (n = 0 unless amplitude_mode 1 ... see n_amp)
     int n_amp;          // amplitude count of the model, whatever the mode
     int esize;          // sizeof the arithmetic type: 8 (GL_PRECISION_F64) or 4 (GL_PRECISION_F32)
@@ -180,10 +182,12 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     {   // light amplitudes in the flat order S18 and their PB slots
         AmpMap& A = c->amp; A.n = 0;
         auto add = [&](int pb_off, int shp) { A.off[A.n] = (short)pb_off; A.shp[A.n] = (unsigned char)shp; ++A.n; };
-        if (L.src >= 0) add(PB_SRC + SB_IE, 0);
+        CompIdx& ci = c->cidx; ci.src = ci.shp0 = ci.ll0 = ci.ll1 = -1; ci.n_coef = L.n_coef;
+        if (L.src >= 0) { ci.src = A.n; add(PB_SRC + SB_IE, 0); }
+        if (L.n_coef > 0) ci.shp0 = A.n;
         for (int k = 0; k < L.n_coef; ++k) add(PB_SHP_A + k, 1);
-        if (L.ll0 >= 0) add(PB_LL0 + SB_IE, 0);
-        if (L.ll1 >= 0) add(PB_LL1 + SB_IE, 0);
+        if (L.ll0 >= 0) { ci.ll0 = A.n; add(PB_LL0 + SB_IE, 0); }
+        if (L.ll1 >= 0) { ci.ll1 = A.n; add(PB_LL1 + SB_IE, 0); }
         c->n_amp = A.n;
         L.amp_mode = d->amplitude_mode;
         if (d->amplitude_mode == 1) {
@@ -231,7 +235,7 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     c->n_nap = G.s * G.s * c->n_chunk_adj;
     c->per_particle_bytes = (size_t)c->esize * ((size_t)PB_STRIDE + ray_stride(G) + gpix_stride(G) + (size_t)c->n_ctile +
                                                 (size_t)c->n_nap * c->na) + sizeof(double) + 6 * 256;
-    if (d->amplitude_mode == 1) c->per_particle_bytes += (size_t)c->esize * c->n_amp * gpix_stride(G);
+    if (d->amplitude_mode == 1) c->per_particle_bytes += (size_t)c->esize * c->n_amp * (gpix_stride(G) + ray_stride(G));
     *out = c;
     return GL_OK;
 }
@@ -242,7 +246,7 @@ extern "C" int32_t gl_config_n_amplitudes(const gl_config* c) { return c ? c->n_
 
 struct Plan {
     int64_t Pc;
-    size_t off_tab, off_kt, off_w, off_sl, off_pb, off_lpd, off_ray, off_gpix, off_chi, off_nap, off_comp, off_zobs, off_uw, total;
+    size_t off_tab, off_kt, off_w, off_sl, off_pb, off_lpd, off_ray, off_gpix, off_chi, off_nap, off_comp, off_cray, off_zobs, off_uw, off_sid, total;
 };
 
 static Plan make_plan(const gl_config* c, int64_t P) {
@@ -264,11 +268,13 @@ static Plan make_plan(const gl_config* c, int64_t P) {
     pl.off_gpix = o; o = align256(o + es * (size_t)pl.Pc * gpix_stride(G));
     pl.off_chi = o;  o = align256(o + es * (size_t)pl.Pc * c->n_ctile);
     pl.off_nap = o;  o = align256(o + es * (size_t)pl.Pc * c->n_nap * c->na);
-    pl.off_comp = pl.off_zobs = pl.off_uw = o;
+    pl.off_comp = pl.off_cray = pl.off_zobs = pl.off_uw = pl.off_sid = o;
     if (c->desc.amplitude_mode == 1) {
         pl.off_comp = o; o = align256(o + es * (size_t)c->n_amp * pl.Pc * gpix_stride(G));
+        pl.off_cray = o; o = align256(o + es * (size_t)c->n_amp * pl.Pc * ray_stride(G));
         pl.off_zobs = o; o = align256(o + sizeof(float) * nsys * G.N * G.N);
         pl.off_uw = o;   o = align256(o + es * nsys * G.N * G.N);
+        pl.off_sid = o;  o = align256(o + sizeof(int32_t) * (size_t)c->n_amp * pl.Pc);
     }
     pl.total = o;
     return pl;
@@ -307,6 +313,24 @@ static void ray_fwd(const gl_config* c, const T* pb, const double* tab, T* ray, 
         case 3: launch_ray_fwd<T, V_E1>(c, pb, tab, ray, Pc, st); break;
         case 4: launch_ray_fwd<T, V_S2>(c, pb, tab, ray, Pc, st); break;
         default: launch_ray_fwd<T, V_E2>(c, pb, tab, ray, Pc, st); break;
+    }
+}
+template <class T, class V>
+static void launch_ray_comp(const gl_config* c, const T* pb, const double* tab, T* cray, int64_t Pc, cudaStream_t st) {
+    dim3 grid(c->G.s * c->G.s * c->n_chunk_fwd, (unsigned)Pc);
+    gl_ray_comp_kernel<T, V, NT_FWD><<<grid, c->nt_fwd, 0, st>>>(c->G, c->cidx, c->amp.n, pb, tab, cray, (size_t)Pc * ray_stride(c->G),
+                                                                 c->rpt_fwd, c->n_chunk_fwd);
+}
+template <class T>
+static void ray_comp(const gl_config* c, const T* pb, const double* tab, T* cray, int64_t Pc, cudaStream_t st) {
+    const int id = c->variant * 2 + c->desc.mass_model;
+    switch (id) {
+        case 0: launch_ray_comp<T, V_S0>(c, pb, tab, cray, Pc, st); break;
+        case 1: launch_ray_comp<T, V_E0>(c, pb, tab, cray, Pc, st); break;
+        case 2: launch_ray_comp<T, V_S1>(c, pb, tab, cray, Pc, st); break;
+        case 3: launch_ray_comp<T, V_E1>(c, pb, tab, cray, Pc, st); break;
+        case 4: launch_ray_comp<T, V_S2>(c, pb, tab, cray, Pc, st); break;
+        default: launch_ray_comp<T, V_E2>(c, pb, tab, cray, Pc, st); break;
     }
 }
 template <class T>
@@ -356,13 +380,24 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
         ++t_launches;
         if (solve) {     // unit-amplitude component images through steps B-D, then the normal equations (gl_linear.cuh)
             const int na = c->amp.n;
-            for (int k = 0; k < na; ++k) {
-                gl_amp_select_kernel<T><<<(unsigned)((Pc * na + 255) / 256), 256, 0, st>>>(c->amp, k, Pc, pb);
+            T* cray = (T*)(w + pl.off_cray);
+            gl_amp_select_kernel<T><<<(unsigned)((Pc * na + 255) / 256), 256, 0, st>>>(c->amp, -1, Pc, pb);
+            ++t_launches;
+            GL_STAGE(ST_RAY_FWD, st, ray_comp<T>(c, pb, tab, cray, Pc, st)); ++t_launches;
+            // step D for all components as na * Pc virtual particles (component-major, like both buffers)
+            int32_t* sid_exp = nullptr;
+            if (system_id) {
+                sid_exp = (int32_t*)(w + pl.off_sid);
+                gl_amp_sid_kernel<<<(unsigned)((Pc * na + 255) / 256), 256, 0, st>>>(system_id + base, Pc, na, sid_exp);
                 ++t_launches;
-                GL_STAGE(ST_RAY_FWD, st, ray_fwd<T>(c, pb, tab, ray, Pc, st)); ++t_launches;
+            }
+            const int kg = c->conv.kind == 0 ? (int)std::max<int64_t>(1, 65535 / Pc) : na;    // generic kernels: grid.y <= 65535
+            for (int k = 0; k < na; k += kg) {
+                const int nk_c = std::min(kg, na - k);
                 int nk = 0;
-                GL_STAGE(ST_CONV_FWD, st, nk = conv_fwd_launch<T>(c->conv, G, ray, sys_kt, unit_w, zobs, system_id, base, Pc,
-                                                 comp + (size_t)k * Pc * gpix_stride(G), chi, nullptr, st));
+                GL_STAGE(ST_CONV_FWD, st, nk = conv_fwd_launch<T>(c->conv, G, cray + (size_t)k * Pc * ray_stride(G), sys_kt, unit_w, zobs,
+                                                 sid_exp ? sid_exp + (size_t)k * Pc : nullptr, 0, (int64_t)nk_c * Pc,
+                                                 comp + (size_t)k * Pc * gpix_stride(G), nullptr, nullptr, st));
                 if (nk < 0) return GL_ERR_CUDA;
                 t_launches += nk;
             }
@@ -370,16 +405,18 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
             if (sm > 40 * 1024 && cudaFuncSetAttribute(gl_amp_solve_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess)
                 return GL_ERR_CUDA;
             GL_STAGE(ST_AMP, st, (gl_amp_solve_kernel<T><<<(unsigned)Pc, 256, sm, st>>>(G, c->amp, comp, Pc, obs, sys_w, system_id, base,
-                                                                                 pb, out_amp)));
+                                                                                 pb, out_amp, gpix, chi, c->n_ctile)));
             ++t_launches;
         }
-        GL_STAGE(ST_RAY_FWD, st, ray_fwd<T>(c, pb, tab, ray, Pc, st)); ++t_launches;
         int nl = 0;
-        GL_STAGE(ST_CONV_FWD, st, nl = conv_fwd_launch<T>(c->conv, G, ray, sys_kt, sys_w, obs, system_id, base, Pc,
-                                         mode == 2 ? nullptr : gpix, mode == 2 ? nullptr : chi,
-                                         mode == 2 ? out_image : nullptr, st));
-        if (nl < 0) return GL_ERR_CUDA;
-        t_launches += nl;
+        if (!solve) {      // backward modelling: gl_amp_solve_kernel has already written g_pix and chi^2 at a*
+            GL_STAGE(ST_RAY_FWD, st, ray_fwd<T>(c, pb, tab, ray, Pc, st)); ++t_launches;
+            GL_STAGE(ST_CONV_FWD, st, nl = conv_fwd_launch<T>(c->conv, G, ray, sys_kt, sys_w, obs, system_id, base, Pc,
+                                             mode == 2 ? nullptr : gpix, mode == 2 ? nullptr : chi,
+                                             mode == 2 ? out_image : nullptr, st));
+            if (nl < 0) return GL_ERR_CUDA;
+            t_launches += nl;
+        }
         if (mode == 2) continue;
         if (mode == 1) {
             GL_STAGE(ST_CONV_BWD, st, nl = conv_bwd_launch<T>(c->conv, G, gpix, sys_kt, system_id, base, Pc, ray, st));

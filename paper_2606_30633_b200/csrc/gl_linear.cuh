@@ -1,15 +1,18 @@
 // gl_linear.cuh -- "backward" amplitude modelling (light intensities solved "by linear inversion";
-// SURVEY 8(f) NEXT-4; reading S21 in DESIGN.md section 15).
+// SURVEY 8(f) NEXT-4; reading S21 in DESIGN.md section 16).
 //
 // The model image is linear in the light amplitudes a_k (I of each Sersic block, the shapelet coefficients).  With
-// amplitude_mode = 1 a call first renders the n_amp unit-amplitude component images A_k through the SAME step B-D
-// kernels (one pass per component with the amplitudes of PB set to the unit vector e_k), then one CTA per particle
+// amplitude_mode = 1 a call first renders the n_amp unit-amplitude component images A_k: ONE pass of steps B-C
+// (gl_ray_comp_kernel: one deflection per ray, every component stored separately) and the step-D kernel once per
+// component (obs = 0, w = 1: its g_pix output is -A_k), then one CTA per particle
 // forms the normal equations  M_kl = sum A_k A_l / sigma^2,  b_k = sum A_k obs / sigma^2  in fp64, factors M = L L^T,
-// writes a* = M^-1 b into PB, and the ordinary forward + adjoint path runs at a*.  Since dL/da = 0 there, the gradient
+// writes a* = M^-1 b into PB and, step D being linear, g_pix and chi^2 at a* from the same component images; the
+// transpose of step D and the ordinary adjoint then run at a*.  Since dL/da = 0 there, the gradient
 // with respect to the other parameters is the ordinary adjoint's (envelope theorem); gl_finalize_kernel zeroes the
 // amplitude entries.  Product path only; shares nothing with oracle/.
 #pragma once
 #include "gl_common.cuh"
+#include "gl_conv.cuh"
 
 namespace gl {
 
@@ -21,14 +24,14 @@ struct AmpMap {                      // component k -> its slot in PB
     unsigned char shp[AMP_MAX];      // 1: shapelet coefficient (PB holds a_k / beta_s: scale by PB[PB_SHP] = 1/beta_s)
 };
 
-// PB amplitudes := unit vector e_k.  One thread per (particle, component).
+// PB amplitudes := unit vector e_k (k < 0: every amplitude 1).  One thread per (particle, component).
 template <class T>
 __global__ void gl_amp_select_kernel(const __grid_constant__ AmpMap am, int k, int64_t Pc, T* __restrict__ pb) {
     const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= Pc * am.n) return;
     const int64_t p = e / am.n; const int j = (int)(e - p * am.n);
     T* o = pb + p * PB_STRIDE;
-    o[am.off[j]] = j == k ? (am.shp[j] ? o[PB_SHP] : T(1)) : T(0);
+    o[am.off[j]] = (j == k || k < 0) ? (am.shp[j] ? o[PB_SHP] : T(1)) : T(0);
 }
 
 // obs = 0 and w = 1 for the component passes: step E then leaves -A_k in its g_pix output.
@@ -36,6 +39,12 @@ template <class T>
 __global__ void gl_amp_fill_kernel(size_t n, float* __restrict__ zero_obs, T* __restrict__ unit_w) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) { zero_obs[i] = 0.f; unit_w[i] = T(1); }
+}
+
+// system_id of the na * Pc virtual particles of the component passes (component-major).
+__global__ void gl_amp_sid_kernel(const int32_t* __restrict__ sid, int64_t Pc, int na, int32_t* __restrict__ out) {
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < Pc * na) out[e] = sid[e % Pc];
 }
 
 // Normal equations + Cholesky solve.  grid = Pc, 256 threads.
@@ -49,7 +58,8 @@ __global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant
                                                            const T* __restrict__ comp, int64_t Pc,
                                                            const float* __restrict__ obs, const T* __restrict__ sys_w,
                                                            const int32_t* __restrict__ system_id, int64_t p_base,
-                                                           T* __restrict__ pb, float* __restrict__ out_amp) {
+                                                           T* __restrict__ pb, float* __restrict__ out_amp,
+                                                           T* __restrict__ gpix, T* __restrict__ chi, int n_ctile) {
     extern __shared__ double asm_[];
     const int n = am.n, np = n + 1, NN = G.N * G.N, tid = threadIdx.x;
     const int64_t p = blockIdx.x;
@@ -58,7 +68,7 @@ __global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant
     double* ct = asm_;                                   // [np][AMP_TP + 1] tile of A_k / sigma (row n: obs / sigma); later M [n][n]
     const int ct_sz = np * (AMP_TP + 1) > n * n ? np * (AMP_TP + 1) : n * n;
     double* pr = asm_ + ct_sz;                           // [npair] sums, pair (k, l), l <= k, at k(k+1)/2 + l
-    double* rhs = pr + npair;                            // [n]
+    double* rhs = pr + (npair > 256 ? npair : 256);     // [n]  (pr doubles as the 256-entry reduction buffer at the end)
     __shared__ int s_fail;
     if (tid == 0) s_fail = 0;
     double acc[AMP_PPT + 1]; int pk[AMP_PPT + 1], pl[AMP_PPT + 1];
@@ -141,12 +151,32 @@ __global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant
         if (out_amp) out_amp[(p_base + p) * n + k] = (float)a;
     }
     if (tid == 0 && fail) o[PB_VALID] = T(0);
+    // Step E at a*: the model image is sum_k a*_k A_k (step D is linear), so g_pix and chi^2 follow from the component
+    // images already in memory and the forward passes B-D need not run again.
+    T* gp = gpix + (size_t)p * gs;
+    zero_gpix_border(G, gp, tid, 256);
+    double c2 = 0;
+    for (int pix = tid; pix < NN; pix += 256) {
+        const int r = pix / G.N, q = pix - r * G.N;
+        const size_t at = (size_t)(r + G.PADg) * G.Wg + q + G.PADg;
+        double m = 0;
+        for (int k = 0; k < n; ++k) m = fma(-rhs[k], (double)comp[((size_t)k * Pc + p) * gs + at], m);
+        const double w = (double)sys_w[(size_t)sys * NN + pix], res = m - (double)obs[(size_t)sys * NN + pix];
+        gp[at] = fail ? T(0) : (T)(-res * w);
+        c2 = fma(res * res, w, c2);
+    }
+    __syncthreads();                                      // pr is free again: block sum in fixed order
+    pr[tid] = c2;
+    __syncthreads();
+    for (int o2 = 128; o2 > 0; o2 >>= 1) { if (tid < o2) pr[tid] += pr[tid + o2]; __syncthreads(); }
+    for (int k = tid; k < n_ctile; k += 256) chi[(size_t)p * n_ctile + k] = k == 0 && !fail ? (T)pr[0] : T(0);
 }
 
 static inline size_t amp_solve_smem(int n) {
     const int np = n + 1;
     const int ct_sz = np * (AMP_TP + 1) > n * n ? np * (AMP_TP + 1) : n * n;
-    return sizeof(double) * ((size_t)ct_sz + (size_t)np * (np + 1) / 2 + n);
+    const size_t npair = (size_t)np * (np + 1) / 2;
+    return sizeof(double) * ((size_t)ct_sz + (npair > 256 ? npair : 256) + n);
 }
 
 }  // namespace gl

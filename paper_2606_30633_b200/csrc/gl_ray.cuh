@@ -220,12 +220,18 @@ __device__ __forceinline__ void sersic_accum(const SersicOut<T>& o, T g, T* __re
 // accumulators spill (measured: shared memory wins only there).
 template <class T, class V> __host__ __device__ constexpr bool coef_in_smem() { return sizeof(T) == 8 && V::NMAX > 6; }
 
+// Component slots of backward modelling (gl_linear.cuh): index of each light component among the amplitudes, -1 = absent.
+struct CompIdx { int src, shp0, n_coef, ll0, ll1; };
+
 // Everything one ray needs.  ADJ = false: returns the surface brightness; ADJ = true: accumulates gbar * dI/d(natural).
-template <class T, class V, bool ADJ>
+// COMP (with ADJ = false; PB amplitudes all set to unity): also stores the surface brightness of every light component
+// separately, component k at acc[k * cstride] (acc = this ray's element of component 0).
+template <class T, class V, bool ADJ, bool COMP = false>
 __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* __restrict__ pb,
                                       const T* __restrict__ cfs, const float* __restrict__ cf32, T fj, T fi, T gbar,
                                       T* __restrict__ acc,
-                                      T* __restrict__ sacc = nullptr, int sstride = 0) {
+                                      T* __restrict__ sacc = nullptr, int sstride = 0,
+                                      const CompIdx* ci = nullptr, size_t cstride = 0) {
     using R = Real<T>;
     const T step = pb[PB_STEP];
     const T cph = pb[PB_M_C], sph = pb[PB_M_S];
@@ -309,6 +315,7 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
         const T px = R::fma(fj, step, sb[SB_XOFF]) - ax, py = R::fma(fi, step, sb[SB_YOFF]) - ay;   // beta - centre
         SersicOut<T> o = sersic_eval<T, ADJ>(tb, sb, px, py);
         Iray += o.I;
+        if constexpr (COMP) { if (ci->src >= 0) acc[(size_t)ci->src * cstride] = o.I; }
         if constexpr (ADJ) {
             sersic_accum(o, gbar, acc + NA_SRC);
             const T Ixr = -sb[SB_KQ] * o.Iu_r2 * o.xr, Iyr = -sb[SB_KQI] * o.Iu_r2 * o.yr;
@@ -322,7 +329,17 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
             hermite<T, NM>(tb, u, fu); hermite<T, NM>(tb, v, fv);
             const T* a = pb + PB_SHP_A;
             T Ish = T(0.);
-            if constexpr (!ADJ) {
+            if constexpr (COMP) {                    // basis function k with unit coefficient: phi_n1(u) phi_n2(v) / beta_s
+#pragma unroll
+                for (int n2 = 0; n2 <= NM; ++n2) {
+                    const T fvb = fv[n2] * ibs;
+#pragma unroll
+                    for (int n1 = 0; n1 <= NM - n2; ++n1) {
+                        const int idx = (n1 + n2) * (n1 + n2 + 1) / 2 + n2;
+                        if (idx < ci->n_coef) acc[(size_t)(ci->shp0 + idx) * cstride] = fu[n1] * fvb;
+                    }
+                }
+            } else if constexpr (!ADJ) {
 #pragma unroll
                 for (int n2 = 0; n2 <= NM; ++n2) {
                     T row = T(0.);
@@ -365,11 +382,13 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
         const T* sb = pb + PB_LL0;
         SersicOut<T> o = sersic_eval<T, ADJ>(tb, sb, R::fma(fj, step, sb[SB_XOFF]), R::fma(fi, step, sb[SB_YOFF]));
         Iray += o.I; if constexpr (ADJ) sersic_accum(o, gbar, acc + NA_LL0);
+        if constexpr (COMP) { if (ci->ll0 >= 0) acc[(size_t)ci->ll0 * cstride] = o.I; }
     }
     if constexpr (V::NLL >= 2) {
         const T* sb = pb + PB_LL1;
         SersicOut<T> o = sersic_eval<T, ADJ>(tb, sb, R::fma(fj, step, sb[SB_XOFF]), R::fma(fi, step, sb[SB_YOFF]));
         Iray += o.I; if constexpr (ADJ) sersic_accum(o, gbar, acc + NA_LL1);
+        if constexpr (COMP) { if (ci->ll1 >= 0) acc[(size_t)ci->ll1 * cstride] = o.I; }
     }
     if constexpr (ADJ) {
         // mass parameters enter through beta only: d/dtheta_mass = -(gbar grad_beta I_src) . dalpha/dtheta_mass
@@ -494,6 +513,45 @@ __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ 
 #pragma unroll
         for (int b = 0; b < RB; ++b)
             if (ok[b]) out[o[b]] = valid ? v[b] : T(0.);
+    }
+}
+
+// Component images of backward modelling: steps B-C once per ray (one deflection), every light component with unit
+// amplitude stored in its own RAY buffer: comp_ray [n_amp][Pc][ray_stride].  Same grid as gl_ray_fwd_kernel.
+template <class T, class V, int NT>
+__global__ void __launch_bounds__(NT) gl_ray_comp_kernel(const __grid_constant__ Geom G, const __grid_constant__ CompIdx ci, int n_amp,
+                                                         const T* __restrict__ pbg, const double* __restrict__ tabg,
+                                                         T* __restrict__ comp_ray, size_t cstride, int RPT, int n_chunk) {
+    __shared__ __align__(16) T pb[PB_STRIDE];
+    __shared__ __align__(128) double tabs[TabStage<T>::N];
+    const int p = blockIdx.y;
+    const T* src = pbg + (size_t)p * PB_STRIDE;
+    for (int k = threadIdx.x; k < V::PB_NEED; k += blockDim.x) pb[k] = src[k];
+    __shared__ __align__(16) T cfs[V::MASS == 1 ? 3 * SER_PITCH : 4];
+    __shared__ __align__(16) float cf32[(sizeof(T) == 8 && V::MASS == 1) ? 3 * SER_PITCH : 4];
+    if constexpr (V::MASS == 1) stage_series<T>(src, cfs, cf32);
+    const typename Real<T>::Tab tb = TabStage<T>::make(tabs, tabg);
+    __syncthreads();
+    PlaneIter it(G, n_chunk, RPT);
+    T* out = comp_ray + (size_t)p * ray_stride(G) + (size_t)it.ph * G.Hp * G.Wp;
+    {
+        const int ck = blockIdx.x - it.ph * n_chunk, tot = G.Hp * G.Wp;
+        for (int e = ck * blockDim.x + threadIdx.x; e < tot; e += n_chunk * blockDim.x) {
+            const int r = e / G.Wp, cc = e - r * G.Wp;
+            if (r < it.oa || r >= it.oa + G.N || cc < it.ob || cc >= it.ob + G.N)
+                for (int k = 0; k < n_amp; ++k) out[(size_t)k * cstride + e] = T(0.);
+        }
+    }
+    const int NN = G.N * G.N;
+    const bool valid = pb[PB_VALID] != T(0.);
+    for (int r = 0; r < RPT; ++r) {
+        int off = 0; asm volatile("" : "+r"(off));
+        if (it.idx < NN) {
+            T* o = out + it.offset(G);
+            if (valid) ray_eval<T, V, false, true>(tb, pb + off, cfs + off, cf32 + off, it.fj<T>(G), it.fi<T>(G), T(0.), o, nullptr, 0, &ci, cstride);
+            else for (int k = 0; k < n_amp; ++k) o[(size_t)k * cstride] = T(0.);
+        }
+        it.next(G);
     }
 }
 

@@ -99,7 +99,7 @@ def test_argument_checks_precede_any_cuda_call(gl):
     assert L.gl_workspace_bytes(null, 8) == 0 and L.gl_config_n_params(null) == 0
     for s in range(0, -7, -1):
         assert L.gl_status_string(s).decode().startswith("GL_")
-    assert L.gl_stage_count() == 7 and L.gl_stage_name(2).decode() == "ray_fwd"
+    assert L.gl_stage_count() == 8 and L.gl_stage_name(2).decode() == "ray_fwd" and L.gl_stage_name(7).decode() == "amplitude_solve"
     gl.gl_config_destroy(h)
 
 
@@ -109,3 +109,28 @@ def test_binding_refuses_to_compute_without_cuda(gl):
         pytest.skip("CUDA present")
     with pytest.raises(RuntimeError):
         gl.LensModel(W.make_spec(1), None, None, None)
+
+
+def test_amplitude_mode_is_validated_on_the_host(gl):
+    """amplitude_mode 1 (backward modelling): accepted with the fixed noise map, refused with the model-dependent
+    variance; gl_config_n_amplitudes counts I of each Sersic block and the shapelet coefficients."""
+    sp = W.make_spec(3)
+    h = gl.gl_config_create(sp)
+    n_names = sum(1 for n in W.param_names(sp.mass_model, sp.has_shear, sp.multipole_mask, sp.n_source_sersic,
+                                           sp.shapelet_nmax, sp.n_lens_sersic) if n.endswith(".I") or n.startswith("shp.a"))
+    assert gl.gl_config_n_amplitudes(h) == n_names
+    gl.gl_config_destroy(h)
+    sp.amplitude_mode = 1
+    h = gl.gl_config_create(sp)
+    assert gl.gl_workspace_bytes(h, 16) > 0
+    L = gl.lib()
+    null = C.c_void_p(0)
+    assert L.gl_linear_amplitudes(h, null, null, null, null, null, 0, null, null, null, 0, null) == 0
+    assert L.gl_linear_amplitudes(h, null, null, null, null, null, 4, null, null, null, 0, null) == -1
+    gl.gl_config_destroy(h)
+    sp.noise_model = 1; sp.t_exp = 100.0
+    with pytest.raises(gl.GLError):
+        gl.gl_config_create(sp)
+    sp.noise_model = 0; sp.amplitude_mode = 2
+    with pytest.raises(gl.GLError):
+        gl.gl_config_create(sp)
