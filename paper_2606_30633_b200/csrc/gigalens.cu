@@ -405,7 +405,7 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
             if (sm > 40 * 1024 && cudaFuncSetAttribute(gl_amp_solve_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) != cudaSuccess)
                 return GL_ERR_CUDA;
             GL_STAGE(ST_AMP, st, (gl_amp_solve_kernel<T><<<(unsigned)Pc, 256, sm, st>>>(G, c->amp, comp, Pc, obs, sys_w, system_id, base,
-                                                                                 pb, out_amp, gpix, chi, c->n_ctile)));
+                                                                                 pb, out_amp, gpix, chi, c->n_ctile, amp_solve_tp(na))));
             ++t_launches;
         }
         int nl = 0;

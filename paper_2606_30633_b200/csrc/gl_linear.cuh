@@ -51,32 +51,53 @@ __global__ void gl_amp_sid_kernel(const int32_t* __restrict__ sid, int64_t Pc, i
 // comp: [n_amp][Pc][gpix_stride] = -A_k in the padded g_pix layout.  sys_w: 1/sigma^2.  out_amp may be NULL.
 // A particle whose normal matrix is not positive definite (a component that leaves no light on the cutout) is
 // marked invalid (PB_VALID = 0: logp = -INF, zero gradient).
-constexpr int AMP_TP = 64;           // pixels per tile
 constexpr int AMP_PPT = 10;          // pairs per thread: (AMP_MAX + 1)(AMP_MAX + 2) / 2 <= 256 * 11
+// Pixels per shared-memory tile.  Few pairs (the split mode below): as many as fit the largest problem's footprint
+// (multiple of 64, up to 1024), which amortises the two barriers per tile; many pairs: 64, where occupancy matters more
+// (config 3: 68 ms with 64-pixel tiles, 86 ms with 128).
+static inline int amp_solve_tp(int n) {
+    if ((n + 1) * (n + 2) / 2 > 128) return 64;
+    int tp = (4608 / (n + 1) - 1) / 64 * 64;
+    return tp < 64 ? 64 : (tp > 1024 ? 1024 : tp);
+}
+static inline size_t amp_solve_smem(int n) {
+    const int np = n + 1, tp = amp_solve_tp(n);
+    size_t ct = (size_t)np * (tp + 1);
+    if (ct < (size_t)n * n) ct = (size_t)n * n;
+    if (ct < 256) ct = 256;
+    const size_t npair = (size_t)np * (np + 1) / 2;
+    return sizeof(double) * (ct + (npair > 256 ? npair : 256) + n);
+}
+
 template <class T>
 __global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant__ Geom G, const __grid_constant__ AmpMap am,
                                                            const T* __restrict__ comp, int64_t Pc,
                                                            const float* __restrict__ obs, const T* __restrict__ sys_w,
                                                            const int32_t* __restrict__ system_id, int64_t p_base,
                                                            T* __restrict__ pb, float* __restrict__ out_amp,
-                                                           T* __restrict__ gpix, T* __restrict__ chi, int n_ctile) {
+                                                           T* __restrict__ gpix, T* __restrict__ chi, int n_ctile, int TP) {
     extern __shared__ double asm_[];
     const int n = am.n, np = n + 1, NN = G.N * G.N, tid = threadIdx.x;
     const int64_t p = blockIdx.x;
     const int sys = system_id ? system_id[p_base + p] : 0;
     const int npair = np * (np + 1) / 2;
-    double* ct = asm_;                                   // [np][AMP_TP + 1] tile of A_k / sigma (row n: obs / sigma); later M [n][n]
-    const int ct_sz = np * (AMP_TP + 1) > n * n ? np * (AMP_TP + 1) : n * n;
+    double* ct = asm_;                                   // [np][TP + 1] tile of A_k / sigma (row n: obs / sigma); later M [n][n]
+    int ct_sz = np * (TP + 1) > n * n ? np * (TP + 1) : n * n;
+    if (ct_sz < 256) ct_sz = 256;
     double* pr = asm_ + ct_sz;                           // [npair] sums, pair (k, l), l <= k, at k(k+1)/2 + l
     double* rhs = pr + (npair > 256 ? npair : 256);     // [n]  (pr doubles as the 256-entry reduction buffer at the end)
     __shared__ int s_fail;
     if (tid == 0) s_fail = 0;
+    // Few pairs (npair <= 128): S = 256 / npair threads share one pair, each taking every S-th pixel of a tile; their
+    // partial sums are added in a fixed order at the end.  Many pairs: one thread owns up to AMP_PPT + 1 pairs.
+    const int S = npair <= 128 ? 256 / npair : 1;
+    const int my = tid / S, g = tid - my * S;             // split mode: pair index, pixel lane
     double acc[AMP_PPT + 1]; int pk[AMP_PPT + 1], pl[AMP_PPT + 1];
 #pragma unroll
     for (int j = 0; j <= AMP_PPT; ++j) {
         acc[j] = 0; pk[j] = 0; pl[j] = 0;
-        const int i = tid + j * 256;
-        if (i < npair) {
+        const int i = S > 1 ? my : tid + j * 256;
+        if (i < npair && (S == 1 || j == 0)) {
             int k = (int)((sqrt(8.0 * i + 1.0) - 1.0) * 0.5);
             while (k * (k + 1) / 2 > i) --k;
             while ((k + 1) * (k + 2) / 2 <= i) ++k;
@@ -84,10 +105,10 @@ __global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant
         }
     }
     const size_t gs = gpix_stride(G);
-    for (int t0 = 0; t0 < NN; t0 += AMP_TP) {
+    for (int t0 = 0; t0 < NN; t0 += TP) {
         __syncthreads();
-        for (int idx = tid; idx < np * AMP_TP; idx += 256) {
-            const int k = idx / AMP_TP, x = idx - k * AMP_TP, pix = t0 + x;
+        for (int idx = tid; idx < np * TP; idx += 256) {
+            const int k = idx / TP, x = idx - k * TP, pix = t0 + x;
             double v = 0;
             if (pix < NN) {
                 const int r = pix / G.N, q = pix - r * G.N;
@@ -96,21 +117,40 @@ __global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant
                           : (double)obs[(size_t)sys * NN + pix];
                 v *= isg;
             }
-            ct[k * (AMP_TP + 1) + x] = v;
+            ct[k * (TP + 1) + x] = v;
         }
         __syncthreads();
+        if (S > 1) {
+            if (my < npair) {
+                const double* a = ct + pk[0] * (TP + 1); const double* b = ct + pl[0] * (TP + 1);
+                double s = acc[0];
+                for (int x = g; x < TP; x += S) s = fma(a[x], b[x], s);
+                acc[0] = s;
+            }
+        } else {
 #pragma unroll
-        for (int j = 0; j <= AMP_PPT; ++j) {
-            if (tid + j * 256 < npair) {
-                const double* a = ct + pk[j] * (AMP_TP + 1); const double* b = ct + pl[j] * (AMP_TP + 1);
-                double s = acc[j];
-                for (int x = 0; x < AMP_TP; ++x) s = fma(a[x], b[x], s);
-                acc[j] = s;
+            for (int j = 0; j <= AMP_PPT; ++j) {
+                if (tid + j * 256 < npair) {
+                    const double* a = ct + pk[j] * (TP + 1); const double* b = ct + pl[j] * (TP + 1);
+                    double s = acc[j];
+                    for (int x0 = 0; x0 < TP; x0 += 64) {        // TP is a multiple of 64: constant trip count inside
+#pragma unroll
+                        for (int x = 0; x < 64; ++x) s = fma(a[x0 + x], b[x0 + x], s);
+                    }
+                    acc[j] = s;
+                }
             }
         }
     }
+    __syncthreads();
+    if (S > 1) {
+        ct[tid] = acc[0];                                 // [pair][S] partials (npair * S <= 256 <= ct_sz)
+        __syncthreads();
+        if (tid < npair) { double s = 0; for (int x = 0; x < S; ++x) s += ct[tid * S + x]; pr[tid] = s; }
+    } else {
 #pragma unroll
-    for (int j = 0; j <= AMP_PPT; ++j) if (tid + j * 256 < npair) pr[tid + j * 256] = acc[j];
+        for (int j = 0; j <= AMP_PPT; ++j) if (tid + j * 256 < npair) pr[tid + j * 256] = acc[j];
+    }
     __syncthreads();
     // full symmetric M and rhs
     double* M = ct;
@@ -172,11 +212,5 @@ __global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant
     for (int k = tid; k < n_ctile; k += 256) chi[(size_t)p * n_ctile + k] = k == 0 && !fail ? (T)pr[0] : T(0);
 }
 
-static inline size_t amp_solve_smem(int n) {
-    const int np = n + 1;
-    const int ct_sz = np * (AMP_TP + 1) > n * n ? np * (AMP_TP + 1) : n * n;
-    const size_t npair = (size_t)np * (np + 1) / 2;
-    return sizeof(double) * ((size_t)ct_sz + (npair > 256 ? npair : 256) + n);
-}
 
 }  // namespace gl
