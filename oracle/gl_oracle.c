@@ -47,9 +47,9 @@ typedef struct {
     int32_t epl_terms;       /* <=0: sum the series to convergence (the model); >0: truncate (debug) */
     int32_t has_shear;
     int32_t multipole_mask;  /* bit0 m=3, bit1 m=4 */
-    int32_t n_source_sersic; /* 0 or 1 */
+    int32_t n_source_sersic; /* 0, 1 or 2 ("Sersic profiles and/or shapelets"; two lensed sources S1, S2) */
     int32_t shapelet_nmax;   /* -1 none */
-    int32_t n_lens_sersic;   /* 0, 1, 2 */
+    int32_t n_lens_sersic;   /* 0..3 ("one or more Sersic profiles"; env, L1, L2) */
     int32_t param_space;     /* 0: z (bijector + log-det); 1: physical theta */
     int32_t n_systems;
     int32_t n_params;
@@ -63,7 +63,7 @@ typedef struct {
 
 /* ---------------------------------------------------------------- parameter layout (S18) -------- */
 typedef struct {
-    int mass, gamma, shear, mp3, mp4, src, shp, ll[2], n;   /* offsets; -1 if absent */
+    int mass, gamma, shear, mp3, mp4, src, src2, shp, ll[3], n;   /* offsets; -1 if absent */
     int n_coef;
 } layout_t;
 
@@ -76,12 +76,13 @@ static void make_layout(const glo_config* c, layout_t* L) {
     if (c->multipole_mask & 1) { L->mp3 = k; k += 2; } else L->mp3 = -1;
     if (c->multipole_mask & 2) { L->mp4 = k; k += 2; } else L->mp4 = -1;
     if (c->n_source_sersic > 0) { L->src = k; k += 7; } else L->src = -1;
+    if (c->n_source_sersic > 1) { L->src2 = k; k += 7; } else L->src2 = -1;   /* second source, same source plane */
     L->n_coef = 0;
     if (c->shapelet_nmax >= 0) {
         L->n_coef = (c->shapelet_nmax + 1) * (c->shapelet_nmax + 2) / 2;
         L->shp = k; k += 1 + L->n_coef;
     } else L->shp = -1;
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < 3; ++i) {
         if (i < c->n_lens_sersic) { L->ll[i] = k; k += 7; } else L->ll[i] = -1;
     }
     L->n = k;
@@ -340,8 +341,9 @@ static double ray_intensity(const glo_config* c, const layout_t* L, const double
     double ax, ay; deflect(c, L, th, x, y, &ax, &ay);
     double bx = x - ax, by = y - ay, Iv = 0.0;
     if (L->src >= 0) Iv += sersic(th + L->src, bx, by, NULL, NULL);
+    if (L->src2 >= 0) Iv += sersic(th + L->src2, bx, by, NULL, NULL);
     if (L->shp >= 0) Iv += shapelets(c->shapelet_nmax, th + L->shp, th[L->src + 4], th[L->src + 5], bx, by, NULL, NULL);
-    for (int i = 0; i < 2; ++i) if (L->ll[i] >= 0) Iv += sersic(th + L->ll[i], x, y, NULL, NULL);
+    for (int i = 0; i < 3; ++i) if (L->ll[i] >= 0) Iv += sersic(th + L->ll[i], x, y, NULL, NULL);
     return Iv;
 }
 
@@ -370,6 +372,11 @@ static void ray_adjoint(const glo_config* c, const layout_t* L, const double* th
         for (int k = 0; k < 7; ++k) out[L->src + k] += gbar * dp[k];
         sx += gbar * dxy[0]; sy += gbar * dxy[1];
     }
+    if (L->src2 >= 0) {
+        double dp[7], dxy[2]; sersic(th + L->src2, bx, by, dp, dxy);
+        for (int k = 0; k < 7; ++k) out[L->src2 + k] += gbar * dp[k];
+        sx += gbar * dxy[0]; sy += gbar * dxy[1];
+    }
     if (L->shp >= 0) {
         double da[1 + 66 + 8], dxy[2];
         shapelets(c->shapelet_nmax, th + L->shp, th[L->src + 4], th[L->src + 5], bx, by, da, dxy);
@@ -377,7 +384,7 @@ static void ray_adjoint(const glo_config* c, const layout_t* L, const double* th
         out[L->src + 4] += -gbar * dxy[0]; out[L->src + 5] += -gbar * dxy[1];
         sx += gbar * dxy[0]; sy += gbar * dxy[1];
     }
-    for (int i = 0; i < 2; ++i) if (L->ll[i] >= 0) {
+    for (int i = 0; i < 3; ++i) if (L->ll[i] >= 0) {
         double dp[7], dxy[2]; sersic(th + L->ll[i], x, y, dp, dxy);
         for (int k = 0; k < 7; ++k) out[L->ll[i] + k] += gbar * dp[k];
     }
@@ -504,8 +511,8 @@ static int theta_valid(const glo_config* c, const layout_t* L, const double* th)
     if (!(th[m] > 0)) return 0;
     if (c->mass_model == 1) { double t = th[L->gamma] - 1.0; if (!(t > 0 && t < 2)) return 0; }
     if (!(th[o] * th[o] + th[o + 1] * th[o + 1] < 1.0)) return 0;
-    int blocks[3] = { L->src, L->ll[0], L->ll[1] };
-    for (int k = 0; k < 3; ++k) { int s = blocks[k]; if (s < 0) continue;
+    int blocks[5] = { L->src, L->src2, L->ll[0], L->ll[1], L->ll[2] };
+    for (int k = 0; k < 5; ++k) { int s = blocks[k]; if (s < 0) continue;
         if (!(th[s] > 0) || !(th[s + 1] > 0)) return 0;
         if (!(th[s + 2] * th[s + 2] + th[s + 3] * th[s + 3] < 1.0)) return 0; }
     if (L->shp >= 0 && !(th[L->shp] > 0)) return 0;

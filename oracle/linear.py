@@ -29,7 +29,7 @@ def amplitude_indices(spec):
     i = (6 if spec.mass_model == 1 else 5) + (2 if spec.has_shear else 0)
     i += 2 * bin(spec.multipole_mask & 3).count("1")
     idx = []
-    if spec.n_source_sersic:
+    for _ in range(spec.n_source_sersic):
         idx.append(i + 6); i += 7
     if spec.shapelet_nmax >= 0:
         nc = (spec.shapelet_nmax + 1) * (spec.shapelet_nmax + 2) // 2

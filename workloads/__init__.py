@@ -43,7 +43,7 @@ class LensSpec:
     epl_terms: int = 30
     has_shear: int = 1
     multipole_mask: int = 0      # bit0 m=3, bit1 m=4
-    n_source_sersic: int = 1
+    n_source_sersic: int = 1      # 0, 1 or 2 (same source plane)
     shapelet_nmax: int = -1
     n_lens_sersic: int = 1
     param_space: int = 0         # 0 unconstrained z, 1 physical theta
@@ -78,13 +78,14 @@ def param_names(mass_model, has_shear, multipole_mask, n_source_sersic, shapelet
     if multipole_mask & 2: n += ["mp.c4", "mp.s4"]
     ser = ["R", "n", "e1", "e2", "x", "y", "I"]
     if n_source_sersic: n += ["src." + s for s in ser]
+    if n_source_sersic > 1: n += ["src2." + s for s in ser]          # second source on the same plane (S1, S2)
     if shapelet_nmax >= 0: n += ["shp.beta"] + ["shp.a%d" % i for i in range(n_shapelet_coef(shapelet_nmax))]
     for k in range(n_lens_sersic): n += ["ll%d." % k + s for s in ser]
     return n
 
 
 # ------------------------------------------------------------------ priors of each config
-def _default_priors(mass_model, multipoles=False, shapelet_nmax=-1, n_lens=1):
+def _default_priors(mass_model, multipoles=False, shapelet_nmax=-1, n_lens=1, n_src=1):
     """SURVEY 8(d) fill-ins for configs 1, 2, 3, 5 (BJ configs[0..2], [4])."""
     p = [Uniform(0.8, 1.5)]
     if mass_model == 1: p += [Uniform(1.6, 2.4)]
@@ -93,6 +94,9 @@ def _default_priors(mass_model, multipoles=False, shapelet_nmax=-1, n_lens=1):
     if multipoles: p += [Normal(0, 0.01)] * 4
     p += [Uniform(0.1, 0.5), Uniform(1, 4), Normal(0, 0.15), Normal(0, 0.15), Normal(0, 0.2), Normal(0, 0.2),
           LogUniform(1, 100)]
+    if n_src > 1:
+        p += [Uniform(0.1, 0.5), Uniform(1, 4), Normal(0, 0.15), Normal(0, 0.15), Normal(0.3, 0.2), Normal(-0.2, 0.2),
+              LogUniform(1, 100)]
     if shapelet_nmax >= 0: p += [Uniform(0.05, 0.3)] + [Normal(0, 1)] * n_shapelet_coef(shapelet_nmax)
     for _ in range(n_lens):
         p += [Uniform(0.5, 1.5), Uniform(2, 6), TruncNormal(0, 0.1, -0.15, 0.15), TruncNormal(0, 0.1, -0.15, 0.15),
