@@ -73,7 +73,7 @@ typedef enum { GL_PRECISION_F64 = 0, GL_PRECISION_F32 = 1 } gl_precision;
  *   main mass [theta_E, (gamma if EPL), e1, e2, x, y] . shear [g1, g2] . multipoles [c3, s3][c4, s4] .
  *   source Sersic [R, n, e1, e2, x, y, I] . shapelets [beta_s, a_0 .. a_{Nc-1}] . lens Sersic 1 . lens Sersic 2
  * with Nc = (nmax+1)(nmax+2)/2 coefficients ordered by n1+n2 then n2 (O5, S9); the shapelet centre is the
- * source Sersic centre, so shapelets require n_source_sersic = 1. */
+ * source Sersic centre, so shapelets require n_source_sersic >= 1. */
 typedef struct {
     int32_t n_pix;            /* N: detector pixels per side, >= 1 */
     int32_t supersample;      /* s: rays per pixel per side, >= 1 */
@@ -85,9 +85,9 @@ typedef struct {
     int32_t epl_terms;        /* number of series terms kept for EPL, 2..30 (S5; BASELINE.json: 30) */
     int32_t has_shear;        /* 0/1 */
     int32_t multipole_mask;   /* bit0: m=3, bit1: m=4 (S7) */
-    int32_t n_source_sersic;  /* 0 or 1 */
+    int32_t n_source_sersic;  /* 0, 1 or 2 Sersic sources on the one source plane (S1, S2) */
     int32_t shapelet_nmax;    /* -1 none, else 0..10 */
-    int32_t n_lens_sersic;    /* 0, 1 or 2 */
+    int32_t n_lens_sersic;    /* 0..3 lens-plane Sersic blocks ("one or more"; env, L1, L2) */
     int32_t param_space;      /* 0: params are unconstrained z (bijector + log-det); 1: physical theta */
     int32_t n_systems;        /* number of (obs, noise_sigma, psf) triples, >= 1 (S19) */
     int32_t n_params;         /* must equal the count implied by the fields above (<= 128) */

@@ -27,7 +27,7 @@ struct gl_config {
     Layout L;
     Geom G;
     PriorTable pt;
-    int variant;        // 0: <.,0,1,-1,1>  1: <.,0,1,6,2>  2: <.,3,1,10,2>
+    int variant;        // 0: <.,0,1,-1,1>  1: <.,0,1,6,2>  2: <.,3,1,10,2>  3: <.,0,2,-1,3>  4: <.,3,2,10,3>
     int na;             // natural accumulators per chunk for the variant
     int nt_fwd, nt_adj, rpt_fwd, rpt_adj, n_chunk_fwd, n_chunk_adj;   // per phase plane
     int n_nap;          // adjoint partials per particle = s*s*n_chunk_adj
@@ -129,10 +129,12 @@ static int layout_from_desc(const gl_config_desc& d, Layout& L) {
     if (d.multipole_mask & 1) { L.mp3 = k; k += 2; } else L.mp3 = -1;
     if (d.multipole_mask & 2) { L.mp4 = k; k += 2; } else L.mp4 = -1;
     if (d.n_source_sersic > 0) { L.src = k; k += 7; } else L.src = -1;
+    if (d.n_source_sersic > 1) { L.src1 = k; k += 7; } else L.src1 = -1;
     L.nmax = d.shapelet_nmax; L.n_coef = 0;
     if (d.shapelet_nmax >= 0) { L.n_coef = (d.shapelet_nmax + 1) * (d.shapelet_nmax + 2) / 2; L.shp = k; k += 1 + L.n_coef; } else L.shp = -1;
     if (d.n_lens_sersic >= 1) { L.ll0 = k; k += 7; } else L.ll0 = -1;
     if (d.n_lens_sersic >= 2) { L.ll1 = k; k += 7; } else L.ll1 = -1;
+    if (d.n_lens_sersic >= 3) { L.ll2 = k; k += 7; } else L.ll2 = -1;
     L.n_params = k; L.param_space = d.param_space; L.mass_model = d.mass_model;
     return k;
 }
@@ -146,9 +148,9 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     if (d->mass_model != 0 && d->mass_model != 1) return GL_ERR_BAD_CONFIG;
     if (d->mass_model == 1 && (d->epl_terms < 2 || d->epl_terms > 30)) return GL_ERR_BAD_CONFIG;
     if ((d->has_shear & ~1) || (d->multipole_mask & ~3) || (d->param_space & ~1)) return GL_ERR_BAD_CONFIG;
-    if (d->n_source_sersic < 0 || d->n_source_sersic > 1 || d->n_lens_sersic < 0 || d->n_lens_sersic > 2) return GL_ERR_BAD_CONFIG;
+    if (d->n_source_sersic < 0 || d->n_source_sersic > 2 || d->n_lens_sersic < 0 || d->n_lens_sersic > 3) return GL_ERR_BAD_CONFIG;
     if (d->shapelet_nmax < -1 || d->shapelet_nmax > 10) return GL_ERR_BAD_CONFIG;
-    if (d->shapelet_nmax >= 0 && d->n_source_sersic != 1) return GL_ERR_BAD_CONFIG;
+    if (d->shapelet_nmax >= 0 && d->n_source_sersic < 1) return GL_ERR_BAD_CONFIG;      // shapelets share the first source's centre
     if (d->n_systems < 1) return GL_ERR_BAD_CONFIG;
     if (d->precision != GL_PRECISION_F64 && d->precision != GL_PRECISION_F32) return GL_ERR_BAD_CONFIG;
     if (d->psf_grid != 0 && d->psf_grid != 1) return GL_ERR_UNSUPPORTED;
@@ -182,12 +184,14 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     {   // light amplitudes in the flat order S18 and their PB slots
         AmpMap& A = c->amp; A.n = 0;
         auto add = [&](int pb_off, int shp) { A.off[A.n] = (short)pb_off; A.shp[A.n] = (unsigned char)shp; ++A.n; };
-        CompIdx& ci = c->cidx; ci.src = ci.shp0 = ci.ll0 = ci.ll1 = -1; ci.n_coef = L.n_coef;
+        CompIdx& ci = c->cidx; ci.src = ci.src1 = ci.shp0 = ci.ll0 = ci.ll1 = ci.ll2 = -1; ci.n_coef = L.n_coef;
         if (L.src >= 0) { ci.src = A.n; add(PB_SRC + SB_IE, 0); }
+        if (L.src1 >= 0) { ci.src1 = A.n; add(PB_SRC1 + SB_IE, 0); }
         if (L.n_coef > 0) ci.shp0 = A.n;
         for (int k = 0; k < L.n_coef; ++k) add(PB_SHP_A + k, 1);
         if (L.ll0 >= 0) { ci.ll0 = A.n; add(PB_LL0 + SB_IE, 0); }
         if (L.ll1 >= 0) { ci.ll1 = A.n; add(PB_LL1 + SB_IE, 0); }
+        if (L.ll2 >= 0) { ci.ll2 = A.n; add(PB_LL2 + SB_IE, 0); }
         c->n_amp = A.n;
         L.amp_mode = d->amplitude_mode;
         if (d->amplitude_mode == 1) {
@@ -197,9 +201,12 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     }
     for (int i = np; i < 128; ++i) { c->pt.kind[i] = 0; c->pt.a[i] = 0; c->pt.b[i] = 1; c->pt.lo[i] = 0; c->pt.hi[i] = 1; }
     // kernel variant: the smallest compiled superset of the requested components
-    if (d->multipole_mask == 0 && d->shapelet_nmax < 0 && d->n_lens_sersic <= 1) { c->variant = 0; L.ker_nmax = -1; c->na = NA_SHA; }
-    else if (d->multipole_mask == 0 && d->shapelet_nmax <= 6) { c->variant = 1; L.ker_nmax = 6; c->na = NA_SHA + 28; }
-    else { c->variant = 2; L.ker_nmax = 10; c->na = NA_SHA + 66; }
+    const bool extra = d->n_source_sersic > 1 || d->n_lens_sersic > 2;       // second source / third lens-light block
+    if (!extra && d->multipole_mask == 0 && d->shapelet_nmax < 0 && d->n_lens_sersic <= 1) { c->variant = 0; L.ker_nmax = -1; c->na = NA_SHA; }
+    else if (!extra && d->multipole_mask == 0 && d->shapelet_nmax <= 6) { c->variant = 1; L.ker_nmax = 6; c->na = NA_SHA + 28; }
+    else if (!extra) { c->variant = 2; L.ker_nmax = 10; c->na = NA_SHA + 66; }
+    else if (d->multipole_mask == 0 && d->shapelet_nmax < 0) { c->variant = 3; L.ker_nmax = -1; c->na = NA_SHA; }
+    else { c->variant = 4; L.ker_nmax = 10; c->na = NA_SHA + 66; }
     c->L = L;
     Geom& G = c->G;
     G.N = d->n_pix; G.s = d->supersample; G.M = (int)M64; G.K = d->psf_size; G.pgrid = d->psf_grid;
@@ -302,6 +309,8 @@ static void launch_ray_adj(const gl_config* c, const T* pb, const double* tab, c
 using V_S0 = Variant<0, 0, 1, -1, 1>; using V_E0 = Variant<1, 0, 1, -1, 1>;
 using V_S1 = Variant<0, 0, 1, 6, 2>;  using V_E1 = Variant<1, 0, 1, 6, 2>;
 using V_S2 = Variant<0, 3, 1, 10, 2>; using V_E2 = Variant<1, 3, 1, 10, 2>;
+using V_S3 = Variant<0, 0, 2, -1, 3>; using V_E3 = Variant<1, 0, 2, -1, 3>;   // the real-system component list
+using V_S4 = Variant<0, 3, 2, 10, 3>; using V_E4 = Variant<1, 3, 2, 10, 3>;   // everything
 
 template <class T>
 static void ray_fwd(const gl_config* c, const T* pb, const double* tab, T* ray, int64_t Pc, cudaStream_t st) {
@@ -312,7 +321,11 @@ static void ray_fwd(const gl_config* c, const T* pb, const double* tab, T* ray, 
         case 2: launch_ray_fwd<T, V_S1>(c, pb, tab, ray, Pc, st); break;
         case 3: launch_ray_fwd<T, V_E1>(c, pb, tab, ray, Pc, st); break;
         case 4: launch_ray_fwd<T, V_S2>(c, pb, tab, ray, Pc, st); break;
-        default: launch_ray_fwd<T, V_E2>(c, pb, tab, ray, Pc, st); break;
+        case 5: launch_ray_fwd<T, V_E2>(c, pb, tab, ray, Pc, st); break;
+        case 6: launch_ray_fwd<T, V_S3>(c, pb, tab, ray, Pc, st); break;
+        case 7: launch_ray_fwd<T, V_E3>(c, pb, tab, ray, Pc, st); break;
+        case 8: launch_ray_fwd<T, V_S4>(c, pb, tab, ray, Pc, st); break;
+        default: launch_ray_fwd<T, V_E4>(c, pb, tab, ray, Pc, st); break;
     }
 }
 template <class T, class V>
@@ -330,7 +343,11 @@ static void ray_comp(const gl_config* c, const T* pb, const double* tab, T* cray
         case 2: launch_ray_comp<T, V_S1>(c, pb, tab, cray, Pc, st); break;
         case 3: launch_ray_comp<T, V_E1>(c, pb, tab, cray, Pc, st); break;
         case 4: launch_ray_comp<T, V_S2>(c, pb, tab, cray, Pc, st); break;
-        default: launch_ray_comp<T, V_E2>(c, pb, tab, cray, Pc, st); break;
+        case 5: launch_ray_comp<T, V_E2>(c, pb, tab, cray, Pc, st); break;
+        case 6: launch_ray_comp<T, V_S3>(c, pb, tab, cray, Pc, st); break;
+        case 7: launch_ray_comp<T, V_E3>(c, pb, tab, cray, Pc, st); break;
+        case 8: launch_ray_comp<T, V_S4>(c, pb, tab, cray, Pc, st); break;
+        default: launch_ray_comp<T, V_E4>(c, pb, tab, cray, Pc, st); break;
     }
 }
 template <class T>
@@ -342,7 +359,11 @@ static void ray_adj(const gl_config* c, const T* pb, const double* tab, const T*
         case 2: launch_ray_adj<T, V_S1>(c, pb, tab, gbar, nap, Pc, st); break;
         case 3: launch_ray_adj<T, V_E1>(c, pb, tab, gbar, nap, Pc, st); break;
         case 4: launch_ray_adj<T, V_S2>(c, pb, tab, gbar, nap, Pc, st); break;
-        default: launch_ray_adj<T, V_E2>(c, pb, tab, gbar, nap, Pc, st); break;
+        case 5: launch_ray_adj<T, V_E2>(c, pb, tab, gbar, nap, Pc, st); break;
+        case 6: launch_ray_adj<T, V_S3>(c, pb, tab, gbar, nap, Pc, st); break;
+        case 7: launch_ray_adj<T, V_E3>(c, pb, tab, gbar, nap, Pc, st); break;
+        case 8: launch_ray_adj<T, V_S4>(c, pb, tab, gbar, nap, Pc, st); break;
+        default: launch_ray_adj<T, V_E4>(c, pb, tab, gbar, nap, Pc, st); break;
     }
 }
 

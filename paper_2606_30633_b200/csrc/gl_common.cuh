@@ -37,7 +37,9 @@ enum : int {
     PB_SER_E = 208,                     // e_m = L_{m+1} a_{m+1}
     PB_SER_M1 = 240, PB_SER_M2 = 241,   // series bands: 4*M1 steps in T, 4*M2 steps in fp32 above them, the rest skipped
     PB_M_H1 = 242, PB_M_H0 = 243,       // amplitude A (b/R)^(t-1) = 2^(H1 log2 R^2 + H0): H1 = -(t-1)/2, H0 = (t-1) log2 b + log2 A
-    PB_STRIDE = 244
+    PB_SRC1 = 244,                      // second source Sersic block (same source plane), 16 floats
+    PB_LL2 = 260,                       // third lens-light Sersic block, 16 floats
+    PB_STRIDE = 276
 };
 // Sersic block offsets
 // The component frame is stored PRE-SCALED: x' = sqrt(q) x_r = A11 px + A12 py, y' = y_r / sqrt(q) = A21 px + A22 py, so that
@@ -57,8 +59,9 @@ enum : int {
     NA_SRC = 18,                         // 8: T0 T1 T2 AX AY BXX BYY BXY
     NA_SHB = 26, NA_SHX = 27, NA_SHY = 28,
     NA_LL0 = 29, NA_LL1 = 37,
-    NA_SHA = 45,                         // Nc coefficient sums
-    NA_MAX = 45 + 66
+    NA_SRC1 = 45, NA_LL2 = 53,           // second source / third lens-light block (8 each, like NA_SRC)
+    NA_SHA = 61,                         // Nc coefficient sums
+    NA_MAX = 61 + 66
 };
 enum : int { SA_T0 = 0, SA_T1 = 1, SA_T2 = 2, SA_AX = 3, SA_AY = 4, SA_BXX = 5, SA_BYY = 6, SA_BXY = 7 };
 
@@ -72,7 +75,7 @@ struct Variant {
     static constexpr int NLL = NLL_;
     static constexpr int NCOEF = NMAX_ >= 0 ? (NMAX_ + 1) * (NMAX_ + 2) / 2 : 0;
     static constexpr int NA = NMAX_ >= 0 ? NA_SHA + NCOEF : NA_SHA;            // accumulators written per chunk
-    static constexpr int PB_NEED = MASS_ == 1 ? PB_STRIDE : PB_SER_A;          // floats of PB a CTA stages
+    static constexpr int PB_NEED = (MASS_ == 1 || NSRC_ > 1 || NLL_ > 2) ? PB_STRIDE : PB_SER_A;   // floats of PB a CTA stages
 };
 
 struct Geom {            // launch-invariant geometry, passed by value

@@ -16,7 +16,7 @@
 
 namespace gl {
 
-constexpr int AMP_MAX = 72;          // 1 + 66 + 2 amplitudes at most (n_max = 10, two lens Sersic blocks)
+constexpr int AMP_MAX = 72;          // 2 + 66 + 3 = 71 amplitudes at most (two sources, n_max = 10, three lens Sersic blocks)
 
 struct AmpMap {                      // component k -> its slot in PB
     int n;

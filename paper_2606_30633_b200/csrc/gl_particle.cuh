@@ -11,14 +11,15 @@ struct PriorTable {                 // passed by value as a kernel parameter (<=
 };
 
 struct Layout {                     // offsets into the flat parameter vector (reading S18); -1 = absent
-    int mass, gamma, ell, shear, mp3, mp4, src, shp, ll0, ll1;
+    int mass, gamma, ell, shear, mp3, mp4, src, src1, shp, ll0, ll1, ll2;
     int n_params, n_coef, nmax, param_space, mass_model;
     int ker_nmax;                   // shapelet order the selected kernel variant is compiled for (>= nmax)
     int amp_mode;                   // 1: light amplitudes solved by linear inversion (gl_linear.cuh); their z entries are ignored
 };
 // Amplitude parameters in the flat order S18: I of each Sersic block, the shapelet coefficients.
 __host__ __device__ inline bool is_amp(const Layout& L, int i) {
-    return (L.src >= 0 && i == L.src + 6) || (L.ll0 >= 0 && i == L.ll0 + 6) || (L.ll1 >= 0 && i == L.ll1 + 6) ||
+    return (L.src >= 0 && i == L.src + 6) || (L.src1 >= 0 && i == L.src1 + 6) || (L.ll0 >= 0 && i == L.ll0 + 6) ||
+           (L.ll1 >= 0 && i == L.ll1 + 6) || (L.ll2 >= 0 && i == L.ll2 + 6) ||
            (L.shp >= 0 && i > L.shp && i <= L.shp + L.n_coef);
 }
 // z of parameter i as the kernels see it: a solved amplitude (amp_mode 1) reads as 1 whatever the caller stored
@@ -171,6 +172,8 @@ __global__ void __launch_bounds__(UNPACK_WPB * 32) gl_unpack_kernel(const __grid
     write_sersic<T>(th, L.src, o + PB_SRC, x_first, ok);
     write_sersic<T>(th, L.ll0, o + PB_LL0, x_first, ok);
     write_sersic<T>(th, L.ll1, o + PB_LL1, x_first, ok);
+    write_sersic<T>(th, L.src1, o + PB_SRC1, x_first, ok);
+    write_sersic<T>(th, L.ll2, o + PB_LL2, x_first, ok);
     // shapelets (coefficients pre-divided by beta_s; orders above the configured nmax are zero)
     if (L.ker_nmax >= 0) {
         double bs = 1.0;
@@ -294,6 +297,8 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
             if (L.src >= 0) sersic_chain(th, L.src, nat + NA_SRC, gth);
             if (L.ll0 >= 0) sersic_chain(th, L.ll0, nat + NA_LL0, gth);
             if (L.ll1 >= 0) sersic_chain(th, L.ll1, nat + NA_LL1, gth);
+            if (L.src1 >= 0) sersic_chain(th, L.src1, nat + NA_SRC1, gth);
+            if (L.ll2 >= 0) sersic_chain(th, L.ll2, nat + NA_LL2, gth);
             if (L.shp >= 0) {
                 double bs = theta_at(th, L.shp);
                 gth[L.shp] = -nat[NA_SHB] / bs;

@@ -221,7 +221,7 @@ __device__ __forceinline__ void sersic_accum(const SersicOut<T>& o, T g, T* __re
 template <class T, class V> __host__ __device__ constexpr bool coef_in_smem() { return sizeof(T) == 8 && V::NMAX > 6; }
 
 // Component slots of backward modelling (gl_linear.cuh): index of each light component among the amplitudes, -1 = absent.
-struct CompIdx { int src, shp0, n_coef, ll0, ll1; };
+struct CompIdx { int src, src1, shp0, n_coef, ll0, ll1, ll2; };
 
 // Everything one ray needs.  ADJ = false: returns the surface brightness; ADJ = true: accumulates gbar * dI/d(natural).
 // COMP (with ADJ = false; PB amplitudes all set to unity): also stores the surface brightness of every light component
@@ -321,6 +321,18 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
             const T Ixr = -sb[SB_KQ] * o.Iu_r2 * o.xr, Iyr = -sb[SB_KQI] * o.Iu_r2 * o.yr;
             gbx = R::fma(sb[SB_C], Ixr, -sb[SB_S] * Iyr); gby = R::fma(sb[SB_S], Ixr, sb[SB_C] * Iyr);
         }
+        if constexpr (V::NSRC >= 2) {                // second source on the same source plane (S1, S2)
+            const T* s1 = pb + PB_SRC1;
+            const T qx1 = R::fma(fj, step, s1[SB_XOFF]) - ax, qy1 = R::fma(fi, step, s1[SB_YOFF]) - ay;
+            SersicOut<T> o1 = sersic_eval<T, ADJ>(tb, s1, qx1, qy1);
+            Iray += o1.I;
+            if constexpr (COMP) { if (ci->src1 >= 0) acc[(size_t)ci->src1 * cstride] = o1.I; }
+            if constexpr (ADJ) {
+                sersic_accum(o1, gbar, acc + NA_SRC1);
+                const T Ixr = -s1[SB_KQ] * o1.Iu_r2 * o1.xr, Iyr = -s1[SB_KQI] * o1.Iu_r2 * o1.yr;
+                gbx += R::fma(s1[SB_C], Ixr, -s1[SB_S] * Iyr); gby += R::fma(s1[SB_S], Ixr, s1[SB_C] * Iyr);
+            }
+        }
         if constexpr (V::NMAX >= 0) {
             constexpr int NM = V::NMAX >= 0 ? V::NMAX : 0;
             const T ibs = pb[PB_SHP];
@@ -389,6 +401,12 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
         SersicOut<T> o = sersic_eval<T, ADJ>(tb, sb, R::fma(fj, step, sb[SB_XOFF]), R::fma(fi, step, sb[SB_YOFF]));
         Iray += o.I; if constexpr (ADJ) sersic_accum(o, gbar, acc + NA_LL1);
         if constexpr (COMP) { if (ci->ll1 >= 0) acc[(size_t)ci->ll1 * cstride] = o.I; }
+    }
+    if constexpr (V::NLL >= 3) {
+        const T* sb = pb + PB_LL2;
+        SersicOut<T> o = sersic_eval<T, ADJ>(tb, sb, R::fma(fj, step, sb[SB_XOFF]), R::fma(fi, step, sb[SB_YOFF]));
+        Iray += o.I; if constexpr (ADJ) sersic_accum(o, gbar, acc + NA_LL2);
+        if constexpr (COMP) { if (ci->ll2 >= 0) acc[(size_t)ci->ll2 * cstride] = o.I; }
     }
     if constexpr (ADJ) {
         // mass parameters enter through beta only: d/dtheta_mass = -(gbar grad_beta I_src) . dalpha/dtheta_mass
@@ -560,7 +578,7 @@ __global__ void __launch_bounds__(NT) gl_ray_comp_kernel(const __grid_constant__
 #define GL_ADJ_MINB 4
 #endif
 template <class T, class V, int NT>
-__global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 ? GL_ADJ_MINB : 1)) gl_ray_adj_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
+__global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC < 2 && V::NLL < 3 ? GL_ADJ_MINB : 1)) gl_ray_adj_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
                                                         const double* __restrict__ tabg, const T* __restrict__ gbar,
                                                         T* __restrict__ nap, int RPT, int n_chunk) {
     __shared__ __align__(16) T pb[PB_STRIDE];

@@ -185,3 +185,83 @@ def test_backward_mode_full_config2_batch_chunks_and_oracle_samples():
     assert np.all(np.abs(lp[idx] - ref["logp"]) <= RTOL_LOGP * np.abs(ref["logp"]))
     assert _grad_ok(g[idx].astype(np.float64), ref["grad"]).all()
     assert np.all(np.abs(amp[idx] - ref["amp"]) <= 1e-4 * np.abs(ref["amp"]).max(axis=1, keepdims=True) + 1e-6)
+
+
+def _multi_case(n_pix, s, K, seed, n_particles, nmax=-1, multipoles=False, mass_model=1, amplitude_mode=0):
+    """Two sources on the source plane and three lens-plane Sersic blocks: the component list of the paper's
+    real-system model (env, L1, L2, S1, S2)."""
+    import oracle
+    pri = W._default_priors(mass_model, multipoles=multipoles, shapelet_nmax=nmax, n_lens=3, n_src=2)
+    sp = W.LensSpec(n_pix, s, K, W._r32(0.11 * 40 / n_pix * 2.4), mass_model=mass_model, epl_terms=30,
+                    multipole_mask=3 if multipoles else 0, n_source_sersic=2, shapelet_nmax=nmax, n_lens_sersic=3,
+                    priors=pri, amplitude_mode=amplitude_mode)
+    assert sp.n_params == len(W.param_names(mass_model, 1, sp.multipole_mask, 2, nmax, 3))
+    rng = np.random.default_rng(seed)
+    step = sp.pix_scale / s
+    psf = W.gaussian_psf(K, 2.5 * step, step)[None].astype(np.float32)
+    truth = oracle.model_image(sp, psf.astype(np.float64), W.draw(rng, pri, 1))
+    sigma = np.full((1, n_pix, n_pix), 0.05, np.float32)
+    obs = (truth + 0.05 * rng.standard_normal(truth.shape)).astype(np.float32)
+    z = W.z_of(pri, W.draw(rng, pri, n_particles)).astype(np.float32)
+    return sp, obs, sigma, psf, z
+
+
+@pytest.mark.parametrize("case", [(40, 2, 11, -1, False, 1), (20, 2, 5, -1, False, 0), (18, 3, 5, 3, True, 1), (16, 2, 5, 8, False, 0)])
+def test_two_sources_three_lens_blocks_sampled_amplitudes(case):
+    """Sampled ("forward") amplitudes, strict north_star bar in fp64 mode; fp32 mode norm-wise.  Kernel variants
+    <.,0,2,-1,3> (the 43-parameter real-system list) and the superset <.,3,2,10,3>."""
+    import copy as _copy
+    import oracle
+    import torch
+    gl = _gl()
+    n_pix, s, K, nmax, mp, mass = case
+    sp, obs, sigma, psf, z = _multi_case(n_pix, s, K, seed=50 + n_pix, n_particles=6, nmax=nmax, multipoles=mp, mass_model=mass)
+    ref = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), epl_terms=30 if mass == 1 else None)
+    fin = np.isfinite(ref["logp"])
+    assert fin.sum() >= 4
+    for prec in (0, 1):
+        spp = _copy.copy(sp); spp.precision = prec
+        m = gl.LensModel(spp, obs, sigma, psf)
+        lp, g = m.logpost_grad(torch.from_numpy(z).cuda())
+        lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+        assert np.array_equal(np.isfinite(lp), fin)
+        if prec == 0:
+            assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+            ok = _grad_ok(g[fin], ref["grad"][fin])
+            assert ok.all(), (np.argwhere(~ok)[:5], g[fin][~ok][:5], ref["grad"][fin][~ok][:5])
+        else:
+            num = np.linalg.norm(g[fin] - ref["grad"][fin], axis=1); den = np.linalg.norm(ref["grad"][fin], axis=1)
+            assert np.all(num <= 2e-2 * den), num / den
+        img = m.model_image(torch.from_numpy(z[fin][:2]).cuda()).cpu().numpy()
+        ref_img = oracle.model_image(sp, psf.astype(np.float64), W.theta_of(sp.priors, z[fin][:2].astype(np.float64)),
+                                     epl_terms=30 if mass == 1 else None)
+        assert np.allclose(img, ref_img, rtol=1e-3, atol=1e-4 * np.abs(ref_img).max())
+
+
+@pytest.mark.parametrize("case", [(40, 2, 11, -1, False), (18, 2, 5, 2, True)])
+def test_real_system_component_list_in_backward_mode(case):
+    """The paper's real-system configuration: backward modelling of mass + shear, three lens-plane
+    Sersic blocks and two sources -- 38 sampled parameters + 5 solved amplitudes -- against oracle/linear.py."""
+    import oracle.linear as OL
+    import torch
+    gl = _gl()
+    n_pix, s, K, nmax, mp = case
+    sp, obs, sigma, psf, z = _multi_case(n_pix, s, K, seed=77, n_particles=6, nmax=nmax, multipoles=mp, amplitude_mode=1)
+    idx = OL.amplitude_indices(sp)
+    if nmax < 0:
+        assert sp.n_params - len(idx) == 38 and len(idx) == 5
+    z[:, idx] = np.float32(np.nan)
+    ref = OL.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), epl_terms=30)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    assert gl.gl_config_n_amplitudes(m.h) == len(idx)
+    lp, g = m.logpost_grad(torch.from_numpy(z).cuda())
+    amp, _ = m.linear_amplitudes(torch.from_numpy(z).cuda())
+    lp, g, amp = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64), amp.cpu().numpy().astype(np.float64)
+    fin = np.isfinite(ref["logp"])
+    assert fin.sum() >= 4 and np.array_equal(np.isfinite(lp), fin)
+    assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+    assert np.all(g[:, idx] == 0)
+    ok = _grad_ok(g[fin], ref["grad"][fin])
+    assert ok.all(), (np.argwhere(~ok)[:5], g[fin][~ok][:5], ref["grad"][fin][~ok][:5])
+    scale = np.abs(ref["amp"][fin]).max(axis=1, keepdims=True)
+    assert np.all(np.abs(amp[fin] - ref["amp"][fin]) <= 1e-4 * scale + 1e-6)
