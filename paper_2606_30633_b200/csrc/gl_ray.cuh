@@ -577,8 +577,11 @@ __global__ void __launch_bounds__(NT) gl_ray_comp_kernel(const __grid_constant__
 #ifndef GL_ADJ_MINB
 #define GL_ADJ_MINB 4
 #endif
+#ifndef GL_ADJ_MINB_X
+#define GL_ADJ_MINB_X 3     // two sources / three lens blocks, no shapelets (61 fp64 sums): 168 registers
+#endif
 template <class T, class V, int NT>
-__global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC < 2 && V::NLL < 3 ? GL_ADJ_MINB : 1)) gl_ray_adj_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
+__global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC < 2 && V::NLL < 3 ? GL_ADJ_MINB : (sizeof(T) == 8 && V::NMAX < 0 ? GL_ADJ_MINB_X : 1))) gl_ray_adj_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
                                                         const double* __restrict__ tabg, const T* __restrict__ gbar,
                                                         T* __restrict__ nap, int RPT, int n_chunk) {
     __shared__ __align__(16) T pb[PB_STRIDE];
