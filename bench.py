@@ -29,7 +29,8 @@ METRIC = "log-posterior+grad particle-evals/sec"
 UNIT = "particle-evals/s"
 WORKLOAD_NAMES = {1: "cfg1 tiny SIE 40x40 s2 K11 P64", 2: "cfg2 DESI-Legacy-like EPL+shear 60x60 s4 K21 Moffat P4096",
                   3: "cfg3 HST-like EPL+shear+shapelets(6) 100x100 s2 K31 P8192",
-                  4: "cfg4 100-system ensemble 60x60 s4 K21 P102400", 5: "cfg5 EPL+multipoles+shapelets(10) 200x200 s4 K41 P2048"}
+                  4: "cfg4 100-system ensemble 60x60 s4 K21 P102400", 5: "cfg5 EPL+multipoles+shapelets(10) 200x200 s4 K41 P2048",
+                  6: "cfg6 (not in BASELINE.json) real-system component list: EPL+shear, 3 lens Sersic, 2 source Sersic, 60x60 s4 K21 P4096"}
 
 # ALU peaks of one B200 from unit counts and clocks: 148 SMs x 128 FP32 lanes (64 FP64 lanes)
 # x sm_max_mhz; an FMA counts as ONE lane-operation.

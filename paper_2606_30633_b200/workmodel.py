@@ -93,7 +93,7 @@ def per_ray(spec, precision="f32"):
     nser = spec.n_source_sersic + spec.n_lens_sersic
     add(FWD, "sersic", nser); add(ADJ, "sersic", nser)
     if spec.n_source_sersic:
-        add(ADJ, "sersic_src_grad")
+        add(ADJ, "sersic_src_grad", spec.n_source_sersic)
     if spec.shapelet_nmax >= 0:
         add(FWD, "shapelet_fixed"); add(ADJ, "shapelet_fixed")
         f += shapelet_fwd(spec.shapelet_nmax); a += shapelet_adj(spec.shapelet_nmax)

@@ -41,7 +41,7 @@ def _dump(name, rep):
         pass
 
 
-@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5, 6])
 def test_parity_subset(k):
     """All parity-subset particles of config k: logp and every gradient component against the oracle."""
     gl, torch, wl, m = _model(k)
@@ -102,7 +102,7 @@ def test_model_image_matches_oracle(k):
     assert np.max(np.abs(img - ref) / scale) < 2e-5
 
 
-@pytest.mark.parametrize("k", [2, 3, 5])
+@pytest.mark.parametrize("k", [2, 3, 5, 6])
 def test_full_batch_rows_are_bit_identical_to_subset_rows(k):
     """BASELINE-size launches (config 2 = 4096 particles, the configuration bench.py times; config 3 = 8192; config 5 =
     2048): rows of the full batch equal the same particles evaluated alone (PAPER.md L83 fn 2: no cross-particle

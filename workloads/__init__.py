@@ -122,7 +122,9 @@ def _eq4(which):
 
 
 def make_spec(k, **over):
-    """LensSpec of BASELINE.json configs[k-1], k = 1..5."""
+    """LensSpec of BASELINE.json configs[k-1], k = 1..5; k = 6 (not a BASELINE.json config): the component list of the
+    paper's real-system model (mass + shear, env / L1 / L2 lens light, S1 / S2 sources; 43 parameters,
+    38 when the amplitudes are solved) on the geometry, PSF and noise recipe of config 2."""
     if k == 1:
         s = LensSpec(40, 2, 11, _r32(0.262), mass_model=0, priors=_default_priors(0))
     elif k == 2:
@@ -135,6 +137,9 @@ def make_spec(k, **over):
     elif k == 5:
         s = LensSpec(200, 4, 41, _r32(0.04), multipole_mask=3, shapelet_nmax=10, n_lens_sersic=2,
                      priors=_default_priors(1, multipoles=True, shapelet_nmax=10, n_lens=2))
+    elif k == 6:
+        s = LensSpec(60, 4, 21, _r32(0.262), n_source_sersic=2, n_lens_sersic=3,
+                     priors=_default_priors(1, n_lens=3, n_src=2))
     else:
         raise ValueError(k)
     for a, v in over.items():
@@ -145,8 +150,8 @@ def make_spec(k, **over):
     return s
 
 
-FULL_PARTICLES = {1: 64, 2: 4096, 3: 8192, 4: 102400, 5: 2048}
-PARITY_PARTICLES = {1: 64, 2: 256, 3: 128, 4: 400, 5: 16}     # SURVEY 8(d) parity subsets
+FULL_PARTICLES = {1: 64, 2: 4096, 3: 8192, 4: 102400, 5: 2048, 6: 4096}
+PARITY_PARTICLES = {1: 64, 2: 256, 3: 128, 4: 400, 5: 16, 6: 64}     # SURVEY 8(d) parity subsets
 
 
 # ------------------------------------------------------------------ sampling and the inverse bijector
@@ -259,7 +264,7 @@ def make_workload(k, n_particles=None, per_system=None):
     noise_unit = s_noise.standard_normal((nsys, N, N))
     # psf
     if k == 1:   psf = gaussian_psf(K, 1.1, step)[None]
-    elif k == 2: psf = moffat_psf(K, 1.2, 3.0, step)[None]
+    elif k in (2, 6): psf = moffat_psf(K, 1.2, 3.0, step)[None]
     elif k == 3: psf = gaussian_psf(K, 0.1, step)[None]
     elif k == 4:
         fw = s_psf.uniform(1.0, 1.5, nsys); bm = s_psf.uniform(2.5, 4.0, nsys)
@@ -269,7 +274,7 @@ def make_workload(k, n_particles=None, per_system=None):
     psf = psf.astype(np.float32)
     # particles
     system_id = None
-    if k in (1, 2, 5):
+    if k in (1, 2, 5, 6):
         P = FULL_PARTICLES[k] if n_particles is None else n_particles
         z = z_of(spec.priors, draw(s_part, spec.priors, FULL_PARTICLES[k]))[:P]
     elif k == 3:
@@ -280,8 +285,8 @@ def make_workload(k, n_particles=None, per_system=None):
         full = truth_z.astype(np.float64)[:, None, :] + 0.02 * s_part.standard_normal((nsys, 1024, spec.n_params))
         z = full[:, :per, :].reshape(nsys * per, spec.n_params)
         system_id = np.repeat(np.arange(nsys, dtype=np.int32), per)
-    sigma_bkg = {1: 0.05, 2: 0.02, 3: 0.01, 4: 0.05, 5: 0.005}[k]
-    t_exp = {1: 0.0, 2: 1000.0, 3: 0.0, 4: 1000.0, 5: 0.0}[k]
+    sigma_bkg = {1: 0.05, 2: 0.02, 3: 0.01, 4: 0.05, 5: 0.005, 6: 0.02}[k]
+    t_exp = {1: 0.0, 2: 1000.0, 3: 0.0, 4: 1000.0, 5: 0.0, 6: 1000.0}[k]
     return Workload(k, spec, psf, truth_z, truth_theta, np.ascontiguousarray(z.astype(np.float32)), system_id,
                     noise_unit, sigma_bkg, t_exp)
 
