@@ -265,3 +265,57 @@ def test_real_system_component_list_in_backward_mode(case):
     assert ok.all(), (np.argwhere(~ok)[:5], g[fin][~ok][:5], ref["grad"][fin][~ok][:5])
     scale = np.abs(ref["amp"][fin]).max(axis=1, keepdims=True)
     assert np.all(np.abs(amp[fin] - ref["amp"][fin]) <= 1e-4 * scale + 1e-6)
+
+
+def test_hmc_transition_in_backward_mode_matches_oracle():
+    """The HMC consumer on a backward-mode model: one transition (3 leapfrog steps, identity mass matrix) of 12 chains
+    near the config-1 truth against oracle/optim.py driven by oracle/linear.py: energy differences, accept decisions,
+    positions and the cached log-posterior / gradient.  The amplitude coordinates feel no force (zero gradient)."""
+    import copy as _copy
+    import torch
+    import oracle.linear as OL
+    from oracle import optim
+    from _cases import observation
+    gl = _gl()
+    wl, obs, sig = observation(1)
+    sp = _copy.copy(wl.spec); sp.amplitude_mode = 1
+    n = sp.n_params
+    idx = OL.amplitude_indices(sp)
+    rng = np.random.default_rng(41)
+    z0 = (wl.truth_z[0][None, :] + 0.01 * rng.standard_normal((12, n))).astype(np.float32)
+    xi = rng.standard_normal((12, n)).astype(np.float32)
+    log_u = np.log(rng.random(12)).astype(np.float32)
+    eps = 2e-5                                                          # stable for gradients of 1e5 (identity mass matrix)
+    m = gl.LensModel(sp, obs, sig, wl.psf)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    zg = d(z0)
+    lpg, gg = m.logpost_grad(zg)
+    acc = torch.zeros(12, dtype=torch.int32, device="cuda"); dh = torch.zeros(12, device="cuda")
+    ws = torch.empty(gl.gl_hmc_workspace_bytes(m.h, 12), dtype=torch.uint8, device="cuda")
+
+    def f(z):
+        r = OL.logpost_grad(sp, obs, sig, wl.psf, z.astype(np.float32).astype(np.float64))
+        return r["logp"], np.where(np.isfinite(r["logp"])[:, None], r["grad"], 0.0)
+
+    prev = [x.cpu().numpy().astype(np.float64) for x in (zg, lpg, gg)]
+    z_o, lp_o, g_o, acc_o, dh_o = optim.hmc_transition(f, prev[0], prev[1], prev[2], optim.tril_pack(np.eye(n)),
+                                                       xi.astype(np.float64), log_u.astype(np.float64),
+                                                       float(np.float32(eps)), 3)
+    gl.gl_hmc_step(m.h, m.obs, m.noise_sigma, m.psf, zg, lpg, gg, None, d(xi), d(log_u), None, eps, 3, acc, dh, ws)
+    torch.cuda.synchronize()
+    dh_g = dh.cpu().numpy().astype(np.float64); acc_g = acc.cpu().numpy().astype(bool)
+    assert np.isfinite(dh_o).all() and np.isfinite(dh_g).all()
+    assert np.all(np.abs(dh_g - dh_o) <= 1e-4 * np.abs(prev[1]) + 1e-6), np.max(np.abs(dh_g - dh_o))
+    decided = np.abs(log_u.astype(np.float64) - dh_o) > 1e-3
+    assert decided.sum() >= 9 and np.array_equal(acc_g[decided], acc_o[decided])
+    same = acc_g == acc_o
+    zz = zg.cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(zz[same] - z_o[same]) <= 2e-7 * np.abs(z_o[same]) + 1e-9)
+    gn = gg.cpu().numpy().astype(np.float64)
+    assert np.all(gn[:, idx] == 0)
+    assert np.all(np.abs(gn[same] - g_o[same]) <= np.maximum(1e-3 * np.abs(g_o[same]), 1e-5))
+    # the force-free amplitude coordinates of an accepted chain moved by exactly n_leapfrog * eps * xi
+    a = same & acc_g
+    assert a.any()
+    want = z0[a][:, idx].astype(np.float64) + 3 * float(np.float32(eps)) * xi[a][:, idx].astype(np.float64)
+    assert np.all(np.abs(zz[a][:, idx] - want) <= 4e-7 * np.abs(want) + 1e-7)
