@@ -71,9 +71,10 @@ typedef enum { GL_PRECISION_F64 = 0, GL_PRECISION_F32 = 1 } gl_precision;
 
 /* Model configuration.  The flat parameter vector has the block order of reading S18:
  *   main mass [theta_E, (gamma if EPL), e1, e2, x, y] . shear [g1, g2] . multipoles [c3, s3][c4, s4] .
- *   source Sersic [R, n, e1, e2, x, y, I] . shapelets [beta_s, a_0 .. a_{Nc-1}] . lens Sersic 1 . lens Sersic 2
+ *   source Sersic 1 [R, n, e1, e2, x, y, I] . source Sersic 2 (same source plane) . shapelets [beta_s, a_0 .. a_{Nc-1}] .
+ *   lens Sersic 1 . lens Sersic 2 . lens Sersic 3                       (absent blocks take no entries)
  * with Nc = (nmax+1)(nmax+2)/2 coefficients ordered by n1+n2 then n2 (O5, S9); the shapelet centre is the
- * source Sersic centre, so shapelets require n_source_sersic >= 1. */
+ * first source Sersic's centre, so shapelets require n_source_sersic >= 1. */
 typedef struct {
     int32_t n_pix;            /* N: detector pixels per side, >= 1 */
     int32_t supersample;      /* s: rays per pixel per side, >= 1 */

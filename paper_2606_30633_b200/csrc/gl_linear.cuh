@@ -76,15 +76,15 @@ __global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant
                                                            const int32_t* __restrict__ system_id, int64_t p_base,
                                                            T* __restrict__ pb, float* __restrict__ out_amp,
                                                            T* __restrict__ gpix, T* __restrict__ chi, int n_ctile, int TP) {
-    extern __shared__ double asm_[];
+    extern __shared__ double amp_sm[];
     const int n = am.n, np = n + 1, NN = G.N * G.N, tid = threadIdx.x;
     const int64_t p = blockIdx.x;
     const int sys = system_id ? system_id[p_base + p] : 0;
     const int npair = np * (np + 1) / 2;
-    double* ct = asm_;                                   // [np][TP + 1] tile of A_k / sigma (row n: obs / sigma); later M [n][n]
+    double* ct = amp_sm;                                   // [np][TP + 1] tile of A_k / sigma (row n: obs / sigma); later M [n][n]
     int ct_sz = np * (TP + 1) > n * n ? np * (TP + 1) : n * n;
     if (ct_sz < 256) ct_sz = 256;
-    double* pr = asm_ + ct_sz;                           // [npair] sums, pair (k, l), l <= k, at k(k+1)/2 + l
+    double* pr = amp_sm + ct_sz;                           // [npair] sums, pair (k, l), l <= k, at k(k+1)/2 + l
     double* rhs = pr + (npair > 256 ? npair : 256);     // [n]  (pr doubles as the 256-entry reduction buffer at the end)
     __shared__ int s_fail;
     if (tid == 0) s_fail = 0;
