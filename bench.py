@@ -249,6 +249,7 @@ def run_ours(a):
 
     # ---- the timed call of each stage (device-resident inputs) and its host-buffer form (pinned copies inside)
     evals_per_particle = 1
+    extra_launches = 0                                       # kernels launched per step outside the last counted API call
     pin = lambda t: t.cpu().pin_memory()
     if a.stage == "grad":
         zh = torch.from_numpy(wl.params).pin_memory()
@@ -288,12 +289,18 @@ def run_ours(a):
         tstep = [0]
         h2d_bytes, d2h_bytes = xih.numel() * 4, 8
 
-        def step():
+        extra_launches = 1
+
+        def step():                                          # fresh draws on the device every iteration (reading S22)
             tstep[0] += 1
+            gl.gl_draw_normal(2026, tstep[0], 0, xi)
             gl.gl_svi_step(m.h, belief, m.obs, m.noise_sigma, m.psf, mu, lt, xi, sid, sm, sv, tstep[0], stats, ws)
 
-        def step_host():
-            xi.copy_(xih, non_blocking=True); step(); statsh.copy_(stats, non_blocking=True)
+        def step_host():                                     # host-made draws through a pinned buffer
+            tstep[0] += 1
+            xi.copy_(xih, non_blocking=True)
+            gl.gl_svi_step(m.h, belief, m.obs, m.noise_sigma, m.psf, mu, lt, xi, sid, sm, sv, tstep[0], stats, ws)
+            statsh.copy_(stats, non_blocking=True)
     else:                                                    # NEXT-3: P chains, one transition of 4 leapfrog steps
         n_leap = 4
         evals_per_particle = n_leap
@@ -308,15 +315,23 @@ def run_ours(a):
         ws = torch.empty(gl.gl_hmc_workspace_bytes(m.h, P), dtype=torch.uint8, device=dev)
         h2d_bytes, d2h_bytes = (xih.numel() + luh.numel()) * 4, acch.numel() * 4
 
-        def step():
+        tstep = [0]
+        extra_launches = 2
+
+        def hmc():
             gl.gl_hmc_step(m.h, m.obs, m.noise_sigma, m.psf, zc, lpc, gc, None, xi, lu, sid, 2e-5, n_leap, acc, dh, ws)
 
-        def step_host():
-            xi.copy_(xih, non_blocking=True); lu.copy_(luh, non_blocking=True); step(); acch.copy_(acc, non_blocking=True)
+        def step():                                          # momenta and acceptance uniforms drawn on the device (S22)
+            tstep[0] += 1
+            gl.gl_draw_normal(2026, tstep[0], 1, xi); gl.gl_draw_log_uniform(2026, tstep[0], 2, lu)
+            hmc()
+
+        def step_host():                                     # host-made draws through pinned buffers
+            xi.copy_(xih, non_blocking=True); lu.copy_(luh, non_blocking=True); hmc(); acch.copy_(acc, non_blocking=True)
 
     for _ in range(max(a.warmup, 3)):
         step()
-    launches_per_step = int(gl.gl_last_launch_count())
+    launches_per_step = int(gl.gl_last_launch_count()) + extra_launches
     sampler = ClockSampler(local)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(a.steps)]
     barrier()

@@ -238,6 +238,19 @@ gl_status gl_hmc_step(const gl_config* cfg, const float* obs, const float* noise
                       int32_t* out_accept, float* out_dh, void* workspace, size_t workspace_bytes,
                       void* stream /* cudaStream_t */);
 
+/* Counter-based random draws for the SVI / HMC consumers (NEXT-2 / NEXT-3; reading S22): the paper draws inside
+ * TFP/JAX and names no generator.  Bits: Philox4x32-10 (Salmon et al., SC'11) with key = seed and
+ * counter = (step lo, step hi, row, stream_id << 24 | element / 4); normals by fp64 Box-Muller on the word pairs (0,1),
+ * (2,3) of a counter, rounded to fp32; uniforms u = (word + 0.5) 2^-32.  Stateless and independent of the launch
+ * geometry: the same (seed, step, stream_id, row, column) always yields the same value.
+ *   gl_draw_normal       out [n_rows][n_cols] fp32 standard normals (xi of gl_svi_step / gl_hmc_step)
+ *   gl_draw_log_uniform  out [n_rows] fp32 ln u, u uniform on (0,1)       (log_u of gl_hmc_step)
+ * DEVICE pointer `out`; stream_id <= 255 separates the uses within one step; n_rows < 2^32.
+ * Errors: GL_ERR_BAD_SHAPE (negative size), GL_ERR_BAD_CONFIG (stream_id or sizes out of range), GL_ERR_NULL, GL_ERR_CUDA. */
+gl_status gl_draw_normal(uint64_t seed, uint64_t step, uint32_t stream_id, int64_t n_rows, int32_t n_cols,
+                         float* out, void* stream);
+gl_status gl_draw_log_uniform(uint64_t seed, uint64_t step, uint32_t stream_id, int64_t n_rows, float* out, void* stream);
+
 /* Number of light amplitudes of a configuration (S18 order: source Sersic I, shapelet coefficients, lens Sersic I's);
  * 0 if cfg is NULL.  Defined for every amplitude_mode. */
 int32_t gl_config_n_amplitudes(const gl_config* cfg);

@@ -23,7 +23,7 @@ EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_wo
            "gl_last_launch_count", "gl_status_string", "gl_version", "gl_stage_timing_enable", "gl_stage_count",
            "gl_stage_name", "gl_stage_times", "gl_probe_pipe", "gl_map_step",
            "gl_svi_workspace_bytes", "gl_svi_step", "gl_hmc_workspace_bytes", "gl_hmc_step",
-           "gl_best_particle", "gl_config_n_amplitudes", "gl_linear_amplitudes"]
+           "gl_best_particle", "gl_config_n_amplitudes", "gl_linear_amplitudes", "gl_draw_normal", "gl_draw_log_uniform"]
 
 
 class GLError(RuntimeError):
@@ -93,6 +93,10 @@ def lib():
         L.gl_svi_workspace_bytes.argtypes = [vp, i64]
         L.gl_svi_step.restype = C.c_int
         L.gl_svi_step.argtypes = [vp, C.POINTER(gl_opt_desc), vp, vp, vp, vp, vp, vp, vp, i64, vp, vp, i64, vp, vp, sz, vp]
+        L.gl_draw_normal.restype = C.c_int
+        L.gl_draw_normal.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, i64, C.c_int32, vp, vp]
+        L.gl_draw_log_uniform.restype = C.c_int
+        L.gl_draw_log_uniform.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, i64, vp, vp]
         L.gl_config_n_amplitudes.restype = C.c_int32
         L.gl_config_n_amplitudes.argtypes = [vp]
         L.gl_linear_amplitudes.restype = C.c_int
@@ -213,6 +217,25 @@ def gl_logpost(h, obs, noise_sigma, psf, params, system_id, out_logp, workspace,
                             _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
                             _ptr(_dev(system_id, torch.int32, "system_id")), n, _ptr(_dev(out_logp, f32, "out_logp")),
                             _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)), "gl_logpost")
+
+
+def gl_draw_normal(seed, step, stream_id, out, stream=None):
+    """Fill the fp32 CUDA tensor out [n_rows][n_cols] with counter-based standard normals (include/gigalens.h)."""
+    torch = _torch()
+    _dev(out, torch.float32, "out")
+    assert out.dim() == 2
+    _check(lib().gl_draw_normal(int(seed), int(step), int(stream_id), out.shape[0], out.shape[1], _ptr(out), _stream(stream)),
+           "gl_draw_normal")
+    return out
+
+
+def gl_draw_log_uniform(seed, step, stream_id, out, stream=None):
+    torch = _torch()
+    _dev(out, torch.float32, "out")
+    assert out.dim() == 1
+    _check(lib().gl_draw_log_uniform(int(seed), int(step), int(stream_id), out.shape[0], _ptr(out), _stream(stream)),
+           "gl_draw_log_uniform")
+    return out
 
 
 def gl_config_n_amplitudes(h):
@@ -414,6 +437,44 @@ class LensModel:
         for t in range(first_step, first_step + n_steps):
             gl_map_step(self.h, opt, self.obs, self.noise_sigma, self.psf, params, sid, m, v, t, lp, g, ws, stream)
         return lp, (m, v)
+
+    def svi_run(self, mu, l_tril, opt, n_steps, n_draws, seed, first_step=1, state=None, stream=None):
+        """n_steps SVI iterations (gl_svi_step) on (mu, l_tril) IN PLACE with the draws made on the device
+        (gl_draw_normal, stream_id 0, step = the iteration number): nothing crosses the host between iterations.
+        Returns (stats [n_steps][2] = (loss, finite draws) per iteration, (m, v) optimiser state)."""
+        torch = _torch()
+        n = self.n_params
+        nt = n * (n + 1) // 2
+        m, v = state if state is not None else (torch.zeros(n + nt, dtype=torch.float32, device=self.device),
+                                                torch.zeros(n + nt, dtype=torch.float32, device=self.device))
+        xi = torch.empty((n_draws, n), dtype=torch.float32, device=self.device)
+        stats = torch.zeros((n_steps, 2), dtype=torch.float32, device=self.device)
+        need = gl_svi_workspace_bytes(self.h, n_draws)
+        ws = torch.empty(max(need, 256), dtype=torch.uint8, device=self.device)
+        for k, t in enumerate(range(first_step, first_step + n_steps)):
+            gl_draw_normal(seed, t, 0, xi, stream)
+            gl_svi_step(self.h, opt, self.obs, self.noise_sigma, self.psf, mu, l_tril, xi, None, m, v, t, stats[k], ws, stream)
+        return stats, (m, v)
+
+    def hmc_run(self, z, l_tril, step_size, n_leapfrog, n_transitions, seed, first_step=1, system_id=None, stream=None):
+        """n_transitions HMC transitions (gl_hmc_step) of the chains `z` IN PLACE, momenta and acceptance uniforms drawn
+        on the device (gl_draw_normal stream_id 1, gl_draw_log_uniform stream_id 2, step = the transition number).
+        Returns (logp, grad, accepted [n_transitions][n_chains] int32)."""
+        torch = _torch()
+        nc = z.shape[0]
+        sid = self._sid(system_id)
+        lp, g = self.logpost_grad(z, system_id, stream)
+        xi = torch.empty((nc, self.n_params), dtype=torch.float32, device=self.device)
+        lu = torch.empty(nc, dtype=torch.float32, device=self.device)
+        acc = torch.zeros((n_transitions, nc), dtype=torch.int32, device=self.device)
+        dh = torch.zeros(nc, dtype=torch.float32, device=self.device)
+        ws = torch.empty(max(gl_hmc_workspace_bytes(self.h, nc), 256), dtype=torch.uint8, device=self.device)
+        for k, t in enumerate(range(first_step, first_step + n_transitions)):
+            gl_draw_normal(seed, t, 1, xi, stream)
+            gl_draw_log_uniform(seed, t, 2, lu, stream)
+            gl_hmc_step(self.h, self.obs, self.noise_sigma, self.psf, z, lp, g, l_tril, xi, lu, sid, step_size, n_leapfrog,
+                        acc[k], dh, ws, stream)
+        return lp, g, acc
 
     def model_image(self, params, system_id=None, stream=None):
         torch = _torch()

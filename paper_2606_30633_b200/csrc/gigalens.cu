@@ -18,6 +18,7 @@
 #include "gl_svi.cuh"
 #include "gl_hmc.cuh"
 #include "gl_linear.cuh"
+#include "gl_rng.cuh"
 
 using namespace gl;
 
@@ -486,6 +487,30 @@ extern "C" gl_status gl_logpost_grad(const gl_config* cfg, const float* obs, con
                                      float* out_logp, float* out_grad, void* workspace, size_t workspace_bytes, void* stream) {
     return run(cfg, 1, obs, noise_sigma, psf, params, system_id, n_particles, out_logp, out_grad, nullptr,
                workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+extern "C" gl_status gl_draw_normal(uint64_t seed, uint64_t step, uint32_t stream_id, int64_t n_rows, int32_t n_cols,
+                                    float* out, void* stream) {
+    t_launches = 0;
+    if (n_rows < 0 || n_cols < 0) return GL_ERR_BAD_SHAPE;
+    if (stream_id > 255u || n_rows > 0xFFFFFFFFll || n_cols > (1 << 26)) return GL_ERR_BAD_CONFIG;
+    if (n_rows == 0 || n_cols == 0) return GL_OK;
+    if (!out) return GL_ERR_NULL;
+    const int64_t n = n_rows * ((n_cols + 3) / 4);
+    gl_draw_normal_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(seed, step, stream_id, n_rows, n_cols, out);
+    ++t_launches;
+    return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
+}
+
+extern "C" gl_status gl_draw_log_uniform(uint64_t seed, uint64_t step, uint32_t stream_id, int64_t n_rows, float* out, void* stream) {
+    t_launches = 0;
+    if (n_rows < 0) return GL_ERR_BAD_SHAPE;
+    if (stream_id > 255u || n_rows > 0xFFFFFFFFll) return GL_ERR_BAD_CONFIG;
+    if (n_rows == 0) return GL_OK;
+    if (!out) return GL_ERR_NULL;
+    gl_draw_log_uniform_kernel<<<(unsigned)((n_rows + 255) / 256), 256, 0, (cudaStream_t)stream>>>(seed, step, stream_id, n_rows, out);
+    ++t_launches;
+    return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
 }
 
 extern "C" gl_status gl_linear_amplitudes(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
