@@ -68,7 +68,7 @@ def parse():
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel at the default
 # workload, from the committed `ncu --set full` capture profiles/r1c_cfg2_f64.md (bench.py cannot run a profiler):
 # keyed by (config, precision, stage).  None elsewhere.
-NCU_TRAFFIC_BYTES = {(2, "f64", "ray_adjoint"): 2.153293e9 + 0.028e9}
+NCU_TRAFFIC_BYTES = {(2, "f64", "ray_adjoint"): 2.153155e9 + 0.035220e9}
 
 
 # ----------------------------------------------------------------------------------------------- clocks
