@@ -124,7 +124,8 @@ int32_t gl_config_n_params(const gl_config* cfg);
 
 /* Bytes of device workspace gl_logpost / gl_logpost_grad / gl_model_image need for n_particles
  * (0 if cfg is NULL or n_particles <= 0).  Grows with n_particles up to an internal chunk size, then stays
- * flat: larger batches are processed in chunks on the same stream.  The workspace must be 256-byte aligned. */
+ * flat (about 4 GiB; about 16 GiB with amplitude_mode 1, which keeps n_amp component images per particle): larger
+ * batches are processed in chunks on the same stream.  The workspace must be 256-byte aligned. */
 size_t gl_workspace_bytes(const gl_config* cfg, int64_t n_particles);
 
 /* log p~ for each particle (O1-O8):

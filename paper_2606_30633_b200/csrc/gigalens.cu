@@ -102,6 +102,9 @@ static constexpr int NT_ADJ = GL_NT_ADJ;
 #endif
 static constexpr int RB_FWD = GL_RB_FWD;  // rays a forward thread evaluates concurrently
 static constexpr size_t WS_BUDGET = (size_t)4096 << 20;   // chunk so that per-chunk buffers stay below ~4 GiB
+// Backward modelling keeps n_amp component images per particle: with the 4 GiB budget a 30-amplitude model is cut into
+// chunks of ~280 particles, too few CTAs for the one-CTA-per-particle kernels (config 3: 506 -> see DESIGN.md section 16).
+static constexpr size_t WS_BUDGET_AMP = (size_t)16384 << 20;
 
 static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -260,7 +263,7 @@ struct Plan {
 static Plan make_plan(const gl_config* c, int64_t P) {
     Plan pl{};
     const Geom& G = c->G;
-    int64_t pc_max = (int64_t)(WS_BUDGET / c->per_particle_bytes);
+    int64_t pc_max = (int64_t)((c->desc.amplitude_mode == 1 ? WS_BUDGET_AMP : WS_BUDGET) / c->per_particle_bytes);
     if (pc_max < 1) pc_max = 1;
     if (pc_max > 32768) pc_max = 32768;
     pl.Pc = P < pc_max ? P : pc_max;

@@ -51,23 +51,32 @@ __global__ void gl_amp_sid_kernel(const int32_t* __restrict__ sid, int64_t Pc, i
 // comp: [n_amp][Pc][gpix_stride] = -A_k in the padded g_pix layout.  sys_w: 1/sigma^2.  out_amp may be NULL.
 // A particle whose normal matrix is not positive definite (a component that leaves no light on the cutout) is
 // marked invalid (PB_VALID = 0: logp = -INF, zero gradient).
-constexpr int AMP_PPT = 10;          // pairs per thread: (AMP_MAX + 1)(AMP_MAX + 2) / 2 <= 256 * 11
-// Pixels per shared-memory tile.  Few pairs (the split mode below): as many as fit the largest problem's footprint
-// (multiple of 64, up to 1024), which amortises the two barriers per tile; many pairs: 64, where occupancy matters more
-// (config 3: 68 ms with 64-pixel tiles, 86 ms with 128).
+// Pixels per shared-memory tile and its layout.  Few pairs (n_pair <= 128, the split mode below): as many pixels as fit
+// the largest problem's footprint (multiple of 64, up to 1024), which amortises the two barriers per tile, row pitch
+// TP + 1.  Many pairs (the tensor-core mode): 64 pixels, rows padded to a multiple of 8, row pitch TP + 4 (an FP64
+// mma fragment load -- 8 rows x 4 consecutive pixels per half-warp pair -- is then bank-conflict free).
+static inline bool amp_solve_mma(int n) { return (n + 1) * (n + 2) / 2 > 128; }
 static inline int amp_solve_tp(int n) {
-    if ((n + 1) * (n + 2) / 2 > 128) return 64;
+    if (amp_solve_mma(n)) return 64;
     int tp = (4608 / (n + 1) - 1) / 64 * 64;
     return tp < 64 ? 64 : (tp > 1024 ? 1024 : tp);
 }
 static inline size_t amp_solve_smem(int n) {
     const int np = n + 1, tp = amp_solve_tp(n);
-    size_t ct = (size_t)np * (tp + 1);
+    size_t ct = amp_solve_mma(n) ? (size_t)((np + 7) / 8 * 8) * (tp + 4) : (size_t)np * (tp + 1);
     if (ct < (size_t)n * n) ct = (size_t)n * n;
     if (ct < 256) ct = 256;
     const size_t npair = (size_t)np * (np + 1) / 2;
     return sizeof(double) * (ct + (npair > 256 ? npair : 256) + n);
 }
+
+// D(8x8) += A(8x4) B(4x8) in fp64 on the tensor cores.  Lane l holds a = A[l/4][l%4], b = B[l%4][l/4],
+// (c0, c1) = C[l/4][2 (l%4) + {0, 1}].
+__device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+constexpr int AMP_TPW = 6;           // 8x8 output tiles per warp: 9 * 10 / 2 = 45 tiles at most over 8 warps
 
 template <class T>
 __global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant__ Geom G, const __grid_constant__ AmpMap am,
@@ -81,75 +90,84 @@ __global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant
     const int64_t p = blockIdx.x;
     const int sys = system_id ? system_id[p_base + p] : 0;
     const int npair = np * (np + 1) / 2;
-    double* ct = amp_sm;                                   // [np][TP + 1] tile of A_k / sigma (row n: obs / sigma); later M [n][n]
-    int ct_sz = np * (TP + 1) > n * n ? np * (TP + 1) : n * n;
+    const bool mma = npair > 128;                        // the normal matrix is a dense contraction over the pixels
+    const int NR = mma ? (np + 7) / 8 * 8 : np, PT = mma ? TP + 4 : TP + 1;
+    double* ct = amp_sm;                                 // [NR][PT] tile of A_k / sigma (row n: obs / sigma, then zero rows); later M [n][n]
+    int ct_sz = NR * PT > n * n ? NR * PT : n * n;
     if (ct_sz < 256) ct_sz = 256;
-    double* pr = amp_sm + ct_sz;                           // [npair] sums, pair (k, l), l <= k, at k(k+1)/2 + l
+    double* pr = amp_sm + ct_sz;                         // [npair] sums, pair (k, l), l <= k, at k(k+1)/2 + l
     double* rhs = pr + (npair > 256 ? npair : 256);     // [n]  (pr doubles as the 256-entry reduction buffer at the end)
     __shared__ int s_fail;
     if (tid == 0) s_fail = 0;
-    // Few pairs (npair <= 128): S = 256 / npair threads share one pair, each taking every S-th pixel of a tile; their
-    // partial sums are added in a fixed order at the end.  Many pairs: one thread owns up to AMP_PPT + 1 pairs.
-    const int S = npair <= 128 ? 256 / npair : 1;
+    // Split mode: S = 256 / npair threads share one pair, each taking every S-th pixel of a tile; their partial sums are
+    // added in a fixed order at the end.  Tensor-core mode: M = A A^T in 8x8 tiles of the lower triangle, warp w owns
+    // tiles w, w + 8, ...; one mma.m8n8k4 per tile and 4 pixels.
+    const int S = mma ? 1 : 256 / npair;
     const int my = tid / S, g = tid - my * S;             // split mode: pair index, pixel lane
-    double acc[AMP_PPT + 1]; int pk[AMP_PPT + 1], pl[AMP_PPT + 1];
+    const int lane = tid & 31, wrp = tid >> 5;
+    auto tri = [](int i, int& k, int& l) {
+        k = (int)((sqrt(8.0 * i + 1.0) - 1.0) * 0.5);
+        while (k * (k + 1) / 2 > i) --k;
+        while ((k + 1) * (k + 2) / 2 <= i) ++k;
+        l = i - k * (k + 1) / 2;
+    };
+    int pk = 0, pl = 0;                                   // split mode: this thread's pair
+    if (!mma && my < npair) tri(my, pk, pl);
+    const int ntile = (NR >> 3) * ((NR >> 3) + 1) / 2;
+    int ti[AMP_TPW], tj[AMP_TPW]; double c0[AMP_TPW], c1[AMP_TPW];
 #pragma unroll
-    for (int j = 0; j <= AMP_PPT; ++j) {
-        acc[j] = 0; pk[j] = 0; pl[j] = 0;
-        const int i = S > 1 ? my : tid + j * 256;
-        if (i < npair && (S == 1 || j == 0)) {
-            int k = (int)((sqrt(8.0 * i + 1.0) - 1.0) * 0.5);
-            while (k * (k + 1) / 2 > i) --k;
-            while ((k + 1) * (k + 2) / 2 <= i) ++k;
-            pk[j] = k; pl[j] = i - k * (k + 1) / 2;
-        }
+    for (int j = 0; j < AMP_TPW; ++j) {
+        ti[j] = tj[j] = 0; c0[j] = c1[j] = 0;
+        if (mma && wrp + 8 * j < ntile) tri(wrp + 8 * j, ti[j], tj[j]);
     }
+    double acc = 0;
     const size_t gs = gpix_stride(G);
     for (int t0 = 0; t0 < NN; t0 += TP) {
         __syncthreads();
-        for (int idx = tid; idx < np * TP; idx += 256) {
+        for (int idx = tid; idx < NR * TP; idx += 256) {
             const int k = idx / TP, x = idx - k * TP, pix = t0 + x;
             double v = 0;
-            if (pix < NN) {
+            if (pix < NN && k < np) {
                 const int r = pix / G.N, q = pix - r * G.N;
                 const double isg = sqrt((double)sys_w[(size_t)sys * NN + pix]);
                 v = k < n ? -(double)comp[((size_t)k * Pc + p) * gs + (size_t)(r + G.PADg) * G.Wg + q + G.PADg]
                           : (double)obs[(size_t)sys * NN + pix];
                 v *= isg;
             }
-            ct[k * (TP + 1) + x] = v;
+            ct[k * PT + x] = v;
         }
         __syncthreads();
-        if (S > 1) {
+        if (!mma) {
             if (my < npair) {
-                const double* a = ct + pk[0] * (TP + 1); const double* b = ct + pl[0] * (TP + 1);
-                double s = acc[0];
-                for (int x = g; x < TP; x += S) s = fma(a[x], b[x], s);
-                acc[0] = s;
+                const double* a = ct + pk * PT; const double* b = ct + pl * PT;
+                for (int x = g; x < TP; x += S) acc = fma(a[x], b[x], acc);
             }
         } else {
 #pragma unroll
-            for (int j = 0; j <= AMP_PPT; ++j) {
-                if (tid + j * 256 < npair) {
-                    const double* a = ct + pk[j] * (TP + 1); const double* b = ct + pl[j] * (TP + 1);
-                    double s = acc[j];
-                    for (int x0 = 0; x0 < TP; x0 += 64) {        // TP is a multiple of 64: constant trip count inside
-#pragma unroll
-                        for (int x = 0; x < 64; ++x) s = fma(a[x0 + x], b[x0 + x], s);
-                    }
-                    acc[j] = s;
+            for (int j = 0; j < AMP_TPW; ++j) {
+                if (wrp + 8 * j < ntile) {               // warp-uniform
+                    const double* a = ct + (8 * ti[j] + (lane >> 2)) * PT + (lane & 3);
+                    const double* b = ct + (8 * tj[j] + (lane >> 2)) * PT + (lane & 3);
+#pragma unroll 4
+                    for (int x0 = 0; x0 < TP; x0 += 4) dmma_m8n8k4(c0[j], c1[j], a[x0], b[x0]);
                 }
             }
         }
     }
     __syncthreads();
-    if (S > 1) {
-        ct[tid] = acc[0];                                 // [pair][S] partials (npair * S <= 256 <= ct_sz)
+    if (!mma) {
+        ct[tid] = acc;                                    // [pair][S] partials (npair * S <= 256 <= ct_sz)
         __syncthreads();
         if (tid < npair) { double s = 0; for (int x = 0; x < S; ++x) s += ct[tid * S + x]; pr[tid] = s; }
     } else {
 #pragma unroll
-        for (int j = 0; j <= AMP_PPT; ++j) if (tid + j * 256 < npair) pr[tid + j * 256] = acc[j];
+        for (int j = 0; j < AMP_TPW; ++j) {
+            if (wrp + 8 * j < ntile) {
+                const int row = 8 * ti[j] + (lane >> 2), col = 8 * tj[j] + 2 * (lane & 3);
+                if (row < np && col <= row) pr[row * (row + 1) / 2 + col] = c0[j];
+                if (row < np && col + 1 <= row) pr[row * (row + 1) / 2 + col + 1] = c1[j];
+            }
+        }
     }
     __syncthreads();
     // full symmetric M and rhs
