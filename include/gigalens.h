@@ -21,7 +21,10 @@
  *     different streams with different workspaces.  The caller must not touch outputs or workspace until the
  *     stream has reached the end of the call.
  *   - Errors are returned as gl_status; nothing is thrown or aborted across the ABI.  All argument checks run
- *     on the host before the first launch; on any error no kernel has been launched.
+ *     on the host before the first launch: on GL_ERR_NULL / _BAD_CONFIG / _BAD_SHAPE / _UNSUPPORTED / _WORKSPACE no
+ *     kernel has been launched.  GL_ERR_CUDA reports a failed launch or runtime call: the kernels enqueued before it
+ *     stay enqueued, nothing is enqueued after it, and the outputs are undefined.  A NON-sticky CUDA error left
+ *     pending by the caller's earlier work on this thread is cleared on entry (it is not this call's error).
  *   - Results are bit-identical for the same particle irrespective of batch composition, order or size
  *     (fixed reduction orders, no atomics): the analogue of P:L83 fn 2.
  *   - There is no CPU fallback.
@@ -65,8 +68,9 @@ typedef struct { int32_t kind; float a, b, lo, hi; } gl_prior;
  *                     (MUFU / FP32 results serve only as seeds of Newton steps): the mode that meets the north_star
  *                     tolerances on EVERY gradient component, including those whose per-ray terms cancel by 1e3-1e5.
  *   GL_PRECISION_F32  FP32 FMA pipe + MUFU approximations, fp64 only in the per-particle prologue/epilogue: about
- *                     1.3x faster; log-posterior within 1e-4 except at accidental cancellations, 99.4-99.9 % of the
- *                     gradient components within the bar (the misses are the ill-conditioned ones). */
+ *                     2x faster (measured 2.1x on config 2); log-posterior within 1e-4 except at accidental
+ *                     cancellations, 99.4-99.9 % of the gradient components within the bar (the misses are the
+ *                     ill-conditioned ones). */
 typedef enum { GL_PRECISION_F64 = 0, GL_PRECISION_F32 = 1 } gl_precision;
 
 /* Model configuration.  The flat parameter vector has the block order of reading S18:
@@ -121,6 +125,11 @@ void gl_config_destroy(gl_config* cfg);
 
 /* Parameter count implied by a configuration (S18); 0 if cfg is NULL. */
 int32_t gl_config_n_params(const gl_config* cfg);
+
+/* Array extents a caller needs to size its buffers (what the Python binding checks tensors against), HOST pointer
+ * out[5] = { n_pix N, psf_size K, n_systems, n_params, n_amplitudes }:  obs / noise_sigma hold n_systems * N * N
+ * floats, psf n_systems * K * K, params n * n_params, out_amp n * n_amplitudes.  Errors: GL_ERR_NULL. */
+gl_status gl_config_shape(const gl_config* cfg, int32_t* out);
 
 /* Bytes of device workspace gl_logpost / gl_logpost_grad / gl_model_image need for n_particles
  * (0 if cfg is NULL or n_particles <= 0).  Grows with n_particles up to an internal chunk size, then stays
@@ -183,8 +192,10 @@ gl_status gl_logpost_grad_host(const gl_config* cfg, const float* obs, const flo
  *   step       t = 1, 2, ... (bias correction)
  *   out_logp   [n] log p~ at the params BEFORE the update;  out_grad [n][n_params] its gradient (also scratch)
  * A particle whose log-posterior or gradient is not finite keeps its params and state.  Update arithmetic in fp64,
- * storage fp32.  Errors as gl_logpost_grad, plus GL_ERR_BAD_CONFIG for an invalid `opt` (lr <= 0, b outside [0,1),
- * eps < 0, step < 1). */
+ * storage fp32.  With amplitude_mode 1 the amplitude entries (ignored on input, zero gradient) are never updated.
+ * Errors as gl_logpost_grad, plus GL_ERR_BAD_CONFIG for an invalid `opt` (lr <= 0, b outside [0,1), eps < 0,
+ * step < 1, or a denominator that can vanish: eps == 0 for Adam, eps == eps_root == 0 for AdaBelief -- an element
+ * whose gradient is exactly 0 from step 1 on would otherwise become 0/0). */
 typedef enum { GL_OPT_ADAM = 0, GL_OPT_ADABELIEF = 1 } gl_opt_kind;
 typedef struct { int32_t kind; float lr, b1, b2, eps, eps_root; } gl_opt_desc;
 gl_status gl_map_step(const gl_config* cfg, const gl_opt_desc* opt, const float* obs, const float* noise_sigma,
@@ -210,6 +221,10 @@ gl_status gl_best_particle(const float* logp, int64_t n_particles, int64_t* out_
  *   xi       [n_draws][n_params]       DEVICE, standard-normal draws supplied by the caller (counter-based or any RNG)
  *   opt_m/opt_v [n_params + n_tril]    DEVICE in/out optimiser state over [mu; l_tril]
  *   out_stats [2] DEVICE: loss estimate, number of draws with a finite log p~ (the others are left out of the means)
+ * With amplitude_mode 1 the surrogate lives on the SAMPLED dimensions only: for every solved amplitude j (zero
+ * gradient by construction) mu_j, the entries of row and column j of L and their optimiser state are left untouched,
+ * and log L_jj and that dimension's (1/2) log(2 pi e) are left out of the loss (otherwise -log L_jj would drive L_jj
+ * to infinity and the loss to -infinity).
  * workspace >= gl_svi_workspace_bytes(cfg, n_draws).  Errors as gl_map_step. */
 size_t gl_svi_workspace_bytes(const gl_config* cfg, int64_t n_draws);
 gl_status gl_svi_step(const gl_config* cfg, const gl_opt_desc* opt, const float* obs, const float* noise_sigma,

@@ -82,32 +82,43 @@ def svi_draw(mu, L_packed, xi):
     return mu[None, :] + xi @ tril_unpack(mu.size, L_packed).T
 
 
-def svi_loss_and_grad(mu, L_packed, xi, logp, grad_logp):
-    """Sampled ELBO loss and its gradient w.r.t. (mu, packed L) from per-draw logp [N] and grad log p [N][n]."""
+def svi_loss_and_grad(mu, L_packed, xi, logp, grad_logp, active=None):
+    """Sampled ELBO loss and its gradient w.r.t. (mu, packed L) from per-draw logp [N] and grad log p [N][n].
+    active [n] bool (default all): the dimensions the surrogate lives on.  Backward modelling (PAPER.md L64, L311;
+    DESIGN.md section 16) solves the light amplitudes inside every evaluation, so log p~ does not depend on their
+    entries of z: the surrogate is the multivariate normal of the SAMPLED dimensions only -- entropy and gradient over
+    the active block, zero gradient for mu_j and for every L entry in a row or column of an inactive dimension."""
     n = np.asarray(mu).size
+    act = np.ones(n, bool) if active is None else np.asarray(active, bool)
     L = tril_unpack(n, L_packed)
     xi = np.asarray(xi, np.float64); g = np.asarray(grad_logp, np.float64); lp = np.asarray(logp, np.float64)
     ok = np.isfinite(lp) & np.all(np.isfinite(g), axis=1)
     N = int(ok.sum())
     d = np.diag(L)
-    loss = -np.sum(np.log(np.abs(d))) - 0.5 * n * np.log(2.0 * np.pi * np.e) - lp[ok].sum() / N
+    loss = -np.sum(np.log(np.abs(d[act]))) - 0.5 * int(act.sum()) * np.log(2.0 * np.pi * np.e) - lp[ok].sum() / N
     g_mu = -g[ok].sum(axis=0) / N
     g_L = -(g[ok].T @ xi[ok]) / N - np.diag(1.0 / d)
+    g_mu = np.where(act, g_mu, 0.0)
+    g_L = np.where(act[:, None] & act[None, :], g_L, 0.0)
     return loss, g_mu, tril_pack(g_L), N
 
 
-def svi_step(logp_grad_fn, mu, L_packed, xi, m, v, t, opt):
+def svi_step(logp_grad_fn, mu, L_packed, xi, m, v, t, opt, active=None):
     """One SVI iteration.  logp_grad_fn(z [N][n]) -> (logp [N], grad [N][n]).  State m, v over the concatenated
-    parameter vector [mu; packed L].  Returns (loss, mu_new, L_new, m_new, v_new, logp)."""
+    parameter vector [mu; packed L].  Entries of inactive dimensions (see svi_loss_and_grad) keep their value and
+    their optimiser state.  Returns (loss, mu_new, L_new, m_new, v_new, logp)."""
     n = np.asarray(mu).size
+    act = np.ones(n, bool) if active is None else np.asarray(active, bool)
     z = svi_draw(mu, L_packed, xi)
     lp, g = logp_grad_fn(z)
-    loss, g_mu, g_L, N = svi_loss_and_grad(mu, L_packed, xi, lp, g)
+    loss, g_mu, g_L, N = svi_loss_and_grad(mu, L_packed, xi, lp, g, act)
     theta = np.concatenate([np.asarray(mu, np.float64), np.asarray(L_packed, np.float64)])[None, :]
     grad_loss = np.concatenate([g_mu, g_L])[None, :]
-    th1, m1, v1 = update(opt["kind"], theta, -grad_loss, np.zeros(1), np.asarray(m, np.float64)[None, :],
-                         np.asarray(v, np.float64)[None, :], t, opt["lr"], opt["b1"], opt["b2"], opt["eps"],
-                         opt.get("eps_root", 0.0))
+    m0 = np.asarray(m, np.float64)[None, :]; v0 = np.asarray(v, np.float64)[None, :]
+    th1, m1, v1 = update(opt["kind"], theta, -grad_loss, np.zeros(1), m0, v0, t, opt["lr"], opt["b1"], opt["b2"],
+                         opt["eps"], opt.get("eps_root", 0.0))
+    live = np.concatenate([act, tril_pack(act[:, None] & act[None, :]).astype(bool)])[None, :]
+    th1 = np.where(live, th1, theta); m1 = np.where(live, m1, m0); v1 = np.where(live, v1, v0)
     return loss, th1[0, :n], th1[0, n:], m1[0], v1[0], lp
 
 

@@ -23,7 +23,8 @@ EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_wo
            "gl_last_launch_count", "gl_status_string", "gl_version", "gl_stage_timing_enable", "gl_stage_count",
            "gl_stage_name", "gl_stage_times", "gl_probe_pipe", "gl_map_step",
            "gl_svi_workspace_bytes", "gl_svi_step", "gl_hmc_workspace_bytes", "gl_hmc_step",
-           "gl_best_particle", "gl_config_n_amplitudes", "gl_linear_amplitudes", "gl_draw_normal", "gl_draw_log_uniform"]
+           "gl_best_particle", "gl_config_n_amplitudes", "gl_linear_amplitudes", "gl_draw_normal", "gl_draw_log_uniform",
+           "gl_config_shape"]
 
 
 class GLError(RuntimeError):
@@ -71,6 +72,8 @@ def lib():
         L.gl_config_destroy.argtypes = [vp]
         L.gl_config_n_params.restype = C.c_int32
         L.gl_config_n_params.argtypes = [vp]
+        L.gl_config_shape.restype = C.c_int
+        L.gl_config_shape.argtypes = [vp, C.POINTER(C.c_int32)]
         L.gl_workspace_bytes.restype = sz
         L.gl_workspace_bytes.argtypes = [vp, i64]
         L.gl_workspace_bytes_host.restype = sz
@@ -144,6 +147,7 @@ def gl_config_create(spec):
 
 
 def gl_config_destroy(h):
+    _shape_cache.pop(h.value if isinstance(h, C.c_void_p) else h, None)
     lib().gl_config_destroy(h)
 
 
@@ -203,6 +207,34 @@ def _ptr(t):
     return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
 
 
+def gl_config_shape(h):
+    """dict(n_pix, psf_size, n_systems, n_params, n_amplitudes) of a handle."""
+    out = (C.c_int32 * 5)()
+    _check(lib().gl_config_shape(h, out), "gl_config_shape")
+    return dict(zip(("n_pix", "psf_size", "n_systems", "n_params", "n_amplitudes"), (int(x) for x in out)))
+
+
+_shape_cache = {}
+
+
+def _extents(h, n, **arrays):
+    """Element-count checks of the tensors of one call against the configuration (the C ABI sees plain pointers, so a
+    wrongly sized tensor would otherwise be a silent out-of-bounds access on the device).  n = rows of the batch."""
+    key = h.value if isinstance(h, C.c_void_p) else h
+    sh = _shape_cache.get(key)
+    if sh is None:
+        sh = _shape_cache[key] = gl_config_shape(h)
+    N2, K2, S, P, A = sh["n_pix"] ** 2, sh["psf_size"] ** 2, sh["n_systems"], sh["n_params"], sh["n_amplitudes"]
+    T = P * (P + 1) // 2
+    want = {"obs": S * N2, "noise_sigma": S * N2, "psf": S * K2, "params": n * P, "system_id": n, "out_logp": n,
+            "out_grad": n * P, "out_image": n * N2, "out_amp": n * A, "opt_m": n * P, "opt_v": n * P, "mu": P, "l_tril": T,
+            "xi": n * P, "svi_m": P + T, "svi_v": P + T, "out_stats": 2, "z": n * P, "logp": n, "grad": n * P, "log_u": n,
+            "out_accept": n, "out_dh": n}
+    for name, t in arrays.items():
+        if t is not None and t.numel() != want[name]:
+            raise ValueError("%s has %d elements, the configuration needs %d" % (name, t.numel(), want[name]))
+
+
 def _stream(stream):
     torch = _torch()
     s = torch.cuda.current_stream() if stream is None else stream
@@ -213,6 +245,7 @@ def gl_logpost(h, obs, noise_sigma, psf, params, system_id, out_logp, workspace,
     torch = _torch()
     f32 = torch.float32
     n = params.shape[0]
+    _extents(h, n, obs=obs, noise_sigma=noise_sigma, psf=psf, params=params, system_id=system_id, out_logp=out_logp)
     _check(lib().gl_logpost(h, _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
                             _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
                             _ptr(_dev(system_id, torch.int32, "system_id")), n, _ptr(_dev(out_logp, f32, "out_logp")),
@@ -246,6 +279,7 @@ def gl_linear_amplitudes(h, obs, noise_sigma, psf, params, system_id, out_amp, o
     torch = _torch()
     f32 = torch.float32
     n = params.shape[0]
+    _extents(h, n, obs=obs, noise_sigma=noise_sigma, psf=psf, params=params, system_id=system_id, out_logp=out_logp, out_amp=out_amp)
     _check(lib().gl_linear_amplitudes(h, _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
                                       _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
                                       _ptr(_dev(system_id, torch.int32, "system_id")), n,
@@ -258,6 +292,7 @@ def gl_logpost_grad(h, obs, noise_sigma, psf, params, system_id, out_logp, out_g
     torch = _torch()
     f32 = torch.float32
     n = params.shape[0]
+    _extents(h, n, obs=obs, noise_sigma=noise_sigma, psf=psf, params=params, system_id=system_id, out_logp=out_logp, out_grad=out_grad)
     _check(lib().gl_logpost_grad(h, _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
                                  _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
                                  _ptr(_dev(system_id, torch.int32, "system_id")), n,
@@ -271,10 +306,10 @@ def gl_map_step(h, opt, obs, noise_sigma, psf, params, system_id, opt_m, opt_v, 
     """opt: dict(kind, lr, b1, b2, eps, eps_root) or a gl_opt_desc.  params / opt_m / opt_v are updated in place."""
     torch = _torch()
     f32 = torch.float32
-    if not isinstance(opt, gl_opt_desc):
-        opt = gl_opt_desc(int(opt["kind"]), float(opt["lr"]), float(opt["b1"]), float(opt["b2"]), float(opt["eps"]),
-                          float(opt.get("eps_root", 0.0)))
+    opt = _opt_desc(opt)
     n = params.shape[0]
+    _extents(h, n, obs=obs, noise_sigma=noise_sigma, psf=psf, params=params, system_id=system_id, out_logp=out_logp, out_grad=out_grad,
+             opt_m=opt_m, opt_v=opt_v)
     _check(lib().gl_map_step(h, C.byref(opt), _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
                              _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
                              _ptr(_dev(system_id, torch.int32, "system_id")), n, _ptr(_dev(opt_m, f32, "opt_m")),
@@ -309,6 +344,8 @@ def gl_hmc_step(h, obs, noise_sigma, psf, z, logp, grad, l_tril, xi, log_u, syst
     """One HMC transition of every chain (row of z); z, logp, grad are updated in place where the proposal is accepted."""
     torch = _torch()
     f32 = torch.float32
+    _extents(h, z.shape[0], obs=obs, noise_sigma=noise_sigma, psf=psf, z=z, logp=logp, grad=grad, l_tril=l_tril, xi=xi, log_u=log_u,
+             system_id=system_id, out_accept=out_accept, out_dh=out_dh)
     _check(lib().gl_hmc_step(h, _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
                              _ptr(_dev(psf, f32, "psf")), _ptr(_dev(z, f32, "z")), _ptr(_dev(logp, f32, "logp")),
                              _ptr(_dev(grad, f32, "grad")), _ptr(_dev(l_tril, f32, "l_tril")), _ptr(_dev(xi, f32, "xi")),
@@ -328,6 +365,8 @@ def gl_svi_step(h, opt, obs, noise_sigma, psf, mu, l_tril, xi, system_id, opt_m,
     torch = _torch()
     f32 = torch.float32
     opt = _opt_desc(opt)
+    _extents(h, xi.shape[0], obs=obs, noise_sigma=noise_sigma, psf=psf, mu=mu, l_tril=l_tril, xi=xi, system_id=system_id, svi_m=opt_m,
+             svi_v=opt_v, out_stats=out_stats)
     _check(lib().gl_svi_step(h, C.byref(opt), _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
                              _ptr(_dev(psf, f32, "psf")), _ptr(_dev(mu, f32, "mu")), _ptr(_dev(l_tril, f32, "l_tril")),
                              _ptr(_dev(xi, f32, "xi")), _ptr(_dev(system_id, torch.int32, "system_id")), xi.shape[0],
@@ -340,6 +379,7 @@ def gl_model_image(h, psf, params, system_id, out_image, workspace, stream=None)
     torch = _torch()
     f32 = torch.float32
     n = params.shape[0]
+    _extents(h, n, psf=psf, params=params, system_id=system_id, out_image=out_image)
     _check(lib().gl_model_image(h, _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
                                 _ptr(_dev(system_id, torch.int32, "system_id")), n,
                                 _ptr(_dev(out_image, f32, "out_image")), _ptr(workspace),
@@ -355,6 +395,8 @@ def gl_logpost_grad_host(h, obs, noise_sigma, psf, params_host, system_id, out_l
         if t is not None and not (isinstance(t, torch.Tensor) and (not t.is_cuda) and t.dtype == f32 and t.is_contiguous()):
             raise TypeError("%s must be a contiguous CPU float32 tensor" % nm)
     n = params_host.shape[0]
+    _extents(h, n, obs=obs, noise_sigma=noise_sigma, psf=psf, params=params_host, system_id=system_id, out_logp=out_logp_host,
+             out_grad=out_grad_host)
     _check(lib().gl_logpost_grad_host(h, _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
                                       _ptr(_dev(psf, f32, "psf")), _ptr(params_host),
                                       _ptr(_dev(system_id, torch.int32, "system_id")), n, _ptr(out_logp_host),
@@ -397,7 +439,12 @@ class LensModel:
         torch = _torch()
         if system_id is None:
             return None
-        return torch.as_tensor(system_id, dtype=torch.int32).contiguous().to(self.device)
+        if not (isinstance(system_id, torch.Tensor) and system_id.is_cuda):      # host ids: range-check before the copy
+            t = torch.as_tensor(system_id, dtype=torch.int32)
+            if t.numel() and (int(t.min()) < 0 or int(t.max()) >= self.spec.n_systems):
+                raise ValueError("system_id outside [0, n_systems)")
+            return t.contiguous().to(self.device)
+        return system_id.to(torch.int32).contiguous()
 
     def logpost(self, params, system_id=None, stream=None):
         torch = _torch()

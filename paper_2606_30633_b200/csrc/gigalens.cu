@@ -254,6 +254,11 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
 extern "C" void gl_config_destroy(gl_config* c) { delete c; }
 extern "C" int32_t gl_config_n_params(const gl_config* c) { return c ? c->L.n_params : 0; }
 extern "C" int32_t gl_config_n_amplitudes(const gl_config* c) { return c ? c->n_amp : 0; }
+extern "C" gl_status gl_config_shape(const gl_config* c, int32_t* out) {
+    if (!c || !out) return GL_ERR_NULL;
+    out[0] = c->desc.n_pix; out[1] = c->desc.psf_size; out[2] = c->desc.n_systems; out[3] = c->L.n_params; out[4] = c->n_amp;
+    return GL_OK;
+}
 
 struct Plan {
     int64_t Pc;
@@ -303,11 +308,15 @@ static void launch_ray_fwd(const gl_config* c, const T* pb, const double* tab, T
     gl_ray_fwd_kernel<T, V, NT_FWD, RB_FWD><<<grid, c->nt_fwd, 0, st>>>(c->G, pb, tab, ray, c->rpt_fwd, c->n_chunk_fwd);
 }
 template <class T, class V>
-static void launch_ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, int64_t Pc, cudaStream_t st) {
+static cudaError_t launch_ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, int64_t Pc, cudaStream_t st) {
     dim3 grid(c->n_nap, (unsigned)Pc);
     const size_t smem = coef_in_smem<T, V>() ? sizeof(T) * (size_t)V::NCOEF * c->nt_adj : 0;   // coefficient sums, one column per thread
-    if (smem > 40 * 1024) cudaFuncSetAttribute(gl_ray_adj_kernel<T, V, NT_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (smem > 40 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(gl_ray_adj_kernel<T, V, NT_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
     gl_ray_adj_kernel<T, V, NT_ADJ><<<grid, c->nt_adj, smem, st>>>(c->G, pb, tab, gbar, nap, c->rpt_adj, c->n_chunk_adj);
+    return cudaSuccess;
 }
 
 using V_S0 = Variant<0, 0, 1, -1, 1>; using V_E0 = Variant<1, 0, 1, -1, 1>;
@@ -355,19 +364,19 @@ static void ray_comp(const gl_config* c, const T* pb, const double* tab, T* cray
     }
 }
 template <class T>
-static void ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, int64_t Pc, cudaStream_t st) {
+static cudaError_t ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, int64_t Pc, cudaStream_t st) {
     const int id = c->variant * 2 + c->desc.mass_model;
     switch (id) {
-        case 0: launch_ray_adj<T, V_S0>(c, pb, tab, gbar, nap, Pc, st); break;
-        case 1: launch_ray_adj<T, V_E0>(c, pb, tab, gbar, nap, Pc, st); break;
-        case 2: launch_ray_adj<T, V_S1>(c, pb, tab, gbar, nap, Pc, st); break;
-        case 3: launch_ray_adj<T, V_E1>(c, pb, tab, gbar, nap, Pc, st); break;
-        case 4: launch_ray_adj<T, V_S2>(c, pb, tab, gbar, nap, Pc, st); break;
-        case 5: launch_ray_adj<T, V_E2>(c, pb, tab, gbar, nap, Pc, st); break;
-        case 6: launch_ray_adj<T, V_S3>(c, pb, tab, gbar, nap, Pc, st); break;
-        case 7: launch_ray_adj<T, V_E3>(c, pb, tab, gbar, nap, Pc, st); break;
-        case 8: launch_ray_adj<T, V_S4>(c, pb, tab, gbar, nap, Pc, st); break;
-        default: launch_ray_adj<T, V_E4>(c, pb, tab, gbar, nap, Pc, st); break;
+        case 0: return launch_ray_adj<T, V_S0>(c, pb, tab, gbar, nap, Pc, st);
+        case 1: return launch_ray_adj<T, V_E0>(c, pb, tab, gbar, nap, Pc, st);
+        case 2: return launch_ray_adj<T, V_S1>(c, pb, tab, gbar, nap, Pc, st);
+        case 3: return launch_ray_adj<T, V_E1>(c, pb, tab, gbar, nap, Pc, st);
+        case 4: return launch_ray_adj<T, V_S2>(c, pb, tab, gbar, nap, Pc, st);
+        case 5: return launch_ray_adj<T, V_E2>(c, pb, tab, gbar, nap, Pc, st);
+        case 6: return launch_ray_adj<T, V_S3>(c, pb, tab, gbar, nap, Pc, st);
+        case 7: return launch_ray_adj<T, V_E3>(c, pb, tab, gbar, nap, Pc, st);
+        case 8: return launch_ray_adj<T, V_S4>(c, pb, tab, gbar, nap, Pc, st);
+        default: return launch_ray_adj<T, V_E4>(c, pb, tab, gbar, nap, Pc, st);
     }
 }
 
@@ -442,28 +451,30 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
             if (nl < 0) return GL_ERR_CUDA;
             t_launches += nl;
         }
-        if (mode == 2) continue;
+        if (mode == 2) { if (cudaPeekAtLastError() != cudaSuccess) return GL_ERR_CUDA; continue; }
         if (mode == 1) {
             GL_STAGE(ST_CONV_BWD, st, nl = conv_bwd_launch<T>(c->conv, G, gpix, sys_kt, system_id, base, Pc, ray, st));
             if (nl < 0) return GL_ERR_CUDA;
             t_launches += nl;
-            GL_STAGE(ST_RAY_ADJ, st, ray_adj<T>(c, pb, tab, ray, nap, Pc, st)); ++t_launches;
+            cudaError_t ea = cudaSuccess;
+            GL_STAGE(ST_RAY_ADJ, st, ea = ray_adj<T>(c, pb, tab, ray, nap, Pc, st)); ++t_launches;
+            if (ea != cudaSuccess) return GL_ERR_CUDA;
         }
         const int wpb = 4;
         GL_STAGE(ST_FINALIZE, st, (gl_finalize_kernel<T><<<(unsigned)((Pc + wpb - 1) / wpb), wpb * 32, wpb * (NA_MAX + 256) * sizeof(double), st>>>(
             c->pt, L, G, params, pb, lpd, chi, c->n_ctile, mode == 1 ? nap : nullptr, c->n_nap, c->na,
             sys_sl, system_id, Pc, base, out_logp, out_grad)));
         ++t_launches;
+        if (cudaPeekAtLastError() != cudaSuccess) return GL_ERR_CUDA;     // a failed launch: enqueue no further chunk
     }
-    cudaError_t e = cudaPeekAtLastError();
-    return e == cudaSuccess ? GL_OK : GL_ERR_CUDA;
+    return GL_OK;
 }
 
-static gl_status run(const gl_config* c, int mode, const float* obs, const float* sigma, const float* psf,
-                     const float* params, const int32_t* system_id, int64_t P, float* out_logp, float* out_grad,
-                     float* out_image, void* ws, size_t ws_bytes, cudaStream_t st, float* out_amp = nullptr) {
-    t_launches = 0;
-    t_timer.reset();
+// Every argument check of the hot path, on the host, BEFORE any launch (the consumers gl_map_step / gl_svi_step /
+// gl_hmc_step call it before their own first kernel).  ws_bytes is what the hot path may use of the workspace.
+static gl_status validate(const gl_config* c, int mode, const float* obs, const float* sigma, const float* psf,
+                          const float* params, int64_t P, const float* out_logp, const float* out_grad,
+                          const float* out_image, const void* ws, size_t ws_bytes) {
     if (!c) return GL_ERR_NULL;
     if (P < 0) return GL_ERR_BAD_SHAPE;
     if (P == 0) return GL_OK;
@@ -471,8 +482,23 @@ static gl_status run(const gl_config* c, int mode, const float* obs, const float
     if (mode != 2 && (!obs || !sigma || !out_logp)) return GL_ERR_NULL;
     if (mode == 1 && !out_grad) return GL_ERR_NULL;
     if (mode == 2 && !out_image) return GL_ERR_NULL;
+    if (ws_bytes < make_plan(c, P).total || ((uintptr_t)ws & 255) != 0) return GL_ERR_WORKSPACE;
+    return GL_OK;
+}
+
+// A non-sticky CUDA error left behind by the caller's earlier work would otherwise be reported by the launch checks
+// of this call as GL_ERR_CUDA: it is cleared on entry (a sticky error stays and is reported).
+static inline void clear_stale_error() { (void)cudaGetLastError(); }
+
+static gl_status run(const gl_config* c, int mode, const float* obs, const float* sigma, const float* psf,
+                     const float* params, const int32_t* system_id, int64_t P, float* out_logp, float* out_grad,
+                     float* out_image, void* ws, size_t ws_bytes, cudaStream_t st, float* out_amp = nullptr) {
+    t_launches = 0;
+    t_timer.reset();
+    const gl_status sv = validate(c, mode, obs, sigma, psf, params, P, out_logp, out_grad, out_image, ws, ws_bytes);
+    if (sv != GL_OK || P == 0) return sv;
+    clear_stale_error();
     const Plan pl = make_plan(c, P);
-    if (ws_bytes < pl.total || ((uintptr_t)ws & 255) != 0) return GL_ERR_WORKSPACE;
     if (c->esize == 8)
         return run_t<double>(c, mode, obs, sigma, psf, params, system_id, P, out_logp, out_grad, out_image, out_amp, ws, pl, st);
     return run_t<float>(c, mode, obs, sigma, psf, params, system_id, P, out_logp, out_grad, out_image, out_amp, ws, pl, st);
@@ -500,6 +526,7 @@ extern "C" gl_status gl_draw_normal(uint64_t seed, uint64_t step, uint32_t strea
     if (n_rows == 0 || n_cols == 0) return GL_OK;
     if (!out) return GL_ERR_NULL;
     const int64_t n = n_rows * ((n_cols + 3) / 4);
+    clear_stale_error();
     gl_draw_normal_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(seed, step, stream_id, n_rows, n_cols, out);
     ++t_launches;
     return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
@@ -511,6 +538,7 @@ extern "C" gl_status gl_draw_log_uniform(uint64_t seed, uint64_t step, uint32_t 
     if (stream_id > 255u || n_rows > 0xFFFFFFFFll) return GL_ERR_BAD_CONFIG;
     if (n_rows == 0) return GL_OK;
     if (!out) return GL_ERR_NULL;
+    clear_stale_error();
     gl_draw_log_uniform_kernel<<<(unsigned)((n_rows + 255) / 256), 256, 0, (cudaStream_t)stream>>>(seed, step, stream_id, n_rows, out);
     ++t_launches;
     return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
@@ -534,6 +562,13 @@ extern "C" gl_status gl_model_image(const gl_config* cfg, const float* psf, cons
 
 static gl_status check_opt(const gl_opt_desc* opt, int64_t step);
 static OptParams opt_params(const gl_opt_desc* opt, int64_t step);
+// parameters no optimiser may move: the solved amplitudes of backward modelling (amplitude_mode 1)
+static DimMask dead_mask(const gl_config* c) {
+    DimMask m{};
+    if (c->desc.amplitude_mode == 1)
+        for (int i = 0; i < c->L.n_params; ++i) if (is_amp(c->L, i)) m.w[i >> 5] |= 1u << (i & 31);
+    return m;
+}
 
 extern "C" gl_status gl_map_step(const gl_config* cfg, const gl_opt_desc* opt, const float* obs, const float* noise_sigma,
                                  const float* psf, float* params, const int32_t* system_id, int64_t n_particles,
@@ -551,7 +586,7 @@ extern "C" gl_status gl_map_step(const gl_config* cfg, const gl_opt_desc* opt, c
     if (s != GL_OK) return s;
     const OptParams o = opt_params(opt, step);
     const int64_t n_elem = n_particles * cfg->L.n_params;
-    gl_opt_update_kernel<<<(unsigned)((n_elem + 255) / 256), 256, 0, st>>>(o, n_elem, cfg->L.n_params, out_logp, out_grad,
+    gl_opt_update_kernel<<<(unsigned)((n_elem + 255) / 256), 256, 0, st>>>(o, dead_mask(cfg), n_elem, cfg->L.n_params, out_logp, out_grad,
                                                                           params, opt_m, opt_v);
     ++t_launches;
     return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
@@ -561,6 +596,7 @@ extern "C" gl_status gl_best_particle(const float* logp, int64_t n, int64_t* out
     t_launches = 0;
     if (n < 0) return GL_ERR_BAD_SHAPE;
     if (!out_index || !out_logp || (n > 0 && !logp)) return GL_ERR_NULL;
+    clear_stale_error();
     gl_best_particle_kernel<<<1, 1024, 0, (cudaStream_t)stream>>>(logp, n, out_index, out_logp);
     t_launches = 1;
     return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
@@ -591,6 +627,8 @@ static gl_status check_opt(const gl_opt_desc* opt, int64_t step) {
     if (!(opt->lr > 0.f) || !(opt->b1 >= 0.f && opt->b1 < 1.f) || !(opt->b2 >= 0.f && opt->b2 < 1.f) || !(opt->eps >= 0.f) ||
         !(opt->eps_root >= 0.f) || step < 1)
         return GL_ERR_BAD_CONFIG;
+    // an element whose gradient is exactly 0 from step 1 makes the update 0 / (sqrt(0) + eps): the denominator must not vanish
+    if (opt->kind == GL_OPT_ADAM ? !(opt->eps > 0.f) : !(opt->eps > 0.f || opt->eps_root > 0.f)) return GL_ERR_BAD_CONFIG;
     return GL_OK;
 }
 static OptParams opt_params(const gl_opt_desc* opt, int64_t step) {
@@ -618,12 +656,15 @@ extern "C" gl_status gl_svi_step(const gl_config* cfg, const gl_opt_desc* opt, c
     float* z = (float*)(w + pl.off_z); float* lp = (float*)(w + pl.off_lp); float* g = (float*)(w + pl.off_g);
     double* part = (double*)(w + pl.off_part);
     const int np = cfg->L.n_params, nslot = 2 + np + np * (np + 1) / 2;
+    s = validate(cfg, 1, obs, noise_sigma, psf, z, n, lp, g, nullptr, workspace, pl.core);     // before the first launch
+    if (s != GL_OK) return s;
+    clear_stale_error();
     gl_svi_draw_kernel<<<(unsigned)((n * np + 255) / 256), 256, 0, st>>>(n, np, mu, l_tril, xi, z);
     s = run(cfg, 1, obs, noise_sigma, psf, z, system_id, n, lp, g, nullptr, workspace, pl.core, st);
     if (s != GL_OK) return s;
     const int64_t launches = t_launches + 1;
     gl_svi_reduce_kernel<<<dim3((nslot + 127) / 128, SVI_NCHUNK), 128, 0, st>>>(n, np, lp, g, xi, part);
-    gl_svi_update_kernel<<<1, 256, 0, st>>>(opt_params(opt, step), np, part, mu, l_tril, opt_m, opt_v, out_stats);
+    gl_svi_update_kernel<<<1, 256, 0, st>>>(opt_params(opt, step), dead_mask(cfg), np, part, mu, l_tril, opt_m, opt_v, out_stats);
     t_launches = launches + 2;
     return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
 }
@@ -666,6 +707,11 @@ extern "C" gl_status gl_hmc_step(const gl_config* cfg, const float* obs, const f
     float* zf = (float*)(w + pl.off_zf); float* g1 = (float*)(w + pl.off_g); float* lp1 = (float*)(w + pl.off_lp);
     const int np = cfg->L.n_params;
     const double eps = (double)step_size;
+    {   // before the first launch
+        const gl_status sv = validate(cfg, 1, obs, noise_sigma, psf, zf, n, lp1, g1, nullptr, workspace, pl.core);
+        if (sv != GL_OK) return sv;
+        clear_stale_error();
+    }
     int64_t launches = 0;
     for (int s = 0; s < n_leapfrog; ++s) {
         // half kick at the first step, the two half kicks of consecutive steps merged into one full kick afterwards

@@ -357,13 +357,20 @@ __global__ void __launch_bounds__(1024) gl_best_particle_kernel(const float* __r
 // One thread per element; a particle with a non-finite log-posterior or gradient row is left untouched (the
 // gradient row of such a particle is all zero by construction of gl_finalize_kernel, its logp is -INF).
 struct OptParams { int kind; double lr, b1, b2, eps, eps_root, c1, c2; };   // c1 = 1/(1-b1^t), c2 = 1/(1-b2^t)
+// One bit per parameter (n_params <= 128): the solved amplitudes of backward modelling, which no optimiser may move.
+struct DimMask {
+    uint32_t w[4];
+    __host__ __device__ bool test(int i) const { return (w[i >> 5] >> (i & 31)) & 1u; }
+    __host__ __device__ int count(int n) const { int c = 0; for (int i = 0; i < n; ++i) c += test(i); return c; }
+};
 
-__global__ void gl_opt_update_kernel(const __grid_constant__ OptParams o, int64_t n_elem, int n_params,
+__global__ void gl_opt_update_kernel(const __grid_constant__ OptParams o, const __grid_constant__ DimMask dead, int64_t n_elem, int n_params,
                                      const float* __restrict__ logp, const float* __restrict__ grad,
                                      float* __restrict__ z, float* __restrict__ m, float* __restrict__ v) {
     const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n_elem) return;
     const int64_t p = e / n_params;
+    if (dead.test((int)(e - p * n_params))) return;               // a solved amplitude: ignored on input, never updated
     const float lp = logp[p];
     const double g = -(double)grad[e];
     if (!isfinite(lp) || !isfinite(g)) return;

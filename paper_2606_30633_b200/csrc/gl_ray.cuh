@@ -1,8 +1,9 @@
 // gl_ray.cuh -- steps B + C (ray-trace + paint light) and the per-ray part of step F (adjoint).
 //
 // One CTA = one chunk of rays of one phase plane of ONE particle; the particle's derived scalars (PB) are staged in
-// shared memory once per CTA and every per-ray quantity lives in registers.  FP32 FMA pipe + MUFU
-// (rsqrt / lg2 / ex2 / rcp).  The 30-term EPL series (BASELINE.json configs[1]; reading S5) is a real-
+// shared memory once per CTA and every per-ray quantity lives in registers.  Arithmetic type T = double (default mode:
+// FP64 FMA pipe, MUFU results only as Newton seeds) or float (FP32 FMA pipe + MUFU rsqrt / lg2 / ex2 / rcp), see
+// gl_math.cuh.  The 30-term EPL series (BASELINE.json configs[1]; reading S5) is a real-
 // coefficient polynomial in w = -f e^{2 i phi}; because |w|^2 = f^2 is a per-particle constant it is
 // evaluated by synthetic division by (x - w)(x - conj w) = x^2 - p x + f^2, p = 2 Re w:
 //     b_k = a_k + p b_{k+1} - f^2 b_{k+2},   P(w) = b_1 w + (a_0 - f^2 b_2)

@@ -66,7 +66,10 @@ __device__ __forceinline__ double svi_total(const double* __restrict__ part, int
 
 // Second-level sums, loss, loss gradient and optimiser update of theta = [mu; packed L].  ONE block of 256 threads.
 // out_stats[0] = loss (Eq. 2 estimate), out_stats[1] = number of finite draws.
-__global__ void __launch_bounds__(256) gl_svi_update_kernel(const __grid_constant__ OptParams o, int np,
+// dead: bit j set = dimension j is not part of the surrogate (a solved amplitude of backward modelling, whose log p~
+// gradient is identically zero): its mu_j, every L entry of row or column j and their optimiser
+// state are left untouched, and log L_jj / the (1/2) log 2 pi e of that dimension stay out of the loss.
+__global__ void __launch_bounds__(256) gl_svi_update_kernel(const __grid_constant__ OptParams o, const __grid_constant__ DimMask dead, int np,
                                                             const double* __restrict__ part, float* __restrict__ mu,
                                                             float* __restrict__ Lp, float* __restrict__ m,
                                                             float* __restrict__ v, float* __restrict__ out_stats) {
@@ -75,12 +78,12 @@ __global__ void __launch_bounds__(256) gl_svi_update_kernel(const __grid_constan
     const double N = svi_total(part, nslot, 1);                  // every thread: same fixed-order sum, same value
     if (threadIdx.x == 0) {                                      // sum_j log |L_jj| from the OLD L, fixed order
         double l = 0.0;
-        for (int j = 0; j < np; ++j) l += log(fabs((double)Lp[(size_t)j * (j + 1) / 2 + j]));
+        for (int j = 0; j < np; ++j) if (!dead.test(j)) l += log(fabs((double)Lp[(size_t)j * (j + 1) / 2 + j]));
         s_logdiag = l;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        const double loss = N > 0 ? -s_logdiag - 0.5 * np * 2.8378770664093453 - svi_total(part, nslot, 0) / N : INFINITY;
+        const double loss = N > 0 ? -s_logdiag - 0.5 * (np - dead.count(np)) * 2.8378770664093453 - svi_total(part, nslot, 0) / N : INFINITY;
         out_stats[0] = (float)loss; out_stats[1] = (float)N;     // 2.8378... = 1 + ln 2 pi
     }
     if (!(N > 0)) return;
@@ -88,9 +91,10 @@ __global__ void __launch_bounds__(256) gl_svi_update_kernel(const __grid_constan
         double g = -svi_total(part, nslot, 2 + e) / N;            // d loss / d theta_e
         float* th = e < np ? mu + e : Lp + (e - np);
         if (e >= np) {
-            const int t = e - np, j = tril_row(t);
-            if (t - j * (j + 1) / 2 == j) g -= 1.0 / (double)*th;
-        }
+            const int t = e - np, j = tril_row(t), k = t - j * (j + 1) / 2;
+            if (dead.test(j) || dead.test(k)) continue;
+            if (k == j) g -= 1.0 / (double)*th;
+        } else if (dead.test(e)) continue;
         const double m1 = o.b1 * (double)m[e] + (1.0 - o.b1) * g;
         const double d = o.kind == 1 ? g - m1 : g;
         const double v1 = o.b2 * (double)v[e] + (1.0 - o.b2) * d * d + (o.kind == 1 ? o.eps_root : 0.0);

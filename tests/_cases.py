@@ -65,3 +65,30 @@ def grad_report(g_gpu, g_ref, gabs=None):
     if gabs is not None:
         rep["cond_aware"] = float(np.max(err / np.maximum(np.asarray(gabs), 1e-300)))
     return ok, rep
+
+
+def small_case(n_pix, s, K, mass_model, multipole_mask, shapelet_nmax, n_lens, seed, n_particles=6, epl_terms=30,
+               psf_grid=0, with_truth=False):
+    """A seeded small problem of arbitrary shape: spec with config-style priors, Gaussian PSF, oracle-rendered truth.
+    Returns (spec, obs, sigma, psf, z [n_particles][n_params] prior draws) and, with_truth, the fp32 truth z [n_params]."""
+    pri = W._default_priors(mass_model, multipoles=bool(multipole_mask), shapelet_nmax=shapelet_nmax, n_lens=n_lens)
+    if multipole_mask and multipole_mask != 3:
+        # _default_priors adds 4 multipole entries; keep 2 for a single order
+        k0 = 1 + (1 if mass_model == 1 else 0) + 4 + 2
+        pri = pri[:k0] + pri[k0 + 2:]
+    sp = W.LensSpec(n_pix, s, K, W._r32(0.11 * 40 / n_pix * 2.4), mass_model=mass_model, epl_terms=epl_terms,
+                    multipole_mask=multipole_mask, shapelet_nmax=shapelet_nmax, n_lens_sersic=n_lens, psf_grid=psf_grid,
+                    priors=pri)
+    sp.names = W.param_names(mass_model, 1, multipole_mask, 1, shapelet_nmax, n_lens)
+    assert len(sp.names) == sp.n_params
+    rng = np.random.default_rng(seed)
+    step = sp.pix_scale / s if psf_grid == 0 else sp.pix_scale      # taps at ray spacing (S10) or pixel spacing (S10b)
+    psf = W.gaussian_psf(K, 2.5 * step, step)[None].astype(np.float32)
+    truth_z = W.z_of(pri, W.draw(rng, pri, 1)).astype(np.float32)
+    truth = oracle.model_image(sp, psf.astype(np.float64), W.theta_of(pri, truth_z.astype(np.float64)))
+    sigma = np.full((1, n_pix, n_pix), 0.05, np.float32)
+    obs = (truth + 0.05 * rng.standard_normal(truth.shape)).astype(np.float32)
+    z = W.z_of(pri, W.draw(rng, pri, n_particles)).astype(np.float32)
+    if with_truth:
+        return sp, obs, sigma, psf, z, truth_z[0]
+    return sp, obs, sigma, psf, z

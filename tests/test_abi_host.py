@@ -134,3 +134,40 @@ def test_amplitude_mode_is_validated_on_the_host(gl):
     sp.noise_model = 0; sp.amplitude_mode = 2
     with pytest.raises(gl.GLError):
         gl.gl_config_create(sp)
+
+
+def test_optimiser_denominator_must_not_vanish_and_consumers_validate_on_the_host(gl):
+    """An update 0 / (sqrt(0) + 0) would write NaN (an element whose gradient is exactly 0 from step 1 on): Adam needs
+    eps > 0, AdaBelief eps > 0 or eps_root > 0.  And gl_svi_step / gl_hmc_step answer a NULL observation with
+    GL_ERR_NULL on the host, before their first kernel (this box has no GPU: a launch would report GL_ERR_CUDA)."""
+    L = gl.lib()
+    h = gl.gl_config_create(W.make_spec(1))
+    null = C.c_void_p(0)
+    bad = [gl.gl_opt_desc(0, 1e-3, 0.9, 0.999, 0.0, 0.0), gl.gl_opt_desc(0, 1e-3, 0.9, 0.999, 0.0, 1e-8),
+           gl.gl_opt_desc(1, 1e-4, 0.95, 0.99, 0.0, 0.0)]
+    for o in bad:
+        assert L.gl_map_step(h, C.byref(o), null, null, null, null, null, 4, null, null, 1, null, null, null, 0, null) == -2
+        assert L.gl_svi_step(h, C.byref(o), null, null, null, null, null, null, null, 4, null, null, 1, null, null, 0, null) == -2
+    ok = gl.gl_opt_desc(1, 1e-4, 0.95, 0.99, 0.0, 1e-16)
+    assert L.gl_map_step(h, C.byref(ok), null, null, null, null, null, 0, null, null, 1, null, null, null, 0, null) == 0
+    # consumers: every pointer of their own set is a (fake, never dereferenced on the host) non-NULL address, the
+    # observation is NULL -> GL_ERR_NULL from the hot path's validation, no launch attempted
+    fake = C.c_void_p(1 << 20)
+    n = 4
+    assert L.gl_svi_step(h, C.byref(ok), null, fake, fake, fake, fake, fake, null, n, fake, fake, 1, fake,
+                         fake, L.gl_svi_workspace_bytes(h, n), null) == -1
+    assert L.gl_hmc_step(h, null, fake, fake, fake, fake, fake, null, fake, fake, null, n, 1e-3, 2, fake, fake,
+                         fake, L.gl_hmc_workspace_bytes(h, n), null) == -1
+    assert L.gl_last_launch_count() == 0
+    gl.gl_config_destroy(h)
+
+
+@pytest.mark.parametrize("k", [1, 3, 4])
+def test_config_shape(gl, k):
+    sp = W.make_spec(k)
+    h = gl.gl_config_create(sp)
+    sh = gl.gl_config_shape(h)
+    assert sh == dict(n_pix=sp.n_pix, psf_size=sp.psf_size, n_systems=sp.n_systems, n_params=sp.n_params,
+                      n_amplitudes=gl.gl_config_n_amplitudes(h))
+    assert gl.lib().gl_config_shape(C.c_void_p(0), (C.c_int32 * 5)()) == -1
+    gl.gl_config_destroy(h)

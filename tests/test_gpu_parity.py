@@ -10,6 +10,7 @@ import pytest
 
 import workloads as W
 from _cases import ATOL_GRAD, RTOL_GRAD, RTOL_LOGP, grad_report, observation, oracle_subset
+from _cases import small_case as _small_case
 
 pytestmark = pytest.mark.gpu
 
@@ -218,31 +219,6 @@ def test_determinism_repeat_calls():
     assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
 
 
-def _small_case(n_pix, s, K, mass_model, multipole_mask, shapelet_nmax, n_lens, seed, n_particles=6, epl_terms=30,
-                psf_grid=0):
-    """A seeded small problem of arbitrary shape: spec with config-style priors, Gaussian PSF, oracle-rendered truth."""
-    import oracle
-    pri = W._default_priors(mass_model, multipoles=bool(multipole_mask), shapelet_nmax=shapelet_nmax, n_lens=n_lens)
-    if multipole_mask and multipole_mask != 3:
-        # _default_priors adds 4 multipole entries; keep 2 for a single order
-        k0 = 1 + (1 if mass_model == 1 else 0) + 4 + 2
-        pri = pri[:k0] + pri[k0 + 2:]
-    sp = W.LensSpec(n_pix, s, K, W._r32(0.11 * 40 / n_pix * 2.4), mass_model=mass_model, epl_terms=epl_terms,
-                    multipole_mask=multipole_mask, shapelet_nmax=shapelet_nmax, n_lens_sersic=n_lens, psf_grid=psf_grid,
-                    priors=pri)
-    sp.names = W.param_names(mass_model, 1, multipole_mask, 1, shapelet_nmax, n_lens)
-    assert len(sp.names) == sp.n_params
-    rng = np.random.default_rng(seed)
-    step = sp.pix_scale / s if psf_grid == 0 else sp.pix_scale      # taps at ray spacing (S10) or pixel spacing (S10b)
-    psf = W.gaussian_psf(K, 2.5 * step, step)[None].astype(np.float32)
-    truth_z = W.z_of(pri, W.draw(rng, pri, 1)).astype(np.float32)
-    truth = oracle.model_image(sp, psf.astype(np.float64), W.theta_of(pri, truth_z.astype(np.float64)))
-    sigma = np.full((1, n_pix, n_pix), 0.05, np.float32)
-    obs = (truth + 0.05 * rng.standard_normal(truth.shape)).astype(np.float32)
-    z = W.z_of(pri, W.draw(rng, pri, n_particles)).astype(np.float32)
-    return sp, obs, sigma, psf, z
-
-
 @pytest.mark.parametrize("shape", [(12, 3, 5), (9, 1, 3), (16, 2, 7), (10, 4, 9), (7, 5, 1)])
 @pytest.mark.parametrize("model", [(0, 0, -1, 1), (1, 3, 4, 2), (1, 2, -1, 0)])
 def test_generic_shapes_strict_parity(shape, model):
@@ -412,3 +388,36 @@ def test_series_bands_across_ellipticity(ell):
     assert np.all(np.abs(lp - ref["logp"]) <= RTOL_LOGP * np.abs(ref["logp"]))
     ok, rep = grad_report(g, ref["grad"])
     assert rep["n_fail"] == 0, rep
+
+
+@pytest.mark.parametrize("ell", [0.0, 1e-13])
+@pytest.mark.parametrize("precision", [0, 1])
+def test_sie_sis_branch_strict_parity(ell, precision):
+    """The SIS branch of the SIE deflection (csrc/gl_ray.cuh ray_eval, q' < 1e-6; oracle sie_frame, pinned by
+    tests/test_oracle_pins.py::test_sie_sis_branch_is_the_singular_isothermal_sphere): SIE spec, mass ellipticity
+    exactly 0 and 1e-13, theta_E from the prior (0.8 .. 1.5, so the branch carries the whole deflection): strict bar on
+    the model image, log-posterior and every gradient component in fp64 mode; the mass-ellipticity gradient is the
+    guard value (prior term only, O9)."""
+    import dataclasses
+    import oracle
+    import torch
+    gl = _gl()
+    sp, obs, sigma, psf, z = _small_case(20, 2, 5, 0, 0, -1, 1, seed=4242, n_particles=8)
+    ang = np.linspace(0.2, 2.8, 8)
+    z[:, 1] = (ell * np.cos(ang)).astype(np.float32); z[:, 2] = (ell * np.sin(ang)).astype(np.float32)
+    sp = dataclasses.replace(sp, precision=precision)
+    ref = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), None, want_model=True)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    zt = torch.from_numpy(z).cuda()
+    lp, g = m.logpost_grad(zt)
+    img = m.model_image(zt).cpu().numpy().astype(np.float64)
+    lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+    assert np.isfinite(ref["logp"]).all() and np.isfinite(lp).all()
+    scale = np.abs(ref["model"]).max(axis=(1, 2), keepdims=True)
+    assert np.max(np.abs(img - ref["model"]) / scale) < (2e-7 if precision == 0 else 2e-5)
+    assert np.all(np.abs(lp - ref["logp"]) <= RTOL_LOGP * np.abs(ref["logp"]))
+    ok, rep = grad_report(g, ref["grad"])
+    if precision == 0:
+        assert rep["n_fail"] == 0, rep
+    else:
+        assert rep["normwise"] <= 2e-3, rep

@@ -99,3 +99,105 @@ def test_svi_argument_checks():
     with pytest.raises(gl.GLError) as e:
         gl.gl_svi_step(m.h, dict(ADAM, b2=1.5), m.obs, m.noise_sigma, m.psf, d(mu), d(lt), d(xi), None, mm, vv, 1, stats, ws)
     assert e.value.status == -2
+
+
+def _big_setup(n_draws, seed, amplitude_mode=0):
+    """The config-3 parameter layout (EPL + shear, Sersic + shapelets n_max = 6, two lens Sersics: 58 parameters) on a
+    16x16, s = 2, K = 5 geometry, so that the oracle evaluates EVERY draw in seconds; dense L."""
+    import dataclasses
+    import torch
+    import paper_2606_30633_b200 as gl
+    from _cases import small_case
+    sp, obs, sig, psf, z, truth_z = small_case(16, 2, 5, 1, 0, 6, 2, seed=seed, n_particles=2, with_truth=True)
+    sp = dataclasses.replace(sp, amplitude_mode=amplitude_mode)
+    n = sp.n_params
+    assert n == 58
+    rng = np.random.default_rng(seed + 1)
+    L = np.tril(0.001 * rng.standard_normal((n, n))) + np.diag(0.004 + 0.004 * rng.random(n))
+    lt = L[np.tril_indices(n)].astype(np.float32)
+    xi = rng.standard_normal((n_draws, n)).astype(np.float32)
+    m = gl.LensModel(sp, obs, sig, psf)
+    return gl, torch, sp, obs, sig, psf, m, truth_z.astype(np.float32).copy(), lt, xi
+
+
+@pytest.mark.parametrize("opt", [ADABELIEF, ADAM], ids=["adabelief", "adam"])
+def test_svi_step_58_params_2048_draws(opt):
+    """gl_svi_reduce_kernel's 32-chunk two-level sums, tril_row and the update over 58 + 1711 surrogate parameters:
+    two iterations of 2048 draws (3 of them thrown out of the model's domain) on the config-3 layout, the oracle
+    evaluating every draw; loss, mu, L and the optimiser state against oracle/optim.py."""
+    import oracle
+    from oracle import optim
+    gl, torch, sp, obs, sig, psf, m, mu, lt, xi = _big_setup(2048, 303)
+    for r in (5, 700, 2047):
+        xi[r, 2] = 5.0e4                                                # mass e1 far outside the unit disc
+    n = sp.n_params; nt = n * (n + 1) // 2
+    opt_o = {k: (float(np.float32(x)) if k != "kind" else x) for k, x in opt.items()}
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    mu_g, lt_g, xi_g = d(mu), d(lt), d(xi)
+    mm, vv = torch.zeros(n + nt, device="cuda"), torch.zeros(n + nt, device="cuda")
+    stats = torch.zeros(2, device="cuda")
+    ws = torch.empty(gl.gl_svi_workspace_bytes(m.h, 2048), dtype=torch.uint8, device="cuda")
+
+    def f(z):
+        r = oracle.logpost_grad(sp, obs, sig, psf, z.astype(np.float32).astype(np.float64), None)
+        return r["logp"], r["grad"]
+
+    for t in (1, 2):
+        prev = [x.cpu().numpy().astype(np.float64) for x in (mu_g, lt_g, mm, vv)]
+        loss_o, mu_o, lt_o, m_o, v_o, lp_o = optim.svi_step(f, prev[0], prev[1], xi.astype(np.float64), prev[2], prev[3], t, opt_o)
+        gl.gl_svi_step(m.h, opt, m.obs, m.noise_sigma, m.psf, mu_g, lt_g, xi_g, None, mm, vv, t, stats, ws)
+        torch.cuda.synchronize()
+        assert int(stats[1]) == int(np.isfinite(lp_o).sum()) == 2045
+        assert abs(float(stats[0]) - loss_o) <= 1e-4 * abs(loss_o)
+        th_prev = np.concatenate(prev[:2]); th_o = np.concatenate([mu_o, lt_o])
+        th_g = np.concatenate([mu_g.cpu().numpy(), lt_g.cpu().numpy()]).astype(np.float64)
+        for got, want, old, c, name in ((th_g, th_o, th_prev, 1.0, "theta"), (mm.cpu().numpy().astype(np.float64), m_o, prev[2], opt_o["b1"], "m"),
+                                        (vv.cpu().numpy().astype(np.float64), v_o, prev[3], opt_o["b2"], "v")):
+            scale = np.abs(c * old) + np.abs(want - c * old)
+            bad = np.abs(got - want) > 2e-3 * np.abs(want - c * old) + 4e-7 * scale + 1e-30
+            assert not bad.any(), (name, t, int(bad.sum()), np.flatnonzero(bad)[:8])
+
+
+def test_svi_backward_mode_surrogate_lives_on_the_sampled_dimensions():
+    """amplitude_mode 1 (the combination of the paper's real-system run): the solved amplitudes have zero
+    gradient, so their mu_j, the rows and columns j of L and their optimiser state must not move and log L_jj must stay out of
+    the loss; everything else follows oracle/optim.py (active mask, pinned in tests/test_oracle_optim.py) on top of
+    oracle/linear.py.  Three iterations; the loss must not drift downwards through the dead dimensions."""
+    import oracle.linear as OL
+    from oracle import optim
+    gl, torch, sp, obs, sig, psf, m, mu, lt, xi = _big_setup(96, 411, amplitude_mode=1)
+    n = sp.n_params; nt = n * (n + 1) // 2
+    amp = np.asarray(OL.amplitude_indices(sp)); act = np.ones(n, bool); act[amp] = False
+    assert (~act).sum() == 31
+    opt = dict(ADAM, lr=2e-4)
+    opt_o = {k: (float(np.float32(x)) if k != "kind" else x) for k, x in opt.items()}
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    mu_g, lt_g = d(mu), d(lt)
+    mm, vv = torch.zeros(n + nt, device="cuda"), torch.zeros(n + nt, device="cuda")
+    stats = torch.zeros(2, device="cuda")
+    ws = torch.empty(gl.gl_svi_workspace_bytes(m.h, 96), dtype=torch.uint8, device="cuda")
+
+    def f(z):
+        r = OL.logpost_grad(sp, obs, sig, psf, z.astype(np.float32).astype(np.float64))
+        return r["logp"], r["grad"]
+
+    live = np.concatenate([act, optim.tril_pack(act[:, None] & act[None, :]).astype(bool)])
+    th0 = np.concatenate([mu, lt]).astype(np.float64)
+    rng = np.random.default_rng(5)
+    losses = []
+    for t in (1, 2, 3):
+        x = rng.standard_normal((96, n)).astype(np.float32)
+        prev = [a.cpu().numpy().astype(np.float64) for a in (mu_g, lt_g, mm, vv)]
+        loss_o, mu_o, lt_o, m_o, v_o, lp_o = optim.svi_step(f, prev[0], prev[1], x.astype(np.float64), prev[2], prev[3], t, opt_o, active=act)
+        gl.gl_svi_step(m.h, opt, m.obs, m.noise_sigma, m.psf, mu_g, lt_g, d(x), None, mm, vv, t, stats, ws)
+        torch.cuda.synchronize()
+        assert int(stats[1]) == int(np.isfinite(lp_o).sum()) >= 90
+        assert abs(float(stats[0]) - loss_o) <= 1e-4 * abs(loss_o)
+        losses.append(float(stats[0]))
+        th_g = np.concatenate([mu_g.cpu().numpy(), lt_g.cpu().numpy()]).astype(np.float64)
+        th_o = np.concatenate([mu_o, lt_o]); th_p = np.concatenate(prev[:2])
+        assert np.array_equal(th_g[~live], th0[~live])                   # dead entries: bit-identical to the start
+        assert np.all(mm.cpu().numpy()[~live] == 0) and np.all(vv.cpu().numpy()[~live] == 0)
+        step = np.abs(th_o - th_p)
+        assert np.all(np.abs(th_g - th_o)[live] <= 2e-3 * step[live] + 4e-7 * (np.abs(th_p) + step)[live] + 1e-30)
+    assert np.isfinite(losses).all()

@@ -144,6 +144,37 @@ def test_gradient_vs_finite_differences(kind, param_space):
         assert abs(g[k] - ref) < 2e-6 * abs(ref) + 1e-5, (k, g[k], ref)
 
 
+@pytest.mark.parametrize("param_space", [1, 0])
+def test_gradient_sis_branch_vs_finite_differences(param_space):
+    """SIE with mass eps == 0 exactly (q' < 1e-6: the SIS branch of sie_frame, theta_E = 0.55 so the lens does deflect):
+    every gradient component except the two mass ellipticities against central differences; the ellipticity
+    components are the guard value 0 (O9: c < 1e-10)."""
+    sp, psf, obs, sig, x0 = _tiny("sie", param_space)
+    x0 = x0.copy(); x0[1] = 0.0; x0[2] = 0.0
+    o = oracle.logpost_grad(sp, obs, sig, psf, [x0])
+    g = o["grad"][0]
+    assert np.isfinite(o["logp"][0])
+    if param_space == 1:
+        assert g[1] == 0.0 and g[2] == 0.0
+    lp = lambda x: oracle.logpost_grad(sp, obs, sig, psf, [x], want_grad=False)["logp"][0]
+    for k in [0] + list(range(3, sp.n_params)):
+        def f(v, k=k):
+            x = x0.copy(); x[k] = v; return lp(x)
+        ref = fd(f, x0[k], 2e-4 * max(1.0, abs(x0[k])))
+        assert abs(g[k] - ref) < 2e-6 * abs(ref) + 1e-5, (k, g[k], ref)
+    # and the branch agrees with the EPL series at gamma = 2 on the same circular lens (same logp, same gradient)
+    ep = W.LensSpec(6, 2, 3, 0.30, mass_model=1, param_space=1)
+    ep.priors = [W.NoPrior()] * 22
+    th = x0 if param_space == 1 else W.theta_of(sp.priors, x0[None])[0]
+    sp1 = W.LensSpec(6, 2, 3, 0.30, mass_model=0, param_space=1); sp1.priors = [W.NoPrior()] * 21
+    a = oracle.logpost_grad(sp1, obs, sig, psf, [th])
+    b = oracle.logpost_grad(ep, obs, sig, psf, [np.concatenate([th[:1], [2.0], th[1:]])])
+    assert abs(a["logp"][0] - b["logp"][0]) < 1e-9 * abs(a["logp"][0])
+    gb = np.delete(b["grad"][0], 1)
+    keep = [0] + list(range(3, 21))
+    assert np.allclose(a["grad"][0][keep], gb[keep], rtol=1e-9, atol=1e-7)
+
+
 def test_gradient_truncated_series_matches_its_own_finite_difference():
     """The epl_terms>0 (debug) mode differentiates the truncated sum term by term."""
     sp, psf, obs, sig, x0 = _tiny("epl_full", 1)

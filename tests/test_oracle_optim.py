@@ -153,6 +153,52 @@ def test_svi_non_finite_draws_are_left_out():
     assert N2 == 15 == N1 and np.isclose(l1, l2) and np.allclose(gm1, gm2) and np.allclose(gl1, gl2)
 
 
+@pytest.mark.parametrize("kind", [optim.ADAM, optim.ADABELIEF])
+def test_svi_inactive_dimensions_reduce_to_the_compact_problem(kind):
+    """Backward modelling: log p~ ignores the solved-amplitude entries of z, so the surrogate is
+    the normal of the sampled dimensions.  Three iterations with `active` on a 6-dimensional problem whose target ignores
+    dimensions 1 and 4 equal the same iterations of the UNMASKED (already pinned) routine on the 4-dimensional compact
+    problem: loss, mu, L and the optimiser state of the active block; the inactive entries never move; and the loss does
+    not drift (the un-masked 6-dimensional run is the failure this guards against: -log L_jj of a dead dimension falls
+    without bound)."""
+    n, N = 6, 48
+    act = np.array([True, False, True, True, False, True])
+    ia = np.flatnonzero(act)
+    mu4, Lp4, xi4, f4, a, A = _svi_setup(n=4, N=N, seed=5)
+
+    def f6(z):                                                   # the target sees the active coordinates only
+        lp, g = f4(z[:, ia])
+        g6 = np.zeros_like(z); g6[:, ia] = g
+        return lp, g6
+
+    rng = np.random.default_rng(9)
+    mu6 = rng.standard_normal(n); mu6[ia] = mu4
+    L6 = np.tril(0.1 * rng.standard_normal((n, n))) + np.diag(0.7 + rng.random(n))
+    L6[np.ix_(ia, ia)] = optim.tril_unpack(4, Lp4)
+    L6[np.ix_(ia, ~act)] = 0.0                                   # active rows do not mix in the dead momenta
+    Lp6 = optim.tril_pack(L6)
+    opt = dict(kind=kind, lr=5e-3, b1=0.9, b2=0.99, eps=1e-8, eps_root=1e-16)
+    m6 = np.zeros(n + 21); v6 = np.zeros(n + 21); m4 = np.zeros(4 + 10); v4 = np.zeros(4 + 10)
+    keep = np.concatenate([act, optim.tril_pack(act[:, None] & act[None, :]).astype(bool)])
+    mu6_0, Lp6_0 = mu6.copy(), Lp6.copy()
+    for t in (1, 2, 3):
+        xi6 = rng.standard_normal((N, n)); xi4 = xi6[:, ia]
+        l6, mu6, Lp6, m6, v6, _ = optim.svi_step(f6, mu6, Lp6, xi6, m6, v6, t, opt, active=act)
+        l4, mu4, Lp4, m4, v4, _ = optim.svi_step(f4, mu4, Lp4, xi4, m4, v4, t, opt)
+        assert np.isclose(l6, l4, rtol=1e-13)
+        assert np.allclose(mu6[ia], mu4, rtol=1e-13) and np.allclose(Lp6[keep[n:]], Lp4, rtol=1e-13, atol=1e-15)
+        assert np.allclose(m6[keep], m4, rtol=1e-12, atol=1e-18) and np.allclose(v6[keep], v4, rtol=1e-12, atol=1e-30)
+    dead = ~keep
+    assert np.array_equal(np.concatenate([mu6, Lp6])[dead], np.concatenate([mu6_0, Lp6_0])[dead])
+    assert np.all(m6[dead] == 0) and np.all(v6[dead] == 0)
+    # without the mask the dead diagonal entries grow at every step and take the loss down with them
+    muu, Lpu, mu_, vu = mu6_0.copy(), Lp6_0.copy(), np.zeros(n + 21), np.zeros(n + 21)
+    d0 = np.diag(optim.tril_unpack(n, Lpu))[~act].copy()
+    for t in (1, 2, 3):
+        _, muu, Lpu, mu_, vu, _ = optim.svi_step(f6, muu, Lpu, rng.standard_normal((N, n)), mu_, vu, t, opt)
+    assert np.all(np.diag(optim.tril_unpack(n, Lpu))[~act] > d0)
+
+
 # ------------------------------------------------------------------------------------------------ HMC (NEXT-3)
 def _gauss(a, A):
     def f(z):

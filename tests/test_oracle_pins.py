@@ -157,6 +157,39 @@ def test_circular_lens_ring_radius(gamma):
     assert abs(r - thE) <= 0.1 / 2 * 0.75
 
 
+@pytest.mark.parametrize("thE", [0.8, 1.3])
+@pytest.mark.parametrize("ell", [0.0, 1e-13])
+def test_sie_sis_branch_is_the_singular_isothermal_sphere(thE, ell):
+    """The q' < 1e-6 branch of sie_frame (the SIS limit of O4; SIE named at PAPER.md L50) with a NON-trivial theta_E:
+    |alpha| = theta_E on every ray and radial (closed form of the SIS); equal to the EPL series at t = 1; equal to the
+    limit of the q' >= 1e-6 closed form (|eps| = 1e-5: O(eps) away); its Jacobian and d/db against central
+    differences of the deflection itself (kappa = theta_E / 2r, pure tangential shear)."""
+    e1, e2, x0, y0 = ell * math.cos(0.4), ell * math.sin(0.4), 0.07, -0.04
+    th = [thE, e1, e2, x0, y0]
+    for (x, y) in ((0.9, 0.3), (-0.2, 1.7), (0.11, -0.05), (-2.4, -0.6)):
+        ax, ay = oracle.deflection(mass_spec(0), th, x, y)
+        r = math.hypot(x - x0, y - y0)
+        assert abs(math.hypot(ax, ay) - thE) < 1e-12
+        assert abs(ax - thE * (x - x0) / r) < 1e-12 and abs(ay - thE * (y - y0) / r) < 1e-12
+        bx, by = oracle.deflection(mass_spec(1), [thE, 2.0, e1, e2, x0, y0], x, y)
+        assert abs(ax - bx) < 1e-12 and abs(ay - by) < 1e-12            # |eps| = 1e-13 itself moves the EPL by O(1e-13)
+        cx, cy = oracle.deflection(mass_spec(0), [thE, 1e-5 * math.cos(0.4), 1e-5 * math.sin(0.4), x0, y0], x, y)
+        assert abs(ax - cx) < 1e-4 * thE and abs(ay - cy) < 1e-4 * thE
+    # frame-level outputs of the branch (b = theta_E at q = 1): alpha, d/db, Jacobian
+    c = ell; q = (1 - c) / (1 + c); b = thE * math.sqrt(q)
+    x, y, h = 0.6, -0.35, 1e-6
+    o = oracle.sie_frame(b, q, x, y)
+    assert math.sqrt(1 - q * q) < 1e-6                                   # this IS the SIS branch
+    al = lambda xx, yy, bb=b: oracle.sie_frame(bb, q, xx, yy)["alpha"]
+    assert abs(o["d_b"] - (al(x, y, b + h) - al(x, y, b - h)) / (2 * h)) < 1e-9
+    dax = (al(x + h, y) - al(x - h, y)) / (2 * h); day = (al(x, y + h) - al(x, y - h)) / (2 * h)
+    Jxx, Jyy, Jxy = o["J"]
+    assert abs(Jxx - dax.real) < 1e-8 and abs(Jyy - day.imag) < 1e-8
+    assert abs(Jxy - dax.imag) < 1e-8 and abs(Jxy - day.real) < 1e-8
+    assert abs(0.5 * (Jxx + Jyy) - thE / (2 * math.hypot(x, y))) < 1e-9  # kappa of the SIS
+    assert o["d_t"] == 0 and o["d_q"] == 0
+
+
 def test_ray_grid_convention():
     b4 = GOLD["B4"]
     sp = W.LensSpec(6, 2, 3, 0.30)
@@ -230,7 +263,6 @@ def test_sersic_total_flux_closed_form_and_half_light():
             inner = sum(integrate.dblquad(f, 0, 2 * math.pi, a, b, epsabs=1e-10, epsrel=1e-10)[0]
                         for a, b in ((0, 0.05), (0.05, Re)))
             assert abs(inner / closed - 0.5) < 3e-3                          # b_n approximation
-    assert abs(oracle.sersic([0.4, 2.5, 0.1, 0.05, 0, 0, 3.0], 0.4 * math.sqrt(1.0), 0.0) - 0) > 0
     # I = I_e on the ellipse r = R_e
     c = math.hypot(0.1, 0.05); q = (1 - c) / (1 + c); phi = 0.5 * math.atan2(0.05, 0.1)
     xr = 0.4 / math.sqrt(q)
@@ -347,7 +379,7 @@ def test_golden_b4_end_to_end():
     o = oracle.logpost_grad(sp, np.zeros((1, 6, 6)), np.full((1, 6, 6), 0.1), psf, [b4["theta"]], want_model=True)
     m = o["model"][0]
     assert abs(m.sum() - b4["sum_model"]) < 1e-10
-    assert abs((m / 0.1) ** 2).sum() - b4["chi2"] < 1e-8
+    assert abs(((m / 0.1) ** 2).sum() - b4["chi2"]) < 1e-8
     assert abs(o["logp"][0] - b4["logL"]) < 1e-9
     for (i, j) in ((0, 0), (2, 3), (3, 4), (5, 5)):
         assert abs(m[i, j] - b4["model_%d_%d" % (i, j)]) < 1e-11
