@@ -3,8 +3,11 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config k] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (unpack/prior, ray-trace, paint, PSF+bin, chi^2,
-adjoint) over one batch of synthetic particles: one gl_logpost_grad call on the full batch of the chosen config
-(default config 2 = BASELINE.json configs[1], the DESI-Legacy-like multi-start MAP batch of 4096 particles).
+adjoint) over one batch of synthetic particles: one gl_logpost_grad call on the full batch of the chosen config.
+BASELINE.json's `metric` names no config, so the default is the LARGEST single-GPU configuration, config 5
+(configs[4]: 200x200 pixels, supersample 4 = 640,000 rays, 41x41 PSF, EPL + shear + multipoles, Sersic + shapelets
+n_max 10, two lens Sersics, 100 parameters, 2048 particles); the default run also times configs 2-4 in fp64 and
+config 5 in fp32 for a few steps each and reports them in `all_configs` / `f32` (compact records, same process).
 `value` times that call with the particles already resident in HBM; `e2e` times gl_logpost_grad_host, i.e. the
 same work plus the host->device copy of the particles from pinned memory and the device->host copy of logp and
 the gradient, every step.  N > 1 runs N replicas (the path does not shard further: SURVEY 8(e)), one process per
@@ -51,7 +54,9 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--no-all-configs", action="store_true",
+                    help="skip the short runs of the other configs and of the fp32 mode (all_configs / f32 records)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
                     help="arithmetic of the CUDA path: f64 = GL_PRECISION_F64 (default; strict parity), f32 = GL_PRECISION_F32")
@@ -65,10 +70,16 @@ def parse():
     return ap.parse_args()
 
 
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel at the default
-# workload, from the committed `ncu --set full` capture profiles/r1c_cfg2_f64.md (bench.py cannot run a profiler):
-# keyed by (config, precision, stage).  None elsewhere.
-NCU_TRAFFIC_BYTES = {(2, "f64", "ray_adjoint"): 2.153155e9 + 0.035220e9}
+def ncu_traffic(k, precision, stage):
+    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the kernel of `stage`, from the committed
+    `ncu --set full` captures: profiles/ncu_traffic.json, written by `python -m paper_2606_30633_b200.ncu_traffic` from the
+    raw-page CSV exports (bench.py cannot run a profiler).  None where no capture exists."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            tab = json.load(f)
+        return tab["cfg%d_%s" % (k, precision)][stage]["dram_bytes_per_launch"]
+    except Exception:
+        return None
 
 
 # ----------------------------------------------------------------------------------------------- clocks
@@ -199,6 +210,142 @@ def whole_job_rate(world, particles_per_rank, steps, seconds):
     return world * particles_per_rank * steps / seconds
 
 
+
+
+# ----------------------------------------------------------------------------------------------- GPU arm: helpers
+def _peak(precision, mhz):
+    lanes = FP64_LANES if precision == "f64" else FP32_LANES
+    return N_SM * lanes * mhz * 1e6 / 1e12, lanes                     # T lane-op/s
+
+
+def make_model(gl, W, torch, k, precision, dev, amplitudes="sampled"):
+    """Workload k on the device: (wl, spec, LensModel).  The observation is the truth rendered by THIS side
+    (gl_model_image) + the seeded noise (workloads docstring)."""
+    wl = W.make_workload(k)
+    sp = wl.spec
+    sp.precision = 0 if precision == "f64" else 1
+    N = sp.n_pix
+    zeros = np.zeros((sp.n_systems, N, N), np.float32)
+    m0 = gl.LensModel(sp, zeros, zeros + 1, wl.psf, device=dev)
+    sid_sys = np.arange(sp.n_systems, dtype=np.int32) if sp.n_systems > 1 else None
+    truth = m0.model_image(torch.from_numpy(wl.truth_z).to(dev), sid_sys).cpu().numpy()
+    m0.close()
+    obs, sig = W.finish_observation(wl, truth)
+    if amplitudes == "solved":
+        sp.amplitude_mode = 1
+    return wl, sp, gl.LensModel(sp, obs, sig, wl.psf, device=dev)
+
+
+def band_means(gl, torch, m, ws, P):
+    """(mean M1, mean M2, particles read) of the series precision bands step A chose (csrc/gl_ray.cuh knuth_banded), over
+    the valid particles of the LAST chunk of the most recent call, read from the workspace (gl_workspace_layout)."""
+    if m.spec.mass_model != 1:
+        return None
+    lay = gl.gl_workspace_layout(m.h, P)
+    n = min(lay["chunk"], P - lay["last_chunk_first"])
+    dt = torch.float64 if lay["elem_bytes"] == 8 else torch.float32
+    nb = n * lay["pb_stride"] * lay["elem_bytes"]
+    pb = ws[lay["off_pb"]:lay["off_pb"] + nb].view(dt).view(n, lay["pb_stride"])
+    ok = pb[:, lay["idx_valid"]] != 0
+    if int(ok.sum()) == 0:
+        return None
+    return float(pb[ok, lay["idx_m1"]].double().mean()), float(pb[ok, lay["idx_m2"]].double().mean()), int(ok.sum())
+
+
+def stage_profile(gl, step, flush, reps):
+    """Per-stage device time of one step from the library's own CUDA events on the launching stream (mean over reps)."""
+    gl.gl_stage_timing_enable(True)
+    stage_ms, stage_n = {}, {}
+    for _ in range(reps):
+        flush.zero_()
+        step()
+        for name, (ms, cnt) in gl.gl_stage_times().items():
+            stage_ms[name] = stage_ms.get(name, 0.0) + ms / reps
+            stage_n[name] = cnt
+    gl.gl_stage_timing_enable(False)
+    return stage_ms, stage_n
+
+
+def roofline_record(workmodel, sp, k, precision, P, evals_per_particle, stage_ms, stage_n, ms_per_step, bands, mhz_max,
+                    peak_src, sm_mhz=None):
+    """The `roofline` object of the contract for the dominant kernel of a measured step.
+    frac          executed-band work: only the series steps that run in the arithmetic type are credited (bands)
+    frac_fixed30  the fixed 30-term formulation (every term credited to the arithmetic type's pipe): the round-1 figure
+    fp32_cofrac   fp64 mode: the series steps run in fp32, as a fraction of the FP32 pipe's peak (same kernel, same time)
+    step_frac     one forward + one reverse sweep credited over the whole step (executed-band), step_frac_fixed30 likewise"""
+    peak, lanes = _peak(precision, mhz_max)
+    pipe = "FP64" if precision == "f64" else "FP32"
+    wm30 = workmodel.per_eval(sp, precision)
+    wmb = workmodel.per_eval(sp, precision, bands[:2]) if bands else wm30
+    dom = max(stage_ms, key=stage_ms.get)
+    dom_t = stage_ms[dom] * 1e-3
+    rate = lambda ops: ops * P * evals_per_particle / dom_t / 1e12 if dom_t > 0 else 0.0
+    achieved = rate(wmb.get(dom, 0))
+    t_step = ms_per_step * 1e-3
+    r = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "T %s lane-op/s (FMA=1)" % pipe,
+         "frac": achieved / peak, "frac_fixed30": rate(wm30.get(dom, 0)) / peak,
+         "traffic": ncu_traffic(k, precision, dom),
+         "peak_source": "148 SM x %d %s lanes x %g MHz (%s)" % (lanes, pipe, mhz_max, peak_src),
+         "kernel_ms_per_launch": stage_ms[dom] / max(stage_n[dom], 1), "kernel_launches_per_step": stage_n[dom],
+         "algorithmic_laneops_per_eval": wmb.get(dom, 0), "algorithmic_laneops_per_eval_fixed30": wm30.get(dom, 0),
+         "series_bands": ({"mean_m1": round(bands[0], 3), "mean_m2": round(bands[1], 3), "particles": bands[2],
+                           "meaning": "4*m1 recurrence steps in %s, 4*m2 in fp32, rest skipped (of 28)" % pipe.lower()}
+                          if bands else None),
+         "stage_ms": {s: round(v, 4) for s, v in stage_ms.items()},
+         "stage_share": {s: round(v / max(sum(stage_ms.values()), 1e-12), 4) for s, v in stage_ms.items()},
+         "step_frac": wmb["total_fwd_grad"] * P * evals_per_particle / t_step / 1e12 / peak,
+         "step_frac_fixed30": wm30["total_fwd_grad"] * P * evals_per_particle / t_step / 1e12 / peak,
+         "step_algorithmic_laneops_per_eval": wmb["total_fwd_grad"],
+         "per_stage_frac": {s: round(wmb[s] * P * evals_per_particle / (stage_ms[s] * 1e-3) / 1e12 / peak, 4)
+                            for s in ("ray_fwd", "conv_chi2", "conv_transpose", "ray_adjoint")
+                            if s in wmb and stage_ms.get(s, 0) > 0}}
+    if precision == "f64":
+        p32, _ = _peak("f32", mhz_max)
+        r["fp32_cofrac"] = rate(wmb.get(dom + "_fp32band", 0)) / p32
+        r["step_frac_of_fp32_peak"] = r["step_frac"] * peak / p32     # the pipe BASELINE.json's metric names
+    else:
+        r["mufu_T_ops_per_s"] = wmb["total_fwd_grad_mufu"] * P * evals_per_particle / t_step / 1e12
+    if sm_mhz:
+        r["frac_at_measured_clock"] = achieved / _peak(precision, sm_mhz)[0]
+    return r
+
+
+def short_run(gl, W, torch, workmodel, k, precision, dev, flush, steps, warmup, mhz_max, peak_src):
+    """A compact record of config k in `precision`: a few gl_logpost_grad steps on the full batch, CUDA events."""
+    wl, sp, m = make_model(gl, W, torch, k, precision, dev)
+    P, n_p = wl.params.shape[0], sp.n_params
+    z = torch.from_numpy(wl.params).to(dev)
+    sid = torch.from_numpy(wl.system_id).to(dev) if wl.system_id is not None else None
+    lp = torch.empty(P, dtype=torch.float32, device=dev); g = torch.empty((P, n_p), dtype=torch.float32, device=dev)
+    ws = m.workspace(P)
+    step = lambda: gl.gl_logpost_grad(m.h, m.obs, m.noise_sigma, m.psf, z, sid, lp, g, ws)
+    for _ in range(max(warmup, 3)):
+        step()
+    launches = int(gl.gl_last_launch_count())
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for e0, e1 in ev:
+        flush.zero_()
+        e0.record(); step(); e1.record()
+    torch.cuda.synchronize()
+    ms = sum(e0.elapsed_time(e1) for e0, e1 in ev) / steps
+    bands = band_means(gl, torch, m, ws, P)
+    stage_ms, stage_n = stage_profile(gl, step, flush, min(steps, 3))
+    roof = roofline_record(workmodel, sp, k, precision, P, 1, stage_ms, stage_n, ms, bands, mhz_max, peak_src)
+    rec = {"cfg": k, "workload": WORKLOAD_NAMES[k], "dtype": precision, "value": P / (ms * 1e-3), "unit": UNIT,
+           "ms_per_step": ms, "steps": steps, "n_particles": P, "gpu_launches_per_step": launches,
+           "finite_fraction": float(torch.isfinite(lp).float().mean()),
+           "kernel": roof["kernel"], "frac": roof["frac"], "frac_fixed30": roof["frac_fixed30"],
+           "step_frac": roof["step_frac"], "step_frac_fixed30": roof["step_frac_fixed30"],
+           "per_stage_frac": roof["per_stage_frac"], "stage_ms": roof["stage_ms"], "traffic": roof["traffic"]}
+    for key in ("fp32_cofrac", "step_frac_of_fp32_peak", "mufu_T_ops_per_s", "series_bands"):
+        if key in roof:
+            rec[key] = roof[key]
+    m.close()
+    del ws, z, lp, g, m
+    torch.cuda.empty_cache()
+    return rec
+
+
 # ----------------------------------------------------------------------------------------------- GPU arm
 def run_ours(a):
     import torch
@@ -224,21 +371,10 @@ def run_ours(a):
         torch.cuda.synchronize()
 
     k = a.config
-    wl = W.make_workload(k)
-    sp = wl.spec
-    sp.precision = 0 if a.precision == "f64" else 1
-    P, n_p, N = wl.params.shape[0], sp.n_params, sp.n_pix
-    # observation: truth rendered by THIS side (gl_model_image), noise from the seeded stream (workloads docstring)
-    zeros = np.zeros((sp.n_systems, N, N), np.float32)
-    m0 = gl.LensModel(sp, zeros, zeros + 1, wl.psf, device=dev)
-    sid_sys = np.arange(sp.n_systems, dtype=np.int32) if sp.n_systems > 1 else None
-    truth = m0.model_image(torch.from_numpy(wl.truth_z).to(dev), sid_sys).cpu().numpy()
-    m0.close()
-    obs, sig = W.finish_observation(wl, truth)
     if a.amplitudes == "solved":
-        sp.amplitude_mode = 1
         a.no_cpu_baseline = True
-    m = gl.LensModel(sp, obs, sig, wl.psf, device=dev)
+    wl, sp, m = make_model(gl, W, torch, k, a.precision, dev, a.amplitudes)
+    P, n_p = wl.params.shape[0], sp.n_params
     z = torch.from_numpy(wl.params).to(dev)
     sid = torch.from_numpy(wl.system_id).to(dev) if wl.system_id is not None else None
     lp = torch.empty(P, dtype=torch.float32, device=dev)
@@ -360,16 +496,8 @@ def run_ours(a):
     finite = float(torch.isfinite(lp).float().mean())
 
     # dominant-kernel roofline: per-stage device time from the library's own CUDA events on the launching stream
-    gl.gl_stage_timing_enable(True)
-    stage_ms, stage_n = {}, {}
-    reps = max(3, min(a.steps, 10))
-    for _ in range(reps):
-        flush.zero_()
-        step()
-        for name, (ms, cnt) in gl.gl_stage_times().items():
-            stage_ms[name] = stage_ms.get(name, 0.0) + ms / reps
-            stage_n[name] = cnt
-    gl.gl_stage_timing_enable(False)
+    bands = band_means(gl, torch, m, ws, P) if a.stage in ("grad", "map") else None
+    stage_ms, stage_n = stage_profile(gl, step, flush, max(3, min(a.steps, 10)))
 
     t_dev, t_e2e = max_over_ranks([t_dev, t_e2e], dev)
     if rank != 0:
@@ -378,33 +506,18 @@ def run_ours(a):
         return
 
     mhz_max, peak_src = _peaks()
-    lanes = FP64_LANES if a.precision == "f64" else FP32_LANES
-    pipe = "FP64" if a.precision == "f64" else "FP32"
-    peak = N_SM * lanes * mhz_max * 1e6 / 1e12                        # T lane-op/s
-    wm = workmodel.per_eval(sp, a.precision)
+    clocks = sampler.summary()
+    roof = roofline_record(workmodel, sp, k, a.precision, P, evals_per_particle, stage_ms, stage_n, t_dev / a.steps * 1e3, bands,
+                           mhz_max, peak_src, clocks.get("sm_mhz"))
     probe = {}
-    for kind, name in ((0, "fp32_fma"), (1, "fp64_fma"), (2, "mufu_ex2"), (4, "fp64_fma_distinct_operands")):
+    for kind, name in ((0, "fp32_fma"), (1, "fp64_fma"), (2, "mufu_ex2"), (4, "fp64_fma_distinct_operands"),
+                       (5, "fp64_mma_m8n8k4"), (6, "fp64_mma_plus_fma")):
         try:
             probe[name] = round(gl.gl_probe_pipe(kind, 256)[0], 3)
-        except Exception as e:                                        # measurement utility only
+        except Exception:                                             # measurement utility only
             probe[name] = None
-    dom = max(stage_ms, key=stage_ms.get)
-    dom_ops = wm.get(dom, 0) * P
-    dom_t = stage_ms[dom] * 1e-3
-    achieved = dom_ops / dom_t / 1e12 if dom_t > 0 else 0.0
-    clocks = sampler.summary()
-    roof = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "T %s lane-op/s (FMA=1)" % pipe,
-            "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((k, a.precision, dom)),
-            "peak_source": "148 SM x %d %s lanes x %g MHz (%s)" % (lanes, pipe, mhz_max, peak_src),
-            "probe_T_laneops_per_s": probe,
-            "kernel_ms_per_launch": stage_ms[dom] / max(stage_n[dom], 1), "kernel_launches_per_step": stage_n[dom],
-            "algorithmic_laneops_per_eval": wm.get(dom, 0),
-            "stage_ms": {s: round(v, 4) for s, v in stage_ms.items()},
-            "stage_share": {s: round(v / max(sum(stage_ms.values()), 1e-12), 4) for s, v in stage_ms.items()},
-            "step_frac": wm["total_fwd_grad"] * P * evals_per_particle * a.steps / t_dev / 1e12 / peak,
-            "step_algorithmic_laneops_per_eval": wm["total_fwd_grad"]}
-    if clocks.get("sm_mhz"):
-        roof["frac_at_measured_clock"] = achieved / (N_SM * lanes * clocks["sm_mhz"] * 1e6 / 1e12)
+    roof["probe_T_laneops_per_s"] = probe
+    wm = workmodel.per_eval(sp, a.precision)
     out = {"metric": METRIC, "value": whole_job_rate(world, P * evals_per_particle, a.steps, t_dev), "unit": UNIT, "n_gpus": world, "steps": a.steps,
            "warmup": max(a.warmup, 3), "ms_per_step": t_dev / a.steps * 1e3, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": a.precision, "data": "synthetic",
@@ -415,6 +528,24 @@ def run_ours(a):
            "e2e": {"value": whole_job_rate(world, P * evals_per_particle, a.steps, t_e2e), "unit": UNIT, "h2d_bytes_per_step": int(h2d_bytes),
                    "d2h_bytes_per_step": int(d2h_bytes), "ms_per_step": t_e2e / a.steps * 1e3},
            "gpu_launches": launches_per_step * a.steps, "clocks": clocks, "roofline": roof}
+    if a.stage == "grad" and a.amplitudes == "sampled" and world == 1 and not a.no_all_configs:
+        # free this config's buffers, then a few steps of every other BASELINE.json config (fp64) and of this one in fp32
+        m.close()
+        m._ws = None
+        del ws
+        torch.cuda.empty_cache()
+        short = max(3, min(a.steps, 5))
+        recs = [{"cfg": k, "workload": WORKLOAD_NAMES[k], "dtype": a.precision, "value": out["value"], "unit": UNIT,
+                 "ms_per_step": out["ms_per_step"], "steps": a.steps, "n_particles": P, "kernel": roof["kernel"],
+                 "frac": roof["frac"], "frac_fixed30": roof["frac_fixed30"], "step_frac": roof["step_frac"],
+                 "step_frac_fixed30": roof["step_frac_fixed30"], "per_stage_frac": roof["per_stage_frac"],
+                 "stage_ms": roof["stage_ms"], "traffic": roof["traffic"]}]
+        for kk in (2, 3, 4, 5):
+            if kk != k:
+                recs.append(short_run(gl, W, torch, workmodel, kk, a.precision, dev, flush, short, 3, mhz_max, peak_src))
+        out["all_configs"] = sorted(recs, key=lambda r: r["cfg"])
+        other = "f32" if a.precision == "f64" else "f64"
+        out[other] = short_run(gl, W, torch, workmodel, k, other, dev, flush, short, 3, mhz_max, peak_src)
     if not a.no_cpu_baseline:
         rate, cores, sample, _ = oracle_rate(k, a.cpu_seconds)
         out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}

@@ -294,11 +294,21 @@ int32_t     gl_stage_count(void);
 const char* gl_stage_name(int32_t i);
 int32_t     gl_stage_times(float* ms_host, int32_t* launches_host, int32_t n);
 
+/* Diagnostic layout of the workspace (for bench.py's work model; no CUDA call): HOST pointer out[8] =
+ * { byte offset of the per-particle block array PB, particles per chunk Pc, elements per PB row, bytes per element
+ *   (8 in GL_PRECISION_F64, 4 in _F32), row index of the series band count M1 (4 M1 recurrence steps in the arithmetic
+ *   type), of M2 (4 M2 steps in fp32 above them, fp64 mode only; terms beyond are numerically zero and skipped), of the
+ *   validity flag, index of the first particle of the last chunk }.  After a compute call the PB rows of the LAST chunk
+ *   are at workspace + out[0].  Errors: GL_ERR_NULL, GL_ERR_BAD_SHAPE (n_particles <= 0). */
+gl_status gl_workspace_layout(const gl_config* cfg, int64_t n_particles, int64_t* out);
+
 /* Measurement utility (NOT part of the hot path; the only call that synchronises): issue-rate probe of one SM
  * pipe, so that bench.py can state a MEASURED ALU peak beside the one derived from unit counts and clocks
  * (BASELINE.json north_star: "achieved fraction of the binding roofline"; MEASURED_PEAKS.json has no FP32, FP64
  * or MUFU figure).  kind 0: FP32 FMA, 1: FP64 FMA, 2: MUFU ex2, 3: FP32 and FP64 FMA interleaved 1:1 (both
- * counted), 4: FP64 FMA with three distinct register operands per chain (kinds 0-3 share multiplier and addend).  Launches 8 CTAs of 256 threads per SM, each thread running 8 independent chains of
+ * counted), 4: FP64 FMA with three distinct register operands per chain (kinds 0-3 share multiplier and addend),
+ * 5: FP64 tensor-core MMA (mma.sync.m8n8k4.f64; one warp instruction = 8 lane-operations per lane), 6: kind 5 and kind 1
+ * interleaved 1:1 (both counted: do the FP64 tensor and vector paths add up?).  Launches 8 CTAs of 256 threads per SM, each thread running 8 independent chains of
  * n_outer * 64 operations, once untimed and once between two CUDA events on `stream`, waits for it, and writes
  * 1e-12 * lane-operations per second (an FMA counts once) to *tera_lane_ops_per_s_host and the kernel time to
  * *ms_host (HOST pointers; ms_host may be NULL).  workspace: DEVICE pointer, >= 256 bytes (never written in

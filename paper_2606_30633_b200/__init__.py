@@ -24,7 +24,7 @@ EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_wo
            "gl_stage_name", "gl_stage_times", "gl_probe_pipe", "gl_map_step",
            "gl_svi_workspace_bytes", "gl_svi_step", "gl_hmc_workspace_bytes", "gl_hmc_step",
            "gl_best_particle", "gl_config_n_amplitudes", "gl_linear_amplitudes", "gl_draw_normal", "gl_draw_log_uniform",
-           "gl_config_shape"]
+           "gl_config_shape", "gl_workspace_layout"]
 
 
 class GLError(RuntimeError):
@@ -76,6 +76,8 @@ def lib():
         L.gl_config_shape.argtypes = [vp, C.POINTER(C.c_int32)]
         L.gl_workspace_bytes.restype = sz
         L.gl_workspace_bytes.argtypes = [vp, i64]
+        L.gl_workspace_layout.restype = C.c_int
+        L.gl_workspace_layout.argtypes = [vp, i64, C.POINTER(i64)]
         L.gl_workspace_bytes_host.restype = sz
         L.gl_workspace_bytes_host.argtypes = [vp, i64]
         L.gl_logpost.restype = C.c_int
@@ -155,6 +157,14 @@ def gl_workspace_bytes(h, n):
     return lib().gl_workspace_bytes(h, int(n))
 
 
+def gl_workspace_layout(h, n):
+    """dict(off_pb, chunk, pb_stride, elem_bytes, idx_m1, idx_m2, idx_valid, last_chunk_first) -- include/gigalens.h."""
+    out = (C.c_int64 * 8)()
+    _check(lib().gl_workspace_layout(h, int(n), out), "gl_workspace_layout")
+    return dict(zip(("off_pb", "chunk", "pb_stride", "elem_bytes", "idx_m1", "idx_m2", "idx_valid", "last_chunk_first"),
+                    (int(x) for x in out)))
+
+
 def gl_workspace_bytes_host(h, n):
     return lib().gl_workspace_bytes_host(h, int(n))
 
@@ -178,7 +188,8 @@ def gl_stage_times():
 
 
 def gl_probe_pipe(kind, n_outer=2048, stream=None):
-    """(tera lane-ops/s, kernel ms) of one SM pipe: kind 0 FP32 FMA, 1 FP64 FMA, 2 MUFU ex2, 3 FP32+FP64 interleaved."""
+    """(tera lane-ops/s, kernel ms) of one SM pipe: kind 0 FP32 FMA, 1 FP64 FMA, 2 MUFU ex2, 3 FP32+FP64 interleaved,
+    4 FP64 FMA with distinct operands, 5 FP64 tensor MMA (m8n8k4), 6 FP64 MMA + FMA interleaved."""
     torch = _torch()
     ws = torch.zeros(256, dtype=torch.uint8, device="cuda")
     rate = C.c_double(); ms = C.c_float()

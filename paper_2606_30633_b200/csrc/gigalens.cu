@@ -301,6 +301,17 @@ extern "C" size_t gl_workspace_bytes(const gl_config* c, int64_t n_particles) {
     return make_plan(c, n_particles).total;
 }
 
+// Diagnostic: where the per-particle block PB of the LAST processed chunk sits in the workspace, so that bench.py can
+// read what step A decided per particle (the precision bands of the series) without a kernel of its own.
+extern "C" gl_status gl_workspace_layout(const gl_config* c, int64_t n_particles, int64_t* out) {
+    if (!c || !out) return GL_ERR_NULL;
+    if (n_particles <= 0) return GL_ERR_BAD_SHAPE;
+    const Plan pl = make_plan(c, n_particles);
+    out[0] = (int64_t)pl.off_pb; out[1] = pl.Pc; out[2] = PB_STRIDE; out[3] = c->esize;
+    out[4] = PB_SER_M1; out[5] = PB_SER_M2; out[6] = PB_VALID; out[7] = (n_particles - 1) / pl.Pc * pl.Pc;   // first particle of the last chunk
+    return GL_OK;
+}
+
 // ----------------------------------------------------------------------------- variant dispatch
 template <class T, class V>
 static void launch_ray_fwd(const gl_config* c, const T* pb, const double* tab, T* ray, int64_t Pc, cudaStream_t st) {
@@ -763,7 +774,7 @@ extern "C" gl_status gl_logpost_grad_host(const gl_config* c, const float* obs, 
 extern "C" gl_status gl_probe_pipe(int32_t kind, int32_t n_outer, void* workspace, size_t workspace_bytes, void* stream,
                                    double* tera_lane_ops_per_s_host, float* ms_host) {
     if (!workspace || !tera_lane_ops_per_s_host) return GL_ERR_NULL;
-    if (kind < 0 || kind > 4 || n_outer < 1) return GL_ERR_BAD_SHAPE;
+    if (kind < 0 || kind > 6 || n_outer < 1) return GL_ERR_BAD_SHAPE;
     if (workspace_bytes < 256) return GL_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, n_sm = 0;
@@ -779,7 +790,9 @@ extern "C" gl_status gl_probe_pipe(int32_t kind, int32_t n_outer, void* workspac
             case 1: gl_probe_kernel<1><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
             case 2: gl_probe_kernel<2><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
             case 3: gl_probe_kernel<3><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
-            default: gl_probe_kernel<4><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+            case 4: gl_probe_kernel<4><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+            case 5: gl_probe_kernel<5><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+            default: gl_probe_kernel<6><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
         }
     };
     launch(n_outer);                                   // warm-up
@@ -791,7 +804,8 @@ extern "C" gl_status gl_probe_pipe(int32_t kind, int32_t n_outer, void* workspac
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     if (e != cudaSuccess || !(ms > 0.f)) return GL_ERR_CUDA;
-    const double ops = (double)ctas * nt * (double)n_outer * PROBE_INNER * PROBE_CHAINS * (kind == 3 ? 2.0 : 1.0);
+    const double per = kind == 3 ? 2.0 : kind == 5 ? 8.0 : kind == 6 ? 9.0 : 1.0;    // lane-operations per chain step
+    const double ops = (double)ctas * nt * (double)n_outer * PROBE_INNER * PROBE_CHAINS * per;
     *tera_lane_ops_per_s_host = ops / (ms * 1e-3) * 1e-12;
     if (ms_host) *ms_host = ms;
     return GL_OK;

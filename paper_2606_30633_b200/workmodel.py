@@ -1,11 +1,20 @@
 """Frozen algorithmic work model of the hot path (SURVEY 8(d) "Algorithmic work per evaluation").
 
-Counts are FP32 lane-operations with an FMA counted ONCE (add, mul and fma each count 1; min/max, selects,
-integer and address arithmetic count 0) and MUFU operations separately, per ray, for the formulation the
-kernels implement (csrc/gl_ray.cuh): the EPL series as a real-coefficient polynomial in w evaluated by
-synthetic division (2 FMA per term, not the 6 of complex Horner that SURVEY 8(d) assumed), Sersic via
-lg2/ex2, shapelets by the three-term recurrence.  They are hand counts of the formulas, frozen before timing;
-recomputation of the forward inside the adjoint kernel is NOT credited (one forward sweep + one reverse sweep).
+Counts are lane-operations with an FMA counted ONCE (add, mul and fma each count 1; min/max, selects, integer and
+address arithmetic count 0) and MUFU operations separately, per ray, for the formulation the kernels implement
+(csrc/gl_ray.cuh): the EPL series as a real-coefficient polynomial in w evaluated by synthetic division (2 FMA per
+term, not the 6 of complex Horner that SURVEY 8(d) assumed), Sersic via lg2/ex2, shapelets by the three-term
+recurrence.  They are hand counts of the formulas, frozen before timing.
+
+Two things a reader must not confuse (round-1 review):
+  * "ray_adjoint" is what the adjoint KERNEL must do: it recomputes steps B + C per ray (nothing is taped), so its
+    count is forward + reverse sweep; the whole-step figure "total_fwd_grad" credits ONE forward and ONE reverse sweep
+    (the recompute is not credited twice).
+  * the series count comes in two forms.  `bands=None`: the fixed 30-term formulation, every term in the arithmetic
+    type (the `frac_fixed30` of bench.py).  `bands=(m1, m2)` (batch means of what step A chose per particle, read back
+    from the workspace): only the 4 m1 recurrence steps that DO run in the arithmetic type are credited to its pipe;
+    the 4 m2 steps that the fp64 mode runs in fp32 on the FP32 pipe are returned separately ("*_fp32band") and the
+    terms beyond 4 (m1 + m2) + 1, which are numerically zero and skipped, are credited to nobody.
 This module holds no arithmetic of the method; bench.py uses it to turn a measured time into a roofline fraction.
 """
 
@@ -70,9 +79,22 @@ def shapelet_adj(nmax):
     return 4 * (nmax + 1) + 2 * ncoef + 2 * (nmax + 1) + ncoef     # derivatives, d/du d/dv contractions, coefficient sums
 
 
-def per_ray(spec, precision="f32"):
-    """(fwd lane-ops, fwd mufu, adjoint-sweep lane-ops, adjoint-sweep mufu) per ray for a LensSpec-like object;
-    precision "f32": FP32 lane-ops + MUFU, "f64": FP64 lane-ops (mufu = 0)."""
+# EPL series by band (csrc/gl_ray.cuh knuth_banded): one polynomial = 4 m recurrence steps of 2 FMA + a tail of 7 (fwd:
+# 3 + the rotation E * P(w) 4); the reverse sweep adds two more polynomials (2 x 8 m) + 18 of tails and rotations.  The
+# fixed 30-term figures above are m = 7: 8 * 7 + 7 = 63 and 2 * 56 + 18 = 130 (134 in fp32: 4 more in the rotations).
+SERIES_M_FULL = 7
+
+
+def series_ops(m, precision):
+    """(forward, reverse-sweep extra) lane-ops of the series with 4 m recurrence steps per polynomial."""
+    tail_adj = 18 if precision == "f64" else 22
+    return 8.0 * m + 7.0, 16.0 * m + tail_adj
+
+
+def per_ray(spec, precision="f32", bands=None):
+    """(fwd lane-ops, fwd mufu, adjoint-sweep lane-ops, adjoint-sweep mufu, fwd fp32-band ops, adjoint fp32-band ops)
+    per ray for a LensSpec-like object; precision "f32": FP32 lane-ops + MUFU, "f64": FP64 lane-ops (mufu = 0).
+    bands = (mean m1, mean m2) or None for the fixed 30-term count (module docstring)."""
     f = m = a = am = 0
     F_, A_ = (FWD64, ADJ64) if precision == "f64" else (FWD, ADJ)
 
@@ -97,16 +119,27 @@ def per_ray(spec, precision="f32"):
     if spec.shapelet_nmax >= 0:
         add(FWD, "shapelet_fixed"); add(ADJ, "shapelet_fixed")
         f += shapelet_fwd(spec.shapelet_nmax); a += shapelet_adj(spec.shapelet_nmax)
-    return f, m, a, am
+    f32f = f32a = 0.0
+    if bands is not None and spec.mass_model == 1:
+        m1, m2 = bands
+        full_f, full_a = series_ops(SERIES_M_FULL, precision)
+        got_f, got_a = series_ops(m1, precision)
+        f += got_f - full_f; a += got_a - full_a
+        if precision == "f64":
+            f32f, f32a = 8.0 * m2, 16.0 * m2
+    return f, m, a, am, f32f, f32a
 
 
-def per_eval(spec, precision="f32"):
-    """Algorithmic lane-ops (FP32 or FP64, by `precision`) of one particle evaluation, by stage, for gl_logpost_grad."""
+def per_eval(spec, precision="f32", bands=None):
+    """Algorithmic lane-ops (FP32 or FP64, by `precision`) of one particle evaluation, by stage, for gl_logpost_grad.
+    bands: see per_ray."""
     M = spec.n_pix * spec.supersample
     rays = M * M
-    f, m, a, am = per_ray(spec, precision)
+    f, m, a, am, f32f, f32a = per_ray(spec, precision, bands)
     ke = spec.psf_size + spec.supersample - 1
     conv = spec.n_pix * spec.n_pix * ke * ke              # stride-s correlation with the pre-boxed kernel (step D)
+    if getattr(spec, "psf_grid", 0) == 1:                 # bin (s^2 adds per pixel), then K x K taps at the pixel scale
+        conv = spec.n_pix * spec.n_pix * (spec.psf_size ** 2 + spec.supersample ** 2)
     return {
         "rays": rays,
         "ray_fwd": f * rays, "ray_fwd_mufu": m * rays,
@@ -117,4 +150,7 @@ def per_eval(spec, precision="f32"):
         "total_fwd": f * rays + conv,
         "total_fwd_grad": (f + a) * rays + 2 * conv,       # one forward + one reverse sweep; recompute not credited
         "total_fwd_grad_mufu": (m + am) * rays,
+        # fp64 mode only: series steps that run in fp32 on the FP32 pipe (not part of the figures above)
+        "ray_fwd_fp32band": f32f * rays, "ray_adjoint_fp32band": (f32f + f32a) * rays,
+        "total_fwd_grad_fp32band": (f32f + f32a) * rays,
     }
