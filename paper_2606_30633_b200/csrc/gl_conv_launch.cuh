@@ -2,8 +2,10 @@
 // input-stationary sliding kernels for the tap counts of the BASELINE.json configs (U = 6, 11, 16 with s*s a
 // multiple of 4), generic kernels for every other shape.
 #pragma once
+#include <cstdlib>
 #include "gl_common.cuh"
 #include "gl_conv.cuh"
+#include "gl_conv_ts.cuh"
 
 namespace gl {
 
@@ -11,15 +13,88 @@ namespace gl {
 #define GL_CONV_CTA 128
 #endif
 
+static inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
 struct ConvPlan {
-    int kind;                 // 0 generic, 1: U=6 CW=4, 2: U=11 CW=2, 3: U=16 CW=2
+    int kind;                 // 0 generic, 1: U=6 CW=4, 2: U=11 CW=2, 3: U=16 CW=2 (round-1 sliding kernels), 4: tap-stationary + TMA
     int CW;                   // output columns per thread
     SlidePlan fwd, bwd;
     size_t fwd_smem, bwd_smem;
     int n_ctile;              // chi^2 partials per particle
+    int ts_id;                // kind 4: which (U, G, NPH, CW) instance (ts_variant)
+    TsPlan tf, tb;            // kind 4: forward / transpose launch plans
 };
 
-static inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+// The compiled tap-stationary instances: id -> (U, G, NPH, CW).  G tap-row groups x NPH planes = lanes per column group.
+#ifndef GL_TS_CW11
+#define GL_TS_CW11 4
+#endif
+#ifndef GL_TS_CW16
+#define GL_TS_CW16 4
+#endif
+struct TsVariant { int U, G, NPH, CW, RPS, wmax_f, wmax_b, maxt; };   // wmax: consumer warps per CTA, forward / transpose
+#ifndef GL_TS_RPS6
+#define GL_TS_RPS6 6
+#endif
+#ifndef GL_TS_RPS11
+#define GL_TS_RPS11 6
+#endif
+#ifndef GL_TS_RPS16
+#define GL_TS_RPS16 8
+#endif
+#ifndef GL_TS_W6
+#define GL_TS_W6 8, 8
+#endif
+#ifndef GL_TS_W11
+#define GL_TS_W11 7, 4
+#endif
+#ifndef GL_TS_W16
+#define GL_TS_W16 4, 4
+#endif
+static constexpr TsVariant k_ts_variants[] = {{6, 1, 4, 4, GL_TS_RPS6, GL_TS_W6, GL_TS_MAXT6}, {6, 1, 16, 4, GL_TS_RPS6, GL_TS_W6, GL_TS_MAXT6},
+                                              {11, 2, 4, GL_TS_CW11, GL_TS_RPS11, GL_TS_W11, GL_TS_MAXT11},
+                                              {11, 2, 16, GL_TS_CW11, GL_TS_RPS11, GL_TS_W11, GL_TS_MAXT11},
+                                              {16, 8, 4, GL_TS_CW16, GL_TS_RPS16, GL_TS_W16, GL_TS_MAXT16}};
+static inline int ts_variant(int U, int NPH) {
+    for (int i = 0; i < (int)(sizeof(k_ts_variants) / sizeof(k_ts_variants[0])); ++i)
+        if (k_ts_variants[i].U == U && k_ts_variants[i].NPH == NPH) return i;
+    return -1;
+}
+#ifndef GL_TS_STAGES
+#define GL_TS_STAGES 3
+#endif
+// Launch plan of one direction.  ncols: output columns to cover; planes_in_box: NPH (forward) or 1 (transpose);
+// pitch_rule: forward rows of different planes sit boxw apart -> boxw * esize = 16 (mod 32) keeps a quarter-warp's
+// 16-byte loads on distinct banks.
+static inline TsPlan ts_plan(const TsVariant& v, int wmax_default, int esize, int ncols, int planes_in_box, int steps, int row0) {
+    TsPlan pl{};
+    const int LPG = v.NPH * v.G, CGW = 32 / LPG, NU = (v.U + v.G - 1) / v.G;
+    (void)NU;
+    const int ve = ((v.CW * esize) % 16 == 0 ? 16 : 8) / esize;
+    const int segp = (v.CW + v.U - 1 + ve - 1) / ve * ve;
+    pl.ncg = (ncols + v.CW - 1) / v.CW;
+    const int warps = (pl.ncg + CGW - 1) / CGW;
+    int wmax = wmax_default, nst = GL_TS_STAGES;
+    if (const char* e = std::getenv("GL_TS_WMAX")) { const int k = std::atoi(e); if (k >= 1) wmax = k; }   // tuning overrides
+    if (const char* e = std::getenv("GL_TS_STAGES")) { const int k = std::atoi(e); if (k >= 2 && k <= 16) nst = k; }
+    if (wmax > v.maxt / 32 - 1) wmax = v.maxt / 32 - 1;
+    pl.n_bands = (warps + wmax - 1) / wmax;
+    pl.wpc = (warps + pl.n_bands - 1) / pl.n_bands;
+    // TMA: the first column of a band must sit on a 16-byte boundary
+    while (pl.n_bands > 1 && (v.CW * pl.wpc * CGW * esize) % 16 != 0) ++pl.wpc;
+    pl.n_bands = (warps + pl.wpc - 1) / pl.wpc;
+    pl.cg_per_cta = pl.wpc * CGW;
+    int bw = v.CW * (pl.cg_per_cta - 1) + segp;
+    const int q = 16 / esize;                                   // TMA: box row a multiple of 16 bytes
+    bw = round_up(bw, q);
+    if (planes_in_box > 1) while ((bw * esize) % 32 != 16) bw += q;
+    pl.boxw = bw;
+    pl.stage_elems = round_up(bw * planes_in_box * v.RPS, 128 / esize);
+    pl.stages = nst;
+    pl.steps = steps; pl.row0 = row0;
+    pl.pbuf_elems = planes_in_box > 1 ? ts_pbuf_elems(v.NPH, v.G, v.CW, v.RPS) : 0;
+    return pl;
+}
 
 // Fill the layout fields of G (UP, Hp, Wp, Hg, Wg, PADg) and choose the kernels.  esize = sizeof(T).
 static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems) {
@@ -49,6 +124,22 @@ static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems) {
     const int LS = pl.kind == 1 ? 4 : 1;                         // lanes per column group (conv_*_launch must agree)
     int ps = U * ((U + 1) & ~1);
     if (LS > 1) while ((2 * ps) % 32 != 8 && (2 * ps) % 32 != 24) ps += 2;   // 4 consecutive planes -> disjoint bank groups
+    {   // tap-stationary kernels (gl_conv_ts.cuh) wherever an instance exists; GL_CONV_TS=0 keeps the round-1 kernels (A/B runs)
+        const char* e = std::getenv("GL_CONV_TS");
+        const int id = ts_variant(U, NPH);
+        if (id >= 0 && !(e && e[0] == '0')) {
+            const TsVariant& v = k_ts_variants[id];
+            const int NU = (v.U + v.G - 1) / v.G, UPAD = NU * v.G;
+            const int omin = G.c / G.s, omax = (G.s - 1 + G.c) / G.s;
+            TsPlan tf = ts_plan(v, v.wmax_f, esize, N, NPH, N + UPAD - 1, 0);
+            TsPlan tb = ts_plan(v, v.wmax_b, esize, N + ob_max, 1, N + (omax - omin) + UPAD - 1, omin);
+            if (tf.boxw <= 256 && tb.boxw <= 256 && (tf.wpc + 1) * 32 <= v.maxt && (tb.wpc + 1) * 32 <= v.maxt &&
+                v.CW * tb.ncg <= G.Wp) {
+                pl.kind = 4; pl.ts_id = id; pl.CW = v.CW; pl.tf = tf; pl.tb = tb; pl.n_ctile = tf.n_bands * tf.wpc;
+                return pl;
+            }
+        }
+    }
     const int nt_max = 256;                 // launch bounds of the compiled specialisations
     auto mk = [&](int ncg, int cta_f64) {
         SlidePlan sp{};
@@ -132,6 +223,94 @@ static inline cudaError_t conv_bwd_is2_launch(const ConvPlan& pl, const Geom& G,
     return cudaSuccess;
 }
 
+// ----------------------------------------------------------------------------- tap-stationary launches (kind 4)
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time dependency on libcuda).
+typedef CUresult (*gl_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                       const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                       CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static inline gl_encode_tiled_fn gl_encode_tiled() {
+    static gl_encode_tiled_fn fn = []() -> gl_encode_tiled_fn {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+            return nullptr;
+        return (gl_encode_tiled_fn)f;
+    }();
+    return fn;
+}
+// 3-D tensor {d0, d1, d2} of T at `base`, dim 0 contiguous, dims 1 and 2 with the given element strides; box {b0, b1, b2}; elements outside the tensor read as zero.
+template <class T>
+static inline bool ts_make_map(CUtensorMap* tm, const void* base, uint64_t d0, uint64_t d1, uint64_t d2, uint64_t stride1, uint64_t stride2,
+                               uint32_t b0, uint32_t b1, uint32_t b2) {
+    gl_encode_tiled_fn enc = gl_encode_tiled();
+    if (!enc) return false;
+    const cuuint64_t dims[3] = {d0, d1, d2};
+    const cuuint64_t strides[2] = {stride1 * sizeof(T), stride2 * sizeof(T)};      // element strides of dims 1 and 2
+    const cuuint32_t box[3] = {b0, b1, b2};
+    const cuuint32_t es[3] = {1, 1, 1};
+    return enc(tm, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(base), dims,
+               strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// Persistent grid: every SM gets as many CTAs as fit (shared-memory carve-out raised to the maximum, else the driver sizes
+// it for ONE block), never more CTAs than work items.
+template <class K>
+static inline cudaError_t ts_grid(K kern, const TsPlan& pl, size_t smem, int64_t Pc, unsigned* grid) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    int dev = 0, n_sm = 0, occ = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, (pl.wpc + 1) * 32, smem)) != cudaSuccess) return e;
+    if (occ < 1) return cudaErrorLaunchOutOfResources;
+    const int64_t items = Pc * pl.n_bands, cap = (int64_t)n_sm * occ;
+    *grid = (unsigned)(items < cap ? items : cap);
+    return cudaSuccess;
+}
+
+template <class T, int U, int G_, int NPH, int CW, int RPS>
+static inline cudaError_t conv_fwd_ts_launch(const ConvPlan& pl, const Geom& G, const T* ray, const T* sys_kt, const T* sys_w,
+                                             const float* obs, const int32_t* system_id, int64_t p_base, int64_t Pc, T* gpix,
+                                             T* chi, float* out_model, cudaStream_t st) {
+    CUtensorMap tm;
+    // plane index in the middle: {Wp, NPH * Pc (stride Hp Wp), Hp (stride Wp)} -> a box lands as [RPS][NPH][boxw]
+    if (!ts_make_map<T>(&tm, ray, (uint64_t)G.Wp, (uint64_t)NPH * (uint64_t)Pc, (uint64_t)G.Hp, (uint64_t)G.Hp * G.Wp, (uint64_t)G.Wp,
+                        (uint32_t)pl.tf.boxw, NPH, RPS))
+        return cudaErrorInvalidValue;
+    auto kern = gl_conv_fwd_ts<T, U, G_, NPH, CW, RPS>;
+    const size_t smem = ts_smem_bytes<T>(pl.tf);
+    unsigned grid = 0;
+    cudaError_t e = ts_grid(kern, pl.tf, smem, Pc, &grid);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, (pl.tf.wpc + 1) * 32, smem, st>>>(tm, G, pl.tf, Pc, sys_kt, sys_w, obs, system_id, p_base, gpix, chi, out_model);
+    return cudaSuccess;
+}
+template <class T, int U, int G_, int NPH, int CW, int RPS>
+static inline cudaError_t conv_bwd_ts_launch(const ConvPlan& pl, const Geom& G, const T* gpix, const T* sys_kt,
+                                             const int32_t* system_id, int64_t p_base, int64_t Pc, T* gbar, cudaStream_t st) {
+    CUtensorMap tm;
+    if (!ts_make_map<T>(&tm, gpix, (uint64_t)G.Wg, (uint64_t)G.Hg, (uint64_t)Pc, (uint64_t)G.Wg, (uint64_t)G.Hg * G.Wg, (uint32_t)pl.tb.boxw,
+                        RPS, 1))
+        return cudaErrorInvalidValue;
+    auto kern = gl_conv_bwd_ts<T, U, G_, NPH, CW, RPS>;
+    const size_t smem = ts_smem_bytes<T>(pl.tb);
+    unsigned grid = 0;
+    cudaError_t e = ts_grid(kern, pl.tb, smem, Pc, &grid);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, (pl.tb.wpc + 1) * 32, smem, st>>>(tm, G, pl.tb, Pc, sys_kt, system_id, p_base, gbar);
+    return cudaSuccess;
+}
+#define GL_TS_DISPATCH(CALL)                                                                                       \
+    switch (pl.ts_id) {                                                                                            \
+        case 0: e = CALL(6, 1, 4, 4, GL_TS_RPS6); break;                                                           \
+        case 1: e = CALL(6, 1, 16, 4, GL_TS_RPS6); break;                                                          \
+        case 2: e = CALL(11, 2, 4, GL_TS_CW11, GL_TS_RPS11); break;                                                \
+        case 3: e = CALL(11, 2, 16, GL_TS_CW11, GL_TS_RPS11); break;                                               \
+        default: e = CALL(16, 8, 4, GL_TS_CW16, GL_TS_RPS16); break;                                               \
+    }
+
 // Step D + E.  Returns the number of kernels launched (negative on a CUDA error).
 template <class T>
 static inline int conv_fwd_launch(const ConvPlan& pl, const Geom& G, const T* ray, const T* sys_kt, const T* sys_w,
@@ -142,6 +321,12 @@ static inline int conv_fwd_launch(const ConvPlan& pl, const Geom& G, const T* ra
         case 1: e = conv_fwd_is_launch<T, 6, 4, 4, 256>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st); break;
         case 2: e = conv_fwd_is2_launch<T, 11, 2, 256>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st); break;
         case 3: e = conv_fwd_is2_launch<T, 16, 2, 256>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st); break;
+        case 4: {
+#define GL_TS_F(U_, G__, NPH_, CW_, RPS_) conv_fwd_ts_launch<T, U_, G__, NPH_, CW_, RPS_>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st)
+            GL_TS_DISPATCH(GL_TS_F)
+#undef GL_TS_F
+            break;
+        }
         default: {
             dim3 grid((G.N * G.N + 255) / 256, (unsigned)Pc);
             gl_conv_fwd_generic<T><<<grid, 256, 0, st>>>(G, ray, sys_kt, sys_w, obs, system_id, p_base, gpix, chi, out_model);
@@ -159,6 +344,12 @@ static inline int conv_bwd_launch(const ConvPlan& pl, const Geom& G, const T* gp
         case 1: e = conv_bwd_is_launch<T, 6, 4, 4, 256>(pl, G, gpix, sys_kt, system_id, p_base, Pc, gbar, st); break;
         case 2: e = conv_bwd_is2_launch<T, 11, 2, 256>(pl, G, gpix, sys_kt, system_id, p_base, Pc, gbar, st); break;
         case 3: e = conv_bwd_is2_launch<T, 16, 2, 256>(pl, G, gpix, sys_kt, system_id, p_base, Pc, gbar, st); break;
+        case 4: {
+#define GL_TS_B(U_, G__, NPH_, CW_, RPS_) conv_bwd_ts_launch<T, U_, G__, NPH_, CW_, RPS_>(pl, G, gpix, sys_kt, system_id, p_base, Pc, gbar, st)
+            GL_TS_DISPATCH(GL_TS_B)
+#undef GL_TS_B
+            break;
+        }
         default: {
             dim3 grid((G.s * G.s * G.N * G.N + 255) / 256, (unsigned)Pc);
             gl_conv_bwd_generic<T><<<grid, 256, 0, st>>>(G, gpix, sys_kt, system_id, p_base, gbar);
