@@ -133,8 +133,9 @@ gl_status gl_config_shape(const gl_config* cfg, int32_t* out);
 
 /* Bytes of device workspace gl_logpost / gl_logpost_grad / gl_model_image need for n_particles
  * (0 if cfg is NULL or n_particles <= 0).  Grows with n_particles up to an internal chunk size, then stays
- * flat (about 4 GiB; about 16 GiB with amplitude_mode 1, which keeps n_amp component images per particle): larger
- * batches are processed in chunks on the same stream.  The workspace must be 256-byte aligned. */
+ * flat (about 4 GiB; about 8 GiB in GL_PRECISION_F64 with shapelet_nmax > 6, whose adjoint keeps two more values per
+ * ray; about 16 GiB with amplitude_mode 1, which keeps n_amp component images per particle): larger batches are
+ * processed in chunks on the same stream.  The workspace must be 256-byte aligned. */
 size_t gl_workspace_bytes(const gl_config* cfg, int64_t n_particles);
 
 /* log p~ for each particle (O1-O8):

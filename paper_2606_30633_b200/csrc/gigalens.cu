@@ -38,6 +38,7 @@ struct gl_config {
     AmpMap amp;         // light amplitudes (n = 0 unless amplitude_mode 1 ... see n_amp)
     int n_amp;          // amplitude count of the model, whatever the mode
     int esize;          // sizeof the arithmetic type: 8 (GL_PRECISION_F64) or 4 (GL_PRECISION_F32)
+    int uv_split;       // 1: the adjoint stores the shapelet coordinates (u, v) of every ray for gl_shp_coef_kernel (coef_split)
     size_t per_particle_bytes;
 };
 
@@ -247,6 +248,8 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     c->per_particle_bytes = (size_t)c->esize * ((size_t)PB_STRIDE + ray_stride(G) + gpix_stride(G) + (size_t)c->n_ctile +
                                                 (size_t)c->n_nap * c->na) + sizeof(double) + 6 * 256;
     if (d->amplitude_mode == 1) c->per_particle_bytes += (size_t)c->esize * c->n_amp * (gpix_stride(G) + ray_stride(G));
+    c->uv_split = (c->esize == 8 && L.ker_nmax > 6) ? 1 : 0;      // must agree with coef_split<T, V>() in gl_ray.cuh
+    if (c->uv_split) c->per_particle_bytes += (size_t)c->esize * 2 * ray_stride(G);
     *out = c;
     return GL_OK;
 }
@@ -262,13 +265,14 @@ extern "C" gl_status gl_config_shape(const gl_config* c, int32_t* out) {
 
 struct Plan {
     int64_t Pc;
-    size_t off_tab, off_kt, off_w, off_sl, off_pb, off_lpd, off_ray, off_gpix, off_chi, off_nap, off_comp, off_cray, off_zobs, off_uw, off_sid, total;
+    size_t off_tab, off_kt, off_w, off_sl, off_pb, off_lpd, off_ray, off_gpix, off_chi, off_nap, off_uv, off_comp, off_cray, off_zobs, off_uw, off_sid, total;
 };
 
 static Plan make_plan(const gl_config* c, int64_t P) {
     Plan pl{};
     const Geom& G = c->G;
-    int64_t pc_max = (int64_t)((c->desc.amplitude_mode == 1 ? WS_BUDGET_AMP : WS_BUDGET) / c->per_particle_bytes);
+    // the split adjoint keeps (u, v) of every ray: twice the budget keeps its chunks as large as the other variants'
+    int64_t pc_max = (int64_t)((c->desc.amplitude_mode == 1 ? WS_BUDGET_AMP : (c->uv_split ? 2 * WS_BUDGET : WS_BUDGET)) / c->per_particle_bytes);
     if (pc_max < 1) pc_max = 1;
     if (pc_max > 32768) pc_max = 32768;
     pl.Pc = P < pc_max ? P : pc_max;
@@ -284,6 +288,8 @@ static Plan make_plan(const gl_config* c, int64_t P) {
     pl.off_gpix = o; o = align256(o + es * (size_t)pl.Pc * gpix_stride(G));
     pl.off_chi = o;  o = align256(o + es * (size_t)pl.Pc * c->n_ctile);
     pl.off_nap = o;  o = align256(o + es * (size_t)pl.Pc * c->n_nap * c->na);
+    pl.off_uv = o;
+    if (c->uv_split) o = align256(o + es * (size_t)pl.Pc * 2 * ray_stride(G));
     pl.off_comp = pl.off_cray = pl.off_zobs = pl.off_uw = pl.off_sid = o;
     if (c->desc.amplitude_mode == 1) {
         pl.off_comp = o; o = align256(o + es * (size_t)c->n_amp * pl.Pc * gpix_stride(G));
@@ -319,14 +325,15 @@ static void launch_ray_fwd(const gl_config* c, const T* pb, const double* tab, T
     gl_ray_fwd_kernel<T, V, NT_FWD, RB_FWD><<<grid, c->nt_fwd, 0, st>>>(c->G, pb, tab, ray, c->rpt_fwd, c->n_chunk_fwd);
 }
 template <class T, class V>
-static cudaError_t launch_ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, int64_t Pc, cudaStream_t st) {
+static cudaError_t launch_ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, T* uv, int64_t Pc, cudaStream_t st) {
     dim3 grid(c->n_nap, (unsigned)Pc);
-    const size_t smem = coef_in_smem<T, V>() ? sizeof(T) * (size_t)V::NCOEF * c->nt_adj : 0;   // coefficient sums, one column per thread
-    if (smem > 40 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(gl_ray_adj_kernel<T, V, NT_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
+    gl_ray_adj_kernel<T, V, NT_ADJ><<<grid, c->nt_adj, 0, st>>>(c->G, pb, tab, gbar, nap, uv, c->rpt_adj, c->n_chunk_adj);
+    if constexpr (coef_split<T, V>()) {     // the shapelet coefficient sums from the stored (u, v): same grid, same partial slots
+        // its own block size (128) and rays per thread: any partition of a plane's rays over the n_chunk_adj CTAs of a plane works
+        const int ntc = 128, rptc = (c->G.N * c->G.N + c->n_chunk_adj * ntc - 1) / (c->n_chunk_adj * ntc);
+        gl_shp_coef_kernel<T, V::NMAX, V::NA, 128><<<grid, ntc, 0, st>>>(c->G, pb, tab, gbar, uv, nap, rptc, c->n_chunk_adj);
+        ++t_launches;
     }
-    gl_ray_adj_kernel<T, V, NT_ADJ><<<grid, c->nt_adj, smem, st>>>(c->G, pb, tab, gbar, nap, c->rpt_adj, c->n_chunk_adj);
     return cudaSuccess;
 }
 
@@ -375,19 +382,19 @@ static void ray_comp(const gl_config* c, const T* pb, const double* tab, T* cray
     }
 }
 template <class T>
-static cudaError_t ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, int64_t Pc, cudaStream_t st) {
+static cudaError_t ray_adj(const gl_config* c, const T* pb, const double* tab, const T* gbar, T* nap, T* uv, int64_t Pc, cudaStream_t st) {
     const int id = c->variant * 2 + c->desc.mass_model;
     switch (id) {
-        case 0: return launch_ray_adj<T, V_S0>(c, pb, tab, gbar, nap, Pc, st);
-        case 1: return launch_ray_adj<T, V_E0>(c, pb, tab, gbar, nap, Pc, st);
-        case 2: return launch_ray_adj<T, V_S1>(c, pb, tab, gbar, nap, Pc, st);
-        case 3: return launch_ray_adj<T, V_E1>(c, pb, tab, gbar, nap, Pc, st);
-        case 4: return launch_ray_adj<T, V_S2>(c, pb, tab, gbar, nap, Pc, st);
-        case 5: return launch_ray_adj<T, V_E2>(c, pb, tab, gbar, nap, Pc, st);
-        case 6: return launch_ray_adj<T, V_S3>(c, pb, tab, gbar, nap, Pc, st);
-        case 7: return launch_ray_adj<T, V_E3>(c, pb, tab, gbar, nap, Pc, st);
-        case 8: return launch_ray_adj<T, V_S4>(c, pb, tab, gbar, nap, Pc, st);
-        default: return launch_ray_adj<T, V_E4>(c, pb, tab, gbar, nap, Pc, st);
+        case 0: return launch_ray_adj<T, V_S0>(c, pb, tab, gbar, nap, uv, Pc, st);
+        case 1: return launch_ray_adj<T, V_E0>(c, pb, tab, gbar, nap, uv, Pc, st);
+        case 2: return launch_ray_adj<T, V_S1>(c, pb, tab, gbar, nap, uv, Pc, st);
+        case 3: return launch_ray_adj<T, V_E1>(c, pb, tab, gbar, nap, uv, Pc, st);
+        case 4: return launch_ray_adj<T, V_S2>(c, pb, tab, gbar, nap, uv, Pc, st);
+        case 5: return launch_ray_adj<T, V_E2>(c, pb, tab, gbar, nap, uv, Pc, st);
+        case 6: return launch_ray_adj<T, V_S3>(c, pb, tab, gbar, nap, uv, Pc, st);
+        case 7: return launch_ray_adj<T, V_E3>(c, pb, tab, gbar, nap, uv, Pc, st);
+        case 8: return launch_ray_adj<T, V_S4>(c, pb, tab, gbar, nap, uv, Pc, st);
+        default: return launch_ray_adj<T, V_E4>(c, pb, tab, gbar, nap, uv, Pc, st);
     }
 }
 
@@ -468,7 +475,7 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
             if (nl < 0) return GL_ERR_CUDA;
             t_launches += nl;
             cudaError_t ea = cudaSuccess;
-            GL_STAGE(ST_RAY_ADJ, st, ea = ray_adj<T>(c, pb, tab, ray, nap, Pc, st)); ++t_launches;
+            GL_STAGE(ST_RAY_ADJ, st, ea = ray_adj<T>(c, pb, tab, ray, nap, (T*)(w + pl.off_uv), Pc, st)); ++t_launches;
             if (ea != cudaSuccess) return GL_ERR_CUDA;
         }
         const int wpb = 4;

@@ -217,9 +217,12 @@ __device__ __forceinline__ void sersic_accum(const SersicOut<T>& o, T g, T* __re
     S[SA_BXX] = R::fma(Wx, o.xr, S[SA_BXX]); S[SA_BYY] = R::fma(Wy, o.yr, S[SA_BYY]); S[SA_BXY] = R::fma(Wx, o.yr, S[SA_BXY]);
 }
 
-// Where the shapelet coefficient sums of the adjoint live: registers, except in fp64 at n_max > 6 where 66 fp64
-// accumulators spill (measured: shared memory wins only there).
-template <class T, class V> __host__ __device__ constexpr bool coef_in_smem() { return sizeof(T) == 8 && V::NMAX > 6; }
+// Where the shapelet coefficient sums of the adjoint are taken: in the registers of gl_ray_adj_kernel, except in fp64 at
+// n_max > 6, where 66 fp64 accumulators do not fit next to the 45 other sums.  Round 1 kept them in shared memory (66
+// read-modify-writes per ray: top stall short_scoreboard at 8 warps per SM, profiles/r2a_cfg5_f64.md); now the adjoint
+// kernel stores the shapelet coordinates (u, v) of every ray (16 bytes) and gl_shp_coef_kernel takes the sums from
+// (gbar, u, v) with all 66 accumulators in registers and nothing else to hold.
+template <class T, class V> __host__ __device__ constexpr bool coef_split() { return sizeof(T) == 8 && V::NMAX > 6; }
 
 // Component slots of backward modelling (gl_linear.cuh): index of each light component among the amplitudes, -1 = absent.
 struct CompIdx { int src, src1, shp0, n_coef, ll0, ll1, ll2; };
@@ -231,7 +234,7 @@ template <class T, class V, bool ADJ, bool COMP = false>
 __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* __restrict__ pb,
                                       const T* __restrict__ cfs, const float* __restrict__ cf32, T fj, T fi, T gbar,
                                       T* __restrict__ acc,
-                                      T* __restrict__ sacc = nullptr, int sstride = 0,
+                                      T* __restrict__ uvp = nullptr, size_t uvstride = 0,
                                       const CompIdx* ci = nullptr, size_t cstride = 0) {
     using R = Real<T>;
     const T step = pb[PB_STEP];
@@ -361,9 +364,13 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
                     Ish = R::fma(row, fv[n2], Ish);
                 }
             } else {
-                // phi_k' = HD[k] phi_{k-1} - u phi_k is formed where it is used (no derivative arrays); the N_coef
-                // coefficient sums live in shared memory (sacc[idx * sstride], one column per thread): 66 fp64
-                // accumulators do not fit the register file next to the 45 other sums.
+                // phi_k' = HD[k] phi_{k-1} - u phi_k, once per ray; the N_coef coefficient sums gbar phi_n1(u) phi_n2(v) are
+                // taken here in registers, or (coef_split) by gl_shp_coef_kernel from the (u, v) stored below.
+                T dfu[NM + 1];
+                dfu[0] = -u * fu[0];
+#pragma unroll
+                for (int k = 1; k <= NM; ++k) dfu[k] = R::fma(hD<T>(k), fu[k - 1], -u * fu[k]);
+                if constexpr (coef_split<T, V>()) { uvp[0] = u; uvp[uvstride] = v; }
                 T Iu = T(0.), Iv = T(0.);
 #pragma unroll
                 for (int n2 = 0; n2 <= NM; ++n2) {
@@ -373,10 +380,8 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
                     for (int n1 = 0; n1 <= NM - n2; ++n1) {
                         const int idx = (n1 + n2) * (n1 + n2 + 1) / 2 + n2;
                         const T ak = a[idx];
-                        const T dfu = n1 == 0 ? -u * fu[0] : R::fma(hD<T>(n1), fu[n1 > 0 ? n1 - 1 : 0], -u * fu[n1]);
-                        row = R::fma(ak, fu[n1], row); drow = R::fma(ak, dfu, drow);
-                        if constexpr (coef_in_smem<T, V>()) sacc[idx * sstride] = R::fma(gfv, fu[n1], sacc[idx * sstride]);
-                        else acc[NA_SHA + idx] = R::fma(gfv, fu[n1], acc[NA_SHA + idx]);
+                        row = R::fma(ak, fu[n1], row); drow = R::fma(ak, dfu[n1], drow);
+                        if constexpr (!coef_split<T, V>()) acc[NA_SHA + idx] = R::fma(gfv, fu[n1], acc[NA_SHA + idx]);
                     }
                     Ish = R::fma(row, fv[n2], Ish); Iu = R::fma(drow, fv[n2], Iu); {
                         const T dfv = n2 == 0 ? -v * fv[0] : R::fma(hD<T>(n2), fv[n2 > 0 ? n2 - 1 : 0], -v * fv[n2]);
@@ -584,10 +589,10 @@ __global__ void __launch_bounds__(NT) gl_ray_comp_kernel(const __grid_constant__
 template <class T, class V, int NT>
 __global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC < 2 && V::NLL < 3 ? GL_ADJ_MINB : (sizeof(T) == 8 && V::NMAX < 0 ? GL_ADJ_MINB_X : 1))) gl_ray_adj_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
                                                         const double* __restrict__ tabg, const T* __restrict__ gbar,
-                                                        T* __restrict__ nap, int RPT, int n_chunk) {
+                                                        T* __restrict__ nap, T* __restrict__ uv, int RPT, int n_chunk) {
     __shared__ __align__(16) T pb[PB_STRIDE];
     __shared__ __align__(128) double tabs[TabStage<T>::N];
-    __shared__ T red[NT / 32][V::NA];
+    __shared__ T red[NT / 32][coef_split<T, V>() ? NA_SHA : V::NA];
     const int p = blockIdx.y;
     const T* src = pbg + (size_t)p * PB_STRIDE;
     for (int k = threadIdx.x; k < V::PB_NEED; k += blockDim.x) pb[k] = src[k];
@@ -599,22 +604,20 @@ __global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC 
     PlaneIter it(G, n_chunk, RPT);
     const T* gb = gbar + (size_t)p * ray_stride(G) + (size_t)it.ph * G.Hp * G.Wp;
     const int NN = G.N * G.N;
-    extern __shared__ __align__(16) unsigned char adj_dyn[];       // shapelet coefficient sums [NCOEF][blockDim.x]
-    T* sacc = reinterpret_cast<T*>(adj_dyn) + threadIdx.x;
-    const int sstride = blockDim.x;
-    constexpr bool CS = coef_in_smem<T, V>();
-    constexpr int NREG = CS ? NA_SHA : V::NA;                     // accumulators kept in registers
-    if constexpr (CS) {
-#pragma unroll 1
-        for (int k = 0; k < V::NCOEF; ++k) sacc[k * sstride] = T(0.);
-    }
+    constexpr bool CS = coef_split<T, V>();
+    constexpr int NREG = CS ? NA_SHA : V::NA;                     // accumulators of this kernel (all in registers)
+    const size_t rs = ray_stride(G);
+    T* uvb = CS ? uv + (size_t)p * 2 * rs + (size_t)it.ph * G.Hp * G.Wp : nullptr;
     T acc[NREG];
 #pragma unroll
     for (int k = 0; k < NREG; ++k) acc[k] = T(0.);
     if (pb[PB_VALID] != T(0.)) {
         for (int r = 0; r < RPT; ++r) {
             int off = 0; asm volatile("" : "+r"(off));      // opaque: keeps the PB scalars in shared memory, not in registers
-            if (it.idx < NN) ray_eval<T, V, true>(tb, pb + off, cfs + off, cf32 + off, it.fj<T>(G), it.fi<T>(G), gb[it.offset(G)], acc, sacc, sstride);
+            if (it.idx < NN) {
+                const size_t o = it.offset(G);
+                ray_eval<T, V, true>(tb, pb + off, cfs + off, cf32 + off, it.fj<T>(G), it.fi<T>(G), gb[o], acc, CS ? uvb + o : nullptr, rs);
+            }
             it.next(G);
         }
     }
@@ -624,16 +627,79 @@ __global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC 
         T v = warp_sum(acc[k]);
         if (lane == 0) red[w][k] = v;
     }
-    if constexpr (CS) {
-#pragma unroll 1
-        for (int k = 0; k < V::NCOEF; ++k) {
-            T v = warp_sum(sacc[k * sstride]);
-            if (lane == 0) red[w][NA_SHA + k] = v;
-        }
-    }
     __syncthreads();
     T* o = nap + ((size_t)p * gridDim.x + blockIdx.x) * V::NA;
-    for (int k = threadIdx.x; k < V::NA; k += blockDim.x) {
+    for (int k = threadIdx.x; k < NREG; k += blockDim.x) {
+        T s = T(0.);
+        for (int ww = 0; ww < nw; ++ww) s += red[ww][k];
+        o[k] = s;
+    }
+}
+
+// Shapelet coefficient sums of step F in the split form (coef_split): nap[..][NA_SHA + k] = sum_rays gbar phi_n1(u) phi_n2(v),
+// k = (n1 + n2)(n1 + n2 + 1)/2 + n2, from the (u, v) gl_ray_adj_kernel stored.  Same grid, block and ray <-> thread mapping as
+// that kernel, so both write the same partial slot of nap; fixed-order warp / CTA reduction, no atomics.
+template <class T, int NMAX, int NA, int NT>
+__global__ void __launch_bounds__(NT) gl_shp_coef_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
+                                                         const double* __restrict__ tabg, const T* __restrict__ gbar,
+                                                         const T* __restrict__ uv, T* __restrict__ nap, int RPT, int n_chunk) {
+    constexpr int NC = (NMAX + 1) * (NMAX + 2) / 2;
+    __shared__ __align__(128) double tabs[TabStage<T>::N];
+    __shared__ T red[NT / 32][NC];
+    const int p = blockIdx.y;
+    const typename Real<T>::Tab tb = TabStage<T>::make(tabs, tabg);
+    __syncthreads();
+    PlaneIter it(G, n_chunk, RPT);
+    const size_t rs = ray_stride(G), pl = (size_t)it.ph * G.Hp * G.Wp;
+    const T* gb = gbar + (size_t)p * rs + pl;
+    const T* ub = uv + (size_t)p * 2 * rs + pl;
+    const int NN = G.N * G.N;
+    T acc[NC];
+#pragma unroll
+    for (int k = 0; k < NC; ++k) acc[k] = T(0.);
+    if (pbg[(size_t)p * PB_STRIDE + PB_VALID] != T(0.)) {
+        // (gbar, u, v) of the next NQ rays are in flight while one ray is worked on: the kernel holds ~220 registers
+        // (2 warps per scheduler), so the HBM latency has to be covered inside the thread.  A ring of NQ register slots
+        // indexed at compile time (a shifted queue would read the newest load one iteration after it was issued).
+        constexpr int NQ = 4;
+        T gq[NQ], uq[NQ], vq[NQ];
+        PlaneIter ld = it;
+        auto fetch = [&](int slot_ray, T& g, T& u, T& v) {
+            const bool ok = ld.idx < NN && slot_ray < RPT;
+            const size_t o = ok ? ld.offset(G) : 0;
+            g = ok ? gb[o] : T(0.); u = ok ? ub[o] : T(0.); v = ok ? ub[rs + o] : T(0.);
+            ld.next(G);
+        };
+#pragma unroll
+        for (int k = 0; k < NQ; ++k) fetch(k, gq[k], uq[k], vq[k]);
+        for (int r0 = 0; r0 < RPT; r0 += NQ) {
+#pragma unroll
+            for (int k = 0; k < NQ; ++k) {
+                const T g = gq[k], u = uq[k], v = vq[k];            // gbar = 0 beyond the plane: such a ray adds nothing
+                fetch(r0 + k + NQ, gq[k], uq[k], vq[k]);
+                T fu[NMAX + 1], fv[NMAX + 1];
+                hermite<T, NMAX>(tb, u, fu); hermite<T, NMAX>(tb, v, fv);
+#pragma unroll
+                for (int n1 = 0; n1 <= NMAX; ++n1) {
+                    const T gf = g * fu[n1];
+#pragma unroll
+                    for (int n2 = 0; n2 <= NMAX - n1; ++n2) {
+                        const int idx = (n1 + n2) * (n1 + n2 + 1) / 2 + n2;
+                        acc[idx] = Real<T>::fma(gf, fv[n2], acc[idx]);
+                    }
+                }
+            }
+        }
+    }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+        const T v = warp_sum(acc[k]);
+        if (lane == 0) red[w][k] = v;
+    }
+    __syncthreads();
+    T* o = nap + ((size_t)p * gridDim.x + blockIdx.x) * NA + NA_SHA;
+    for (int k = threadIdx.x; k < NC; k += blockDim.x) {
         T s = T(0.);
         for (int ww = 0; ww < nw; ++ww) s += red[ww][k];
         o[k] = s;
