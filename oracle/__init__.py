@@ -27,7 +27,7 @@ class _Config(C.Structure):
                 ("multipole_mask", C.c_int32), ("n_source_sersic", C.c_int32), ("shapelet_nmax", C.c_int32),
                 ("n_lens_sersic", C.c_int32), ("param_space", C.c_int32), ("n_systems", C.c_int32),
                 ("n_params", C.c_int32), ("psf_grid", C.c_int32), ("noise_model", C.c_int32), ("t_exp", C.c_double),
-                ("priors", C.POINTER(_Prior))]
+                ("source2_plane", C.c_int32), ("priors", C.POINTER(_Prior))]
 
 
 _lib = None
@@ -82,7 +82,8 @@ def _make_config(spec, epl_terms=None, param_space=None):
                   spec.n_source_sersic, spec.shapelet_nmax, spec.n_lens_sersic,
                   spec.param_space if param_space is None else int(param_space),
                   spec.n_systems, spec.n_params, int(getattr(spec, "psf_grid", 0)),
-                  int(getattr(spec, "noise_model", 0)), float(getattr(spec, "t_exp", 1.0)), pri)
+                  int(getattr(spec, "noise_model", 0)), float(getattr(spec, "t_exp", 1.0)),
+                  int(getattr(spec, "source2_plane", 0)), pri)
     cfg._keep = pri
     return cfg
 
@@ -137,6 +138,7 @@ def model_image(spec, psf, theta, epl_terms=None, system_id=None):
         "n_pix supersample psf_size pix_scale mass_model epl_terms has_shear multipole_mask n_source_sersic "
         "shapelet_nmax n_lens_sersic n_systems n_params").split()})
     s.psf_grid = int(getattr(spec, "psf_grid", 0))
+    s.source2_plane = int(getattr(spec, "source2_plane", 0))
     s.param_space = 1
     s.priors = [(PRIOR_NONE, 0, 1, 0, 1)] * spec.n_params
     out = logpost_grad(s, obs, sig, psf, theta, system_id, want_grad=False, want_model=True, epl_terms=epl_terms)

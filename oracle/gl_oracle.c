@@ -58,12 +58,15 @@ typedef struct {
     int32_t noise_model;     /* 0: fixed sigma map (S12); 1: model-dependent variance
                                 v_p = sigma_p^2 + max(model_p, 0) / t_exp (NEXT-4, reading S12b) */
     double  t_exp;           /* exposure time of noise_model 1 (> 0) */
+    int32_t source2_plane;   /* 1: the second source Sersic sits on its OWN source plane ("multi-source-plane systems";
+                                SURVEY 8(f) NEXT-4, reading S23): its rays are deflected by eta2 * alpha, with one more
+                                sampled parameter eta2 right after its block; 0: both sources on one plane */
     const glo_prior* priors;
 } glo_config;
 
 /* ---------------------------------------------------------------- parameter layout (S18) -------- */
 typedef struct {
-    int mass, gamma, shear, mp3, mp4, src, src2, shp, ll[3], n;   /* offsets; -1 if absent */
+    int mass, gamma, shear, mp3, mp4, src, src2, eta2, shp, ll[3], n;   /* offsets; -1 if absent */
     int n_coef;
 } layout_t;
 
@@ -76,7 +79,8 @@ static void make_layout(const glo_config* c, layout_t* L) {
     if (c->multipole_mask & 1) { L->mp3 = k; k += 2; } else L->mp3 = -1;
     if (c->multipole_mask & 2) { L->mp4 = k; k += 2; } else L->mp4 = -1;
     if (c->n_source_sersic > 0) { L->src = k; k += 7; } else L->src = -1;
-    if (c->n_source_sersic > 1) { L->src2 = k; k += 7; } else L->src2 = -1;   /* second source, same source plane */
+    if (c->n_source_sersic > 1) { L->src2 = k; k += 7; } else L->src2 = -1;   /* second source */
+    if (c->n_source_sersic > 1 && c->source2_plane) { L->eta2 = k; k += 1; } else L->eta2 = -1;   /* its own plane: eta2 */
     L->n_coef = 0;
     if (c->shapelet_nmax >= 0) {
         L->n_coef = (c->shapelet_nmax + 1) * (c->shapelet_nmax + 2) / 2;
@@ -341,7 +345,12 @@ static double ray_intensity(const glo_config* c, const layout_t* L, const double
     double ax, ay; deflect(c, L, th, x, y, &ax, &ay);
     double bx = x - ax, by = y - ay, Iv = 0.0;
     if (L->src >= 0) Iv += sersic(th + L->src, bx, by, NULL, NULL);
-    if (L->src2 >= 0) Iv += sersic(th + L->src2, bx, by, NULL, NULL);
+    /* S23: a source on another plane sees the same lens-plane deflection scaled by the ratio eta2 of the lensing
+     * efficiencies D_ls/D_s of the two planes: beta_2 = theta - eta2 alpha(theta) (the first source carries no mass) */
+    if (L->src2 >= 0) {
+        double eta = L->eta2 >= 0 ? th[L->eta2] : 1.0;
+        Iv += sersic(th + L->src2, x - eta * ax, y - eta * ay, NULL, NULL);
+    }
     if (L->shp >= 0) Iv += shapelets(c->shapelet_nmax, th + L->shp, th[L->src + 4], th[L->src + 5], bx, by, NULL, NULL);
     for (int i = 0; i < 3; ++i) if (L->ll[i] >= 0) Iv += sersic(th + L->ll[i], x, y, NULL, NULL);
     return Iv;
@@ -373,9 +382,11 @@ static void ray_adjoint(const glo_config* c, const layout_t* L, const double* th
         sx += gbar * dxy[0]; sy += gbar * dxy[1];
     }
     if (L->src2 >= 0) {
-        double dp[7], dxy[2]; sersic(th + L->src2, bx, by, dp, dxy);
+        double eta = L->eta2 >= 0 ? th[L->eta2] : 1.0;
+        double dp[7], dxy[2]; sersic(th + L->src2, x - eta * ax, y - eta * ay, dp, dxy);
         for (int k = 0; k < 7; ++k) out[L->src2 + k] += gbar * dp[k];
-        sx += gbar * dxy[0]; sy += gbar * dxy[1];
+        sx += eta * gbar * dxy[0]; sy += eta * gbar * dxy[1];      /* d beta_2 / d(mass) = -eta2 d alpha / d(mass) */
+        if (L->eta2 >= 0) out[L->eta2] += -gbar * (dxy[0] * ax + dxy[1] * ay);   /* d beta_2 / d eta2 = -alpha */
     }
     if (L->shp >= 0) {
         double da[1 + 66 + 8], dxy[2];

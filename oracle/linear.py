@@ -29,8 +29,9 @@ def amplitude_indices(spec):
     i = (6 if spec.mass_model == 1 else 5) + (2 if spec.has_shear else 0)
     i += 2 * bin(spec.multipole_mask & 3).count("1")
     idx = []
-    for _ in range(spec.n_source_sersic):
+    for k in range(spec.n_source_sersic):
         idx.append(i + 6); i += 7
+        if k == 1 and getattr(spec, "source2_plane", 0): i += 1       # eta2 follows the second source block (S23)
     if spec.shapelet_nmax >= 0:
         nc = (spec.shapelet_nmax + 1) * (spec.shapelet_nmax + 2) // 2
         idx += list(range(i + 1, i + 1 + nc)); i += 1 + nc

@@ -221,3 +221,75 @@ def test_two_sources_three_lens_blocks_add_up_from_single_component_models():
     assert sp.n_params == 43 and W.param_names(1, 1, 0, 2, -1, 3)[15] == "src2.R"
     # each piece carries light (the test would pass trivially on dark components)
     assert all(np.abs(p).max() > 1e-3 * np.abs(full).max() for p in pieces)
+
+
+# --------------------------------------------------------------------------- two source planes (NEXT-4, reading S23)
+def _two_plane(param_space, eta):
+    """EPL + shear, two source Sersics (the second on its own plane, eta2 = `eta`), two lens-light blocks, 8x8, s = 2."""
+    rng = np.random.default_rng(23)
+    sp = W.LensSpec(8, 2, 5, 0.25, mass_model=1, n_source_sersic=2, n_lens_sersic=2, source2_plane=1, param_space=param_space)
+    pri = W._default_priors(1, n_lens=2, n_src=2, src2_plane=True)
+    pri[0] = W.Uniform(0.3, 1.5)
+    sp.priors = pri
+    th = np.array([0.62, 2.1, 0.12, -0.07, 0.03, -0.02, 0.04, -0.03,
+                   0.22, 1.6, 0.1, 0.06, 0.06, -0.05, 9.0, 0.31, 2.2, -0.08, 0.05, 0.25, -0.21, 5.0, eta,
+                   0.7, 3.1, -0.05, 0.08, 0.01, 0.02, 4.0, 1.2, 2.4, 0.04, -0.03, -0.01, 0.015, 1.5])
+    assert len(th) == sp.n_params == 37 and W.param_names(1, 1, 0, 2, -1, 2, 1)[22] == "src2.eta"
+    K = sp.psf_size
+    psf = rng.uniform(0.2, 1.0, (1, K, K)); psf /= psf.sum()
+    obs = rng.normal(0.5, 0.3, (1, 8, 8)); sig = rng.uniform(0.05, 0.2, (1, 8, 8))
+    return sp, psf, obs, sig, th
+
+
+def test_two_source_planes_end_points_and_shear_closed_form():
+    """beta_2 = theta - eta2 alpha(theta) ("multi-source-plane systems"; reading S23).  eta2 = 1 IS the one-plane
+    model, bit for bit; eta2 = 0 leaves the second source unlensed, i.e. it renders like a lens-plane Sersic block with
+    the same parameters; under a pure external shear the total flux of the second source is F / (1 - eta2^2 |gamma|^2)
+    (the shear-only magnification with the shear scaled by eta2: closed form at an intermediate eta2)."""
+    import dataclasses
+    sp, psf, obs, sig, th = _two_plane(1, 1.0)
+    one = dataclasses.replace(sp, source2_plane=0, priors=sp.priors[:22] + sp.priors[23:])
+    a = oracle.logpost_grad(sp, obs, sig, psf, [th], want_model=True)
+    b = oracle.logpost_grad(one, obs, sig, psf, [np.delete(th, 22)], want_model=True)
+    assert np.array_equal(a["model"], b["model"]) and a["logp"][0] == b["logp"][0]
+    assert np.array_equal(np.delete(a["grad"][0], 22), b["grad"][0])
+    # eta2 = 0: second source unlensed == (second source dark) + (a third lens-light block with its parameters)
+    th0 = th.copy(); th0[22] = 0.0
+    m0 = oracle.model_image(sp, psf, [th0])[0]
+    three = W.LensSpec(8, 2, 5, 0.25, mass_model=1, n_source_sersic=2, n_lens_sersic=3, source2_plane=1, param_space=1)
+    three.priors = sp.priors + W._default_priors(1)[-7:]
+    dark = th0.copy(); dark[21] = 0.0
+    m1 = oracle.model_image(three, psf, [np.concatenate([dark, th0[15:22]])])[0]
+    assert np.allclose(m0, m1, rtol=1e-13, atol=1e-13 * np.abs(m0).max())
+    assert np.abs(m0 - oracle.model_image(sp, psf, [th])[0]).max() > 1e-3 * np.abs(m0).max()      # eta2 matters
+    # shear-only lens (theta_E -> 0), first source dark: flux of the second source = F / (1 - eta^2 (g1^2 + g2^2))
+    g1, g2, R, n, Ie = 0.05, -0.03, 0.15, 1.0, 2.0
+    bn = 1.9992 * n - 0.3271
+    F = 2 * math.pi * n * Ie * R * R * math.exp(bn) * math.gamma(2 * n) / bn ** (2 * n)
+    fl = W.LensSpec(200, 1, 3, 0.02, mass_model=0, has_shear=1, n_source_sersic=2, n_lens_sersic=0, source2_plane=1, param_space=1)
+    fl.priors = [W.NoPrior()] * 22
+    for eta in (0.6, 1.0, 1.4):
+        ray = oracle.ray_image(fl, [1e-13, 0, 0, 0, 0, g1, g2, R, n, 0, 0, 0, 0, 0.0, R, n, 0.1, -0.05, 0.01, -0.02, Ie, eta])
+        assert abs(ray.sum() * 0.02 ** 2 / (F / (1 - eta * eta * (g1 * g1 + g2 * g2))) - 1) < 2e-3, eta
+    r1 = oracle.ray_image(fl, [1e-13, 0, 0, 0, 0, g1, g2, R, n, 0, 0, 0, 0, 0.0, R, n, 0.1, -0.05, 0.01, -0.02, Ie, 0.6]).sum()
+    r2 = oracle.ray_image(fl, [1e-13, 0, 0, 0, 0, g1, g2, R, n, 0, 0, 0, 0, 0.0, R, n, 0.1, -0.05, 0.01, -0.02, Ie, 1.4]).sum()
+    assert abs(r2 / r1 - (1 - 0.36 * (g1 * g1 + g2 * g2)) / (1 - 1.96 * (g1 * g1 + g2 * g2))) < 2e-5    # the eta dependence itself
+
+
+@pytest.mark.parametrize("param_space", [1, 0])
+@pytest.mark.parametrize("eta", [0.8, 1.35])
+def test_two_source_planes_gradient_vs_finite_differences(param_space, eta):
+    """Every component, eta2 included (d beta_2 / d eta2 = -alpha; the mass parameters see the second source through
+    eta2 d alpha / d theta_mass)."""
+    sp, psf, obs, sig, th = _two_plane(param_space, eta)
+    x0 = th if param_space == 1 else W.z_of(sp.priors, th)[0]
+    o = oracle.logpost_grad(sp, obs, sig, psf, [x0])
+    assert np.isfinite(o["logp"][0])
+    g = o["grad"][0]
+    lp = lambda x: oracle.logpost_grad(sp, obs, sig, psf, [x], want_grad=False)["logp"][0]
+    for k in range(sp.n_params):
+        def f(v, k=k):
+            x = x0.copy(); x[k] = v; return lp(x)
+        ref = fd(f, x0[k], 2e-4 * max(1.0, abs(x0[k])))
+        assert abs(g[k] - ref) < 2e-6 * abs(ref) + 1e-5, (k, g[k], ref)
+    assert abs(g[22]) > 1e-2                                             # eta2 carries a real gradient

@@ -52,6 +52,7 @@ class LensSpec:
     noise_model: int = 0         # 0: fixed sigma map (S12); 1: variance sigma^2 + max(model,0)/t_exp (NEXT-4, S12b)
     t_exp: float = 1.0           # exposure time of noise_model 1
     amplitude_mode: int = 0      # 0: amplitudes sampled ("forward"); 1: solved by linear inversion ("backward", NEXT-4, S21)
+    source2_plane: int = 0       # 1: the second source Sersic on its own source plane, one more parameter eta2 (NEXT-4, S23)
     precision: int = 0           # 0 GL_PRECISION_F64, 1 GL_PRECISION_F32 (CUDA path only; the oracle is always fp64)
     priors: list = field(default_factory=list)
     names: list = field(default_factory=list)
@@ -69,7 +70,7 @@ def n_shapelet_coef(nmax):
     return (nmax + 1) * (nmax + 2) // 2 if nmax >= 0 else 0
 
 
-def param_names(mass_model, has_shear, multipole_mask, n_source_sersic, shapelet_nmax, n_lens_sersic):
+def param_names(mass_model, has_shear, multipole_mask, n_source_sersic, shapelet_nmax, n_lens_sersic, source2_plane=0):
     """Flat parameter order (reading S18)."""
     n = ["theta_E"] + (["gamma"] if mass_model == 1 else []) + ["e1", "e2", "x", "y"]
     n = ["mass." + s for s in n]
@@ -78,14 +79,15 @@ def param_names(mass_model, has_shear, multipole_mask, n_source_sersic, shapelet
     if multipole_mask & 2: n += ["mp.c4", "mp.s4"]
     ser = ["R", "n", "e1", "e2", "x", "y", "I"]
     if n_source_sersic: n += ["src." + s for s in ser]
-    if n_source_sersic > 1: n += ["src2." + s for s in ser]          # second source on the same plane (S1, S2)
+    if n_source_sersic > 1: n += ["src2." + s for s in ser]          # second source (S1, S2)
+    if n_source_sersic > 1 and source2_plane: n += ["src2.eta"]      # ... on its own plane: deflection scale eta2 (S23)
     if shapelet_nmax >= 0: n += ["shp.beta"] + ["shp.a%d" % i for i in range(n_shapelet_coef(shapelet_nmax))]
     for k in range(n_lens_sersic): n += ["ll%d." % k + s for s in ser]
     return n
 
 
 # ------------------------------------------------------------------ priors of each config
-def _default_priors(mass_model, multipoles=False, shapelet_nmax=-1, n_lens=1, n_src=1):
+def _default_priors(mass_model, multipoles=False, shapelet_nmax=-1, n_lens=1, n_src=1, src2_plane=False):
     """SURVEY 8(d) fill-ins for configs 1, 2, 3, 5 (BJ configs[0..2], [4])."""
     p = [Uniform(0.8, 1.5)]
     if mass_model == 1: p += [Uniform(1.6, 2.4)]
@@ -97,6 +99,7 @@ def _default_priors(mass_model, multipoles=False, shapelet_nmax=-1, n_lens=1, n_
     if n_src > 1:
         p += [Uniform(0.1, 0.5), Uniform(1, 4), Normal(0, 0.15), Normal(0, 0.15), Normal(0.3, 0.2), Normal(-0.2, 0.2),
               LogUniform(1, 100)]
+        if src2_plane: p += [Uniform(0.6, 1.6)]                      # eta2: ratio of the lensing efficiencies of the two planes
     if shapelet_nmax >= 0: p += [Uniform(0.05, 0.3)] + [Normal(0, 1)] * n_shapelet_coef(shapelet_nmax)
     for _ in range(n_lens):
         p += [Uniform(0.5, 1.5), Uniform(2, 6), TruncNormal(0, 0.1, -0.15, 0.15), TruncNormal(0, 0.1, -0.15, 0.15),
@@ -145,7 +148,7 @@ def make_spec(k, **over):
     for a, v in over.items():
         setattr(s, a, v)
     s.names = param_names(s.mass_model, s.has_shear, s.multipole_mask, s.n_source_sersic, s.shapelet_nmax,
-                          s.n_lens_sersic)
+                          s.n_lens_sersic, s.source2_plane)
     assert len(s.names) == s.n_params, (len(s.names), s.n_params)
     return s
 
