@@ -75,7 +75,7 @@ typedef enum { GL_PRECISION_F64 = 0, GL_PRECISION_F32 = 1 } gl_precision;
 
 /* Model configuration.  The flat parameter vector has the block order of reading S18:
  *   main mass [theta_E, (gamma if EPL), e1, e2, x, y] . shear [g1, g2] . multipoles [c3, s3][c4, s4] .
- *   source Sersic 1 [R, n, e1, e2, x, y, I] . source Sersic 2 (same source plane) . shapelets [beta_s, a_0 .. a_{Nc-1}] .
+ *   source Sersic 1 [R, n, e1, e2, x, y, I] . source Sersic 2 [same 7, then eta2 if source2_plane] . shapelets [beta_s, a_0 .. a_{Nc-1}] .
  *   lens Sersic 1 . lens Sersic 2 . lens Sersic 3                       (absent blocks take no entries)
  * with Nc = (nmax+1)(nmax+2)/2 coefficients ordered by n1+n2 then n2 (O5, S9); the shapelet centre is the
  * first source Sersic's centre, so shapelets require n_source_sersic >= 1. */
@@ -110,6 +110,11 @@ typedef struct {
                                     normal matrix is not positive definite gets logp = -INF.  Needs noise_model 0
                                     (else GL_ERR_UNSUPPORTED).  In gl_model_image, which has no obs to invert, the
                                     amplitude entries ARE the amplitudes, untransformed. */
+    int32_t source2_plane;    /* 0: both source Sersics on one source plane; 1 (needs n_source_sersic = 2): the second one
+                                 on its OWN plane ("multi-source-plane systems"; NEXT-4, reading S23): its rays are
+                                 deflected by eta2 * alpha(theta), beta_2 = theta - eta2 alpha, with eta2 (the ratio of the
+                                 lensing efficiencies D_ls / D_s of the two planes; the first source carries no mass) one
+                                 more SAMPLED parameter directly after the second source's block */
     const gl_prior* priors;   /* HOST pointer, n_params entries, copied by gl_config_create */
 } gl_config_desc;
 

@@ -51,7 +51,8 @@ class gl_config_desc(C.Structure):
                 ("multipole_mask", C.c_int32), ("n_source_sersic", C.c_int32), ("shapelet_nmax", C.c_int32),
                 ("n_lens_sersic", C.c_int32), ("param_space", C.c_int32), ("n_systems", C.c_int32),
                 ("n_params", C.c_int32), ("precision", C.c_int32), ("noise_model", C.c_int32),
-                ("exposure_time", C.c_float), ("amplitude_mode", C.c_int32), ("priors", C.POINTER(gl_prior))]
+                ("exposure_time", C.c_float), ("amplitude_mode", C.c_int32), ("source2_plane", C.c_int32),
+                ("priors", C.POINTER(gl_prior))]
 
 
 _lib = None
@@ -142,7 +143,8 @@ def gl_config_create(spec):
                        spec.multipole_mask, spec.n_source_sersic, spec.shapelet_nmax, spec.n_lens_sersic,
                        spec.param_space, spec.n_systems, int(getattr(spec, "n_params", n)),
                        int(getattr(spec, "precision", GL_PRECISION_F64)), int(getattr(spec, "noise_model", 0)),
-                       float(getattr(spec, "t_exp", 1.0)), int(getattr(spec, "amplitude_mode", 0)), pri)
+                       float(getattr(spec, "t_exp", 1.0)), int(getattr(spec, "amplitude_mode", 0)),
+                       int(getattr(spec, "source2_plane", 0)), pri)
     h = C.c_void_p()
     _check(lib().gl_config_create(C.byref(d), C.byref(h)), "gl_config_create")
     return h

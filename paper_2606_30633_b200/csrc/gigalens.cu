@@ -135,6 +135,7 @@ static int layout_from_desc(const gl_config_desc& d, Layout& L) {
     if (d.multipole_mask & 2) { L.mp4 = k; k += 2; } else L.mp4 = -1;
     if (d.n_source_sersic > 0) { L.src = k; k += 7; } else L.src = -1;
     if (d.n_source_sersic > 1) { L.src1 = k; k += 7; } else L.src1 = -1;
+    if (d.n_source_sersic > 1 && d.source2_plane) { L.eta2 = k; k += 1; } else L.eta2 = -1;
     L.nmax = d.shapelet_nmax; L.n_coef = 0;
     if (d.shapelet_nmax >= 0) { L.n_coef = (d.shapelet_nmax + 1) * (d.shapelet_nmax + 2) / 2; L.shp = k; k += 1 + L.n_coef; } else L.shp = -1;
     if (d.n_lens_sersic >= 1) { L.ll0 = k; k += 7; } else L.ll0 = -1;
@@ -162,6 +163,8 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     if (d->noise_model != 0 && d->noise_model != 1) return GL_ERR_BAD_CONFIG;
     if (d->noise_model == 1 && !(d->exposure_time > 0.f && std::isfinite(d->exposure_time))) return GL_ERR_BAD_CONFIG;
     if (d->amplitude_mode != 0 && d->amplitude_mode != 1) return GL_ERR_BAD_CONFIG;
+    if (d->source2_plane != 0 && d->source2_plane != 1) return GL_ERR_BAD_CONFIG;
+    if (d->source2_plane == 1 && d->n_source_sersic < 2) return GL_ERR_BAD_CONFIG;
     if (d->amplitude_mode == 1 && d->noise_model != 0) return GL_ERR_UNSUPPORTED;     // chi^2 must be quadratic in the amplitudes
     Layout L{};
     int np = layout_from_desc(*d, L);

@@ -47,7 +47,8 @@ enum : int {
 // C, S (unscaled cos/sin phi) rotate source-plane gradients back.  The adjoint's moment sums are taken in (x', y') and
 // unscaled per particle in gl_finalize_kernel (sersic_chain).
 enum : int { SB_XOFF = 0, SB_YOFF = 1, SB_C = 2, SB_S = 3, SB_A11 = 4, SB_A12 = 5, SB_K1 = 6, SB_K0 = 7,
-             SB_C1 = 8, SB_IE = 9, SB_KQ = 10, SB_KQI = 11, SB_A21 = 12, SB_A22 = 13 };
+             SB_C1 = 8, SB_IE = 9, SB_KQ = 10, SB_KQI = 11, SB_A21 = 12, SB_A22 = 13,
+             SB_ETA = 14 };             // PB_SRC1 only: eta2, the deflection scale of the second source's plane (1 on one plane)
 
 // ----------------------------------------------------------------------------- natural accumulators (NA)
 // Per-ray sums the adjoint kernel produces; gl_finalize_kernel applies the per-particle chain rule in fp64.
@@ -60,8 +61,9 @@ enum : int {
     NA_SHB = 26, NA_SHX = 27, NA_SHY = 28,
     NA_LL0 = 29, NA_LL1 = 37,
     NA_SRC1 = 45, NA_LL2 = 53,           // second source / third lens-light block (8 each, like NA_SRC)
-    NA_SHA = 61,                         // Nc coefficient sums
-    NA_MAX = 61 + 66
+    NA_ETA = 61,                         // second source plane: -sum gbar grad_beta I_src2 . alpha  (= d logL / d eta2)
+    NA_SHA = 62,                         // Nc coefficient sums
+    NA_MAX = 62 + 66
 };
 enum : int { SA_T0 = 0, SA_T1 = 1, SA_T2 = 2, SA_AX = 3, SA_AY = 4, SA_BXX = 5, SA_BYY = 6, SA_BXY = 7 };
 

@@ -11,7 +11,7 @@ struct PriorTable {                 // passed by value as a kernel parameter (<=
 };
 
 struct Layout {                     // offsets into the flat parameter vector (reading S18); -1 = absent
-    int mass, gamma, ell, shear, mp3, mp4, src, src1, shp, ll0, ll1, ll2;
+    int mass, gamma, ell, shear, mp3, mp4, src, src1, eta2, shp, ll0, ll1, ll2;   // eta2: deflection scale of the 2nd source's plane
     int n_params, n_coef, nmax, param_space, mass_model;
     int ker_nmax;                   // shapelet order the selected kernel variant is compiled for (>= nmax)
     int amp_mode;                   // 1: light amplitudes solved by linear inversion (gl_linear.cuh); their z entries are ignored
@@ -173,6 +173,7 @@ __global__ void __launch_bounds__(UNPACK_WPB * 32) gl_unpack_kernel(const __grid
     write_sersic<T>(th, L.ll0, o + PB_LL0, x_first, ok);
     write_sersic<T>(th, L.ll1, o + PB_LL1, x_first, ok);
     write_sersic<T>(th, L.src1, o + PB_SRC1, x_first, ok);
+    o[PB_SRC1 + SB_ETA] = L.eta2 >= 0 ? (T)theta_at(th, L.eta2) : T(1);
     write_sersic<T>(th, L.ll2, o + PB_LL2, x_first, ok);
     // shapelets (coefficients pre-divided by beta_s; orders above the configured nmax are zero)
     if (L.ker_nmax >= 0) {
@@ -298,6 +299,7 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
             if (L.ll0 >= 0) sersic_chain(th, L.ll0, nat + NA_LL0, gth);
             if (L.ll1 >= 0) sersic_chain(th, L.ll1, nat + NA_LL1, gth);
             if (L.src1 >= 0) sersic_chain(th, L.src1, nat + NA_SRC1, gth);
+            if (L.eta2 >= 0) gth[L.eta2] = nat[NA_ETA];
             if (L.ll2 >= 0) sersic_chain(th, L.ll2, nat + NA_LL2, gth);
             if (L.shp >= 0) {
                 double bs = theta_at(th, L.shp);

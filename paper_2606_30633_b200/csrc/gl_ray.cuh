@@ -326,15 +326,19 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
             gbx = R::fma(sb[SB_C], Ixr, -sb[SB_S] * Iyr); gby = R::fma(sb[SB_S], Ixr, sb[SB_C] * Iyr);
         }
         if constexpr (V::NSRC >= 2) {                // second source on the same source plane (S1, S2)
+            // second source: same plane (eta2 = 1, exactly the one-plane arithmetic) or its own plane, beta_2 = theta - eta2 alpha
             const T* s1 = pb + PB_SRC1;
-            const T qx1 = R::fma(fj, step, s1[SB_XOFF]) - ax, qy1 = R::fma(fi, step, s1[SB_YOFF]) - ay;
+            const T eta = s1[SB_ETA];
+            const T qx1 = R::fma(-eta, ax, R::fma(fj, step, s1[SB_XOFF])), qy1 = R::fma(-eta, ay, R::fma(fi, step, s1[SB_YOFF]));
             SersicOut<T> o1 = sersic_eval<T, ADJ>(tb, s1, qx1, qy1);
             Iray += o1.I;
             if constexpr (COMP) { if (ci->src1 >= 0) acc[(size_t)ci->src1 * cstride] = o1.I; }
             if constexpr (ADJ) {
                 sersic_accum(o1, gbar, acc + NA_SRC1);
                 const T Ixr = -s1[SB_KQ] * o1.Iu_r2 * o1.xr, Iyr = -s1[SB_KQI] * o1.Iu_r2 * o1.yr;
-                gbx += R::fma(s1[SB_C], Ixr, -s1[SB_S] * Iyr); gby += R::fma(s1[SB_S], Ixr, s1[SB_C] * Iyr);
+                const T g1x = R::fma(s1[SB_C], Ixr, -s1[SB_S] * Iyr), g1y = R::fma(s1[SB_S], Ixr, s1[SB_C] * Iyr);
+                gbx = R::fma(eta, g1x, gbx); gby = R::fma(eta, g1y, gby);             // d beta_2 / d(mass) = -eta2 d alpha / d(mass)
+                acc[NA_ETA] = R::fma(-gbar, R::fma(g1x, ax, g1y * ay), acc[NA_ETA]);   // d beta_2 / d eta2 = -alpha
             }
         }
         if constexpr (V::NMAX >= 0) {

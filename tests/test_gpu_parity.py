@@ -421,3 +421,79 @@ def test_sie_sis_branch_strict_parity(ell, precision):
         assert rep["n_fail"] == 0, rep
     else:
         assert rep["normwise"] <= 2e-3, rep
+
+
+def _two_plane_case(n_pix, s, K, mass_model, multipoles, nmax, n_lens, seed, n_particles=6, amplitude_mode=0, source2_plane=1):
+    import oracle
+    pri = W._default_priors(mass_model, multipoles=multipoles, shapelet_nmax=nmax, n_lens=n_lens, n_src=2,
+                            src2_plane=bool(source2_plane))
+    sp = W.LensSpec(n_pix, s, K, W._r32(0.11 * 40 / n_pix * 2.4), mass_model=mass_model, multipole_mask=3 if multipoles else 0,
+                    n_source_sersic=2, shapelet_nmax=nmax, n_lens_sersic=n_lens, source2_plane=source2_plane,
+                    amplitude_mode=amplitude_mode, priors=pri)
+    sp.names = W.param_names(mass_model, 1, sp.multipole_mask, 2, nmax, n_lens, source2_plane)
+    assert len(sp.names) == sp.n_params
+    rng = np.random.default_rng(seed)
+    step = sp.pix_scale / s
+    psf = W.gaussian_psf(K, 2.5 * step, step)[None].astype(np.float32)
+    truth = oracle.model_image(sp, psf.astype(np.float64), W.draw(rng, pri, 1))
+    sigma = np.full((1, n_pix, n_pix), 0.05, np.float32)
+    obs = (truth + 0.05 * rng.standard_normal(truth.shape)).astype(np.float32)
+    z = W.z_of(pri, W.draw(rng, pri, n_particles)).astype(np.float32)
+    return sp, obs, sigma, psf, z
+
+
+@pytest.mark.parametrize("case", [(24, 2, 5, 1, False, -1, 2), (20, 2, 5, 0, False, -1, 1), (22, 2, 5, 1, True, 3, 3), (60, 4, 21, 1, False, -1, 1)])
+def test_two_source_planes_strict_parity(case):
+    """SURVEY 8(f) NEXT-4 remainder (reading S23): the second source on its own plane, beta_2 = theta - eta2 alpha,
+    eta2 sampled.  Both kernel variants that carry a second source (no shapelets / shapelets + multipoles), SIE and EPL, the
+    config-2 geometry: model image, log-posterior and every gradient component (eta2 included) at the strict bar."""
+    import oracle
+    import torch
+    gl = _gl()
+    n_pix, s, K, mass_model, mp, nmax, n_lens = case
+    sp, obs, sigma, psf, z = _two_plane_case(n_pix, s, K, mass_model, mp, nmax, n_lens, seed=7000 + n_pix)
+    ref = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), None, want_model=True)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    zt = torch.from_numpy(z).cuda()
+    lp, g = m.logpost_grad(zt)
+    img = m.model_image(zt).cpu().numpy().astype(np.float64)
+    lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+    fin = np.isfinite(ref["logp"])
+    assert fin.sum() >= 4 and np.array_equal(fin, np.isfinite(lp))
+    scale = np.abs(ref["model"][fin]).max(axis=(1, 2), keepdims=True)
+    assert np.max(np.abs(img[fin] - ref["model"][fin]) / scale) < 2e-7
+    assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+    ok, rep = grad_report(g[fin], ref["grad"][fin])
+    assert rep["n_fail"] == 0, rep
+    k_eta = sp.names.index("src2.eta")
+    assert np.all(np.abs(ref["grad"][fin][:, k_eta]) > 0)                  # the eta2 column is exercised
+
+
+def test_two_source_planes_eta_one_is_the_one_plane_model_and_backward_mode():
+    """eta2 = 1 (theta space: z of a Uniform prior at its theta = 1) reproduces the one-plane two-source model bit for bit
+    in logp and in every shared gradient component; and backward modelling (amplitude_mode 1) on two planes follows
+    oracle/linear.py at the strict bar."""
+    import dataclasses
+    import torch
+    import oracle.linear as OL
+    gl = _gl()
+    sp, obs, sigma, psf, z = _two_plane_case(24, 2, 5, 1, False, -1, 2, seed=7100)
+    k_eta = sp.names.index("src2.eta")
+    sp1 = dataclasses.replace(sp, param_space=1, priors=[W.NoPrior()] * sp.n_params)
+    th = W.theta_of(sp.priors, z.astype(np.float64)).astype(np.float32)
+    th[:, k_eta] = 1.0
+    one = dataclasses.replace(sp1, source2_plane=0, priors=[W.NoPrior()] * (sp.n_params - 1))
+    a = gl.LensModel(sp1, obs, sigma, psf).logpost_grad(torch.from_numpy(th).cuda())
+    b = gl.LensModel(one, obs, sigma, psf).logpost_grad(torch.from_numpy(np.delete(th, k_eta, axis=1)).cuda())
+    keep = [i for i in range(sp.n_params) if i != k_eta]
+    assert torch.equal(a[0], b[0]) and torch.equal(a[1][:, keep], b[1])
+    # backward mode on two planes
+    spb, obs, sigma, psf, z = _two_plane_case(22, 2, 5, 1, False, -1, 2, seed=7200, amplitude_mode=1)
+    ref = OL.logpost_grad(spb, obs, sigma, psf, z.astype(np.float64))
+    lp, g = gl.LensModel(spb, obs, sigma, psf).logpost_grad(torch.from_numpy(z).cuda())
+    lp, g = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+    fin = np.isfinite(ref["logp"])
+    assert fin.sum() >= 4 and np.array_equal(fin, np.isfinite(lp))
+    assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+    ok, rep = grad_report(g[fin], ref["grad"][fin])
+    assert rep["n_fail"] == 0, rep
