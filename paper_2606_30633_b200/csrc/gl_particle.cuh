@@ -138,79 +138,86 @@ __global__ void __launch_bounds__(UNPACK_WPB * 32) gl_unpack_kernel(const __grid
     ok = __all_sync(0xffffffffu, ok);
     for (int k = lane; k < PB_STRIDE; k += 32) o[k] = T(0);
     __syncwarp();
-    if (lane == 0) {
-    const double step = (double)pix_scale / G.s;
-    // Ray coordinates are x_j = (j - (M-1)/2) * step (O3 rewritten about the grid centre, which the ray kernels use so
-    // that position - centre keeps its RELATIVE accuracy near a component centre): the per-component offsets are -x0.
-    const double x_first = 0.0;
-    // main deflector
-    double thE = theta_at(th, L.mass);
-    double t = L.gamma >= 0 ? theta_at(th, L.gamma) - 1.0 : 1.0;
-    double e1 = theta_at(th, L.ell), e2 = theta_at(th, L.ell + 1);
-    double x0 = theta_at(th, L.ell + 2), y0 = theta_at(th, L.ell + 3);
-    if (!(thE > 0) || !(t > 0 && t < 2) || !(e1 * e1 + e2 * e2 < 1.0)) { ok = false; thE = 1; t = 1; e1 = e2 = 0; }
-    Ell E = make_ell(e1, e2);
-    double b = thE * sqrt(E.q), f = (1 - E.q) / (1 + E.q);
-    o[PB_M_XOFF] = (T)(x_first - x0); o[PB_M_YOFF] = (T)(x_first - y0);
-    o[PB_M_C] = (T)E.cphi; o[PB_M_S] = (T)E.sphi; o[PB_M_Q] = (T)E.q; o[PB_M_B] = (T)b;
-    o[PB_M_T] = (T)t; o[PB_M_F] = (T)f; o[PB_M_L2B] = (T)log2(b); o[PB_M_A] = (T)(2 * b / (1 + E.q));
-    double qp = sqrt(fmax(1 - E.q * E.q, 0.0));
-    o[PB_M_QP] = (T)qp; o[PB_M_BQP] = (T)(qp > 0 ? b / qp : 0.0);
-    o[PB_M_F2] = (T)(f * f); o[PB_M_TM1] = (T)(t - 1);
-    {   // kappa = KAPC * amp / R with amp = A (b/R)^(t-1) (the amplitude the ray kernels form in one exp2, PB_M_H1 / _H0)
-        const double A = 2 * b / (1 + E.q);
-        o[PB_M_KAPC] = (T)(0.5 * (2 - t) * b / A);
-        o[PB_M_H1] = (T)(-0.5 * (t - 1)); o[PB_M_H0] = (T)((t - 1) * log2(b) + log2(A));
+    // The derived scalars are independent per component: lanes 0-4 take one Sersic block each (absent blocks get the neutral
+    // block), lane 5 the main deflector, shear, multipoles and grid, every lane a share of the shapelet coefficients and
+    // ONE term of the series (ratios in parallel, running product / sum by a shuffle scan): a serial lane-0 version spent
+    // ~35 us per call on dependent fp64 divisions and libdevice calls, most of the latency of a small batch.
+    const double x_first = 0.0;   // ray coordinates are x_j = (j - (M-1)/2) * step about the grid centre: offsets are -x0
+    {
+        const int blk_off[5] = {L.src, L.ll0, L.ll1, L.src1, L.ll2};
+        const int blk_pb[5] = {PB_SRC, PB_LL0, PB_LL1, PB_SRC1, PB_LL2};
+        if (lane < 5) write_sersic<T>(th, blk_off[lane], o + blk_pb[lane], x_first, ok);
+        if (lane == 3) o[PB_SRC1 + SB_ETA] = L.eta2 >= 0 ? (T)theta_at(th, L.eta2) : T(1);
     }
-    o[PB_G1] = L.shear >= 0 ? (T)theta_at(th, L.shear) : T(0);
-    o[PB_G2] = L.shear >= 0 ? (T)theta_at(th, L.shear + 1) : T(0);
-    o[PB_C3] = L.mp3 >= 0 ? (T)theta_at(th, L.mp3) : T(0);
-    o[PB_S3] = L.mp3 >= 0 ? (T)theta_at(th, L.mp3 + 1) : T(0);
-    o[PB_C4] = L.mp4 >= 0 ? (T)theta_at(th, L.mp4) : T(0);
-    o[PB_S4] = L.mp4 >= 0 ? (T)theta_at(th, L.mp4 + 1) : T(0);
-    o[PB_XFIRST] = (T)x_first; o[PB_STEP] = (T)step;
-    write_sersic<T>(th, L.src, o + PB_SRC, x_first, ok);
-    write_sersic<T>(th, L.ll0, o + PB_LL0, x_first, ok);
-    write_sersic<T>(th, L.ll1, o + PB_LL1, x_first, ok);
-    write_sersic<T>(th, L.src1, o + PB_SRC1, x_first, ok);
-    o[PB_SRC1 + SB_ETA] = L.eta2 >= 0 ? (T)theta_at(th, L.eta2) : T(1);
-    write_sersic<T>(th, L.ll2, o + PB_LL2, x_first, ok);
+    double t = L.gamma >= 0 ? theta_at(th, L.gamma) - 1.0 : 1.0;
+    double e1 = theta_at(th, L.ell), e2 = theta_at(th, L.ell + 1), thE = theta_at(th, L.mass);
+    if (!(thE > 0) || !(t > 0 && t < 2) || !(e1 * e1 + e2 * e2 < 1.0)) { ok = false; thE = 1; t = 1; e1 = e2 = 0; }
+    if (lane == 5) {
+        const double step = (double)pix_scale / G.s;
+        const double x0 = theta_at(th, L.ell + 2), y0 = theta_at(th, L.ell + 3);
+        Ell E = make_ell(e1, e2);
+        double b = thE * sqrt(E.q), f = (1 - E.q) / (1 + E.q);
+        o[PB_M_XOFF] = (T)(x_first - x0); o[PB_M_YOFF] = (T)(x_first - y0);
+        o[PB_M_C] = (T)E.cphi; o[PB_M_S] = (T)E.sphi; o[PB_M_Q] = (T)E.q; o[PB_M_B] = (T)b;
+        o[PB_M_T] = (T)t; o[PB_M_F] = (T)f; o[PB_M_L2B] = (T)log2(b); o[PB_M_A] = (T)(2 * b / (1 + E.q));
+        double qp = sqrt(fmax(1 - E.q * E.q, 0.0));
+        o[PB_M_QP] = (T)qp; o[PB_M_BQP] = (T)(qp > 0 ? b / qp : 0.0);
+        o[PB_M_F2] = (T)(f * f); o[PB_M_TM1] = (T)(t - 1);
+        {   // kappa = KAPC * amp / R with amp = A (b/R)^(t-1) (the amplitude the ray kernels form in one exp2, PB_M_H1 / _H0)
+            const double A = 2 * b / (1 + E.q);
+            o[PB_M_KAPC] = (T)(0.5 * (2 - t) * b / A);
+            o[PB_M_H1] = (T)(-0.5 * (t - 1)); o[PB_M_H0] = (T)((t - 1) * log2(b) + log2(A));
+        }
+        o[PB_G1] = L.shear >= 0 ? (T)theta_at(th, L.shear) : T(0);
+        o[PB_G2] = L.shear >= 0 ? (T)theta_at(th, L.shear + 1) : T(0);
+        o[PB_C3] = L.mp3 >= 0 ? (T)theta_at(th, L.mp3) : T(0);
+        o[PB_S3] = L.mp3 >= 0 ? (T)theta_at(th, L.mp3 + 1) : T(0);
+        o[PB_C4] = L.mp4 >= 0 ? (T)theta_at(th, L.mp4) : T(0);
+        o[PB_S4] = L.mp4 >= 0 ? (T)theta_at(th, L.mp4 + 1) : T(0);
+        o[PB_XFIRST] = (T)x_first; o[PB_STEP] = (T)step;
+        if (L.mass_model == 1) {
+            // precision bands of the series (knuth_banded in gl_ray.cuh): smallest k with 30 f^k below the threshold
+            const double lf = f > 0 ? log(f) : -1e30;
+            auto first_below = [&](double thr) { double k = ceil(log(thr / 30.0) / lf); return k < 1 ? 1 : (k > 64 ? 64 : (int)k); };
+            const bool dbl = sizeof(T) == 8;
+            const int k_top = first_below(dbl ? 3e-16 : 3e-9) - 1;      // keep terms k <= kt, kt >= k_top
+            const int k_dp = dbl ? first_below(1e-4) - 1 : k_top;       // fp32 steps only above 4 M1 >= k_dp (fp64 mode)
+            int mt = (k_top - 1 + 3) / 4; if (mt < 1) mt = 1; if (mt > 7) mt = 7;
+            int m1 = (k_dp + 3) / 4; if (m1 < 1) m1 = 1; if (m1 > mt) m1 = mt;
+            o[PB_SER_M1] = (T)m1; o[PB_SER_M2] = (T)(mt - m1);
+        }
+    }
     // shapelets (coefficients pre-divided by beta_s; orders above the configured nmax are zero)
     if (L.ker_nmax >= 0) {
         double bs = 1.0;
         if (L.shp >= 0) { bs = theta_at(th, L.shp); if (!(bs > 0)) { ok = false; bs = 1; } }
-        o[PB_SHP] = (T)(1.0 / bs); o[PB_SHP + 1] = o[PB_SHP + 2] = o[PB_SHP + 3] = T(0);
-        int nck = (L.ker_nmax + 1) * (L.ker_nmax + 2) / 2;
-        for (int k = 0; k < nck; ++k)
-            o[PB_SHP_A + k] = (L.shp >= 0 && k < L.n_coef) ? (T)(theta_at(th, L.shp + 1 + k) / bs) : T(0);
+        const double ibs = 1.0 / bs;
+        if (lane == 6) { o[PB_SHP] = (T)ibs; o[PB_SHP + 1] = o[PB_SHP + 2] = o[PB_SHP + 3] = T(0); }
+        const int nck = (L.ker_nmax + 1) * (L.ker_nmax + 2) / 2;
+        for (int k = lane; k < nck; k += 32)
+            o[PB_SHP_A + k] = (L.shp >= 0 && k < L.n_coef) ? (T)(theta_at(th, L.shp + 1 + k) * ibs) : T(0);
     }
-    // EPL series coefficients: a_n = prod_{k<=n} (2k-2+t)/(2k+2-t); d_m = (m+1) a_{m+1}; e_m = L_{m+1} a_{m+1}
+    // EPL series coefficients: a_n = prod_{k<=n} (2k-2+t)/(2k+2-t); d_m = (m+1) a_{m+1}; e_m = L_{m+1} a_{m+1}, with
+    // L_n = sum_{k<=n} 4k/((2k+2-t)(2k-2+t)).  Lane n holds term n: inclusive scans over the lanes give a_n and L_n.
     if (L.mass_model == 1) {
-        double an = 1.0, Ln = 0.0;
-        o[PB_SER_A] = T(1);
-        for (int n = 1; n < 32; ++n) {
-            an *= (2.0 * n - 2.0 + t) / (2.0 * n + 2.0 - t);
-            Ln += 4.0 * n / ((2.0 * n + 2.0 - t) * (2.0 * n - 2.0 + t));
-            bool keep = n < G.n_terms;
-            o[PB_SER_A + n] = keep ? (T)an : T(0);
-            o[PB_SER_D + n - 1] = keep ? (T)(n * an) : T(0);
-            o[PB_SER_E + n - 1] = keep ? (T)(Ln * an) : T(0);
+        const double n = (double)lane;
+        double an = lane == 0 ? 1.0 : (2.0 * n - 2.0 + t) / (2.0 * n + 2.0 - t);
+        double Ln = lane == 0 ? 0.0 : 4.0 * n / ((2.0 * n + 2.0 - t) * (2.0 * n - 2.0 + t));
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const double pa_ = __shfl_up_sync(0xffffffffu, an, d), pl_ = __shfl_up_sync(0xffffffffu, Ln, d);
+            if (lane >= d) { an *= pa_; Ln += pl_; }
         }
-        o[PB_SER_D + 31] = T(0); o[PB_SER_E + 31] = T(0);
-        // precision bands of the series (knuth_banded in gl_ray.cuh): smallest k with 30 f^k below the threshold
-        const double lf = f > 0 ? log(f) : -1e30;
-        auto first_below = [&](double thr) { double k = ceil(log(thr / 30.0) / lf); return k < 1 ? 1 : (k > 64 ? 64 : (int)k); };
-        const bool dbl = sizeof(T) == 8;
-        const int k_top = first_below(dbl ? 3e-16 : 3e-9) - 1;      // keep terms k <= kt, kt >= k_top
-        const int k_dp = dbl ? first_below(1e-4) - 1 : k_top;       // fp32 steps only above 4 M1 >= k_dp (fp64 mode)
-        int mt = (k_top - 1 + 3) / 4; if (mt < 1) mt = 1; if (mt > 7) mt = 7;
-        int m1 = (k_dp + 3) / 4; if (m1 < 1) m1 = 1; if (m1 > mt) m1 = mt;
-        o[PB_SER_M1] = (T)m1; o[PB_SER_M2] = (T)(mt - m1);
+        const bool keep = lane < G.n_terms;
+        o[PB_SER_A + lane] = keep ? (T)an : T(0);
+        if (lane >= 1) {
+            o[PB_SER_D + lane - 1] = keep ? (T)(n * an) : T(0);
+            o[PB_SER_E + lane - 1] = keep ? (T)(Ln * an) : T(0);
+        } else { o[PB_SER_D + 31] = T(0); o[PB_SER_E + 31] = T(0); }
     }
+    ok = __all_sync(0xffffffffu, ok);
     if (!isfinite(lp)) ok = false;
-    o[PB_VALID] = ok ? T(1) : T(0);
-    lpd[p] = lp;
-    }   // lane 0
+    if (lane == 0) { o[PB_VALID] = ok ? T(1) : T(0); lpd[p] = lp; }
     __syncwarp();
     T* dst = pb + p * PB_STRIDE;
     for (int k = lane; k < PB_STRIDE; k += 32) dst[k] = o[k];
@@ -271,6 +278,8 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
         }
         for (int k = lane; k < L.n_params; k += 32) { gth[k] = 0; th[k] = transform_one(pt, k, L.param_space, z_in(L, z, k)).theta; }
         __syncwarp();
+        // chain rule natural -> theta, one component per lane: lane 0 the mass block, shear and multipoles, lanes 1-5 one
+        // Sersic block each; the shapelet terms that add to the first source's centre follow after a warp barrier
         if (lane == 0 && valid) {
             double thE = theta_at(th, L.mass);
             double t = L.gamma >= 0 ? theta_at(th, L.gamma) - 1.0 : 1.0;
@@ -295,17 +304,18 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
             if (L.mp3 >= 0) { gth[L.mp3] = nat[NA_C3]; gth[L.mp3 + 1] = nat[NA_S3]; }
             if (L.mp4 >= 0) { gth[L.mp4] = nat[NA_C4]; gth[L.mp4 + 1] = nat[NA_S4]; }
             if (L.mp3 >= 0 || L.mp4 >= 0) { gth[L.ell + 2] += nat[NA_MCX]; gth[L.ell + 3] += nat[NA_MCY]; }
-            if (L.src >= 0) sersic_chain(th, L.src, nat + NA_SRC, gth);
-            if (L.ll0 >= 0) sersic_chain(th, L.ll0, nat + NA_LL0, gth);
-            if (L.ll1 >= 0) sersic_chain(th, L.ll1, nat + NA_LL1, gth);
-            if (L.src1 >= 0) sersic_chain(th, L.src1, nat + NA_SRC1, gth);
             if (L.eta2 >= 0) gth[L.eta2] = nat[NA_ETA];
-            if (L.ll2 >= 0) sersic_chain(th, L.ll2, nat + NA_LL2, gth);
-            if (L.shp >= 0) {
-                double bs = theta_at(th, L.shp);
-                gth[L.shp] = -nat[NA_SHB] / bs;
-                gth[L.src + 4] -= nat[NA_SHX]; gth[L.src + 5] -= nat[NA_SHY];
-            }
+        }
+        if (lane >= 1 && lane <= 5 && valid) {
+            const int blk_off[5] = {L.src, L.ll0, L.ll1, L.src1, L.ll2};
+            const int blk_na[5] = {NA_SRC, NA_LL0, NA_LL1, NA_SRC1, NA_LL2};
+            if (blk_off[lane - 1] >= 0) sersic_chain(th, blk_off[lane - 1], nat + blk_na[lane - 1], gth);
+        }
+        __syncwarp();
+        if (lane == 0 && valid && L.shp >= 0) {
+            double bs = theta_at(th, L.shp);
+            gth[L.shp] = -nat[NA_SHB] / bs;
+            gth[L.src + 4] -= nat[NA_SHX]; gth[L.src + 5] -= nat[NA_SHY];
         }
         __syncwarp();
         if (L.shp >= 0 && valid) {

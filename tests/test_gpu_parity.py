@@ -497,3 +497,18 @@ def test_two_source_planes_eta_one_is_the_one_plane_model_and_backward_mode():
     assert np.all(np.abs(lp[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
     ok, rep = grad_report(g[fin], ref["grad"][fin])
     assert rep["n_fail"] == 0, rep
+
+
+def test_graph_replay_matches_direct_call():
+    """LensModel.capture_logpost_grad (CUDA graph of the seven kernels, for small batches): replays follow in-place updates
+    of the captured parameter tensor and are bit-identical to direct calls."""
+    gl, torch, wl, m = _model(1)
+    z = torch.from_numpy(wl.params[:64].copy()).cuda()
+    replay, lp, g = m.capture_logpost_grad(z)
+    for shift in (0.0, 0.01):
+        z.copy_(torch.from_numpy(wl.params[:64] + np.float32(shift)).cuda())
+        replay()
+        torch.cuda.synchronize()
+        m2 = gl.LensModel(wl.spec, *observation(1)[1:], wl.psf)
+        lp2, g2 = m2.logpost_grad(z)
+        assert torch.equal(lp, lp2) and torch.equal(g, g2)
