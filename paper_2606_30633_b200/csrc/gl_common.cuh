@@ -92,6 +92,8 @@ struct Geom {            // launch-invariant geometry, passed by value
     int UP;              // U rounded up to a multiple of the tap rows one conv thread handles
     int Hp, Wp;          // rows / row pitch of one padded phase plane of RAY
     int Hg, Wg, PADg;    // rows / row pitch / border of the padded GPIX image
+    int binned;          // 1 (psf_grid 1, dedicated path): step D runs on the BINNED image held in phase plane 0 and the
+                         // transpose writes plane 0 only; every plane's gbar is that plane (gl_ray_adj_kernel reads plane 0)
 };
 __host__ __device__ inline int phase_shift(const Geom& G, int a) { return (a + G.c) / G.s; }      // o_a
 __host__ __device__ inline size_t ray_stride(const Geom& G) { return (size_t)G.s * G.s * G.Hp * G.Wp; }

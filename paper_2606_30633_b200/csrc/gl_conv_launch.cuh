@@ -16,7 +16,8 @@ namespace gl {
 static inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
 struct ConvPlan {
-    int kind;                 // 0 generic, 1: U=6 CW=4, 2: U=11 CW=2, 3: U=16 CW=2 (round-1 sliding kernels), 4: tap-stationary + TMA
+    int kind;                 // 0 generic, 1: U=6 CW=4, 2: U=11 CW=2, 3: U=16 CW=2 (round-1 sliding kernels), 4: tap-stationary + TMA,
+                              // 5: psf_grid 1 dedicated: bin the planes, then tap-stationary on ONE plane with the K x K taps
     int CW;                   // output columns per thread
     SlidePlan fwd, bwd;
     size_t fwd_smem, bwd_smem;
@@ -51,6 +52,17 @@ struct TsVariant { int U, G, NPH, CW, RPS, wmax_f, wmax_b, maxt; };   // wmax: c
 #ifndef GL_TS_W16
 #define GL_TS_W16 4, 4
 #endif
+#ifndef GL_TS_W1
+#define GL_TS_W1 4, 4
+#endif
+// single-plane instances of the dedicated psf_grid = 1 path: (U = K, G, NPH = 1)
+static constexpr TsVariant k_ts1_variants[] = {{5, 1, 1, 4, 5, GL_TS_W1, 256}, {7, 1, 1, 4, 7, GL_TS_W1, 256}, {11, 2, 1, 4, 6, GL_TS_W1, 256},
+                                               {21, 8, 1, 4, 6, GL_TS_W1, 256}};     // K is odd; other K: box-expanded path
+static inline int ts1_variant(int U) {
+    for (int i = 0; i < (int)(sizeof(k_ts1_variants) / sizeof(k_ts1_variants[0])); ++i)
+        if (k_ts1_variants[i].U == U) return i;
+    return -1;
+}
 static constexpr TsVariant k_ts_variants[] = {{6, 1, 4, 4, GL_TS_RPS6, GL_TS_W6, GL_TS_MAXT6}, {6, 1, 16, 4, GL_TS_RPS6, GL_TS_W6, GL_TS_MAXT6},
                                               {11, 2, 4, GL_TS_CW11, GL_TS_RPS11, GL_TS_W11, GL_TS_MAXT11},
                                               {11, 2, 16, GL_TS_CW11, GL_TS_RPS11, GL_TS_W11, GL_TS_MAXT11},
@@ -66,7 +78,7 @@ static inline int ts_variant(int U, int NPH) {
 // Launch plan of one direction.  ncols: output columns to cover; planes_in_box: NPH (forward) or 1 (transpose);
 // pitch_rule: forward rows of different planes sit boxw apart -> boxw * esize = 16 (mod 32) keeps a quarter-warp's
 // 16-byte loads on distinct banks.
-static inline TsPlan ts_plan(const TsVariant& v, int wmax_default, int esize, int ncols, int planes_in_box, int steps, int row0) {
+static inline TsPlan ts_plan(const TsVariant& v, int wmax_default, int esize, int ncols, int planes_in_box, int steps, int row0, bool fwd) {
     TsPlan pl{};
     const int LPG = v.NPH * v.G, CGW = 32 / LPG, NU = (v.U + v.G - 1) / v.G;
     (void)NU;
@@ -92,7 +104,7 @@ static inline TsPlan ts_plan(const TsVariant& v, int wmax_default, int esize, in
     pl.stage_elems = round_up(bw * planes_in_box * v.RPS, 128 / esize);
     pl.stages = nst;
     pl.steps = steps; pl.row0 = row0;
-    pl.pbuf_elems = planes_in_box > 1 ? ts_pbuf_elems(v.NPH, v.G, v.CW, v.RPS) : 0;
+    pl.pbuf_elems = fwd ? ts_pbuf_elems(v.NPH, v.G, v.CW, v.RPS) : 0;
     return pl;
 }
 
@@ -117,6 +129,22 @@ static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems) {
     int wg = N + 2 * (U - 1);
     if (wg < CW * (ncg_b - 1) + SEG) wg = CW * (ncg_b - 1) + SEG;
     G.Wg = round_up(wg, 4);
+    G.binned = 0;
+    {   // psf_grid 1: the dedicated bin-then-convolve path wherever a single-plane instance exists (GL_CONV_BIN=0: box-expanded)
+        const char* e = std::getenv("GL_CONV_BIN");
+        const int id = G.pgrid == 1 ? ts1_variant(U) : -1;
+        if (id >= 0 && !(e && e[0] == '0')) {
+            const TsVariant& v = k_ts1_variants[id];
+            const int NU = (v.U + v.G - 1) / v.G, UPAD = NU * v.G, o = G.c / G.s;     // every plane has the shift o = (K - 1) / 2
+            TsPlan tf = ts_plan(v, v.wmax_f, esize, N, 1, N + UPAD - 1, 0, true);
+            TsPlan tb = ts_plan(v, v.wmax_b, esize, N + o, 1, N + UPAD - 1, o, false);
+            if (tf.boxw <= 256 && tb.boxw <= 256 && v.CW * tb.ncg <= G.Wp) {
+                pl.kind = 5; pl.ts_id = id; pl.CW = v.CW; pl.tf = tf; pl.tb = tb; pl.n_ctile = tf.n_bands * tf.wpc;
+                G.binned = 1;
+                return pl;
+            }
+        }
+    }
     if (pl.kind == 0) {
         pl.n_ctile = (N * N + 255) / 256;
         return pl;
@@ -131,8 +159,8 @@ static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems) {
             const TsVariant& v = k_ts_variants[id];
             const int NU = (v.U + v.G - 1) / v.G, UPAD = NU * v.G;
             const int omin = G.c / G.s, omax = (G.s - 1 + G.c) / G.s;
-            TsPlan tf = ts_plan(v, v.wmax_f, esize, N, NPH, N + UPAD - 1, 0);
-            TsPlan tb = ts_plan(v, v.wmax_b, esize, N + ob_max, 1, N + (omax - omin) + UPAD - 1, omin);
+            TsPlan tf = ts_plan(v, v.wmax_f, esize, N, NPH, N + UPAD - 1, 0, true);
+            TsPlan tb = ts_plan(v, v.wmax_b, esize, N + ob_max, 1, N + (omax - omin) + UPAD - 1, omin, false);
             if (tf.boxw <= 256 && tb.boxw <= 256 && (tf.wpc + 1) * 32 <= v.maxt && (tb.wpc + 1) * 32 <= v.maxt &&
                 v.CW * tb.ncg <= G.Wp) {
                 pl.kind = 4; pl.ts_id = id; pl.CW = v.CW; pl.tf = tf; pl.tb = tb; pl.n_ctile = tf.n_bands * tf.wpc;
@@ -275,10 +303,13 @@ static inline cudaError_t conv_fwd_ts_launch(const ConvPlan& pl, const Geom& G, 
                                              const float* obs, const int32_t* system_id, int64_t p_base, int64_t Pc, T* gpix,
                                              T* chi, float* out_model, cudaStream_t st) {
     CUtensorMap tm;
-    // plane index in the middle: {Wp, NPH * Pc (stride Hp Wp), Hp (stride Wp)} -> a box lands as [RPS][NPH][boxw]
-    if (!ts_make_map<T>(&tm, ray, (uint64_t)G.Wp, (uint64_t)NPH * (uint64_t)Pc, (uint64_t)G.Hp, (uint64_t)G.Hp * G.Wp, (uint64_t)G.Wp,
+    // plane index in the middle: {Wp, NPH * Pc (stride Hp Wp), Hp (stride Wp)} -> a box lands as [RPS][NPH][boxw];
+    // binned path (NPH = 1): plane 0 of every particle, one ray_stride apart
+    const uint64_t pstride = G.binned ? (uint64_t)ray_stride(G) : (uint64_t)G.Hp * G.Wp;
+    if (!ts_make_map<T>(&tm, ray, (uint64_t)G.Wp, (uint64_t)NPH * (uint64_t)Pc, (uint64_t)G.Hp, pstride, (uint64_t)G.Wp,
                         (uint32_t)pl.tf.boxw, NPH, RPS))
         return cudaErrorInvalidValue;
+    if (G.binned) gl_bin_planes_kernel<T><<<dim3((unsigned)(((size_t)G.Hp * G.Wp + 255) / 256), (unsigned)Pc), 256, 0, st>>>(G, const_cast<T*>(ray));
     auto kern = gl_conv_fwd_ts<T, U, G_, NPH, CW, RPS>;
     const size_t smem = ts_smem_bytes<T>(pl.tf);
     unsigned grid = 0;
@@ -311,6 +342,14 @@ static inline cudaError_t conv_bwd_ts_launch(const ConvPlan& pl, const Geom& G, 
         default: e = CALL(16, 8, 4, GL_TS_CW16, GL_TS_RPS16); break;                                               \
     }
 
+#define GL_TS1_DISPATCH(CALL)                                                                                      \
+    switch (pl.ts_id) {                                                                                            \
+        case 0: e = CALL(5, 1, 1, 4, 5); break;                                                                    \
+        case 1: e = CALL(7, 1, 1, 4, 7); break;                                                                    \
+        case 2: e = CALL(11, 2, 1, 4, 6); break;                                                                   \
+        default: e = CALL(21, 8, 1, 4, 6); break;                                                                  \
+    }
+
 // Step D + E.  Returns the number of kernels launched (negative on a CUDA error).
 template <class T>
 static inline int conv_fwd_launch(const ConvPlan& pl, const Geom& G, const T* ray, const T* sys_kt, const T* sys_w,
@@ -324,8 +363,12 @@ static inline int conv_fwd_launch(const ConvPlan& pl, const Geom& G, const T* ra
         case 4: {
 #define GL_TS_F(U_, G__, NPH_, CW_, RPS_) conv_fwd_ts_launch<T, U_, G__, NPH_, CW_, RPS_>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st)
             GL_TS_DISPATCH(GL_TS_F)
-#undef GL_TS_F
             break;
+        }
+        case 5: {
+            GL_TS1_DISPATCH(GL_TS_F)
+#undef GL_TS_F
+            return e == cudaSuccess ? 2 : -1;          // bin + step D
         }
         default: {
             dim3 grid((G.N * G.N + 255) / 256, (unsigned)Pc);
@@ -347,6 +390,10 @@ static inline int conv_bwd_launch(const ConvPlan& pl, const Geom& G, const T* gp
         case 4: {
 #define GL_TS_B(U_, G__, NPH_, CW_, RPS_) conv_bwd_ts_launch<T, U_, G__, NPH_, CW_, RPS_>(pl, G, gpix, sys_kt, system_id, p_base, Pc, gbar, st)
             GL_TS_DISPATCH(GL_TS_B)
+            break;
+        }
+        case 5: {
+            GL_TS1_DISPATCH(GL_TS_B)
 #undef GL_TS_B
             break;
         }

@@ -144,7 +144,7 @@ __device__ __forceinline__ void ts_row_step(T (&A)[NU][CW], const T (&tap)[NU][U
 #define GL_TS_MINB16 2
 #endif
 constexpr int GL_TS_MAXT = 288;       // largest block of any instance (plan check)
-template <int U> __host__ __device__ constexpr int ts_maxt() { return U == 6 ? GL_TS_MAXT6 : (U == 11 ? GL_TS_MAXT11 : GL_TS_MAXT16); }
+template <int U> __host__ __device__ constexpr int ts_maxt() { return U == 6 ? GL_TS_MAXT6 : (U == 11 ? GL_TS_MAXT11 : (U == 16 ? GL_TS_MAXT16 : 256)); }
 template <int U> __host__ __device__ constexpr int ts_minb() { return U == 16 ? GL_TS_MINB16 : 1; }
 
 // Shared-memory carve-up: ring [stages][stage_elems] T | full[stages], empty[stages] mbarriers
@@ -154,7 +154,8 @@ template <class T> __host__ __device__ inline size_t ts_smem_bytes(const TsPlan&
 }
 // forward kernel: per-warp buffer of per-plane partial rows of one fill, [RPS][CGW * CW][NPH + 2] (plane index fastest;
 // the + 2 makes the 16-byte reads of the plane sums and the 8-byte writes of the partials bank-conflict free)
-__host__ __device__ constexpr int ts_pbuf_elems(int NPH, int G, int CW, int RPS) { return RPS * (32 / (NPH * G)) * CW * (NPH + 2); }
+__host__ __device__ constexpr int ts_pj(int NPH) { return NPH == 1 ? 1 : NPH + 2; }
+__host__ __device__ constexpr int ts_pbuf_elems(int NPH, int G, int CW, int RPS) { return RPS * (32 / (NPH * G)) * CW * ts_pj(NPH); }
 
 // Step E for one pixel from values already in registers (ob = obs, w = 1 / sigma^2, or sigma^2 with noise_model 1):
 // returns the chi^2 term, g = d(-chi^2 / 2 [- ln v / 2]) / d model.  Same arithmetic as pixel_epilogue (gl_conv.cuh).
@@ -170,6 +171,20 @@ __device__ __forceinline__ T ts_pixel_terms(const Geom& G, T m, float ob, T w, T
     }
     g = -r * w;
     return r * r * w;
+}
+
+// psf_grid 1, dedicated path: the PSF acts at the pixel scale on the BINNED image, and with the
+// half-width s (K - 1) / 2 every phase plane has the same shift, so binning is the element-wise sum of the s*s padded planes:
+// plane 0 += planes 1 .. NPH - 1 (fixed order).  grid = (ceil(Hp Wp / 256), n_images), block = 256.
+template <class T>
+__global__ void __launch_bounds__(256) gl_bin_planes_kernel(const __grid_constant__ Geom Gm, T* __restrict__ ray) {
+    const size_t plane = (size_t)Gm.Hp * Gm.Wp;
+    const size_t e = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (e >= plane) return;
+    T* p0 = ray + (size_t)blockIdx.y * ray_stride(Gm) + e;
+    T sum = p0[0];
+    for (int ph = 1; ph < Gm.s * Gm.s; ++ph) sum += p0[(size_t)ph * plane];
+    p0[0] = sum;
 }
 
 // ----------------------------------------------------------------------------- step D + E
@@ -228,7 +243,7 @@ __global__ void __launch_bounds__((ts_maxt<U>()), (ts_minb<U>())) gl_conv_fwd_ts
     T tap[NU][U];
     int cur_sys = -1;
     const T* my = ring + (size_t)j * pl.boxw + CW * cgl;           // this lane's window: row 0 of stage 0
-    constexpr int PJ = NPH + 2;
+    constexpr int PJ = ts_pj(NPH);
     T* pbuf = reinterpret_cast<T*>(empty + pl.stages) + (size_t)warp * pl.pbuf_elems;     // this warp's partial-row buffer
     T* pb_w = pbuf + (size_t)cgw * CW * PJ + j;                                           // + (i CGW CW + q) PJ
     int st = 0; uint32_t ph = 0;
@@ -256,9 +271,10 @@ __global__ void __launch_bounds__((ts_maxt<U>()), (ts_minb<U>())) gl_conv_fwd_ts
         constexpr int NOUT = (RPS * CGW * CW + 31) / 32;           // outputs of a fill per lane
         for (int f = 0; f < F; ++f) {
             // step-E operands of this lane's outputs of the fill: loaded now, used after the FMAs
-            float ob_r[NOUT]; T w_r[NOUT];
+            constexpr bool PFE = NOUT <= 4;                          // many outputs per lane (single-plane instances): load at use
+            float ob_r[PFE ? NOUT : 1]; T w_r[PFE ? NOUT : 1];
 #pragma unroll
-            for (int k = 0; k < NOUT; ++k) {
+            for (int k = 0; k < (PFE ? NOUT : 0); ++k) {
                 const int o = lane + 32 * k, i = o / (CGW * CW), c = o - i * (CGW * CW);
                 const int prow = f * RPS + i - (UPAD - 1), pc = CW * cg0 + c;
                 const bool ok = o < RPS * CGW * CW && prow >= 0 && prow < N && pc < N && gp_img != nullptr;
@@ -287,10 +303,17 @@ __global__ void __launch_bounds__((ts_maxt<U>()), (ts_minb<U>())) gl_conv_fwd_ts
                 const int o = lane + 32 * k, i = o / (CGW * CW), c = o - i * (CGW * CW);
                 const int prow = f * RPS + i - (UPAD - 1), pc = CW * cg0 + c;
                 const bool ok = o < RPS * CGW * CW && prow >= 0 && prow < N && pc < N;
-                const float ob = ob_r[k]; const T w = w_r[k];
+                float ob; T w;
+                if constexpr (PFE) { ob = ob_r[k]; w = w_r[k]; }
+                else {
+                    const bool ld = ok && gp_img != nullptr;
+                    ob = ld ? obs[(size_t)sys * NN + (size_t)prow * N + pc] : 0.f;
+                    w = ld ? sys_w[(size_t)sys * NN + (size_t)prow * N + pc] : T(0);
+                }
                 const T* src = pbuf + (size_t)(o < RPS * CGW * CW ? o : 0) * PJ;
                 T m = T(0);
-                if constexpr (sizeof(T) == 8) {
+                if constexpr (NPH == 1) m = src[0];
+                else if constexpr (sizeof(T) == 8) {
 #pragma unroll
                     for (int jj = 0; jj < NPH; jj += 2) { const double2 x = *reinterpret_cast<const double2*>(src + jj); m += x.x; m += x.y; }
                 } else {

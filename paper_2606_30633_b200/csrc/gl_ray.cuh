@@ -606,7 +606,7 @@ __global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC 
     const typename Real<T>::Tab tb = TabStage<T>::make(tabs, tabg);
     __syncthreads();
     PlaneIter it(G, n_chunk, RPT);
-    const T* gb = gbar + (size_t)p * ray_stride(G) + (size_t)it.ph * G.Hp * G.Wp;
+    const T* gb = gbar + (size_t)p * ray_stride(G) + (size_t)(G.binned ? 0 : it.ph) * G.Hp * G.Wp;   // binned: one gbar plane for all
     const int NN = G.N * G.N;
     constexpr bool CS = coef_split<T, V>();
     constexpr int NREG = CS ? NA_SHA : V::NA;                     // accumulators of this kernel (all in registers)
@@ -655,7 +655,7 @@ __global__ void __launch_bounds__(NT) gl_shp_coef_kernel(const __grid_constant__
     __syncthreads();
     PlaneIter it(G, n_chunk, RPT);
     const size_t rs = ray_stride(G), pl = (size_t)it.ph * G.Hp * G.Wp;
-    const T* gb = gbar + (size_t)p * rs + pl;
+    const T* gb = gbar + (size_t)p * rs + (G.binned ? 0 : pl);
     const T* ub = uv + (size_t)p * 2 * rs + pl;
     const int NN = G.N * G.N;
     T acc[NC];

@@ -267,11 +267,13 @@ def test_truncated_series_matches_truncated_oracle():
     assert np.max(np.abs(refc["logp"] - ref8["logp"]) / np.abs(refc["logp"])) > 1e-6      # the truncation is visible
 
 
-@pytest.mark.parametrize("shape", [(12, 2, 5), (14, 4, 11), (16, 2, 11), (9, 3, 3), (10, 1, 7)])
+@pytest.mark.parametrize("shape", [(12, 2, 5), (14, 4, 11), (16, 2, 11), (9, 3, 3), (10, 1, 7), (60, 4, 21), (33, 2, 7), (21, 4, 9),
+                                   (3, 2, 11)])
 def test_detector_grid_psf_strict_parity(shape):
-    """SURVEY 8(f) NEXT-4, psf_grid = 1 (bin, then convolve with a PSF sampled at the pixel scale): the CUDA path runs it
-    as the same stride-s correlation with the box-expanded kernel; strict bar against the oracle's literal
-    bin-then-convolve, model image included.  (14,4,11) and (16,2,11) take the tuned U = 11 kernels, the rest the generic."""
+    """SURVEY 8(f) NEXT-4, psf_grid = 1 (bin, then convolve with a PSF sampled at the pixel scale).  K = 5, 7, 11, 21 take the
+    dedicated path (gl_bin_planes_kernel sums the s*s phase planes, then the single-plane tap-stationary kernels apply the
+    K x K taps: s*s fewer FMAs; (60, 4, 21) is the config-2 geometry, (10, 1, 7) has s = 1), K = 3 and 9 the box-expanded
+    stride-s correlation on the generic kernels; strict bar against the oracle's literal bin-then-convolve, model image included."""
     import oracle
     import torch
     gl = _gl()
