@@ -590,8 +590,11 @@ __global__ void __launch_bounds__(NT) gl_ray_comp_kernel(const __grid_constant__
 #ifndef GL_ADJ_MINB_X
 #define GL_ADJ_MINB_X 3     // two sources / three lens blocks, no shapelets (61 fp64 sums): 168 registers
 #endif
+#ifndef GL_ADJ_MINB_S
+#define GL_ADJ_MINB_S 1     // shapelet variants in fp64
+#endif
 template <class T, class V, int NT>
-__global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC < 2 && V::NLL < 3 ? GL_ADJ_MINB : (sizeof(T) == 8 && V::NMAX < 0 ? GL_ADJ_MINB_X : 1))) gl_ray_adj_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
+__global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC < 2 && V::NLL < 3 ? GL_ADJ_MINB : (sizeof(T) == 8 && V::NMAX < 0 ? GL_ADJ_MINB_X : (sizeof(T) == 8 ? GL_ADJ_MINB_S : 1)))) gl_ray_adj_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
                                                         const double* __restrict__ tabg, const T* __restrict__ gbar,
                                                         T* __restrict__ nap, T* __restrict__ uv, int RPT, int n_chunk) {
     __shared__ __align__(16) T pb[PB_STRIDE];
@@ -640,6 +643,12 @@ __global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC 
     }
 }
 
+#ifndef GL_COEF_NS
+#define GL_COEF_NS 8
+#endif
+__device__ __forceinline__ void coef_cp8(void* smem_dst, const void* gsrc) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
 // Shapelet coefficient sums of step F in the split form (coef_split): nap[..][NA_SHA + k] = sum_rays gbar phi_n1(u) phi_n2(v),
 // k = (n1 + n2)(n1 + n2 + 1)/2 + n2, from the (u, v) gl_ray_adj_kernel stored.  Same grid, block and ray <-> thread mapping as
 // that kernel, so both write the same partial slot of nap; fixed-order warp / CTA reduction, no atomics.
@@ -648,8 +657,10 @@ __global__ void __launch_bounds__(NT) gl_shp_coef_kernel(const __grid_constant__
                                                          const double* __restrict__ tabg, const T* __restrict__ gbar,
                                                          const T* __restrict__ uv, T* __restrict__ nap, int RPT, int n_chunk) {
     constexpr int NC = (NMAX + 1) * (NMAX + 2) / 2;
+    constexpr int NS = GL_COEF_NS;                              // cp.async ring depth (rays in flight per thread)
     __shared__ __align__(128) double tabs[TabStage<T>::N];
     __shared__ T red[NT / 32][NC];
+    __shared__ __align__(16) T stg[NS][3][NT];
     const int p = blockIdx.y;
     const typename Real<T>::Tab tb = TabStage<T>::make(tabs, tabg);
     __syncthreads();
@@ -662,25 +673,31 @@ __global__ void __launch_bounds__(NT) gl_shp_coef_kernel(const __grid_constant__
 #pragma unroll
     for (int k = 0; k < NC; ++k) acc[k] = T(0.);
     if (pbg[(size_t)p * PB_STRIDE + PB_VALID] != T(0.)) {
-        // (gbar, u, v) of the next NQ rays are in flight while one ray is worked on: the kernel holds ~220 registers
-        // (2 warps per scheduler), so the HBM latency has to be covered inside the thread.  A ring of NQ register slots
-        // indexed at compile time (a shifted queue would read the newest load one iteration after it was issued).
-        constexpr int NQ = 4;
-        T gq[NQ], uq[NQ], vq[NQ];
+        // (gbar, u, v) of the next NS rays of this thread are in flight as 8-byte cp.async copies into a shared-memory
+        // ring of its own slots: the kernel holds ~230 registers (2 warps per scheduler), so the HBM latency has to be
+        // covered by the thread itself (config 5, ms per step: 29.9 without prefetch, 21.6 / 18.5 with 4 / 8 register slots,
+        // 17.9 with this ring at depth 8; depth 12 costs a resident CTA and is slower).  A thread reads only what it copied:
+        // no CTA barrier.
         PlaneIter ld = it;
-        auto fetch = [&](int slot_ray, T& g, T& u, T& v) {
-            const bool ok = ld.idx < NN && slot_ray < RPT;
-            const size_t o = ok ? ld.offset(G) : 0;
-            g = ok ? gb[o] : T(0.); u = ok ? ub[o] : T(0.); v = ok ? ub[rs + o] : T(0.);
+        auto fetch = [&](int k, int ray) {
+            const bool ok = ld.idx < NN && ray < RPT;
+            T* d = &stg[k][0][threadIdx.x];
+            if (ok) {
+                const size_t o = ld.offset(G);
+                coef_cp8(d, gb + o); coef_cp8(d + NT, ub + o); coef_cp8(d + 2 * NT, ub + rs + o);
+            } else { d[0] = T(0.); d[NT] = T(0.); d[2 * NT] = T(0.); }     // gbar = 0: such a ray adds nothing
+            asm volatile("cp.async.commit_group;" ::: "memory");
             ld.next(G);
         };
 #pragma unroll
-        for (int k = 0; k < NQ; ++k) fetch(k, gq[k], uq[k], vq[k]);
-        for (int r0 = 0; r0 < RPT; r0 += NQ) {
+        for (int k = 0; k < NS; ++k) fetch(k, k);
+        for (int r0 = 0; r0 < RPT; r0 += NS) {
 #pragma unroll
-            for (int k = 0; k < NQ; ++k) {
-                const T g = gq[k], u = uq[k], v = vq[k];            // gbar = 0 beyond the plane: such a ray adds nothing
-                fetch(r0 + k + NQ, gq[k], uq[k], vq[k]);
+            for (int k = 0; k < NS; ++k) {
+                asm volatile("cp.async.wait_group %0;" ::"n"(NS - 1) : "memory");
+                const T* d = &stg[k][0][threadIdx.x];
+                const T g = d[0], u = d[NT], v = d[2 * NT];
+                fetch(k, r0 + k + NS);
                 T fu[NMAX + 1], fv[NMAX + 1];
                 hermite<T, NMAX>(tb, u, fu); hermite<T, NMAX>(tb, v, fv);
 #pragma unroll
@@ -694,6 +711,7 @@ __global__ void __launch_bounds__(NT) gl_shp_coef_kernel(const __grid_constant__
                 }
             }
         }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
 #pragma unroll
