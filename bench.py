@@ -267,7 +267,7 @@ def stage_profile(gl, step, flush, reps):
 
 
 def roofline_record(workmodel, sp, k, precision, P, evals_per_particle, stage_ms, stage_n, ms_per_step, bands, mhz_max,
-                    peak_src, sm_mhz=None):
+                    peak_src, sm_mhz=None, evals_in_stage_times=None):
     """The `roofline` object of the contract for the dominant kernel of a measured step.
     frac          executed-band work: only the series steps that run in the arithmetic type are credited (bands)
     frac_fixed30  the fixed 30-term formulation (every term credited to the arithmetic type's pipe): the round-1 figure
@@ -279,7 +279,9 @@ def roofline_record(workmodel, sp, k, precision, P, evals_per_particle, stage_ms
     wmb = workmodel.per_eval(sp, precision, bands[:2]) if bands else wm30
     dom = max(stage_ms, key=stage_ms.get)
     dom_t = stage_ms[dom] * 1e-3
-    rate = lambda ops: ops * P * evals_per_particle / dom_t / 1e12 if dom_t > 0 else 0.0
+    # the stage timer holds the LAST gl_logpost_grad of a step (an HMC transition makes several: one of them is timed)
+    n_st = evals_per_particle if evals_in_stage_times is None else evals_in_stage_times
+    rate = lambda ops: ops * P * n_st / dom_t / 1e12 if dom_t > 0 else 0.0
     achieved = rate(wmb.get(dom, 0))
     t_step = ms_per_step * 1e-3
     r = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "T %s lane-op/s (FMA=1)" % pipe,
@@ -296,7 +298,7 @@ def roofline_record(workmodel, sp, k, precision, P, evals_per_particle, stage_ms
          "step_frac": wmb["total_fwd_grad"] * P * evals_per_particle / t_step / 1e12 / peak,
          "step_frac_fixed30": wm30["total_fwd_grad"] * P * evals_per_particle / t_step / 1e12 / peak,
          "step_algorithmic_laneops_per_eval": wmb["total_fwd_grad"],
-         "per_stage_frac": {s: round(wmb[s] * P * evals_per_particle / (stage_ms[s] * 1e-3) / 1e12 / peak, 4)
+         "per_stage_frac": {s: round(wmb[s] * P * n_st / (stage_ms[s] * 1e-3) / 1e12 / peak, 4)
                             for s in ("ray_fwd", "conv_chi2", "conv_transpose", "ray_adjoint")
                             if s in wmb and stage_ms.get(s, 0) > 0}}
     if precision == "f64":
@@ -508,7 +510,7 @@ def run_ours(a):
     mhz_max, peak_src = _peaks()
     clocks = sampler.summary()
     roof = roofline_record(workmodel, sp, k, a.precision, P, evals_per_particle, stage_ms, stage_n, t_dev / a.steps * 1e3, bands,
-                           mhz_max, peak_src, clocks.get("sm_mhz"))
+                           mhz_max, peak_src, clocks.get("sm_mhz"), evals_in_stage_times=1 if a.stage == "hmc" else None)
     probe = {}
     for kind, name in ((0, "fp32_fma"), (1, "fp64_fma"), (2, "mufu_ex2"), (4, "fp64_fma_distinct_operands"),
                        (5, "fp64_mma_m8n8k4"), (6, "fp64_mma_plus_fma")):

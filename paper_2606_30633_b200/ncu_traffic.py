@@ -22,7 +22,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 STAGE_OF = (("gl_ray_fwd_kernel", "ray_fwd"), ("gl_ray_comp_kernel", "ray_fwd"), ("gl_conv_fwd", "conv_chi2"),
             ("gl_conv_bwd", "conv_transpose"), ("gl_ray_adj_kernel", "ray_adjoint"), ("gl_unpack_kernel", "unpack_prior"),
             ("gl_finalize_kernel", "finalize"), ("gl_prep_kernel", "prep"), ("gl_amp_solve_kernel", "amplitude_solve"),
-            ("gl_pix_conv", "conv_chi2"))
+            ("gl_shp_coef_kernel", "ray_adjoint_coef"), ("gl_bin_planes_kernel", "bin_planes"))
 SHOW = ["gpu__time_duration.sum", "launch__registers_per_thread", "launch__block_size", "launch__grid_size",
         "launch__occupancy_limit_registers", "launch__occupancy_limit_shared_mem", "launch__occupancy_limit_warps",
         "sm__warps_active.avg.pct_of_peak_sustained_active", "sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active",
