@@ -191,12 +191,12 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     }
     {   // light amplitudes in the flat order S18 and their PB slots
         AmpMap& A = c->amp; A.n = 0;
-        auto add = [&](int pb_off, int shp) { A.off[A.n] = (short)pb_off; A.shp[A.n] = (unsigned char)shp; ++A.n; };
+        auto add = [&](int pb_off, int shp, double scl = 1.0) { A.off[A.n] = (short)pb_off; A.shp[A.n] = (unsigned char)shp; A.scl[A.n] = (float)scl; ++A.n; };
         CompIdx& ci = c->cidx; ci.src = ci.src1 = ci.shp0 = ci.ll0 = ci.ll1 = ci.ll2 = -1; ci.n_coef = L.n_coef;
         if (L.src >= 0) { ci.src = A.n; add(PB_SRC + SB_IE, 0); }
         if (L.src1 >= 0) { ci.src1 = A.n; add(PB_SRC1 + SB_IE, 0); }
         if (L.n_coef > 0) ci.shp0 = A.n;
-        for (int k = 0; k < L.n_coef; ++k) add(PB_SHP_A + k, 1);
+        for (int k = 0; k < L.n_coef; ++k) add(PB_SHP_A + k, 1, shp_scale_host(k));
         if (L.ll0 >= 0) { ci.ll0 = A.n; add(PB_LL0 + SB_IE, 0); }
         if (L.ll1 >= 0) { ci.ll1 = A.n; add(PB_LL1 + SB_IE, 0); }
         if (L.ll2 >= 0) { ci.ll2 = A.n; add(PB_LL2 + SB_IE, 0); }

@@ -99,6 +99,21 @@ __host__ __device__ inline int phase_shift(const Geom& G, int a) { return (a + G
 __host__ __device__ inline size_t ray_stride(const Geom& G) { return (size_t)G.s * G.s * G.Hp * G.Wp; }
 __host__ __device__ inline size_t gpix_stride(const Geom& G) { return (size_t)G.Hg * G.Wg; }
 
+// ----------------------------------------------------------------------------- scaled shapelet basis (gl_ray.cuh)
+// psi_k = phi_k / c_k with c_k = sqrt(2^k / k!); the per-coefficient factor c_n1 c_n2 is folded into the coefficients of
+// PB by step A and into the coefficient sums by the finalize.  Coefficient k = (n1 + n2)(n1 + n2 + 1)/2 + n2.
+#define GL_HC_TABLE {1.0, 1.4142135623730951, 1.4142135623730951, 1.1547005383792515, 0.816496580927726, 0.5163977794943222, \
+                     0.29814239699997197, 0.15936381457791915, 0.07968190728895957, 0.037562411321267405,                   \
+                     0.01679842102263232, 0.007162870791336714}
+__constant__ double d_HC[12] = GL_HC_TABLE;
+__host__ __device__ inline void shp_orders(int k, int& n1, int& n2) {
+    int o = 0;
+    while ((o + 1) * (o + 2) / 2 <= k) ++o;
+    n2 = k - o * (o + 1) / 2; n1 = o - n2;
+}
+__device__ __forceinline__ double shp_scale(int k) { int n1, n2; shp_orders(k, n1, n2); return d_HC[n1] * d_HC[n2]; }
+inline double shp_scale_host(int k) { static const double hc[12] = GL_HC_TABLE; int n1, n2; shp_orders(k, n1, n2); return hc[n1] * hc[n2]; }
+
 template <class T>
 __device__ __forceinline__ T warp_sum(T v) {
 #pragma unroll

@@ -21,7 +21,8 @@ constexpr int AMP_MAX = 72;          // 2 + 66 + 3 = 71 amplitudes at most (two 
 struct AmpMap {                      // component k -> its slot in PB
     int n;
     short off[AMP_MAX];              // PB offset of the amplitude
-    unsigned char shp[AMP_MAX];      // 1: shapelet coefficient (PB holds a_k / beta_s: scale by PB[PB_SHP] = 1/beta_s)
+    unsigned char shp[AMP_MAX];      // 1: shapelet coefficient (PB holds a_k c_n1 c_n2 / beta_s: scale by PB[PB_SHP] = 1/beta_s and scl)
+    float scl[AMP_MAX];              // c_n1 c_n2 of the scaled shapelet basis (gl_ray.cuh), 1 for the other amplitudes
 };
 
 // PB amplitudes := unit vector e_k (k < 0: every amplitude 1).  One thread per (particle, component).
@@ -31,7 +32,7 @@ __global__ void gl_amp_select_kernel(const __grid_constant__ AmpMap am, int k, i
     if (e >= Pc * am.n) return;
     const int64_t p = e / am.n; const int j = (int)(e - p * am.n);
     T* o = pb + p * PB_STRIDE;
-    o[am.off[j]] = (j == k || k < 0) ? (am.shp[j] ? o[PB_SHP] : T(1)) : T(0);
+    o[am.off[j]] = (j == k || k < 0) ? (am.shp[j] ? (T)((double)o[PB_SHP] * (double)am.scl[j]) : T(1)) : T(0);
 }
 
 // obs = 0 and w = 1 for the component passes: step E then leaves -A_k in its g_pix output.
@@ -205,7 +206,7 @@ __global__ void __launch_bounds__(256) gl_amp_solve_kernel(const __grid_constant
     const bool fail = s_fail != 0;
     for (int k = tid; k < n; k += 256) {
         const double a = fail ? 0.0 : rhs[k];
-        o[am.off[k]] = am.shp[k] ? (T)(a * (double)o[PB_SHP]) : (T)a;
+        o[am.off[k]] = am.shp[k] ? (T)(a * (double)o[PB_SHP] * (double)am.scl[k]) : (T)a;
         if (out_amp) out_amp[(p_base + p) * n + k] = (float)a;
     }
     if (tid == 0 && fail) o[PB_VALID] = T(0);

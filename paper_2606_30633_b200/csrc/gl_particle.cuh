@@ -187,7 +187,8 @@ __global__ void __launch_bounds__(UNPACK_WPB * 32) gl_unpack_kernel(const __grid
             o[PB_SER_M1] = (T)m1; o[PB_SER_M2] = (T)(mt - m1);
         }
     }
-    // shapelets (coefficients pre-divided by beta_s; orders above the configured nmax are zero)
+    // shapelets (coefficients pre-divided by beta_s and multiplied by the basis scale c_n1 c_n2 of gl_ray.cuh; orders above
+    // the configured nmax are zero)
     if (L.ker_nmax >= 0) {
         double bs = 1.0;
         if (L.shp >= 0) { bs = theta_at(th, L.shp); if (!(bs > 0)) { ok = false; bs = 1; } }
@@ -195,7 +196,7 @@ __global__ void __launch_bounds__(UNPACK_WPB * 32) gl_unpack_kernel(const __grid
         if (lane == 6) { o[PB_SHP] = (T)ibs; o[PB_SHP + 1] = o[PB_SHP + 2] = o[PB_SHP + 3] = T(0); }
         const int nck = (L.ker_nmax + 1) * (L.ker_nmax + 2) / 2;
         for (int k = lane; k < nck; k += 32)
-            o[PB_SHP_A + k] = (L.shp >= 0 && k < L.n_coef) ? (T)(theta_at(th, L.shp + 1 + k) * ibs) : T(0);
+            o[PB_SHP_A + k] = (L.shp >= 0 && k < L.n_coef) ? (T)(theta_at(th, L.shp + 1 + k) * ibs * shp_scale(k)) : T(0);
     }
     // EPL series coefficients: a_n = prod_{k<=n} (2k-2+t)/(2k+2-t); d_m = (m+1) a_{m+1}; e_m = L_{m+1} a_{m+1}, with
     // L_n = sum_{k<=n} 4k/((2k+2-t)(2k-2+t)).  Lane n holds term n: inclusive scans over the lanes give a_n and L_n.
@@ -320,7 +321,7 @@ __global__ void gl_finalize_kernel(const __grid_constant__ PriorTable pt, const 
         __syncwarp();
         if (L.shp >= 0 && valid) {
             double bs = theta_at(th, L.shp);
-            for (int k = lane; k < L.n_coef; k += 32) gth[L.shp + 1 + k] = nat[NA_SHA + k] / bs;
+            for (int k = lane; k < L.n_coef; k += 32) gth[L.shp + 1 + k] = nat[NA_SHA + k] * shp_scale(k) / bs;   // sums taken in the scaled basis
         }
         __syncwarp();
         // theta -> z, priors, log-det; a non-finite component invalidates the particle

@@ -15,30 +15,15 @@
 namespace gl {
 
 
-// Gauss-Hermite recurrence constants: phi_{k+1} = HA[k] u phi_k - HB[k] phi_{k-1};  phi_k' = HD[k] phi_{k-1} - u phi_k
-__constant__ float c_HA[12] = {1.41421356237309505f, 1.0f, 0.81649658092772603f, 0.70710678118654752f, 0.63245553203367587f,
-                               0.57735026918962576f, 0.53452248382484879f, 0.5f, 0.47140452079103168f, 0.44721359549995794f,
-                               0.42640143271122088f, 0.40824829046386302f};
-__constant__ float c_HB[12] = {0.0f, 0.70710678118654752f, 0.81649658092772603f, 0.86602540378443865f, 0.89442719099991588f,
-                               0.91287092917527686f, 0.92582009977255146f, 0.93541434669348535f, 0.94280904158206337f,
-                               0.94868329805051380f, 0.95346258924559232f, 0.95742710775633811f};
-__constant__ float c_HD[12] = {0.0f, 1.41421356237309505f, 2.0f, 2.44948974278317810f, 2.82842712474619010f, 3.16227766016837933f,
-                               3.46410161513775459f, 3.74165738677394139f, 4.0f, 4.24264068711928515f, 4.47213595499957939f,
-                               4.69041575982342955f};
-
-__constant__ double d_HA[12] = {1.41421356237309505, 1.0, 0.81649658092772603, 0.70710678118654752, 0.63245553203367587,
-                               0.57735026918962576, 0.53452248382484879, 0.5, 0.47140452079103168, 0.44721359549995794,
-                               0.42640143271122088, 0.40824829046386302};
-__constant__ double d_HB[12] = {0.0, 0.70710678118654752, 0.81649658092772603, 0.86602540378443865, 0.89442719099991588,
-                               0.91287092917527686, 0.92582009977255146, 0.93541434669348535, 0.94280904158206337,
-                               0.94868329805051380, 0.95346258924559232, 0.95742710775633811};
-__constant__ double d_HD[12] = {0.0, 1.41421356237309505, 2.0, 2.44948974278317810, 2.82842712474619010, 3.16227766016837933,
-                               3.46410161513775459, 3.74165738677394139, 4.0, 4.24264068711928515, 4.47213595499957939,
-                               4.69041575982342955};
-
-template <class T> __device__ __forceinline__ T hA(int k) { if constexpr (sizeof(T) == 8) return d_HA[k]; else return c_HA[k]; }
-template <class T> __device__ __forceinline__ T hB(int k) { if constexpr (sizeof(T) == 8) return d_HB[k]; else return c_HB[k]; }
-template <class T> __device__ __forceinline__ T hD(int k) { if constexpr (sizeof(T) == 8) return d_HD[k]; else return c_HD[k]; }
+// Shapelet basis in the SCALED form psi_k = phi_k / c_k, c_k = sqrt(2^k / k!) (c_{k+1} = sqrt(2/(k+1)) c_k): the orthonormal
+// Gauss-Hermite functions phi_{k+1} = sqrt(2/(k+1)) u phi_k - sqrt(k/(k+1)) phi_{k-1} become
+//     psi_{k+1} = u psi_k - (k/2) psi_{k-1}          (2 operations per step instead of 3),
+//     psi_k'    = (k/2) psi_{k-1} - psi_{k+1}        (1 operation: the product is the recurrence's own).
+// The factors c_n1 c_n2 are per-coefficient constants: gl_unpack_kernel folds them into the coefficients in PB, and
+// gl_finalize_kernel into the coefficient sums (shp_scale).  In fp64 the two Gaussians of phi_n1(u) phi_n2(v) are ONE
+// exp2 of u^2 + v^2 carried by the u family (the v family is then the bare polynomial); fp32 keeps one Gaussian per
+// family so that the polynomial cannot overflow where the Gaussian has already underflowed.
+// (d_HC, shp_scale: gl_common.cuh)
 
 // P(w) = sum_{k<=TOP} cf[k] w^k for real coefficients cf (shared memory, zero beyond the kept terms).
 template <class T, int TOP>
@@ -175,14 +160,41 @@ __device__ __forceinline__ void knuth_banded(const T* __restrict__ cf, const flo
     }
 }
 
-template <class T, int NMAX>
-__device__ __forceinline__ void hermite(const typename Real<T>::Tab& tb, T u, T* f) {
+// The two Gaussian factors of a ray (see above): gu multiplies the u family, gv the v family.
+template <class T>
+__device__ __forceinline__ void shp_gauss(const typename Real<T>::Tab& tb, T u, T v, T& gu, T& gv) {
     using R = Real<T>;
-    // pi^{-1/4} exp(-u^2/2) = ex2(-0.5 log2(e) u^2 + log2(pi^{-1/4}))
-    f[0] = R::ex2(tb, R::fma(-T(0.72134752044448170) * u, u, -T(0.41287403236807968)));
-    if constexpr (NMAX >= 1) f[1] = hA<T>(0) * u * f[0];
+    if constexpr (sizeof(T) == 8) {      // pi^{-1/2} exp(-(u^2 + v^2)/2) = ex2(-0.5 log2(e) (u^2 + v^2) - 0.5 log2(pi))
+        gu = R::ex2(tb, R::fma(-T(0.72134752044448170), R::fma(u, u, v * v), -T(0.82574806473615936)));
+        gv = T(1.);
+    } else {
+        gu = R::ex2(tb, R::fma(-T(0.72134752044448170) * u, u, -T(0.41287403236807968)));
+        gv = R::ex2(tb, R::fma(-T(0.72134752044448170) * v, v, -T(0.41287403236807968)));
+    }
+}
+// f[k] = f0 psi-polynomial_k(x), k = 0..NMAX
+template <class T, int NMAX>
+__device__ __forceinline__ void hermite(T x, T f0, T* f) {
+    using R = Real<T>;
+    f[0] = f0;
+    if constexpr (NMAX >= 1) f[1] = x * f0;
 #pragma unroll
-    for (int k = 1; k < NMAX; ++k) f[k + 1] = R::fma(hA<T>(k) * u, f[k], -hB<T>(k) * f[k - 1]);
+    for (int k = 1; k < NMAX; ++k) f[k + 1] = R::fma(x, f[k], T(-0.5 * k) * f[k - 1]);
+}
+// the same plus d[k] = d/dx of (f0(x) polynomial_k(x)) = (k/2) f[k-1] - f[k+1] (f0 a Gaussian in x, or constant times one)
+template <class T, int NMAX>
+__device__ __forceinline__ void hermite_d(T x, T f0, T* f, T* d) {
+    using R = Real<T>;
+    f[0] = f0;
+    T nxt = x * f0;                      // f[k+1]
+    d[0] = -nxt;
+#pragma unroll
+    for (int k = 1; k <= NMAX; ++k) {
+        f[k] = nxt;
+        const T t = T(0.5 * k) * f[k - 1];
+        nxt = R::fma(x, f[k], -t);
+        d[k] = t - nxt;
+    }
 }
 
 template <class T> struct SersicOut { T I, xr, yr, u, lu, Iu_r2; };
@@ -345,21 +357,24 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
             constexpr int NM = V::NMAX >= 0 ? V::NMAX : 0;
             const T ibs = pb[PB_SHP];
             const T u = px * ibs, v = py * ibs;
+            T gu, gv;
+            shp_gauss<T>(tb, u, v, gu, gv);
             T fu[NM + 1], fv[NM + 1];
-            hermite<T, NM>(tb, u, fu); hermite<T, NM>(tb, v, fv);
-            const T* a = pb + PB_SHP_A;
+            const T* a = pb + PB_SHP_A;              // a_k c_n1 c_n2 / beta_s (scaled basis, see hermite)
             T Ish = T(0.);
             if constexpr (COMP) {                    // basis function k with unit coefficient: phi_n1(u) phi_n2(v) / beta_s
+                hermite<T, NM>(u, gu, fu); hermite<T, NM>(v, gv, fv);
 #pragma unroll
                 for (int n2 = 0; n2 <= NM; ++n2) {
                     const T fvb = fv[n2] * ibs;
 #pragma unroll
                     for (int n1 = 0; n1 <= NM - n2; ++n1) {
                         const int idx = (n1 + n2) * (n1 + n2 + 1) / 2 + n2;
-                        if (idx < ci->n_coef) acc[(size_t)(ci->shp0 + idx) * cstride] = fu[n1] * fvb;
+                        if (idx < ci->n_coef) acc[(size_t)(ci->shp0 + idx) * cstride] = fu[n1] * fvb * (T)(d_HC[n1] * d_HC[n2]);
                     }
                 }
             } else if constexpr (!ADJ) {
+                hermite<T, NM>(u, gu, fu); hermite<T, NM>(v, gv, fv);
 #pragma unroll
                 for (int n2 = 0; n2 <= NM; ++n2) {
                     T row = T(0.);
@@ -368,12 +383,10 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
                     Ish = R::fma(row, fv[n2], Ish);
                 }
             } else {
-                // phi_k' = HD[k] phi_{k-1} - u phi_k, once per ray; the N_coef coefficient sums gbar phi_n1(u) phi_n2(v) are
-                // taken here in registers, or (coef_split) by gl_shp_coef_kernel from the (u, v) stored below.
-                T dfu[NM + 1];
-                dfu[0] = -u * fu[0];
-#pragma unroll
-                for (int k = 1; k <= NM; ++k) dfu[k] = R::fma(hD<T>(k), fu[k - 1], -u * fu[k]);
+                // the N_coef coefficient sums gbar psi_n1(u) psi_n2(v) are taken here in registers, or (coef_split) by
+                // gl_shp_coef_kernel from the (u, v) stored below.
+                T dfu[NM + 1], dfv[NM + 1];
+                hermite_d<T, NM>(u, gu, fu, dfu); hermite_d<T, NM>(v, gv, fv, dfv);
                 if constexpr (coef_split<T, V>()) { uvp[0] = u; uvp[uvstride] = v; }
                 T Iu = T(0.), Iv = T(0.);
 #pragma unroll
@@ -387,10 +400,7 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
                         row = R::fma(ak, fu[n1], row); drow = R::fma(ak, dfu[n1], drow);
                         if constexpr (!coef_split<T, V>()) acc[NA_SHA + idx] = R::fma(gfv, fu[n1], acc[NA_SHA + idx]);
                     }
-                    Ish = R::fma(row, fv[n2], Ish); Iu = R::fma(drow, fv[n2], Iu); {
-                        const T dfv = n2 == 0 ? -v * fv[0] : R::fma(hD<T>(n2), fv[n2 > 0 ? n2 - 1 : 0], -v * fv[n2]);
-                        Iv = R::fma(row, dfv, Iv);
-                    }
+                    Ish = R::fma(row, fv[n2], Ish); Iu = R::fma(drow, fv[n2], Iu); Iv = R::fma(row, dfv[n2], Iv);
                 }
                 acc[NA_SHB] = R::fma(gbar, Ish + R::fma(u, Iu, v * Iv), acc[NA_SHB]);
                 const T Ibx = Iu * ibs, Iby = Iv * ibs;
@@ -698,8 +708,9 @@ __global__ void __launch_bounds__(NT) gl_shp_coef_kernel(const __grid_constant__
                 const T* d = &stg[k][0][threadIdx.x];
                 const T g = d[0], u = d[NT], v = d[2 * NT];
                 fetch(k, r0 + k + NS);
-                T fu[NMAX + 1], fv[NMAX + 1];
-                hermite<T, NMAX>(tb, u, fu); hermite<T, NMAX>(tb, v, fv);
+                T gu, gv, fu[NMAX + 1], fv[NMAX + 1];
+                shp_gauss<T>(tb, u, v, gu, gv);
+                hermite<T, NMAX>(u, gu, fu); hermite<T, NMAX>(v, gv, fv);
 #pragma unroll
                 for (int n1 = 0; n1 <= NMAX; ++n1) {
                     const T gf = g * fu[n1];
