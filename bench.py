@@ -513,7 +513,8 @@ def run_ours(a):
                            mhz_max, peak_src, clocks.get("sm_mhz"), evals_in_stage_times=1 if a.stage == "hmc" else None)
     probe = {}
     for kind, name in ((0, "fp32_fma"), (1, "fp64_fma"), (2, "mufu_ex2"), (4, "fp64_fma_distinct_operands"),
-                       (5, "fp64_mma_m8n8k4"), (6, "fp64_mma_plus_fma")):
+                       (5, "fp64_mma_m8n8k4"), (6, "fp64_mma_plus_fma"),
+                       (7, "fp64_fma_two_vector_one_uniform_operand"), (8, "fp64_fma_three_vector_operands_one_shared")):
         try:
             probe[name] = round(gl.gl_probe_pipe(kind, 256)[0], 3)
         except Exception:                                             # measurement utility only

@@ -314,7 +314,9 @@ gl_status gl_workspace_layout(const gl_config* cfg, int64_t n_particles, int64_t
  * or MUFU figure).  kind 0: FP32 FMA, 1: FP64 FMA, 2: MUFU ex2, 3: FP32 and FP64 FMA interleaved 1:1 (both
  * counted), 4: FP64 FMA with three distinct register operands per chain (kinds 0-3 share multiplier and addend),
  * 5: FP64 tensor-core MMA (mma.sync.m8n8k4.f64; one warp instruction = 8 lane-operations per lane), 6: kind 5 and kind 1
- * interleaved 1:1 (both counted: do the FP64 tensor and vector paths add up?).  Launches 8 CTAs of 256 threads per SM, each thread running 8 independent chains of
+ * interleaved 1:1 (both counted: do the FP64 tensor and vector paths add up?), 7: FP64 FMA with two distinct vector-register
+ * operands and one warp-uniform operand, 8: FP64 FMA with three vector-register operands whose multiplier is shared by
+ * consecutive instructions (operand-reuse cache).  Launches 8 CTAs of 256 threads per SM, each thread running 8 independent chains of
  * n_outer * 64 operations, once untimed and once between two CUDA events on `stream`, waits for it, and writes
  * 1e-12 * lane-operations per second (an FMA counts once) to *tera_lane_ops_per_s_host and the kernel time to
  * *ms_host (HOST pointers; ms_host may be NULL).  workspace: DEVICE pointer, >= 256 bytes (never written in

@@ -191,7 +191,8 @@ def gl_stage_times():
 
 def gl_probe_pipe(kind, n_outer=2048, stream=None):
     """(tera lane-ops/s, kernel ms) of one SM pipe: kind 0 FP32 FMA, 1 FP64 FMA, 2 MUFU ex2, 3 FP32+FP64 interleaved,
-    4 FP64 FMA with distinct operands, 5 FP64 tensor MMA (m8n8k4), 6 FP64 MMA + FMA interleaved."""
+    4 FP64 FMA with distinct operands, 5 FP64 tensor MMA (m8n8k4), 6 FP64 MMA + FMA interleaved, 7 FP64 FMA with two vector
+    operands + one uniform operand, 8 FP64 FMA with three vector operands, multiplier shared by neighbours."""
     torch = _torch()
     ws = torch.zeros(256, dtype=torch.uint8, device="cuda")
     rate = C.c_double(); ms = C.c_float()

@@ -784,7 +784,7 @@ extern "C" gl_status gl_logpost_grad_host(const gl_config* c, const float* obs, 
 extern "C" gl_status gl_probe_pipe(int32_t kind, int32_t n_outer, void* workspace, size_t workspace_bytes, void* stream,
                                    double* tera_lane_ops_per_s_host, float* ms_host) {
     if (!workspace || !tera_lane_ops_per_s_host) return GL_ERR_NULL;
-    if (kind < 0 || kind > 6 || n_outer < 1) return GL_ERR_BAD_SHAPE;
+    if (kind < 0 || kind > 8 || n_outer < 1) return GL_ERR_BAD_SHAPE;
     if (workspace_bytes < 256) return GL_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, n_sm = 0;
@@ -802,7 +802,9 @@ extern "C" gl_status gl_probe_pipe(int32_t kind, int32_t n_outer, void* workspac
             case 3: gl_probe_kernel<3><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
             case 4: gl_probe_kernel<4><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
             case 5: gl_probe_kernel<5><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
-            default: gl_probe_kernel<6><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+            case 6: gl_probe_kernel<6><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+            case 7: gl_probe_kernel<7><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
+            default: gl_probe_kernel<8><<<ctas, nt, 0, st>>>(n, 1.f, sink); break;
         }
     };
     launch(n_outer);                                   // warm-up

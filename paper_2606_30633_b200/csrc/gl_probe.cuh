@@ -15,6 +15,9 @@ constexpr int PROBE_INNER = 64;     // FMAs per chain per outer iteration
 //    the chains, which lets the operand-reuse cache feed the pipe: kind 4 is what ordinary fp64 code can sustain)
 // 5: FP64 tensor-core MMA (mma.sync.m8n8k4.f64, SASS DMMA), 8 independent accumulator pairs per thread; one warp
 //    instruction is 8 x 8 x 4 = 256 FMAs = 8 lane-operations per lane (counted so);
+// 7: FP64 FMA with two distinct vector-register operands and one warp-uniform operand (uniform register / constant);
+// 8: FP64 FMA with three vector-register operands of which the multiplier is the same register in consecutive instructions
+//    (what the operand-reuse cache can serve): 7 and 8 separate "three operands" from "three register-file reads";
 // 6: kind 5 and kind 1 interleaved 1:1 (one DMMA, one DFMA, both counted): do the tensor and the vector FP64 paths add up?
 template <int KIND>
 __global__ void __launch_bounds__(256) gl_probe_kernel(int n_outer, float seed, float* __restrict__ sink) {
@@ -38,6 +41,8 @@ __global__ void __launch_bounds__(256) gl_probe_kernel(int n_outer, float seed, 
                 if constexpr (KIND == 1 || KIND == 3) d[k] = fma(d[k], md, cd);
                 if constexpr (KIND == 2) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(a[k]));
                 if constexpr (KIND == 4) d[k] = fma(d[k], e[k], f[k]);
+                if constexpr (KIND == 7) d[k] = fma(d[k], e[k], cd);            // two distinct vector registers + a uniform addend
+                if constexpr (KIND == 8) d[k] = fma(d[k], e[0], f[k]);          // three vector registers, the multiplier shared by neighbours
                 if constexpr (KIND == 5 || KIND == 6)
                     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
                                  : "+d"(t0[k]), "+d"(t1[k]) : "d"(e[k]), "d"(f[k]));
