@@ -5,6 +5,7 @@
 #include <cmath>
 #include <algorithm>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -40,9 +41,23 @@ struct gl_config {
     int esize;          // sizeof the arithmetic type: 8 (GL_PRECISION_F64) or 4 (GL_PRECISION_F32)
     int uv_split;       // 1: the adjoint stores the shapelet coordinates (u, v) of every ray for gl_shp_coef_kernel (coef_split)
     size_t per_particle_bytes;
+    int ct_slot;        // slot of the process-wide constant tap table (gl_conv_ct.cuh), -1: none
 };
 
 static thread_local int64_t t_launches = 0;
+
+// Slots of the constant tap table c_ctap (gl_conv_ct.cuh): process-wide, handed out at gl_config_create, returned at destroy.
+static std::mutex g_ct_mu;
+static bool g_ct_used[CT_NSLOT] = {};
+static int ct_slot_acquire() {
+    std::lock_guard<std::mutex> lk(g_ct_mu);
+    for (int i = 0; i < CT_NSLOT; ++i) if (!g_ct_used[i]) { g_ct_used[i] = true; return i; }
+    return -1;
+}
+static void ct_slot_release(int i) {
+    std::lock_guard<std::mutex> lk(g_ct_mu);
+    if (i >= 0 && i < CT_NSLOT) g_ct_used[i] = false;
+}
 
 // ----------------------------------------------------------------------------- optional per-stage timing (diagnostic)
 enum { ST_PREP = 0, ST_UNPACK, ST_RAY_FWD, ST_CONV_FWD, ST_CONV_BWD, ST_RAY_ADJ, ST_FINALIZE, ST_AMP, ST_COUNT };
@@ -182,6 +197,7 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     if (M64 > 4096 || d->psf_size > 255) return GL_ERR_UNSUPPORTED;
     gl_config* c = new (std::nothrow) gl_config();
     if (!c) return GL_ERR_BAD_CONFIG;
+    c->ct_slot = -1;
     c->desc = *d;
     c->priors.assign(d->priors, d->priors + np);
     c->desc.priors = c->priors.data();
@@ -229,7 +245,9 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     G.delta2 = (double)d->pix_scale * (double)d->pix_scale;
     (void)M64;
     c->esize = d->precision == GL_PRECISION_F64 ? 8 : 4;
-    c->conv = conv_plan(G, c->esize, d->n_systems);       // also fills the padded-layout fields of G
+    c->ct_slot = d->n_systems == 1 ? ct_slot_acquire() : -1;      // constant-memory tap table of the uniform-tap step D
+    c->conv = conv_plan(G, c->esize, d->n_systems, c->ct_slot);   // also fills the padded-layout fields of G
+    if (c->conv.kind != 6 && c->ct_slot >= 0) { ct_slot_release(c->ct_slot); c->ct_slot = -1; }
     c->n_ctile = c->conv.n_ctile;
     // ray kernels: one CTA per (particle, phase plane, chunk); pick the block size that wastes the fewest lanes
     const int NN = G.N * G.N;
@@ -257,7 +275,7 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     return GL_OK;
 }
 
-extern "C" void gl_config_destroy(gl_config* c) { delete c; }
+extern "C" void gl_config_destroy(gl_config* c) { if (c) ct_slot_release(c->ct_slot); delete c; }
 extern "C" int32_t gl_config_n_params(const gl_config* c) { return c ? c->L.n_params : 0; }
 extern "C" int32_t gl_config_n_amplitudes(const gl_config* c) { return c ? c->n_amp : 0; }
 extern "C" gl_status gl_config_shape(const gl_config* c, int32_t* out) {
@@ -268,6 +286,7 @@ extern "C" gl_status gl_config_shape(const gl_config* c, int32_t* out) {
 
 struct Plan {
     int64_t Pc;
+    size_t off_ctap;    // plane-ordered tap table of the uniform-tap step D (staging for the constant slot)
     size_t off_tab, off_kt, off_w, off_sl, off_pb, off_lpd, off_ray, off_gpix, off_chi, off_nap, off_uv, off_comp, off_cray, off_zobs, off_uw, off_sid, total;
 };
 
@@ -283,6 +302,7 @@ static Plan make_plan(const gl_config* c, int64_t P) {
     const size_t nsys = (size_t)c->desc.n_systems, es = (size_t)c->esize;
     pl.off_tab = o;  o = align256(o + sizeof(double) * MATH_TAB_DOUBLES);
     pl.off_kt = o;   o = align256(o + es * nsys * G.s * G.s * G.U * G.U);
+    pl.off_ctap = o; o = align256(o + es * (size_t)G.s * G.s * G.U * ((G.U + 1) & ~1));
     pl.off_w = o;    o = align256(o + es * nsys * G.N * G.N);
     pl.off_sl = o;   o = align256(o + sizeof(double) * nsys);
     pl.off_pb = o;   o = align256(o + es * (size_t)pl.Pc * PB_STRIDE);
@@ -423,6 +443,11 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
     GL_STAGE(ST_PREP, st, (gl_prep_kernel<T><<<c->desc.n_systems, 256, 0, st>>>(G, psf, mode == 2 ? nullptr : sigma, sys_kt, sys_w,
                                                                              sys_sl, tab_out)));
     ++t_launches;
+    if (c->conv.kind == 6) {                 // uniform-tap step D: refill this configuration's constant slot from the PSF of this call
+        const int nk = conv_ct_upload<T>(c->conv, G, sys_kt, (T*)(w + pl.off_ctap), st);
+        if (nk < 0) return GL_ERR_CUDA;
+        t_launches += nk;
+    }
     if (solve) {
         const size_t n = (size_t)c->desc.n_systems * G.N * G.N;
         gl_amp_fill_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, zobs, unit_w);

@@ -6,6 +6,7 @@
 #include "gl_common.cuh"
 #include "gl_conv.cuh"
 #include "gl_conv_ts.cuh"
+#include "gl_conv_ct.cuh"
 
 namespace gl {
 
@@ -16,7 +17,7 @@ namespace gl {
 static inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
 struct ConvPlan {
-    int kind;                 // 0 generic, 1: U=6 CW=4, 2: U=11 CW=2, 3: U=16 CW=2 (round-1 sliding kernels), 4: tap-stationary + TMA,
+    int kind;                 // 6: uniform taps (single system; gl_conv_ct.cuh); 0 generic, 1: U=6 CW=4, 2: U=11 CW=2, 3: U=16 CW=2 (round-1 sliding kernels), 4: tap-stationary + TMA,
                               // 5: psf_grid 1 dedicated: bin the planes, then tap-stationary on ONE plane with the K x K taps
     int CW;                   // output columns per thread
     SlidePlan fwd, bwd;
@@ -24,7 +25,34 @@ struct ConvPlan {
     int n_ctile;              // chi^2 partials per particle
     int ts_id;                // kind 4: which (U, G, NPH, CW) instance (ts_variant)
     TsPlan tf, tb;            // kind 4: forward / transpose launch plans
+    int ct_slot;              // kind 6 (uniform taps from constant memory, gl_conv_ct.cuh): slot of c_ctap
+    CtPlan cf, cb;            // kind 6: forward / transpose launch plans
 };
+
+// Uniform-tap instances: output columns per thread for each compiled tap count
+#ifndef GL_CT_CW6
+#define GL_CT_CW6 4
+#endif
+#ifndef GL_CT_CW11
+#define GL_CT_CW11 4
+#endif
+#ifndef GL_CT_CW16
+#define GL_CT_CW16 2
+#endif
+#ifndef GL_CT_BAND_ROWS
+#define GL_CT_BAND_ROWS 50
+#endif
+#ifndef GL_CT_CW16B
+#define GL_CT_CW16B 4
+#endif
+// U = 6 (36 taps per plane) stays on the tap-stationary kernels: measured on config 2, 0.96 / 1.00 ms here against 0.95 / 0.71 ms
+// there (too few FMAs per row step to amortise the row bookkeeping); GL_CT_U6=1 compiles the instance in for A/B runs.
+#ifndef GL_CT_U6
+#define GL_CT_U6 0
+#endif
+static inline int ct_cw(int U) { return (U == 6 && GL_CT_U6) ? GL_CT_CW6 : (U == 11 ? GL_CT_CW11 : (U == 16 ? GL_CT_CW16 : 0)); }     // forward
+static inline int ct_cwb(int U) { return U == 16 ? GL_CT_CW16B : ct_cw(U); }                                            // transpose
+static inline bool ct_fits(int U, int NPH) { return ct_cw(U) > 0 && NPH * U * ((U + 1) & ~1) <= CT_SLOT; }
 
 // The compiled tap-stationary instances: id -> (U, G, NPH, CW).  G tap-row groups x NPH planes = lanes per column group.
 #ifndef GL_TS_CW11
@@ -109,7 +137,7 @@ static inline TsPlan ts_plan(const TsVariant& v, int wmax_default, int esize, in
 }
 
 // Fill the layout fields of G (UP, Hp, Wp, Hg, Wg, PADg) and choose the kernels.  esize = sizeof(T).
-static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems) {
+static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems, int ct_slot = -1) {
     ConvPlan pl{};
     const int U = G.U, N = G.N, NPH = G.s * G.s;
     pl.kind = 0;
@@ -148,6 +176,29 @@ static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems) {
     if (pl.kind == 0) {
         pl.n_ctile = (N * N + 255) / 256;
         return pl;
+    }
+    pl.ct_slot = -1;
+    {   // uniform taps (gl_conv_ct.cuh): one system, a free constant slot, a compiled tap count; GL_CONV_CT=0: off (A/B runs)
+        const char* e = std::getenv("GL_CONV_CT");
+        if (ct_slot >= 0 && n_systems == 1 && ct_fits(U, NPH) && !(e && e[0] == '0')) {
+            const int cw = ct_cw(U), seg = (cw + U - 1 + 1) & ~1, cwb = ct_cwb(U), segb = (cwb + U - 1 + 1) & ~1;
+            const int nf = (N + cw - 1) / cw, nb = (N + ob_max + cwb - 1) / cwb;
+            int wp2 = G.Wp, wg2 = G.Wg;
+            if (wp2 < cw * (nf - 1) + seg) wp2 = cw * (nf - 1) + seg;
+            if (wp2 < cwb * nb) wp2 = cwb * nb;
+            if (wg2 < cwb * (nb - 1) + segb) wg2 = cwb * (nb - 1) + segb;
+            G.Wp = round_up(wp2, 4); G.Wg = round_up(wg2, 4);
+            auto mkc = [&](int ncg) {
+                CtPlan cp{};
+                cp.ncg = ncg;
+                cp.n_bands = N / GL_CT_BAND_ROWS < 1 ? 1 : N / GL_CT_BAND_ROWS;      // geometry only (bit-identical chi^2 at any batch size)
+                cp.rbh = (N + cp.n_bands - 1) / cp.n_bands;
+                return cp;
+            };
+            pl.cf = mkc(nf); pl.cb = mkc(nb);
+            pl.kind = 6; pl.CW = cw; pl.ct_slot = ct_slot; pl.n_ctile = pl.cf.n_bands * pl.cf.ncg;
+            return pl;
+        }
     }
     const int LS = pl.kind == 1 ? 4 : 1;                         // lanes per column group (conv_*_launch must agree)
     int ps = U * ((U + 1) & ~1);
@@ -333,6 +384,32 @@ static inline cudaError_t conv_bwd_ts_launch(const ConvPlan& pl, const Geom& G, 
     kern<<<grid, (pl.tb.wpc + 1) * 32, smem, st>>>(tm, G, pl.tb, Pc, sys_kt, system_id, p_base, gbar);
     return cudaSuccess;
 }
+// ----------------------------------------------------------------------------- uniform-tap launches (kind 6)
+template <class T, int U, int CW>
+static inline cudaError_t conv_fwd_ct_launch(const ConvPlan& pl, const Geom& G, const T* ray, const T* sys_w, const float* obs,
+                                             int64_t p_base, int64_t Pc, T* gpix, T* chi, float* out_model, cudaStream_t st) {
+    const dim3 grid((unsigned)((Pc * pl.cf.ncg + CT_NT - 1) / CT_NT), (unsigned)pl.cf.n_bands);
+    gl_conv_fwd_ct<T, U, CW><<<grid, CT_NT, 0, st>>>(G, pl.cf, pl.ct_slot, Pc, ray, sys_w, obs, p_base, gpix, chi, out_model);
+    return cudaSuccess;
+}
+template <class T, int U, int CW>
+static inline cudaError_t conv_bwd_ct_launch(const ConvPlan& pl, const Geom& G, const T* gpix, int64_t Pc, T* gbar, cudaStream_t st) {
+    const dim3 grid((unsigned)((Pc * pl.cb.ncg + CT_NT - 1) / CT_NT), (unsigned)(G.s * G.s));
+    gl_conv_bwd_ct<T, U, CW><<<grid, CT_NT, 0, st>>>(G, pl.cb, pl.ct_slot, Pc, gpix, gbar);
+    return cudaSuccess;
+}
+// Refill the constant slot from the taps gl_prep_kernel wrote (system 0): plane-ordered table into `stage`, then a
+// device-to-device copy into c_ctap on the same stream.  Returns the number of kernels launched, negative on error.
+template <class T>
+static inline int conv_ct_upload(const ConvPlan& pl, const Geom& G, const T* sys_kt, T* stage, cudaStream_t st) {
+    const int n = G.s * G.s * G.U * ((G.U + 1) & ~1);
+    gl_ctap_stage_kernel<T><<<(n + 255) / 256, 256, 0, st>>>(G, sys_kt, stage);
+    if (cudaMemcpyToSymbolAsync(c_ctap, stage, (size_t)n * sizeof(T), (size_t)pl.ct_slot * CT_SLOT * sizeof(double),
+                                cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        return -1;
+    return 1;
+}
+
 #define GL_TS_DISPATCH(CALL)                                                                                       \
     switch (pl.ts_id) {                                                                                            \
         case 0: e = CALL(6, 1, 4, 4, GL_TS_RPS6); break;                                                           \
@@ -370,6 +447,11 @@ static inline int conv_fwd_launch(const ConvPlan& pl, const Geom& G, const T* ra
 #undef GL_TS_F
             return e == cudaSuccess ? 2 : -1;          // bin + step D
         }
+        case 6:
+            if (G.U == 6) e = conv_fwd_ct_launch<T, 6, GL_CT_CW6>(pl, G, ray, sys_w, obs, p_base, Pc, gpix, chi, out_model, st);
+            else if (G.U == 11) e = conv_fwd_ct_launch<T, 11, GL_CT_CW11>(pl, G, ray, sys_w, obs, p_base, Pc, gpix, chi, out_model, st);
+            else e = conv_fwd_ct_launch<T, 16, GL_CT_CW16>(pl, G, ray, sys_w, obs, p_base, Pc, gpix, chi, out_model, st);
+            break;
         default: {
             dim3 grid((G.N * G.N + 255) / 256, (unsigned)Pc);
             gl_conv_fwd_generic<T><<<grid, 256, 0, st>>>(G, ray, sys_kt, sys_w, obs, system_id, p_base, gpix, chi, out_model);
@@ -397,6 +479,11 @@ static inline int conv_bwd_launch(const ConvPlan& pl, const Geom& G, const T* gp
 #undef GL_TS_B
             break;
         }
+        case 6:
+            if (G.U == 6) e = conv_bwd_ct_launch<T, 6, GL_CT_CW6>(pl, G, gpix, Pc, gbar, st);
+            else if (G.U == 11) e = conv_bwd_ct_launch<T, 11, GL_CT_CW11>(pl, G, gpix, Pc, gbar, st);
+            else e = conv_bwd_ct_launch<T, 16, GL_CT_CW16B>(pl, G, gpix, Pc, gbar, st);
+            break;
         default: {
             dim3 grid((G.s * G.s * G.N * G.N + 255) / 256, (unsigned)Pc);
             gl_conv_bwd_generic<T><<<grid, 256, 0, st>>>(G, gpix, sys_kt, system_id, p_base, gbar);
