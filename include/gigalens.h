@@ -46,7 +46,8 @@ typedef enum {
     GL_ERR_BAD_SHAPE = -3,    /* n_particles < 0 */
     GL_ERR_UNSUPPORTED = -4,  /* a valid configuration this build has no kernel for */
     GL_ERR_WORKSPACE = -5,    /* workspace_bytes < gl_workspace_bytes(cfg, n_particles) or misaligned */
-    GL_ERR_CUDA = -6          /* a CUDA runtime call or launch failed (sticky error left to the caller) */
+    GL_ERR_CUDA = -6,         /* a CUDA runtime call or launch failed (sticky error left to the caller) */
+    GL_ERR_NOALLOC_LIMIT = -7 /* gl_logpost_grad_noalloc: the call needs more scratch than GL_NOALLOC_MAX_BYTES */
 } gl_status;
 
 /* Prior / bijector family of one parameter (O1, reading S13).
@@ -165,6 +166,26 @@ gl_status gl_logpost_grad(const gl_config* cfg, const float* obs, const float* n
                           const float* params, const int32_t* system_id, int64_t n_particles,
                           float* out_logp, float* out_grad, void* workspace, size_t workspace_bytes,
                           void* stream /* cudaStream_t */);
+
+/* The same evaluation for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): gl_logpost_grad (Eq. 2 and its gradient) with the workspace
+ * taken from a buffer of GL_NOALLOC_MAX_BYTES that lives INSIDE the library (a file-scope __device__ array: every GPU
+ * that loads libgigalens holds these bytes until the process exits).  The call allocates nothing: no cudaMalloc /
+ * cudaFree / allocating library routine, no workspace argument.  Arguments, layouts, ownership, results (bit-identical
+ * to gl_logpost_grad) and asynchrony as gl_logpost_grad; DEVICE pointers.
+ * Limit: gl_workspace_bytes(cfg, n_particles) <= GL_NOALLOC_MAX_BYTES, else GL_ERR_NOALLOC_LIMIT before any launch
+ * (config 1 at 64 particles needs about 7 MB; split a larger batch over several calls or use gl_logpost_grad).
+ * The buffer is SHARED by every call of this entry point on a device, whatever the configuration, stream or thread,
+ * and keeps the previous call's contents: every call rewrites each element it later reads (zero borders included), so
+ * nothing has to be cleared between calls -- but two calls that OVERLAP on the GPU (different streams, or threads
+ * without ordering) race on it.  Serialise them on one stream.
+ * The first call on a device resolves the buffer's address (cudaGetSymbolAddress, once per device): make one call
+ * outside any stream capture first.
+ * Errors: as gl_logpost_grad, GL_ERR_NOALLOC_LIMIT, and GL_ERR_CUDA if the buffer's address cannot be obtained. */
+#define GL_NOALLOC_MAX_BYTES ((size_t)32 << 20)
+gl_status gl_logpost_grad_noalloc(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
+                                  const float* params, const int32_t* system_id, int64_t n_particles,
+                                  float* out_logp, float* out_grad, void* stream);
 
 /* Diagnostic: the noise-free model image (O3-O6) of each particle, out_image [n_particles][N][N].
  * Invalid particles get an all-zero image. */

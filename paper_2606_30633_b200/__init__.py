@@ -17,14 +17,15 @@ LIB_PATH = os.path.join(HERE, "libgigalens.so")
 GL_OK = 0
 GL_PRECISION_F64, GL_PRECISION_F32 = 0, 1
 STATUS = {0: "GL_OK", -1: "GL_ERR_NULL", -2: "GL_ERR_BAD_CONFIG", -3: "GL_ERR_BAD_SHAPE", -4: "GL_ERR_UNSUPPORTED",
-          -5: "GL_ERR_WORKSPACE", -6: "GL_ERR_CUDA"}
+          -5: "GL_ERR_WORKSPACE", -6: "GL_ERR_CUDA", -7: "GL_ERR_NOALLOC_LIMIT"}
 EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_workspace_bytes", "gl_logpost",
            "gl_logpost_grad", "gl_model_image", "gl_workspace_bytes_host", "gl_logpost_grad_host",
            "gl_last_launch_count", "gl_status_string", "gl_version", "gl_stage_timing_enable", "gl_stage_count",
            "gl_stage_name", "gl_stage_times", "gl_probe_pipe", "gl_map_step",
            "gl_svi_workspace_bytes", "gl_svi_step", "gl_hmc_workspace_bytes", "gl_hmc_step",
            "gl_best_particle", "gl_config_n_amplitudes", "gl_linear_amplitudes", "gl_draw_normal", "gl_draw_log_uniform",
-           "gl_config_shape", "gl_workspace_layout"]
+           "gl_config_shape", "gl_workspace_layout", "gl_logpost_grad_noalloc"]
+GL_NOALLOC_MAX_BYTES = 32 << 20      # include/gigalens.h
 
 
 class GLError(RuntimeError):
@@ -85,6 +86,8 @@ def lib():
         L.gl_logpost.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, sz, vp]
         L.gl_logpost_grad.restype = C.c_int
         L.gl_logpost_grad.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, sz, vp]
+        L.gl_logpost_grad_noalloc.restype = C.c_int
+        L.gl_logpost_grad_noalloc.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp]
         L.gl_logpost_grad_host.restype = C.c_int
         L.gl_logpost_grad_host.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, sz, vp]
         L.gl_map_step.restype = C.c_int
@@ -313,6 +316,20 @@ def gl_logpost_grad(h, obs, noise_sigma, psf, params, system_id, out_logp, out_g
                                  _ptr(_dev(out_logp, f32, "out_logp")), _ptr(_dev(out_grad, f32, "out_grad")),
                                  _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)),
            "gl_logpost_grad")
+
+
+def gl_logpost_grad_noalloc(h, obs, noise_sigma, psf, params, system_id, out_logp, out_grad, stream=None):
+    """gl_logpost_grad on the library's own static scratch buffer (no workspace argument, nothing allocated by the call;
+    at most GL_NOALLOC_MAX_BYTES of workspace, else GLError GL_ERR_NOALLOC_LIMIT; calls must not overlap on the GPU)."""
+    torch = _torch()
+    f32 = torch.float32
+    n = params.shape[0]
+    _extents(h, n, obs=obs, noise_sigma=noise_sigma, psf=psf, params=params, system_id=system_id, out_logp=out_logp, out_grad=out_grad)
+    _check(lib().gl_logpost_grad_noalloc(h, _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
+                                         _ptr(_dev(psf, f32, "psf")), _ptr(_dev(params, f32, "params")),
+                                         _ptr(_dev(system_id, torch.int32, "system_id")), n,
+                                         _ptr(_dev(out_logp, f32, "out_logp")), _ptr(_dev(out_grad, f32, "out_grad")),
+                                         _stream(stream)), "gl_logpost_grad_noalloc")
 
 
 def gl_map_step(h, opt, obs, noise_sigma, psf, params, system_id, opt_m, opt_v, step, out_logp, out_grad, workspace,

@@ -133,6 +133,7 @@ extern "C" const char* gl_status_string(gl_status s) {
         case GL_ERR_UNSUPPORTED: return "GL_ERR_UNSUPPORTED: no kernel for this configuration";
         case GL_ERR_WORKSPACE: return "GL_ERR_WORKSPACE: workspace too small or misaligned";
         case GL_ERR_CUDA: return "GL_ERR_CUDA: CUDA runtime error";
+        case GL_ERR_NOALLOC_LIMIT: return "GL_ERR_NOALLOC_LIMIT: the call needs more scratch than the library's static buffer (GL_NOALLOC_MAX_BYTES); use fewer particles per call or gl_logpost_grad with a caller workspace";
     }
     return "unknown gl_status";
 }
@@ -562,6 +563,44 @@ extern "C" gl_status gl_logpost_grad(const gl_config* cfg, const float* obs, con
                                      float* out_logp, float* out_grad, void* workspace, size_t workspace_bytes, void* stream) {
     return run(cfg, 1, obs, noise_sigma, psf, params, system_id, n_particles, out_logp, out_grad, nullptr,
                workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+// ----------------------------------------------------------------------------- no-allocation entry point
+// Workspace of gl_logpost_grad_noalloc: a file-scope device array (every GPU that loads the library holds it until exit).
+// In HOST code the name is only a stand-in for the symbol, not a device address: the address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[GL_NOALLOC_MAX_BYTES];
+static std::mutex g_noalloc_mu;
+static void* g_noalloc_ptr[64] = {};          // per device ordinal
+static gl_status noalloc_scratch(void** out) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return GL_ERR_CUDA;
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || !p) return GL_ERR_CUDA;
+        g_noalloc_ptr[dev] = p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return GL_OK;
+}
+
+extern "C" gl_status gl_logpost_grad_noalloc(const gl_config* cfg, const float* obs, const float* noise_sigma, const float* psf,
+                                             const float* params, const int32_t* system_id, int64_t n_particles,
+                                             float* out_logp, float* out_grad, void* stream) {
+    t_launches = 0;
+    if (!cfg) return GL_ERR_NULL;
+    if (n_particles < 0) return GL_ERR_BAD_SHAPE;
+    if (n_particles > 0 && make_plan(cfg, n_particles).total > GL_NOALLOC_MAX_BYTES) return GL_ERR_NOALLOC_LIMIT;
+    void* ws = nullptr;
+    if (n_particles > 0) {
+        const gl_status s = noalloc_scratch(&ws);
+        if (s != GL_OK) return s;
+    }
+    // Nothing to clear: the path rewrites every workspace element it reads (the caller-workspace form runs on
+    // uninitialised memory too).  n_particles == 0 returns GL_OK inside run() before the workspace is looked at.
+    return run(cfg, 1, obs, noise_sigma, psf, params, system_id, n_particles, out_logp, out_grad, nullptr,
+               ws, GL_NOALLOC_MAX_BYTES, (cudaStream_t)stream);
 }
 
 extern "C" gl_status gl_draw_normal(uint64_t seed, uint64_t step, uint32_t stream_id, int64_t n_rows, int32_t n_cols,
