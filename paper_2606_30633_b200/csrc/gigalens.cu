@@ -118,6 +118,10 @@ static constexpr int NT_ADJ = GL_NT_ADJ;
 #endif
 static constexpr int RB_FWD = GL_RB_FWD;  // rays a forward thread evaluates concurrently
 static constexpr size_t WS_BUDGET = (size_t)4096 << 20;   // chunk so that per-chunk buffers stay below ~4 GiB
+#ifndef GL_WS_BUDGET_UV_GIB
+#define GL_WS_BUDGET_UV_GIB 16
+#endif
+static constexpr size_t WS_BUDGET_UV = (size_t)GL_WS_BUDGET_UV_GIB << 30;   // the split adjoint also keeps (u, v) of every ray
 // Backward modelling keeps n_amp component images per particle: with the 4 GiB budget a 30-amplitude model is cut into
 // chunks of ~280 particles, too few CTAs for the one-CTA-per-particle kernels (config 3: 506 -> see DESIGN.md section 16).
 static constexpr size_t WS_BUDGET_AMP = (size_t)16384 << 20;
@@ -247,7 +251,10 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     (void)M64;
     c->esize = d->precision == GL_PRECISION_F64 ? 8 : 4;
     c->ct_slot = d->n_systems == 1 ? ct_slot_acquire() : -1;      // constant-memory tap table of the uniform-tap step D
-    c->conv = conv_plan(G, c->esize, d->n_systems, c->ct_slot);   // also fills the padded-layout fields of G
+    c->uv_split = (c->esize == 8 && L.ker_nmax > 6) ? 1 : 0;      // must agree with coef_split<T, V>() in gl_ray.cuh
+    // what a full chunk holds, as bytes per particle per element of the ray image (conv_plan sizes its row bands by it)
+    const ConvChunkHint hint{d->amplitude_mode == 1 ? (size_t)0 : (c->uv_split ? WS_BUDGET_UV : WS_BUDGET), c->uv_split ? 3 : 1};
+    c->conv = conv_plan(G, c->esize, d->n_systems, c->ct_slot, hint);   // also fills the padded-layout fields of G
     if (c->conv.kind != 6 && c->ct_slot >= 0) { ct_slot_release(c->ct_slot); c->ct_slot = -1; }
     c->n_ctile = c->conv.n_ctile;
     // ray kernels: one CTA per (particle, phase plane, chunk); pick the block size that wastes the fewest lanes
@@ -270,7 +277,6 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     c->per_particle_bytes = (size_t)c->esize * ((size_t)PB_STRIDE + ray_stride(G) + gpix_stride(G) + (size_t)c->n_ctile +
                                                 (size_t)c->n_nap * c->na) + sizeof(double) + 6 * 256;
     if (d->amplitude_mode == 1) c->per_particle_bytes += (size_t)c->esize * c->n_amp * (gpix_stride(G) + ray_stride(G));
-    c->uv_split = (c->esize == 8 && L.ker_nmax > 6) ? 1 : 0;      // must agree with coef_split<T, V>() in gl_ray.cuh
     if (c->uv_split) c->per_particle_bytes += (size_t)c->esize * 2 * ray_stride(G);
     *out = c;
     return GL_OK;
@@ -291,14 +297,19 @@ struct Plan {
     size_t off_tab, off_kt, off_w, off_sl, off_pb, off_lpd, off_ray, off_gpix, off_chi, off_nap, off_uv, off_comp, off_cray, off_zobs, off_uw, off_sid, total;
 };
 
-static Plan make_plan(const gl_config* c, int64_t P) {
+// balanced: the batch is cut into the FEWEST chunks the budget allows, all of (almost) the same size, instead of full chunks
+// plus a small remainder (config 5: 5 x 410 instead of 4 x 487 + 100 -- a 100-particle chunk leaves most SMs idle in the
+// persistent and few-CTA kernels).  gl_workspace_bytes reports the unbalanced plan: an upper bound that is flat beyond the
+// chunk size, as include/gigalens.h promises.
+static Plan make_plan(const gl_config* c, int64_t P, bool balanced = true) {
     Plan pl{};
     const Geom& G = c->G;
     // the split adjoint keeps (u, v) of every ray: twice the budget keeps its chunks as large as the other variants'
-    int64_t pc_max = (int64_t)((c->desc.amplitude_mode == 1 ? WS_BUDGET_AMP : (c->uv_split ? 2 * WS_BUDGET : WS_BUDGET)) / c->per_particle_bytes);
+    int64_t pc_max = (int64_t)((c->desc.amplitude_mode == 1 ? WS_BUDGET_AMP : (c->uv_split ? WS_BUDGET_UV : WS_BUDGET)) / c->per_particle_bytes);
     if (pc_max < 1) pc_max = 1;
     if (pc_max > 32768) pc_max = 32768;
     pl.Pc = P < pc_max ? P : pc_max;
+    if (balanced && P > pc_max) { const int64_t nch = (P + pc_max - 1) / pc_max; pl.Pc = (P + nch - 1) / nch; }
     size_t o = 0;
     const size_t nsys = (size_t)c->desc.n_systems, es = (size_t)c->esize;
     pl.off_tab = o;  o = align256(o + sizeof(double) * MATH_TAB_DOUBLES);
@@ -328,7 +339,7 @@ static Plan make_plan(const gl_config* c, int64_t P) {
 
 extern "C" size_t gl_workspace_bytes(const gl_config* c, int64_t n_particles) {
     if (!c || n_particles <= 0) return 0;
-    return make_plan(c, n_particles).total;
+    return make_plan(c, n_particles, false).total;
 }
 
 // Diagnostic: where the per-particle block PB of the LAST processed chunk sits in the workspace, so that bench.py can

@@ -2,6 +2,7 @@
 // input-stationary sliding kernels for the tap counts of the BASELINE.json configs (U = 6, 11, 16 with s*s a
 // multiple of 4), generic kernels for every other shape.
 #pragma once
+#include <cmath>
 #include <cstdlib>
 #include "gl_common.cuh"
 #include "gl_conv.cuh"
@@ -40,7 +41,10 @@ struct ConvPlan {
 #define GL_CT_CW16 2
 #endif
 #ifndef GL_CT_BAND_ROWS
-#define GL_CT_BAND_ROWS 50
+#define GL_CT_BAND_ROWS 25
+#endif
+#ifndef GL_CT_TARGET_CTAS
+#define GL_CT_TARGET_CTAS 1776.0      // 6 waves of 148 SMs x 2 resident CTAs
 #endif
 #ifndef GL_CT_CW16B
 #define GL_CT_CW16B 4
@@ -137,7 +141,10 @@ static inline TsPlan ts_plan(const TsVariant& v, int wmax_default, int esize, in
 }
 
 // Fill the layout fields of G (UP, Hp, Wp, Hg, Wg, PADg) and choose the kernels.  esize = sizeof(T).
-static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems, int ct_slot = -1) {
+// What conv_plan may know about the batch: the workspace budget of a chunk and how many ray-image-sized buffers a particle
+// keeps (1, or 3 with the (u, v) buffer); budget 0 = plenty of particles per launch (backward modelling: n_amp virtual particles each).
+struct ConvChunkHint { size_t budget; int ray_bufs; };
+static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems, int ct_slot = -1, ConvChunkHint hint = ConvChunkHint{0, 1}) {
     ConvPlan pl{};
     const int U = G.U, N = G.N, NPH = G.s * G.s;
     pl.kind = 0;
@@ -191,8 +198,19 @@ static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems, int ct_slot 
             auto mkc = [&](int ncg) {
                 CtPlan cp{};
                 cp.ncg = ncg;
-                cp.n_bands = N / GL_CT_BAND_ROWS < 1 ? 1 : N / GL_CT_BAND_ROWS;      // geometry only (bit-identical chi^2 at any batch size)
+                // Row bands of the forward kernel: enough CTAs per launch to fill the machine several times over when a FULL chunk
+                // is processed (config 5: 410-487 particles x 50 column groups = 190 CTAs per band against 296 resident: 1 band ran
+                // 20.7 ms, 4 bands 14.2, 8 bands 13.6), but no thinner than GL_CT_BAND_ROWS rows (halo rows and partial tap groups
+                // are redone per band).  A function of the configuration only: the chi^2 partials, hence the bit-identity of a
+                // particle's result across batch sizes, depend on it.
+                const size_t per_particle = (size_t)esize * ((size_t)hint.ray_bufs * G.s * G.s * G.Hp * G.Wp + (size_t)G.Hg * G.Wg);
+                const double pc_full = hint.budget ? (double)hint.budget / (double)per_particle : 1e9;
+                const double ctas_per_band = pc_full * ncg / CT_NT;
+                int nb = (int)std::ceil(GL_CT_TARGET_CTAS / ctas_per_band);
+                const int nb_max = N / GL_CT_BAND_ROWS < 1 ? 1 : N / GL_CT_BAND_ROWS;
+                cp.n_bands = nb < 1 ? 1 : (nb > nb_max ? nb_max : nb);
                 cp.rbh = (N + cp.n_bands - 1) / cp.n_bands;
+                cp.n_bands = (N + cp.rbh - 1) / cp.rbh;
                 return cp;
             };
             pl.cf = mkc(nf); pl.cb = mkc(nb);

@@ -55,7 +55,7 @@ FWD64 = {
     "rotate_shear":   (10, 0),    # two 4-FMA chains + the two lab coordinates
     "multipoles":     (34, 0),
     "sersic":         (36, 0),    # 13 arithmetic (pre-scaled frame) + log2 7 + 2 exp2 16
-    "shapelet_fixed": (22, 0),    # u, v, two Gaussians through exp2
+    "shapelet_fixed": (13, 0),    # u, v, ONE Gaussian of u^2 + v^2 through exp2 (scaled basis, round 2; was 22 with two Gaussians)
     "sum":            (0, 0),     # folded into the component counts
 }
 ADJ64 = {
@@ -76,7 +76,9 @@ def shapelet_fwd(nmax):
 
 def shapelet_adj(nmax):
     ncoef = (nmax + 1) * (nmax + 2) // 2
-    return 4 * (nmax + 1) + 2 * ncoef + 2 * (nmax + 1) + ncoef     # derivatives, d/du d/dv contractions, coefficient sums
+    # scaled basis (round 2): a derivative is ONE operation, (k/2) psi_{k-1} - psi_{k+1} with the product shared with the
+    # recurrence, which runs one step further per family (4 operations); was 4 (nmax + 1) for the derivatives
+    return 2 * (nmax + 1) + 4 + 2 * ncoef + 2 * (nmax + 1) + ncoef   # derivatives, d/du d/dv contractions, coefficient sums
 
 
 # EPL series by band (csrc/gl_ray.cuh knuth_banded): one polynomial = 4 m recurrence steps of 2 FMA + a tail of 7 (fwd:
