@@ -141,7 +141,9 @@ __global__ void __launch_bounds__(CT_NT) gl_conv_fwd_ct(const __grid_constant__ 
     if (chi && act) chi[(p * cp.n_bands + band) * cp.ncg + g] = c2;
 }
 
-// Transpose of step D.  grid = (ceil(Pc * ncg / CT_NT), s*s): one phase plane per CTA row, every plane its own output.
+// Transpose of step D.  grid = (s*s, ceil(Pc * ncg / CT_NT)): one phase plane per CTA, every plane its own output; the plane is
+// the FASTEST grid index, so the s*s CTAs that read the same g_pix rows run together and share them in L2 (with the plane as the
+// slow index every plane re-read g_pix from DRAM: 4.0 GB per config-5 launch against 0.28 GB of g_pix).
 //   gbar_ab[R][j'] = sum_{k,l<U} kt_ab[U-1-k][U-1-l] gp[R + k][j' + l],  R in [oa, oa + N)
 template <class T, int U, int CW>
 __global__ void __launch_bounds__(CT_NT) gl_conv_bwd_ct(const __grid_constant__ Geom G, const CtPlan cp, int slot_c, int64_t Pc,
@@ -149,13 +151,13 @@ __global__ void __launch_bounds__(CT_NT) gl_conv_bwd_ct(const __grid_constant__ 
     using V2 = typename Vec2<T>::type;
     constexpr int SEG = (CW + U - 1 + 1) & ~1, UP2 = (U + 1) & ~1;
     const int N = G.N, s = G.s;
-    const int64_t item = (int64_t)blockIdx.x * CT_NT + threadIdx.x;
+    const int64_t item = (int64_t)blockIdx.y * CT_NT + threadIdx.x;
     const int64_t p = item / cp.ncg;
     const int g = (int)(item - p * cp.ncg);
     const bool act = p < Pc;                                         // idle lanes walk item 0 (convergent loop, see the forward kernel)
     const int64_t pa = act ? p : 0;
     const int ga = act ? g : 0;
-    const int ph = blockIdx.y, a = ph / s, oa = phase_shift(G, a);
+    const int ph = blockIdx.x, a = ph / s, oa = phase_shift(G, a);
     const T* in = gpix + (size_t)pa * gpix_stride(G) + (size_t)oa * G.Wg + (size_t)CW * ga;
     T* out = gbar + (size_t)pa * ray_stride(G) + ((size_t)ph * G.Hp + oa) * G.Wp + (size_t)CW * ga;
     T acc[U][CW];

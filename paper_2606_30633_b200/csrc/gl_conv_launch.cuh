@@ -2,6 +2,7 @@
 // input-stationary sliding kernels for the tap counts of the BASELINE.json configs (U = 6, 11, 16 with s*s a
 // multiple of 4), generic kernels for every other shape.
 #pragma once
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include "gl_common.cuh"
@@ -412,8 +413,13 @@ static inline cudaError_t conv_fwd_ct_launch(const ConvPlan& pl, const Geom& G, 
 }
 template <class T, int U, int CW>
 static inline cudaError_t conv_bwd_ct_launch(const ConvPlan& pl, const Geom& G, const T* gpix, int64_t Pc, T* gbar, cudaStream_t st) {
-    const dim3 grid((unsigned)((Pc * pl.cb.ncg + CT_NT - 1) / CT_NT), (unsigned)(G.s * G.s));
-    gl_conv_bwd_ct<T, U, CW><<<grid, CT_NT, 0, st>>>(G, pl.cb, pl.ct_slot, Pc, gpix, gbar);
+    // grid.y carries the items (the plane is the fastest index, gl_conv_ct.cuh): at most 65535 CTAs per launch -> slices of particles
+    const int64_t p_slice = std::max<int64_t>(1, (int64_t)65535 * CT_NT / pl.cb.ncg);
+    for (int64_t p0 = 0; p0 < Pc; p0 += p_slice) {
+        const int64_t n = std::min<int64_t>(p_slice, Pc - p0);
+        const dim3 grid((unsigned)(G.s * G.s), (unsigned)((n * pl.cb.ncg + CT_NT - 1) / CT_NT));
+        gl_conv_bwd_ct<T, U, CW><<<grid, CT_NT, 0, st>>>(G, pl.cb, pl.ct_slot, n, gpix + (size_t)p0 * gpix_stride(G), gbar + (size_t)p0 * ray_stride(G));
+    }
     return cudaSuccess;
 }
 // Refill the constant slot from the taps gl_prep_kernel wrote (system 0): plane-ordered table into `stage`, then a
