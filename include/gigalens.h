@@ -18,7 +18,10 @@
  *     allocates or frees device memory inside a call and keeps no reference to caller memory after return.
  *   - All arrays are fp32 (system_id: int32), C-contiguous, row index = y, column index = x (reading S1).
  *   - Calls are asynchronous on `stream`: no host synchronisation, no device-to-host copy.  Re-entrant on
- *     different streams with different workspaces.  The caller must not touch outputs or workspace until the
+ *     different streams with different workspaces -- with one proviso: calls that share a gl_config and overlap on
+ *     the GPU must pass the SAME psf (a single-system configuration may keep its convolution taps in a
+ *     per-configuration slot of constant memory that every call refills from its psf; to evaluate different PSFs
+ *     concurrently, create one configuration per PSF).  The caller must not touch outputs or workspace until the
  *     stream has reached the end of the call.
  *   - Errors are returned as gl_status; nothing is thrown or aborted across the ABI.  All argument checks run
  *     on the host before the first launch: on GL_ERR_NULL / _BAD_CONFIG / _BAD_SHAPE / _UNSUPPORTED / _WORKSPACE no

@@ -514,3 +514,58 @@ def test_graph_replay_matches_direct_call():
         m2 = gl.LensModel(wl.spec, *observation(1)[1:], wl.psf)
         lp2, g2 = m2.logpost_grad(z)
         assert torch.equal(lp, lp2) and torch.equal(g, g2)
+
+
+@pytest.mark.parametrize("shape", [(26, 2, 21), (22, 2, 31)])
+def test_uniform_tap_slots_many_live_configurations(shape):
+    """The uniform-tap step D keeps the taps of a single-system configuration in one of THREE slots of constant memory,
+    refilled by every call.  Five configurations of the same shape with different PSFs and
+    observations, alive together and evaluated in turn: the first three hold a slot (one launch more per call: the tap
+    staging kernel), the others run the tap-stationary kernels; every one must meet the strict bar against the oracle,
+    a second round of calls must reproduce the first bit for bit (no cross-talk between slots), and a configuration
+    created after one was destroyed inherits the freed slot."""
+    import gc
+    import oracle
+    import torch
+    gl = _gl()
+    gc.collect()                                 # configurations of earlier tests still waiting for collection would hold slots
+    n_pix, s, K = shape
+    cases = []
+    for i in range(5):
+        sp, obs, sigma, psf, z = _small_case(n_pix, s, K, 1, 0, -1, 1, seed=700 + 13 * i + K, n_particles=5)
+        rng = np.random.default_rng(50 + i)
+        psf = (psf * (1.0 + 0.3 * rng.random(psf.shape))).astype(np.float32)          # a different PSF per configuration
+        psf /= psf.sum(dtype=np.float64).astype(np.float32)
+        ref = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), None)
+        cases.append((sp, obs, sigma, psf, z, ref))
+
+    def check(m, c, first=None):
+        lp, g = m.logpost_grad(torch.from_numpy(c[4]).cuda())
+        n_launch = gl.gl_last_launch_count()
+        torch.cuda.synchronize()
+        if first is not None:
+            assert torch.equal(lp, first[0]) and torch.equal(g, first[1])
+        ref = c[5]
+        a, b = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+        fin = np.isfinite(ref["logp"])
+        assert fin.sum() >= 3 and np.array_equal(fin, np.isfinite(a))
+        assert np.all(np.abs(a[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+        ok, rep = grad_report(b[fin], ref["grad"][fin])
+        assert rep["n_fail"] == 0, rep
+        return (lp, g), n_launch
+
+    models = [gl.LensModel(c[0], c[1], c[2], c[3]) for c in cases[:4]]
+    first = [check(m, c) for m, c in zip(models, cases)]
+    launches = [n for _, n in first]
+    assert launches[0] == launches[1] == launches[2] == launches[3] + 1, launches     # three slots, then the fallback
+    for m, c, f in zip(models, cases, first):                                          # second round, same order
+        check(m, c, first=f[0])
+    for m, c, f in reversed(list(zip(models, cases, first))):                          # and in reverse order
+        check(m, c, first=f[0])
+    models[1].close()                                                                  # frees slot 1 ...
+    m5 = gl.LensModel(*cases[4][:4])                                                   # ... which the next configuration takes
+    _, n5 = check(m5, cases[4])
+    assert n5 == launches[0]
+    check(models[0], cases[0], first=first[0][0]); check(models[2], cases[2], first=first[2][0])
+    for m in (models[0], models[2], models[3], m5):
+        m.close()
