@@ -478,7 +478,8 @@ def run_ours(a):
         flush.zero_()                                    # evict L2 between timed iterations (outside the event pair)
         e0.record(); step(); e1.record()
     barrier()
-    t_dev = sum(e0.elapsed_time(e1) for e0, e1 in ev) * 1e-3
+    t_steps = [e0.elapsed_time(e1) for e0, e1 in ev]        # per-step device times (ms): median and min go into the line
+    t_dev = sum(t_steps) * 1e-3
     # e2e: host buffers (pinned), copies inside the timed region
     for _ in range(3):
         step_host()
@@ -493,6 +494,21 @@ def run_ours(a):
     t_e2e = sum(e0.elapsed_time(e1) for e0, e1 in ev2) * 1e-3
     if a.stage == "grad":
         assert torch.equal(lph, lp.cpu()) and torch.equal(gh, g.cpu()), "host-buffer path disagrees with the device path"
+    fwd_only = None
+    if a.stage == "grad" and a.amplitudes == "sampled":
+        # SURVEY 8(d) timing protocol: gl_logpost (steps A-E, no adjoint) timed separately, same batch, same L2 flush
+        nf = max(3, min(a.steps, 5))
+        for _ in range(3):
+            gl.gl_logpost(m.h, m.obs, m.noise_sigma, m.psf, z, sid, lp, ws)
+        ev3 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nf)]
+        for e0, e1 in ev3:
+            flush.zero_()
+            e0.record(); gl.gl_logpost(m.h, m.obs, m.noise_sigma, m.psf, z, sid, lp, ws); e1.record()
+        torch.cuda.synchronize()
+        tf = sorted(e0.elapsed_time(e1) for e0, e1 in ev3)
+        fwd_only = {"call": "gl_logpost", "value": P / (float(np.median(tf)) * 1e-3), "unit": UNIT, "steps": nf,
+                    "ms_per_step_median": float(np.median(tf)), "ms_per_step_min": tf[0]}
+        gl.gl_logpost_grad(m.h, m.obs, m.noise_sigma, m.psf, z, sid, lp, g, ws)      # lp, g of the gradient call again
     if a.stage == "hmc":
         lp = lpc
     finite = float(torch.isfinite(lp).float().mean())
@@ -522,7 +538,8 @@ def run_ours(a):
     roof["probe_T_laneops_per_s"] = probe
     wm = workmodel.per_eval(sp, a.precision)
     out = {"metric": METRIC, "value": whole_job_rate(world, P * evals_per_particle, a.steps, t_dev), "unit": UNIT, "n_gpus": world, "steps": a.steps,
-           "warmup": max(a.warmup, 3), "ms_per_step": t_dev / a.steps * 1e3, "higher_is_better": True,
+           "warmup": max(a.warmup, 3), "ms_per_step": t_dev / a.steps * 1e3, "ms_per_step_median": float(np.median(t_steps)),
+           "ms_per_step_min": float(min(t_steps)), "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": a.precision, "data": "synthetic",
            "config": {"workload": WORKLOAD_NAMES[k], "n_particles_per_gpu": P, "n_params": n_p,
                       "rays_per_particle": wm["rays"], "parallelism": "replicas x%d" % world, "stage": a.stage,
@@ -531,6 +548,8 @@ def run_ours(a):
            "e2e": {"value": whole_job_rate(world, P * evals_per_particle, a.steps, t_e2e), "unit": UNIT, "h2d_bytes_per_step": int(h2d_bytes),
                    "d2h_bytes_per_step": int(d2h_bytes), "ms_per_step": t_e2e / a.steps * 1e3},
            "gpu_launches": launches_per_step * a.steps, "clocks": clocks, "roofline": roof}
+    if fwd_only is not None:
+        out["forward_only"] = fwd_only
     if a.stage == "grad" and a.amplitudes == "sampled" and world == 1 and not a.no_all_configs:
         # free this config's buffers, then a few steps of every other BASELINE.json config (fp64) and of this one in fp32
         m.close()
