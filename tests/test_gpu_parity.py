@@ -516,6 +516,33 @@ def test_graph_replay_matches_direct_call():
         assert torch.equal(lp, lp2) and torch.equal(g, g2)
 
 
+def test_graph_replay_with_uniform_tap_step_d():
+    """The same for a configuration on the uniform-tap step D: the refill of the constant-memory
+    slot (a device-to-device copy to the symbol) is captured as a node of the graph, so a replay after ANOTHER
+    configuration has used a different slot, and after the captured parameters changed, equals a direct call."""
+    import gc
+    import torch
+    gl = _gl()
+    gc.collect()
+    sp, obs, sigma, psf, z0 = _small_case(26, 2, 21, 1, 0, -1, 1, seed=911, n_particles=6)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    z = torch.from_numpy(z0.copy()).cuda()
+    replay, lp, g = m.capture_logpost_grad(z)
+    sp_b, obs_b, sigma_b, psf_b, z_b = _small_case(26, 2, 21, 1, 0, -1, 1, seed=912, n_particles=6)
+    other = gl.LensModel(sp_b, obs_b, sigma_b, (psf_b * np.float32(1.25)))
+    for shift in (0.0, 0.02):
+        other.logpost_grad(torch.from_numpy(z_b).cuda())                       # another configuration between replays
+        z.copy_(torch.from_numpy(z0 + np.float32(shift)).cuda())
+        replay()
+        torch.cuda.synchronize()
+        m2 = gl.LensModel(sp, obs, sigma, psf)
+        lp2, g2 = m2.logpost_grad(z)
+        assert torch.isfinite(lp2).sum() >= 3
+        assert torch.equal(lp, lp2) and torch.equal(g, g2)
+        m2.close()
+    m.close(); other.close()
+
+
 @pytest.mark.parametrize("shape", [(26, 2, 21), (22, 2, 31)])
 def test_uniform_tap_slots_many_live_configurations(shape):
     """The uniform-tap step D keeps the taps of a single-system configuration in one of THREE slots of constant memory,
