@@ -455,7 +455,7 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
     GL_STAGE(ST_PREP, st, (gl_prep_kernel<T><<<c->desc.n_systems, 256, 0, st>>>(G, psf, mode == 2 ? nullptr : sigma, sys_kt, sys_w,
                                                                              sys_sl, tab_out)));
     ++t_launches;
-    if (c->conv.kind == 6) {                 // uniform-tap step D: refill this configuration's constant slot from the PSF of this call
+    if (c->conv.kind == 6 || c->conv.kind == 7) {                 // uniform-tap step D: refill this configuration's constant slot from the PSF of this call
         const int nk = conv_ct_upload<T>(c->conv, G, sys_kt, (T*)(w + pl.off_ctap), st);
         if (nk < 0) return GL_ERR_CUDA;
         t_launches += nk;

@@ -35,8 +35,8 @@ __device__ __forceinline__ T ctap(int slot, int idx) {
 // Tap table of ONE system in plane order, rows padded to UP2 = U rounded up to even: out[ph][u][UP2] with plane (a, b)
 // using kt[(a + c) % s][(b + c) % s]; this is what the constant slot holds.
 template <class T>
-__global__ void gl_ctap_stage_kernel(const __grid_constant__ Geom G, const T* __restrict__ sys_kt, T* __restrict__ out) {
-    const int s = G.s, U = G.U, UP2 = (U + 1) & ~1, NPH = s * s;
+__global__ void gl_ctap_stage_kernel(const __grid_constant__ Geom G, int NPH, const T* __restrict__ sys_kt, T* __restrict__ out) {
+    const int s = G.s, U = G.U, UP2 = (U + 1) & ~1;
     for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < NPH * U * UP2; e += gridDim.x * blockDim.x) {
         const int v = e % UP2, u = (e / UP2) % U, ph = e / (UP2 * U);
         const int a = ph / s, b = ph - a * s;
@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(CT_NT) gl_conv_fwd_ct(const __grid_constant__ 
                                                         const float* __restrict__ obs, int64_t p_base, T* __restrict__ gpix,
                                                         T* __restrict__ chi, float* __restrict__ out_model) {
     constexpr int SEG = (CW + U - 1 + 1) & ~1, UP2 = (U + 1) & ~1;
-    const int N = G.N, NPH = G.s * G.s;
+    const int N = G.N, NPH = G.binned ? 1 : G.s * G.s;         // binned (psf_grid 1, dedicated path): the image is plane 0
     const int64_t item = (int64_t)blockIdx.x * CT_NT + threadIdx.x;
     const int64_t p = item / cp.ncg;
     const int g = (int)(item - p * cp.ncg);

@@ -19,7 +19,7 @@ namespace gl {
 static inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
 struct ConvPlan {
-    int kind;                 // 6: uniform taps (single system; gl_conv_ct.cuh); 0 generic, 1: U=6 CW=4, 2: U=11 CW=2, 3: U=16 CW=2 (round-1 sliding kernels), 4: tap-stationary + TMA,
+    int kind;                 // 6: uniform taps (single system; gl_conv_ct.cuh); 7: the same on the binned plane of psf_grid 1; 0 generic, 1: U=6 CW=4, 2: U=11 CW=2, 3: U=16 CW=2 (round-1 sliding kernels), 4: tap-stationary + TMA,
                               // 5: psf_grid 1 dedicated: bin the planes, then tap-stationary on ONE plane with the K x K taps
     int CW;                   // output columns per thread
     SlidePlan fwd, bwd;
@@ -55,7 +55,10 @@ struct ConvPlan {
 #ifndef GL_CT_U6
 #define GL_CT_U6 0
 #endif
-static inline int ct_cw(int U) { return (U == 6 && GL_CT_U6) ? GL_CT_CW6 : (U == 11 ? GL_CT_CW11 : (U == 16 ? GL_CT_CW16 : 0)); }     // forward
+// U = 5, 7, 21 occur on the dedicated psf_grid = 1 path only (one binned plane, U = K taps per side)
+static inline int ct_cw(int U) {                                                                                       // forward
+    return (U == 6 && GL_CT_U6) ? GL_CT_CW6 : (U == 11 ? GL_CT_CW11 : (U == 16 ? GL_CT_CW16 : (U == 5 || U == 7 ? 4 : (U == 21 ? 2 : 0))));
+}
 static inline int ct_cwb(int U) { return U == 16 ? GL_CT_CW16B : ct_cw(U); }                                            // transpose
 static inline bool ct_fits(int U, int NPH) { return ct_cw(U) > 0 && NPH * U * ((U + 1) & ~1) <= CT_SLOT; }
 
@@ -166,29 +169,12 @@ static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems, int ct_slot 
     if (wg < CW * (ncg_b - 1) + SEG) wg = CW * (ncg_b - 1) + SEG;
     G.Wg = round_up(wg, 4);
     G.binned = 0;
-    {   // psf_grid 1: the dedicated bin-then-convolve path wherever a single-plane instance exists (GL_CONV_BIN=0: box-expanded)
-        const char* e = std::getenv("GL_CONV_BIN");
-        const int id = G.pgrid == 1 ? ts1_variant(U) : -1;
-        if (id >= 0 && !(e && e[0] == '0')) {
-            const TsVariant& v = k_ts1_variants[id];
-            const int NU = (v.U + v.G - 1) / v.G, UPAD = NU * v.G, o = G.c / G.s;     // every plane has the shift o = (K - 1) / 2
-            TsPlan tf = ts_plan(v, v.wmax_f, esize, N, 1, N + UPAD - 1, 0, true);
-            TsPlan tb = ts_plan(v, v.wmax_b, esize, N + o, 1, N + UPAD - 1, o, false);
-            if (tf.boxw <= 256 && tb.boxw <= 256 && v.CW * tb.ncg <= G.Wp) {
-                pl.kind = 5; pl.ts_id = id; pl.CW = v.CW; pl.tf = tf; pl.tb = tb; pl.n_ctile = tf.n_bands * tf.wpc;
-                G.binned = 1;
-                return pl;
-            }
-        }
-    }
-    if (pl.kind == 0) {
-        pl.n_ctile = (N * N + 255) / 256;
-        return pl;
-    }
     pl.ct_slot = -1;
-    {   // uniform taps (gl_conv_ct.cuh): one system, a free constant slot, a compiled tap count; GL_CONV_CT=0: off (A/B runs)
+    // uniform taps (gl_conv_ct.cuh): one system, a free constant slot, a compiled tap count; GL_CONV_CT=0: off (A/B runs).
+    // planes = s*s, or 1 on the dedicated psf_grid = 1 path (kind 7: the binned image in plane 0)
+    auto try_ct = [&](int planes, int kind) -> bool {
         const char* e = std::getenv("GL_CONV_CT");
-        if (ct_slot >= 0 && n_systems == 1 && ct_fits(U, NPH) && !(e && e[0] == '0')) {
+        if (ct_slot >= 0 && n_systems == 1 && ct_fits(U, planes) && !(e && e[0] == '0')) {
             const int cw = ct_cw(U), seg = (cw + U - 1 + 1) & ~1, cwb = ct_cwb(U), segb = (cwb + U - 1 + 1) & ~1;
             const int nf = (N + cw - 1) / cw, nb = (N + ob_max + cwb - 1) / cwb;
             int wp2 = G.Wp, wg2 = G.Wg;
@@ -215,10 +201,32 @@ static inline ConvPlan conv_plan(Geom& G, int esize, int n_systems, int ct_slot 
                 return cp;
             };
             pl.cf = mkc(nf); pl.cb = mkc(nb);
-            pl.kind = 6; pl.CW = cw; pl.ct_slot = ct_slot; pl.n_ctile = pl.cf.n_bands * pl.cf.ncg;
-            return pl;
+            pl.kind = kind; pl.CW = cw; pl.ct_slot = ct_slot; pl.n_ctile = pl.cf.n_bands * pl.cf.ncg;
+            return true;
+        }
+        return false;
+    };
+    {   // psf_grid 1: the dedicated bin-then-convolve path wherever a single-plane instance exists (GL_CONV_BIN=0: box-expanded)
+        const char* e = std::getenv("GL_CONV_BIN");
+        const int id = G.pgrid == 1 ? ts1_variant(U) : -1;
+        if (id >= 0 && !(e && e[0] == '0')) {
+            if (try_ct(1, 7)) { G.binned = 1; return pl; }      // uniform taps on the single binned plane
+            const TsVariant& v = k_ts1_variants[id];
+            const int NU = (v.U + v.G - 1) / v.G, UPAD = NU * v.G, o = G.c / G.s;     // every plane has the shift o = (K - 1) / 2
+            TsPlan tf = ts_plan(v, v.wmax_f, esize, N, 1, N + UPAD - 1, 0, true);
+            TsPlan tb = ts_plan(v, v.wmax_b, esize, N + o, 1, N + UPAD - 1, o, false);
+            if (tf.boxw <= 256 && tb.boxw <= 256 && v.CW * tb.ncg <= G.Wp) {
+                pl.kind = 5; pl.ts_id = id; pl.CW = v.CW; pl.tf = tf; pl.tb = tb; pl.n_ctile = tf.n_bands * tf.wpc;
+                G.binned = 1;
+                return pl;
+            }
         }
     }
+    if (pl.kind == 0) {
+        pl.n_ctile = (N * N + 255) / 256;
+        return pl;
+    }
+    if (try_ct(NPH, 6)) return pl;
     const int LS = pl.kind == 1 ? 4 : 1;                         // lanes per column group (conv_*_launch must agree)
     int ps = U * ((U + 1) & ~1);
     if (LS > 1) while ((2 * ps) % 32 != 8 && (2 * ps) % 32 != 24) ps += 2;   // 4 consecutive planes -> disjoint bank groups
@@ -417,7 +425,7 @@ static inline cudaError_t conv_bwd_ct_launch(const ConvPlan& pl, const Geom& G, 
     const int64_t p_slice = std::max<int64_t>(1, (int64_t)65535 * CT_NT / pl.cb.ncg);
     for (int64_t p0 = 0; p0 < Pc; p0 += p_slice) {
         const int64_t n = std::min<int64_t>(p_slice, Pc - p0);
-        const dim3 grid((unsigned)(G.s * G.s), (unsigned)((n * pl.cb.ncg + CT_NT - 1) / CT_NT));
+        const dim3 grid((unsigned)(G.binned ? 1 : G.s * G.s), (unsigned)((n * pl.cb.ncg + CT_NT - 1) / CT_NT));   // binned: plane 0 only
         gl_conv_bwd_ct<T, U, CW><<<grid, CT_NT, 0, st>>>(G, pl.cb, pl.ct_slot, n, gpix + (size_t)p0 * gpix_stride(G), gbar + (size_t)p0 * ray_stride(G));
     }
     return cudaSuccess;
@@ -426,8 +434,9 @@ static inline cudaError_t conv_bwd_ct_launch(const ConvPlan& pl, const Geom& G, 
 // device-to-device copy into c_ctap on the same stream.  Returns the number of kernels launched, negative on error.
 template <class T>
 static inline int conv_ct_upload(const ConvPlan& pl, const Geom& G, const T* sys_kt, T* stage, cudaStream_t st) {
-    const int n = G.s * G.s * G.U * ((G.U + 1) & ~1);
-    gl_ctap_stage_kernel<T><<<(n + 255) / 256, 256, 0, st>>>(G, sys_kt, stage);
+    const int nph = G.binned ? 1 : G.s * G.s;            // binned (psf_grid 1): every plane has the same taps, plane 0 is the image
+    const int n = nph * G.U * ((G.U + 1) & ~1);
+    gl_ctap_stage_kernel<T><<<(n + 255) / 256, 256, 0, st>>>(G, nph, sys_kt, stage);
     if (cudaMemcpyToSymbolAsync(c_ctap, stage, (size_t)n * sizeof(T), (size_t)pl.ct_slot * CT_SLOT * sizeof(double),
                                 cudaMemcpyDeviceToDevice, st) != cudaSuccess)
         return -1;
@@ -471,10 +480,21 @@ static inline int conv_fwd_launch(const ConvPlan& pl, const Geom& G, const T* ra
 #undef GL_TS_F
             return e == cudaSuccess ? 2 : -1;          // bin + step D
         }
+        case 7:
+            gl_bin_planes_kernel<T><<<dim3((unsigned)(((size_t)G.Hp * G.Wp + 255) / 256), (unsigned)Pc), 256, 0, st>>>(G, const_cast<T*>(ray));
+            [[fallthrough]];
         case 6:
-            if (G.U == 6) e = conv_fwd_ct_launch<T, 6, GL_CT_CW6>(pl, G, ray, sys_w, obs, p_base, Pc, gpix, chi, out_model, st);
-            else if (G.U == 11) e = conv_fwd_ct_launch<T, 11, GL_CT_CW11>(pl, G, ray, sys_w, obs, p_base, Pc, gpix, chi, out_model, st);
-            else e = conv_fwd_ct_launch<T, 16, GL_CT_CW16>(pl, G, ray, sys_w, obs, p_base, Pc, gpix, chi, out_model, st);
+#define GL_CT_F(U_, CW_) conv_fwd_ct_launch<T, U_, CW_>(pl, G, ray, sys_w, obs, p_base, Pc, gpix, chi, out_model, st)
+            switch (G.U) {
+                case 5: e = GL_CT_F(5, 4); break;
+                case 6: e = GL_CT_F(6, GL_CT_CW6); break;
+                case 7: e = GL_CT_F(7, 4); break;
+                case 11: e = GL_CT_F(11, GL_CT_CW11); break;
+                case 16: e = GL_CT_F(16, GL_CT_CW16); break;
+                default: e = GL_CT_F(21, 2); break;
+            }
+#undef GL_CT_F
+            if (pl.kind == 7) return e == cudaSuccess ? 2 : -1;   // bin + step D
             break;
         default: {
             dim3 grid((G.N * G.N + 255) / 256, (unsigned)Pc);
@@ -504,9 +524,17 @@ static inline int conv_bwd_launch(const ConvPlan& pl, const Geom& G, const T* gp
             break;
         }
         case 6:
-            if (G.U == 6) e = conv_bwd_ct_launch<T, 6, GL_CT_CW6>(pl, G, gpix, Pc, gbar, st);
-            else if (G.U == 11) e = conv_bwd_ct_launch<T, 11, GL_CT_CW11>(pl, G, gpix, Pc, gbar, st);
-            else e = conv_bwd_ct_launch<T, 16, GL_CT_CW16B>(pl, G, gpix, Pc, gbar, st);
+        case 7:
+#define GL_CT_B(U_, CW_) conv_bwd_ct_launch<T, U_, CW_>(pl, G, gpix, Pc, gbar, st)
+            switch (G.U) {
+                case 5: e = GL_CT_B(5, 4); break;
+                case 6: e = GL_CT_B(6, GL_CT_CW6); break;
+                case 7: e = GL_CT_B(7, 4); break;
+                case 11: e = GL_CT_B(11, GL_CT_CW11); break;
+                case 16: e = GL_CT_B(16, GL_CT_CW16B); break;
+                default: e = GL_CT_B(21, 2); break;
+            }
+#undef GL_CT_B
             break;
         default: {
             dim3 grid((G.s * G.s * G.N * G.N + 255) / 256, (unsigned)Pc);
