@@ -32,6 +32,7 @@ struct gl_config {
     int variant;        // 0: <.,0,1,-1,1>  1: <.,0,1,6,2>  2: <.,3,1,10,2>  3: <.,0,2,-1,3>  4: <.,3,2,10,3>
     int na;             // natural accumulators per chunk for the variant
     int nt_fwd, nt_adj, rpt_fwd, rpt_adj, n_chunk_fwd, n_chunk_adj;   // per phase plane
+    int nt_fwd_b, rpt_fwd_b, n_chunk_fwd_b;   // binned forward kernel (psf_grid 1, dedicated path): pixels per thread, chunks per particle
     int n_nap;          // adjoint partials per particle = s*s*n_chunk_adj
     int n_ctile;        // chi^2 partials per particle
     ConvPlan conv;
@@ -273,6 +274,7 @@ extern "C" gl_status gl_config_create(const gl_config_desc* d, gl_config** out) 
     };
     pick(NT_FWD, GL_RPT_FWD, c->nt_fwd, c->rpt_fwd, c->n_chunk_fwd);
     pick(NT_ADJ, GL_RPT_ADJ, c->nt_adj, c->rpt_adj, c->n_chunk_adj);
+    pick(NT_FWD, std::max(1, GL_RPT_FWD / (G.s * G.s)), c->nt_fwd_b, c->rpt_fwd_b, c->n_chunk_fwd_b);   // a pixel = s*s rays
     c->n_nap = G.s * G.s * c->n_chunk_adj;
     c->per_particle_bytes = (size_t)c->esize * ((size_t)PB_STRIDE + ray_stride(G) + gpix_stride(G) + (size_t)c->n_ctile +
                                                 (size_t)c->n_nap * c->na) + sizeof(double) + 6 * 256;
@@ -356,6 +358,11 @@ extern "C" gl_status gl_workspace_layout(const gl_config* c, int64_t n_particles
 // ----------------------------------------------------------------------------- variant dispatch
 template <class T, class V>
 static void launch_ray_fwd(const gl_config* c, const T* pb, const double* tab, T* ray, int64_t Pc, cudaStream_t st) {
+    if (c->G.binned) {       // psf_grid 1, dedicated path: the binned image straight into plane 0 (gl_ray_fwd_binned_kernel)
+        dim3 grid(c->n_chunk_fwd_b, (unsigned)Pc);
+        gl_ray_fwd_binned_kernel<T, V, NT_FWD><<<grid, c->nt_fwd_b, 0, st>>>(c->G, pb, tab, ray, c->rpt_fwd_b, c->n_chunk_fwd_b);
+        return;
+    }
     dim3 grid(c->G.s * c->G.s * c->n_chunk_fwd, (unsigned)Pc);
     gl_ray_fwd_kernel<T, V, NT_FWD, RB_FWD><<<grid, c->nt_fwd, 0, st>>>(c->G, pb, tab, ray, c->rpt_fwd, c->n_chunk_fwd);
 }
@@ -505,7 +512,7 @@ static gl_status run_t(const gl_config* c, int mode, const float* obs, const flo
             GL_STAGE(ST_RAY_FWD, st, ray_fwd<T>(c, pb, tab, ray, Pc, st)); ++t_launches;
             GL_STAGE(ST_CONV_FWD, st, nl = conv_fwd_launch<T>(c->conv, G, ray, sys_kt, sys_w, obs, system_id, base, Pc,
                                              mode == 2 ? nullptr : gpix, mode == 2 ? nullptr : chi,
-                                             mode == 2 ? out_image : nullptr, st));
+                                             mode == 2 ? out_image : nullptr, st, /*prebinned=*/G.binned != 0));
             if (nl < 0) return GL_ERR_CUDA;
             t_launches += nl;
         }

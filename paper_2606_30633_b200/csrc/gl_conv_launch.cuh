@@ -379,7 +379,7 @@ static inline cudaError_t ts_grid(K kern, const TsPlan& pl, size_t smem, int64_t
 template <class T, int U, int G_, int NPH, int CW, int RPS>
 static inline cudaError_t conv_fwd_ts_launch(const ConvPlan& pl, const Geom& G, const T* ray, const T* sys_kt, const T* sys_w,
                                              const float* obs, const int32_t* system_id, int64_t p_base, int64_t Pc, T* gpix,
-                                             T* chi, float* out_model, cudaStream_t st) {
+                                             T* chi, float* out_model, cudaStream_t st, bool prebinned = false) {
     CUtensorMap tm;
     // plane index in the middle: {Wp, NPH * Pc (stride Hp Wp), Hp (stride Wp)} -> a box lands as [RPS][NPH][boxw];
     // binned path (NPH = 1): plane 0 of every particle, one ray_stride apart
@@ -387,7 +387,7 @@ static inline cudaError_t conv_fwd_ts_launch(const ConvPlan& pl, const Geom& G, 
     if (!ts_make_map<T>(&tm, ray, (uint64_t)G.Wp, (uint64_t)NPH * (uint64_t)Pc, (uint64_t)G.Hp, pstride, (uint64_t)G.Wp,
                         (uint32_t)pl.tf.boxw, NPH, RPS))
         return cudaErrorInvalidValue;
-    if (G.binned) gl_bin_planes_kernel<T><<<dim3((unsigned)(((size_t)G.Hp * G.Wp + 255) / 256), (unsigned)Pc), 256, 0, st>>>(G, const_cast<T*>(ray));
+    if (G.binned && !prebinned) gl_bin_planes_kernel<T><<<dim3((unsigned)(((size_t)G.Hp * G.Wp + 255) / 256), (unsigned)Pc), 256, 0, st>>>(G, const_cast<T*>(ray));
     auto kern = gl_conv_fwd_ts<T, U, G_, NPH, CW, RPS>;
     const size_t smem = ts_smem_bytes<T>(pl.tf);
     unsigned grid = 0;
@@ -464,24 +464,25 @@ static inline int conv_ct_upload(const ConvPlan& pl, const Geom& G, const T* sys
 template <class T>
 static inline int conv_fwd_launch(const ConvPlan& pl, const Geom& G, const T* ray, const T* sys_kt, const T* sys_w,
                                   const float* obs, const int32_t* system_id, int64_t p_base, int64_t Pc,
-                                  T* gpix, T* chi, float* out_model, cudaStream_t st) {
+                                  T* gpix, T* chi, float* out_model, cudaStream_t st, bool prebinned = false) {
+    // prebinned (psf_grid 1, dedicated path): plane 0 already holds the binned image (gl_ray_fwd_binned_kernel): no bin pass
     cudaError_t e = cudaSuccess;
     switch (pl.kind) {
         case 1: e = conv_fwd_is_launch<T, 6, 4, 4, 256>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st); break;
         case 2: e = conv_fwd_is2_launch<T, 11, 2, 256>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st); break;
         case 3: e = conv_fwd_is2_launch<T, 16, 2, 256>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st); break;
         case 4: {
-#define GL_TS_F(U_, G__, NPH_, CW_, RPS_) conv_fwd_ts_launch<T, U_, G__, NPH_, CW_, RPS_>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st)
+#define GL_TS_F(U_, G__, NPH_, CW_, RPS_) conv_fwd_ts_launch<T, U_, G__, NPH_, CW_, RPS_>(pl, G, ray, sys_kt, sys_w, obs, system_id, p_base, Pc, gpix, chi, out_model, st, prebinned)
             GL_TS_DISPATCH(GL_TS_F)
             break;
         }
         case 5: {
             GL_TS1_DISPATCH(GL_TS_F)
 #undef GL_TS_F
-            return e == cudaSuccess ? 2 : -1;          // bin + step D
+            return e == cudaSuccess ? (prebinned ? 1 : 2) : -1;          // (bin +) step D
         }
         case 7:
-            gl_bin_planes_kernel<T><<<dim3((unsigned)(((size_t)G.Hp * G.Wp + 255) / 256), (unsigned)Pc), 256, 0, st>>>(G, const_cast<T*>(ray));
+            if (!prebinned) gl_bin_planes_kernel<T><<<dim3((unsigned)(((size_t)G.Hp * G.Wp + 255) / 256), (unsigned)Pc), 256, 0, st>>>(G, const_cast<T*>(ray));
             [[fallthrough]];
         case 6:
 #define GL_CT_F(U_, CW_) conv_fwd_ct_launch<T, U_, CW_>(pl, G, ray, sys_w, obs, p_base, Pc, gpix, chi, out_model, st)
@@ -494,7 +495,7 @@ static inline int conv_fwd_launch(const ConvPlan& pl, const Geom& G, const T* ra
                 default: e = GL_CT_F(21, 2); break;
             }
 #undef GL_CT_F
-            if (pl.kind == 7) return e == cudaSuccess ? 2 : -1;   // bin + step D
+            if (pl.kind == 7) return e == cudaSuccess ? (prebinned ? 1 : 2) : -1;   // (bin +) step D
             break;
         default: {
             dim3 grid((G.N * G.N + 255) / 256, (unsigned)Pc);

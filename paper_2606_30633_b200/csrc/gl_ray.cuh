@@ -554,6 +554,53 @@ __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ 
     }
 }
 
+// Steps B + C on the dedicated psf_grid = 1 path (Geom.binned): that path convolves the BINNED image, the sum of the s*s
+// phase planes, which all carry the same shift o there.  One thread evaluates the s*s rays of a detector pixel and adds them
+// in the order of the bin pass (plane 0, 1, ..., s*s - 1: bit-identical to writing the planes and running
+// gl_bin_planes_kernel), and only plane 0 is written: no bin pass (s*s + 1 plane-sized HBM transfers per particle) and s*s times
+// fewer bytes stored here.  grid = (n_chunk, Pc); CTA ck handles pixels [ck nt RPT, (ck + 1) nt RPT) of the N*N.
+template <class T, class V, int NT>
+__global__ void __launch_bounds__(NT) gl_ray_fwd_binned_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
+                                                               const double* __restrict__ tabg, T* __restrict__ ray, int RPT,
+                                                               int n_chunk) {
+    __shared__ __align__(16) T pb[PB_STRIDE];
+    __shared__ __align__(128) double tabs[TabStage<T>::N];
+    const int p = blockIdx.y, ck = blockIdx.x;
+    const T* src = pbg + (size_t)p * PB_STRIDE;
+    for (int k = threadIdx.x; k < V::PB_NEED; k += blockDim.x) pb[k] = src[k];
+    __shared__ __align__(16) T cfs[V::MASS == 1 ? 3 * SER_PITCH : 4];
+    __shared__ __align__(16) float cf32[(sizeof(T) == 8 && V::MASS == 1) ? 3 * SER_PITCH : 4];
+    if constexpr (V::MASS == 1) stage_series<T>(src, cfs, cf32);
+    const typename Real<T>::Tab tb = TabStage<T>::make(tabs, tabg);
+    __syncthreads();
+    T* out = ray + (size_t)p * ray_stride(G);                       // plane 0
+    const int o = phase_shift(G, 0), N = G.N, s = G.s;
+    {
+        const int tot = G.Hp * G.Wp;
+        for (int e = ck * blockDim.x + threadIdx.x; e < tot; e += n_chunk * blockDim.x) {
+            const int r = e / G.Wp, cc = e - r * G.Wp;
+            if (r < o || r >= o + N || cc < o || cc >= o + N) out[e] = T(0.);
+        }
+    }
+    const int NN = N * N;
+    const bool valid = pb[PB_VALID] != T(0.);
+    const float half = 0.5f * (float)(G.M - 1);
+    int idx = ck * (blockDim.x * RPT) + threadIdx.x;
+    for (int r = 0; r < RPT; ++r, idx += blockDim.x) {
+        if (idx >= NN) break;
+        const int i1 = idx / N, j1 = idx - i1 * N;
+        T sum = T(0.);
+        for (int a = 0; a < s; ++a)
+            for (int b = 0; b < s; ++b) {
+                int off = 0; asm volatile("" : "+r"(off));      // opaque: keeps the PB scalars in shared memory, not in registers
+                const T v = ray_eval<T, V, false>(tb, pb + off, cfs + off, cf32 + off, (T)((float)(s * j1 + b) - half),
+                                                  (T)((float)(s * i1 + a) - half), T(0.), nullptr);
+                sum = (a | b) == 0 ? v : sum + v;
+            }
+        out[(size_t)(i1 + o) * G.Wp + (j1 + o)] = valid ? sum : T(0.);
+    }
+}
+
 // Component images of backward modelling: steps B-C once per ray (one deflection), every light component with unit
 // amplitude stored in its own RAY buffer: comp_ray [n_amp][Pc][ray_stride].  Same grid as gl_ray_fwd_kernel.
 template <class T, class V, int NT>
