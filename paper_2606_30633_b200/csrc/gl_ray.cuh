@@ -11,6 +11,7 @@
 #pragma once
 #include "gl_common.cuh"
 #include "gl_math.cuh"
+#include <type_traits>
 
 namespace gl {
 
@@ -479,9 +480,40 @@ __device__ __forceinline__ T ray_eval(const typename Real<T>::Tab& tb, const T* 
 // Ray coordinates are taken relative to the grid CENTRE (fj = j - (M-1)/2, exact in fp32), so that a position minus a
 // component centre keeps its relative accuracy near that centre, where the light profiles are steepest.
 struct PlaneIter {
+    int ph, a, b, oa, ob, idx, j1, dj, off, doff, wrap_off;
+    float fjf, fif, dfj, dfi, wrap_fj, wrap_fi;       // centre-relative ray coordinates, exact in fp32 (multiples of 1/2 below 2^12)
+    // Everything a ray needs from its index -- element offset in the plane, (fj, fi) -- advances by additions: the products
+    // and int -> float conversions per ray were ~5 % of the forward kernel's instructions on config 2.
+    __device__ __forceinline__ PlaneIter(const Geom& G, int n_chunk, int RPT) {
+        ph = blockIdx.x / n_chunk;
+        const int ck = blockIdx.x - ph * n_chunk;
+        a = ph / G.s; b = ph - a * G.s; oa = phase_shift(G, a); ob = phase_shift(G, b);
+        idx = ck * (blockDim.x * RPT) + threadIdx.x;
+        const int i1 = idx / G.N;
+        j1 = idx - i1 * G.N;
+        const int di = blockDim.x / G.N;
+        dj = blockDim.x - di * G.N;
+        const float half = 0.5f * (float)(G.M - 1);
+        off = (i1 + oa) * G.Wp + (j1 + ob); doff = di * G.Wp + dj; wrap_off = G.Wp - G.N;
+        fjf = (float)(G.s * j1 + b) - half; fif = (float)(G.s * i1 + a) - half;
+        dfj = (float)(G.s * dj); dfi = (float)(G.s * di); wrap_fj = -(float)(G.s * G.N); wrap_fi = (float)G.s;
+    }
+    __device__ __forceinline__ void next(const Geom& G) {
+        idx += blockDim.x; j1 += dj; off += doff; fjf += dfj; fif += dfi;
+        if (j1 >= G.N) { j1 -= G.N; off += wrap_off; fjf += wrap_fj; fif += wrap_fi; }
+    }
+    template <class T> __device__ __forceinline__ T fj(const Geom&) const { return (T)fjf; }
+    template <class T> __device__ __forceinline__ T fi(const Geom&) const { return (T)fif; }
+    __device__ __forceinline__ size_t offset(const Geom&) const { return (size_t)off; }
+};
+
+// The same mapping with the smallest state (index, row, column; offset and coordinates computed per ray): for the adjoint
+// variants that keep the shapelet coefficient sums in registers next to everything else (fp64, n_max <= 6: 254 registers), where
+// the six more live values of PlaneIter cost more than the instructions they save (config 3: 17.5 against 18.2 ms).
+struct PlaneIterLean {
     int ph, a, b, oa, ob, idx, i1, j1, di, dj;
     float half;
-    __device__ __forceinline__ PlaneIter(const Geom& G, int n_chunk, int RPT) {
+    __device__ __forceinline__ PlaneIterLean(const Geom& G, int n_chunk, int RPT) {
         ph = blockIdx.x / n_chunk;
         const int ck = blockIdx.x - ph * n_chunk;
         a = ph / G.s; b = ph - a * G.s; oa = phase_shift(G, a); ob = phase_shift(G, b);
@@ -510,6 +542,20 @@ template <> struct TabStage<double> {
     static __device__ __forceinline__ MathTab make(double* sm, const double* g) { stage_math_tab(sm, g); return math_tab(sm); }
 };
 
+// Zero the border of one padded plane (everything outside the N x N interior at (oa, ob)); element e = first, first + stride, ...
+// Row and column advance incrementally: one integer division per thread instead of one per element (the division loop was 7 % of
+// the forward kernel's instructions on config 2).
+template <class T>
+__device__ __forceinline__ void zero_plane_border(const Geom& G, T* __restrict__ out, int oa, int ob, int first, int stride) {
+    const int tot = G.Hp * G.Wp, dr = stride / G.Wp, dc = stride - dr * G.Wp;
+    int r = first / G.Wp, cc = first - r * G.Wp;
+    for (int e = first; e < tot; e += stride) {
+        if (r < oa || r >= oa + G.N || cc < ob || cc >= ob + G.N) out[e] = T(0.);
+        r += dr; cc += dc;
+        if (cc >= G.Wp) { cc -= G.Wp; ++r; }
+    }
+}
+
 // Steps B + C.  Writes the plane interior and zeroes this CTA's share of the plane border.
 template <class T, class V, int NT, int RB>
 __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ Geom G, const T* __restrict__ pbg,
@@ -527,13 +573,7 @@ __global__ void __launch_bounds__(NT) gl_ray_fwd_kernel(const __grid_constant__ 
     __syncthreads();
     PlaneIter it(G, n_chunk, RPT);
     T* out = ray + (size_t)p * ray_stride(G) + (size_t)it.ph * G.Hp * G.Wp;
-    {
-        const int ck = blockIdx.x - it.ph * n_chunk, tot = G.Hp * G.Wp;
-        for (int e = ck * blockDim.x + threadIdx.x; e < tot; e += n_chunk * blockDim.x) {
-            const int r = e / G.Wp, cc = e - r * G.Wp;
-            if (r < it.oa || r >= it.oa + G.N || cc < it.ob || cc >= it.ob + G.N) out[e] = T(0.);
-        }
-    }
+    zero_plane_border(G, out, it.oa, it.ob, (blockIdx.x - it.ph * n_chunk) * blockDim.x + threadIdx.x, n_chunk * blockDim.x);
     const int NN = G.N * G.N;
     const bool valid = pb[PB_VALID] != T(0.);
     // RB rays per step, evaluated unconditionally in one basic block so that the scheduler interleaves their
@@ -575,13 +615,7 @@ __global__ void __launch_bounds__(NT) gl_ray_fwd_binned_kernel(const __grid_cons
     __syncthreads();
     T* out = ray + (size_t)p * ray_stride(G);                       // plane 0
     const int o = phase_shift(G, 0), N = G.N, s = G.s;
-    {
-        const int tot = G.Hp * G.Wp;
-        for (int e = ck * blockDim.x + threadIdx.x; e < tot; e += n_chunk * blockDim.x) {
-            const int r = e / G.Wp, cc = e - r * G.Wp;
-            if (r < o || r >= o + N || cc < o || cc >= o + N) out[e] = T(0.);
-        }
-    }
+    zero_plane_border(G, out, o, o, ck * blockDim.x + threadIdx.x, n_chunk * blockDim.x);
     const int NN = N * N;
     const bool valid = pb[PB_VALID] != T(0.);
     const float half = 0.5f * (float)(G.M - 1);
@@ -619,14 +653,8 @@ __global__ void __launch_bounds__(NT) gl_ray_comp_kernel(const __grid_constant__
     __syncthreads();
     PlaneIter it(G, n_chunk, RPT);
     T* out = comp_ray + (size_t)p * ray_stride(G) + (size_t)it.ph * G.Hp * G.Wp;
-    {
-        const int ck = blockIdx.x - it.ph * n_chunk, tot = G.Hp * G.Wp;
-        for (int e = ck * blockDim.x + threadIdx.x; e < tot; e += n_chunk * blockDim.x) {
-            const int r = e / G.Wp, cc = e - r * G.Wp;
-            if (r < it.oa || r >= it.oa + G.N || cc < it.ob || cc >= it.ob + G.N)
-                for (int k = 0; k < n_amp; ++k) out[(size_t)k * cstride + e] = T(0.);
-        }
-    }
+    for (int k = 0; k < n_amp; ++k)
+        zero_plane_border(G, out + (size_t)k * cstride, it.oa, it.ob, (blockIdx.x - it.ph * n_chunk) * blockDim.x + threadIdx.x, n_chunk * blockDim.x);
     const int NN = G.N * G.N;
     const bool valid = pb[PB_VALID] != T(0.);
     for (int r = 0; r < RPT; ++r) {
@@ -665,7 +693,8 @@ __global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC 
     if constexpr (V::MASS == 1) stage_series<T>(src, cfs, cf32);
     const typename Real<T>::Tab tb = TabStage<T>::make(tabs, tabg);
     __syncthreads();
-    PlaneIter it(G, n_chunk, RPT);
+    using Iter = typename std::conditional<(sizeof(T) == 8 && V::NMAX >= 0 && !coef_split<T, V>()), PlaneIterLean, PlaneIter>::type;
+    Iter it(G, n_chunk, RPT);
     const T* gb = gbar + (size_t)p * ray_stride(G) + (size_t)(G.binned ? 0 : it.ph) * G.Hp * G.Wp;   // binned: one gbar plane for all
     const int NN = G.N * G.N;
     constexpr bool CS = coef_split<T, V>();
@@ -680,7 +709,7 @@ __global__ void __launch_bounds__(NT, (sizeof(T) == 8 && V::NMAX < 0 && V::NSRC 
             int off = 0; asm volatile("" : "+r"(off));      // opaque: keeps the PB scalars in shared memory, not in registers
             if (it.idx < NN) {
                 const size_t o = it.offset(G);
-                ray_eval<T, V, true>(tb, pb + off, cfs + off, cf32 + off, it.fj<T>(G), it.fi<T>(G), gb[o], acc, CS ? uvb + o : nullptr, rs);
+                ray_eval<T, V, true>(tb, pb + off, cfs + off, cf32 + off, it.template fj<T>(G), it.template fi<T>(G), gb[o], acc, CS ? uvb + o : nullptr, rs);
             }
             it.next(G);
         }
