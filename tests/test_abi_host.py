@@ -97,7 +97,14 @@ def test_argument_checks_precede_any_cuda_call(gl):
     assert L.gl_model_image(h, null, null, null, 0, null, null, 0, null) == 0
     assert L.gl_logpost_grad_host(h, null, null, null, null, null, 0, null, null, null, 0, null) == 0
     assert L.gl_workspace_bytes(null, 8) == 0 and L.gl_config_n_params(null) == 0
-    for s in range(0, -7, -1):
+    # gl_logpost_grad_noalloc: the same checks, and the size limit, answered before any CUDA call
+    assert L.gl_logpost_grad_noalloc(null, null, null, null, null, null, 4, null, null, null) == -1
+    assert L.gl_logpost_grad_noalloc(h, null, null, null, null, null, -1, null, null, null) == -3
+    assert L.gl_logpost_grad_noalloc(h, null, null, null, null, null, 0, null, null, null) == 0
+    assert gl.gl_workspace_bytes(h, 10 ** 6) > gl.GL_NOALLOC_MAX_BYTES
+    assert L.gl_logpost_grad_noalloc(h, null, null, null, null, null, 10 ** 6, null, null, null) == -7
+    assert "GL_NOALLOC_MAX_BYTES" in L.gl_status_string(-7).decode()
+    for s in range(0, -8, -1):
         assert L.gl_status_string(s).decode().startswith("GL_")
     assert L.gl_stage_count() == 8 and L.gl_stage_name(2).decode() == "ray_fwd" and L.gl_stage_name(7).decode() == "amplitude_solve"
     gl.gl_config_destroy(h)
