@@ -54,12 +54,14 @@ struct CtPlan {
 constexpr int CT_NT = 128;      // no minimum-blocks bound: ptxas then settles at 168 registers (3 CTAs per SM) for the U = 11 transpose; (CT_NT, 1) took 182 and measured 30 % slower, (CT_NT, 3) spills at U = 16
 
 // acc[u][q] += sum_v tap[u][v] seg[q + v] for the tap rows u in [ulo, uhi]; FLIP: the transpose's taps kt[U-1-u][U-1-v].
-// Tap rows are taken in groups of GU with the tap column v as the OUTER loop inside a group, so that two FMAs into the same
+// Tap rows are taken in groups of GU = 4 with the tap column v as the OUTER loop inside a group, so that two FMAs into the same
 // accumulator are GU * CW instructions apart (with u outermost they were CW apart: the kernel waited on the FP64 latency);
-// a group runs if any of its rows is wanted -- the other rows of it then add into accumulators that are never emitted.
+// a group runs if any of its rows is wanted -- the other rows of it then add into accumulators that are never emitted, which is
+// the price of coarse groups at the edges of a row band (measured: at CW = 2 groups of 4 beat groups of 8, config 3 step D 7.17 ->
+// 6.26 ms; at CW = 4 groups of 4 beat groups of 2 and 3).
 template <class T, int U, int CW, int SEG, bool FLIP>
 __device__ __forceinline__ void ct_slide(T (&acc)[U][CW], int slot, int tbase, const T (&seg)[SEG], int ulo, int uhi) {
-    constexpr int UP2 = (U + 1) & ~1, GU = (16 / CW) < 1 ? 1 : 16 / CW;
+    constexpr int UP2 = (U + 1) & ~1, GU = CW >= 4 ? ((16 / CW) < 1 ? 1 : 16 / CW) : 4;
 #pragma unroll
     for (int u0 = 0; u0 < U; u0 += GU) {
         if (u0 + GU - 1 >= ulo && u0 <= uhi) {
