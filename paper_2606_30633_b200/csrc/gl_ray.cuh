@@ -42,7 +42,7 @@ __device__ __forceinline__ void knuth(const T* __restrict__ cf, T p, T nf2, T wr
 
 // K real-coefficient polynomials in the same w at once, in precision bands (all bounds are per-particle, hence
 // CTA-uniform: no divergence).  Term k of the series is O(f^k) relative to the sum, so (gl_unpack_kernel picks M1, M2):
-//   k > kt = 4(M1+M2)+1      dropped: 30 f^(kt+1) <= 3e-16 (fp64 mode) -- numerically zero;
+//   k > kt = 4(M1+M2)+1      dropped: 30 f^(kt+1) <= 1e-12 (fp64 mode, GL_SERIES_DROP) -- an order below the fp32 band's rounding;
 //   4 M1 < k <= kt           recurrence steps in fp32 on the otherwise idle FP32 pipe: their rounding enters the sum
 //                            scaled by f^k, 30 f^(4 M1 + 1) 1e-7 <= 1e-11;
 //   k <= 4 M1                recurrence steps in T.
