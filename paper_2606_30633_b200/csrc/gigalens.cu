@@ -111,11 +111,15 @@ static constexpr int NT_ADJ = GL_NT_ADJ;
 #ifndef GL_RB_FWD
 #define GL_RB_FWD 1
 #endif
+// Rays per thread the ray kernels aim for (a plane's rays are cut into chunks of about nt * RPT): every CTA stages the particle's
+// block and the series coefficients before its first ray, so longer threads amortise that better -- 40 / 64 (round 1, tuned on
+// config 2 where a plane is one chunk anyway) against 160 / 256: config 5 adjoint 90.3 -> 87.8 ms, forward 37.4 -> 37.0, config 3
+// 17.2 -> 16.9 and 7.43 -> 7.24; 512 gains another 1 % on config 5 but leaves 32 CTAs per particle.
 #ifndef GL_RPT_FWD
-#define GL_RPT_FWD 40
+#define GL_RPT_FWD 160
 #endif
 #ifndef GL_RPT_ADJ
-#define GL_RPT_ADJ 64
+#define GL_RPT_ADJ 256
 #endif
 static constexpr int RB_FWD = GL_RB_FWD;  // rays a forward thread evaluates concurrently
 static constexpr size_t WS_BUDGET = (size_t)4096 << 20;   // chunk so that per-chunk buffers stay below ~4 GiB
