@@ -129,7 +129,10 @@ typedef struct gl_config gl_config;   /* opaque, immutable, host-side, library-o
 gl_status gl_config_create(const gl_config_desc* desc, gl_config** out);
 
 /* Free a handle from gl_config_create (NULL is a no-op).  Must not race with a host call using it;
- * work already enqueued on a stream does not reference the handle. */
+ * work already enqueued on a stream does not reference the handle.  One resource outlives it: a single-system
+ * configuration may hold a slot of constant memory for its convolution taps, which the next configuration created
+ * may take over -- the first call on that new configuration must be ordered after the destroyed one's enqueued work
+ * (same stream, or an event), as it is whenever one stream is used. */
 void gl_config_destroy(gl_config* cfg);
 
 /* Parameter count implied by a configuration (S18); 0 if cfg is NULL. */
