@@ -596,3 +596,39 @@ def test_uniform_tap_slots_many_live_configurations(shape):
     check(models[0], cases[0], first=first[0][0]); check(models[2], cases[2], first=first[2][0])
     for m in (models[0], models[2], models[3], m5):
         m.close()
+
+
+@pytest.mark.parametrize("shape", [(23, 2, 21), (21, 2, 31), (13, 4, 41), (37, 2, 11)])
+def test_tap_stationary_kernels_when_uniform_taps_are_off(shape, monkeypatch):
+    """Single-system configurations with U = 11 or 16 run the uniform-tap step D by default, so the tap-stationary TMA
+    kernels of those tap counts are reached only by configurations with several systems or without a free slot.  Here
+    they are selected explicitly (GL_CONV_CT=0 is read when the configuration is created): strict bar against the oracle,
+    one launch fewer per call than the uniform-tap path, and agreement with that path inside the bar."""
+    import oracle
+    import torch
+    gl = _gl()
+    n_pix, s, K = shape
+    sp, obs, sigma, psf, z = _small_case(n_pix, s, K, 1, 0, -1, 1, seed=31 * n_pix + K, n_particles=5)
+    ref = oracle.logpost_grad(sp, obs, sigma, psf, z.astype(np.float64), None)
+    zt = torch.from_numpy(z).cuda()
+    m_ct = gl.LensModel(sp, obs, sigma, psf)
+    lp_ct, g_ct = m_ct.logpost_grad(zt)
+    n_ct = gl.gl_last_launch_count()
+    monkeypatch.setenv("GL_CONV_CT", "0")
+    m_ts = gl.LensModel(sp, obs, sigma, psf)
+    monkeypatch.delenv("GL_CONV_CT")
+    lp_ts, g_ts = m_ts.logpost_grad(zt)
+    n_ts = gl.gl_last_launch_count()
+    torch.cuda.synchronize()
+    U = (K + s - 1 + s - 1) // s
+    if U in (11, 16):
+        assert n_ct == n_ts + 1, (n_ct, n_ts)                      # the tap staging kernel of the uniform-tap path
+    fin = np.isfinite(ref["logp"])
+    assert fin.sum() >= 3
+    for lp, g in ((lp_ts, g_ts), (lp_ct, g_ct)):
+        a, b = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
+        assert np.array_equal(fin, np.isfinite(a))
+        assert np.all(np.abs(a[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
+        ok, rep = grad_report(b[fin], ref["grad"][fin])
+        assert rep["n_fail"] == 0, rep
+    m_ct.close(); m_ts.close()
