@@ -603,7 +603,8 @@ def test_tap_stationary_kernels_when_uniform_taps_are_off(shape, monkeypatch):
     """Single-system configurations with U = 11 or 16 run the uniform-tap step D by default, so the tap-stationary TMA
     kernels of those tap counts are reached only by configurations with several systems or without a free slot.  Here
     they are selected explicitly (GL_CONV_CT=0 is read when the configuration is created): strict bar against the oracle,
-    one launch fewer per call than the uniform-tap path, and agreement with that path inside the bar."""
+    one launch fewer per call than the uniform-tap path; round 1's sliding kernels (GL_CONV_TS=0 as well), kept for A/B runs, are
+    held to the same bar."""
     import oracle
     import torch
     gl = _gl()
@@ -619,16 +620,20 @@ def test_tap_stationary_kernels_when_uniform_taps_are_off(shape, monkeypatch):
     monkeypatch.delenv("GL_CONV_CT")
     lp_ts, g_ts = m_ts.logpost_grad(zt)
     n_ts = gl.gl_last_launch_count()
+    monkeypatch.setenv("GL_CONV_CT", "0"); monkeypatch.setenv("GL_CONV_TS", "0")     # round 1's sliding kernels (A/B fallback)
+    m_is = gl.LensModel(sp, obs, sigma, psf)
+    monkeypatch.delenv("GL_CONV_CT"); monkeypatch.delenv("GL_CONV_TS")
+    lp_is, g_is = m_is.logpost_grad(zt)
     torch.cuda.synchronize()
     U = (K + s - 1 + s - 1) // s
     if U in (11, 16):
         assert n_ct == n_ts + 1, (n_ct, n_ts)                      # the tap staging kernel of the uniform-tap path
     fin = np.isfinite(ref["logp"])
     assert fin.sum() >= 3
-    for lp, g in ((lp_ts, g_ts), (lp_ct, g_ct)):
+    for lp, g in ((lp_ts, g_ts), (lp_ct, g_ct), (lp_is, g_is)):
         a, b = lp.cpu().numpy().astype(np.float64), g.cpu().numpy().astype(np.float64)
         assert np.array_equal(fin, np.isfinite(a))
         assert np.all(np.abs(a[fin] - ref["logp"][fin]) <= RTOL_LOGP * np.abs(ref["logp"][fin]))
         ok, rep = grad_report(b[fin], ref["grad"][fin])
         assert rep["n_fail"] == 0, rep
-    m_ct.close(); m_ts.close()
+    m_ct.close(); m_ts.close(); m_is.close()
