@@ -103,6 +103,60 @@ def svi_loss_and_grad(mu, L_packed, xi, logp, grad_logp, active=None):
     return loss, g_mu, tril_pack(g_L), N
 
 
+# Score-function estimator: Eq. 3 AS PRINTED,
+#   grad_phi ELBO = E_q[ (log q~(z) - log p~(z)) grad_phi log q~(z; phi) ],            phi = (mu~, L),  z held fixed,
+# which needs log p~ only (no gradient of the model).  For the normal surrogate, with xi = L^-1 (z - mu) and s = L^-T xi:
+#   log q~(z)       = -1/2 |xi|^2 - sum_j log L_jj - (n/2) log 2 pi
+#   d log q~/d mu_j = s_j                      d log q~/d L_jk = s_j xi_k - delta_jk / L_jj         (k <= j)
+# Sampled with N draws:  g^_phi = (1/N) sum_i c_i grad_phi log q~(z_i),  c_i = w_i - b_i,  w_i = log q~(z_i) - log p~(z_i).
+# Reading: b_i = 0 is the estimator as printed; `baseline=True` takes the leave-one-out mean
+# b_i = mean_{k != i} w_k, i.e. c_i = N/(N-1) (w_i - mean w) -- still unbiased (b_i is independent of draw i and
+# E grad log q~ = 0) and the standard way to make the estimator usable (the paper prints no variance reduction).
+# The loss reported is the same closed-entropy estimate as above.  Draws with a non-finite log p~ are left out.
+
+def svi_score_terms(mu, L_packed, xi):
+    """(log q~(z_i) [N], s_i = L^-T xi_i [N][n]) for the draws z_i = mu + L xi_i."""
+    n = np.asarray(mu).size
+    L = tril_unpack(n, L_packed)
+    xi = np.asarray(xi, np.float64)
+    logq = -0.5 * np.sum(xi * xi, axis=1) - np.sum(np.log(np.abs(np.diag(L)))) - 0.5 * n * np.log(2.0 * np.pi)
+    s = np.linalg.solve(L.T, xi.T).T
+    return logq, s
+
+
+def svi_loss_and_grad_score(mu, L_packed, xi, logp, baseline=True):
+    """Sampled ELBO loss (closed-form entropy) and the score-function estimate of its gradient w.r.t. (mu, packed L)
+    from per-draw log p~ [N] alone.  Returns (loss, g_mu, g_L_packed, N_finite)."""
+    n = np.asarray(mu).size
+    L = tril_unpack(n, L_packed)
+    xi = np.asarray(xi, np.float64); lp = np.asarray(logp, np.float64)
+    ok = np.isfinite(lp)
+    N = int(ok.sum())
+    logq, s = svi_score_terms(mu, L_packed, xi)
+    w = logq[ok] - lp[ok]
+    c = (w - w.mean()) * (N / (N - 1.0)) if baseline else w
+    d = np.diag(L)
+    loss = -np.sum(np.log(np.abs(d))) - 0.5 * n * np.log(2.0 * np.pi * np.e) - lp[ok].sum() / N
+    g_mu = (c[:, None] * s[ok]).sum(axis=0) / N
+    g_L = (s[ok] * c[:, None]).T @ xi[ok] / N - np.diag(c.sum() / N / d)
+    return loss, g_mu, tril_pack(np.tril(g_L)), N
+
+
+def svi_step_score(logp_fn, mu, L_packed, xi, m, v, t, opt, baseline=True):
+    """One SVI iteration with the score-function gradient.  logp_fn(z [N][n]) -> logp [N].
+    Returns (loss, mu_new, L_new, m_new, v_new, logp)."""
+    n = np.asarray(mu).size
+    z = svi_draw(mu, L_packed, xi)
+    lp = logp_fn(z)
+    loss, g_mu, g_L, N = svi_loss_and_grad_score(mu, L_packed, xi, lp, baseline)
+    theta = np.concatenate([np.asarray(mu, np.float64), np.asarray(L_packed, np.float64)])[None, :]
+    grad_loss = np.concatenate([g_mu, g_L])[None, :]
+    m0 = np.asarray(m, np.float64)[None, :]; v0 = np.asarray(v, np.float64)[None, :]
+    th1, m1, v1 = update(opt["kind"], theta, -grad_loss, np.zeros(1), m0, v0, t, opt["lr"], opt["b1"], opt["b2"],
+                         opt["eps"], opt.get("eps_root", 0.0))
+    return loss, th1[0, :n], th1[0, n:], m1[0], v1[0], lp
+
+
 def svi_step(logp_grad_fn, mu, L_packed, xi, m, v, t, opt, active=None):
     """One SVI iteration.  logp_grad_fn(z [N][n]) -> (logp [N], grad [N][n]).  State m, v over the concatenated
     parameter vector [mu; packed L].  Entries of inactive dimensions (see svi_loss_and_grad) keep their value and

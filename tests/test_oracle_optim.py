@@ -275,3 +275,107 @@ def test_hmc_rejects_non_finite_proposals():
     xi = np.array([[3.0, 0.0], [0.1, 0.1]])
     z1, lp1, g1, acc, dH = optim.hmc_transition(f, z, lp, g, optim.tril_pack(np.eye(2)), xi, np.log([0.999, 1e-9]), 0.2, 3)
     assert not acc[0] and np.array_equal(z1[0], z[0]) and acc[1]
+
+
+# ------------------------------------------------------------------------------------------------ score-function SVI (Eq. 3)
+def test_svi_score_terms_are_log_q_and_its_derivatives():
+    """log q~ against scipy's multivariate-normal log-density with covariance L L^T, and d log q~/d(mu, L) at FIXED z against
+    central differences of that independent routine (this fixes which of L^-1, L^-T acts where, and the diagonal term)."""
+    from scipy.stats import multivariate_normal
+    mu, Lp, xi, _, _, _ = _svi_setup(n=4, N=5, seed=21)
+    n = mu.size
+    z = optim.svi_draw(mu, Lp, xi)
+    logq, s = optim.svi_score_terms(mu, Lp, xi)
+
+    def lq(mu_, Lp_):
+        L_ = optim.tril_unpack(n, Lp_)
+        return multivariate_normal(mean=mu_, cov=L_ @ L_.T).logpdf(z)
+
+    assert np.allclose(logq, lq(mu, Lp), rtol=1e-12, atol=1e-12)
+    h = 1e-6
+    for j in range(n):
+        e = np.zeros(n); e[j] = h
+        assert np.allclose((lq(mu + e, Lp) - lq(mu - e, Lp)) / (2 * h), s[:, j], rtol=1e-6, atol=1e-7)
+    L = optim.tril_unpack(n, Lp)
+    rows, cols = np.tril_indices(n)
+    for t, (j, k) in enumerate(zip(rows, cols)):
+        e = np.zeros_like(Lp); e[t] = h
+        want = s[:, j] * xi[:, k] - (1.0 / L[j, j] if j == k else 0.0)
+        assert np.allclose((lq(mu, Lp + e) - lq(mu, Lp - e)) / (2 * h), want, rtol=1e-6, atol=1e-7)
+
+
+@pytest.mark.parametrize("baseline", [True, False])
+def test_svi_score_estimator_is_unbiased(baseline):
+    """Gaussian target N(a, A^-1): the exact gradient of the loss is d/dmu = A (mu - a), d/dL = tril(A L) - diag(1/L_jj).
+    Twenty independent estimates of 20,000 draws each scatter around it: their mean lies within 5 standard errors in
+    every entry, with the leave-one-out baseline and (at a much larger scatter) as Eq. 3 prints it."""
+    mu, Lp, _, _, a, A = _svi_setup(n=3, seed=5)
+    n = mu.size
+    L = optim.tril_unpack(n, Lp)
+    exact = np.concatenate([A @ (mu - a), optim.tril_pack(np.tril(A @ L) - np.diag(1.0 / np.diag(L)))])
+    rng = np.random.default_rng(77)
+    est = []
+    for _ in range(20):
+        xi = rng.standard_normal((20000, n))
+        d = optim.svi_draw(mu, Lp, xi) - a
+        lp = -0.5 * np.einsum("ij,jk,ik->i", d, A, d) + 3.7             # an additive constant must not matter on average
+        _, g_mu, g_L, N = optim.svi_loss_and_grad_score(mu, Lp, xi, lp, baseline)
+        assert N == 20000
+        est.append(np.concatenate([g_mu, g_L]))
+    est = np.array(est)
+    se = est.std(axis=0, ddof=1) / np.sqrt(est.shape[0])
+    assert np.all(np.abs(est.mean(axis=0) - exact) < 5 * se + 1e-12), (est.mean(axis=0) - exact) / se
+    if baseline:
+        assert np.all(se < 0.05 * (1 + np.abs(exact)))                  # and it is tight enough to mean something
+
+
+def test_svi_score_agrees_with_the_pathwise_estimator():
+    """Both estimators estimate the same gradient: on the non-Gaussian toy target their averages over many draws agree
+    within the score estimator's standard error."""
+    mu, Lp, _, f, _, _ = _svi_setup(n=3, seed=9)
+    rng = np.random.default_rng(4)
+    sc, pw = [], []
+    for _ in range(20):
+        xi = rng.standard_normal((20000, mu.size))
+        lp, g = f(optim.svi_draw(mu, Lp, xi))
+        _, a1, b1, _ = optim.svi_loss_and_grad_score(mu, Lp, xi, lp, True)
+        _, a2, b2, _ = optim.svi_loss_and_grad(mu, Lp, xi, lp, g)
+        sc.append(np.concatenate([a1, b1])); pw.append(np.concatenate([a2, b2]))
+    sc, pw = np.array(sc), np.array(pw)
+    se = np.sqrt(sc.var(axis=0, ddof=1) + pw.var(axis=0, ddof=1)) / np.sqrt(sc.shape[0])
+    assert np.all(np.abs(sc.mean(axis=0) - pw.mean(axis=0)) < 5 * se)
+
+
+def test_svi_score_constant_weight_and_non_finite_draws():
+    """w_i constant (log p~ = log q~ - const): the baseline form returns exactly zero, the printed form const * mean of
+    grad log q~ (which is O(1/sqrt N)); draws with a non-finite log p~ are left out."""
+    mu, Lp, xi, f, _, _ = _svi_setup(n=4, N=4000, seed=12)
+    logq, s = optim.svi_score_terms(mu, Lp, xi)
+    _, g_mu, g_L, _ = optim.svi_loss_and_grad_score(mu, Lp, xi, logq - 2.5, True)
+    assert np.max(np.abs(g_mu)) < 1e-12 and np.max(np.abs(g_L)) < 1e-12
+    _, g_mu, g_L, _ = optim.svi_loss_and_grad_score(mu, Lp, xi, logq - 2.5, False)
+    assert np.allclose(g_mu, 2.5 * s.mean(axis=0)) and np.max(np.abs(g_mu)) < 2.5 * 5 / np.sqrt(4000) * np.abs(s).max()
+    lp, _ = f(optim.svi_draw(mu, Lp, xi))
+    lp2 = lp.copy(); lp2[7] = -np.inf
+    r1 = optim.svi_loss_and_grad_score(mu, Lp, np.delete(xi, 7, 0), np.delete(lp, 7), True)
+    r2 = optim.svi_loss_and_grad_score(mu, Lp, xi, lp2, True)
+    assert r1[3] == r2[3] == 3999 and np.isclose(r1[0], r2[0]) and np.allclose(r1[1], r2[1]) and np.allclose(r1[2], r2[2])
+
+
+def test_svi_score_fits_a_gaussian_target():
+    """The score-function iteration (log p~ only) recovers mean and covariance of a Gaussian target."""
+    rng = np.random.default_rng(1)
+    n = 2
+    A = np.array([[2.0, 0.4], [0.4, 1.0]]); a = np.array([0.5, -1.0])
+
+    def logp(z):
+        d = z - a
+        return -0.5 * np.einsum("ij,jk,ik->i", d, A, d)
+
+    mu = np.zeros(n); Lp = optim.tril_pack(np.eye(n)); m = np.zeros(n + 3); v = np.zeros(n + 3)
+    opt = dict(kind=optim.ADAM, lr=2e-2, b1=0.9, b2=0.999, eps=1e-8)
+    for t in range(1, 1201):
+        _, mu, Lp, m, v, _ = optim.svi_step_score(logp, mu, Lp, rng.standard_normal((512, n)), m, v, t, opt, True)
+    L = optim.tril_unpack(n, Lp)
+    assert np.allclose(mu, a, atol=0.08)
+    assert np.allclose(L @ L.T, np.linalg.inv(A), atol=0.12)
