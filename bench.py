@@ -60,9 +60,11 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
                     help="arithmetic of the CUDA path: f64 = GL_PRECISION_F64 (default; strict parity), f32 = GL_PRECISION_F32")
-    ap.add_argument("--stage", default="grad", choices=["grad", "map", "svi", "hmc"],
+    ap.add_argument("--stage", default="grad", choices=["grad", "map", "svi", "svi_score", "hmc"],
                     help="grad: one gl_logpost_grad call per step (the headline); map / svi / hmc: one fused gl_map_step (Adam), "
-                         "gl_svi_step (AdaBelief) or gl_hmc_step (4 leapfrog steps) per step")
+                         "gl_svi_step (AdaBelief) or gl_hmc_step (4 leapfrog steps) per step; svi_score: gl_svi_step_score, the "
+                         "score-function iteration of the paper's Eq. 3 (forward pass only; the metric then counts log-posterior "
+                         "evaluations WITHOUT gradient)")
     ap.add_argument("--amplitudes", default="sampled", choices=["sampled", "solved"],
                     help="solved: backward modelling (amplitude_mode 1, DESIGN.md section 16); a diagnostic line, no cpu_baseline")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the cpu_baseline sample")
@@ -267,7 +269,7 @@ def stage_profile(gl, step, flush, reps):
 
 
 def roofline_record(workmodel, sp, k, precision, P, evals_per_particle, stage_ms, stage_n, ms_per_step, bands, mhz_max,
-                    peak_src, sm_mhz=None, evals_in_stage_times=None):
+                    peak_src, sm_mhz=None, evals_in_stage_times=None, forward_only=False):
     """The `roofline` object of the contract for the dominant kernel of a measured step.
     frac          executed-band work: only the series steps that run in the arithmetic type are credited (bands)
     frac_fixed30  the fixed 30-term formulation (every term credited to the arithmetic type's pipe): the round-1 figure
@@ -277,6 +279,8 @@ def roofline_record(workmodel, sp, k, precision, P, evals_per_particle, stage_ms
     pipe = "FP64" if precision == "f64" else "FP32"
     wm30 = workmodel.per_eval(sp, precision)
     wmb = workmodel.per_eval(sp, precision, bands[:2]) if bands else wm30
+    if forward_only:                     # a step that runs steps A-E only (gl_logpost): credit one forward sweep
+        wm30 = dict(wm30, total_fwd_grad=wm30["total_fwd"]); wmb = dict(wmb, total_fwd_grad=wmb["total_fwd"])
     dom = max(stage_ms, key=stage_ms.get)
     dom_t = stage_ms[dom] * 1e-3
     # the stage timer holds the LAST gl_logpost_grad of a step (an HMC transition makes several: one of them is timed)
@@ -413,7 +417,7 @@ def run_ours(a):
 
         def step_host():
             step(); lph.copy_(lp, non_blocking=True)
-    elif a.stage == "svi":                                   # NEXT-2: P draws of one surrogate; xi in, loss out
+    elif a.stage in ("svi", "svi_score"):                    # NEXT-2: P draws of one surrogate; xi in, loss out
         if sp.n_systems != 1:
             raise SystemExit("--stage svi needs a single-system config")
         nt = n_p * (n_p + 1) // 2
@@ -429,15 +433,21 @@ def run_ours(a):
 
         extra_launches = 1
 
+        def svi_call(t):
+            if a.stage == "svi":
+                gl.gl_svi_step(m.h, belief, m.obs, m.noise_sigma, m.psf, mu, lt, xi, sid, sm, sv, t, stats, ws)
+            else:                                            # Eq. 3 as printed + leave-one-out baseline: gl_logpost only
+                gl.gl_svi_step_score(m.h, belief, m.obs, m.noise_sigma, m.psf, mu, lt, xi, sid, sm, sv, t, 1, stats, ws)
+
         def step():                                          # fresh draws on the device every iteration (reading S22)
             tstep[0] += 1
             gl.gl_draw_normal(2026, tstep[0], 0, xi)
-            gl.gl_svi_step(m.h, belief, m.obs, m.noise_sigma, m.psf, mu, lt, xi, sid, sm, sv, tstep[0], stats, ws)
+            svi_call(tstep[0])
 
         def step_host():                                     # host-made draws through a pinned buffer
             tstep[0] += 1
             xi.copy_(xih, non_blocking=True)
-            gl.gl_svi_step(m.h, belief, m.obs, m.noise_sigma, m.psf, mu, lt, xi, sid, sm, sv, tstep[0], stats, ws)
+            svi_call(tstep[0])
             statsh.copy_(stats, non_blocking=True)
     else:                                                    # NEXT-3: P chains, one transition of 4 leapfrog steps
         n_leap = 4
@@ -526,7 +536,8 @@ def run_ours(a):
     mhz_max, peak_src = _peaks()
     clocks = sampler.summary()
     roof = roofline_record(workmodel, sp, k, a.precision, P, evals_per_particle, stage_ms, stage_n, t_dev / a.steps * 1e3, bands,
-                           mhz_max, peak_src, clocks.get("sm_mhz"), evals_in_stage_times=1 if a.stage == "hmc" else None)
+                           mhz_max, peak_src, clocks.get("sm_mhz"), evals_in_stage_times=1 if a.stage == "hmc" else None,
+                           forward_only=a.stage == "svi_score")
     probe = {}
     for kind, name in ((0, "fp32_fma"), (1, "fp64_fma"), (2, "mufu_ex2"), (4, "fp64_fma_distinct_operands"),
                        (5, "fp64_mma_m8n8k4"), (6, "fp64_mma_plus_fma"),

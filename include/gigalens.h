@@ -265,6 +265,21 @@ gl_status gl_svi_step(const gl_config* cfg, const gl_opt_desc* opt, const float*
                       int64_t n_draws, float* opt_m, float* opt_v, int64_t step, float* out_stats,
                       void* workspace, size_t workspace_bytes, void* stream /* cudaStream_t */);
 
+/* The same iteration with the SCORE-FUNCTION gradient, Eq. 3 as the paper prints it:
+ *   grad_phi ELBO = E_q[(log q~(z) - log p~(z)) grad_phi log q~(z; phi)],  phi = (mu~, L), z held fixed,
+ * sampled as (1/N) sum_i c_i grad_phi log q~(z_i) with log q~(z_i) = -|xi_i|^2/2 - sum_j log L_jj - (n/2) log 2 pi,
+ * d log q~/d mu_j = s_j, d log q~/d L_jk = s_j xi_k - delta_jk / L_jj, s = L^-T xi.  It needs log p~ only: the hot path
+ * runs FORWARD ONLY on the draws (gl_logpost: about three times the rate of the gradient call).
+ *   baseline  0: c_i = w_i = log q~(z_i) - log p~(z_i), the estimator as printed;  1: c_i = N/(N-1) (w_i - mean w), the
+ *             leave-one-out control variate (still unbiased) -- the usable form at n_VI ~ 10^3
+ * Other arguments, the loss estimate in out_stats, the treatment of non-finite draws and the workspace as gl_svi_step.
+ * Errors as gl_svi_step, plus GL_ERR_UNSUPPORTED with amplitude_mode 1 (use gl_svi_step) and GL_ERR_BAD_CONFIG for a
+ * baseline other than 0 or 1. */
+gl_status gl_svi_step_score(const gl_config* cfg, const gl_opt_desc* opt, const float* obs, const float* noise_sigma,
+                            const float* psf, float* mu, float* l_tril, const float* xi, const int32_t* system_id,
+                            int64_t n_draws, float* opt_m, float* opt_v, int64_t step, int32_t baseline, float* out_stats,
+                            void* workspace, size_t workspace_bytes, void* stream /* cudaStream_t */);
+
 /* ---- one HMC transition of n independent chains on the device -------------------------------
  * Standard leapfrog HMC (mass matrix from the surrogate covariance) in the whitened momentum
  * xi = L^T p, Sigma = L L^T = M^-1:  H = -log p~(z) + |xi|^2/2;  per leapfrog step

@@ -24,7 +24,7 @@ EXPORTS = ["gl_config_create", "gl_config_destroy", "gl_config_n_params", "gl_wo
            "gl_stage_name", "gl_stage_times", "gl_probe_pipe", "gl_map_step",
            "gl_svi_workspace_bytes", "gl_svi_step", "gl_hmc_workspace_bytes", "gl_hmc_step",
            "gl_best_particle", "gl_config_n_amplitudes", "gl_linear_amplitudes", "gl_draw_normal", "gl_draw_log_uniform",
-           "gl_config_shape", "gl_workspace_layout", "gl_logpost_grad_noalloc"]
+           "gl_config_shape", "gl_workspace_layout", "gl_logpost_grad_noalloc", "gl_svi_step_score"]
 GL_NOALLOC_MAX_BYTES = 32 << 20      # include/gigalens.h
 
 
@@ -102,6 +102,8 @@ def lib():
         L.gl_svi_workspace_bytes.argtypes = [vp, i64]
         L.gl_svi_step.restype = C.c_int
         L.gl_svi_step.argtypes = [vp, C.POINTER(gl_opt_desc), vp, vp, vp, vp, vp, vp, vp, i64, vp, vp, i64, vp, vp, sz, vp]
+        L.gl_svi_step_score.restype = C.c_int
+        L.gl_svi_step_score.argtypes = [vp, C.POINTER(gl_opt_desc), vp, vp, vp, vp, vp, vp, vp, i64, vp, vp, i64, C.c_int32, vp, vp, sz, vp]
         L.gl_draw_normal.restype = C.c_int
         L.gl_draw_normal.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, i64, C.c_int32, vp, vp]
         L.gl_draw_log_uniform.restype = C.c_int
@@ -406,6 +408,23 @@ def gl_svi_step(h, opt, obs, noise_sigma, psf, mu, l_tril, xi, system_id, opt_m,
                              workspace.numel() * workspace.element_size(), _stream(stream)), "gl_svi_step")
 
 
+def gl_svi_step_score(h, opt, obs, noise_sigma, psf, mu, l_tril, xi, system_id, opt_m, opt_v, step, baseline, out_stats,
+                      workspace, stream=None):
+    """One SVI iteration with the score-function gradient (Eq. 3 of the paper as printed; log p~ only, forward pass only);
+    baseline 0 / 1: as printed / leave-one-out control variate.  Arguments otherwise as gl_svi_step."""
+    torch = _torch()
+    f32 = torch.float32
+    opt = _opt_desc(opt)
+    _extents(h, xi.shape[0], obs=obs, noise_sigma=noise_sigma, psf=psf, mu=mu, l_tril=l_tril, xi=xi, system_id=system_id, svi_m=opt_m,
+             svi_v=opt_v, out_stats=out_stats)
+    _check(lib().gl_svi_step_score(h, C.byref(opt), _ptr(_dev(obs, f32, "obs")), _ptr(_dev(noise_sigma, f32, "noise_sigma")),
+                                   _ptr(_dev(psf, f32, "psf")), _ptr(_dev(mu, f32, "mu")), _ptr(_dev(l_tril, f32, "l_tril")),
+                                   _ptr(_dev(xi, f32, "xi")), _ptr(_dev(system_id, torch.int32, "system_id")), xi.shape[0],
+                                   _ptr(_dev(opt_m, f32, "opt_m")), _ptr(_dev(opt_v, f32, "opt_v")), int(step), int(baseline),
+                                   _ptr(_dev(out_stats, f32, "out_stats")), _ptr(workspace),
+                                   workspace.numel() * workspace.element_size(), _stream(stream)), "gl_svi_step_score")
+
+
 def gl_model_image(h, psf, params, system_id, out_image, workspace, stream=None):
     torch = _torch()
     f32 = torch.float32
@@ -538,10 +557,11 @@ class LensModel:
             gl_map_step(self.h, opt, self.obs, self.noise_sigma, self.psf, params, sid, m, v, t, lp, g, ws, stream)
         return lp, (m, v)
 
-    def svi_run(self, mu, l_tril, opt, n_steps, n_draws, seed, first_step=1, state=None, stream=None):
+    def svi_run(self, mu, l_tril, opt, n_steps, n_draws, seed, first_step=1, state=None, stream=None, estimator="pathwise"):
         """n_steps SVI iterations (gl_svi_step) on (mu, l_tril) IN PLACE with the draws made on the device
         (gl_draw_normal, stream_id 0, step = the iteration number): nothing crosses the host between iterations.
-        Returns (stats [n_steps][2] = (loss, finite draws) per iteration, (m, v) optimiser state)."""
+        estimator: "pathwise" (gl_svi_step), "score" (gl_svi_step_score with the leave-one-out baseline) or "score_printed"
+        (Eq. 3 as printed, no baseline).  Returns (stats [n_steps][2] = (loss, finite draws) per iteration, (m, v) optimiser state)."""
         torch = _torch()
         n = self.n_params
         nt = n * (n + 1) // 2
@@ -553,7 +573,11 @@ class LensModel:
         ws = torch.empty(max(need, 256), dtype=torch.uint8, device=self.device)
         for k, t in enumerate(range(first_step, first_step + n_steps)):
             gl_draw_normal(seed, t, 0, xi, stream)
-            gl_svi_step(self.h, opt, self.obs, self.noise_sigma, self.psf, mu, l_tril, xi, None, m, v, t, stats[k], ws, stream)
+            if estimator == "pathwise":
+                gl_svi_step(self.h, opt, self.obs, self.noise_sigma, self.psf, mu, l_tril, xi, None, m, v, t, stats[k], ws, stream)
+            else:
+                gl_svi_step_score(self.h, opt, self.obs, self.noise_sigma, self.psf, mu, l_tril, xi, None, m, v, t,
+                                  0 if estimator == "score_printed" else 1, stats[k], ws, stream)
         return stats, (m, v)
 
     def hmc_run(self, z, l_tril, step_size, n_leapfrog, n_transitions, seed, first_step=1, system_id=None, stream=None):

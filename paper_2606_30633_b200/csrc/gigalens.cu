@@ -776,6 +776,48 @@ extern "C" gl_status gl_svi_step(const gl_config* cfg, const gl_opt_desc* opt, c
     return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
 }
 
+// Score-function SVI iteration (Eq. 3 as printed): the hot path runs FORWARD ONLY (gl_logpost) on the draws; the gradient of the
+// loss w.r.t. (mu, L) comes from log p~ and the surrogate's own score (gl_svi.cuh).  Same workspace as gl_svi_step: the draws'
+// buffer holds c_i and three scalars once the hot path has consumed z, the gradient buffer holds the pseudo-gradient rows.
+extern "C" gl_status gl_svi_step_score(const gl_config* cfg, const gl_opt_desc* opt, const float* obs, const float* noise_sigma,
+                                       const float* psf, float* mu, float* l_tril, const float* xi, const int32_t* system_id,
+                                       int64_t n, float* opt_m, float* opt_v, int64_t step, int32_t baseline, float* out_stats,
+                                       void* workspace, size_t workspace_bytes, void* stream) {
+    t_launches = 0;
+    if (!cfg) return GL_ERR_NULL;
+    gl_status s = check_opt(opt, step);
+    if (s != GL_OK) return s;
+    if (baseline != 0 && baseline != 1) return GL_ERR_BAD_CONFIG;
+    if (cfg->desc.amplitude_mode == 1) return GL_ERR_UNSUPPORTED;          // surrogate on a subset of the dimensions: pathwise only
+    if (n < 0) return GL_ERR_BAD_SHAPE;
+    if (n == 0) return GL_OK;
+    if (!mu || !l_tril || !xi || !opt_m || !opt_v || !out_stats || !workspace) return GL_ERR_NULL;
+    const SviPlan pl = svi_plan(cfg, n);
+    if (workspace_bytes < pl.total || ((uintptr_t)workspace & 255) != 0) return GL_ERR_WORKSPACE;
+    const int np = cfg->L.n_params, nslot = 2 + np + np * (np + 1) / 2;
+    if ((size_t)n * np * sizeof(float) < ((size_t)n + 4) * sizeof(double)) return GL_ERR_UNSUPPORTED;   // n_params < 3
+    cudaStream_t st = (cudaStream_t)stream;
+    char* w = (char*)workspace;
+    float* z = (float*)(w + pl.off_z); float* lp = (float*)(w + pl.off_lp); float* g = (float*)(w + pl.off_g);
+    double* part = (double*)(w + pl.off_part);
+    s = validate(cfg, 0, obs, noise_sigma, psf, z, n, lp, nullptr, nullptr, workspace, pl.core);     // before the first launch
+    if (s != GL_OK) return s;
+    clear_stale_error();
+    gl_svi_draw_kernel<<<(unsigned)((n * np + 255) / 256), 256, 0, st>>>(n, np, mu, l_tril, xi, z);
+    s = run(cfg, 0, obs, noise_sigma, psf, z, system_id, n, lp, nullptr, nullptr, workspace, pl.core, st);
+    if (s != GL_OK) return s;
+    const int64_t launches = t_launches + 1;
+    double* c = (double*)z;                       // z has been consumed: c_i [n], then scal[3]
+    double* scal = c + n;
+    gl_svi_score_w_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(n, np, lp, xi, l_tril, c);
+    gl_svi_score_c_kernel<<<1, 256, 0, st>>>(n, baseline, c, scal);
+    gl_svi_score_grad_kernel<<<(unsigned)((n + 63) / 64), 64, 0, st>>>(n, np, l_tril, xi, c, g);
+    gl_svi_reduce_kernel<<<dim3((nslot + 127) / 128, SVI_NCHUNK), 128, 0, st>>>(n, np, lp, g, xi, part);
+    gl_svi_update_kernel<<<1, 256, 0, st>>>(opt_params(opt, step), dead_mask(cfg), np, part, mu, l_tril, opt_m, opt_v, out_stats, scal);
+    t_launches = launches + 5;
+    return cudaPeekAtLastError() == cudaSuccess ? GL_OK : GL_ERR_CUDA;
+}
+
 struct HmcPlan { size_t core, off_zd, off_xd, off_zf, off_g, off_lp, total; };
 static HmcPlan hmc_plan(const gl_config* c, int64_t n) {
     HmcPlan p{};

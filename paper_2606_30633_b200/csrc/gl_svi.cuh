@@ -72,8 +72,12 @@ __device__ __forceinline__ double svi_total(const double* __restrict__ part, int
 __global__ void __launch_bounds__(256) gl_svi_update_kernel(const __grid_constant__ OptParams o, const __grid_constant__ DimMask dead, int np,
                                                             const double* __restrict__ part, float* __restrict__ mu,
                                                             float* __restrict__ Lp, float* __restrict__ m,
-                                                            float* __restrict__ v, float* __restrict__ out_stats) {
+                                                            float* __restrict__ v, float* __restrict__ out_stats,
+                                                            const double* __restrict__ diag_coef = nullptr) {
+    // diag_coef: coefficient of the -1 / L_jj term of d loss / d L_jj: 1 for the pathwise estimator (NULL), (1/N) sum_i c_i for
+    // the score-function estimator (gl_svi_score_* kernels below), read from device memory
     const int ntril = np * (np + 1) / 2, nslot = 2 + np + ntril;
+    const double dcoef = diag_coef ? diag_coef[0] : 1.0;
     __shared__ double s_logdiag;
     const double N = svi_total(part, nslot, 1);                  // every thread: same fixed-order sum, same value
     if (threadIdx.x == 0) {                                      // sum_j log |L_jj| from the OLD L, fixed order
@@ -93,7 +97,7 @@ __global__ void __launch_bounds__(256) gl_svi_update_kernel(const __grid_constan
         if (e >= np) {
             const int t = e - np, j = tril_row(t), k = t - j * (j + 1) / 2;
             if (dead.test(j) || dead.test(k)) continue;
-            if (k == j) g -= 1.0 / (double)*th;
+            if (k == j) g -= dcoef / (double)*th;
         } else if (dead.test(e)) continue;
         const double m1 = o.b1 * (double)m[e] + (1.0 - o.b1) * g;
         const double d = o.kind == 1 ? g - m1 : g;
@@ -101,6 +105,71 @@ __global__ void __launch_bounds__(256) gl_svi_update_kernel(const __grid_constan
         const double t1 = (double)*th - o.lr * (m1 * o.c1) / (sqrt(v1 * o.c2) + o.eps);
         m[e] = (float)m1; v[e] = (float)v1; *th = (float)t1;
     }
+}
+
+// ----------------------------------------------------------------------------- score-function estimator (Eq. 3 as printed)
+// grad_phi loss = (1/N) sum_i c_i grad_phi log q~(z_i), c_i = w_i - b_i, w_i = log q~(z_i) - log p~(z_i); needs log p~ only.
+//   log q~(z_i) = -1/2 |xi_i|^2 - sum_j log L_jj - (n/2) log 2 pi;  d log q~/d mu_j = s_j,  d log q~/d L_jk = s_j xi_k - delta_jk / L_jj,
+//   s = L^-T xi.  Readings: DESIGN.md section 12 (b_i = 0: as printed; leave-one-out mean: c_i = N/(N-1) (w_i - mean w)).
+// The kernels below turn that into the quantities the pathwise path already reduces: a "pseudo-gradient" row
+// G_i = -c_i s_i in place of grad log p~(z_i), so that gl_svi_reduce_kernel's sums of G_ij and G_ij xi_ik and
+// gl_svi_update_kernel (with diag_coef = (1/N) sum_i c_i) produce exactly the score-function gradient.
+
+// w_i for every draw (NaN marks a draw with a non-finite log p~).  One thread per draw.
+__global__ void gl_svi_score_w_kernel(int64_t n, int np, const float* __restrict__ logp, const float* __restrict__ xi,
+                                      const float* __restrict__ Lp, double* __restrict__ w) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float lp = logp[i];
+    if (!isfinite(lp)) { w[i] = nan(""); return; }
+    double q = 0.0, ld = 0.0;
+    for (int j = 0; j < np; ++j) {
+        const double x = (double)xi[i * np + j];
+        q = fma(x, x, q);
+        ld += log(fabs((double)Lp[(size_t)j * (j + 1) / 2 + j]));
+    }
+    w[i] = -0.5 * q - ld - 0.5 * np * 1.8378770664093453 - (double)lp;         // ln 2 pi
+}
+
+// fixed-order sum over a strided subset per thread, then a fixed tree; ONE block of 256 threads
+__device__ __forceinline__ double svi_block_sum(double v, double* sm) {
+    sm[threadIdx.x] = v;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) { if (threadIdx.x < o) sm[threadIdx.x] += sm[threadIdx.x + o]; __syncthreads(); }
+    const double r = sm[0];
+    __syncthreads();
+    return r;
+}
+// w (in place) -> c;  scal[0] = (1/N) sum_i c_i (the diagonal coefficient), scal[1] = N, scal[2] = mean w
+__global__ void __launch_bounds__(256) gl_svi_score_c_kernel(int64_t n, int baseline, double* __restrict__ w, double* __restrict__ scal) {
+    __shared__ double sm[256];
+    double sw = 0.0, cnt = 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += 256) { const double x = w[i]; if (x == x) { sw += x; cnt += 1.0; } }
+    const double N = svi_block_sum(cnt, sm), W = svi_block_sum(sw, sm);
+    const double wbar = N > 0 ? W / N : 0.0, f = (baseline && N > 1) ? N / (N - 1.0) : 1.0;
+    double sc = 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += 256) {
+        const double x = w[i];
+        const double c = (x == x) ? (baseline ? f * (x - wbar) : x) : 0.0;
+        w[i] = c; sc += c;
+    }
+    const double C = svi_block_sum(sc, sm);
+    if (threadIdx.x == 0) { scal[0] = N > 0 ? C / N : 0.0; scal[1] = N; scal[2] = wbar; }
+}
+
+// G_i = -c_i L^-T xi_i (back-substitution, fp64), stored as the fp32 "gradient" rows the reduction reads.  One thread per draw.
+__global__ void gl_svi_score_grad_kernel(int64_t n, int np, const float* __restrict__ Lp, const float* __restrict__ xi,
+                                         const double* __restrict__ c, float* __restrict__ g) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double s[128];
+    const double ci = c[i];
+    for (int j = np - 1; j >= 0; --j) {               // s_j = (xi_j - sum_{k > j} L_kj s_k) / L_jj
+        double a = (double)xi[i * np + j];
+        for (int k = j + 1; k < np; ++k) a = fma(-(double)Lp[(size_t)k * (k + 1) / 2 + j], s[k], a);
+        s[j] = a / (double)Lp[(size_t)j * (j + 1) / 2 + j];
+    }
+    for (int j = 0; j < np; ++j) g[i * np + j] = (float)(-ci * s[j]);
 }
 
 }  // namespace gl

@@ -201,3 +201,84 @@ def test_svi_backward_mode_surrogate_lives_on_the_sampled_dimensions():
         step = np.abs(th_o - th_p)
         assert np.all(np.abs(th_g - th_o)[live] <= 2e-3 * step[live] + 4e-7 * (np.abs(th_p) + step)[live] + 1e-30)
     assert np.isfinite(losses).all()
+
+
+# ------------------------------------------------------------------------------------------------ score-function estimator
+def _score_compare(gl, torch, m, spec, obs, sig, psf, mu, lt, xi, opt, baseline, n_finite, n_launch=None):
+    """Two iterations of gl_svi_step_score against oracle/optim.py::svi_step_score; the oracle's log p~ is rounded to fp32,
+    the storage in which the interface hands it from the hot path to the estimator."""
+    import oracle
+    from oracle import optim
+    n = spec.n_params; nt = n * (n + 1) // 2
+    opt_o = {k: (float(np.float32(x)) if k != "kind" else x) for k, x in opt.items()}
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    mu_g, lt_g, xi_g = d(mu), d(lt), d(xi)
+    mm, vv = torch.zeros(n + nt, device="cuda"), torch.zeros(n + nt, device="cuda")
+    stats = torch.zeros(2, device="cuda")
+    ws = torch.empty(gl.gl_svi_workspace_bytes(m.h, xi.shape[0]), dtype=torch.uint8, device="cuda")
+
+    def logp(z):
+        r = oracle.logpost_grad(spec, obs, sig, psf, z.astype(np.float32).astype(np.float64), None, want_grad=False)
+        return r["logp"].astype(np.float32).astype(np.float64)
+
+    for t in (1, 2):
+        prev = [x.cpu().numpy().astype(np.float64) for x in (mu_g, lt_g, mm, vv)]
+        loss_o, mu_o, lt_o, m_o, v_o, lp_o = optim.svi_step_score(logp, prev[0], prev[1], xi.astype(np.float64), prev[2], prev[3], t,
+                                                                  opt_o, bool(baseline))
+        gl.gl_svi_step_score(m.h, opt, m.obs, m.noise_sigma, m.psf, mu_g, lt_g, xi_g, None, mm, vv, t, baseline, stats, ws)
+        torch.cuda.synchronize()
+        assert int(stats[1]) == n_finite == int(np.isfinite(lp_o).sum())
+        assert abs(float(stats[0]) - loss_o) <= 1e-4 * abs(loss_o)
+        th_prev = np.concatenate(prev[:2]); th_o = np.concatenate([mu_o, lt_o])
+        th_g = np.concatenate([mu_g.cpu().numpy(), lt_g.cpu().numpy()]).astype(np.float64)
+        for got, want, old, c, name in ((th_g, th_o, th_prev, 1.0, "theta"), (mm.cpu().numpy().astype(np.float64), m_o, prev[2], opt_o["b1"], "m"),
+                                        (vv.cpu().numpy().astype(np.float64), v_o, prev[3], opt_o["b2"], "v")):
+            scale = np.abs(c * old) + np.abs(want - c * old)
+            bad = np.abs(got - want) > 2e-3 * np.abs(want - c * old) + 4e-7 * scale + 1e-30
+            assert not bad.any(), (name, t, int(bad.sum()), np.flatnonzero(bad)[:8])
+    if n_launch is not None:
+        assert gl.gl_last_launch_count() == n_launch
+
+
+@pytest.mark.parametrize("baseline", [1, 0], ids=["leave_one_out", "as_printed"])
+@pytest.mark.parametrize("opt", [ADABELIEF, ADAM], ids=["adabelief", "adam"])
+def test_svi_score_steps_match_oracle(opt, baseline):
+    """Eq. 3 of the paper as printed (score-function gradient, log p~ only): two consecutive iterations, 48 draws around the
+    seeded truth of config 1, one of them invalid; the hot path runs forward only (draw + 5 path kernels + 5 kernels of the
+    estimator, reduction and update)."""
+    gl, torch, wl, obs, sig, m, mu, lt, xi = _setup(1, 48, 13)
+    xi[9, 2] = 4.0e3                                                    # e1 far outside the unit disc: invalid draw
+    _score_compare(gl, torch, m, wl.spec, obs, sig, wl.psf, mu, lt, xi, opt, baseline, 47, n_launch=11)
+
+
+def test_svi_score_step_58_params_2048_draws():
+    """The same on the config-3 parameter layout with a dense L: 2048 draws x 58 parameters (back-substitution over 58 rows per
+    draw, the 32-chunk reduction of the pseudo-gradient and its products with xi), three draws thrown out of the domain."""
+    gl, torch, sp, obs, sig, psf, m, mu, lt, xi = _big_setup(2048, 307)
+    for r in (11, 900, 2040):
+        xi[r, 2] = 5.0e4
+    _score_compare(gl, torch, m, sp, obs, sig, psf, mu, lt, xi, ADABELIEF, 1, 2045)
+
+
+def test_svi_score_argument_checks_and_run_loop():
+    """baseline outside {0, 1}, backward modelling (surrogate on a subset of the dimensions: pathwise only), and
+    LensModel.svi_run with the score estimator: the loss estimate falls over 150 iterations of 1024 fresh draws."""
+    import dataclasses
+    gl, torch, wl, obs, sig, m, mu, lt, xi = _setup(1, 8, 2)
+    n = wl.spec.n_params; nt = n * (n + 1) // 2
+    d = lambda a: torch.from_numpy(a).cuda()
+    mm, vv, stats = torch.zeros(n + nt, device="cuda"), torch.zeros(n + nt, device="cuda"), torch.zeros(2, device="cuda")
+    ws = torch.empty(gl.gl_svi_workspace_bytes(m.h, 8), dtype=torch.uint8, device="cuda")
+    with pytest.raises(gl.GLError) as e:
+        gl.gl_svi_step_score(m.h, ADAM, m.obs, m.noise_sigma, m.psf, d(mu), d(lt), d(xi), None, mm, vv, 1, 2, stats, ws)
+    assert e.value.status == -2
+    mb = gl.LensModel(dataclasses.replace(wl.spec, amplitude_mode=1), obs, sig, wl.psf)
+    with pytest.raises(gl.GLError) as e:
+        gl.gl_svi_step_score(mb.h, ADAM, mb.obs, mb.noise_sigma, mb.psf, d(mu), d(lt), d(xi), None, mm, vv, 1, 1, stats, ws)
+    assert e.value.status == -4
+    rng = np.random.default_rng(23)
+    mu_g = torch.from_numpy((mu + 0.03 * rng.standard_normal(n)).astype(np.float32)).cuda(); lt_g = torch.from_numpy(lt).cuda()
+    st, _ = m.svi_run(mu_g, lt_g, dict(ADABELIEF, lr=1e-3), 150, 1024, seed=99, estimator="score")
+    st = st.cpu().numpy()
+    assert np.isfinite(st).all() and st[-10:, 0].mean() < st[:10, 0].mean(), (st[:3], st[-3:])
+    assert torch.all(torch.isfinite(mu_g)) and torch.all(torch.isfinite(lt_g))
