@@ -637,3 +637,47 @@ def test_tap_stationary_kernels_when_uniform_taps_are_off(shape, monkeypatch):
         ok, rep = grad_report(b[fin], ref["grad"][fin])
         assert rep["n_fail"] == 0, rep
     m_ct.close(); m_ts.close(); m_is.close()
+
+
+@pytest.mark.parametrize("case", [(26, 2, 21, 0, 0), (22, 2, 31, 0, 0), (13, 4, 41, 0, 0), (17, 4, 21, 0, 0), (19, 3, 7, 0, 0),
+                                  (24, 4, 21, 1, 0), (20, 2, 11, 1, 0), (22, 2, 21, 0, 1), (18, 4, 21, 1, 1)],
+                         ids=lambda c: "N%d_s%d_K%d_pg%d_amp%d" % c)
+def test_workspace_and_output_guards_stay_intact(case):
+    """compute-sanitizer is closed on this GPU pool, so overruns are looked for directly: the workspace handed to the
+    library is the middle of a larger buffer and the outputs sit between guard rows; after gl_logpost_grad, gl_logpost and
+    gl_model_image (every step-D kernel family is reached by one of the shapes: uniform-tap, tap-stationary, generic, the
+    binned psf_grid = 1 path, backward modelling) the guards still hold their pattern, with the workspace sized EXACTLY as
+    gl_workspace_bytes says."""
+    import dataclasses
+    import torch
+    gl = _gl()
+    n_pix, s, K, pgrid, amp = case
+    sp, obs, sigma, psf, z = _small_case(n_pix, s, K, 1, 0, -1, 1, seed=3 * n_pix + K + pgrid, n_particles=9, psf_grid=pgrid)
+    sp = dataclasses.replace(sp, amplitude_mode=amp)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    P, n = z.shape
+    need = gl.gl_workspace_bytes(m.h, P)
+    G = 1 << 20
+    big = torch.full((need + 2 * G,), 0xA5, dtype=torch.uint8, device="cuda")
+    assert big.data_ptr() % 256 == 0
+    ws = big[G:G + need]
+    zt = torch.from_numpy(z).cuda()
+    outs = torch.full((P * (1 + n + 1 + n_pix * n_pix) + 5 * 64,), -7.25, dtype=torch.float32, device="cuda")
+    o = 64
+    lp = outs[o:o + P]; o += P + 64
+    g = outs[o:o + P * n].view(P, n); o += P * n + 64
+    lp2 = outs[o:o + P]; o += P + 64
+    img = outs[o:o + P * n_pix * n_pix].view(P, n_pix, n_pix)
+    mask = torch.ones_like(outs, dtype=torch.bool)
+    for t in (lp, g, lp2, img):
+        a = (t.data_ptr() - outs.data_ptr()) // 4
+        mask[a:a + t.numel()] = False
+    for _ in range(2):
+        gl.gl_logpost_grad(m.h, m.obs, m.noise_sigma, m.psf, zt, None, lp, g, ws)
+        gl.gl_logpost(m.h, m.obs, m.noise_sigma, m.psf, zt, None, lp2, ws)
+        gl.gl_model_image(m.h, m.psf, zt, None, img, ws)
+    torch.cuda.synchronize()
+    assert bool((big[:G] == 0xA5).all()) and bool((big[G + need:] == 0xA5).all()), "write outside the workspace"
+    assert bool((outs[mask] == -7.25).all()), "write outside an output array"
+    assert torch.isfinite(lp).sum() >= 3 and torch.equal(lp, lp2)
+    m.close()
