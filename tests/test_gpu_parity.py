@@ -681,3 +681,58 @@ def test_workspace_and_output_guards_stay_intact(case):
     assert bool((outs[mask] == -7.25).all()), "write outside an output array"
     assert torch.isfinite(lp).sum() >= 3 and torch.equal(lp, lp2)
     m.close()
+
+
+def test_consumer_workspace_guards_stay_intact():
+    """The same overrun check for the fused consumers, each with its workspace sized exactly as its own *_workspace_bytes
+    function says, inside a patterned buffer: gl_map_step, gl_svi_step, gl_svi_step_score, gl_hmc_step (dense L) on an
+    EPL + shapelets case that runs the uniform-tap step D."""
+    import torch
+    gl = _gl()
+    sp, obs, sigma, psf, z, truth = _small_case(22, 2, 31, 1, 0, 3, 2, seed=77, n_particles=24, with_truth=True)
+    m = gl.LensModel(sp, obs, sigma, psf)
+    P, n = z.shape
+    nt = n * (n + 1) // 2
+    G = 1 << 20
+    rng = np.random.default_rng(3)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+    def guarded(need):
+        big = torch.full((need + 2 * G,), 0x5A, dtype=torch.uint8, device="cuda")
+        return big, big[G:G + need]
+
+    def intact(big, need):
+        return bool((big[:G] == 0x5A).all()) and bool((big[G + need:] == 0x5A).all())
+
+    adam = dict(kind=0, lr=1e-4, b1=0.9, b2=0.999, eps=1e-8, eps_root=0.0)
+    lp = torch.empty(P, device="cuda"); g = torch.empty((P, n), device="cuda")
+    # MAP
+    need = gl.gl_workspace_bytes(m.h, P)
+    big, ws = guarded(need)
+    zt = d(np.tile(truth, (P, 1)) + 0.01 * rng.standard_normal((P, n)).astype(np.float32))
+    om, ov = torch.zeros_like(zt), torch.zeros_like(zt)
+    for t in (1, 2):
+        gl.gl_map_step(m.h, adam, m.obs, m.noise_sigma, m.psf, zt, None, om, ov, t, lp, g, ws)
+    torch.cuda.synchronize()
+    assert intact(big, need) and torch.isfinite(lp).sum() >= P // 2
+    # SVI, both estimators
+    need = gl.gl_svi_workspace_bytes(m.h, P)
+    big, ws = guarded(need)
+    L = np.tril(0.001 * rng.standard_normal((n, n))) + np.diag(0.004 + 0.004 * rng.random(n))
+    lt = d(L[np.tril_indices(n)].astype(np.float32)); mu = d(truth.copy())
+    sm, sv, stats = torch.zeros(n + nt, device="cuda"), torch.zeros(n + nt, device="cuda"), torch.zeros(2, device="cuda")
+    xi = d(rng.standard_normal((P, n)).astype(np.float32))
+    gl.gl_svi_step(m.h, adam, m.obs, m.noise_sigma, m.psf, mu, lt, xi, None, sm, sv, 1, stats, ws)
+    gl.gl_svi_step_score(m.h, adam, m.obs, m.noise_sigma, m.psf, mu, lt, xi, None, sm, sv, 2, 1, stats, ws)
+    torch.cuda.synchronize()
+    assert intact(big, need) and float(stats[1]) >= P // 2
+    # HMC with a dense L
+    need = gl.gl_hmc_workspace_bytes(m.h, P)
+    big, ws = guarded(need)
+    gl.gl_logpost_grad(m.h, m.obs, m.noise_sigma, m.psf, zt, None, lp, g, m.workspace(P))
+    acc, dh = torch.zeros(P, dtype=torch.int32, device="cuda"), torch.zeros(P, device="cuda")
+    lu = d(np.log(rng.random(P)).astype(np.float32))
+    gl.gl_hmc_step(m.h, m.obs, m.noise_sigma, m.psf, zt, lp, g, lt, xi, lu, None, 1e-3, 3, acc, dh, ws)
+    torch.cuda.synchronize()
+    assert intact(big, need) and not torch.isnan(dh).any()
+    m.close()
